@@ -1,0 +1,444 @@
+"""fp64 CPU oracle of the ORBIT per-GPU training step -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It shares no code with paper_2404_14712_b200/ (the CUDA path) and imports nothing but
+numpy.  Every function is the plain definition written out in float64, in the paper's order and
+notation; numpy `@` (a library matmul) is the only primitive used as a step.  No blocking, fusion or
+algebraic reformulation: in particular the variable aggregation forms the K/V projections of every
+variable token explicitly (the CUDA path uses a collapsed form -- that is the thing being checked).
+
+Citations are `PAPER.md:<line>` and SURVEY.md §8(c) readings (listed in
+DESIGN.md "Readings").  Where the paper is silent the reading is named.
+
+Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): central finite differences for every
+fwd/bwd pair; softmax rows sum to 1 / shift invariance; LayerNorm zero-mean unit-variance; attention
+over identical keys = mean of values; Eq. (2)/(3) shard sums = unsharded product; tokeniser = strided
+convolution (torch conv2d, float64); whole block fwd+bwd = torch float64 autograd of textbook ops;
+aggregation V=1 closed form, permutation invariance, dbk == 0, dbv == sum(do).
+Parity unpinned: none.
+
+Layout conventions (same as include/orbit.h): row-major, weights [in, out] so y = x A exactly as in
+Eq. (1)-(3); Wqkv columns [Q | K | V], heads contiguous inside each third;
+tok[B, L, V, D]; patches row-major over the grid, pixels row-major inside a patch.
+"""
+from __future__ import annotations
+
+import math
+import numpy as np
+
+F64 = np.float64
+
+
+def _f64(a):
+    return np.asarray(a, dtype=F64)
+
+
+# ---------------------------------------------------------------------------------------------
+# elementary functions
+# ---------------------------------------------------------------------------------------------
+_erf = np.vectorize(math.erf, otypes=[F64])
+
+
+def erf(u):
+    """libm erf, elementwise (SURVEY.md §8(c) pin table: 'GELU ... libm erf')."""
+    u = _f64(u)
+    try:  # scipy's erf is the same libm-quality function, vectorised; fall back to math.erf
+        from scipy.special import erf as _serf
+        return _serf(u)
+    except Exception:  # pragma: no cover
+        return _erf(u)
+
+
+def gelu(u):
+    """GELU(u) = u * Phi(u) = 0.5 u (1 + erf(u / sqrt 2)).  PAPER.md:88 "GeLU (xA) B"; exact erf
+    form (reading 7)."""
+    u = _f64(u)
+    return 0.5 * u * (1.0 + erf(u / math.sqrt(2.0)))
+
+
+def gelu_grad(u):
+    """d GELU / du = Phi(u) + u phi(u), Phi/phi the standard normal cdf/pdf."""
+    u = _f64(u)
+    Phi = 0.5 * (1.0 + erf(u / math.sqrt(2.0)))
+    phi = np.exp(-0.5 * u * u) / math.sqrt(2.0 * math.pi)
+    return Phi + u * phi
+
+
+def softmax_lastdim(s):
+    """softmax over the last axis with max subtraction (PAPER.md:88 softmax(QK^T)V)."""
+    s = _f64(s)
+    e = np.exp(s - s.max(axis=-1, keepdims=True))
+    return e / e.sum(axis=-1, keepdims=True)
+
+
+def layernorm(z, gamma, beta, eps):
+    """LN(z)_i = gamma_i (z_i - mu) / sqrt(var + eps) + beta_i, mu and *biased* var over the last
+    axis (reading 6).  Returns (out, zhat, rstd)."""
+    z = _f64(z)
+    mu = z.mean(axis=-1, keepdims=True)
+    var = ((z - mu) ** 2).mean(axis=-1, keepdims=True)
+    rstd = 1.0 / np.sqrt(var + eps)
+    zhat = (z - mu) * rstd
+    return zhat * _f64(gamma) + _f64(beta), zhat, rstd
+
+
+def layernorm_bwd(dout, zhat, rstd, gamma):
+    """Given d(out): dgamma = sum_rows dout*zhat; dbeta = sum_rows dout;
+    dz = (ghat - mean(ghat) - zhat * mean(ghat*zhat)) * rstd with ghat = dout*gamma."""
+    dout = _f64(dout)
+    D = dout.shape[-1]
+    flat = dout.reshape(-1, D)
+    dgamma = (flat * zhat.reshape(-1, D)).sum(axis=0)
+    dbeta = flat.sum(axis=0)
+    ghat = dout * _f64(gamma)
+    dz = (ghat - ghat.mean(axis=-1, keepdims=True)
+          - zhat * (ghat * zhat).mean(axis=-1, keepdims=True)) * rstd
+    return dz, dgamma, dbeta
+
+
+# ---------------------------------------------------------------------------------------------
+# TOK -- per-variable patch tokenisation ("independent patch tokenization for each
+# channel input"; PAPER.md:155 sample shape; reading 1)
+# ---------------------------------------------------------------------------------------------
+def patches(x, p):
+    """pix[b, v, l, r] = x[b, v, i*p+di, j*p+dj], l = i*(Wg/p)+j, r = di*p+dj."""
+    x = _f64(x)
+    B, V, Hg, Wg = x.shape
+    gh, gw = Hg // p, Wg // p
+    pix = x.reshape(B, V, gh, p, gw, p).transpose(0, 1, 2, 4, 3, 5)   # b v i j di dj
+    return pix.reshape(B, V, gh * gw, p * p)
+
+
+def tokenize(x, Wp, bp, p):
+    """tok[b, l, v, :] = sum_r pix(b, v, l, r) Wp[v, r, :] + bp[v, :].   -> [B, L, V, D]"""
+    pix = patches(x, p)                                             # [B, V, L, p^2]
+    Wp, bp = _f64(Wp), _f64(bp)
+    B, V, L, _ = pix.shape
+    D = Wp.shape[2]
+    tok = np.empty((B, L, V, D), dtype=F64)
+    for v in range(V):                                              # independent per channel
+        tok[:, :, v, :] = pix[:, v] @ Wp[v] + bp[v]
+    return tok
+
+
+def tokenize_bwd(x, dtok, p):
+    """dWp[v, r, :] = sum_{b,l} pix(b,v,l,r) dtok[b,l,v,:];  dbp[v, :] = sum_{b,l} dtok[b,l,v,:].
+    No dx (x is input data)."""
+    pix = patches(x, p)
+    dtok = _f64(dtok)
+    B, V, L, P2 = pix.shape
+    D = dtok.shape[3]
+    dWp = np.empty((V, P2, D), dtype=F64)
+    dbp = np.empty((V, D), dtype=F64)
+    for v in range(V):
+        dWp[v] = pix[:, v].reshape(B * L, P2).T @ dtok[:, :, v, :].reshape(B * L, D)
+        dbp[v] = dtok[:, :, v, :].reshape(B * L, D).sum(axis=0)
+    return dWp, dbp
+
+
+# ---------------------------------------------------------------------------------------------
+# A2 -- variable aggregation ("aggregated together across different channels using
+# cross-attention"; "same as the ClimaX"; readings 3, 4)
+# ---------------------------------------------------------------------------------------------
+def var_aggregate(tok, P, heads, pos=None):
+    """At every (b, l), X = tok[b, l] in R^{V x D}:
+         qt = q Wq + bq;  K = X Wk + bk;  U = X Wv + bv;
+         per head a (d_a = D/heads): s_v = qt_a . K_{v,a} / sqrt(d_a); alpha = softmax_v(s);
+         o_a = sum_v alpha_v U_{v,a};  agg[b, l] = concat_a(o_a) Wo + bo (+ pos[l]).
+    Returns (agg [B, L, D], cache)."""
+    tok = _f64(tok)
+    B, L, V, D = tok.shape
+    da = D // heads
+    q, Wq, bq = _f64(P["q"]), _f64(P["Wq"]), _f64(P["bq"])
+    Wk, bk, Wv, bv = _f64(P["Wk"]), _f64(P["bk"]), _f64(P["Wv"]), _f64(P["bv"])
+    Wo, bo = _f64(P["Wo"]), _f64(P["bo"])
+    qt = q @ Wq + bq                                               # [D], data independent
+    K = tok @ Wk + bk                                              # [B, L, V, D]
+    U = tok @ Wv + bv
+    Kh = K.reshape(B, L, V, heads, da)
+    Uh = U.reshape(B, L, V, heads, da)
+    qh = qt.reshape(heads, da)
+    s = np.einsum("ac,blvac->blav", qh, Kh) / math.sqrt(da)        # [B, L, heads, V]
+    alpha = softmax_lastdim(s)
+    o = np.einsum("blav,blvac->blac", alpha, Uh).reshape(B, L, D)
+    agg = o @ Wo + bo
+    if pos is not None:
+        agg = agg + _f64(pos)[None, :, :]
+    cache = dict(tok=tok, qt=qt, Kh=Kh, Uh=Uh, alpha=alpha, o=o, heads=heads)
+    return agg, cache
+
+
+def var_aggregate_bwd(dagg, P, cache, want_dpos=False):
+    """Backward of var_aggregate, given g = dagg[b, l]:
+       dbo += g; dWo += o^T g; dpos[l] += g; do = g Wo^T;
+       per head: dalpha_v = do_a . U_{v,a}; dU_{v,a} = alpha_v do_a;
+                 ds_v = alpha_v (dalpha_v - sum_w alpha_w dalpha_w);
+                 dqt_a += sum_v ds_v K_{v,a}/sqrt(d_a); dK_{v,a} = ds_v qt_a/sqrt(d_a);
+       dWk += X^T dK; dbk += sum dK; dWv += X^T dU; dbv += sum dU; dtok = dK Wk^T + dU Wv^T;
+       dbq = dqt; dWq = q^T dqt; dq = dqt Wq^T."""
+    dagg = _f64(dagg)
+    tok, qt, Kh, Uh, alpha, o = (cache[k] for k in ("tok", "qt", "Kh", "Uh", "alpha", "o"))
+    heads = cache["heads"]
+    B, L, V, D = tok.shape
+    da = D // heads
+    q, Wq = _f64(P["q"]), _f64(P["Wq"])
+    Wk, Wv, Wo = _f64(P["Wk"]), _f64(P["Wv"]), _f64(P["Wo"])
+    G = {}
+    g2 = dagg.reshape(B * L, D)
+    G["bo"] = g2.sum(axis=0)
+    G["Wo"] = o.reshape(B * L, D).T @ g2
+    dpos = dagg.sum(axis=0) if want_dpos else None
+    do = (dagg @ Wo.T).reshape(B, L, heads, da)
+    dalpha = np.einsum("blac,blvac->blav", do, Uh)
+    dUh = np.einsum("blav,blac->blvac", alpha, do)
+    ds = alpha * (dalpha - (alpha * dalpha).sum(axis=-1, keepdims=True))
+    qh = qt.reshape(heads, da)
+    dqt = (np.einsum("blav,blvac->ac", ds, Kh) / math.sqrt(da)).reshape(D)
+    dKh = np.einsum("blav,ac->blvac", ds, qh) / math.sqrt(da)
+    dK = dKh.reshape(B * L * V, D)
+    dU = dUh.reshape(B * L * V, D)
+    X = tok.reshape(B * L * V, D)
+    G["Wk"] = X.T @ dK
+    G["bk"] = dK.sum(axis=0)
+    G["Wv"] = X.T @ dU
+    G["bv"] = dU.sum(axis=0)
+    dtok = (dK @ Wk.T + dU @ Wv.T).reshape(B, L, V, D)
+    G["bq"] = dqt
+    G["Wq"] = np.outer(q, dqt)
+    G["q"] = dqt @ Wq.T
+    return dtok, G, dpos
+
+
+# ---------------------------------------------------------------------------------------------
+# BLK -- one ViT block, pre-LN residual form (readings 5-8, 10)
+# ---------------------------------------------------------------------------------------------
+def attention(Q, K, V, heads):
+    """Per (b, head j): S = Q_j K_j^T / sqrt(d_h); P = softmax over keys; O_j = P V_j
+    (PAPER.md:88 softmax(QK^T)V; :114 "scaled dot product").  Q, K, V: [B, N, D] -> O [B, N, D],
+    P [B, heads, N, N]."""
+    B, N, D = Q.shape
+    dh = D // heads
+    O = np.empty((B, N, D), dtype=F64)
+    Pm = np.empty((B, heads, N, N), dtype=F64)
+    for b in range(B):
+        for j in range(heads):
+            c = slice(j * dh, (j + 1) * dh)
+            S = (Q[b, :, c] @ K[b, :, c].T) / math.sqrt(dh)
+            Pj = softmax_lastdim(S)
+            Pm[b, j] = Pj
+            O[b, :, c] = Pj @ V[b, :, c]
+    return O, Pm
+
+
+def attention_bwd(dO, Q, K, V, Pm, heads):
+    """Per head: dV = P^T dO_j; dP = dO_j V_j^T; dS = P o (dP - rowsum(dP o P));
+    dQ = dS K_j / sqrt(d_h); dK = dS^T Q_j / sqrt(d_h)."""
+    B, N, D = Q.shape
+    dh = D // heads
+    dQ = np.empty_like(Q)
+    dK = np.empty_like(K)
+    dV = np.empty_like(V)
+    for b in range(B):
+        for j in range(heads):
+            c = slice(j * dh, (j + 1) * dh)
+            Pj = Pm[b, j]
+            dV[b, :, c] = Pj.T @ dO[b, :, c]
+            dP = dO[b, :, c] @ V[b, :, c].T
+            dS = Pj * (dP - (dP * Pj).sum(axis=-1, keepdims=True))
+            dQ[b, :, c] = dS @ K[b, :, c] / math.sqrt(dh)
+            dK[b, :, c] = dS.T @ Q[b, :, c] / math.sqrt(dh)
+    return dQ, dK, dV
+
+
+def block_fwd(x, P, heads, eps=1e-5):
+    """a = LN1(x); [Q|K|V] = a Wqkv + bqkv; O = attention; x1 = x + O Wproj + bproj;
+    m = LN2(x1); u = m Wfc1 + bfc1; g = GELU(u); y = x1 + g Wfc2 + bfc2.    x: [B, N, D]."""
+    x = _f64(x)
+    B, N, D = x.shape
+    a, xhat, rstd1 = layernorm(x, P["ln1_g"], P["ln1_b"], eps)
+    qkv = a @ _f64(P["Wqkv"]) + _f64(P["bqkv"])
+    Q, K, V = qkv[..., 0:D], qkv[..., D:2 * D], qkv[..., 2 * D:3 * D]
+    O, Pm = attention(Q, K, V, heads)
+    x1 = x + O @ _f64(P["Wproj"]) + _f64(P["bproj"])
+    m, x1hat, rstd2 = layernorm(x1, P["ln2_g"], P["ln2_b"], eps)
+    u = m @ _f64(P["Wfc1"]) + _f64(P["bfc1"])
+    g = gelu(u)
+    y = x1 + g @ _f64(P["Wfc2"]) + _f64(P["bfc2"])
+    cache = dict(xhat=xhat, rstd1=rstd1, a=a, Q=Q, K=K, V=V, Pm=Pm, O=O, x1=x1, x1hat=x1hat,
+                 rstd2=rstd2, m=m, u=u, g=g, heads=heads)
+    return y, cache
+
+
+def block_bwd(dy, P, cache):
+    """SURVEY.md §8(c)-BLK': dx and the 12 parameter gradients, given dy."""
+    dy = _f64(dy)
+    B, N, D = dy.shape
+    M = B * N
+    c = cache
+    heads = c["heads"]
+    G = {}
+    dy2 = dy.reshape(M, D)
+    F = c["u"].shape[-1]
+    G["bfc2"] = dy2.sum(axis=0)
+    G["Wfc2"] = c["g"].reshape(M, F).T @ dy2
+    dg = dy @ _f64(P["Wfc2"]).T
+    du = dg * gelu_grad(c["u"])
+    du2 = du.reshape(M, F)
+    G["bfc1"] = du2.sum(axis=0)
+    G["Wfc1"] = c["m"].reshape(M, D).T @ du2
+    dm = du @ _f64(P["Wfc1"]).T
+    dz2, G["ln2_g"], G["ln2_b"] = layernorm_bwd(dm, c["x1hat"], c["rstd2"], P["ln2_g"])
+    dx1 = dy + dz2
+    dx12 = dx1.reshape(M, D)
+    G["bproj"] = dx12.sum(axis=0)
+    G["Wproj"] = c["O"].reshape(M, D).T @ dx12
+    dO = dx1 @ _f64(P["Wproj"]).T
+    dQ, dK, dV = attention_bwd(dO, c["Q"], c["K"], c["V"], c["Pm"], heads)
+    dqkv = np.concatenate([dQ, dK, dV], axis=-1)
+    dqkv2 = dqkv.reshape(M, 3 * D)
+    G["bqkv"] = dqkv2.sum(axis=0)
+    G["Wqkv"] = c["a"].reshape(M, D).T @ dqkv2
+    da = dqkv @ _f64(P["Wqkv"]).T
+    dz1, G["ln1_g"], G["ln1_b"] = layernorm_bwd(da, c["xhat"], c["rstd1"], P["ln1_g"])
+    dx = dx1 + dz1
+    return dx, G
+
+
+# ---------------------------------------------------------------------------------------------
+# SHARD -- Hybrid-STOP shard-local arithmetic (Eq. 1-3, Fig. 3; readings 13-16)
+# implemented SEPARATELY from BLK; tests assert the two agree to ~1e-13.
+# ---------------------------------------------------------------------------------------------
+def chain_sharded(x, A_cols, B_rows):
+    """Eq. (2):  y = sum_k (x A_{*,k}) B_{k,*}."""
+    y = None
+    for Ak, Bk in zip(A_cols, B_rows):
+        part = (_f64(x) @ _f64(Ak)) @ _f64(Bk)
+        y = part if y is None else y + part
+    return y
+
+
+def chain_sharded_dx(dy, A_cols, B_rows):
+    """Eq. (3): row-wise dx = dy (sum_k B_{k,*}^T A_{*,k}^T); rows independent
+    (the "(x) I"), so no Kronecker product is formed (reading 16)."""
+    dx = None
+    for Ak, Bk in zip(A_cols, B_rows):
+        part = (_f64(dy) @ _f64(Bk).T) @ _f64(Ak).T
+        dx = part if dx is None else dx + part
+    return dx
+
+
+def block_fwd_sharded(x, Pc, shards, heads, eps=1e-5):
+    """Forward with T shards run one after another (Fig. 3a):
+       a = LN1(x) once; for k: qkv^k = a Wqkv^k + bqkv^k -> attention on that shard's heads/T heads
+       -> O^k [.., D/T] -> P^k = O^k Wproj^k;  x1 = x + sum_k P^k + bproj;
+       m = LN2(x1); for k: g^k = GELU(m Wfc1^k + bfc1^k); Y^k = g^k Wfc2^k; y = x1 + sum_k Y^k + bfc2.
+    Pc: the unsharded parameters ln1_g, ln1_b, ln2_g, ln2_b, bproj, bfc2 (reading 14: bias and
+    residual enter once, after the combine)."""
+    x = _f64(x)
+    B, N, D = x.shape
+    T = len(shards)
+    hk = heads // T
+    dc = D // T
+    a, xhat, rstd1 = layernorm(x, Pc["ln1_g"], Pc["ln1_b"], eps)
+    per = []
+    acc = np.zeros_like(x)
+    for S in shards:
+        qkv = a @ _f64(S["Wqkv"]) + _f64(S["bqkv"])
+        Q, K, V = qkv[..., 0:dc], qkv[..., dc:2 * dc], qkv[..., 2 * dc:3 * dc]
+        O, Pm = attention(Q, K, V, hk)
+        acc = acc + O @ _f64(S["Wproj"])
+        per.append(dict(Q=Q, K=K, V=V, Pm=Pm, O=O))
+    x1 = x + acc + _f64(Pc["bproj"])
+    m, x1hat, rstd2 = layernorm(x1, Pc["ln2_g"], Pc["ln2_b"], eps)
+    acc2 = np.zeros_like(x)
+    for S, c in zip(shards, per):
+        u = m @ _f64(S["Wfc1"]) + _f64(S["bfc1"])
+        g = gelu(u)
+        acc2 = acc2 + g @ _f64(S["Wfc2"])
+        c["u"], c["g"] = u, g
+    y = x1 + acc2 + _f64(Pc["bfc2"])
+    cache = dict(xhat=xhat, rstd1=rstd1, a=a, x1=x1, x1hat=x1hat, rstd2=rstd2, m=m, per=per,
+                 heads=heads)
+    return y, cache
+
+
+def block_bwd_sharded(dy, Pc, shards, cache):
+    """Backward mirror (Eq. 3): per-shard grads as in BLK' with
+    dm = sum_k du^k Wfc1^k^T and da = sum_k dqkv^k Wqkv^k^T ("add their activation gradients
+    together")."""
+    dy = _f64(dy)
+    B, N, D = dy.shape
+    M = B * N
+    T = len(shards)
+    hk = cache["heads"] // T
+    Gc = {}
+    Gs = [dict() for _ in shards]
+    dy2 = dy.reshape(M, D)
+    Gc["bfc2"] = dy2.sum(axis=0)
+    dm = np.zeros_like(dy)
+    for S, c, G in zip(shards, cache["per"], Gs):
+        Fk = c["u"].shape[-1]
+        G["Wfc2"] = c["g"].reshape(M, Fk).T @ dy2
+        du = (dy @ _f64(S["Wfc2"]).T) * gelu_grad(c["u"])
+        G["bfc1"] = du.reshape(M, Fk).sum(axis=0)
+        G["Wfc1"] = cache["m"].reshape(M, D).T @ du.reshape(M, Fk)
+        dm = dm + du @ _f64(S["Wfc1"]).T
+    dz2, Gc["ln2_g"], Gc["ln2_b"] = layernorm_bwd(dm, cache["x1hat"], cache["rstd2"], Pc["ln2_g"])
+    dx1 = dy + dz2
+    dx12 = dx1.reshape(M, D)
+    Gc["bproj"] = dx12.sum(axis=0)
+    da = np.zeros_like(dy)
+    for S, c, G in zip(shards, cache["per"], Gs):
+        dc = c["O"].shape[-1]
+        G["Wproj"] = c["O"].reshape(M, dc).T @ dx12
+        dO = dx1 @ _f64(S["Wproj"]).T
+        dQ, dK, dV = attention_bwd(dO, c["Q"], c["K"], c["V"], c["Pm"], hk)
+        dqkv = np.concatenate([dQ, dK, dV], axis=-1)
+        G["bqkv"] = dqkv.reshape(M, 3 * dc).sum(axis=0)
+        G["Wqkv"] = cache["a"].reshape(M, D).T @ dqkv.reshape(M, 3 * dc)
+        da = da + dqkv @ _f64(S["Wqkv"]).T
+    dz1, Gc["ln1_g"], Gc["ln1_b"] = layernorm_bwd(da, cache["xhat"], cache["rstd1"], Pc["ln1_g"])
+    dx = dx1 + dz1
+    return dx, Gc, Gs
+
+
+# ---------------------------------------------------------------------------------------------
+# Harness loss (BASELINE.json config 1: "target is an N(0,1) field with MSE loss")
+# ---------------------------------------------------------------------------------------------
+def mse_loss(y, t):
+    """loss = mean((y - t)^2); dy = 2 (y - t) / numel."""
+    y, t = _f64(y), _f64(t)
+    d = y - t
+    return float((d * d).mean()), 2.0 * d / d.size
+
+
+# ---------------------------------------------------------------------------------------------
+# Whole step (tokenise -> aggregate -> depth x block, forward and backward)
+# ---------------------------------------------------------------------------------------------
+def step(x, emb, agg, blocks, target, p, heads, eps=1e-5, pos=None):
+    """One training step of the hot path.  Returns dict with every output and gradient."""
+    tok = tokenize(x, emb["Wp"], emb["bp"], p)
+    z, acache = var_aggregate(tok, agg, heads, pos)
+    caches = []
+    h = z
+    for P in blocks:
+        h, c = block_fwd(h, P, heads, eps)
+        caches.append(c)
+    loss, dh = mse_loss(h, target)
+    out = dict(tok=tok, agg=z, y=h, loss=loss, dy=dh, block_grads=[None] * len(blocks))
+    for i in reversed(range(len(blocks))):
+        dh, G = block_bwd(dh, blocks[i], caches[i])
+        out["block_grads"][i] = G
+    out["dagg"] = dh
+    dtok, Ga, dpos = var_aggregate_bwd(dh, agg, acache, want_dpos=pos is not None)
+    out["dtok"], out["agg_grads"], out["dpos"] = dtok, Ga, dpos
+    out["dWp"], out["dbp"] = tokenize_bwd(x, dtok, p)
+    return out
+
+
+def rel_fro(got, ref):
+    """||got - ref||_F / ||ref||_F -- the parity metric north_star names."""
+    got, ref = _f64(got), _f64(ref)
+    den = float(np.sqrt((ref * ref).sum()))
+    num = float(np.sqrt(((got - ref) ** 2).sum()))
+    return num / den if den > 0 else num

@@ -1,0 +1,148 @@
+/* orbit.h -- C-ABI of liborbit.so: the per-GPU dense training step of ORBIT's ClimaX-style ViT
+ * (arxiv 2404.14712), hand-written CUDA for sm_100a (B200).
+ *
+ * Citations are PAPER.md:<line> (the paper text) and DESIGN.md "Readings" R<n> where the paper is silent.
+ *
+ * Conventions:
+ *  - All tensor pointers are DEVICE memory owned by the caller; descriptors and parameter structs are HOST
+ *    memory, read during the call only.  The library allocates no device memory, keeps no pointer after
+ *    return, and writes only outputs, `saved`, `ws` and gradients.  Outputs are overwritten (no accumulate).
+ *  - Dense row-major, last index contiguous.  Weights are [in, out] so that y = x A exactly as in Eq. (1)-(3)
+ *    (PAPER.md:70-82): a column shard is A[:, k n/T:(k+1) n/T], a row shard is B[k n/T:(k+1) n/T, :].
+ *    Wqkv columns are [Q | K | V], heads contiguous inside each third.  tok is [B, L, V, D].
+ *  - Execution is asynchronous on `stream` (a cudaStream_t passed as void*); no host synchronisation.
+ *  - Errors: return code only (never abort/throw).  All argument checks precede the first launch, so a
+ *    non-OK return other than ORBIT_ERR_CUDA means nothing was written.  orbit_last_error() gives text.
+ *  - Precision: ORBIT_BF16 = bf16 storage, every contraction accumulates in fp32, LayerNorm statistics /
+ *    softmax / GELU in fp32, one round-to-nearest-even at each store; Hybrid-STOP shard partials stay fp32
+ *    until summed.  ORBIT_F32 = fp32 storage and true fp32 FMA (no TF32).  (R17.)
+ *  - No CPU fallback and no other-architecture fallback: a device that is not compute capability 10.x
+ *    yields ORBIT_ERR_ARCH.
+ */
+#ifndef ORBIT_H_
+#define ORBIT_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORBIT_VERSION 100
+
+typedef enum {
+  ORBIT_OK = 0,
+  ORBIT_ERR_NULL = 1,        /* a required pointer is NULL */
+  ORBIT_ERR_SHAPE = 2,       /* Hg%p, Wg%p, D%heads, heads%T, F%T, non-positive or unsupported sizes */
+  ORBIT_ERR_DTYPE = 3,       /* unknown dtype, or resid_dtype incompatible with dtype */
+  ORBIT_ERR_ALIGN = 4,       /* base pointer not 16-byte aligned */
+  ORBIT_ERR_WORKSPACE = 5,   /* ws_bytes smaller than the matching *_workspace_bytes() */
+  ORBIT_ERR_UNSUPPORTED = 6, /* reserved flag set, in-place call */
+  ORBIT_ERR_ARCH = 7,        /* device is not sm_100-class */
+  ORBIT_ERR_CUDA = 8         /* a CUDA runtime call or launch failed (see orbit_last_error) */
+} orbit_status;
+
+typedef enum { ORBIT_F32 = 0, ORBIT_BF16 = 1 } orbit_dtype;
+
+/* flags of orbit_block_desc (reserved: setting one returns ORBIT_ERR_UNSUPPORTED) */
+#define ORBIT_QK_NORM   1u   /* QK-LayerNorm, PAPER.md:114 -- SURVEY NEXT-2 */
+#define ORBIT_RECOMPUTE 2u   /* activation checkpointing, PAPER.md:124 -- SURVEY NEXT-2 */
+
+/* ---- a1 / a1': per-variable patch tokenisation (R1, R2) --------------------------- */
+typedef struct {
+  int B, V, Hg, Wg, p, D;      /* batch, variables, lat x lon grid, patch size, embed dim; L=(Hg/p)*(Wg/p) */
+  orbit_dtype dtype;           /* dtype of Wp, bp, tok, dtok, dWp, dbp (x is always fp32) */
+} orbit_embed_desc;
+
+/* tok[b,l,v,:] = sum_r pix(b,v,l,r) Wp[v,r,:] + bp[v,:],  l = i*(Wg/p)+j, r = di*p+dj,
+ * pix = x[b,v,i*p+di,j*p+dj].   x [B,V,Hg,Wg] fp32; Wp [V,p*p,D]; bp [V,D]; tok [B,L,V,D]. */
+int orbit_tokenize(const orbit_embed_desc* d, const float* x, const void* Wp, const void* bp, void* tok,
+                   void* stream);
+/* dWp[v,r,:] = sum_{b,l} pix dtok[b,l,v,:];  dbp[v,:] = sum_{b,l} dtok[b,l,v,:].  No dx (input data). */
+int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dtok, void* dWp, void* dbp,
+                       void* ws, size_t ws_bytes, void* stream);
+size_t orbit_tokenize_bwd_workspace_bytes(const orbit_embed_desc* d);
+
+/* ---- a2 / a2': variable aggregation, cross-attention over the V tokens of a patch (R3, R4)
+ * At every (b,l), X = tok[b,l] (V x D):  qt = q Wq + bq;  K = X Wk + bk;  U = X Wv + bv;  per head a:
+ * s_v = qt_a . K_{v,a} / sqrt(d_a); alpha = softmax_v(s); o_a = sum_v alpha_v U_{v,a};
+ * agg[b,l] = concat(o_a) Wo + bo (+ pos[l]).   The kernels use the exact collapsed form of DESIGN.md §4. */
+typedef struct {
+  int B, L, V, D, heads;
+  orbit_dtype dtype;           /* tok, dtok, parameters, parameter grads */
+  orbit_dtype resid_dtype;     /* agg, dagg, pos, dpos (the residual stream) */
+} orbit_agg_desc;
+typedef struct { const void *q /*[D]*/, *Wq, *bq, *Wk, *bk, *Wv, *bv, *Wo, *bo /* W:[D,D] b:[D] */; } orbit_agg_params;
+typedef struct { void *q, *Wq, *bq, *Wk, *bk, *Wv, *bv, *Wo, *bo; } orbit_agg_grads; /* dbk is written (== 0) */
+
+int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_agg_params* P,
+                        const void* pos /* [L,D] nullable */, void* agg /* [B,L,D] */, void* saved,
+                        void* ws, size_t ws_bytes, void* stream);
+int orbit_var_aggregate_bwd(const orbit_agg_desc* d, const void* tok, const orbit_agg_params* P,
+                            const void* dagg, const void* saved, void* dtok, orbit_agg_grads* G,
+                            void* dpos /* [L,D] nullable */, void* ws, size_t ws_bytes, void* stream);
+size_t orbit_var_aggregate_workspace_bytes(const orbit_agg_desc* d);
+size_t orbit_var_aggregate_bwd_workspace_bytes(const orbit_agg_desc* d);
+size_t orbit_var_aggregate_saved_bytes(const orbit_agg_desc* d);
+
+/* ---- a3-a7: one ViT block, pre-LN residual form (R5-R8, R10), optionally in Hybrid-STOP
+ * shard-local mode with T shards run one after another on this GPU (Eq. 1-3; R13-R15):
+ *   a = LN1(x); qkv = a Wqkv + bqkv; O = softmax(Q K^T / sqrt(d_h)) V per head; x1 = x + O Wproj + bproj;
+ *   m = LN2(x1); u = m Wfc1 + bfc1; g = GELU_erf(u); y = x1 + g Wfc2 + bfc2.
+ * T > 1: Wqkv, Wfc1 column shards (head aligned), Wproj, Wfc2 row shards; the T fp32 partial products are
+ * summed on the device, then bproj / bfc2 and the residual are added once. */
+typedef struct {
+  int B, N, D, heads, F, T;    /* batch, tokens per sample, embed dim, heads, MLP width, shards (1 = unsharded) */
+  float ln_eps;
+  orbit_dtype dtype;           /* weights, grads, internal activations */
+  orbit_dtype resid_dtype;     /* x, y, dx, dy: F32 or BF16 when dtype is BF16; must be F32 when dtype is F32 */
+  unsigned flags;
+} orbit_block_desc;
+typedef struct { const void *Wqkv /*[D,3D/T]*/, *bqkv /*[3D/T]*/, *Wproj /*[D/T,D]*/, *Wfc1 /*[D,F/T]*/,
+                 *bfc1 /*[F/T]*/, *Wfc2 /*[F/T,D]*/; } orbit_block_shard;
+typedef struct { const void *ln1_g, *ln1_b, *ln2_g, *ln2_b, *bproj, *bfc2 /* all [D] */;
+                 const orbit_block_shard* shards /* T of them, host array */; } orbit_block_params;
+typedef struct { void *Wqkv, *bqkv, *Wproj, *Wfc1, *bfc1, *Wfc2; } orbit_block_shard_grads;
+typedef struct { void *ln1_g, *ln1_b, *ln2_g, *ln2_b, *bproj, *bfc2;
+                 const orbit_block_shard_grads* shards; } orbit_block_grads;
+
+int orbit_block_fwd(const orbit_block_desc* d, const void* x /* [B,N,D] */, const orbit_block_params* P,
+                    void* y, void* saved, void* ws, size_t ws_bytes, void* stream);
+int orbit_block_bwd(const orbit_block_desc* d, const void* dy, const orbit_block_params* P, const void* saved,
+                    void* dx, orbit_block_grads* G, void* ws, size_t ws_bytes, void* stream);
+size_t orbit_block_fwd_workspace_bytes(const orbit_block_desc* d);
+size_t orbit_block_bwd_workspace_bytes(const orbit_block_desc* d);
+size_t orbit_block_saved_bytes(const orbit_block_desc* d);
+
+/* ---- bare Eq. (2)/(3) chain, used by the fp32 shard-recombination check (R15):
+ *   y = sum_k (x A_k) B_k   with A_k [d, n/T] column shards and B_k [n/T, e] row shards;
+ *   dx = sum_k (dy B_k^T) A_k^T.  x [m,d], y [m,e]; fp32 partials combined on device.
+ *   ws must hold m*(n/T) elements of `dtype` + m*max(d,e) floats. */
+int orbit_chain_fwd(int m, int d, int n, int e, int T, orbit_dtype dtype, const void* x,
+                    const void* const* A_cols, const void* const* B_rows, void* y,
+                    void* ws, size_t ws_bytes, void* stream);
+int orbit_chain_bwd(int m, int d, int n, int e, int T, orbit_dtype dtype, const void* dy,
+                    const void* const* A_cols, const void* const* B_rows, void* dx,
+                    void* ws, size_t ws_bytes, void* stream);
+size_t orbit_chain_workspace_bytes(int m, int d, int n, int e, int T, orbit_dtype dtype);
+
+/* ---- harness loss (BASELINE.json config 1: "target is an N(0,1) field with MSE loss"):
+ *   loss = mean((y - t)^2) (fp32 scalar, device), dy = 2 (y - t) / n.  y, t, dy: n elements of `dtype`. */
+int orbit_mse_loss_grad(orbit_dtype dtype, size_t n, const void* y, const void* t, void* dy, float* loss,
+                        void* stream);
+
+/* ---- diagnostics ---------------------------------------------------------------------------------------- */
+const char* orbit_last_error(void);   /* thread-local, static storage */
+int orbit_version(void);
+/* Number of kernels launched by this library on the calling thread since the last reset (bench.py's
+ * gpu_launches claim). */
+long long orbit_launch_count(void);
+void orbit_reset_launch_count(void);
+/* 0 = automatic (tcgen05 tensor-core kernels for bf16 where shapes allow), 1 = force the SIMT fp32-FMA
+ * kernels everywhere (debug cross-check only; never used by bench.py). */
+void orbit_set_debug_force_simt(int on);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ORBIT_H_ */

@@ -1,0 +1,271 @@
+"""Thin ctypes binding over liborbit.so -- same names as the C entry points of include/orbit.h.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the C-ABI.  torch is used
+for device memory and streams (tensor.data_ptr(), torch.cuda.current_stream()).  There is NO fallback: if
+liborbit.so is missing or fails to load, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liborbit.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} not found: build it with `python -m paper_2404_14712_b200.build` "
+        "(there is no CPU or PyTorch fallback for the ORBIT hot path)")
+lib = C.CDLL(LIB_PATH)
+
+ORBIT_OK = 0
+ORBIT_F32, ORBIT_BF16 = 0, 1
+STATUS_NAMES = {0: "OK", 1: "ERR_NULL", 2: "ERR_SHAPE", 3: "ERR_DTYPE", 4: "ERR_ALIGN", 5: "ERR_WORKSPACE",
+                6: "ERR_UNSUPPORTED", 7: "ERR_ARCH", 8: "ERR_CUDA"}
+DTYPES = {"f32": ORBIT_F32, "bf16": ORBIT_BF16}
+TORCH_DTYPES = {"f32": torch.float32, "bf16": torch.bfloat16}
+
+
+class OrbitError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib.orbit_last_error().decode(errors="replace")
+        super().__init__(f"{where}: {STATUS_NAMES.get(status, status)}: {msg}")
+
+
+# ---- descriptor / parameter structs (mirror include/orbit.h) -------------------------------------------
+class orbit_embed_desc(C.Structure):
+    _fields_ = [("B", C.c_int), ("V", C.c_int), ("Hg", C.c_int), ("Wg", C.c_int), ("p", C.c_int), ("D", C.c_int),
+                ("dtype", C.c_int)]
+
+
+class orbit_agg_desc(C.Structure):
+    _fields_ = [("B", C.c_int), ("L", C.c_int), ("V", C.c_int), ("D", C.c_int), ("heads", C.c_int),
+                ("dtype", C.c_int), ("resid_dtype", C.c_int)]
+
+
+_AGG_NAMES = ("q", "Wq", "bq", "Wk", "bk", "Wv", "bv", "Wo", "bo")
+
+
+class orbit_agg_params(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _AGG_NAMES]
+
+
+class orbit_agg_grads(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _AGG_NAMES]
+
+
+class orbit_block_desc(C.Structure):
+    _fields_ = [("B", C.c_int), ("N", C.c_int), ("D", C.c_int), ("heads", C.c_int), ("F", C.c_int), ("T", C.c_int),
+                ("ln_eps", C.c_float), ("dtype", C.c_int), ("resid_dtype", C.c_int), ("flags", C.c_uint)]
+
+
+_SHARD_NAMES = ("Wqkv", "bqkv", "Wproj", "Wfc1", "bfc1", "Wfc2")
+_COMMON_NAMES = ("ln1_g", "ln1_b", "ln2_g", "ln2_b", "bproj", "bfc2")
+
+
+class orbit_block_shard(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _SHARD_NAMES]
+
+
+class orbit_block_params(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _COMMON_NAMES] + [("shards", C.POINTER(orbit_block_shard))]
+
+
+class orbit_block_grads(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _COMMON_NAMES] + [("shards", C.POINTER(orbit_block_shard))]
+
+
+# ---- prototypes ---------------------------------------------------------------------------------------------
+def _proto(name, restype, argtypes):
+    f = getattr(lib, name)
+    f.restype = restype
+    f.argtypes = argtypes
+    return f
+
+
+_vp, _sz = C.c_void_p, C.c_size_t
+_proto("orbit_last_error", C.c_char_p, [])
+_proto("orbit_version", C.c_int, [])
+_proto("orbit_launch_count", C.c_longlong, [])
+_proto("orbit_reset_launch_count", None, [])
+_proto("orbit_set_debug_force_simt", None, [C.c_int])
+_proto("orbit_tokenize", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp])
+_proto("orbit_tokenize_bwd", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp, _sz, _vp])
+_proto("orbit_tokenize_bwd_workspace_bytes", _sz, [C.POINTER(orbit_embed_desc)])
+_proto("orbit_var_aggregate", C.c_int,
+       [C.POINTER(orbit_agg_desc), _vp, C.POINTER(orbit_agg_params), _vp, _vp, _vp, _vp, _sz, _vp])
+_proto("orbit_var_aggregate_bwd", C.c_int,
+       [C.POINTER(orbit_agg_desc), _vp, C.POINTER(orbit_agg_params), _vp, _vp, _vp, C.POINTER(orbit_agg_grads), _vp,
+        _vp, _sz, _vp])
+for _n in ("orbit_var_aggregate_workspace_bytes", "orbit_var_aggregate_bwd_workspace_bytes",
+           "orbit_var_aggregate_saved_bytes"):
+    _proto(_n, _sz, [C.POINTER(orbit_agg_desc)])
+_proto("orbit_block_fwd", C.c_int,
+       [C.POINTER(orbit_block_desc), _vp, C.POINTER(orbit_block_params), _vp, _vp, _vp, _sz, _vp])
+_proto("orbit_block_bwd", C.c_int,
+       [C.POINTER(orbit_block_desc), _vp, C.POINTER(orbit_block_params), _vp, _vp, C.POINTER(orbit_block_grads), _vp,
+        _sz, _vp])
+for _n in ("orbit_block_fwd_workspace_bytes", "orbit_block_bwd_workspace_bytes", "orbit_block_saved_bytes"):
+    _proto(_n, _sz, [C.POINTER(orbit_block_desc)])
+_proto("orbit_chain_fwd", C.c_int, [C.c_int] * 5 + [C.c_int, _vp, C.POINTER(_vp), C.POINTER(_vp), _vp, _vp, _sz, _vp])
+_proto("orbit_chain_bwd", C.c_int, [C.c_int] * 5 + [C.c_int, _vp, C.POINTER(_vp), C.POINTER(_vp), _vp, _vp, _sz, _vp])
+_proto("orbit_chain_workspace_bytes", _sz, [C.c_int] * 5 + [C.c_int])
+_proto("orbit_mse_loss_grad", C.c_int, [C.c_int, _sz, _vp, _vp, _vp, _vp, _vp])
+
+EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace_bytes", "orbit_var_aggregate",
+           "orbit_var_aggregate_bwd", "orbit_var_aggregate_workspace_bytes",
+           "orbit_var_aggregate_bwd_workspace_bytes", "orbit_var_aggregate_saved_bytes", "orbit_block_fwd",
+           "orbit_block_bwd", "orbit_block_fwd_workspace_bytes", "orbit_block_bwd_workspace_bytes",
+           "orbit_block_saved_bytes", "orbit_mse_loss_grad", "orbit_chain_fwd", "orbit_chain_bwd", "orbit_chain_workspace_bytes",
+           "orbit_last_error", "orbit_version", "orbit_launch_count", "orbit_reset_launch_count",
+           "orbit_set_debug_force_simt"]
+
+
+# ---- marshalling helpers --------------------------------------------------------------------------------------
+def _ptr(t):
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    assert t.is_cuda and t.is_contiguous(), "device-resident contiguous tensor required"
+    return t.data_ptr()
+
+
+def _stream(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return s.cuda_stream
+
+
+def _check(status, where):
+    if status != ORBIT_OK:
+        raise OrbitError(status, where)
+
+
+def embed_desc(B, V, Hg, Wg, p, D, dtype):
+    return orbit_embed_desc(B, V, Hg, Wg, p, D, DTYPES[dtype])
+
+
+def agg_desc(B, L, V, D, heads, dtype, resid_dtype):
+    return orbit_agg_desc(B, L, V, D, heads, DTYPES[dtype], DTYPES[resid_dtype])
+
+
+def block_desc(B, N, D, heads, F, T=1, ln_eps=1e-5, dtype="bf16", resid_dtype="bf16", flags=0):
+    return orbit_block_desc(B, N, D, heads, F, T, ln_eps, DTYPES[dtype], DTYPES[resid_dtype], flags)
+
+
+def _agg_struct(cls, P):
+    return cls(*[_ptr(P[n]) for n in _AGG_NAMES])
+
+
+def _block_struct(cls, common, shards):
+    arr = (orbit_block_shard * len(shards))(*[orbit_block_shard(*[_ptr(S[n]) for n in _SHARD_NAMES]) for S in shards])
+    st = cls(*[_ptr(common[n]) for n in _COMMON_NAMES], arr)
+    st._keep = arr
+    return st
+
+
+# ---- entry points (same names as the C-ABI) ------------------------------------------------------------------
+def orbit_tokenize(d, x, Wp, bp, tok, stream=None):
+    _check(lib.orbit_tokenize(C.byref(d), _ptr(x), _ptr(Wp), _ptr(bp), _ptr(tok), _stream(stream)), "orbit_tokenize")
+
+
+def orbit_tokenize_bwd_workspace_bytes(d):
+    return lib.orbit_tokenize_bwd_workspace_bytes(C.byref(d))
+
+
+def orbit_tokenize_bwd(d, x, dtok, dWp, dbp, ws, stream=None):
+    _check(lib.orbit_tokenize_bwd(C.byref(d), _ptr(x), _ptr(dtok), _ptr(dWp), _ptr(dbp), _ptr(ws), ws.numel() * ws.element_size(),
+                                  _stream(stream)), "orbit_tokenize_bwd")
+
+
+def orbit_var_aggregate_saved_bytes(d):
+    return lib.orbit_var_aggregate_saved_bytes(C.byref(d))
+
+
+def orbit_var_aggregate_workspace_bytes(d):
+    return lib.orbit_var_aggregate_workspace_bytes(C.byref(d))
+
+
+def orbit_var_aggregate_bwd_workspace_bytes(d):
+    return lib.orbit_var_aggregate_bwd_workspace_bytes(C.byref(d))
+
+
+def orbit_var_aggregate(d, tok, P, pos, agg, saved, ws, stream=None):
+    ps = _agg_struct(orbit_agg_params, P)
+    _check(lib.orbit_var_aggregate(C.byref(d), _ptr(tok), C.byref(ps), _ptr(pos), _ptr(agg), _ptr(saved), _ptr(ws),
+                                   ws.numel() * ws.element_size(), _stream(stream)), "orbit_var_aggregate")
+
+
+def orbit_var_aggregate_bwd(d, tok, P, dagg, saved, dtok, G, dpos, ws, stream=None):
+    ps = _agg_struct(orbit_agg_params, P)
+    gs = _agg_struct(orbit_agg_grads, G)
+    _check(lib.orbit_var_aggregate_bwd(C.byref(d), _ptr(tok), C.byref(ps), _ptr(dagg), _ptr(saved), _ptr(dtok),
+                                       C.byref(gs), _ptr(dpos), _ptr(ws), ws.numel() * ws.element_size(),
+                                       _stream(stream)), "orbit_var_aggregate_bwd")
+
+
+def orbit_block_saved_bytes(d):
+    return lib.orbit_block_saved_bytes(C.byref(d))
+
+
+def orbit_block_fwd_workspace_bytes(d):
+    return lib.orbit_block_fwd_workspace_bytes(C.byref(d))
+
+
+def orbit_block_bwd_workspace_bytes(d):
+    return lib.orbit_block_bwd_workspace_bytes(C.byref(d))
+
+
+def orbit_block_fwd(d, x, common, shards, y, saved, ws, stream=None):
+    """common: dict ln1_g, ln1_b, ln2_g, ln2_b, bproj, bfc2; shards: list of T dicts Wqkv, bqkv, Wproj, Wfc1, bfc1, Wfc2."""
+    ps = _block_struct(orbit_block_params, common, shards)
+    _check(lib.orbit_block_fwd(C.byref(d), _ptr(x), C.byref(ps), _ptr(y), _ptr(saved), _ptr(ws),
+                               ws.numel() * ws.element_size(), _stream(stream)), "orbit_block_fwd")
+
+
+def orbit_block_bwd(d, dy, common, shards, saved, dx, gcommon, gshards, ws, stream=None):
+    ps = _block_struct(orbit_block_params, common, shards)
+    gs = _block_struct(orbit_block_grads, gcommon, gshards)
+    _check(lib.orbit_block_bwd(C.byref(d), _ptr(dy), C.byref(ps), _ptr(saved), _ptr(dx), C.byref(gs), _ptr(ws),
+                               ws.numel() * ws.element_size(), _stream(stream)), "orbit_block_bwd")
+
+
+def _ptr_array(ts):
+    return (_vp * len(ts))(*[_ptr(t) for t in ts])
+
+
+def orbit_chain_workspace_bytes(m, d, n, e, T, dtype):
+    return lib.orbit_chain_workspace_bytes(m, d, n, e, T, DTYPES[dtype])
+
+
+def orbit_chain_fwd(m, d, n, e, T, dtype, x, A_cols, B_rows, y, ws, stream=None):
+    _check(lib.orbit_chain_fwd(m, d, n, e, T, DTYPES[dtype], _ptr(x), _ptr_array(A_cols), _ptr_array(B_rows), _ptr(y),
+                               _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)), "orbit_chain_fwd")
+
+
+def orbit_chain_bwd(m, d, n, e, T, dtype, dy, A_cols, B_rows, dx, ws, stream=None):
+    _check(lib.orbit_chain_bwd(m, d, n, e, T, DTYPES[dtype], _ptr(dy), _ptr_array(A_cols), _ptr_array(B_rows), _ptr(dx),
+                               _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)), "orbit_chain_bwd")
+
+
+def orbit_mse_loss_grad(dtype, y, t, dy, loss, stream=None):
+    _check(lib.orbit_mse_loss_grad(DTYPES[dtype], y.numel(), _ptr(y), _ptr(t), _ptr(dy), _ptr(loss), _stream(stream)),
+           "orbit_mse_loss_grad")
+
+
+def orbit_version():
+    return lib.orbit_version()
+
+
+def orbit_launch_count():
+    return lib.orbit_launch_count()
+
+
+def orbit_reset_launch_count():
+    lib.orbit_reset_launch_count()
+
+
+def orbit_set_debug_force_simt(on: bool):
+    lib.orbit_set_debug_force_simt(1 if on else 0)

@@ -1,0 +1,158 @@
+// api_common.cu -- error state, device check, diagnostics, tokenise and Eq.(2)/(3) chain entry points.
+#include <stdarg.h>
+#include <string.h>
+#include "api_util.cuh"
+#include "frontend.cuh"
+
+namespace orbit {
+
+static thread_local char g_err[512] = "";
+thread_local long long g_launches = 0;
+int g_force_simt = 0;
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int check_device() {
+  static thread_local int cached = -1;
+  if (cached >= 0) return cached;
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    set_error("no usable CUDA device");
+    return ORBIT_ERR_ARCH;
+  }
+  if (prop.major != 10) {
+    set_error("device '%s' is sm_%d%d; liborbit is built for sm_100a only (no fallback)", prop.name, prop.major,
+              prop.minor);
+    return ORBIT_ERR_ARCH;
+  }
+  cached = ORBIT_OK;
+  return cached;
+}
+
+bool valid_dtype(int dt) { return dt == ORBIT_F32 || dt == ORBIT_BF16; }
+bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
+
+}  // namespace orbit
+
+using namespace orbit;
+
+extern "C" {
+
+const char* orbit_last_error(void) { return g_err; }
+int orbit_version(void) { return ORBIT_VERSION; }
+long long orbit_launch_count(void) { return g_launches; }
+void orbit_reset_launch_count(void) { g_launches = 0; }
+void orbit_set_debug_force_simt(int on) { g_force_simt = on; }
+
+// ------------------------------------------------------------------------------------------------------
+// a1 / a1'
+// ------------------------------------------------------------------------------------------------------
+static int check_embed(const orbit_embed_desc* d) {
+  if (!d) { set_error("embed desc is NULL"); return ORBIT_ERR_NULL; }
+  if (!valid_dtype(d->dtype)) { set_error("embed: bad dtype %d", (int)d->dtype); return ORBIT_ERR_DTYPE; }
+  if (d->B <= 0 || d->V <= 0 || d->Hg <= 0 || d->Wg <= 0 || d->p <= 0 || d->D <= 0 || d->Hg % d->p || d->Wg % d->p ||
+      d->D % 8 || (d->p != 1 && d->p != 2 && d->p != 4)) {
+    set_error("embed: bad shape B=%d V=%d Hg=%d Wg=%d p=%d D=%d (need Hg%%p==0, Wg%%p==0, D%%8==0, p in {1,2,4})", d->B,
+              d->V, d->Hg, d->Wg, d->p, d->D);
+    return ORBIT_ERR_SHAPE;
+  }
+  return ORBIT_OK;
+}
+
+int orbit_tokenize(const orbit_embed_desc* d, const float* x, const void* Wp, const void* bp, void* tok, void* stream) {
+  ORBIT_TRY(check_embed(d));
+  if (!x || !Wp || !bp || !tok) { set_error("tokenize: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!aligned16(x) || !aligned16(Wp) || !aligned16(bp) || !aligned16(tok)) { set_error("tokenize: pointer not 16B aligned"); return ORBIT_ERR_ALIGN; }
+  ORBIT_TRY(check_device());
+  return tokenize_fwd(*d, x, Wp, bp, tok, (cudaStream_t)stream);
+}
+
+size_t orbit_tokenize_bwd_workspace_bytes(const orbit_embed_desc* d) {
+  if (!d) return 0;
+  return align_up((size_t)d->V * (d->p * d->p + 1) * d->D * sizeof(float), 256);
+}
+
+int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dtok, void* dWp, void* dbp, void* ws,
+                       size_t ws_bytes, void* stream) {
+  ORBIT_TRY(check_embed(d));
+  if (!x || !dtok || !dWp || !dbp || !ws) { set_error("tokenize_bwd: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!aligned16(x) || !aligned16(dtok) || !aligned16(dWp) || !aligned16(dbp) || !aligned16(ws)) { set_error("tokenize_bwd: pointer not 16B aligned"); return ORBIT_ERR_ALIGN; }
+  if (ws_bytes < orbit_tokenize_bwd_workspace_bytes(d)) { set_error("tokenize_bwd: workspace too small"); return ORBIT_ERR_WORKSPACE; }
+  ORBIT_TRY(check_device());
+  cudaStream_t s = (cudaStream_t)stream;
+  const int P2 = d->p * d->p;
+  float* accW = (float*)ws;
+  float* accB = accW + (size_t)d->V * P2 * d->D;
+  ORBIT_TRY(fill_zero(ws, (size_t)d->V * (P2 + 1) * d->D * sizeof(float), s));
+  ORBIT_TRY(tokenize_bwd_acc(*d, x, dtok, accW, accB, s));
+  ORBIT_TRY(cast_copy(accW, ORBIT_F32, dWp, d->dtype, (size_t)d->V * P2 * d->D, s));
+  ORBIT_TRY(cast_copy(accB, ORBIT_F32, dbp, d->dtype, (size_t)d->V * d->D, s));
+  return ORBIT_OK;
+}
+
+int orbit_mse_loss_grad(orbit_dtype dtype, size_t n, const void* y, const void* t, void* dy, float* loss, void* stream) {
+  if (!y || !t || !dy || !loss) { set_error("mse: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!valid_dtype(dtype)) { set_error("mse: bad dtype"); return ORBIT_ERR_DTYPE; }
+  ORBIT_TRY(check_device());
+  return mse_loss_grad(y, t, dtype, dy, loss, n, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Eq. (2) / Eq. (3) chain
+// ------------------------------------------------------------------------------------------------------
+size_t orbit_chain_workspace_bytes(int m, int d, int n, int e, int T, orbit_dtype dtype) {
+  if (T <= 0) return 0;
+  size_t big = (size_t)(d > e ? d : e);
+  return align_up((size_t)m * (n / T) * dsize(dtype), 256) + align_up((size_t)m * big * sizeof(float), 256);
+}
+
+static int chain_common(int m, int d, int n, int e, int T, orbit_dtype dtype, const void* in, const void* const* A_cols,
+                        const void* const* B_rows, void* out, void* ws, size_t ws_bytes, void* stream, bool bwd) {
+  if (!in || !A_cols || !B_rows || !out || !ws) { set_error("chain: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!valid_dtype(dtype)) { set_error("chain: bad dtype"); return ORBIT_ERR_DTYPE; }
+  if (m <= 0 || d <= 0 || n <= 0 || e <= 0 || T <= 0 || n % T) { set_error("chain: bad shape"); return ORBIT_ERR_SHAPE; }
+  for (int k = 0; k < T; k++)
+    if (!A_cols[k] || !B_rows[k]) { set_error("chain: NULL shard pointer"); return ORBIT_ERR_NULL; }
+  if (ws_bytes < orbit_chain_workspace_bytes(m, d, n, e, T, dtype)) { set_error("chain: workspace too small"); return ORBIT_ERR_WORKSPACE; }
+  ORBIT_TRY(check_device());
+  cudaStream_t s = (cudaStream_t)stream;
+  const int nk = n / T;
+  void* tmp = ws;
+  float* acc = (float*)((char*)ws + align_up((size_t)m * nk * dsize(dtype), 256));
+  const int outw = bwd ? d : e;
+  for (int k = 0; k < T; k++) {
+    GemmArgs g1, g2;
+    g1.in_dtype = g2.in_dtype = dtype;
+    g1.M = m; g1.N = nk; g1.C = tmp; g1.ldc = nk; g1.out_dtype = dtype;
+    g2.M = m; g2.K = nk; g2.A = tmp; g2.a_rs = nk; g2.a_cs = 1; g2.C = acc; g2.ldc = outw; g2.out_dtype = ORBIT_F32;
+    g2.accumulate = k > 0; g2.N = outw;
+    if (!bwd) {  // t = x A_k ; y += t B_k
+      g1.K = d; g1.A = in; g1.a_rs = d; g1.a_cs = 1; g1.B = A_cols[k]; g1.b_rs = nk; g1.b_cs = 1;
+      g2.B = B_rows[k]; g2.b_rs = e; g2.b_cs = 1;
+    } else {     // t = dy B_k^T ; dx += t A_k^T
+      g1.K = e; g1.A = in; g1.a_rs = e; g1.a_cs = 1; g1.B = B_rows[k]; g1.b_rs = 1; g1.b_cs = e;
+      g2.B = A_cols[k]; g2.b_rs = 1; g2.b_cs = nk;
+    }
+    ORBIT_TRY(gemm(g1, s));
+    ORBIT_TRY(gemm(g2, s));
+  }
+  return cast_copy(acc, ORBIT_F32, out, dtype, (size_t)m * outw, s);
+}
+
+int orbit_chain_fwd(int m, int d, int n, int e, int T, orbit_dtype dtype, const void* x, const void* const* A_cols,
+                    const void* const* B_rows, void* y, void* ws, size_t ws_bytes, void* stream) {
+  return chain_common(m, d, n, e, T, dtype, x, A_cols, B_rows, y, ws, ws_bytes, stream, false);
+}
+int orbit_chain_bwd(int m, int d, int n, int e, int T, orbit_dtype dtype, const void* dy, const void* const* A_cols,
+                    const void* const* B_rows, void* dx, void* ws, size_t ws_bytes, void* stream) {
+  return chain_common(m, d, n, e, T, dtype, dy, A_cols, B_rows, dx, ws, ws_bytes, stream, true);
+}
+
+}  // extern "C"

@@ -1,0 +1,153 @@
+// common.cuh -- shared device/host helpers of liborbit (sm_100a).  Not shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "../../include/orbit.h"
+
+namespace orbit {
+
+typedef __nv_bfloat16 bf16;
+
+// ---- error state (thread-local) --------------------------------------------------------------
+void set_error(const char* fmt, ...);
+extern thread_local long long g_launches;
+extern int g_force_simt;
+inline void count_launch(int n = 1) { g_launches += n; }
+
+#define ORBIT_CUDA_CHECK(expr)                                                                   \
+  do {                                                                                           \
+    cudaError_t _e = (expr);                                                                     \
+    if (_e != cudaSuccess) {                                                                     \
+      orbit::set_error("%s:%d %s -> %s", __FILE__, __LINE__, #expr, cudaGetErrorString(_e));     \
+      return ORBIT_ERR_CUDA;                                                                     \
+    }                                                                                            \
+  } while (0)
+
+#define ORBIT_LAUNCH_CHECK()                                                                     \
+  do {                                                                                           \
+    orbit::count_launch();                                                                       \
+    cudaError_t _e = cudaGetLastError();                                                         \
+    if (_e != cudaSuccess) {                                                                     \
+      orbit::set_error("%s:%d launch -> %s", __FILE__, __LINE__, cudaGetErrorString(_e));        \
+      return ORBIT_ERR_CUDA;                                                                     \
+    }                                                                                            \
+  } while (0)
+
+#define ORBIT_TRY(expr)                                                                          \
+  do {                                                                                           \
+    int _s = (expr);                                                                             \
+    if (_s != ORBIT_OK) return _s;                                                               \
+  } while (0)
+
+inline size_t dsize(int dt) { return dt == ORBIT_BF16 ? 2 : 4; }
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// ---- runtime-dtype scalar access (warp-uniform branch) ----------------------------------------
+__device__ __forceinline__ float ldf(const void* p, size_t i, int dt) {
+  return dt == ORBIT_BF16 ? __bfloat162float(((const bf16*)p)[i]) : ((const float*)p)[i];
+}
+__device__ __forceinline__ void stf(void* p, size_t i, float v, int dt) {
+  if (dt == ORBIT_BF16) ((bf16*)p)[i] = __float2bfloat16_rn(v);
+  else ((float*)p)[i] = v;
+}
+template <typename T> __device__ __forceinline__ float to_f(T v);
+template <> __device__ __forceinline__ float to_f<float>(float v) { return v; }
+template <> __device__ __forceinline__ float to_f<bf16>(bf16 v) { return __bfloat162float(v); }
+template <typename T> __device__ __forceinline__ T from_f(float v);
+template <> __device__ __forceinline__ float from_f<float>(float v) { return v; }
+template <> __device__ __forceinline__ bf16 from_f<bf16>(float v) { return __float2bfloat16_rn(v); }
+
+// ---- math --------------------------------------------------------------------------------------
+// exact-erf GELU ("GeLU"; reading R7) and its derivative Phi(u) + u phi(u)
+__device__ __forceinline__ float gelu_f(float u) { return 0.5f * u * (1.0f + erff(u * 0.70710678118654752f)); }
+__device__ __forceinline__ float gelu_grad_f(float u) {
+  float Phi = 0.5f * (1.0f + erff(u * 0.70710678118654752f));
+  float phi = 0.39894228040143268f * __expf(-0.5f * u * u);
+  return Phi + u * phi;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+// block-wide sum, blockDim.x multiple of 32, <= 1024 threads; `sh` >= 32 floats
+__device__ __forceinline__ float block_sum(float v, float* sh) {
+  int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) sh[w] = v;
+  __syncthreads();
+  float r = lane < nw ? sh[lane] : 0.f;
+  r = warp_sum(r);
+  return r;
+}
+
+// ---- internal GEMM interface ---------------------------------------------------------------------
+// C[m,n] = epi( alpha * sum_k A(m,k) B(k,n) ), A(m,k) = A[m*a_rs + k*a_cs], B(k,n) = B[k*b_rs + n*b_cs]
+enum { ACT_NONE = 0, ACT_GELU = 1 /* C = gelu(v), aux_out = v */, ACT_GELU_GRAD = 2 /* C = v * gelu'(aux_in) */ };
+struct GemmArgs {
+  const void* A = nullptr; long long a_rs = 0, a_cs = 0;
+  const void* B = nullptr; long long b_rs = 0, b_cs = 0;
+  void* C = nullptr; long long ldc = 0;
+  int M = 0, N = 0, K = 0;
+  int in_dtype = ORBIT_F32;      // dtype of A and B
+  int out_dtype = ORBIT_F32;     // dtype of C (and aux_out)
+  float alpha = 1.f;
+  const void* bias = nullptr; int bias_dtype = ORBIT_F32;              // [N]
+  const void* resid = nullptr; int resid_dtype = ORBIT_F32; long long ldr = 0; int resid_row_mod = 0;
+  int accumulate = 0;            // C += (only meaningful for fp32 C)
+  int act = ACT_NONE;
+  void* aux_out = nullptr; const void* aux_in = nullptr; long long ld_aux = 0; int aux_dtype = ORBIT_F32;
+};
+int gemm(const GemmArgs& g, cudaStream_t s);           // dispatcher (tensor-core path or SIMT)
+int gemm_simt(const GemmArgs& g, cudaStream_t s);      // fp32-FMA kernels, any dtype/stride
+int gemm_tc(const GemmArgs& g, cudaStream_t s);        // tcgen05 + TMA, bf16 in / fp32 accumulate
+bool gemm_tc_supported(const GemmArgs& g);
+
+// ---- row-wise / reduction kernels (rowops.cu) -----------------------------------------------------
+int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,
+                  float* mean, float* rstd, int M, int D, float eps, void* x_copy, cudaStream_t s);
+// dz from d(out); dx_out = add (nullable, add_dt) + dz, written as f32 to dx_f32 (nullable) and as out_dt to
+// dx_out (nullable); dgamma/dbeta accumulated into fp32 acc buffers (zeroed by the caller).
+int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
+                  const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
+                  int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s);
+// out[n] = sum_m in[m*ld + n]  (fp32 atomics into acc, caller zeroes) ; optional bf16/f32 copy of `in`
+int colsum(const void* in, int in_dt, long long ld, int M, int N, float* acc, void* copy_out, int copy_dt,
+           long long ld_copy, cudaStream_t s);
+int cast_copy(const void* in, int in_dt, void* out, int out_dt, size_t n, cudaStream_t s);
+int fill_zero(void* p, size_t bytes, cudaStream_t s);
+// out = a (a_dt) + b_f32 + bias (p_dt)  (combine of fp32 Hybrid-STOP partials)
+int add_partial(const void* a, int a_dt, const float* part, const void* bias, int p_dt, void* out, int out_dt,
+                int M, int D, cudaStream_t s);
+
+int mse_loss_grad(const void* y, const void* t, int dt, void* dy, float* loss, size_t n, cudaStream_t s);
+
+// ---- attention (attention_simt.cu / attention_tc.cu) ------------------------------------------------
+// qkv: [B*N, ld] with Q at column q_off + j*dh, K at k_off + j*dh, V at v_off + j*dh for head j
+struct AttnArgs {
+  const void* qkv = nullptr; long long ld = 0; int q_off = 0, k_off = 0, v_off = 0;
+  int B = 0, N = 0, heads = 0, dh = 0; int dtype = ORBIT_F32;
+  void* O = nullptr; long long ldo = 0;               // [B*N, heads*dh]
+  float* lse = nullptr;                               // [B, heads, N] natural-log sum-exp of scaled logits
+  // backward
+  const void* dO = nullptr; long long lddo = 0;
+  void* dqkv = nullptr;                               // same layout as qkv
+  float* delta = nullptr;                             // [B, heads, N] workspace
+  float* dq_acc = nullptr;                            // [B*N, heads*dh] fp32 workspace (tensor-core path)
+};
+int attention_fwd(const AttnArgs& a, cudaStream_t s);
+int attention_bwd(const AttnArgs& a, cudaStream_t s);
+int attention_fwd_simt(const AttnArgs& a, cudaStream_t s);
+int attention_bwd_simt(const AttnArgs& a, cudaStream_t s);
+
+}  // namespace orbit

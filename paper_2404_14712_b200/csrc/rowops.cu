@@ -1,0 +1,335 @@
+// rowops.cu -- HBM-bound row-wise kernels: LayerNorm fwd/bwd, column sums (bias grads), casts, combines.
+// All are one pass over their inputs with 16-byte vector accesses; statistics and sums in fp32.
+#include "common.cuh"
+
+namespace orbit {
+
+namespace {
+
+// 8 consecutive elements starting at element index i (i % 8 == 0, base 16B aligned)
+__device__ __forceinline__ void ld8(const void* p, size_t i, int dt, float* v) {
+  if (dt == ORBIT_BF16) {
+    uint4 raw = *reinterpret_cast<const uint4*>((const bf16*)p + i);
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&raw);
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+      float2 f = __bfloat1622float2(h[j]);
+      v[2 * j] = f.x; v[2 * j + 1] = f.y;
+    }
+  } else {
+    const float4* q = reinterpret_cast<const float4*>((const float*)p + i);
+    float4 a = q[0], b = q[1];
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+  }
+}
+__device__ __forceinline__ void st8(void* p, size_t i, int dt, const float* v) {
+  if (dt == ORBIT_BF16) {
+    uint4 raw;
+    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&raw);
+#pragma unroll
+    for (int j = 0; j < 4; j++) h[j] = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+    *reinterpret_cast<uint4*>((bf16*)p + i) = raw;
+  } else {
+    float4* q = reinterpret_cast<float4*>((float*)p + i);
+    q[0] = make_float4(v[0], v[1], v[2], v[3]);
+    q[1] = make_float4(v[4], v[5], v[6], v[7]);
+  }
+}
+
+__device__ __forceinline__ float2 block_sum2(float2 v, float2* sh) {
+  int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v.x = warp_sum(v.x); v.y = warp_sum(v.y);
+  __syncthreads();
+  if (lane == 0) sh[w] = v;
+  __syncthreads();
+  float2 r = lane < nw ? sh[lane] : make_float2(0.f, 0.f);
+  r.x = warp_sum(r.x); r.y = warp_sum(r.y);
+  return r;
+}
+
+// ---- LayerNorm forward: one block per row (persistent over rows), row cached in registers ------------
+template <int MAXCH>
+__global__ void __launch_bounds__(1024) ln_fwd_kernel(const void* __restrict__ x, int x_dt,
+    const void* __restrict__ gamma, const void* __restrict__ beta, int p_dt, void* __restrict__ out, int out_dt,
+    float* __restrict__ mean, float* __restrict__ rstd, int M, int D, float eps, void* __restrict__ x_copy) {
+  __shared__ float2 sh[32];
+  const int nch = D >> 3;
+  for (int row = blockIdx.x; row < M; row += gridDim.x) {
+    float v[MAXCH][8];
+    float s = 0.f;
+#pragma unroll
+    for (int c = 0; c < MAXCH; c++) {
+      int ch = threadIdx.x + c * blockDim.x;
+      if (ch < nch) {
+        ld8(x, (size_t)row * D + (size_t)ch * 8, x_dt, v[c]);
+        if (x_copy) st8(x_copy, (size_t)row * D + (size_t)ch * 8, x_dt, v[c]);
+#pragma unroll
+        for (int j = 0; j < 8; j++) s += v[c][j];
+      }
+    }
+    float2 r = block_sum2(make_float2(s, 0.f), sh);
+    const float mu = r.x / D;
+    float q = 0.f;
+#pragma unroll
+    for (int c = 0; c < MAXCH; c++) {
+      int ch = threadIdx.x + c * blockDim.x;
+      if (ch < nch) {
+#pragma unroll
+        for (int j = 0; j < 8; j++) { float d = v[c][j] - mu; q += d * d; }
+      }
+    }
+    r = block_sum2(make_float2(q, 0.f), sh);
+    const float rs = rsqrtf(r.x / D + eps);
+    if (threadIdx.x == 0) { mean[row] = mu; rstd[row] = rs; }
+#pragma unroll
+    for (int c = 0; c < MAXCH; c++) {
+      int ch = threadIdx.x + c * blockDim.x;
+      if (ch < nch) {
+        float g[8], b[8], o[8];
+        ld8(gamma, (size_t)ch * 8, p_dt, g);
+        ld8(beta, (size_t)ch * 8, p_dt, b);
+#pragma unroll
+        for (int j = 0; j < 8; j++) o[j] = (v[c][j] - mu) * rs * g[j] + b[j];
+        st8(out, (size_t)row * D + (size_t)ch * 8, out_dt, o);
+      }
+    }
+  }
+}
+
+// ---- LayerNorm backward ------------------------------------------------------------------------------
+template <int MAXCH>
+__global__ void __launch_bounds__(1024) ln_bwd_kernel(const void* __restrict__ dout, int dout_dt,
+    const void* __restrict__ x, int x_dt, const float* __restrict__ mean, const float* __restrict__ rstd,
+    const void* __restrict__ gamma, int p_dt, const void* __restrict__ add, int add_dt,
+    float* __restrict__ dx_f32, void* __restrict__ dx_out, int out_dt,
+    float* __restrict__ dgamma_acc, float* __restrict__ dbeta_acc, int M, int D) {
+  __shared__ float2 sh[32];
+  const int nch = D >> 3;
+  float dg[MAXCH][8], db[MAXCH][8], gm[MAXCH][8];
+#pragma unroll
+  for (int c = 0; c < MAXCH; c++) {
+    int ch = threadIdx.x + c * blockDim.x;
+#pragma unroll
+    for (int j = 0; j < 8; j++) { dg[c][j] = 0.f; db[c][j] = 0.f; gm[c][j] = 0.f; }
+    if (ch < nch) ld8(gamma, (size_t)ch * 8, p_dt, gm[c]);
+  }
+  for (int row = blockIdx.x; row < M; row += gridDim.x) {
+    const float mu = mean[row], rs = rstd[row];
+    float zh[MAXCH][8], gh[MAXCH][8];
+    float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int c = 0; c < MAXCH; c++) {
+      int ch = threadIdx.x + c * blockDim.x;
+      if (ch < nch) {
+        float xv[8], dv[8];
+        ld8(x, (size_t)row * D + (size_t)ch * 8, x_dt, xv);
+        ld8(dout, (size_t)row * D + (size_t)ch * 8, dout_dt, dv);
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+          float z = (xv[j] - mu) * rs;
+          zh[c][j] = z;
+          dg[c][j] += dv[j] * z;
+          db[c][j] += dv[j];
+          float g = dv[j] * gm[c][j];
+          gh[c][j] = g;
+          s1 += g; s2 += g * z;
+        }
+      }
+    }
+    float2 r = block_sum2(make_float2(s1, s2), sh);
+    const float m1 = r.x / D, m2 = r.y / D;
+#pragma unroll
+    for (int c = 0; c < MAXCH; c++) {
+      int ch = threadIdx.x + c * blockDim.x;
+      if (ch < nch) {
+        float o[8];
+        size_t off = (size_t)row * D + (size_t)ch * 8;
+        if (add) ld8(add, off, add_dt, o);
+        else {
+#pragma unroll
+          for (int j = 0; j < 8; j++) o[j] = 0.f;
+        }
+#pragma unroll
+        for (int j = 0; j < 8; j++) o[j] += (gh[c][j] - m1 - zh[c][j] * m2) * rs;
+        if (dx_f32) st8(dx_f32, off, ORBIT_F32, o);
+        if (dx_out) st8(dx_out, off, out_dt, o);
+      }
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < MAXCH; c++) {
+    int ch = threadIdx.x + c * blockDim.x;
+    if (ch < nch) {
+#pragma unroll
+      for (int j = 0; j < 8; j++) {
+        atomicAdd(dgamma_acc + (size_t)ch * 8 + j, dg[c][j]);
+        atomicAdd(dbeta_acc + (size_t)ch * 8 + j, db[c][j]);
+      }
+    }
+  }
+}
+
+// ---- column sums (+ optional dtype-converting copy) ---------------------------------------------------
+__global__ void __launch_bounds__(256) colsum_kernel(const void* __restrict__ in, int in_dt, long long ld, int M,
+    int N, float* __restrict__ acc, void* __restrict__ copy_out, int copy_dt, long long ld_copy,
+    int rows_per_block) {
+  __shared__ float sh[8][32][9];
+  const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
+  const int col = (blockIdx.x * 32 + cx) * 8;
+  const int r0 = blockIdx.y * rows_per_block;
+  const int r1 = min(M, r0 + rows_per_block);
+  float s[8];
+#pragma unroll
+  for (int j = 0; j < 8; j++) s[j] = 0.f;
+  if (col < N) {
+    for (int r = r0 + ry; r < r1; r += 8) {
+      float v[8];
+      ld8(in, (size_t)r * ld + col, in_dt, v);
+#pragma unroll
+      for (int j = 0; j < 8; j++) s[j] += v[j];
+      if (copy_out) st8(copy_out, (size_t)r * ld_copy + col, copy_dt, v);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 8; j++) sh[ry][cx][j] = s[j];
+  __syncthreads();
+  if (ry == 0 && col < N) {
+#pragma unroll
+    for (int j = 0; j < 8; j++) {
+      float t = 0.f;
+#pragma unroll
+      for (int y = 0; y < 8; y++) t += sh[y][cx][j];
+      atomicAdd(acc + col + j, t);
+    }
+  }
+}
+
+__global__ void cast_kernel(const void* __restrict__ in, int in_dt, void* __restrict__ out, int out_dt, size_t n) {
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  size_t nv = n >> 3;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += stride) {
+    float v[8];
+    ld8(in, i * 8, in_dt, v);
+    st8(out, i * 8, out_dt, v);
+  }
+  for (size_t i = (nv << 3) + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+    stf(out, i, ldf(in, i, in_dt), out_dt);
+}
+
+__global__ void add_partial_kernel(const void* __restrict__ a, int a_dt, const float* __restrict__ part,
+    const void* __restrict__ bias, int p_dt, void* __restrict__ out, int out_dt, size_t n8, int D8) {
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += stride) {
+    float va[8], vp[8], vb[8], o[8];
+    ld8(a, i * 8, a_dt, va);
+    ld8(part, i * 8, ORBIT_F32, vp);
+    ld8(bias, (i % D8) * 8, p_dt, vb);
+#pragma unroll
+    for (int j = 0; j < 8; j++) o[j] = va[j] + vp[j] + vb[j];
+    st8(out, i * 8, out_dt, o);
+  }
+}
+
+// dy = 2 (y - t) / n ; loss += sum (y - t)^2 / n      (harness loss, BASELINE.json config 1: MSE)
+__global__ void mse_kernel(const void* __restrict__ y, const void* __restrict__ t, int dt, void* __restrict__ dy,
+                           float* __restrict__ loss, size_t n) {
+  __shared__ float sh[32];
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  float acc = 0.f;
+  const float inv = 1.0f / (float)n;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    float d = ldf(y, i, dt) - ldf(t, i, dt);
+    acc += d * d;
+    stf(dy, i, 2.f * d * inv, dt);
+  }
+  acc = block_sum(acc, sh);
+  if (threadIdx.x == 0) atomicAdd(loss, acc * inv);
+}
+
+int ln_threads(int D) {
+  int nch = D / 8;
+  int t = ((nch + 31) / 32) * 32;
+  return t > 1024 ? 1024 : t;
+}
+}  // namespace
+
+int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,
+                  float* mean, float* rstd, int M, int D, float eps, void* x_copy, cudaStream_t s) {
+  int thr = ln_threads(D);
+  int maxch = cdiv(D / 8, thr);
+  int grid = M < 148 * 4 ? M : 148 * 4;
+  if (maxch <= 1) ln_fwd_kernel<1><<<grid, thr, 0, s>>>(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy);
+  else if (maxch <= 2) ln_fwd_kernel<2><<<grid, thr, 0, s>>>(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy);
+  else if (maxch <= 4) ln_fwd_kernel<4><<<grid, thr, 0, s>>>(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy);
+  else if (maxch <= 8) ln_fwd_kernel<8><<<grid, thr, 0, s>>>(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy);
+  else { set_error("layernorm: D=%d too large", D); return ORBIT_ERR_SHAPE; }
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
+                  const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
+                  int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s) {
+  int thr = ln_threads(D);
+  int maxch = cdiv(D / 8, thr);
+  int grid = M < 148 * 2 ? M : 148 * 2;
+#define LNB(C) ln_bwd_kernel<C><<<grid, thr, 0, s>>>(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, \
+                                                     dx_f32, dx_out, out_dt, dgamma_acc, dbeta_acc, M, D)
+  if (maxch <= 1) LNB(1);
+  else if (maxch <= 2) LNB(2);
+  else if (maxch <= 4) LNB(4);
+  else { set_error("layernorm_bwd: D=%d too large", D); return ORBIT_ERR_SHAPE; }
+#undef LNB
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int colsum(const void* in, int in_dt, long long ld, int M, int N, float* acc, void* copy_out, int copy_dt,
+           long long ld_copy, cudaStream_t s) {
+  int gx = cdiv(N, 256);
+  int want_y = cdiv(148 * 4, gx);
+  int rows_per_block = cdiv(M, want_y);
+  rows_per_block = ((rows_per_block + 7) / 8) * 8;
+  if (rows_per_block < 8) rows_per_block = 8;
+  dim3 grid(gx, cdiv(M, rows_per_block));
+  colsum_kernel<<<grid, 256, 0, s>>>(in, in_dt, ld, M, N, acc, copy_out, copy_dt, ld_copy, rows_per_block);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int cast_copy(const void* in, int in_dt, void* out, int out_dt, size_t n, cudaStream_t s) {
+  if (n == 0) return ORBIT_OK;
+  size_t blocks = (n / 8 + 255) / 256;
+  if (blocks < 1) blocks = 1;
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  cast_kernel<<<(int)blocks, 256, 0, s>>>(in, in_dt, out, out_dt, n);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fill_zero(void* p, size_t bytes, cudaStream_t s) {
+  if (bytes == 0) return ORBIT_OK;
+  ORBIT_CUDA_CHECK(cudaMemsetAsync(p, 0, bytes, s));
+  return ORBIT_OK;
+}
+
+int mse_loss_grad(const void* y, const void* t, int dt, void* dy, float* loss, size_t n, cudaStream_t s) {
+  ORBIT_CUDA_CHECK(cudaMemsetAsync(loss, 0, sizeof(float), s));
+  size_t blocks = (n + 255) / 256;
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  mse_kernel<<<(int)blocks, 256, 0, s>>>(y, t, dt, dy, loss, n);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int add_partial(const void* a, int a_dt, const float* part, const void* bias, int p_dt, void* out, int out_dt,
+                int M, int D, cudaStream_t s) {
+  size_t n8 = (size_t)M * D / 8;
+  size_t blocks = (n8 + 255) / 256;
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  add_partial_kernel<<<(int)blocks, 256, 0, s>>>(a, a_dt, part, bias, p_dt, out, out_dt, n8, D / 8);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+}  // namespace orbit

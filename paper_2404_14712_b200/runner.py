@@ -1,0 +1,149 @@
+"""Sequencing of the C-ABI calls for a whole ORBIT step (the public Python API a user calls).
+
+No arithmetic lives here: tensors are allocated with torch (device memory only), parameters are copied to
+the device, and the liborbit entry points are called in order on the current stream:
+    orbit_tokenize -> orbit_var_aggregate -> depth x orbit_block_fwd -> orbit_mse_loss_grad
+    -> depth x orbit_block_bwd -> orbit_var_aggregate_bwd -> orbit_tokenize_bwd
+(SURVEY.md §3(ii)).
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as ob
+from .inputs import Config
+
+TD = ob.TORCH_DTYPES
+
+
+def to_dev(a: np.ndarray, dtype: str, device="cuda") -> torch.Tensor:
+    """numpy (float32 holding storage-exact values) -> device tensor of the storage dtype."""
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(device=device, dtype=TD[dtype]).contiguous()
+
+
+def to_np(t: torch.Tensor) -> np.ndarray:
+    return t.detach().to(torch.float32).cpu().numpy()
+
+
+def _bytes(n, device="cuda"):
+    return torch.empty(max(int(n), 256), dtype=torch.uint8, device=device)
+
+
+class BlockRunner:
+    """One ViT block (optionally Hybrid-STOP sharded) behind orbit_block_fwd / orbit_block_bwd."""
+
+    COMMON = ob._COMMON_NAMES
+    SHARD = ob._SHARD_NAMES
+
+    def __init__(self, B, N, D, heads, F, T, dtype, resid_dtype, common: dict, shards: list, ln_eps=1e-5,
+                 device="cuda"):
+        self.desc = ob.block_desc(B, N, D, heads, F, T, ln_eps, dtype, resid_dtype)
+        self.B, self.N, self.D, self.heads, self.F, self.T = B, N, D, heads, F, T
+        self.dtype, self.resid_dtype, self.device = dtype, resid_dtype, device
+        self.common = {k: to_dev(common[k], dtype, device) for k in self.COMMON}
+        self.shards = [{k: to_dev(S[k], dtype, device) for k in self.SHARD} for S in shards]
+        self.gcommon = {k: torch.empty_like(v) for k, v in self.common.items()}
+        self.gshards = [{k: torch.empty_like(v) for k, v in S.items()} for S in self.shards]
+        self.saved = _bytes(ob.orbit_block_saved_bytes(self.desc), device)
+        self.ws_f = _bytes(ob.orbit_block_fwd_workspace_bytes(self.desc), device)
+        self.ws_b = None
+        self.y = torch.empty(B, N, D, dtype=TD[resid_dtype], device=device)
+        self.dx = torch.empty(B, N, D, dtype=TD[resid_dtype], device=device)
+
+    def share_bwd_ws(self, ws):
+        self.ws_b = ws
+
+    def fwd(self, x):
+        ob.orbit_block_fwd(self.desc, x, self.common, self.shards, self.y, self.saved, self.ws_f)
+        return self.y
+
+    def bwd(self, dy):
+        if self.ws_b is None:
+            self.ws_b = _bytes(ob.orbit_block_bwd_workspace_bytes(self.desc), self.device)
+        ob.orbit_block_bwd(self.desc, dy, self.common, self.shards, self.saved, self.dx, self.gcommon, self.gshards,
+                           self.ws_b)
+        return self.dx
+
+
+class FrontRunner:
+    """orbit_tokenize + orbit_var_aggregate and their backward."""
+
+    def __init__(self, B, V, Hg, Wg, p, D, heads, dtype, resid_dtype, emb: dict, agg: dict, pos=None, device="cuda"):
+        self.L = (Hg // p) * (Wg // p)
+        self.ed = ob.embed_desc(B, V, Hg, Wg, p, D, dtype)
+        self.ad = ob.agg_desc(B, self.L, V, D, heads, dtype, resid_dtype)
+        self.dtype, self.resid_dtype, self.device = dtype, resid_dtype, device
+        self.Wp, self.bp = to_dev(emb["Wp"], dtype, device), to_dev(emb["bp"], dtype, device)
+        self.agg = {k: to_dev(agg[k], dtype, device) for k in ob._AGG_NAMES}
+        self.pos = None if pos is None else to_dev(pos, resid_dtype, device)
+        self.tok = torch.empty(B, self.L, V, D, dtype=TD[dtype], device=device)
+        self.out = torch.empty(B, self.L, D, dtype=TD[resid_dtype], device=device)
+        self.saved = _bytes(ob.orbit_var_aggregate_saved_bytes(self.ad), device)
+        self.ws_f = _bytes(ob.orbit_var_aggregate_workspace_bytes(self.ad), device)
+        self.ws_b = None
+        self.dtok = None
+        self.gagg = {k: torch.empty_like(v) for k, v in self.agg.items()}
+        self.dpos = None if pos is None else torch.empty_like(self.pos)
+        self.dWp, self.dbp = torch.empty_like(self.Wp), torch.empty_like(self.bp)
+        self.ws_t = _bytes(ob.orbit_tokenize_bwd_workspace_bytes(self.ed), device)
+
+    def fwd(self, x):
+        ob.orbit_tokenize(self.ed, x, self.Wp, self.bp, self.tok)
+        ob.orbit_var_aggregate(self.ad, self.tok, self.agg, self.pos, self.out, self.saved, self.ws_f)
+        return self.out
+
+    def bwd(self, dagg):
+        if self.ws_b is None:
+            self.ws_b = _bytes(ob.orbit_var_aggregate_bwd_workspace_bytes(self.ad), self.device)
+            self.dtok = torch.empty_like(self.tok)
+        ob.orbit_var_aggregate_bwd(self.ad, self.tok, self.agg, dagg, self.saved, self.dtok, self.gagg, self.dpos,
+                                   self.ws_b)
+        ob.orbit_tokenize_bwd(self.ed, self.x_last, self.dtok, self.dWp, self.dbp, self.ws_t)
+
+    def fwd_keep(self, x):
+        self.x_last = x
+        return self.fwd(x)
+
+
+class StepRunner:
+    """Whole hot path for a Config: tokenise -> aggregate -> depth x block, forward + backward, MSE loss."""
+
+    def __init__(self, cfg: Config, emb=None, agg=None, blocks=None, pos=None, device="cuda"):
+        self.cfg = cfg
+        self.front = None
+        if cfg.V is not None:
+            self.front = FrontRunner(cfg.B, cfg.V, cfg.Hg, cfg.Wg, cfg.p, cfg.D, cfg.heads, cfg.dtype, cfg.resid_dtype,
+                                     emb, agg, pos, device)
+        self.blocks = []
+        ws = None
+        for common, shards in blocks:
+            br = BlockRunner(cfg.B, cfg.L, cfg.D, cfg.heads, cfg.F, cfg.T, cfg.dtype, cfg.resid_dtype, common, shards,
+                             cfg.ln_eps, device)
+            if ws is None:
+                ws = _bytes(ob.orbit_block_bwd_workspace_bytes(br.desc), device)
+            br.share_bwd_ws(ws)
+            self.blocks.append(br)
+        self.loss = torch.zeros(1, dtype=torch.float32, device=device)
+        self.dy = torch.empty(cfg.B, cfg.L, cfg.D, dtype=TD[cfg.resid_dtype], device=device)
+
+    def forward(self, x):
+        h = self.front.fwd_keep(x) if self.front is not None else x
+        for b in self.blocks:
+            h = b.fwd(h)
+        return h
+
+    def backward(self, dy):
+        g = dy
+        for b in reversed(self.blocks):
+            g = b.bwd(g)
+        if self.front is not None:
+            self.front.bwd(g)
+        return g
+
+    def step(self, x, target):
+        """x: fields [B,V,Hg,Wg] fp32 (or block input [B,N,D] for block-only configs); target [B,L,D]."""
+        y = self.forward(x)
+        ob.orbit_mse_loss_grad(self.cfg.resid_dtype, y, target, self.dy, self.loss)
+        self.backward(self.dy)
+        return self.loss

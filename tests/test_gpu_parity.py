@@ -1,0 +1,219 @@
+"""GPU parity: the CUDA path (through the C-ABI via paper_2404_14712_b200.binding) against the fp64 oracle,
+element by element on the same seeded inputs.  Tolerances (north_star): relative Frobenius error <= 1e-2 for
+bf16 paths, <= 1e-4 for fp32 and for the fp32 shard-recombination check.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import orbit_oracle as orc
+from paper_2404_14712_b200 import inputs as syn
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": 1e-4, "bf16": 1e-2}
+
+
+@pytest.fixture(scope="module")
+def ob():
+    from paper_2404_14712_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def rn():
+    from paper_2404_14712_b200 import runner
+    return runner
+
+
+def check(name, got, ref, tol):
+    got = got.detach().to(torch.float32).cpu().numpy() if isinstance(got, torch.Tensor) else got
+    err = orc.rel_fro(got.reshape(ref.shape), ref)
+    assert np.isfinite(got).all(), f"{name}: non-finite values"
+    assert err <= tol, f"{name}: rel Frobenius error {err:.3e} > {tol:.1e}"
+    return err
+
+
+def make_block_case(seed, B, N, D, heads, F, T, dtype, resid_dtype):
+    P = syn.block_params(seed, D, F, dtype)
+    shards = syn.shard_block_params(P, heads, T)
+    x = syn.normal(seed, "blk.x", (B, N, D), dtype=resid_dtype)
+    dy = syn.normal(seed, "blk.dy", (B, N, D), dtype=resid_dtype)
+    return P, shards, x, dy
+
+
+def run_block(rn, B, N, D, heads, F, T, dtype, resid_dtype, P, shards, x, dy):
+    br = rn.BlockRunner(B, N, D, heads, F, T, dtype, resid_dtype, P, shards)
+    xd, dyd = rn.to_dev(x, resid_dtype), rn.to_dev(dy, resid_dtype)
+    y = br.fwd(xd)
+    dx = br.bwd(dyd)
+    torch.cuda.synchronize()
+    return br, y, dx
+
+
+def compare_block(br, y, dx, P, x, dy, heads, T, tol, eps=1e-5):
+    yo, cache = orc.block_fwd(x, P, heads, eps)
+    dxo, G = orc.block_bwd(dy, P, cache)
+    errs = {"y": check("y", y, yo, tol), "dx": check("dx", dx, dxo, tol)}
+    for k in br.COMMON:
+        errs[k] = check("d" + k, br.gcommon[k], G[k], tol)
+    gs = [{k: v.detach().to(torch.float32).cpu().numpy() for k, v in S.items()} for S in br.gshards]
+    Gu = syn.unshard_block_grads(gs, T)
+    for k in Gu:
+        errs[k] = check("d" + k, Gu[k], G[k], tol)
+    return errs
+
+
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("T", [1, 2, 4])
+def test_block_fp32_shard_recombination(rn, T):
+    """fp32 shard-recombination check (north_star; R15): sharded CUDA block (fp32 storage, true fp32
+    FMA, fp32 partials) vs the UNSHARDED fp64 oracle, <= 1e-4."""
+    B, N, D, heads, F = 2, 256, 256, 8, 1024
+    P, shards, x, dy = make_block_case(11, B, N, D, heads, F, T, "f32", "f32")
+    br, y, dx = run_block(rn, B, N, D, heads, F, T, "f32", "f32", P, shards, x, dy)
+    compare_block(br, y, dx, P, x, dy, heads, T, 1e-4)
+
+
+def test_block_fp32_c1_shape_ragged_tokens(rn):
+    """C1's block shape with a ragged token count (N = 100 is not a multiple of any tile)."""
+    B, N, D, heads, F = 2, 100, 128, 4, 512
+    P, shards, x, dy = make_block_case(12, B, N, D, heads, F, 1, "f32", "f32")
+    br, y, dx = run_block(rn, B, N, D, heads, F, 1, "f32", "f32", P, shards, x, dy)
+    compare_block(br, y, dx, P, x, dy, heads, 1, 1e-4)
+
+
+def test_block_softmax_stress_logits_x30(rn):
+    """Logits scaled x30 exercise the max-subtraction path."""
+    B, N, D, heads, F = 1, 96, 64, 2, 128
+    P, shards, x, dy = make_block_case(13, B, N, D, heads, F, 1, "f32", "f32")
+    P["Wqkv"] = (P["Wqkv"] * np.float32(math.sqrt(30.0) * 3)).astype(np.float32)
+    shards = syn.shard_block_params(P, heads, 1)
+    br, y, dx = run_block(rn, B, N, D, heads, F, 1, "f32", "f32", P, shards, x, dy)
+    compare_block(br, y, dx, P, x, dy, heads, 1, 2e-4)
+
+
+@pytest.mark.parametrize("shape", [
+    (2, 384, 512, 8, 2048, 1, "bf16"),      # several 128x256 tiles, d_h = 64
+    (1, 200, 256, 2, 1024, 1, "f32"),       # d_h = 128, ragged N, fp32 residual stream
+    (2, 256, 512, 4, 1536, 2, "bf16"),      # Hybrid-STOP T = 2, d_h = 128
+    (1, 520, 1024, 8, 4096, 4, "f32"),      # T = 4, ragged N spanning tile tails
+])
+def test_block_bf16_vs_oracle(rn, shape):
+    B, N, D, heads, F, T, rdt = shape
+    P, shards, x, dy = make_block_case(21, B, N, D, heads, F, T, "bf16", rdt)
+    br, y, dx = run_block(rn, B, N, D, heads, F, T, "bf16", rdt, P, shards, x, dy)
+    errs = compare_block(br, y, dx, P, x, dy, heads, T, 1e-2)
+    print("bf16 block errs", {k: f"{v:.2e}" for k, v in errs.items()})
+
+
+def test_chain_eq2_eq3(ob, rn):
+    """Bare Eq. (2)/(3) chain on the GPU in fp32: sum_k (x A_k) B_k vs x A B in fp64."""
+    m, d, n, e, T = 300, 256, 512, 192, 4
+    x = syn.normal(31, "ch.x", (m, d))
+    A = syn.xavier_uniform(31, "ch.A", (d, n), d, n)
+    Bm = syn.xavier_uniform(31, "ch.B", (n, e), n, e)
+    dy = syn.normal(31, "ch.dy", (m, e))
+    Ac = [np.ascontiguousarray(A[:, k * n // T:(k + 1) * n // T]) for k in range(T)]
+    Br = [np.ascontiguousarray(Bm[k * n // T:(k + 1) * n // T]) for k in range(T)]
+    Ad = [rn.to_dev(a, "f32") for a in Ac]
+    Bd = [rn.to_dev(b, "f32") for b in Br]
+    ws = torch.empty(ob.orbit_chain_workspace_bytes(m, d, n, e, T, "f32"), dtype=torch.uint8, device="cuda")
+    y = torch.empty(m, e, device="cuda")
+    dx = torch.empty(m, d, device="cuda")
+    ob.orbit_chain_fwd(m, d, n, e, T, "f32", rn.to_dev(x, "f32"), Ad, Bd, y, ws)
+    ob.orbit_chain_bwd(m, d, n, e, T, "f32", rn.to_dev(dy, "f32"), Ad, Bd, dx, ws)
+    torch.cuda.synchronize()
+    x64, A64, B64, dy64 = (np.asarray(t, dtype=np.float64) for t in (x, A, Bm, dy))
+    check("chain y", y, x64 @ A64 @ B64, 1e-4)
+    check("chain dx", dx, dy64 @ B64.T @ A64.T, 1e-4)
+    check("chain y vs sharded oracle", y, orc.chain_sharded(x, Ac, Br), 1e-4)
+
+
+# ---------------------------------------------------------------------------------------------------------
+def make_step_case(cfg, seed, depth=None):
+    depth = cfg.depth if depth is None else depth
+    emb = syn.embed_params(seed, cfg.V, cfg.p, cfg.D, cfg.dtype)
+    agg = syn.agg_params(seed, cfg.D, cfg.dtype)
+    blocks = [syn.block_params(seed, cfg.D, cfg.F, cfg.dtype, tag=f"blk{i}") for i in range(depth)]
+    x = syn.fields(seed, cfg.B, cfg.V, cfg.Hg, cfg.Wg, per_variable_scale=cfg.name != "C1")
+    tgt = syn.normal(seed, "target", (cfg.B, cfg.L, cfg.D), dtype=cfg.resid_dtype)
+    pos = syn.normal(seed, "pos", (cfg.L, cfg.D), 0.02, dtype=cfg.resid_dtype)
+    return emb, agg, blocks, x, tgt, pos
+
+
+def run_and_compare_step(rn, cfg, seed, tol, with_pos=True):
+    emb, agg, blocks, x, tgt, pos = make_step_case(cfg, seed)
+    if not with_pos:
+        pos = None
+    sr = rn.StepRunner(cfg, emb, agg, [(P, syn.shard_block_params(P, cfg.heads, 1)) for P in blocks], pos)
+    loss = sr.step(rn.to_dev(x, "f32"), rn.to_dev(tgt, cfg.resid_dtype))
+    torch.cuda.synchronize()
+    out = orc.step(x, emb, agg, blocks, tgt, cfg.p, cfg.heads, cfg.ln_eps, pos)
+    errs = {}
+    errs["tok"] = check("tok", sr.front.tok, out["tok"], tol)
+    errs["agg"] = check("agg", sr.front.out, out["agg"], tol)
+    errs["y"] = check("y", sr.blocks[-1].y, out["y"], tol)
+    assert abs(float(loss.item()) - out["loss"]) <= 5 * tol * abs(out["loss"])
+    for i, br in enumerate(sr.blocks):
+        G = out["block_grads"][i]
+        for k in br.COMMON:
+            errs[f"b{i}.{k}"] = check(f"b{i}.d{k}", br.gcommon[k], G[k], tol)
+        for k in br.SHARD:
+            errs[f"b{i}.{k}"] = check(f"b{i}.d{k}", br.gshards[0][k], G[k], tol)
+    errs["dagg"] = check("dagg", sr.blocks[0].dx, out["dagg"], tol)
+    errs["dtok"] = check("dtok", sr.front.dtok, out["dtok"], tol)
+    for k, g in out["agg_grads"].items():
+        if k == "bk":   # analytically zero: compare absolutely against the scale of its siblings
+            got = rn.to_np(sr.front.gagg[k])
+            assert np.abs(got).max() <= 1e-6 * max(1.0, np.abs(out["agg_grads"]["bv"]).max())
+        else:
+            errs["agg." + k] = check("agg.d" + k, sr.front.gagg[k], g, tol)
+    if pos is not None:
+        errs["dpos"] = check("dpos", sr.front.dpos, out["dpos"], tol)
+    errs["dWp"] = check("dWp", sr.front.dWp, out["dWp"], tol)
+    errs["dbp"] = check("dbp", sr.front.dbp, out["dbp"], tol)
+    return errs
+
+
+def test_c1_full_step_fp32(rn):
+    """BASELINE.json config 1 (tiny ORBIT step, fp32): tokenise + aggregate + block fwd+bwd + MSE, <= 1e-4."""
+    errs = run_and_compare_step(rn, syn.CONFIGS["C1"], syn.seed_of("C1"), 1e-4)
+    print("C1 max err", max(errs.values()))
+
+
+def test_small_bf16_full_step(rn):
+    """A shrunken C2 (bf16 storage, fp32 residual stream, V = 7 variables, patch 2, depth 2), <= 1e-2."""
+    cfg = syn.Config("S2", B=2, V=7, Hg=16, Wg=32, p=2, D=256, heads=4, F=1024, depth=2, dtype="bf16",
+                     resid_dtype="f32")
+    errs = run_and_compare_step(rn, cfg, 42, 1e-2)
+    print("S2 errs", {k: f"{v:.2e}" for k, v in errs.items()})
+
+
+def test_front_end_v91_ragged(rn):
+    """Front end with V = 91 (odd, > 64), patch 4, no positional embedding, bf16 stream."""
+    cfg = syn.Config("S3", B=1, V=91, Hg=16, Wg=24, p=4, D=128, heads=16, F=256, depth=1, dtype="bf16",
+                     resid_dtype="bf16")
+    run_and_compare_step(rn, cfg, 43, 1e-2, with_pos=False)
+
+
+# ---------------------------------------------------------------------------------------------------------
+def test_error_codes(ob, rn):
+    P = syn.block_params(1, 64, 128, "bf16")
+    with pytest.raises(ob.OrbitError) as e:          # D % heads != 0
+        br = rn.BlockRunner(1, 16, 64, 3, 128, 1, "bf16", "bf16", P, syn.shard_block_params(P, 1, 1))
+        br.fwd(torch.zeros(1, 16, 64, device="cuda", dtype=torch.bfloat16))
+    assert e.value.status == 2                      # ORBIT_ERR_SHAPE
+    P = syn.block_params(1, 64, 128, "bf16")
+    br = rn.BlockRunner(1, 16, 64, 2, 128, 1, "bf16", "bf16", P, syn.shard_block_params(P, 2, 1))
+    br.desc.flags = 1                               # reserved QK-norm flag
+    with pytest.raises(ob.OrbitError) as e:
+        br.fwd(torch.zeros(1, 16, 64, device="cuda", dtype=torch.bfloat16))
+    assert e.value.status == 6                      # ORBIT_ERR_UNSUPPORTED
+    br.desc.flags = 0
+    br.ws_f = torch.empty(16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(ob.OrbitError) as e:
+        br.fwd(torch.zeros(1, 16, 64, device="cuda", dtype=torch.bfloat16))
+    assert e.value.status == 5                      # ORBIT_ERR_WORKSPACE

@@ -141,6 +141,11 @@ void orbit_reset_launch_count(void);
 /* 0 = automatic (tcgen05 tensor-core kernels for bf16 where shapes allow), 1 = force the SIMT fp32-FMA
  * kernels everywhere (debug cross-check only; never used by bench.py). */
 void orbit_set_debug_force_simt(int on);
+/* Kernel-level diagnostic: C[M,N] (fp32, row-major) = A B through the library's GEMM dispatcher.
+ * A(m,k) = A[m*a_rs + k*a_cs], B(k,n) = B[k*b_rs + n*b_cs] (element strides); dtype of A and B = `dtype`.
+ * Exercises every operand-major combination the block uses (K-major / MN-major A and B). */
+int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,
+                     const void* B, long long b_rs, long long b_cs, float* C, void* stream);
 
 #ifdef __cplusplus
 }

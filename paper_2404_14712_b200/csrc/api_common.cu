@@ -97,6 +97,18 @@ int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dt
   return ORBIT_OK;
 }
 
+int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,
+                     const void* B, long long b_rs, long long b_cs, float* C, void* stream) {
+  if (!A || !B || !C) { set_error("debug_gemm: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!valid_dtype(dtype)) { set_error("debug_gemm: bad dtype"); return ORBIT_ERR_DTYPE; }
+  if (M <= 0 || N <= 0 || K <= 0) { set_error("debug_gemm: bad shape"); return ORBIT_ERR_SHAPE; }
+  ORBIT_TRY(check_device());
+  GemmArgs g;
+  g.A = A; g.a_rs = a_rs; g.a_cs = a_cs; g.B = B; g.b_rs = b_rs; g.b_cs = b_cs; g.C = C; g.ldc = N;
+  g.M = M; g.N = N; g.K = K; g.in_dtype = dtype; g.out_dtype = ORBIT_F32;
+  return gemm(g, (cudaStream_t)stream);
+}
+
 int orbit_mse_loss_grad(orbit_dtype dtype, size_t n, const void* y, const void* t, void* dy, float* loss, void* stream) {
   if (!y || !t || !dy || !loss) { set_error("mse: NULL pointer"); return ORBIT_ERR_NULL; }
   if (!valid_dtype(dtype)) { set_error("mse: bad dtype"); return ORBIT_ERR_DTYPE; }

@@ -1,0 +1,64 @@
+"""Kernel-level parity of the GEMM dispatcher (tcgen05 path for bf16, fp32-FMA path otherwise) against the
+definition C = A B evaluated in float64 (numpy matmul), for every operand-major combination the block uses
+(forward x A, backward dy B^T, weight gradient x^T dy) and for ragged sizes that leave partial
+tiles in M, N and K."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2404_14712_b200 import inputs as syn
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ob():
+    from paper_2404_14712_b200 import binding
+    return binding
+
+
+def run_gemm(ob, M, N, K, a_major, b_major, dtype, simt=False):
+    A = syn.normal(5, f"A{M}{K}", (M, K), dtype=dtype)
+    B = syn.normal(5, f"B{K}{N}", (K, N), dtype=dtype)
+    td = ob.TORCH_DTYPES[dtype]
+    At, Bt = torch.from_numpy(A).cuda().to(td), torch.from_numpy(B).cuda().to(td)
+    if a_major == "K":
+        Ad, a_rs, a_cs = At.contiguous(), K, 1
+    else:
+        Ad, a_rs, a_cs = At.t().contiguous(), 1, M
+    if b_major == "N":
+        Bd, b_rs, b_cs = Bt.contiguous(), N, 1
+    else:
+        Bd, b_rs, b_cs = Bt.t().contiguous(), 1, K
+    C = torch.full((M, N), float("nan"), device="cuda", dtype=torch.float32)
+    ob.orbit_set_debug_force_simt(simt)
+    try:
+        ob.orbit_debug_gemm(M, N, K, dtype, Ad, a_rs, a_cs, Bd, b_rs, b_cs, C)
+        torch.cuda.synchronize()
+    finally:
+        ob.orbit_set_debug_force_simt(False)
+    ref = A.astype(np.float64) @ B.astype(np.float64)
+    got = C.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    return np.linalg.norm(got - ref) / np.linalg.norm(ref)
+
+
+SHAPES = [(128, 256, 64), (256, 512, 256), (200, 264, 136), (1024, 768, 520), (2048, 1024, 2048), (64, 64, 32)]
+
+
+@pytest.mark.parametrize("a_major", ["K", "M"])
+@pytest.mark.parametrize("b_major", ["N", "K"])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_gemm_bf16_tensor_core(ob, shape, a_major, b_major):
+    M, N, K = shape
+    err = run_gemm(ob, M, N, K, a_major, b_major, "bf16")
+    assert err < 1e-4, f"{shape} A:{a_major}-major B:{b_major}-major rel err {err:.3e}"
+
+
+@pytest.mark.parametrize("a_major", ["K", "M"])
+@pytest.mark.parametrize("b_major", ["N", "K"])
+def test_gemm_fp32_fma(ob, a_major, b_major):
+    err = run_gemm(ob, 200, 264, 136, a_major, b_major, "f32")
+    assert err < 1e-5
+    err = run_gemm(ob, 200, 264, 136, a_major, b_major, "bf16", simt=True)
+    assert err < 1e-5

@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- ORBIT hot path on B200: ViT block fwd+bwd bf16 TFLOP/s (BASELINE.json metric) on the 113B-class
+block C5 (default), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C5|C4|C3|C2]
+
+N > 1 (torchrun): replicas only -- the path does not shard across GPUs (north_star: no collectives); every rank
+runs the same workload, timing is the max over ranks, value is the sum ("weak").
+--impl reference: the fp64 CPU oracle, as it stands, on a bounded sample of the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2404_14712_b200 import inputs as syn  # noqa: E402
+
+METRIC = "vit_block_fwd_bwd_bf16_tflops"
+UNIT = "TFLOP/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return dict(bf16=float(d["bf16_tflops"]), bf16_sustained=float(d.get("bf16_tflops_sustained", 0) or 0),
+                        hbm=float(d["hbm_gbs"]), src="measured")
+        except Exception:
+            pass
+    return dict(bf16=1590.0, bf16_sustained=1400.0, hbm=6650.0, src="fallback")
+
+
+def workload_string(cfg):
+    if cfg.V is None:
+        return (f"{cfg.name}: one ViT block fwd+bwd, B={cfg.B} N={cfg.L} D={cfg.D} heads={cfg.heads} F={cfg.F} T={cfg.T} "
+                f"{cfg.dtype}")
+    return (f"{cfg.name}: tokenise+aggregate+{cfg.depth} blocks fwd+bwd, B={cfg.B} V={cfg.V} grid={cfg.Hg}x{cfg.Wg} p={cfg.p} "
+            f"L={cfg.L} D={cfg.D} heads={cfg.heads} F={cfg.F} {cfg.dtype}")
+
+
+def step_flops(cfg):
+    """Model FLOPs of one step's blocks (2 per MAC; backward = 2x forward; no recompute) -- SURVEY.md §8(d)."""
+    return 3.0 * cfg.block_flops_fwd() * cfg.depth
+
+
+# ------------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle on a bounded sample
+# ------------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, n_tokens):
+    """Block fwd+bwd of the oracle at cfg's widths on n_tokens tokens (B=1).  Returns a closure running one
+    sample step and the sample's model FLOPs.  Weights are widened to float64 outside the timed call (input
+    preparation, not arithmetic of the method)."""
+    from oracle import orbit_oracle as orc
+    seed = syn.seed_of(cfg.name)
+    P = syn.block_params(seed, cfg.D, cfg.F, cfg.dtype)
+    P = {k: np.asarray(v, dtype=np.float64) for k, v in P.items()}
+    x = np.asarray(syn.normal(seed, "blk.x", (1, n_tokens, cfg.D), dtype=cfg.resid_dtype), dtype=np.float64)
+    dy = np.asarray(syn.normal(seed, "blk.dy", (1, n_tokens, cfg.D), dtype=cfg.resid_dtype), dtype=np.float64)
+    flops = 3.0 * (2.0 * n_tokens * cfg.D * (4 * cfg.D + 2 * cfg.F) + 4.0 * n_tokens * n_tokens * cfg.D)
+
+    def run():
+        y, cache = orc.block_fwd(x, P, cfg.heads, cfg.ln_eps)
+        dx, G = orc.block_bwd(dy, P, cache)
+        return float(y[0, 0, 0]) + float(dx[0, 0, 0])
+
+    return run, flops
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i.get("num_threads") for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return int(max(n))
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_tok = 16
+    run, flops = oracle_sample(cfg, n_tok)
+    for _ in range(args.warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    dt = (time.perf_counter() - t0) / args.steps
+    val = flops / dt / 1e12
+    sample = f"oracle block fwd+bwd at {cfg.name} widths on {n_tok} of {cfg.L} tokens (B=1), fp64 numpy/OpenBLAS"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_string(cfg), "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-i", str(gpu_index), "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons, pw = [], [], set(), []
+        for ln in self.f.read().splitlines():
+            c = [t.strip() for t in ln.split(",")]
+            if len(c) < 8:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            hi = sorted(sm)[len(sm) // 2:]          # upper half = samples under load
+            out = {"sm_mhz": float(np.median(hi)), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                   "power_w_max": max(pw), "samples": len(sm)}
+        return out
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2404_14712_b200 import binding as ob, runner as rn
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    seed = syn.seed_of(cfg.name)
+
+    # ---- build the workload (inputs resident in HBM) ----
+    if cfg.V is None:
+        P = syn.block_params(seed, cfg.D, cfg.F, cfg.dtype)
+        sr = rn.StepRunner(cfg, blocks=[(P, syn.shard_block_params(P, cfg.heads, cfg.T))])
+        del P
+        x_h = syn.normal(seed, "blk.x", (cfg.B, cfg.L, cfg.D), dtype=cfg.resid_dtype)
+        dy_h = syn.normal(seed, "blk.dy", (cfg.B, cfg.L, cfg.D), dtype=cfg.resid_dtype)
+        x_d, dy_d = rn.to_dev(x_h, cfg.resid_dtype), rn.to_dev(dy_h, cfg.resid_dtype)
+
+        def step():
+            sr.forward(x_d)
+            sr.backward(dy_d)
+        tdt = ob.TORCH_DTYPES[cfg.resid_dtype]
+        hx = torch.from_numpy(x_h).to(tdt).pin_memory()
+        hdy = torch.from_numpy(dy_h).to(tdt).pin_memory()
+        hy, hdx = torch.empty_like(hx).pin_memory(), torch.empty_like(hx).pin_memory()
+        h2d = hx.numel() * hx.element_size() * 2
+        d2h = h2d
+
+        def step_e2e():
+            x_d.copy_(hx, non_blocking=True)
+            dy_d.copy_(hdy, non_blocking=True)
+            sr.forward(x_d)
+            sr.backward(dy_d)
+            hy.copy_(sr.blocks[-1].y, non_blocking=True)
+            hdx.copy_(sr.blocks[0].dx, non_blocking=True)
+    else:
+        emb = syn.embed_params(seed, cfg.V, cfg.p, cfg.D, cfg.dtype)
+        agg = syn.agg_params(seed, cfg.D, cfg.dtype)
+        blocks = []
+        for i in range(cfg.depth):
+            P = syn.block_params(seed, cfg.D, cfg.F, cfg.dtype, tag=f"blk{i}")
+            blocks.append((P, syn.shard_block_params(P, cfg.heads, 1)))
+        sr = rn.StepRunner(cfg, emb, agg, blocks)
+        del blocks
+        x_h = syn.fields(seed, cfg.B, cfg.V, cfg.Hg, cfg.Wg, per_variable_scale=True)
+        t_h = syn.normal(seed, "target", (cfg.B, cfg.L, cfg.D), dtype=cfg.resid_dtype)
+        x_d, t_d = rn.to_dev(x_h, "f32"), rn.to_dev(t_h, cfg.resid_dtype)
+
+        def step():
+            sr.step(x_d, t_d)
+        hx = torch.from_numpy(x_h).pin_memory()
+        ht = torch.from_numpy(t_h).to(ob.TORCH_DTYPES[cfg.resid_dtype]).pin_memory()
+        hloss = torch.zeros(1).pin_memory()
+        h2d = hx.numel() * 4 + ht.numel() * ht.element_size()
+        d2h = 4
+
+        def step_e2e():
+            x_d.copy_(hx, non_blocking=True)
+            t_d.copy_(ht, non_blocking=True)
+            sr.step(x_d, t_d)
+            hloss.copy_(sr.loss, non_blocking=True)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    # ---- timed region: device-resident inputs ----
+    sampler = ClockSampler(local) if rank == 0 else None
+    ob.orbit_profile_gemm(True)
+    ob.orbit_reset_launch_count()
+    ms = timed(step, args.steps)
+    launches = ob.orbit_launch_count()
+    gemm_ms, gemm_flops, gemm_n = ob.orbit_profile_gemm_collect()
+    ob.orbit_profile_gemm(False)
+    clocks = sampler.stop() if sampler else None
+    # ---- end to end through the public API with host buffers ----
+    for _ in range(2):
+        step_e2e()
+    ms_e2e = timed(step_e2e, args.steps)
+
+    flops = step_flops(cfg)
+    ms_step = ms / args.steps
+    tflops = flops / (ms_step * 1e-3) / 1e12 * world
+    tflops_e2e = flops / (ms_e2e / args.steps * 1e-3) / 1e12 * world
+    tokens_s = cfg.B * cfg.L / (ms_step * 1e-3) * world
+    peaks = measured_peaks()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    achieved = gemm_flops / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(cfg.name)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (tcgen05 bf16 GEMM, all 12 GEMMs of the block)",
+                "achieved": achieved, "peak": peaks["bf16"], "unit": "TFLOP/s", "frac": achieved / peaks["bf16"],
+                "peak_source": f"{peaks['src']} burst bf16 (MEASURED_PEAKS.json bf16_tflops)",
+                "frac_of_sustained": (achieved / peaks["bf16_sustained"]) if peaks["bf16_sustained"] else None,
+                "launches": gemm_n, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
+                "share_of_step": gemm_ms / ms if ms > 0 else None, "traffic": traffic}
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only) ----
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_tok = 64 if cfg.D >= 8192 else 256
+        run, sflops = oracle_sample(cfg, n_tok)
+        t0 = time.perf_counter()
+        run()
+        dt = time.perf_counter() - t0
+        cpu = {"value": sflops / dt / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+               "sample": f"oracle block fwd+bwd at {cfg.name} widths on {n_tok} of {cfg.L} tokens (B=1), fp64 "
+                         f"numpy/OpenBLAS, {dt:.1f} s"}
+    line = {
+        "metric": METRIC, "value": tflops, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": workload_string(cfg), "l2": "inputs larger than L2 (weights + saved activations "
+                   "streamed every step; no flush needed)", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "model_flops_per_step": flops},
+        "tokens_per_s": tokens_s,
+        "frac_of_peak_measured_burst": tflops / world / peaks["bf16"],
+        "frac_of_peak_measured_sustained": (tflops / world / peaks["bf16_sustained"]) if peaks["bf16_sustained"] else None,
+        "frac_of_peak_nominal_2250": tflops / world / 2250.0,
+        "clocks": clocks,
+        "e2e": {"value": tflops_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C5", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = syn.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

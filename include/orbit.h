@@ -141,6 +141,12 @@ void orbit_reset_launch_count(void);
 /* 0 = automatic (tcgen05 tensor-core kernels for bf16 where shapes allow), 1 = force the SIMT fp32-FMA
  * kernels everywhere (debug cross-check only; never used by bench.py). */
 void orbit_set_debug_force_simt(int on);
+/* Per-launch CUDA-event timing of the tensor-core GEMM kernel (the dominant kernel; bench.py's roofline leg).
+ * orbit_profile_gemm(1) starts recording an event pair around every tcgen05 GEMM launch on its stream;
+ * orbit_profile_gemm_collect() waits for them, returns the summed kernel milliseconds, the summed algorithmic
+ * FLOPs (2 M N K per launch) and the number of launches recorded, and clears the record. */
+int orbit_profile_gemm(int on);
+int orbit_profile_gemm_collect(double* ms, double* flops, long long* launches);
 /* Kernel-level diagnostic: C[M,N] (fp32, row-major) = A B through the library's GEMM dispatcher.
  * A(m,k) = A[m*a_rs + k*a_cs], B(k,n) = B[k*b_rs + n*b_cs] (element strides); dtype of A and B = `dtype`.
  * Exercises every operand-major combination the block uses (K-major / MN-major A and B). */

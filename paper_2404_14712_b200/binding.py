@@ -113,6 +113,8 @@ _proto("orbit_chain_fwd", C.c_int, [C.c_int] * 5 + [C.c_int, _vp, C.POINTER(_vp)
 _proto("orbit_chain_bwd", C.c_int, [C.c_int] * 5 + [C.c_int, _vp, C.POINTER(_vp), C.POINTER(_vp), _vp, _vp, _sz, _vp])
 _proto("orbit_chain_workspace_bytes", _sz, [C.c_int] * 5 + [C.c_int])
 _proto("orbit_mse_loss_grad", C.c_int, [C.c_int, _sz, _vp, _vp, _vp, _vp, _vp])
+_proto("orbit_profile_gemm", C.c_int, [C.c_int])
+_proto("orbit_profile_gemm_collect", C.c_int, [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)])
 _proto("orbit_debug_gemm", C.c_int, [C.c_int] * 4 + [_vp, C.c_longlong, C.c_longlong, _vp, C.c_longlong, C.c_longlong, _vp, _vp])
 
 EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace_bytes", "orbit_var_aggregate",
@@ -121,7 +123,8 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_block_bwd", "orbit_block_fwd_workspace_bytes", "orbit_block_bwd_workspace_bytes",
            "orbit_block_saved_bytes", "orbit_mse_loss_grad", "orbit_chain_fwd", "orbit_chain_bwd", "orbit_chain_workspace_bytes",
            "orbit_last_error", "orbit_version", "orbit_launch_count", "orbit_reset_launch_count",
-           "orbit_set_debug_force_simt", "orbit_debug_gemm"]
+           "orbit_set_debug_force_simt", "orbit_debug_gemm", "orbit_profile_gemm",
+           "orbit_profile_gemm_collect"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -259,6 +262,16 @@ def orbit_mse_loss_grad(dtype, y, t, dy, loss, stream=None):
 def orbit_debug_gemm(M, N, K, dtype, A, a_rs, a_cs, B, b_rs, b_cs, Cout, stream=None):
     _check(lib.orbit_debug_gemm(M, N, K, DTYPES[dtype], _ptr(A), a_rs, a_cs, _ptr(B), b_rs, b_cs, _ptr(Cout),
                                 _stream(stream)), "orbit_debug_gemm")
+
+
+def orbit_profile_gemm(on: bool):
+    _check(lib.orbit_profile_gemm(1 if on else 0), "orbit_profile_gemm")
+
+
+def orbit_profile_gemm_collect():
+    ms, fl, n = C.c_double(0), C.c_double(0), C.c_longlong(0)
+    _check(lib.orbit_profile_gemm_collect(C.byref(ms), C.byref(fl), C.byref(n)), "orbit_profile_gemm_collect")
+    return ms.value, fl.value, n.value
 
 
 def orbit_version():

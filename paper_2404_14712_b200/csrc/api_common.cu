@@ -97,6 +97,11 @@ int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dt
   return ORBIT_OK;
 }
 
+int orbit_profile_gemm(int on) { return gemm_profile_enable(on); }
+int orbit_profile_gemm_collect(double* ms, double* flops, long long* launches) {
+  return gemm_profile_collect(ms, flops, launches);
+}
+
 int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,
                      const void* B, long long b_rs, long long b_cs, float* C, void* stream) {
   if (!A || !B || !C) { set_error("debug_gemm: NULL pointer"); return ORBIT_ERR_NULL; }

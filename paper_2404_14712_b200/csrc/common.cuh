@@ -112,6 +112,8 @@ int gemm(const GemmArgs& g, cudaStream_t s);           // dispatcher (tensor-cor
 int gemm_simt(const GemmArgs& g, cudaStream_t s);      // fp32-FMA kernels, any dtype/stride
 int gemm_tc(const GemmArgs& g, cudaStream_t s);        // tcgen05 + TMA, bf16 in / fp32 accumulate
 bool gemm_tc_supported(const GemmArgs& g);
+int gemm_profile_enable(int on);
+int gemm_profile_collect(double* ms, double* flops, long long* launches);
 
 // ---- row-wise / reduction kernels (rowops.cu) -----------------------------------------------------
 int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,

@@ -289,6 +289,16 @@ int num_sms() {
   return n;
 }
 
+// ---- optional per-launch CUDA-event timing of the tensor-core GEMM (bench.py's roofline leg) ----------------
+struct Prof {
+  bool on = false;
+  static constexpr int MAXP = 16384;
+  cudaEvent_t* ev = nullptr;     // 2 * MAXP events, created lazily
+  double* flops = nullptr;
+  int n = 0;
+};
+Prof g_prof;
+
 template <int A_MN, int B_MN>
 int launch(const CUtensorMap& ma, const CUtensorMap& mb, const Epi& e, int M, int N, int K, cudaStream_t s) {
   static bool attr_set = false;
@@ -299,11 +309,42 @@ int launch(const CUtensorMap& ma, const CUtensorMap& mb, const Epi& e, int M, in
   }
   const int tiles = cdiv(M, BM) * cdiv(N, BN);
   const int grid = tiles < num_sms() ? tiles : num_sms();
+  const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
+  if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
   gemm_tc_kernel<A_MN, B_MN><<<grid, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K);
+  if (rec) {
+    ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n + 1], s));
+    g_prof.flops[g_prof.n++] = 2.0 * M * N * K;
+  }
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
 }  // namespace
+
+int gemm_profile_enable(int on) {
+  if (on && !g_prof.ev) {
+    g_prof.ev = new cudaEvent_t[2 * Prof::MAXP];
+    g_prof.flops = new double[Prof::MAXP];
+    for (int i = 0; i < 2 * Prof::MAXP; i++) ORBIT_CUDA_CHECK(cudaEventCreate(&g_prof.ev[i]));
+  }
+  g_prof.on = on != 0;
+  g_prof.n = 0;
+  return ORBIT_OK;
+}
+int gemm_profile_collect(double* ms, double* flops, long long* launches) {
+  double t = 0, f = 0;
+  for (int i = 0; i < g_prof.n; i++) {
+    float e = 0.f;
+    ORBIT_CUDA_CHECK(cudaEventSynchronize(g_prof.ev[2 * i + 1]));
+    ORBIT_CUDA_CHECK(cudaEventElapsedTime(&e, g_prof.ev[2 * i], g_prof.ev[2 * i + 1]));
+    t += e; f += g_prof.flops[i];
+  }
+  if (ms) *ms = t;
+  if (flops) *flops = f;
+  if (launches) *launches = g_prof.n;
+  g_prof.n = 0;
+  return ORBIT_OK;
+}
 
 bool gemm_tc_supported(const GemmArgs& g) {
   if (g.in_dtype != ORBIT_BF16 || g.alpha != 1.f) return false;

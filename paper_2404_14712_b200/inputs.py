@@ -73,9 +73,12 @@ def round_bf16(a: np.ndarray) -> np.ndarray:
     """Round float64/float32 values to the nearest bfloat16 (ties to even); returns float32 holding
     bf16-exact values."""
     f = np.ascontiguousarray(a, dtype=np.float32)
-    u = f.view(np.uint32).astype(np.uint64)
-    rounded = ((u + 0x7FFF + ((u >> 16) & 1)) >> 16) << 16
-    return rounded.astype(np.uint32).view(np.float32).reshape(f.shape)
+    u = f.view(np.uint32)
+    r = (u >> np.uint32(16)) & np.uint32(1)      # uint32 arithmetic: finite inputs cannot wrap
+    r += np.uint32(0x7FFF)
+    r += u
+    r &= np.uint32(0xFFFF0000)
+    return r.view(np.float32).reshape(f.shape)
 
 
 def round_storage(a: np.ndarray, dtype: str) -> np.ndarray:
@@ -96,23 +99,49 @@ def _rng(seed: int, name: str) -> np.random.Generator:
     return np.random.Generator(np.random.Philox(key=[seed & (2**64 - 1), tag & (2**64 - 1)]))
 
 
+_CHUNK = 1 << 22   # elements per independently seeded chunk (result does not depend on the thread count)
+
+
+def _draw(seed, name, shape, kind, a, b, dtype):
+    """Fill an array of `shape` chunk by chunk (chunk c draws from sub-stream (seed, name, c)); chunks are
+    generated on a thread pool.  kind "normal": a*N(0,1)+b ; kind "uniform": U(a, b)."""
+    n = int(np.prod(shape))
+    out = np.empty(n, dtype=np.float32)
+
+    def fill(c):
+        lo, hi = c * _CHUNK, min(n, (c + 1) * _CHUNK)
+        g = _rng(seed, f"{name}#{c}" if c else name)
+        if kind == "normal":
+            v = g.standard_normal(size=hi - lo, dtype=np.float32)
+            if a != 1.0:
+                v *= np.float32(a)
+            if b != 0.0:
+                v += np.float32(b)
+        else:
+            v = g.random(size=hi - lo, dtype=np.float32)
+            v *= np.float32(b - a)
+            v += np.float32(a)
+        out[lo:hi] = round_storage(v, dtype)
+
+    nchunks = (n + _CHUNK - 1) // _CHUNK
+    if nchunks <= 1:
+        fill(0)
+    else:
+        from concurrent.futures import ThreadPoolExecutor
+        import os
+        with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+            list(ex.map(fill, range(nchunks)))
+    return out.reshape(shape)
+
+
 def normal(seed, name, shape, scale=1.0, loc=0.0, dtype="f32"):
-    g = _rng(seed, name)
-    a = g.standard_normal(size=shape, dtype=np.float32)
-    if scale != 1.0:
-        a *= np.float32(scale)
-    if loc != 0.0:
-        a += np.float32(loc)
-    return round_storage(a, dtype)
+    return _draw(seed, name, shape, "normal", float(scale), float(loc), dtype)
 
 
 def xavier_uniform(seed, name, shape, fan_in, fan_out, dtype="f32"):
     """U(+-sqrt(6/(fan_in+fan_out))) as BASELINE.json's configs say ("Xavier-uniform from a seed")."""
-    g = _rng(seed, name)
     bound = math.sqrt(6.0 / (fan_in + fan_out))
-    a = g.random(size=shape, dtype=np.float32)
-    a = (a * np.float32(2.0 * bound)) - np.float32(bound)
-    return round_storage(a, dtype)
+    return _draw(seed, name, shape, "uniform", -bound, bound, dtype)
 
 
 # --------------------------------------------------------------------------------------------

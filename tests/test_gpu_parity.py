@@ -121,8 +121,8 @@ def test_chain_eq2_eq3(ob, rn):
     Ad = [rn.to_dev(a, "f32") for a in Ac]
     Bd = [rn.to_dev(b, "f32") for b in Br]
     ws = torch.empty(ob.orbit_chain_workspace_bytes(m, d, n, e, T, "f32"), dtype=torch.uint8, device="cuda")
-    y = torch.empty(m, e, device="cuda")
-    dx = torch.empty(m, d, device="cuda")
+    y = torch.empty(m, e, device="cuda", dtype=torch.float32)
+    dx = torch.empty(m, d, device="cuda", dtype=torch.float32)
     ob.orbit_chain_fwd(m, d, n, e, T, "f32", rn.to_dev(x, "f32"), Ad, Bd, y, ws)
     ob.orbit_chain_bwd(m, d, n, e, T, "f32", rn.to_dev(dy, "f32"), Ad, Bd, dx, ws)
     torch.cuda.synchronize()

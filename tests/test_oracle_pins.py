@@ -15,7 +15,6 @@ import torch
 from oracle import orbit_oracle as orc
 from paper_2404_14712_b200 import inputs as syn
 
-torch.set_default_dtype(torch.float64)
 RNG = np.random.default_rng(7)
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 

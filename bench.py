@@ -282,10 +282,13 @@ def run_ours(args, cfg):
 
     achieved = gemm_flops / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(cfg.name)
+            import csv
+            for row in csv.DictReader(open(tp)):
+                if row["workload"] == cfg.name:
+                    traffic = float(row["dram_bytes_per_launch"])
         except Exception:
             traffic = None
     roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (tcgen05 bf16 GEMM, all 12 GEMMs of the block)",

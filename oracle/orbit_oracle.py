@@ -216,10 +216,10 @@ def attention(Q, K, V, heads):
     """Per (b, head j): S = Q_j K_j^T / sqrt(d_h); P = softmax over keys; O_j = P V_j
     (PAPER.md:88 softmax(QK^T)V; :114 "scaled dot product").  Q, K, V: [B, N, D] -> O [B, N, D],
     P [B, heads, N, N]."""
-    B, N, D = Q.shape
+    B, N, D = Q.shape                       # Q may hold a subset of the query rows (N != K.shape[1])
     dh = D // heads
     O = np.empty((B, N, D), dtype=F64)
-    Pm = np.empty((B, heads, N, N), dtype=F64)
+    Pm = np.empty((B, heads, N, K.shape[1]), dtype=F64)
     for b in range(B):
         for j in range(heads):
             c = slice(j * dh, (j + 1) * dh)
@@ -400,6 +400,52 @@ def block_bwd_sharded(dy, Pc, shards, cache):
     dz1, Gc["ln1_g"], Gc["ln1_b"] = layernorm_bwd(da, cache["xhat"], cache["rstd1"], Pc["ln1_g"])
     dx = dx1 + dz1
     return dx, Gc, Gs
+
+
+# ---------------------------------------------------------------------------------------------
+# Sampled outputs at full size.  The same formulas as TOK / A2 / BLK / BLK' restricted to the outputs a
+# test samples, for sizes where the whole oracle would take too long (tests pin each of them to the
+# corresponding slice of the full functions on small shapes).
+# ---------------------------------------------------------------------------------------------
+def tokenize_patches(x, Wp, bp, p, ls):
+    """tok[:, ls, :, :] of tokenize(): tokens of the sampled patches `ls` only."""
+    pix = patches(x, p)[:, :, ls, :]                                  # [B, V, S, p^2]
+    Wp, bp = _f64(Wp), _f64(bp)
+    B, V, S, _ = pix.shape
+    tok = np.empty((B, S, V, Wp.shape[2]), dtype=F64)
+    for v in range(V):
+        tok[:, :, v, :] = pix[:, v] @ Wp[v] + bp[v]
+    return tok
+
+
+def block_sampled(x, dy, P, heads, eps, rows, fcols):
+    """Outputs of block_fwd / block_bwd that can be had one by one without the whole backward:
+       y[:, rows, :];  dbfc2;  and for the sampled MLP columns f in fcols: dWfc2[f, :], dWfc1[:, f],
+       dbfc1[f].  The first half (LN1, QKV, attention, proj, LN2) is computed in full exactly as in
+       block_fwd; the MLP is evaluated on the sampled rows (for y) and the sampled columns (for grads)."""
+    x, dy = _f64(x), _f64(dy)
+    B, N, D = x.shape
+    M = B * N
+    a, _, _ = layernorm(x, P["ln1_g"], P["ln1_b"], eps)
+    qkv = a @ _f64(P["Wqkv"]) + _f64(P["bqkv"])
+    O, _ = attention(qkv[..., 0:D], qkv[..., D:2 * D], qkv[..., 2 * D:3 * D], heads)
+    x1 = x + O @ _f64(P["Wproj"]) + _f64(P["bproj"])
+    m, _, _ = layernorm(x1, P["ln2_g"], P["ln2_b"], eps)
+    out = {"x1": x1}
+    # y on the sampled rows: u = m Wfc1 + bfc1; g = GELU(u); y = x1 + g Wfc2 + bfc2
+    Wfc1, Wfc2 = _f64(P["Wfc1"]), _f64(P["Wfc2"])
+    u_r = m[:, rows, :] @ Wfc1 + _f64(P["bfc1"])
+    out["y_rows"] = x1[:, rows, :] + gelu(u_r) @ Wfc2 + _f64(P["bfc2"])
+    # MLP gradients on the sampled columns
+    dy2, m2 = dy.reshape(M, D), m.reshape(M, D)
+    out["bfc2"] = dy2.sum(axis=0)
+    u_f = m2 @ Wfc1[:, fcols] + _f64(P["bfc1"])[fcols]                # [M, |f|]
+    g_f = gelu(u_f)
+    out["Wfc2_rows"] = g_f.T @ dy2                                    # dWfc2[f, :]
+    du_f = (dy2 @ Wfc2[fcols, :].T) * gelu_grad(u_f)
+    out["bfc1_cols"] = du_f.sum(axis=0)
+    out["Wfc1_cols"] = m2.T @ du_f                                    # dWfc1[:, f]
+    return out
 
 
 # ---------------------------------------------------------------------------------------------

@@ -402,3 +402,30 @@ def test_bf16_rounding_helper():
     r = syn.round_bf16(a)
     ref = torch.tensor(a, dtype=torch.float32).to(torch.bfloat16).to(torch.float32).numpy()
     assert np.array_equal(r, ref)
+
+
+# ------------------------------------------------------------------ sampled-output helpers -----
+def test_sampled_helpers_equal_slices_of_full_functions():
+    """block_sampled / tokenize_patches (used by the full-size GPU tests) are slices of the full definitions;
+    attention with a query subset equals the rows of the full attention."""
+    B, N, D, h, F = 2, 12, 16, 4, 40
+    P = rand_block_params(D, F)
+    x, dy = rnd(B, N, D), rnd(B, N, D)
+    y, cache = orc.block_fwd(x, P, h, 1e-5)
+    dx, G = orc.block_bwd(dy, P, cache)
+    rows, fcols = np.array([0, 5, 11]), np.array([1, 7, 39])
+    s = orc.block_sampled(x, dy, P, h, 1e-5, rows, fcols)
+    assert orc.rel_fro(s["y_rows"], y[:, rows]) < 1e-13
+    assert orc.rel_fro(s["x1"], cache["x1"]) < 1e-14
+    assert orc.rel_fro(s["bfc2"], G["bfc2"]) < 1e-13
+    assert orc.rel_fro(s["Wfc2_rows"], G["Wfc2"][fcols]) < 1e-13
+    assert orc.rel_fro(s["Wfc1_cols"], G["Wfc1"][:, fcols]) < 1e-13
+    assert orc.rel_fro(s["bfc1_cols"], G["bfc1"][fcols]) < 1e-13
+    Q, K, V = rnd(B, N, D), rnd(B, N, D), rnd(B, N, D)
+    O, _ = orc.attention(Q, K, V, h)
+    Os, _ = orc.attention(Q[:, rows], K, V, h)
+    assert np.allclose(Os, O[:, rows], atol=1e-14)
+    xf = rnd(2, 3, 8, 12)
+    Wp, bp = rnd(3, 4, 5), rnd(3, 5)
+    ls = np.array([0, 7, 23])
+    assert np.array_equal(orc.tokenize_patches(xf, Wp, bp, 2, ls), orc.tokenize(xf, Wp, bp, 2)[:, ls])

@@ -9,7 +9,7 @@ namespace {
 
 struct AggSaved {
   float *alpha, *qt, *Ut;
-  void *o, *Xbar;
+  void *o, *Xbar, *Utb;
   size_t bytes;
 };
 AggSaved carve_agg_saved(const orbit_agg_desc& d, void* base) {
@@ -21,6 +21,7 @@ AggSaved carve_agg_saved(const orbit_agg_desc& d, void* base) {
   s.Ut = c.take_n<float>(D * h);                // collapsed key projection [D, heads]
   s.o = c.take(BL * D * dsize(d.dtype));        // concat_a o_a  [B*L, D]
   s.Xbar = c.take(BL * h * D * dsize(d.dtype)); // sum_v alpha[v,a] X_v  [B*L, heads, D]
+  s.Utb = c.take(agg_tc_utb_bytes((int)D));     // bf16 copy of Ut^T for the tensor-core kernels
   s.bytes = c.off;
   return s;
 }
@@ -93,7 +94,9 @@ int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_ag
     ORBIT_TRY(gemm_simt(g, s));
   }
   ORBIT_TRY(agg_make_u(P->Wk, dt, sv.qt, sv.Ut, D, h, s));
-  ORBIT_TRY(agg_patch_fwd(tok, dt, sv.Ut, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
+  const bool tc = !g_force_simt && agg_tc_supported(dt, d->V, D, h);
+  if (tc) ORBIT_TRY(agg_patch_fwd_tc(tok, sv.Ut, sv.Utb, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
+  else ORBIT_TRY(agg_patch_fwd(tok, dt, sv.Ut, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
   for (int a = 0; a < h; a++) {  // o_a = Xbar_a Wv[:, a] + bv[a]
     GemmArgs g;
     g.A = offs(sv.Xbar, (size_t)a * D, dt); g.a_rs = (long long)h * D; g.a_cs = 1;
@@ -168,7 +171,9 @@ int orbit_var_aggregate_bwd(const orbit_agg_desc* d, const void* tok, const orbi
     gx.in_dtype = dt; gx.out_dtype = dt;
     ORBIT_TRY(gemm(gx, s));
   }
-  ORBIT_TRY(agg_patch_bwd(tok, dt, sv.Ut, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
+  const bool tc = !g_force_simt && agg_tc_supported(dt, d->V, D, h);
+  if (tc) ORBIT_TRY(agg_patch_bwd_tc(tok, sv.Utb, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
+  else ORBIT_TRY(agg_patch_bwd(tok, dt, sv.Ut, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
   ORBIT_TRY(agg_param_bwd(acc_dUt, sv.qt, P->q, P->Wq, P->Wk, dt, G->Wk, G->bk, G->bq, G->Wq, G->q, dqt, D, h, s));
   ORBIT_TRY(cast_copy(acc_bo, ORBIT_F32, G->bo, dt, D, s));
   ORBIT_TRY(cast_copy(acc_bv, ORBIT_F32, G->bv, dt, D, s));

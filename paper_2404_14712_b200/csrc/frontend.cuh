@@ -26,5 +26,12 @@ int agg_param_bwd(const float* dUt, const float* qt, const void* q, const void* 
 //   dpos[l,:] = sum_b dagg[b,l,:]
 int agg_dpos(const void* dagg, int dt, void* dpos, int B, int L, int D, cudaStream_t s);
 size_t agg_patch_bwd_smem(int V, int D, int heads);
+// tensor-core (mma.sync) per-patch kernels, bf16 only (aggregate_tc.cu)
+bool agg_tc_supported(int dt, int V, int D, int heads);
+size_t agg_tc_utb_bytes(int D);
+int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, void* Xbar, int BL, int V, int D, int heads,
+                     cudaStream_t s);
+int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const void* dXbar, void* dtok, float* dUt_acc,
+                     int BL, int V, int D, int heads, cudaStream_t s);
 
 }  // namespace orbit

@@ -94,7 +94,7 @@ int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_ag
     ORBIT_TRY(gemm_simt(g, s));
   }
   ORBIT_TRY(agg_make_u(P->Wk, dt, sv.qt, sv.Ut, D, h, s));
-  const bool tc = !g_force_simt && agg_tc_supported(dt, d->V, D, h);
+  const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);
   if (tc) ORBIT_TRY(agg_patch_fwd_tc(tok, sv.Ut, sv.Utb, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
   else ORBIT_TRY(agg_patch_fwd(tok, dt, sv.Ut, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
   for (int a = 0; a < h; a++) {  // o_a = Xbar_a Wv[:, a] + bv[a]
@@ -171,7 +171,7 @@ int orbit_var_aggregate_bwd(const orbit_agg_desc* d, const void* tok, const orbi
     gx.in_dtype = dt; gx.out_dtype = dt;
     ORBIT_TRY(gemm(gx, s));
   }
-  const bool tc = !g_force_simt && agg_tc_supported(dt, d->V, D, h);
+  const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);
   if (tc) ORBIT_TRY(agg_patch_bwd_tc(tok, sv.Utb, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
   else ORBIT_TRY(agg_patch_bwd(tok, dt, sv.Ut, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
   ORBIT_TRY(agg_param_bwd(acc_dUt, sv.qt, P->q, P->Wq, P->Wk, dt, G->Wk, G->bk, G->bq, G->Wq, G->q, dqt, D, h, s));

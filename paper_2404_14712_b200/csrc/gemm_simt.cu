@@ -97,7 +97,7 @@ int gemm_simt(const GemmArgs& g, cudaStream_t s) {
 }
 
 int gemm(const GemmArgs& g, cudaStream_t s) {
-  if (!g_force_simt && gemm_tc_supported(g)) return gemm_tc(g, s);
+  if (g_force_simt != 1 && gemm_tc_supported(g)) return gemm_tc(g, s);
   return gemm_simt(g, s);
 }
 

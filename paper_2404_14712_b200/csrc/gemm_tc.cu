@@ -309,17 +309,13 @@ int launch(const CUtensorMap& ma, const CUtensorMap& mb, const Epi& e, int M, in
   }
   const int tiles = cdiv(M, BM) * cdiv(N, BN);
   const int grid = tiles < num_sms() ? tiles : num_sms();
-  const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
-  if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
   gemm_tc_kernel<A_MN, B_MN><<<grid, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K);
-  if (rec) {
-    ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n + 1], s));
-    g_prof.flops[g_prof.n++] = 2.0 * M * N * K;
-  }
-  ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
 }  // namespace
+
+int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, bool a_mn, bool b_mn, int sms,
+                    cudaStream_t s);   // gemm_tc2.cu
 
 int gemm_profile_enable(int on) {
   if (on && !g_prof.ev) {
@@ -365,20 +361,35 @@ bool gemm_tc_supported(const GemmArgs& g) {
 int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   const bool a_mn = !(g.a_cs == 1 && g.a_rs % 8 == 0);
   const bool b_mn = (g.b_cs == 1 && g.b_rs % 8 == 0);
+  // CTA-pair kernel (256 x 256 tiles) when the problem has at least one full pair tile; g_force_simt == 2
+  // forces the single-CTA kernel (debug / A-B comparison)
+  const bool pair = g_force_simt != 2 && g.M >= 256 && g.N >= 256;
   CUtensorMap ma, mb;
-  if (a_mn) ORBIT_TRY(make_map(&ma, g.A, g.M, g.K, g.a_cs, 64, 64));     // [K rows, M contiguous]
-  else      ORBIT_TRY(make_map(&ma, g.A, g.K, g.M, g.a_rs, 64, BM));     // [M rows, K contiguous]
-  if (b_mn) ORBIT_TRY(make_map(&mb, g.B, g.N, g.K, g.b_rs, 64, 64));     // [K rows, N contiguous]
-  else      ORBIT_TRY(make_map(&mb, g.B, g.K, g.N, g.b_cs, 64, BN));     // [N rows, K contiguous]
-  Epi e;
-  e.C = g.C; e.ldc = g.ldc; e.out_dt = g.out_dtype; e.bias = g.bias; e.bias_dt = g.bias_dtype;
-  e.resid = g.resid; e.resid_dt = g.resid_dtype; e.ldr = g.ldr; e.resid_row_mod = g.resid_row_mod;
-  e.accumulate = g.accumulate; e.act = g.act; e.aux_out = g.aux_out; e.aux_in = g.aux_in; e.ld_aux = g.ld_aux;
-  e.aux_dt = g.aux_dtype;
-  if (!a_mn && b_mn) return launch<0, 1>(ma, mb, e, g.M, g.N, g.K, s);
-  if (!a_mn && !b_mn) return launch<0, 0>(ma, mb, e, g.M, g.N, g.K, s);
-  if (a_mn && b_mn) return launch<1, 1>(ma, mb, e, g.M, g.N, g.K, s);
-  return launch<1, 0>(ma, mb, e, g.M, g.N, g.K, s);
+  if (a_mn) ORBIT_TRY(make_map(&ma, g.A, g.M, g.K, g.a_cs, 64, 64));               // [K rows, M contiguous]
+  else      ORBIT_TRY(make_map(&ma, g.A, g.K, g.M, g.a_rs, 64, BM));               // [M rows, K contiguous]
+  if (b_mn) ORBIT_TRY(make_map(&mb, g.B, g.N, g.K, g.b_rs, 64, 64));               // [K rows, N contiguous]
+  else      ORBIT_TRY(make_map(&mb, g.B, g.K, g.N, g.b_cs, 64, pair ? 128 : BN));  // [N rows, K contiguous]
+  const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
+  if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
+  if (pair) {
+    ORBIT_TRY(gemm_tc2_launch(ma, mb, g, a_mn, b_mn, num_sms(), s));
+  } else {
+    Epi e;
+    e.C = g.C; e.ldc = g.ldc; e.out_dt = g.out_dtype; e.bias = g.bias; e.bias_dt = g.bias_dtype;
+    e.resid = g.resid; e.resid_dt = g.resid_dtype; e.ldr = g.ldr; e.resid_row_mod = g.resid_row_mod;
+    e.accumulate = g.accumulate; e.act = g.act; e.aux_out = g.aux_out; e.aux_in = g.aux_in; e.ld_aux = g.ld_aux;
+    e.aux_dt = g.aux_dtype;
+    if (!a_mn && b_mn) ORBIT_TRY((launch<0, 1>(ma, mb, e, g.M, g.N, g.K, s)));
+    else if (!a_mn && !b_mn) ORBIT_TRY((launch<0, 0>(ma, mb, e, g.M, g.N, g.K, s)));
+    else if (a_mn && b_mn) ORBIT_TRY((launch<1, 1>(ma, mb, e, g.M, g.N, g.K, s)));
+    else ORBIT_TRY((launch<1, 0>(ma, mb, e, g.M, g.N, g.K, s)));
+  }
+  if (rec) {
+    ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n + 1], s));
+    g_prof.flops[g_prof.n++] = 2.0 * g.M * g.N * g.K;
+  }
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
 }
 
 }  // namespace orbit

@@ -1,0 +1,196 @@
+// gemm_tc2.cu -- CTA-pair (cta_group::2) variant of the tcgen05 bf16 GEMM: a cluster of two CTAs on one TPC
+// computes a 256 x 256 output tile.  Each CTA loads its own 128 rows of A and its own 128 columns of B (so the
+// per-SM shared-memory traffic per MMA is halved), the leader CTA issues tcgen05.mma.cta_group::2 (M = 256),
+// and each CTA drains its own 128 x 256 half of the accumulator from its own TMEM.
+// Stage = 16 KB (A half) + 16 KB (B half) -> 6 stages in 192 KB.  Same operand-major handling and fused epilogue
+// as gemm_tc.cu.  Synchronisation:
+//   full[s]   (leader's, count 1): the leader's producer arrives expecting the bytes of BOTH CTAs; the peer's TMA
+//                                  complete_tx on it too (a remote arrive per stage costs ~1400 cycles: measured)
+//   empty[s]  (per CTA, count 1) : tcgen05.commit multicast to both CTAs frees the stage
+//   tfull[a]  (per CTA, count 1) : tcgen05.commit multicast -> both epilogues
+//   tempty[a] (leader's, count 8): the 4 epilogue warps of both CTAs release the accumulator
+#include <cuda.h>
+#include "common.cuh"
+#include "gemm_epi.cuh"
+#include "ptx.cuh"
+
+namespace orbit {
+namespace {
+
+constexpr int BM2 = 256, BN2 = 256, BK = 64, UK = 16;
+constexpr int STAGES = 6;
+constexpr int A_BYTES = 128 * BK * 2;           // this CTA's half of A
+constexpr int B_BYTES = 128 * BK * 2;           // this CTA's half of B
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
+constexpr int NTHREADS = 192;
+constexpr int TMEM_COLS = 512;
+constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 + 256;
+
+__device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, int& mb, int& nb) {
+  constexpr int GROUP = 8;                      // 8 x 256 rows of A shared through L2 by concurrent clusters
+  const int group_size = GROUP * tiles_n;
+  const int g = t / group_size, r = t - g * group_size;
+  const int first_m = g * GROUP;
+  const int gm = min(GROUP, tiles_m - first_m);
+  mb = first_m + r % gm;
+  nb = r / gm;
+}
+
+template <int A_MN, int B_MN>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, epi::Args e, int M, int N, int K) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = ptx::cluster_ctarank();
+  const bool leader = rank == 0;
+  const int tiles_m = (M + BM2 - 1) / BM2, tiles_n = (N + BN2 - 1) / BN2;
+  const int num_tiles = tiles_m * tiles_n;
+  const int num_kb = (K + BK - 1) / BK;
+  const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmA);
+    ptx::prefetch_tmap(&tmB);
+    for (int s = 0; s < STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 8); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) {
+    ptx::tmem_alloc_2sm(tmem_slot, TMEM_COLS);
+    ptx::tmem_relinquish_2sm();
+  }
+  ptx::tc_fence_before();
+  ptx::cluster_sync_all();                       // barrier inits and TMEM allocation visible in both CTAs
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  if (warp == 0) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (lane == 0) {
+      int s = 0; uint32_t ph = 0;
+      for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+        int mb, nb;
+        tile_coords2(t, tiles_m, tiles_n, mb, nb);
+        const int m0 = mb * BM2 + (int)rank * 128, n0 = nb * BN2 + (int)rank * 128;
+        for (int kb = 0; kb < num_kb; kb++) {
+          ptx::mbar_wait(empty_bar(s), ph ^ 1);
+          const uint32_t lfull = ptx::mapa(full_bar(s), 0);
+          if (leader) ptx::mbar_expect_tx(full_bar(s), 2 * STAGE_BYTES);
+          const uint32_t sa = smem_base + s * STAGE_BYTES, sb = sa + A_BYTES;
+          const int k0 = kb * BK;
+          if (A_MN) {
+#pragma unroll
+            for (int i = 0; i < 2; i++) ptx::tma_load_2d_2sm(sa + i * 8192, &tmA, lfull, m0 + i * 64, k0);
+          } else {
+            ptx::tma_load_2d_2sm(sa, &tmA, lfull, k0, m0);
+          }
+          if (B_MN) {
+#pragma unroll
+            for (int i = 0; i < 2; i++) ptx::tma_load_2d_2sm(sb + i * 8192, &tmB, lfull, n0 + i * 64, k0);
+          } else {
+            ptx::tma_load_2d_2sm(sb, &tmB, lfull, k0, n0);
+          }
+          if (++s == STAGES) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (leader CTA only) =====================
+    if (leader && lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(BM2, BN2, A_MN, B_MN);
+      constexpr uint32_t a_lbo = A_MN ? 8192 : 16, a_sbo = 1024, a_step = A_MN ? 2048 : 32;
+      constexpr uint32_t b_lbo = B_MN ? 8192 : 16, b_sbo = 1024, b_step = B_MN ? 2048 : 32;
+      int s = 0; uint32_t ph = 0;
+      int acc = 0; uint32_t aph = 0;
+      for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+        ptx::mbar_wait(tempty_bar(acc), aph ^ 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * BN2;
+        for (int kb = 0; kb < num_kb; kb++) {
+          ptx::mbar_wait(full_bar(s), ph);
+          ptx::tc_fence_after();
+          const uint32_t sa = smem_base + s * STAGE_BYTES, sb = sa + A_BYTES;
+#pragma unroll
+          for (int k = 0; k < BK / UK; k++) {
+            const uint64_t da = ptx::make_smem_desc(sa + k * a_step, a_lbo, a_sbo);
+            const uint64_t db = ptx::make_smem_desc(sb + k * b_step, b_lbo, b_sbo);
+            ptx::mma_f16_ss_2sm(d_tmem, da, db, idesc, (kb | k) != 0);
+          }
+          ptx::mma_commit_2sm(empty_bar(s), 3);
+          if (++s == STAGES) { s = 0; ph ^= 1; }
+        }
+        ptx::mma_commit_2sm(tfull_bar(acc), 3);
+        if (++acc == 2) { acc = 0; aph ^= 1; }
+      }
+    }
+  } else {
+    // ===================== epilogue (both CTAs, own half of the rows) =====================
+    const int quarter = warp & 3;
+    int acc = 0; uint32_t aph = 0;
+    for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+      int mb, nb;
+      tile_coords2(t, tiles_m, tiles_n, mb, nb);
+      const int row = mb * BM2 + (int)rank * 128 + quarter * 32 + lane;
+      const int n0 = nb * BN2;
+      ptx::mbar_wait(tfull_bar(acc), aph);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + acc * BN2 + ((uint32_t)(quarter * 32) << 16);
+      const int rrow = e.resid_row_mod > 0 ? (row % e.resid_row_mod) : row;
+#pragma unroll 1
+      for (int c = 0; c < BN2 / 32; c++) {
+        uint32_t r[32];
+        ptx::tmem_ld_32x32(taddr + c * 32, r);
+        ptx::tmem_ld_wait();
+        if (row < M) epi::chunk32(e, r, row, rrow, n0 + c * 32, N);
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), 0));
+      if (++acc == 2) { acc = 0; aph ^= 1; }
+    }
+  }
+  ptx::tc_fence_before();
+  ptx::cluster_sync_all();                       // peer smem / barriers stay alive until both CTAs are done
+  if (warp == 1) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc_2sm(tmem_base, TMEM_COLS);
+  }
+}
+
+template <int A_MN, int B_MN>
+int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const epi::Args& e, int M, int N, int K, int sms, cudaStream_t s) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)gemm_tc2_kernel<A_MN, B_MN>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+    attr_set = true;
+  }
+  const int tiles = cdiv(M, BM2) * cdiv(N, BN2);
+  int clusters = sms / 2;
+  if (tiles < clusters) clusters = tiles;
+  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K);
+  return ORBIT_OK;
+}
+}  // namespace
+
+// called by gemm_tc() (gemm_tc.cu), which builds the tensor maps: A boxes as in the 1-CTA kernel, B boxes with
+// 128 rows (K-major) or 64 x 64 (N-major)
+int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, bool a_mn, bool b_mn, int sms,
+                    cudaStream_t s) {
+  const epi::Args e = epi::from_gemm(g);
+  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, e, g.M, g.N, g.K, sms, s);
+  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, e, g.M, g.N, g.K, sms, s);
+  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, e, g.M, g.N, g.K, sms, s);
+  return launch2<1, 0>(ma, mb, e, g.M, g.N, g.K, sms, s);
+}
+
+}  // namespace orbit

@@ -8,7 +8,7 @@
 //                                  complete_tx on it too (a remote arrive per stage costs ~1400 cycles: measured)
 //   empty[s]  (per CTA, count 1) : tcgen05.commit multicast to both CTAs frees the stage
 //   tfull[a]  (per CTA, count 1) : tcgen05.commit multicast -> both epilogues
-//   tempty[a] (leader's, count 8): the 4 epilogue warps of both CTAs release the accumulator
+//   tempty[a] (leader's, count 16): the 8 epilogue warps of both CTAs release the accumulator
 #include <cuda.h>
 #include "common.cuh"
 #include "gemm_epi.cuh"
@@ -22,7 +22,7 @@ constexpr int STAGES = 6;
 constexpr int A_BYTES = 128 * BK * 2;           // this CTA's half of A
 constexpr int B_BYTES = 128 * BK * 2;           // this CTA's half of B
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
-constexpr int NTHREADS = 192;
+constexpr int NTHREADS = 320;                   // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (2 per TMEM lane quarter)
 constexpr int TMEM_COLS = 512;
 constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 + 256;
 
@@ -60,7 +60,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     ptx::prefetch_tmap(&tmA);
     ptx::prefetch_tmap(&tmB);
     for (int s = 0; s < STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 8); }
+    for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 16); }
     ptx::fence_barrier_init();
   }
   if (warp == 1) {
@@ -134,7 +134,8 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
   } else {
     // ===================== epilogue (both CTAs, own half of the rows) =====================
-    const int quarter = warp & 3;
+    const int quarter = warp & 3;                // TMEM lanes [32*quarter, +32)
+    const int chalf = (warp - 2) >> 2;           // which 128 of the 256 accumulator columns
     int acc = 0; uint32_t aph = 0;
     for (int t = cluster_id; t < num_tiles; t += num_clusters) {
       int mb, nb;
@@ -146,7 +147,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       const uint32_t taddr = tmem_base + acc * BN2 + ((uint32_t)(quarter * 32) << 16);
       const int rrow = e.resid_row_mod > 0 ? (row % e.resid_row_mod) : row;
 #pragma unroll 1
-      for (int c = 0; c < BN2 / 32; c++) {
+      for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
         uint32_t r[32];
         ptx::tmem_ld_32x32(taddr + c * 32, r);
         ptx::tmem_ld_wait();

@@ -193,15 +193,42 @@ __global__ void __launch_bounds__(256) agg_patch_bwd_kernel(const void* __restri
   }
 }
 
-// dqt[c] = sum_d dUt[d,a(c)] Wk[d,c] / sqrt(d_a)
-__global__ void agg_dqt_kernel(const float* __restrict__ dUt, const void* __restrict__ Wk, int p_dt,
-                               float* __restrict__ dqt, int D, int h) {
-  int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= D) return;
-  int da = D / h, a = c / da;
+// dqt[c] = sum_d dUt[d,a(c)] Wk[d,c] / sqrt(d_a): 32 columns x 8 row-lanes per block, rows strided over lanes
+__global__ void __launch_bounds__(256) agg_dqt_kernel(const float* __restrict__ dUt, const void* __restrict__ Wk, int p_dt,
+                                                      float* __restrict__ dqt, int D, int h) {
+  __shared__ float sh[8][33];
+  const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
+  const int c = blockIdx.x * 32 + cx;
+  const int da = D / h, a = c < D ? c / da : 0;
   float s = 0.f;
-  for (int d = 0; d < D; d++) s = fmaf(dUt[(size_t)d * h + a], ldf(Wk, (size_t)d * D + c, p_dt), s);
-  dqt[c] = s * rsqrtf((float)da);
+  if (c < D)
+    for (int d = ry; d < D; d += 8) s = fmaf(dUt[(size_t)d * h + a], ldf(Wk, (size_t)d * D + c, p_dt), s);
+  sh[ry][cx] = s;
+  __syncthreads();
+  if (ry == 0 && c < D) {
+    float t = 0.f;
+#pragma unroll
+    for (int y = 0; y < 8; y++) t += sh[y][cx];
+    dqt[c] = t * rsqrtf((float)da);
+  }
+}
+// qt[n] = sum_k q[k] Wq[k,n] + bq[n]   (one learned query, R4: a GEMV, same column-strided scheme)
+__global__ void __launch_bounds__(256) agg_qt_kernel(const void* __restrict__ q, const void* __restrict__ Wq,
+                                                     const void* __restrict__ bq, int p_dt, float* __restrict__ qt, int D) {
+  __shared__ float sh[8][33];
+  const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
+  const int n = blockIdx.x * 32 + cx;
+  float s = 0.f;
+  if (n < D)
+    for (int k = ry; k < D; k += 8) s = fmaf(ldf(q, k, p_dt), ldf(Wq, (size_t)k * D + n, p_dt), s);
+  sh[ry][cx] = s;
+  __syncthreads();
+  if (ry == 0 && n < D) {
+    float t = 0.f;
+#pragma unroll
+    for (int y = 0; y < 8; y++) t += sh[y][cx];
+    qt[n] = t + ldf(bq, n, p_dt);
+  }
 }
 // dWk[d,c] = dUt[d,a(c)] qt[c]/sqrt(d_a); dWq[i,c] = q[i] dqt[c]; dbk = 0; dbq = dqt
 __global__ void agg_outer_kernel(const float* __restrict__ dUt, const float* __restrict__ qt,
@@ -232,6 +259,12 @@ __global__ void agg_dpos_kernel(const void* __restrict__ dagg, int dt, void* __r
   stf(dpos, i, s, dt);
 }
 }  // namespace
+
+int agg_make_qt(const void* q, const void* Wq, const void* bq, int p_dt, float* qt, int D, cudaStream_t s) {
+  agg_qt_kernel<<<cdiv(D, 32), 256, 0, s>>>(q, Wq, bq, p_dt, qt, D);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
 
 int agg_make_u(const void* Wk, int p_dt, const float* qt, float* Ut, int D, int heads, cudaStream_t s) {
   long long threads = (long long)D * heads * 32;
@@ -283,7 +316,7 @@ int agg_patch_bwd(const void* tok, int dt, const float* Ut, const float* alpha, 
 int agg_param_bwd(const float* dUt, const float* qt, const void* q, const void* Wq, const void* Wk, int p_dt,
                   void* dWk, void* dbk, void* dbq, void* dWq, void* dq, float* dqt_ws, int D, int heads,
                   cudaStream_t s) {
-  agg_dqt_kernel<<<cdiv(D, 128), 128, 0, s>>>(dUt, Wk, p_dt, dqt_ws, D, heads);
+  agg_dqt_kernel<<<cdiv(D, 32), 256, 0, s>>>(dUt, Wk, p_dt, dqt_ws, D, heads);
   ORBIT_LAUNCH_CHECK();
   agg_outer_kernel<<<cdiv((long long)D * D, 256), 256, 0, s>>>(dUt, qt, dqt_ws, q, p_dt, dWk, dWq, dbk, dbq, D, heads);
   ORBIT_LAUNCH_CHECK();

@@ -87,12 +87,7 @@ int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_ag
   cudaStream_t s = (cudaStream_t)stream;
   const int BL = d->B * d->L, D = d->D, h = d->heads, da = D / h, dt = d->dtype, rt = d->resid_dtype;
   AggSaved sv = carve_agg_saved(*d, saved);
-  {  // qt = q Wq + bq   (data independent, PAPER-silent detail: R3)
-    GemmArgs g;
-    g.A = P->q; g.a_rs = D; g.a_cs = 1; g.B = P->Wq; g.b_rs = D; g.b_cs = 1; g.C = sv.qt; g.ldc = D;
-    g.M = 1; g.N = D; g.K = D; g.in_dtype = dt; g.out_dtype = ORBIT_F32; g.bias = P->bq; g.bias_dtype = dt;
-    ORBIT_TRY(gemm_simt(g, s));
-  }
+  ORBIT_TRY(agg_make_qt(P->q, P->Wq, P->bq, dt, sv.qt, D, s));   // qt = q Wq + bq (data independent; R3, R4)
   ORBIT_TRY(agg_make_u(P->Wk, dt, sv.qt, sv.Ut, D, h, s));
   const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);
   if (tc) ORBIT_TRY(agg_patch_fwd_tc(tok, sv.Ut, sv.Utb, sv.alpha, sv.Xbar, BL, d->V, D, h, s));

@@ -12,6 +12,8 @@ int tokenize_bwd_acc(const orbit_embed_desc& d, const float* x, const void* dtok
 
 // a2 helpers (collapsed form):
 //   Ut[d,a] = sum_{c in head a} Wk[d,c] qt[c] / sqrt(d_a)
+//   qt[n] = sum_k q[k] Wq[k,n] + bq[n]
+int agg_make_qt(const void* q, const void* Wq, const void* bq, int p_dt, float* qt, int D, cudaStream_t s);
 int agg_make_u(const void* Wk, int p_dt, const float* qt, float* Ut, int D, int heads, cudaStream_t s);
 //   per patch: s[v,a] = X_v . Ut[:,a]; alpha = softmax_v; Xbar[a,:] = sum_v alpha[v,a] X_v
 int agg_patch_fwd(const void* tok, int dt, const float* Ut, float* alpha, void* Xbar, int BL, int V, int D,

@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(1024) ln_fwd_kernel(const void* __restrict__ x
 
 // ---- LayerNorm backward ------------------------------------------------------------------------------
 template <int MAXCH>
-__global__ void __launch_bounds__(1024) ln_bwd_kernel(const void* __restrict__ dout, int dout_dt,
+__global__ void __launch_bounds__(MAXCH == 1 ? 1024 : 512) ln_bwd_kernel(const void* __restrict__ dout, int dout_dt,
     const void* __restrict__ x, int x_dt, const float* __restrict__ mean, const float* __restrict__ rstd,
     const void* __restrict__ gamma, int p_dt, const void* __restrict__ add, int add_dt,
     float* __restrict__ dx_f32, void* __restrict__ dx_out, int out_dt,
@@ -270,13 +270,21 @@ int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, 
 int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
                   const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
                   int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s) {
+  // <= 512 threads once a thread owns more than one 8-column chunk: the per-column dgamma/dbeta accumulators
+  // (16 registers per chunk) then fit without spills
+  const int nch = D / 8;
   int thr = ln_threads(D);
-  int maxch = cdiv(D / 8, thr);
-  int grid = M < 148 * 2 ? M : 148 * 2;
+  int maxch = cdiv(nch, thr);
+  if (maxch > 1) {
+    maxch = cdiv(nch, 512);
+    thr = ((cdiv(nch, maxch) + 31) / 32) * 32;
+  }
+  int grid = M < 148 * 4 ? M : 148 * 4;
 #define LNB(C) ln_bwd_kernel<C><<<grid, thr, 0, s>>>(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, \
                                                      dx_f32, dx_out, out_dt, dgamma_acc, dbeta_acc, M, D)
   if (maxch <= 1) LNB(1);
   else if (maxch <= 2) LNB(2);
+  else if (maxch <= 3) LNB(3);
   else if (maxch <= 4) LNB(4);
   else { set_error("layernorm_bwd: D=%d too large", D); return ORBIT_ERR_SHAPE; }
 #undef LNB

@@ -71,6 +71,7 @@ int orbit_tokenize(const orbit_embed_desc* d, const float* x, const void* Wp, co
   if (!x || !Wp || !bp || !tok) { set_error("tokenize: NULL pointer"); return ORBIT_ERR_NULL; }
   if (!aligned16(x) || !aligned16(Wp) || !aligned16(bp) || !aligned16(tok)) { set_error("tokenize: pointer not 16B aligned"); return ORBIT_ERR_ALIGN; }
   ORBIT_TRY(check_device());
+  if (g_force_simt != 1 && tokenize_tc_supported(*d)) return tokenize_fwd_tc(*d, x, Wp, bp, tok, (cudaStream_t)stream);
   return tokenize_fwd(*d, x, Wp, bp, tok, (cudaStream_t)stream);
 }
 
@@ -91,7 +92,8 @@ int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dt
   float* accW = (float*)ws;
   float* accB = accW + (size_t)d->V * P2 * d->D;
   ORBIT_TRY(fill_zero(ws, (size_t)d->V * (P2 + 1) * d->D * sizeof(float), s));
-  ORBIT_TRY(tokenize_bwd_acc(*d, x, dtok, accW, accB, s));
+  if (g_force_simt != 1 && tokenize_tc_supported(*d)) ORBIT_TRY(tokenize_bwd_acc_tc(*d, x, dtok, accW, accB, s));
+  else ORBIT_TRY(tokenize_bwd_acc(*d, x, dtok, accW, accB, s));
   ORBIT_TRY(cast_copy(accW, ORBIT_F32, dWp, d->dtype, (size_t)d->V * P2 * d->D, s));
   ORBIT_TRY(cast_copy(accB, ORBIT_F32, dbp, d->dtype, (size_t)d->V * d->D, s));
   return ORBIT_OK;

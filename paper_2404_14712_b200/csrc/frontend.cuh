@@ -10,6 +10,11 @@ int tokenize_fwd(const orbit_embed_desc& d, const float* x, const void* Wp, cons
 int tokenize_bwd_acc(const orbit_embed_desc& d, const float* x, const void* dtok, float* accW, float* accB,
                      cudaStream_t s);
 
+// tensor-core versions (bf16; tokenize_tc.cu)
+bool tokenize_tc_supported(const orbit_embed_desc& d);
+int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, const void* bp, void* tok, cudaStream_t s);
+int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* dtok, float* accW, float* accB, cudaStream_t s);
+
 // a2 helpers (collapsed form):
 //   Ut[d,a] = sum_{c in head a} Wk[d,c] qt[c] / sqrt(d_a)
 //   qt[n] = sum_k q[k] Wq[k,n] + bq[n]

@@ -1,0 +1,256 @@
+// tokenize_tc.cu -- a1 / a1' on tensor cores (bf16 storage): "independent patch tokenization for each
+// channel input".  At patch 4 the K = p^2 = 16 contraction costs 16 FMA per 2 output bytes on CUDA cores
+// (ALU-bound, ~2x the HBM time); as one or two mma.sync k-steps it disappears under the token stream.
+//
+// fp32 pixels are split exactly into bf16 hi + lo parts (pix = hi + lo + O(2^-17)), so the contraction is
+// [hi | lo] (K = 2 p^2) against [Wp ; Wp] and loses nothing against the fp32-FMA kernel.
+//   forward : tok[b, l, v, c0:c0+512] for 128 patches of one (b, v) per CTA; B = [Wp[v]; Wp[v]] chunk in smem.
+//   backward: dWp[v] (p^2 x D) and dbp[v] = sum over patches of pix^T dtok / dtok: CTA = (v, 512 columns, a range
+//             of patches); dtok rows stream through a 4-stage cp.async ring; A fragments are built from pixels.
+#include "frontend.cuh"
+
+namespace orbit {
+namespace {
+
+constexpr int NT = 256;
+constexpr int DCH = 512;                 // columns per CTA
+constexpr int BROW = (DCH + 8) * 2;      // padded smem row of the B tiles (bytes): conflict-free ldmatrix
+
+__device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void ldsm4(uint32_t addr, uint32_t* r) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm4t(uint32_t addr, uint32_t* r) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void mma16816(float* c, const uint32_t* a, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ void split_bf16(float x, bf16& hi, bf16& lo) {
+  hi = __float2bfloat16_rn(x);
+  lo = __float2bfloat16_rn(x - __bfloat162float(hi));
+}
+// B fragments of an N-major tile with padded rows: 16 k from k0, 16 n from n0
+__device__ __forceinline__ void ldB(uint32_t base, int k0, int n0, uint32_t* r) {
+  int lane = threadIdx.x & 31;
+  ldsm4t(base + (k0 + (lane & 7) + ((lane >> 3) & 1) * 8) * BROW + (n0 + (lane >> 4) * 8) * 2, r);
+}
+__device__ __forceinline__ float pixel(const float* x, int V, int Hg, int Wg, int p, int bl, int L, int v, int r) {
+  const int b = bl / L, l = bl - b * L, gw = Wg / p;
+  const int i = l / gw, j = l - i * gw, di = r / p, dj = r - di * p;
+  return x[(((size_t)b * V + v) * Hg + i * p + di) * Wg + j * p + dj];
+}
+
+// ---------------------------------------------------------------- forward ----------------------------------
+// KP = contraction length after the hi/lo split, padded to a multiple of 16 (p = 4: 32; p = 2: 16; p = 1: 16)
+template <int P2, int KP>
+__global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, const float* __restrict__ x,
+    const bf16* __restrict__ Wp, const bf16* __restrict__ bp, bf16* __restrict__ tok, int L) {
+  constexpr int PT = 128, AROW = (KP + 8) * 2;          // patches per CTA; padded A row (bytes)
+  extern __shared__ __align__(128) uint8_t smem[];
+  uint8_t* sA = smem;                                     // [PT][KP + 8] bf16
+  uint8_t* sB = smem + PT * AROW;                         // [KP][DCH + 8] bf16
+  const int v = blockIdx.y, c0 = blockIdx.z * DCH;
+  const int BL = d.B * L, bl0 = blockIdx.x * PT;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int ncol = min(DCH, d.D - c0);
+  // A: [hi | lo | 0] of the pixels
+  for (int idx = threadIdx.x; idx < PT * KP; idx += NT) {
+    const int pr = idx / KP, k = idx - pr * KP;
+    bf16 val = __float2bfloat16_rn(0.f);
+    if (k < 2 * P2 && bl0 + pr < BL) {
+      bf16 hi, lo;
+      split_bf16(pixel(x, d.V, d.Hg, d.Wg, d.p, bl0 + pr, L, v, k % P2), hi, lo);
+      val = k < P2 ? hi : lo;
+    }
+    *reinterpret_cast<bf16*>(sA + pr * AROW + k * 2) = val;
+  }
+  // B: [Wp[v]; Wp[v]; 0] columns c0..c0+ncol
+  for (int idx = threadIdx.x; idx < KP * (DCH / 8); idx += NT) {
+    const int k = idx / (DCH / 8), ch = idx - k * (DCH / 8);
+    uint4 val = make_uint4(0, 0, 0, 0);
+    if (k < 2 * P2 && ch * 8 < ncol) val = *reinterpret_cast<const uint4*>(Wp + ((size_t)v * P2 + (k % P2)) * d.D + c0 + ch * 8);
+    *reinterpret_cast<uint4*>(sB + k * BROW + ch * 16) = val;
+  }
+  __syncthreads();
+  uint32_t af[KP / 16][4];
+  {
+    const int row = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+#pragma unroll
+    for (int ks = 0; ks < KP / 16; ks++) ldsm4(s_u32(sA) + row * AROW + (ks * 16 + (lane >> 4) * 8) * 2, af[ks]);
+  }
+  const int r_lo = bl0 + warp * 16 + g, r_hi = r_lo + 8;
+  bf16* o_lo = tok + ((size_t)r_lo * d.V + v) * d.D + c0;
+  bf16* o_hi = tok + ((size_t)r_hi * d.V + v) * d.D + c0;
+  const bf16* bias = bp + (size_t)v * d.D + c0;
+  const uint32_t sBu = s_u32(sB);
+#pragma unroll 2
+  for (int np = 0; np < DCH / 16; np++) {
+    if (np * 16 >= ncol) break;
+    float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+    for (int ks = 0; ks < KP / 16; ks++) {
+      uint32_t b[4];
+      ldB(sBu, ks * 16, np * 16, b);
+      mma16816(acc[0], af[ks], b[0], b[1]);
+      mma16816(acc[1], af[ks], b[2], b[3]);
+    }
+#pragma unroll
+    for (int nt = 0; nt < 2; nt++) {
+      const int col = np * 16 + nt * 8 + 2 * t;
+      const float2 bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + col));
+      if (r_lo < BL) *reinterpret_cast<uint32_t*>(o_lo + col) = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
+      if (r_hi < BL) *reinterpret_cast<uint32_t*>(o_hi + col) = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
+    }
+  }
+}
+
+// ---------------------------------------------------------------- backward ---------------------------------
+// accW[v, r, c] += sum_patches pix[patch, r] dtok[patch, v, c];  accB[v, c] += sum_patches dtok[patch, v, c]
+template <int P2>
+__global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, const float* __restrict__ x,
+    const bf16* __restrict__ dtok, float* __restrict__ accW, float* __restrict__ accB, int L, int patches_per_cta) {
+  constexpr int STG = 4, KC = 16;                         // ring stages; patches per k-chunk
+  extern __shared__ __align__(128) uint8_t smem[];
+  uint8_t* sB = smem;                                     // [STG][KC][DCH + 8] bf16
+  float* sP = reinterpret_cast<float*>(smem + STG * KC * BROW);   // [STG][KC][16] pixels (fp32)
+  const int v = blockIdx.y, c0 = blockIdx.z * DCH;
+  const int BL = d.B * L;
+  const int p0 = blockIdx.x * patches_per_cta, p1 = min(BL, p0 + patches_per_cta);
+  const int nchunks = (p1 - p0 + KC - 1) / KC;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int ncol = min(DCH, d.D - c0);
+
+  auto load = [&](int ci) {
+    const int st = ci % STG, base = p0 + ci * KC;
+    for (int idx = threadIdx.x; idx < KC * (DCH / 8); idx += NT) {
+      const int k = idx / (DCH / 8), ch = idx - k * (DCH / 8);
+      const uint32_t dst = s_u32(sB + (st * KC + k) * BROW + ch * 16);
+      if (base + k < p1 && ch * 8 < ncol) cp_async16(dst, dtok + ((size_t)(base + k) * d.V + v) * d.D + c0 + ch * 8);
+      else *reinterpret_cast<uint4*>(sB + (st * KC + k) * BROW + ch * 16) = make_uint4(0, 0, 0, 0);
+    }
+    {
+      const int k = threadIdx.x >> 4, r = threadIdx.x & 15;     // 16 x 16 pixels per chunk
+      float pv = 0.f;
+      if (r < P2 && base + k < p1) pv = pixel(x, d.V, d.Hg, d.Wg, d.p, base + k, L, v, r);
+      sP[(st * KC + k) * 16 + r] = pv;
+    }
+    cp_commit();
+  };
+
+  float aw[8][4], ab[8][4];
+#pragma unroll
+  for (int i = 0; i < 8; i++) { aw[i][0] = aw[i][1] = aw[i][2] = aw[i][3] = 0.f; ab[i][0] = ab[i][1] = ab[i][2] = ab[i][3] = 0.f; }
+  uint32_t ones[4];
+  ones[0] = (g == 0) ? 0x3F803F80u : 0u;                   // row 0 of the A tile = 1.0 (bf16 pair), other rows 0
+  ones[1] = 0u; ones[2] = ones[0]; ones[3] = 0u;
+
+  for (int i = 0; i < STG - 1; i++) { if (i < nchunks) load(i); else cp_commit(); }
+  for (int ci = 0; ci < nchunks; ci++) {
+    cp_wait<STG - 2>();
+    __syncthreads();
+    if (ci + STG - 1 < nchunks) load(ci + STG - 1); else cp_commit();
+    const int st = ci % STG;
+    // A fragments (rows = pixel index r, cols = patch k) straight from the pixel tile, split hi / lo
+    const float* pt = sP + st * KC * 16;
+    uint32_t ah[4], al[4];
+    {
+      bf16 h0, l0, h1, l1;
+      split_bf16(pt[(2 * t) * 16 + g], h0, l0); split_bf16(pt[(2 * t + 1) * 16 + g], h1, l1);
+      ah[0] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[0] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
+      split_bf16(pt[(2 * t) * 16 + g + 8], h0, l0); split_bf16(pt[(2 * t + 1) * 16 + g + 8], h1, l1);
+      ah[1] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[1] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
+      split_bf16(pt[(2 * t + 8) * 16 + g], h0, l0); split_bf16(pt[(2 * t + 9) * 16 + g], h1, l1);
+      ah[2] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[2] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
+      split_bf16(pt[(2 * t + 8) * 16 + g + 8], h0, l0); split_bf16(pt[(2 * t + 9) * 16 + g + 8], h1, l1);
+      ah[3] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[3] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
+    }
+    const uint32_t bt = s_u32(sB + st * KC * BROW);
+#pragma unroll
+    for (int np = 0; np < 4; np++) {                       // this warp's 64 columns = 4 pairs of n-tiles
+      uint32_t b[4];
+      ldB(bt, 0, warp * 64 + np * 16, b);
+      mma16816(aw[2 * np], ah, b[0], b[1]);     mma16816(aw[2 * np + 1], ah, b[2], b[3]);
+      mma16816(aw[2 * np], al, b[0], b[1]);     mma16816(aw[2 * np + 1], al, b[2], b[3]);
+      mma16816(ab[2 * np], ones, b[0], b[1]);   mma16816(ab[2 * np + 1], ones, b[2], b[3]);
+    }
+  }
+#pragma unroll
+  for (int nt = 0; nt < 8; nt++) {
+    const int col = warp * 64 + nt * 8 + 2 * t;
+    if (col < ncol) {
+      if (g < P2) {
+        atomicAdd(accW + ((size_t)v * P2 + g) * d.D + c0 + col, aw[nt][0]);
+        atomicAdd(accW + ((size_t)v * P2 + g) * d.D + c0 + col + 1, aw[nt][1]);
+      }
+      if (g + 8 < P2) {
+        atomicAdd(accW + ((size_t)v * P2 + g + 8) * d.D + c0 + col, aw[nt][2]);
+        atomicAdd(accW + ((size_t)v * P2 + g + 8) * d.D + c0 + col + 1, aw[nt][3]);
+      }
+      if (g == 0) {
+        atomicAdd(accB + (size_t)v * d.D + c0 + col, ab[nt][0]);
+        atomicAdd(accB + (size_t)v * d.D + c0 + col + 1, ab[nt][1]);
+      }
+    }
+  }
+}
+}  // namespace
+
+bool tokenize_tc_supported(const orbit_embed_desc& d) {
+  return d.dtype == ORBIT_BF16 && (d.p == 1 || d.p == 2 || d.p == 4) && d.D % 16 == 0;
+}
+
+int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, const void* bp, void* tok, cudaStream_t s) {
+  const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
+  dim3 grid(cdiv((long long)d.B * L, 128), d.V, cdiv(d.D, DCH));
+#define TF(P, K) do {                                                                                         \
+    const size_t smb = (size_t)128 * (K + 8) * 2 + (size_t)K * BROW;                                          \
+    static bool set = false;                                                                                  \
+    if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)tok_fwd_tc_kernel<P, K>,                  \
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }       \
+    tok_fwd_tc_kernel<P, K><<<grid, NT, smb, s>>>(d, x, (const bf16*)Wp, (const bf16*)bp, (bf16*)tok, L); } while (0)
+  if (P2 == 16) TF(16, 32);
+  else if (P2 == 4) TF(4, 16);
+  else TF(1, 16);
+#undef TF
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* dtok, float* accW, float* accB, cudaStream_t s) {
+  const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
+  const long long BL = (long long)d.B * L;
+  const int nz = cdiv(d.D, DCH);
+  int splits = cdiv(148 * 6, d.V * nz);
+  int ppc = cdiv(BL, splits);
+  ppc = ((ppc + 15) / 16) * 16;
+  if (ppc < 64) ppc = 64;
+  dim3 grid(cdiv(BL, ppc), d.V, nz);
+  const size_t smb = (size_t)4 * 16 * BROW + (size_t)4 * 16 * 16 * sizeof(float);
+#define TB(P) do {                                                                                            \
+    static bool set = false;                                                                                  \
+    if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)tok_bwd_tc_kernel<P>,                     \
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }       \
+    tok_bwd_tc_kernel<P><<<grid, NT, smb, s>>>(d, x, (const bf16*)dtok, accW, accB, L, ppc); } while (0)
+  if (P2 == 16) TB(16);
+  else if (P2 == 4) TB(4);
+  else TB(1);
+#undef TB
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+}  // namespace orbit

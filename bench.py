@@ -178,6 +178,8 @@ def run_ours(args, cfg):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     seed = syn.seed_of(cfg.name)
+    if args.debug_mode:
+        ob.lib.orbit_set_debug_force_simt(args.debug_mode)
 
     # ---- build the workload (inputs resident in HBM) ----
     if cfg.V is None:
@@ -339,6 +341,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C2", "C3", "C4", "C5"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--debug-mode", type=int, default=0, help="orbit_set_debug_force_simt value (A/B comparisons only)")
     args = ap.parse_args()
     cfg = syn.CONFIGS[args.workload]
     if args.impl == "reference":

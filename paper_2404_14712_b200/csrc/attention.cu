@@ -1,4 +1,8 @@
-// attention.cu -- dispatch between the tensor-core (bf16) and the fp32-FMA attention kernels.
+// attention.cu -- dispatch between the attention kernels:
+//   forward : tcgen05/TMEM flash kernel (attention_tc5.cu) for bf16, d_h in {64, 128}, N >= 128;
+//             mma.sync flash kernel (attention_tc.cu) otherwise for bf16 d_h in {64, 128}; fp32-FMA kernels else.
+//   backward: mma.sync flash kernels (dQ and dK/dV) for bf16; fp32-FMA kernels else.
+// orbit_set_debug_force_simt: 1 = fp32-FMA kernels everywhere, 3 = skip the tcgen05 attention (A/B comparison).
 #include "common.cuh"
 
 namespace orbit {
@@ -6,8 +10,11 @@ namespace orbit {
 bool attention_tc_supported(const AttnArgs& a);
 int attention_fwd_tc(const AttnArgs& a, cudaStream_t s);
 int attention_bwd_tc(const AttnArgs& a, cudaStream_t s);
+bool attention_tc5_supported(const AttnArgs& a);
+int attention_fwd_tc5(const AttnArgs& a, cudaStream_t s);
 
 int attention_fwd(const AttnArgs& a, cudaStream_t s) {
+  if (g_force_simt != 1 && g_force_simt != 3 && attention_tc5_supported(a)) return attention_fwd_tc5(a, s);
   if (g_force_simt != 1 && attention_tc_supported(a)) return attention_fwd_tc(a, s);
   return attention_fwd_simt(a, s);
 }

@@ -1,8 +1,8 @@
 // attention.cu -- dispatch between the attention kernels:
-//   forward : tcgen05/TMEM flash kernel (attention_tc5.cu) for bf16, d_h in {64, 128}, N >= 128;
-//             mma.sync flash kernel (attention_tc.cu) otherwise for bf16 d_h in {64, 128}; fp32-FMA kernels else.
-//   backward: mma.sync flash kernels (dQ and dK/dV) for bf16; fp32-FMA kernels else.
-// orbit_set_debug_force_simt: 1 = fp32-FMA kernels everywhere, 3 = skip the tcgen05 attention (A/B comparison).
+//   tcgen05/TMEM flash kernels (attention_tc5.cu), forward and backward, for bf16, d_h in {64, 128}, N >= 128;
+//   mma.sync flash kernels (attention_tc.cu) otherwise for bf16 d_h in {64, 128}; fp32-FMA kernels else.
+// orbit_set_debug_force_simt: 1 = fp32-FMA kernels everywhere, 3 = skip the tcgen05 attention (A/B comparison),
+// 4 = tcgen05 forward only (mma.sync backward).
 #include "common.cuh"
 
 namespace orbit {
@@ -11,7 +11,9 @@ bool attention_tc_supported(const AttnArgs& a);
 int attention_fwd_tc(const AttnArgs& a, cudaStream_t s);
 int attention_bwd_tc(const AttnArgs& a, cudaStream_t s);
 bool attention_tc5_supported(const AttnArgs& a);
+bool attention_bwd_tc5_supported(const AttnArgs& a);
 int attention_fwd_tc5(const AttnArgs& a, cudaStream_t s);
+int attention_bwd_tc5(const AttnArgs& a, cudaStream_t s);
 
 int attention_fwd(const AttnArgs& a, cudaStream_t s) {
   if (g_force_simt != 1 && g_force_simt != 3 && attention_tc5_supported(a)) return attention_fwd_tc5(a, s);
@@ -19,6 +21,8 @@ int attention_fwd(const AttnArgs& a, cudaStream_t s) {
   return attention_fwd_simt(a, s);
 }
 int attention_bwd(const AttnArgs& a, cudaStream_t s) {
+  if (g_force_simt != 1 && g_force_simt != 3 && g_force_simt != 4 && attention_tc5_supported(a) && attention_bwd_tc5_supported(a))
+    return attention_bwd_tc5(a, s);
   if (g_force_simt != 1 && attention_tc_supported(a)) return attention_bwd_tc(a, s);
   return attention_bwd_simt(a, s);
 }

@@ -221,6 +221,376 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
 }
 
+// =====================================================================================================
+// Backward on tcgen05 (split as in attention_tc.cu: a dK/dV kernel with rows = keys and a dQ kernel with rows =
+// queries; 7 tile products, no atomics).  The stationary operand (128 rows) stays in shared memory; the other
+// index streams in tiles of 64 rows through a 2-stage TMA ring.  S^T / dP^T (resp. S / dP) accumulate in TMEM
+// (double buffered, 64 columns each); the 128 "softmax" threads (thread <-> TMEM lane <-> row) turn them into
+// P^T and dS^T (resp. dS) as bf16 K-major operand tiles in shared memory; the gradient accumulators live in TMEM.
+// A streamed [64 x d_h] tile is used twice from the same bytes: as a K-major B operand (contraction over d_h)
+// and as an MN-major B operand (contraction over its 64 rows).
+// =====================================================================================================
+constexpr int BT = 64;
+
+template <int DH>
+struct CfgB {
+  static constexpr int NBLK = DH / 64;
+  static constexpr int BIG = 128 * DH * 2;        // stationary [128 x DH] tile
+  static constexpr int SMALL = BT * DH * 2;       // streamed [64 x DH] tile
+  static constexpr int PT = 128 * BT * 2;         // [128 x 64] bf16 operand tile written by the softmax threads
+  static constexpr int SMEM_DKV = 2 * BIG + 4 * SMALL + 2 * PT + 1024 /*stats*/ + 1024 + 256;
+  static constexpr int SMEM_DQ = 2 * BIG + 4 * SMALL + PT + 1024 + 256;
+};
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// write 64 bf16 (this thread's row r) into a K-major [128 x 64] operand tile (128-byte rows, 128B swizzle)
+__device__ __forceinline__ void write_row64(uint32_t tile, int r, const float* v) {
+#pragma unroll
+  for (int c = 0; c < 8; c++) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      __nv_bfloat162 t2 = __floats2bfloat162_rn(v[c * 8 + 2 * i], v[c * 8 + 2 * i + 1]);
+      pk[i] = *reinterpret_cast<uint32_t*>(&t2);
+    }
+    const uint32_t addr = tile + r * 128 + ((c ^ (r & 7)) << 4);
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+  }
+}
+// TMEM accumulator row (DH fp32 columns of this thread's lane) * scale -> bf16 -> global row
+template <int DH>
+__device__ __forceinline__ void store_acc_row(uint32_t taddr, bf16* dst, float scale, bool ok) {
+#pragma unroll
+  for (int c = 0; c < DH / 32; c++) {
+    uint32_t o[32];
+    ptx::tmem_ld_32x32(taddr + c * 32, o);
+    ptx::tmem_ld_wait();
+    if (ok) {
+#pragma unroll
+      for (int g8 = 0; g8 < 4; g8++) {
+        uint4 v;
+        uint32_t* pv = reinterpret_cast<uint32_t*>(&v);
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+          __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(o[g8 * 8 + 2 * i]) * scale, __uint_as_float(o[g8 * 8 + 2 * i + 1]) * scale);
+          pv[i] = *reinterpret_cast<uint32_t*>(&t2);
+        }
+        *reinterpret_cast<uint4*>(dst + c * 32 + g8 * 8) = v;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- dK, dV : rows = keys -------------------
+template <int DH>
+__global__ void __launch_bounds__(NTH, 1)
+attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
+                        const __grid_constant__ CUtensorMap tmdO, AttnArgs a, float scale, float sl2) {
+  using C = CfgB<DH>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sK = base, sV = sK + C::BIG, sRing = sV + C::BIG, sPt = sRing + 4 * C::SMALL, sdSt = sPt + C::PT,
+                 sStat = sdSt + C::PT, bar = sStat + 1024;
+  auto sQ = [&](int st) { return sRing + st * 2 * C::SMALL; };
+  auto sdO = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
+  float* stat = reinterpret_cast<float*>(smem_raw + (sStat - ptx::smem_u32(smem_raw)));   // [2][2][64]
+  const uint32_t kv_full = bar, qdo_full0 = bar + 8, qdo_empty0 = bar + 24, st_full0 = bar + 40, st_empty0 = bar + 56,
+                 p_full = bar + 72, p_done = bar + 80, tmem_slot = bar + 88;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
+  const int k0 = blockIdx.x * 128;
+  const int ntiles = (N + BT - 1) / BT;
+  const int row0 = b * N;
+  const int qc = a.q_off + h * DH, kc = a.k_off + h * DH, vc = a.v_off + h * DH;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdO);
+    ptx::mbar_init(kv_full, 1);
+    for (int i = 0; i < 2; i++) {
+      ptx::mbar_init(qdo_full0 + 8 * i, 1); ptx::mbar_init(qdo_empty0 + 8 * i, 1);
+      ptx::mbar_init(st_full0 + 8 * i, 1);  ptx::mbar_init(st_empty0 + 8 * i, 4);
+    }
+    ptx::mbar_init(p_full, 4);
+    ptx::mbar_init(p_done, 1);
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
+  const uint32_t tSt = tmem, tdPt = tmem + 128, tdV = tmem + 256, tdK = tmem + 256 + DH;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      ptx::mbar_expect_tx(kv_full, 2 * C::BIG);
+#pragma unroll
+      for (int bk = 0; bk < C::NBLK; bk++) {
+        ptx::tma_load_2d(sK + bk * 16384, &tmBig, kv_full, kc + bk * 64, row0 + k0);
+        ptx::tma_load_2d(sV + bk * 16384, &tmBig, kv_full, vc + bk * 64, row0 + k0);
+      }
+      for (int j = 0; j < ntiles; j++) {
+        const int st = j & 1;
+        ptx::mbar_wait(qdo_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        ptx::mbar_expect_tx(qdo_full0 + 8 * st, 2 * C::SMALL);
+#pragma unroll
+        for (int bk = 0; bk < C::NBLK; bk++) {
+          ptx::tma_load_2d(sQ(st) + bk * 8192, &tmSmall, qdo_full0 + 8 * st, qc + bk * 64, row0 + j * BT);
+          ptx::tma_load_2d(sdO(st) + bk * 8192, &tmdO, qdo_full0 + 8 * st, h * DH + bk * 64, row0 + j * BT);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
+      constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
+      auto issue_s = [&](int j) {
+        const int st = j & 1;
+        ptx::mbar_wait(qdo_full0 + 8 * st, (j >> 1) & 1);
+        ptx::mbar_wait(st_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < DH / 16; ks++) {
+          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+          ptx::mma_f16_ss(tSt + st * BT, ptx::make_smem_desc(sK + ob, 16, 1024), ptx::make_smem_desc(sQ(st) + os, 16, 1024), idesc_s, ks != 0);
+        }
+#pragma unroll
+        for (int ks = 0; ks < DH / 16; ks++) {
+          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+          ptx::mma_f16_ss(tdPt + st * BT, ptx::make_smem_desc(sV + ob, 16, 1024), ptx::make_smem_desc(sdO(st) + os, 16, 1024), idesc_s, ks != 0);
+        }
+        ptx::mma_commit(st_full0 + 8 * st);
+      };
+      ptx::mbar_wait(kv_full, 0);
+      issue_s(0);
+      for (int j = 0; j < ntiles; j++) {
+        if (j + 1 < ntiles) issue_s(j + 1);
+        ptx::mbar_wait(p_full, j & 1);
+        ptx::tc_fence_after();
+        const int st = j & 1;
+#pragma unroll
+        for (int ks = 0; ks < BT / 16; ks++)      // dV += P^T dO_j   (contraction over the tile's 64 queries)
+          ptx::mma_f16_ss(tdV, ptx::make_smem_desc(sPt + ks * 32, 16, 1024), ptx::make_smem_desc(sdO(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
+#pragma unroll
+        for (int ks = 0; ks < BT / 16; ks++)      // dK += dS^T Q_j
+          ptx::mma_f16_ss(tdK, ptx::make_smem_desc(sdSt + ks * 32, 16, 1024), ptx::make_smem_desc(sQ(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
+        ptx::mma_commit(qdo_empty0 + 8 * st);
+        ptx::mma_commit(p_done);
+      }
+    }
+  } else {
+    const int quarter = warp & 3;
+    const int r = quarter * 32 + lane;                       // key row within the CTA tile = TMEM lane
+    const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
+    const int gi = threadIdx.x - 64;                         // 0..127: stats loader index
+    auto load_stat = [&](int j) -> float {
+      const int q = j * BT + (gi & 63);
+      if (j >= ntiles || q >= N) return 0.f;
+      return (gi >> 6) ? a.delta[(size_t)bh * N + q] : a.lse[(size_t)bh * N + q] * LOG2E;
+    };
+    float nxt = load_stat(0);
+    for (int j = 0; j < ntiles; j++) {
+      const int st = j & 1;
+      stat[st * 128 + gi] = nxt;                             // [st][0][c] = lse2, [st][1][c] = delta
+      named_bar_sync(1, 128);
+      nxt = load_stat(j + 1);
+      const float* lse2 = stat + st * 128;
+      const float* dl = lse2 + 64;
+      ptx::mbar_wait(st_full0 + 8 * st, (j >> 1) & 1);
+      ptx::tc_fence_after();
+      uint32_t s[64], dp[64];
+      ptx::tmem_ld_32x32(tSt + st * BT + lane_off, s);
+      ptx::tmem_ld_32x32(tSt + st * BT + 32 + lane_off, s + 32);
+      ptx::tmem_ld_32x32(tdPt + st * BT + lane_off, dp);
+      ptx::tmem_ld_32x32(tdPt + st * BT + 32 + lane_off, dp + 32);
+      ptx::tmem_ld_wait();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(st_empty0 + 8 * st);
+      float p[64];
+      const int nvalid = N - j * BT;                         // queries (columns) >= N are masked
+#pragma unroll
+      for (int c = 0; c < 64; c++) p[c] = (c < nvalid) ? exp2f(__uint_as_float(s[c]) * sl2 - lse2[c]) : 0.f;
+      if (j > 0) ptx::mbar_wait(p_done, (j - 1) & 1);        // P^T / dS^T tiles are free again
+      write_row64(sPt, r, p);
+#pragma unroll
+      for (int c = 0; c < 64; c++) p[c] *= __uint_as_float(dp[c]) - dl[c];
+      write_row64(sdSt, r, p);
+      ptx::fence_proxy_async();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(p_full);
+    }
+    ptx::mbar_wait(p_done, (ntiles - 1) & 1);
+    ptx::tc_fence_after();
+    const int krow = k0 + r;
+    bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld;
+    store_acc_row<DH>(tdV + lane_off, out + vc, 1.f, krow < N);
+    store_acc_row<DH>(tdK + lane_off, out + kc, scale, krow < N);
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
+}
+
+// ---------------------------------------------------------------- dQ : rows = queries -------------------
+template <int DH>
+__global__ void __launch_bounds__(NTH, 1)
+attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
+                       const __grid_constant__ CUtensorMap tmdOBig, AttnArgs a, float scale, float sl2) {
+  using C = CfgB<DH>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = base, sdO = sQ + C::BIG, sRing = sdO + C::BIG, sdS = sRing + 4 * C::SMALL, bar = sdS + C::PT;
+  auto sK = [&](int st) { return sRing + st * 2 * C::SMALL; };
+  auto sV = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
+  const uint32_t q_full = bar, kv_full0 = bar + 8, kv_empty0 = bar + 24, s_full0 = bar + 40, s_empty0 = bar + 56,
+                 p_full = bar + 72, p_done = bar + 80, tmem_slot = bar + 88;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
+  const int q0 = blockIdx.x * 128;
+  const int ntiles = (N + BT - 1) / BT;
+  const int row0 = b * N;
+  const int qc = a.q_off + h * DH, kc = a.k_off + h * DH, vc = a.v_off + h * DH;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdOBig);
+    ptx::mbar_init(q_full, 1);
+    for (int i = 0; i < 2; i++) {
+      ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1);
+      ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 4);
+    }
+    ptx::mbar_init(p_full, 4);
+    ptx::mbar_init(p_done, 1);
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
+  const uint32_t tS = tmem, tdP = tmem + 128, tdQ = tmem + 256;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      ptx::mbar_expect_tx(q_full, 2 * C::BIG);
+#pragma unroll
+      for (int bk = 0; bk < C::NBLK; bk++) {
+        ptx::tma_load_2d(sQ + bk * 16384, &tmBig, q_full, qc + bk * 64, row0 + q0);
+        ptx::tma_load_2d(sdO + bk * 16384, &tmdOBig, q_full, h * DH + bk * 64, row0 + q0);
+      }
+      for (int j = 0; j < ntiles; j++) {
+        const int st = j & 1;
+        ptx::mbar_wait(kv_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        ptx::mbar_expect_tx(kv_full0 + 8 * st, 2 * C::SMALL);
+#pragma unroll
+        for (int bk = 0; bk < C::NBLK; bk++) {
+          ptx::tma_load_2d(sK(st) + bk * 8192, &tmSmall, kv_full0 + 8 * st, kc + bk * 64, row0 + j * BT);
+          ptx::tma_load_2d(sV(st) + bk * 8192, &tmSmall, kv_full0 + 8 * st, vc + bk * 64, row0 + j * BT);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
+      constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
+      auto issue_s = [&](int j) {
+        const int st = j & 1;
+        ptx::mbar_wait(kv_full0 + 8 * st, (j >> 1) & 1);
+        ptx::mbar_wait(s_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < DH / 16; ks++) {
+          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+          ptx::mma_f16_ss(tS + st * BT, ptx::make_smem_desc(sQ + ob, 16, 1024), ptx::make_smem_desc(sK(st) + os, 16, 1024), idesc_s, ks != 0);
+        }
+#pragma unroll
+        for (int ks = 0; ks < DH / 16; ks++) {
+          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+          ptx::mma_f16_ss(tdP + st * BT, ptx::make_smem_desc(sdO + ob, 16, 1024), ptx::make_smem_desc(sV(st) + os, 16, 1024), idesc_s, ks != 0);
+        }
+        ptx::mma_commit(s_full0 + 8 * st);
+      };
+      ptx::mbar_wait(q_full, 0);
+      issue_s(0);
+      for (int j = 0; j < ntiles; j++) {
+        if (j + 1 < ntiles) issue_s(j + 1);
+        ptx::mbar_wait(p_full, j & 1);
+        ptx::tc_fence_after();
+        const int st = j & 1;
+#pragma unroll
+        for (int ks = 0; ks < BT / 16; ks++)      // dQ += dS K_j   (contraction over the tile's 64 keys)
+          ptx::mma_f16_ss(tdQ, ptx::make_smem_desc(sdS + ks * 32, 16, 1024), ptx::make_smem_desc(sK(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
+        ptx::mma_commit(kv_empty0 + 8 * st);
+        ptx::mma_commit(p_done);
+      }
+    }
+  } else {
+    const int quarter = warp & 3;
+    const int r = quarter * 32 + lane;
+    const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
+    const int qrow = q0 + r;
+    const float lse2 = qrow < N ? a.lse[(size_t)bh * N + qrow] * LOG2E : 0.f;
+    const float dl = qrow < N ? a.delta[(size_t)bh * N + qrow] : 0.f;
+    for (int j = 0; j < ntiles; j++) {
+      const int st = j & 1;
+      ptx::mbar_wait(s_full0 + 8 * st, (j >> 1) & 1);
+      ptx::tc_fence_after();
+      uint32_t s[64], dp[64];
+      ptx::tmem_ld_32x32(tS + st * BT + lane_off, s);
+      ptx::tmem_ld_32x32(tS + st * BT + 32 + lane_off, s + 32);
+      ptx::tmem_ld_32x32(tdP + st * BT + lane_off, dp);
+      ptx::tmem_ld_32x32(tdP + st * BT + 32 + lane_off, dp + 32);
+      ptx::tmem_ld_wait();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
+      float ds[64];
+      const int nvalid = N - j * BT;                         // keys (columns) >= N are masked
+#pragma unroll
+      for (int c = 0; c < 64; c++) {
+        const float p = (c < nvalid) ? exp2f(__uint_as_float(s[c]) * sl2 - lse2) : 0.f;
+        ds[c] = p * (__uint_as_float(dp[c]) - dl);
+      }
+      if (j > 0) ptx::mbar_wait(p_done, (j - 1) & 1);
+      write_row64(sdS, r, ds);
+      ptx::fence_proxy_async();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(p_full);
+    }
+    ptx::mbar_wait(p_done, (ntiles - 1) & 1);
+    ptx::tc_fence_after();
+    store_acc_row<DH>(tdQ + lane_off, (bf16*)a.dqkv + (size_t)(row0 + qrow) * a.ld + qc, scale, qrow < N);
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
+}
+
+// delta[b,h,i] = sum_d dO[i, h*dh+d] * O[i, h*dh+d]
+__global__ void attn_delta5_kernel(AttnArgs a) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  const int total = a.B * a.heads * a.N;
+  if (w >= total) return;
+  const int bh = w / a.N, i = w - bh * a.N, b = bh / a.heads, h = bh - b * a.heads;
+  const size_t row = (size_t)b * a.N + i;
+  const bf16* po = (const bf16*)a.O + row * a.ldo + h * a.dh;
+  const bf16* pd = (const bf16*)a.dO + row * a.lddo + h * a.dh;
+  float s = 0.f;
+  for (int d = lane * 2; d < a.dh; d += 64) {
+    float2 x = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(po + d));
+    float2 y = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(pd + d));
+    s += x.x * y.x + x.y * y.y;
+  }
+  s = warp_sum(s);
+  if (lane == 0) a.delta[w] = s;
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -259,7 +629,54 @@ int launch_fwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
+int make_map5(CUtensorMap* tm, const void* basep, long long ld, long long rows, int box_rows) {
+  EncodeTiledFn enc = get_encode5();
+  if (!enc) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
+  cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+  cuuint32_t es[2] = {1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(basep), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("attention: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
+  return ORBIT_OK;
+}
+
+template <int DH>
+int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
+  const long long rows = (long long)a.B * a.N;
+  CUtensorMap tmBig, tmSmall, tmdOBig, tmdOSmall;
+  ORBIT_TRY(make_map5(&tmBig, a.qkv, a.ld, rows, 128));
+  ORBIT_TRY(make_map5(&tmSmall, a.qkv, a.ld, rows, 64));
+  ORBIT_TRY(make_map5(&tmdOBig, a.dO, a.lddo, rows, 128));
+  ORBIT_TRY(make_map5(&tmdOSmall, a.dO, a.lddo, rows, 64));
+  static bool set = false;
+  if (!set) {
+    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_bwd_dkv_tc5_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, CfgB<DH>::SMEM_DKV));
+    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_bwd_dq_tc5_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, CfgB<DH>::SMEM_DQ));
+    set = true;
+  }
+  const int total_w = a.B * a.heads * a.N;
+  attn_delta5_kernel<<<cdiv((long long)total_w * 32, 256), 256, 0, s>>>(a);
+  ORBIT_LAUNCH_CHECK();
+  dim3 grid(cdiv(a.N, 128), a.B * a.heads);
+  const float scale = 1.0f / sqrtf((float)DH);
+  attn_bwd_dq_tc5_kernel<DH><<<grid, NTH, CfgB<DH>::SMEM_DQ, s>>>(tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E);
+  ORBIT_LAUNCH_CHECK();
+  attn_bwd_dkv_tc5_kernel<DH><<<grid, NTH, CfgB<DH>::SMEM_DKV, s>>>(tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
 }  // namespace
+
+int attention_bwd_tc5(const AttnArgs& a, cudaStream_t s) {
+  return a.dh == 64 ? launch_bwd5<64>(a, s) : launch_bwd5<128>(a, s);
+}
+bool attention_bwd_tc5_supported(const AttnArgs& a) {
+  auto al16 = [](const void* p) { return (((uintptr_t)p) & 15) == 0; };
+  return a.dO && al16(a.dO) && a.lddo % 8 == 0 && al16(a.dqkv);
+}
 
 bool attention_tc5_supported(const AttnArgs& a) {
   if (a.dtype != ORBIT_BF16 || (a.dh != 64 && a.dh != 128)) return false;

@@ -214,7 +214,7 @@ def run_ours(args, cfg):
         for i in range(cfg.depth):
             P = syn.block_params(seed, cfg.D, cfg.F, cfg.dtype, tag=f"blk{i}")
             blocks.append((P, syn.shard_block_params(P, cfg.heads, 1)))
-        sr = rn.StepRunner(cfg, emb, agg, blocks)
+        sr = rn.StepRunner(cfg, emb, agg, blocks, fused_front=args.front == "fused")
         del blocks
         x_h = syn.fields(seed, cfg.B, cfg.V, cfg.Hg, cfg.Wg, per_variable_scale=True)
         t_h = syn.normal(seed, "target", (cfg.B, cfg.L, cfg.D), dtype=cfg.resid_dtype)
@@ -316,6 +316,7 @@ def run_ours(args, cfg):
         "data": "synthetic",
         "config": {"workload": workload_string(cfg), "l2": "inputs larger than L2 (weights + saved activations "
                    "streamed every step; no flush needed)", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "front_end": (args.front if cfg.V is not None else None),
                    "model_flops_per_step": flops},
         "tokens_per_s": tokens_s,
         "frac_of_peak_measured_burst": tflops / world / peaks["bf16"],
@@ -340,6 +341,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--front", default="fused", choices=["fused", "twocall"],
+                    help="front end of C2/C3: orbit_embed_fused (pixel space, no tok tensor) or orbit_tokenize + "
+                         "orbit_var_aggregate (tok materialised)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--debug-mode", type=int, default=0, help="orbit_set_debug_force_simt value (A/B comparisons only)")
     args = ap.parse_args()

@@ -85,6 +85,30 @@ size_t orbit_var_aggregate_workspace_bytes(const orbit_agg_desc* d);
 size_t orbit_var_aggregate_bwd_workspace_bytes(const orbit_agg_desc* d);
 size_t orbit_var_aggregate_saved_bytes(const orbit_agg_desc* d);
 
+/* ---- a1+a2 fused in pixel space: same result as orbit_tokenize
+ * followed by orbit_var_aggregate (and, backward, orbit_var_aggregate_bwd followed by orbit_tokenize_bwd), but the
+ * [B, L, V, D] token tensor and its gradient are never formed.  Tokenisation is affine and nothing non-linear
+ * precedes the K/V projections, so with pixext[v, r] = (pix(b,v,l,r), 1), Wpb[(r,v), :] = (Wp[v,r,:] ; bp[v,:]):
+ *   s[v,a] = sum_r pixext[v,r] (Wpb Ut)[(r,v), a];  alpha = softmax_v(s);
+ *   o[:, a] = sum_{r,v} alpha[v,a] pixext[v,r] (Wpb Wv)[(r,v), a-columns] + bv[a];  agg = o Wo + bo (+ pos[l])
+ * (DESIGN.md §4b).  Limits: V <= 128, p in {1,2,4}, heads <= 16 -> ORBIT_ERR_SHAPE otherwise.
+ * x [B,V,Hg,Wg] fp32; Wp [V,p*p,D]; bp [V,D]; agg, dagg [B,L,D] (resid_dtype); dWp, dbp, G as in the two-call path.
+ * `saved` (orbit_embed_fused_saved_bytes) carries alpha and the A operand to the backward call. */
+typedef struct {
+  int B, V, Hg, Wg, p, D, heads;
+  orbit_dtype dtype;           /* parameters, parameter grads, internal operands */
+  orbit_dtype resid_dtype;     /* agg, dagg, pos, dpos */
+} orbit_front_desc;
+int orbit_embed_fused(const orbit_front_desc* d, const float* x, const void* Wp, const void* bp,
+                      const orbit_agg_params* P, const void* pos /* [L,D] nullable */, void* agg, void* saved,
+                      void* ws, size_t ws_bytes, void* stream);
+int orbit_embed_fused_bwd(const orbit_front_desc* d, const float* x, const void* Wp, const void* bp,
+                          const orbit_agg_params* P, const void* dagg, const void* saved, void* dWp, void* dbp,
+                          orbit_agg_grads* G, void* dpos /* [L,D] nullable */, void* ws, size_t ws_bytes, void* stream);
+size_t orbit_embed_fused_workspace_bytes(const orbit_front_desc* d);
+size_t orbit_embed_fused_bwd_workspace_bytes(const orbit_front_desc* d);
+size_t orbit_embed_fused_saved_bytes(const orbit_front_desc* d);
+
 /* ---- a3-a7: one ViT block, pre-LN residual form (R5-R8, R10), optionally in Hybrid-STOP
  * shard-local mode with T shards run one after another on this GPU (Eq. 1-3; R13-R15):
  *   a = LN1(x); qkv = a Wqkv + bqkv; O = softmax(Q K^T / sqrt(d_h)) V per head; x1 = x + O Wproj + bproj;
@@ -152,6 +176,11 @@ int orbit_profile_gemm_collect(double* ms, double* flops, long long* launches);
  * Exercises every operand-major combination the block uses (K-major / MN-major A and B). */
 int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,
                      const void* B, long long b_rs, long long b_cs, float* C, void* stream);
+/* Strided-batch form (the per-head products of the front end): problem i reads A + i*a_bs, B + i*b_bs and writes
+ * C + i*c_bs (element offsets, multiples of 8), C row stride ldc. */
+int orbit_debug_gemm_batched(int M, int N, int K, int batch, orbit_dtype dtype, const void* A, long long a_rs,
+                             long long a_cs, long long a_bs, const void* B, long long b_rs, long long b_cs,
+                             long long b_bs, float* C, long long ldc, long long c_bs, void* stream);
 
 #ifdef __cplusplus
 }

@@ -56,6 +56,11 @@ class orbit_agg_grads(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in _AGG_NAMES]
 
 
+class orbit_front_desc(C.Structure):
+    _fields_ = [("B", C.c_int), ("V", C.c_int), ("Hg", C.c_int), ("Wg", C.c_int), ("p", C.c_int), ("D", C.c_int),
+                ("heads", C.c_int), ("dtype", C.c_int), ("resid_dtype", C.c_int)]
+
+
 class orbit_block_desc(C.Structure):
     _fields_ = [("B", C.c_int), ("N", C.c_int), ("D", C.c_int), ("heads", C.c_int), ("F", C.c_int), ("T", C.c_int),
                 ("ln_eps", C.c_float), ("dtype", C.c_int), ("resid_dtype", C.c_int), ("flags", C.c_uint)]
@@ -102,6 +107,13 @@ _proto("orbit_var_aggregate_bwd", C.c_int,
 for _n in ("orbit_var_aggregate_workspace_bytes", "orbit_var_aggregate_bwd_workspace_bytes",
            "orbit_var_aggregate_saved_bytes"):
     _proto(_n, _sz, [C.POINTER(orbit_agg_desc)])
+_proto("orbit_embed_fused", C.c_int,
+       [C.POINTER(orbit_front_desc), _vp, _vp, _vp, C.POINTER(orbit_agg_params), _vp, _vp, _vp, _vp, _sz, _vp])
+_proto("orbit_embed_fused_bwd", C.c_int,
+       [C.POINTER(orbit_front_desc), _vp, _vp, _vp, C.POINTER(orbit_agg_params), _vp, _vp, _vp, _vp,
+        C.POINTER(orbit_agg_grads), _vp, _vp, _sz, _vp])
+for _n in ("orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes", "orbit_embed_fused_saved_bytes"):
+    _proto(_n, _sz, [C.POINTER(orbit_front_desc)])
 _proto("orbit_block_fwd", C.c_int,
        [C.POINTER(orbit_block_desc), _vp, C.POINTER(orbit_block_params), _vp, _vp, _vp, _sz, _vp])
 _proto("orbit_block_bwd", C.c_int,
@@ -116,6 +128,8 @@ _proto("orbit_mse_loss_grad", C.c_int, [C.c_int, _sz, _vp, _vp, _vp, _vp, _vp])
 _proto("orbit_profile_gemm", C.c_int, [C.c_int])
 _proto("orbit_profile_gemm_collect", C.c_int, [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)])
 _proto("orbit_debug_gemm", C.c_int, [C.c_int] * 4 + [_vp, C.c_longlong, C.c_longlong, _vp, C.c_longlong, C.c_longlong, _vp, _vp])
+_ll = C.c_longlong
+_proto("orbit_debug_gemm_batched", C.c_int, [C.c_int] * 5 + [_vp, _ll, _ll, _ll, _vp, _ll, _ll, _ll, _vp, _ll, _ll, _vp])
 
 EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace_bytes", "orbit_var_aggregate",
            "orbit_var_aggregate_bwd", "orbit_var_aggregate_workspace_bytes",
@@ -124,7 +138,9 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_block_saved_bytes", "orbit_mse_loss_grad", "orbit_chain_fwd", "orbit_chain_bwd", "orbit_chain_workspace_bytes",
            "orbit_last_error", "orbit_version", "orbit_launch_count", "orbit_reset_launch_count",
            "orbit_set_debug_force_simt", "orbit_debug_gemm", "orbit_profile_gemm",
-           "orbit_profile_gemm_collect"]
+           "orbit_profile_gemm_collect", "orbit_embed_fused", "orbit_embed_fused_bwd",
+           "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
+           "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -153,6 +169,10 @@ def embed_desc(B, V, Hg, Wg, p, D, dtype):
 
 def agg_desc(B, L, V, D, heads, dtype, resid_dtype):
     return orbit_agg_desc(B, L, V, D, heads, DTYPES[dtype], DTYPES[resid_dtype])
+
+
+def front_desc(B, V, Hg, Wg, p, D, heads, dtype, resid_dtype):
+    return orbit_front_desc(B, V, Hg, Wg, p, D, heads, DTYPES[dtype], DTYPES[resid_dtype])
 
 
 def block_desc(B, N, D, heads, F, T=1, ln_eps=1e-5, dtype="bf16", resid_dtype="bf16", flags=0):
@@ -210,6 +230,32 @@ def orbit_var_aggregate_bwd(d, tok, P, dagg, saved, dtok, G, dpos, ws, stream=No
                                        _stream(stream)), "orbit_var_aggregate_bwd")
 
 
+def orbit_embed_fused_saved_bytes(d):
+    return lib.orbit_embed_fused_saved_bytes(C.byref(d))
+
+
+def orbit_embed_fused_workspace_bytes(d):
+    return lib.orbit_embed_fused_workspace_bytes(C.byref(d))
+
+
+def orbit_embed_fused_bwd_workspace_bytes(d):
+    return lib.orbit_embed_fused_bwd_workspace_bytes(C.byref(d))
+
+
+def orbit_embed_fused(d, x, Wp, bp, P, pos, agg, saved, ws, stream=None):
+    ps = _agg_struct(orbit_agg_params, P)
+    _check(lib.orbit_embed_fused(C.byref(d), _ptr(x), _ptr(Wp), _ptr(bp), C.byref(ps), _ptr(pos), _ptr(agg), _ptr(saved),
+                                 _ptr(ws), ws.numel() * ws.element_size(), _stream(stream)), "orbit_embed_fused")
+
+
+def orbit_embed_fused_bwd(d, x, Wp, bp, P, dagg, saved, dWp, dbp, G, dpos, ws, stream=None):
+    ps = _agg_struct(orbit_agg_params, P)
+    gs = _agg_struct(orbit_agg_grads, G)
+    _check(lib.orbit_embed_fused_bwd(C.byref(d), _ptr(x), _ptr(Wp), _ptr(bp), C.byref(ps), _ptr(dagg), _ptr(saved),
+                                     _ptr(dWp), _ptr(dbp), C.byref(gs), _ptr(dpos), _ptr(ws),
+                                     ws.numel() * ws.element_size(), _stream(stream)), "orbit_embed_fused_bwd")
+
+
 def orbit_block_saved_bytes(d):
     return lib.orbit_block_saved_bytes(C.byref(d))
 
@@ -262,6 +308,11 @@ def orbit_mse_loss_grad(dtype, y, t, dy, loss, stream=None):
 def orbit_debug_gemm(M, N, K, dtype, A, a_rs, a_cs, B, b_rs, b_cs, Cout, stream=None):
     _check(lib.orbit_debug_gemm(M, N, K, DTYPES[dtype], _ptr(A), a_rs, a_cs, _ptr(B), b_rs, b_cs, _ptr(Cout),
                                 _stream(stream)), "orbit_debug_gemm")
+
+
+def orbit_debug_gemm_batched(M, N, K, batch, dtype, A, a_rs, a_cs, a_bs, B, b_rs, b_cs, b_bs, Cout, ldc, c_bs, stream=None):
+    _check(lib.orbit_debug_gemm_batched(M, N, K, batch, DTYPES[dtype], _ptr(A), a_rs, a_cs, a_bs, _ptr(B), b_rs, b_cs, b_bs,
+                                        _ptr(Cout), ldc, c_bs, _stream(stream)), "orbit_debug_gemm_batched")
 
 
 def orbit_profile_gemm(on: bool):

@@ -92,12 +92,12 @@ int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_ag
   const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);
   if (tc) ORBIT_TRY(agg_patch_fwd_tc(tok, sv.Ut, sv.Utb, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
   else ORBIT_TRY(agg_patch_fwd(tok, dt, sv.Ut, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
-  for (int a = 0; a < h; a++) {  // o_a = Xbar_a Wv[:, a] + bv[a]
+  {  // o_a = Xbar_a Wv[:, a] + bv[a], the `heads` products as one strided-batch launch
     GemmArgs g;
-    g.A = offs(sv.Xbar, (size_t)a * D, dt); g.a_rs = (long long)h * D; g.a_cs = 1;
-    g.B = offs(P->Wv, (size_t)a * da, dt); g.b_rs = D; g.b_cs = 1;
-    g.C = offs(sv.o, (size_t)a * da, dt); g.ldc = D; g.M = BL; g.N = da; g.K = D;
-    g.in_dtype = dt; g.out_dtype = dt; g.bias = offs(P->bv, (size_t)a * da, dt); g.bias_dtype = dt;
+    g.A = sv.Xbar; g.a_rs = (long long)h * D; g.a_cs = 1; g.B = P->Wv; g.b_rs = D; g.b_cs = 1;
+    g.C = sv.o; g.ldc = D; g.M = BL; g.N = da; g.K = D;
+    g.in_dtype = dt; g.out_dtype = dt; g.bias = P->bv; g.bias_dtype = dt;
+    g.batch = h; g.a_bs = D; g.b_bs = da; g.c_bs = da; g.bias_bs = da;
     ORBIT_TRY(gemm(g, s));
   }
   {  // agg = o Wo + bo (+ pos[l])
@@ -153,17 +153,16 @@ int orbit_var_aggregate_bwd(const orbit_agg_desc* d, const void* tok, const orbi
     ORBIT_TRY(gemm(g, s));
   }
   ORBIT_TRY(colsum(w.dob, dt, D, BL, D, acc_bv, nullptr, dt, D, s));   // dbv = sum do   (sum_v alpha = 1)
-  for (int a = 0; a < h; a++) {
-    GemmArgs gw;   // dWv[:, a] = Xbar_a^T do_a
-    gw.A = offs(sv.Xbar, (size_t)a * D, dt); gw.a_rs = 1; gw.a_cs = (long long)h * D;
-    gw.B = offs(w.dob, (size_t)a * da, dt); gw.b_rs = D; gw.b_cs = 1;
-    gw.C = offs(G->Wv, (size_t)a * da, dt); gw.ldc = D; gw.M = D; gw.N = da; gw.K = BL; gw.in_dtype = dt; gw.out_dtype = dt;
+  {
+    GemmArgs gw;   // dWv[:, a] = Xbar_a^T do_a   (strided batch over the heads)
+    gw.A = sv.Xbar; gw.a_rs = 1; gw.a_cs = (long long)h * D; gw.B = w.dob; gw.b_rs = D; gw.b_cs = 1;
+    gw.C = G->Wv; gw.ldc = D; gw.M = D; gw.N = da; gw.K = BL; gw.in_dtype = dt; gw.out_dtype = dt;
+    gw.batch = h; gw.a_bs = D; gw.b_bs = da; gw.c_bs = da;
     ORBIT_TRY(gemm(gw, s));
     GemmArgs gx;   // dXbar_a = do_a Wv[:, a]^T
-    gx.A = offs(w.dob, (size_t)a * da, dt); gx.a_rs = D; gx.a_cs = 1;
-    gx.B = offs(P->Wv, (size_t)a * da, dt); gx.b_rs = 1; gx.b_cs = D;
-    gx.C = offs(w.dXbar, (size_t)a * D, dt); gx.ldc = (long long)h * D; gx.M = BL; gx.N = D; gx.K = da;
-    gx.in_dtype = dt; gx.out_dtype = dt;
+    gx.A = w.dob; gx.a_rs = D; gx.a_cs = 1; gx.B = P->Wv; gx.b_rs = 1; gx.b_cs = D;
+    gx.C = w.dXbar; gx.ldc = (long long)h * D; gx.M = BL; gx.N = D; gx.K = da; gx.in_dtype = dt; gx.out_dtype = dt;
+    gx.batch = h; gx.a_bs = da; gx.b_bs = da; gx.c_bs = D;
     ORBIT_TRY(gemm(gx, s));
   }
   const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);

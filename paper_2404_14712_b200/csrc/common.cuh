@@ -107,6 +107,9 @@ struct GemmArgs {
   int accumulate = 0;            // C += (only meaningful for fp32 C)
   int act = ACT_NONE;
   void* aux_out = nullptr; const void* aux_in = nullptr; long long ld_aux = 0; int aux_dtype = ORBIT_F32;
+  // strided batch: problem i uses A + i*a_bs, B + i*b_bs, C + i*c_bs, bias + i*bias_bs (element offsets; the
+  // per-head products of the front end).  resid / aux / accumulate must be unset when batch > 1.
+  int batch = 1; long long a_bs = 0, b_bs = 0, c_bs = 0, bias_bs = 0;
 };
 int gemm(const GemmArgs& g, cudaStream_t s);           // dispatcher (tensor-core path or SIMT)
 int gemm_simt(const GemmArgs& g, cudaStream_t s);      // fp32-FMA kernels, any dtype/stride

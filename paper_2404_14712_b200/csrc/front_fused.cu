@@ -1,0 +1,414 @@
+// front_fused.cu -- kernels of the fused pixel-space front end (a1 + a2 and a2' + a1' with
+// the [B, L, V, D] token tensor never materialised).
+//
+// Tokenisation is affine in the pixels ("independent patch tokenization for each channel input") and
+// nothing non-linear sits between it and the K/V projections of the aggregation cross-attention (PAPER.md:46
+// "aggregated together across different channels using cross-attention"), so with
+//     pixext[v, r] = pix(b, v, l, r) for r < p^2,  1 for r = p^2            (R = p^2 + 1 entries per variable)
+//     Wpb[(r, v), :] = Wp[v, r, :] for r < p^2,    bp[v, :] for r = p^2     (the tokeniser as one [R*V, D] matrix)
+// the collapsed aggregation of DESIGN.md §4 becomes, exactly (real arithmetic):
+//     s[v, a]  = X_v . Ut[:, a]              = sum_r pixext[v, r] G[(r, v), a],        G = Wpb Ut        [R*V, heads]
+//     o[:, a]  = (sum_v alpha[v, a] X_v) Wv[:, a] + bv[a]
+//              = sum_{r, v} (alpha[v, a] pixext[v, r]) H[(r, v), a-columns] + bv[a],   H = Wpb Wv        [R*V, D]
+// i.e. per head a GEMM  o_a = A_a H_a  with  A_a[bl, (r, v)] = alpha[bl, v, a] pixext[bl, v, r]  (K = R*V, 1547 at
+// C3) instead of V token rows of D elements per patch.  The k index is (r, v) with v fastest and V padded to Vp
+// (a multiple of 8) so that a warp's lanes (= variables) write and read A / dA contiguously.
+//
+// Kernels here (the GEMMs are the library's tcgen05 / SIMT GEMM, strided-batched over the heads):
+//   fe_pack_wpb      Wpb  <- (Wp, bp)
+//   fe_make_g        G    <- Wpb Ut                     (fp32, [R][Vp][HP])
+//   fe_patch_fwd     per patch (one warp): scores, softmax over V, alpha, A
+//   fe_patch_bwd     per patch (one warp): dalpha = <dA, pixext>, ds -> dsT [Vp][BL][HP]
+//   fe_dg            dG[(r, v), a] = sum_bl pixext ds           (score path, reduction over patches)
+//   fe_dut           dUt = Wpb^T dG                              (feeds agg_param_bwd: dWk, dbq, dWq, dq)
+//   fe_finish_dwp    dWp, dbp <- dH Wv^T (fp32 from the GEMM) + dG Ut^T
+#include "front_fused.cuh"
+
+namespace orbit {
+namespace {
+
+constexpr int HP = FE_HP;
+
+template <typename T> struct Pair;
+template <> struct Pair<float> {
+  typedef float2 type;
+  static __device__ __forceinline__ float2 make(float a, float b) { return make_float2(a, b); }
+  static __device__ __forceinline__ float2 unpack(float2 v) { return v; }
+};
+template <> struct Pair<bf16> {
+  typedef __nv_bfloat162 type;
+  static __device__ __forceinline__ __nv_bfloat162 make(float a, float b) { return __floats2bfloat162_rn(a, b); }
+  static __device__ __forceinline__ float2 unpack(__nv_bfloat162 v) { return __bfloat1622float2(v); }
+};
+
+// pixels of patch (b, i, j) of variable v: out[di*P + dj] = x[b, v, i*P + di, j*P + dj]
+template <int P>
+__device__ __forceinline__ void load_pix(const float* __restrict__ x, int V, int Hg, int Wg, int b, int v, int i, int j,
+                                         float* out) {
+  const float* base = x + (((size_t)b * V + v) * Hg + (size_t)i * P) * Wg + (size_t)j * P;
+#pragma unroll
+  for (int di = 0; di < P; di++) {
+    if (P == 4) {
+      const float4 q = *reinterpret_cast<const float4*>(base + (size_t)di * Wg);
+      out[di * 4 + 0] = q.x; out[di * 4 + 1] = q.y; out[di * 4 + 2] = q.z; out[di * 4 + 3] = q.w;
+    } else if (P == 2) {
+      const float2 q = *reinterpret_cast<const float2*>(base + (size_t)di * Wg);
+      out[di * 2 + 0] = q.x; out[di * 2 + 1] = q.y;
+    } else {
+#pragma unroll
+      for (int dj = 0; dj < P; dj++) out[di * P + dj] = base[(size_t)di * Wg + dj];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void fe_pack_wpb_kernel(const T* __restrict__ Wp, const T* __restrict__ bp, T* __restrict__ Wpb, int V, int Vp,
+                                   int P2, int D) {
+  const size_t n = (size_t)(P2 + 1) * Vp * D;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
+    const int d = (int)(idx % D);
+    const int k = (int)(idx / D), r = k / Vp, v = k - r * Vp;
+    T val = from_f<T>(0.f);
+    if (v < V) val = r < P2 ? Wp[((size_t)v * P2 + r) * D + d] : bp[(size_t)v * D + d];
+    Wpb[idx] = val;
+  }
+}
+
+// G[(r, v), a] = sum_d Wpb[(r, v), d] Ut[d, a]; one warp per k row, lanes stride over d
+template <typename T>
+__global__ void fe_make_g_kernel(const T* __restrict__ Wpb, const float* __restrict__ Ut, float* __restrict__ G, int KVp,
+                                 int D, int h) {
+  const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= KVp) return;
+  float acc[HP];
+#pragma unroll
+  for (int a = 0; a < HP; a++) acc[a] = 0.f;
+  for (int d = lane; d < D; d += 32) {
+    const float w = to_f<T>(Wpb[(size_t)k * D + d]);
+#pragma unroll
+    for (int a = 0; a < HP; a++)
+      if (a < h) acc[a] = fmaf(w, Ut[(size_t)d * h + a], acc[a]);
+  }
+#pragma unroll
+  for (int a = 0; a < HP; a++) acc[a] = warp_sum(acc[a]);
+  if (lane == 0) {
+#pragma unroll
+    for (int a = 0; a < HP; a++) G[(size_t)k * HP + a] = acc[a];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// forward, one warp per patch; lane owns the variable pairs (64 n + 2 lane, +1), n < NV
+template <typename T, int P, int NV>
+__global__ void __launch_bounds__(256) fe_patch_fwd_kernel(const float* __restrict__ x, const float* __restrict__ G,
+    float* __restrict__ alpha, T* __restrict__ A, int V, int Vp, int Hg, int Wg, int h, int BL) {
+  constexpr int P2 = P * P, R = P2 + 1, E = 2 * NV;
+  typedef typename Pair<T>::type pair_t;
+  const int lane = threadIdx.x & 31;
+  const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+  const int gw = Wg / P, L = (Hg / P) * gw, KVp = R * Vp;
+  for (int bl = warp0; bl < BL; bl += nwarps) {
+    const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
+    float pix[E][P2], s[E][HP];
+#pragma unroll
+    for (int e = 0; e < E; e++) {
+      const int v = 64 * (e >> 1) + 2 * lane + (e & 1);
+      if (v < V) {
+        load_pix<P>(x, V, Hg, Wg, b, v, i, j, pix[e]);
+        const float4* g4 = reinterpret_cast<const float4*>(G + ((size_t)P2 * Vp + v) * HP);
+#pragma unroll
+        for (int q = 0; q < HP / 4; q++) {
+          const float4 g = __ldg(g4 + q);
+          s[e][4 * q] = g.x; s[e][4 * q + 1] = g.y; s[e][4 * q + 2] = g.z; s[e][4 * q + 3] = g.w;
+        }
+#pragma unroll
+        for (int r = 0; r < P2; r++) {
+          const float4* gr = reinterpret_cast<const float4*>(G + ((size_t)r * Vp + v) * HP);
+#pragma unroll
+          for (int q = 0; q < HP / 4; q++) {
+            const float4 g = __ldg(gr + q);
+            s[e][4 * q] = fmaf(pix[e][r], g.x, s[e][4 * q]);
+            s[e][4 * q + 1] = fmaf(pix[e][r], g.y, s[e][4 * q + 1]);
+            s[e][4 * q + 2] = fmaf(pix[e][r], g.z, s[e][4 * q + 2]);
+            s[e][4 * q + 3] = fmaf(pix[e][r], g.w, s[e][4 * q + 3]);
+          }
+        }
+      } else {
+#pragma unroll
+        for (int r = 0; r < P2; r++) pix[e][r] = 0.f;
+#pragma unroll
+        for (int a = 0; a < HP; a++) s[e][a] = -INFINITY;
+      }
+    }
+    // softmax over the variables, per head (R3): alpha replaces s
+#pragma unroll
+    for (int a = 0; a < HP; a++) {
+      if (a < h) {
+        float m = s[0][a];
+#pragma unroll
+        for (int e = 1; e < E; e++) m = fmaxf(m, s[e][a]);
+        m = warp_max(m);
+        float sum = 0.f;
+#pragma unroll
+        for (int e = 0; e < E; e++) { s[e][a] = __expf(s[e][a] - m); sum += s[e][a]; }
+        sum = warp_sum(sum);
+        const float inv = 1.f / sum;
+#pragma unroll
+        for (int e = 0; e < E; e++) s[e][a] *= inv;
+      }
+    }
+    // alpha [BL, h, Vp] fp32 and A [BL, h, R*Vp] (k = r*Vp + v); padded variables get exact zeros
+#pragma unroll
+    for (int a = 0; a < HP; a++) {
+      if (a < h) {
+#pragma unroll
+        for (int n = 0; n < NV; n++) {
+          const int v0 = 64 * n + 2 * lane;
+          if (v0 < Vp) {
+            const float a0 = s[2 * n][a], a1 = s[2 * n + 1][a];
+            *reinterpret_cast<float2*>(alpha + ((size_t)bl * h + a) * Vp + v0) = make_float2(a0, a1);
+            T* row = A + ((size_t)bl * h + a) * KVp + v0;
+#pragma unroll
+            for (int r = 0; r < P2; r++)
+              *reinterpret_cast<pair_t*>(row + (size_t)r * Vp) = Pair<T>::make(a0 * pix[2 * n][r], a1 * pix[2 * n + 1][r]);
+            *reinterpret_cast<pair_t*>(row + (size_t)P2 * Vp) = Pair<T>::make(a0, a1);
+          }
+        }
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// backward, one warp per patch: dalpha[v, a] = sum_r dA[bl, a, (r, v)] pixext[v, r];
+// ds = alpha (dalpha - sum_w alpha_w dalpha_w) -> dsT[v][bl][a]
+template <typename T, int P, int NV>
+__global__ void __launch_bounds__(256) fe_patch_bwd_kernel(const float* __restrict__ x, const float* __restrict__ alpha,
+    const T* __restrict__ dA, float* __restrict__ dsT, int V, int Vp, int Hg, int Wg, int h, int BL) {
+  constexpr int P2 = P * P, R = P2 + 1, E = 2 * NV;
+  typedef typename Pair<T>::type pair_t;
+  const int lane = threadIdx.x & 31;
+  const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+  const int gw = Wg / P, L = (Hg / P) * gw, KVp = R * Vp;
+  for (int bl = warp0; bl < BL; bl += nwarps) {
+    const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
+    float pix[E][P2], ds[E][HP];
+#pragma unroll
+    for (int e = 0; e < E; e++) {
+      const int v = 64 * (e >> 1) + 2 * lane + (e & 1);
+      if (v < V) load_pix<P>(x, V, Hg, Wg, b, v, i, j, pix[e]);
+      else {
+#pragma unroll
+        for (int r = 0; r < P2; r++) pix[e][r] = 0.f;
+      }
+    }
+#pragma unroll
+    for (int a = 0; a < HP; a++) {
+      if (a < h) {
+        float al[E], da[E];
+        float dot = 0.f;
+#pragma unroll
+        for (int n = 0; n < NV; n++) {
+          const int v0 = 64 * n + 2 * lane;
+          al[2 * n] = al[2 * n + 1] = 0.f; da[2 * n] = da[2 * n + 1] = 0.f;
+          if (v0 < Vp) {
+            const float2 aa = *reinterpret_cast<const float2*>(alpha + ((size_t)bl * h + a) * Vp + v0);
+            al[2 * n] = aa.x; al[2 * n + 1] = aa.y;
+            const T* row = dA + ((size_t)bl * h + a) * KVp + v0;
+            float2 acc = Pair<T>::unpack(*reinterpret_cast<const pair_t*>(row + (size_t)P2 * Vp));
+#pragma unroll
+            for (int r = 0; r < P2; r++) {
+              const float2 g = Pair<T>::unpack(*reinterpret_cast<const pair_t*>(row + (size_t)r * Vp));
+              acc.x = fmaf(g.x, pix[2 * n][r], acc.x);
+              acc.y = fmaf(g.y, pix[2 * n + 1][r], acc.y);
+            }
+            da[2 * n] = acc.x; da[2 * n + 1] = acc.y;
+            dot += aa.x * acc.x + aa.y * acc.y;     // padded variables have alpha == 0
+          }
+        }
+        dot = warp_sum(dot);
+#pragma unroll
+        for (int e = 0; e < E; e++) ds[e][a] = al[e] * (da[e] - dot);
+      } else {
+#pragma unroll
+        for (int e = 0; e < E; e++) ds[e][a] = 0.f;
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < E; e++) {
+      const int v = 64 * (e >> 1) + 2 * lane + (e & 1);
+      if (v < V) {
+        float4* o = reinterpret_cast<float4*>(dsT + ((size_t)v * BL + bl) * HP);
+#pragma unroll
+        for (int q = 0; q < HP / 4; q++) o[q] = make_float4(ds[e][4 * q], ds[e][4 * q + 1], ds[e][4 * q + 2], ds[e][4 * q + 3]);
+      }
+    }
+  }
+}
+
+// dG[(r, v), a] += sum_{bl in this split} pixext[bl, v, r] dsT[v][bl][a]; block = (v, split), thread = (r, a)
+template <int P>
+__global__ void fe_dg_kernel(const float* __restrict__ x, const float* __restrict__ dsT, float* __restrict__ dG, int V, int Vp,
+                             int Hg, int Wg, int BL, int per_split) {
+  constexpr int P2 = P * P, R = P2 + 1;
+  const int v = blockIdx.x, t = threadIdx.x;
+  if (t >= R * HP) return;
+  const int r = t / HP, a = t - r * HP;
+  const int gw = Wg / P, L = (Hg / P) * gw;
+  const int di = r / P, dj = r - di * P;
+  const int bl0 = blockIdx.y * per_split, bl1 = min(BL, bl0 + per_split);
+  float acc = 0.f;
+  const float* dsv = dsT + (size_t)v * BL * HP + a;
+#pragma unroll 4
+  for (int bl = bl0; bl < bl1; bl++) {
+    float pv = 1.f;
+    if (r < P2) {
+      const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
+      pv = __ldg(x + (((size_t)b * V + v) * Hg + (size_t)i * P + di) * Wg + (size_t)j * P + dj);
+    }
+    acc = fmaf(pv, dsv[(size_t)bl * HP], acc);
+  }
+  atomicAdd(dG + ((size_t)r * Vp + v) * HP + a, acc);
+}
+
+// dUt[d, a] += sum_{k in split} Wpb[k, d] dG[k, a]
+template <typename T>
+__global__ void fe_dut_kernel(const T* __restrict__ Wpb, const float* __restrict__ dG, float* __restrict__ dUt, int KVp, int D,
+                              int h, int per_split) {
+  const int d = blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= D) return;
+  const int k0 = blockIdx.y * per_split, k1 = min(KVp, k0 + per_split);
+  float acc[HP];
+#pragma unroll
+  for (int a = 0; a < HP; a++) acc[a] = 0.f;
+  for (int k = k0; k < k1; k++) {
+    const float w = to_f<T>(Wpb[(size_t)k * D + d]);
+    const float4* g4 = reinterpret_cast<const float4*>(dG + (size_t)k * HP);
+#pragma unroll
+    for (int q = 0; q < HP / 4; q++) {
+      const float4 g = __ldg(g4 + q);
+      acc[4 * q] = fmaf(w, g.x, acc[4 * q]); acc[4 * q + 1] = fmaf(w, g.y, acc[4 * q + 1]);
+      acc[4 * q + 2] = fmaf(w, g.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(w, g.w, acc[4 * q + 3]);
+    }
+  }
+#pragma unroll
+  for (int a = 0; a < HP; a++)
+    if (a < h) atomicAdd(dUt + (size_t)d * h + a, acc[a]);
+}
+
+// dWp[v, r, d] / dbp[v, d] = accW[(r, v), d] + sum_a dG[(r, v), a] Ut[d, a]
+template <typename T>
+__global__ void fe_finish_dwp_kernel(const float* __restrict__ accW, const float* __restrict__ dG, const float* __restrict__ Ut,
+                                     T* __restrict__ dWp, T* __restrict__ dbp, int V, int Vp, int P2, int D, int h) {
+  const size_t n = (size_t)(P2 + 1) * V * D;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
+    const int d = (int)(idx % D);
+    const int rv = (int)(idx / D), r = rv / V, v = rv - r * V;
+    const size_t k = (size_t)r * Vp + v;
+    float val = accW[k * D + d];
+    for (int a = 0; a < h; a++) val = fmaf(dG[k * HP + a], Ut[(size_t)d * h + a], val);
+    if (r < P2) dWp[((size_t)v * P2 + r) * D + d] = from_f<T>(val);
+    else dbp[(size_t)v * D + d] = from_f<T>(val);
+  }
+}
+
+int grid_for(size_t n, int block) {
+  size_t g = (n + block - 1) / block;
+  return (int)(g > 148 * 16 ? 148 * 16 : (g ? g : 1));
+}
+}  // namespace
+
+bool fe_supported(int V, int p, int heads) { return V <= 64 * 2 && (p == 1 || p == 2 || p == 4) && heads <= HP; }
+
+int fe_pack_wpb(const void* Wp, const void* bp, int dt, void* Wpb, int V, int Vp, int P2, int D, cudaStream_t s) {
+  const size_t n = (size_t)(P2 + 1) * Vp * D;
+  if (dt == ORBIT_BF16) fe_pack_wpb_kernel<bf16><<<grid_for(n, 256), 256, 0, s>>>((const bf16*)Wp, (const bf16*)bp, (bf16*)Wpb, V, Vp, P2, D);
+  else fe_pack_wpb_kernel<float><<<grid_for(n, 256), 256, 0, s>>>((const float*)Wp, (const float*)bp, (float*)Wpb, V, Vp, P2, D);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fe_make_g(const void* Wpb, int dt, const float* Ut, float* G, int KVp, int D, int h, cudaStream_t s) {
+  const int grid = cdiv((long long)KVp * 32, 256);
+  if (dt == ORBIT_BF16) fe_make_g_kernel<bf16><<<grid, 256, 0, s>>>((const bf16*)Wpb, Ut, G, KVp, D, h);
+  else fe_make_g_kernel<float><<<grid, 256, 0, s>>>((const float*)Wpb, Ut, G, KVp, D, h);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fe_patch_fwd(const float* x, const float* G, float* alpha, void* A, int dt, int V, int Vp, int Hg, int Wg, int p, int h,
+                 int BL, cudaStream_t s) {
+#define ARGS_F(TT) x, G, alpha, (TT*)A, V, Vp, Hg, Wg, h, BL
+  const int nv = V <= 64 ? 1 : 2;
+  const int grid = cdiv(BL, 8) < 148 * 8 ? cdiv(BL, 8) : 148 * 8;
+#define LF(TT, PP, NN) fe_patch_fwd_kernel<TT, PP, NN><<<grid, 256, 0, s>>>(ARGS_F(TT))
+  if (dt == ORBIT_BF16) {
+    if (p == 4) { if (nv == 1) LF(bf16, 4, 1); else LF(bf16, 4, 2); }
+    else if (p == 2) { if (nv == 1) LF(bf16, 2, 1); else LF(bf16, 2, 2); }
+    else { if (nv == 1) LF(bf16, 1, 1); else LF(bf16, 1, 2); }
+  } else {
+    if (p == 4) { if (nv == 1) LF(float, 4, 1); else LF(float, 4, 2); }
+    else if (p == 2) { if (nv == 1) LF(float, 2, 1); else LF(float, 2, 2); }
+    else { if (nv == 1) LF(float, 1, 1); else LF(float, 1, 2); }
+  }
+#undef LF
+#undef ARGS_F
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fe_patch_bwd(const float* x, const float* alpha, const void* dA, int dt, float* dsT, int V, int Vp, int Hg, int Wg, int p,
+                 int h, int BL, cudaStream_t s) {
+#define ARGS_B(TT) x, alpha, (const TT*)dA, dsT, V, Vp, Hg, Wg, h, BL
+  const int nv = V <= 64 ? 1 : 2;
+  const int grid = cdiv(BL, 8) < 148 * 8 ? cdiv(BL, 8) : 148 * 8;
+#define LB(TT, PP, NN) fe_patch_bwd_kernel<TT, PP, NN><<<grid, 256, 0, s>>>(ARGS_B(TT))
+  if (dt == ORBIT_BF16) {
+    if (p == 4) { if (nv == 1) LB(bf16, 4, 1); else LB(bf16, 4, 2); }
+    else if (p == 2) { if (nv == 1) LB(bf16, 2, 1); else LB(bf16, 2, 2); }
+    else { if (nv == 1) LB(bf16, 1, 1); else LB(bf16, 1, 2); }
+  } else {
+    if (p == 4) { if (nv == 1) LB(float, 4, 1); else LB(float, 4, 2); }
+    else if (p == 2) { if (nv == 1) LB(float, 2, 1); else LB(float, 2, 2); }
+    else { if (nv == 1) LB(float, 1, 1); else LB(float, 1, 2); }
+  }
+#undef LB
+#undef ARGS_B
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fe_dg(const float* x, const float* dsT, float* dG, int V, int Vp, int Hg, int Wg, int p, int BL, cudaStream_t s) {
+  const int P2 = p * p, R = P2 + 1;
+  int splits = cdiv(148 * 4, V);
+  if (splits > cdiv(BL, 64)) splits = cdiv(BL, 64);
+  const int per = cdiv(BL, splits);
+  dim3 grid(V, cdiv(BL, per));
+  const int nt = ((R * HP + 31) / 32) * 32;
+  if (p == 4) fe_dg_kernel<4><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, BL, per);
+  else if (p == 2) fe_dg_kernel<2><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, BL, per);
+  else fe_dg_kernel<1><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, BL, per);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fe_dut(const void* Wpb, int dt, const float* dG, float* dUt, int KVp, int D, int h, cudaStream_t s) {
+  const int splits = KVp >= 256 ? 16 : 1, per = cdiv(KVp, splits);
+  dim3 grid(cdiv(D, 128), cdiv(KVp, per));
+  if (dt == ORBIT_BF16) fe_dut_kernel<bf16><<<grid, 128, 0, s>>>((const bf16*)Wpb, dG, dUt, KVp, D, h, per);
+  else fe_dut_kernel<float><<<grid, 128, 0, s>>>((const float*)Wpb, dG, dUt, KVp, D, h, per);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int fe_finish_dwp(const float* accW, const float* dG, const float* Ut, void* dWp, void* dbp, int dt, int V, int Vp, int P2,
+                  int D, int h, cudaStream_t s) {
+  const size_t n = (size_t)(P2 + 1) * V * D;
+  if (dt == ORBIT_BF16) fe_finish_dwp_kernel<bf16><<<grid_for(n, 256), 256, 0, s>>>(accW, dG, Ut, (bf16*)dWp, (bf16*)dbp, V, Vp, P2, D, h);
+  else fe_finish_dwp_kernel<float><<<grid_for(n, 256), 256, 0, s>>>(accW, dG, Ut, (float*)dWp, (float*)dbp, V, Vp, P2, D, h);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+}  // namespace orbit

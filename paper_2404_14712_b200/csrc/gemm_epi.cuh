@@ -24,6 +24,12 @@ inline Args from_gemm(const GemmArgs& g) {
   return e;
 }
 
+// strided batch (GemmArgs::batch): problem `bi` writes C + bi*c_bs and reads bias + bi*bias_bs (element offsets)
+__device__ __forceinline__ void offset_batch(Args& e, int bi, long long c_bs, long long bias_bs) {
+  e.C = (char*)e.C + (size_t)bi * c_bs * (e.out_dt == ORBIT_BF16 ? 2 : 4);
+  if (e.bias) e.bias = (const char*)e.bias + (size_t)bi * bias_bs * (e.bias_dt == ORBIT_BF16 ? 2 : 4);
+}
+
 __device__ __forceinline__ void load8(const void* p, size_t i, int dt, float* v) {
   if (dt == ORBIT_BF16) {
     uint4 raw = *reinterpret_cast<const uint4*>((const bf16*)p + i);

@@ -9,6 +9,13 @@ namespace {
 constexpr int BM = 64, BN = 64, BK = 16, NT = 256;
 
 __global__ void __launch_bounds__(NT) gemm_simt_kernel(GemmArgs g) {
+  if (g.batch > 1) {   // strided batch: blockIdx.z selects the problem
+    const size_t i = blockIdx.z;
+    g.A = (const char*)g.A + i * g.a_bs * (g.in_dtype == ORBIT_BF16 ? 2 : 4);
+    g.B = (const char*)g.B + i * g.b_bs * (g.in_dtype == ORBIT_BF16 ? 2 : 4);
+    g.C = (char*)g.C + i * g.c_bs * (g.out_dtype == ORBIT_BF16 ? 2 : 4);
+    if (g.bias) g.bias = (const char*)g.bias + i * g.bias_bs * (g.bias_dtype == ORBIT_BF16 ? 2 : 4);
+  }
   __shared__ float As[BK][BM + 4];
   __shared__ float Bs[BK][BN + 4];
   const int t = threadIdx.x;
@@ -90,7 +97,7 @@ __global__ void __launch_bounds__(NT) gemm_simt_kernel(GemmArgs g) {
 
 int gemm_simt(const GemmArgs& g, cudaStream_t s) {
   if (g.M <= 0 || g.N <= 0) return ORBIT_OK;
-  dim3 grid(cdiv(g.N, BN), cdiv(g.M, BM));
+  dim3 grid(cdiv(g.N, BN), cdiv(g.M, BM), g.batch > 1 ? g.batch : 1);
   gemm_simt_kernel<<<grid, NT, 0, s>>>(g);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;

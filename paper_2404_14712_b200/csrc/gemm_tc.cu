@@ -8,53 +8,24 @@
 // the same kernel: only the TMA boxes, the UMMA descriptors' LBO/SBO and the per-k-step advance differ.
 #include <cuda.h>
 #include "common.cuh"
+#include "gemm_epi.cuh"
 #include "ptx.cuh"
 
 namespace orbit {
 namespace {
 
-constexpr int BM = 128, BN = 256, BK = 64, UK = 16;
-constexpr int STAGES = 4;
-constexpr int A_BYTES = BM * BK * 2;            // 16 KB
-constexpr int B_BYTES = BN * BK * 2;            // 32 KB
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 48 KB
+constexpr int BM = 128, BK = 64, UK = 16;
 constexpr int NTHREADS = 192;
-constexpr int TMEM_COLS = 512;                  // two 128x256 fp32 accumulators
-constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
-
-struct Epi {
-  void* C; long long ldc; int out_dt;
-  const void* bias; int bias_dt;
-  const void* resid; int resid_dt; long long ldr; int resid_row_mod;
-  int accumulate; int act;
-  void* aux_out; const void* aux_in; long long ld_aux; int aux_dt;
+constexpr int A_BYTES = BM * BK * 2;            // 16 KB
+// per-BN configuration: BN = 256 (4 stages of 48 KB) for the wide GEMMs, BN = 128 (6 stages of 32 KB) for
+// the d_a-wide per-head products of the front end
+template <int BN> struct TcCfg {
+  static constexpr int B_BYTES = BN * BK * 2;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int STAGES = BN == 256 ? 4 : 6;
+  static constexpr int TMEM_COLS = 2 * BN;      // two 128 x BN fp32 accumulators
+  static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
 };
-
-__device__ __forceinline__ void load8(const void* p, size_t i, int dt, float* v) {
-  if (dt == ORBIT_BF16) {
-    uint4 raw = *reinterpret_cast<const uint4*>((const bf16*)p + i);
-    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&raw);
-#pragma unroll
-    for (int j = 0; j < 4; j++) { float2 f = __bfloat1622float2(h[j]); v[2 * j] = f.x; v[2 * j + 1] = f.y; }
-  } else {
-    const float4* q = reinterpret_cast<const float4*>((const float*)p + i);
-    float4 a = q[0], b = q[1];
-    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-  }
-}
-__device__ __forceinline__ void store8(void* p, size_t i, int dt, const float* v) {
-  if (dt == ORBIT_BF16) {
-    uint4 raw;
-    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&raw);
-#pragma unroll
-    for (int j = 0; j < 4; j++) h[j] = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
-    *reinterpret_cast<uint4*>((bf16*)p + i) = raw;
-  } else {
-    float4* q = reinterpret_cast<float4*>((float*)p + i);
-    q[0] = make_float4(v[0], v[1], v[2], v[3]);
-    q[1] = make_float4(v[4], v[5], v[6], v[7]);
-  }
-}
 
 __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int& mb, int& nb) {
   // groups of 16 M-blocks swept along N: concurrently running CTAs share A and B tiles through L2
@@ -67,9 +38,12 @@ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int
   nb = r / gm;
 }
 
-template <int A_MN, int B_MN>
+template <int A_MN, int B_MN, int BN>
 __global__ void __launch_bounds__(NTHREADS, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, Epi e, int M, int N, int K) {
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, epi::Args e0, int M, int N, int K,
+               int batch, long long c_bs, long long bias_bs) {
+  using Cf = TcCfg<BN>;
+  constexpr int STAGES = Cf::STAGES, STAGE_BYTES = Cf::STAGE_BYTES;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
@@ -82,7 +56,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tiles_m = (M + BM - 1) / BM, tiles_n = (N + BN - 1) / BN;
-  const int num_tiles = tiles_m * tiles_n;
+  const int tiles_per_batch = tiles_m * tiles_n;
+  const int num_tiles = tiles_per_batch * batch;
   const int num_kb = (K + BK - 1) / BK;
 
   if (warp == 0 && lane == 0) {
@@ -93,7 +68,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     ptx::fence_barrier_init();
   }
   if (warp == 1) {
-    ptx::tmem_alloc(tmem_slot, TMEM_COLS);
+    ptx::tmem_alloc(tmem_slot, Cf::TMEM_COLS);
     ptx::tmem_relinquish();
   }
   ptx::tc_fence_before();
@@ -107,8 +82,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
       for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+        const int bi = t / tiles_per_batch;
         int mb, nb;
-        tile_coords(t, tiles_m, tiles_n, mb, nb);
+        tile_coords(t - bi * tiles_per_batch, tiles_m, tiles_n, mb, nb);
         const int m0 = mb * BM, n0 = nb * BN;
         for (int kb = 0; kb < num_kb; kb++) {
           ptx::mbar_wait(empty_bar(s), ph ^ 1);
@@ -117,15 +93,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const int k0 = kb * BK;
           if (A_MN) {  // A stored [K, M], M contiguous: boxes of 64 (M) x 64 (K)
 #pragma unroll
-            for (int i = 0; i < BM / 64; i++) ptx::tma_load_2d(sa + i * 8192, &tmA, full_bar(s), m0 + i * 64, k0);
+            for (int i = 0; i < BM / 64; i++) ptx::tma_load_3d(sa + i * 8192, &tmA, full_bar(s), m0 + i * 64, k0, bi);
           } else {     // A stored [M, K], K contiguous: one box of 64 (K) x 128 (M)
-            ptx::tma_load_2d(sa, &tmA, full_bar(s), k0, m0);
+            ptx::tma_load_3d(sa, &tmA, full_bar(s), k0, m0, bi);
           }
           if (B_MN) {  // B stored [K, N], N contiguous
 #pragma unroll
-            for (int i = 0; i < BN / 64; i++) ptx::tma_load_2d(sb + i * 8192, &tmB, full_bar(s), n0 + i * 64, k0);
-          } else {     // B stored [N, K], K contiguous: one box of 64 (K) x 256 (N)
-            ptx::tma_load_2d(sb, &tmB, full_bar(s), k0, n0);
+            for (int i = 0; i < BN / 64; i++) ptx::tma_load_3d(sb + i * 8192, &tmB, full_bar(s), n0 + i * 64, k0, bi);
+          } else {     // B stored [N, K], K contiguous: one box of 64 (K) x BN (N)
+            ptx::tma_load_3d(sb, &tmB, full_bar(s), k0, n0, bi);
           }
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
@@ -167,10 +143,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int quarter = warp & 3;                 // TMEM lanes [32*quarter, +32) are this warp's
     int acc = 0; uint32_t aph = 0;
     for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+      const int bi = t / tiles_per_batch;
       int mb, nb;
-      tile_coords(t, tiles_m, tiles_n, mb, nb);
+      tile_coords(t - bi * tiles_per_batch, tiles_m, tiles_n, mb, nb);
       const int row = mb * BM + quarter * 32 + lane;
       const int n0 = nb * BN;
+      epi::Args e = e0;
+      if (batch > 1) epi::offset_batch(e, bi, c_bs, bias_bs);
       ptx::mbar_wait(tfull_bar(acc), aph);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + acc * BN + ((uint32_t)(quarter * 32) << 16);
@@ -180,53 +159,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         uint32_t r[32];
         ptx::tmem_ld_32x32(taddr + c * 32, r);
         ptx::tmem_ld_wait();
-        if (row < M) {
-#pragma unroll
-          for (int g8 = 0; g8 < 4; g8++) {
-            const int col = n0 + c * 32 + g8 * 8;
-            if (col < N) {
-              float v[8];
-#pragma unroll
-              for (int j = 0; j < 8; j++) v[j] = __uint_as_float(r[g8 * 8 + j]);
-              if (e.bias) {
-                float b[8];
-                load8(e.bias, col, e.bias_dt, b);
-#pragma unroll
-                for (int j = 0; j < 8; j++) v[j] += b[j];
-              }
-              if (e.act == ACT_GELU) {
-                if (e.aux_out) {
-                  store8(e.aux_out, (size_t)row * e.ld_aux + col, e.aux_dt, v);
-                  if (e.aux_dt == ORBIT_BF16) {
-#pragma unroll
-                    for (int j = 0; j < 8; j++) v[j] = __bfloat162float(__float2bfloat16_rn(v[j]));
-                  }
-                }
-#pragma unroll
-                for (int j = 0; j < 8; j++) v[j] = gelu_f(v[j]);
-              } else if (e.act == ACT_GELU_GRAD) {
-                float u[8];
-                load8(e.aux_in, (size_t)row * e.ld_aux + col, e.aux_dt, u);
-#pragma unroll
-                for (int j = 0; j < 8; j++) v[j] *= gelu_grad_f(u[j]);
-              }
-              if (e.resid) {
-                float q[8];
-                load8(e.resid, (size_t)rrow * e.ldr + col, e.resid_dt, q);
-#pragma unroll
-                for (int j = 0; j < 8; j++) v[j] += q[j];
-              }
-              const size_t ci = (size_t)row * e.ldc + col;
-              if (e.accumulate) {
-                float q[8];
-                load8(e.C, ci, e.out_dt, q);
-#pragma unroll
-                for (int j = 0; j < 8; j++) v[j] += q[j];
-              }
-              store8(e.C, ci, e.out_dt, v);
-            }
-          }
-        }
+        if (row < M) epi::chunk32(e, r, row, rrow, n0 + c * 32, N);
       }
       ptx::tc_fence_before();
       __syncwarp();
@@ -238,7 +171,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   __syncthreads();
   if (warp == 1) {
     ptx::tc_fence_after();
-    ptx::tmem_dealloc(tmem_base, TMEM_COLS);
+    ptx::tmem_dealloc(tmem_base, Cf::TMEM_COLS);
   }
 }
 
@@ -258,21 +191,24 @@ EncodeTiledFn get_encode() {
   return fn;
 }
 
-// 2-D bf16 tensor map: `inner` contiguous elements, `outer` rows `ld` elements apart; 128B swizzle
+// bf16 tensor map over `batch` 2-D problems `bstride` elements apart: `inner` contiguous elements, `outer` rows `ld`
+// elements apart; 128B swizzle; box = box_inner x box_outer x 1 (out-of-bounds elements read as zero per problem)
 int make_map(CUtensorMap* m, const void* base, long long inner, long long outer, long long ld, int box_inner,
-             int box_outer) {
+             int box_outer, int batch, long long bstride) {
   EncodeTiledFn enc = get_encode();
   if (!enc) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
-  cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
-  cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
-  cuuint32_t box[2] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer};
-  cuuint32_t es[2] = {1, 1};
-  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, es,
+  if (batch <= 1) { batch = 1; bstride = ld * outer; }
+  cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)outer, (cuuint64_t)batch};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * 2, (cuuint64_t)bstride * 2};
+  if (batch == 1) strides[1] = strides[0] * dims[1];
+  cuuint32_t box[3] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer, 1};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
-    set_error("cuTensorMapEncodeTiled failed (%d): inner=%lld outer=%lld ld=%lld box=%dx%d", (int)r, inner, outer, ld,
-              box_inner, box_outer);
+    set_error("cuTensorMapEncodeTiled failed (%d): inner=%lld outer=%lld ld=%lld box=%dx%d batch=%d bstride=%lld", (int)r,
+              inner, outer, ld, box_inner, box_outer, batch, bstride);
     return ORBIT_ERR_CUDA;
   }
   return ORBIT_OK;
@@ -299,18 +235,28 @@ struct Prof {
 };
 Prof g_prof;
 
-template <int A_MN, int B_MN>
-int launch(const CUtensorMap& ma, const CUtensorMap& mb, const Epi& e, int M, int N, int K, cudaStream_t s) {
+template <int A_MN, int B_MN, int BN>
+int launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, cudaStream_t s) {
+  using Cf = TcCfg<BN>;
   static bool attr_set = false;
   if (!attr_set) {
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)gemm_tc_kernel<A_MN, B_MN>,
-                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)gemm_tc_kernel<A_MN, B_MN, BN>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cf::SMEM_BYTES));
     attr_set = true;
   }
-  const int tiles = cdiv(M, BM) * cdiv(N, BN);
-  const int grid = tiles < num_sms() ? tiles : num_sms();
-  gemm_tc_kernel<A_MN, B_MN><<<grid, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K);
+  const int batch = g.batch > 1 ? g.batch : 1;
+  const long long tiles = (long long)cdiv(g.M, BM) * cdiv(g.N, BN) * batch;
+  const int grid = tiles < num_sms() ? (int)tiles : num_sms();
+  gemm_tc_kernel<A_MN, B_MN, BN><<<grid, NTHREADS, Cf::SMEM_BYTES, s>>>(ma, mb, epi::from_gemm(g), g.M, g.N, g.K, batch,
+                                                                       g.c_bs, g.bias_bs);
   return ORBIT_OK;
+}
+template <int BN>
+int launch_bn(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, bool a_mn, bool b_mn, cudaStream_t s) {
+  if (!a_mn && b_mn) return launch<0, 1, BN>(ma, mb, g, s);
+  if (!a_mn && !b_mn) return launch<0, 0, BN>(ma, mb, g, s);
+  if (a_mn && b_mn) return launch<1, 1, BN>(ma, mb, g, s);
+  return launch<1, 0, BN>(ma, mb, g, s);
 }
 }  // namespace
 
@@ -355,6 +301,10 @@ bool gemm_tc_supported(const GemmArgs& g) {
   if (g.resid && (!al16(g.resid) || g.ldr % 8)) return false;
   if ((g.aux_out && (!al16(g.aux_out) || g.ld_aux % 8)) || (g.aux_in && (!al16(g.aux_in) || g.ld_aux % 8))) return false;
   if (g.accumulate && g.out_dtype != ORBIT_F32) return false;
+  if (g.batch > 1) {
+    if (g.resid || g.aux_out || g.aux_in || g.accumulate) return false;
+    if ((g.a_bs % 8) || (g.b_bs % 8) || (g.c_bs % 8) || (g.bias && (g.bias_bs % 8))) return false;
+  }
   return true;
 }
 
@@ -362,31 +312,22 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   const bool a_mn = !(g.a_cs == 1 && g.a_rs % 8 == 0);
   const bool b_mn = (g.b_cs == 1 && g.b_rs % 8 == 0);
   // CTA-pair kernel (256 x 256 tiles) when the problem has at least one full pair tile; g_force_simt == 2
-  // forces the single-CTA kernel (debug / A-B comparison)
+  // forces the single-CTA kernel (debug / A-B comparison).  Narrow outputs (N <= 128) use 128 x 128 tiles.
   const bool pair = g_force_simt != 2 && g.M >= 256 && g.N >= 256;
+  const int bn = pair ? 128 : (g.N <= 128 ? 128 : 256);   // rows of a K-major B box
   CUtensorMap ma, mb;
-  if (a_mn) ORBIT_TRY(make_map(&ma, g.A, g.M, g.K, g.a_cs, 64, 64));               // [K rows, M contiguous]
-  else      ORBIT_TRY(make_map(&ma, g.A, g.K, g.M, g.a_rs, 64, BM));               // [M rows, K contiguous]
-  if (b_mn) ORBIT_TRY(make_map(&mb, g.B, g.N, g.K, g.b_rs, 64, 64));               // [K rows, N contiguous]
-  else      ORBIT_TRY(make_map(&mb, g.B, g.K, g.N, g.b_cs, 64, pair ? 128 : BN));  // [N rows, K contiguous]
+  if (a_mn) ORBIT_TRY(make_map(&ma, g.A, g.M, g.K, g.a_cs, 64, 64, g.batch, g.a_bs));   // [K rows, M contiguous]
+  else      ORBIT_TRY(make_map(&ma, g.A, g.K, g.M, g.a_rs, 64, BM, g.batch, g.a_bs));   // [M rows, K contiguous]
+  if (b_mn) ORBIT_TRY(make_map(&mb, g.B, g.N, g.K, g.b_rs, 64, 64, g.batch, g.b_bs));   // [K rows, N contiguous]
+  else      ORBIT_TRY(make_map(&mb, g.B, g.K, g.N, g.b_cs, 64, bn, g.batch, g.b_bs));   // [N rows, K contiguous]
   const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
   if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
-  if (pair) {
-    ORBIT_TRY(gemm_tc2_launch(ma, mb, g, a_mn, b_mn, num_sms(), s));
-  } else {
-    Epi e;
-    e.C = g.C; e.ldc = g.ldc; e.out_dt = g.out_dtype; e.bias = g.bias; e.bias_dt = g.bias_dtype;
-    e.resid = g.resid; e.resid_dt = g.resid_dtype; e.ldr = g.ldr; e.resid_row_mod = g.resid_row_mod;
-    e.accumulate = g.accumulate; e.act = g.act; e.aux_out = g.aux_out; e.aux_in = g.aux_in; e.ld_aux = g.ld_aux;
-    e.aux_dt = g.aux_dtype;
-    if (!a_mn && b_mn) ORBIT_TRY((launch<0, 1>(ma, mb, e, g.M, g.N, g.K, s)));
-    else if (!a_mn && !b_mn) ORBIT_TRY((launch<0, 0>(ma, mb, e, g.M, g.N, g.K, s)));
-    else if (a_mn && b_mn) ORBIT_TRY((launch<1, 1>(ma, mb, e, g.M, g.N, g.K, s)));
-    else ORBIT_TRY((launch<1, 0>(ma, mb, e, g.M, g.N, g.K, s)));
-  }
+  if (pair) ORBIT_TRY(gemm_tc2_launch(ma, mb, g, a_mn, b_mn, num_sms(), s));
+  else if (bn == 128) ORBIT_TRY(launch_bn<128>(ma, mb, g, a_mn, b_mn, s));
+  else ORBIT_TRY(launch_bn<256>(ma, mb, g, a_mn, b_mn, s));
   if (rec) {
     ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n + 1], s));
-    g_prof.flops[g_prof.n++] = 2.0 * g.M * g.N * g.K;
+    g_prof.flops[g_prof.n++] = 2.0 * g.M * g.N * g.K * (g.batch > 1 ? g.batch : 1);
   }
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;

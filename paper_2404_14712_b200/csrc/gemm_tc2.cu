@@ -38,7 +38,8 @@ __device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, in
 
 template <int A_MN, int B_MN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
-gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, epi::Args e, int M, int N, int K) {
+gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, epi::Args e0, int M, int N, int K,
+                int batch, long long c_bs, long long bias_bs) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
@@ -52,7 +53,8 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const uint32_t rank = ptx::cluster_ctarank();
   const bool leader = rank == 0;
   const int tiles_m = (M + BM2 - 1) / BM2, tiles_n = (N + BN2 - 1) / BN2;
-  const int num_tiles = tiles_m * tiles_n;
+  const int tiles_per_batch = tiles_m * tiles_n;
+  const int num_tiles = tiles_per_batch * batch;
   const int num_kb = (K + BK - 1) / BK;
   const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
 
@@ -78,8 +80,9 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
       for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+        const int bi = t / tiles_per_batch;
         int mb, nb;
-        tile_coords2(t, tiles_m, tiles_n, mb, nb);
+        tile_coords2(t - bi * tiles_per_batch, tiles_m, tiles_n, mb, nb);
         const int m0 = mb * BM2 + (int)rank * 128, n0 = nb * BN2 + (int)rank * 128;
         for (int kb = 0; kb < num_kb; kb++) {
           ptx::mbar_wait(empty_bar(s), ph ^ 1);
@@ -89,15 +92,15 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           const int k0 = kb * BK;
           if (A_MN) {
 #pragma unroll
-            for (int i = 0; i < 2; i++) ptx::tma_load_2d_2sm(sa + i * 8192, &tmA, lfull, m0 + i * 64, k0);
+            for (int i = 0; i < 2; i++) ptx::tma_load_3d_2sm(sa + i * 8192, &tmA, lfull, m0 + i * 64, k0, bi);
           } else {
-            ptx::tma_load_2d_2sm(sa, &tmA, lfull, k0, m0);
+            ptx::tma_load_3d_2sm(sa, &tmA, lfull, k0, m0, bi);
           }
           if (B_MN) {
 #pragma unroll
-            for (int i = 0; i < 2; i++) ptx::tma_load_2d_2sm(sb + i * 8192, &tmB, lfull, n0 + i * 64, k0);
+            for (int i = 0; i < 2; i++) ptx::tma_load_3d_2sm(sb + i * 8192, &tmB, lfull, n0 + i * 64, k0, bi);
           } else {
-            ptx::tma_load_2d_2sm(sb, &tmB, lfull, k0, n0);
+            ptx::tma_load_3d_2sm(sb, &tmB, lfull, k0, n0, bi);
           }
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
@@ -138,8 +141,11 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int chalf = (warp - 2) >> 2;           // which 128 of the 256 accumulator columns
     int acc = 0; uint32_t aph = 0;
     for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+      const int bi = t / tiles_per_batch;
       int mb, nb;
-      tile_coords2(t, tiles_m, tiles_n, mb, nb);
+      tile_coords2(t - bi * tiles_per_batch, tiles_m, tiles_n, mb, nb);
+      epi::Args e = e0;
+      if (batch > 1) epi::offset_batch(e, bi, c_bs, bias_bs);
       const int row = mb * BM2 + (int)rank * 128 + quarter * 32 + lane;
       const int n0 = nb * BN2;
       ptx::mbar_wait(tfull_bar(acc), aph);
@@ -168,17 +174,19 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 }
 
 template <int A_MN, int B_MN>
-int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const epi::Args& e, int M, int N, int K, int sms, cudaStream_t s) {
+int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, int sms, cudaStream_t s) {
+  const epi::Args e = epi::from_gemm(g);
+  const int M = g.M, N = g.N, K = g.K, batch = g.batch > 1 ? g.batch : 1;
   static bool attr_set = false;
   if (!attr_set) {
     ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)gemm_tc2_kernel<A_MN, B_MN>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
     attr_set = true;
   }
-  const int tiles = cdiv(M, BM2) * cdiv(N, BN2);
+  const long long tiles = (long long)cdiv(M, BM2) * cdiv(N, BN2) * batch;
   int clusters = sms / 2;
-  if (tiles < clusters) clusters = tiles;
-  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K);
+  if (tiles < clusters) clusters = (int)tiles;
+  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K, batch, g.c_bs, g.bias_bs);
   return ORBIT_OK;
 }
 }  // namespace
@@ -187,11 +195,10 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const epi::Args& e, in
 // 128 rows (K-major) or 64 x 64 (N-major)
 int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, bool a_mn, bool b_mn, int sms,
                     cudaStream_t s) {
-  const epi::Args e = epi::from_gemm(g);
-  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, e, g.M, g.N, g.K, sms, s);
-  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, e, g.M, g.N, g.K, sms, s);
-  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, e, g.M, g.N, g.K, sms, s);
-  return launch2<1, 0>(ma, mb, e, g.M, g.N, g.K, sms, s);
+  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, g, sms, s);
+  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, g, sms, s);
+  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, g, sms, s);
+  return launch2<1, 0>(ma, mb, g, sms, s);
 }
 
 }  // namespace orbit

@@ -106,14 +106,44 @@ class FrontRunner:
         return self.fwd(x)
 
 
+class FusedFrontRunner:
+    """orbit_embed_fused and its backward: tokenise + aggregate in pixel space, tok never materialised."""
+
+    def __init__(self, B, V, Hg, Wg, p, D, heads, dtype, resid_dtype, emb: dict, agg: dict, pos=None, device="cuda"):
+        self.L = (Hg // p) * (Wg // p)
+        self.fd = ob.front_desc(B, V, Hg, Wg, p, D, heads, dtype, resid_dtype)
+        self.dtype, self.resid_dtype, self.device = dtype, resid_dtype, device
+        self.Wp, self.bp = to_dev(emb["Wp"], dtype, device), to_dev(emb["bp"], dtype, device)
+        self.agg = {k: to_dev(agg[k], dtype, device) for k in ob._AGG_NAMES}
+        self.pos = None if pos is None else to_dev(pos, resid_dtype, device)
+        self.out = torch.empty(B, self.L, D, dtype=TD[resid_dtype], device=device)
+        self.saved = _bytes(ob.orbit_embed_fused_saved_bytes(self.fd), device)
+        self.ws_f = _bytes(ob.orbit_embed_fused_workspace_bytes(self.fd), device)
+        self.ws_b = None
+        self.gagg = {k: torch.empty_like(v) for k, v in self.agg.items()}
+        self.dpos = None if pos is None else torch.empty_like(self.pos)
+        self.dWp, self.dbp = torch.empty_like(self.Wp), torch.empty_like(self.bp)
+
+    def fwd_keep(self, x):
+        self.x_last = x
+        ob.orbit_embed_fused(self.fd, x, self.Wp, self.bp, self.agg, self.pos, self.out, self.saved, self.ws_f)
+        return self.out
+
+    def bwd(self, dagg):
+        if self.ws_b is None:
+            self.ws_b = _bytes(ob.orbit_embed_fused_bwd_workspace_bytes(self.fd), self.device)
+        ob.orbit_embed_fused_bwd(self.fd, self.x_last, self.Wp, self.bp, self.agg, dagg, self.saved, self.dWp, self.dbp,
+                                 self.gagg, self.dpos, self.ws_b)
+
+
 class StepRunner:
     """Whole hot path for a Config: tokenise -> aggregate -> depth x block, forward + backward, MSE loss."""
 
-    def __init__(self, cfg: Config, emb=None, agg=None, blocks=None, pos=None, device="cuda"):
+    def __init__(self, cfg: Config, emb=None, agg=None, blocks=None, pos=None, device="cuda", fused_front=False):
         self.cfg = cfg
         self.front = None
         if cfg.V is not None:
-            self.front = FrontRunner(cfg.B, cfg.V, cfg.Hg, cfg.Wg, cfg.p, cfg.D, cfg.heads, cfg.dtype, cfg.resid_dtype,
+            self.front = (FusedFrontRunner if fused_front else FrontRunner)(cfg.B, cfg.V, cfg.Hg, cfg.Wg, cfg.p, cfg.D, cfg.heads, cfg.dtype, cfg.resid_dtype,
                                      emb, agg, pos, device)
         self.blocks = []
         ws = None

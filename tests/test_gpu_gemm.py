@@ -62,3 +62,29 @@ def test_gemm_fp32_fma(ob, a_major, b_major):
     assert err < 1e-5
     err = run_gemm(ob, 200, 264, 136, a_major, b_major, "bf16", simt=True)
     assert err < 1e-5
+
+
+@pytest.mark.parametrize("case", [
+    # (M, N, K, batch): the three per-head products of the front end (N = d_a = 128; ragged M / K tails)
+    (1000, 128, 1632, 4), (1632, 128, 520, 3), (520, 1632, 128, 5), (300, 64, 72, 2), (512, 512, 256, 3),
+])
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_gemm_strided_batch(ob, case, dtype):
+    """Strided-batch GEMM (3-D TMA maps, batch folded into the persistent tile loop) against float64 per problem:
+    A_i = columns [i*K, (i+1)*K) of one [M, batch*K] matrix, B_i / C_i = column blocks of [K, batch*N] / [M, batch*N]."""
+    M, N, K, nb = case
+    rng = np.random.default_rng(5)
+    tdt = torch.bfloat16 if dtype == "bf16" else torch.float32
+    A = torch.from_numpy(rng.standard_normal((M, nb * K)).astype(np.float32)).to(tdt)
+    B = torch.from_numpy(rng.standard_normal((K, nb * N)).astype(np.float32)).to(tdt)
+    Ad, Bd = A.cuda().contiguous(), B.cuda().contiguous()
+    C = torch.full((M, nb * N), float("nan"), device="cuda", dtype=torch.float32)
+    ob.orbit_debug_gemm_batched(M, N, K, nb, dtype, Ad, nb * K, 1, K, Bd, nb * N, 1, N, C, nb * N, N)
+    torch.cuda.synchronize()
+    got = C.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    A64, B64 = A.to(torch.float64).numpy(), B.to(torch.float64).numpy()
+    for i in range(nb):
+        ref = A64[:, i * K:(i + 1) * K] @ B64[:, i * N:(i + 1) * N]
+        err = np.linalg.norm(got[:, i * N:(i + 1) * N] - ref) / np.linalg.norm(ref)
+        assert err < 1e-4, f"{case} {dtype} batch {i}: rel err {err:.3e}"

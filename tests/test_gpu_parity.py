@@ -144,16 +144,20 @@ def make_step_case(cfg, seed, depth=None):
     return emb, agg, blocks, x, tgt, pos
 
 
-def run_and_compare_step(rn, cfg, seed, tol, with_pos=True):
+def run_and_compare_step(rn, cfg, seed, tol, with_pos=True, fused=False):
+    """fused=True runs the front end through orbit_embed_fused(_bwd) (pixel-space form, no tok / dtok); its
+    outputs are held to the same oracle (tokenize -> var_aggregate and their backward)."""
     emb, agg, blocks, x, tgt, pos = make_step_case(cfg, seed)
     if not with_pos:
         pos = None
-    sr = rn.StepRunner(cfg, emb, agg, [(P, syn.shard_block_params(P, cfg.heads, 1)) for P in blocks], pos)
+    sr = rn.StepRunner(cfg, emb, agg, [(P, syn.shard_block_params(P, cfg.heads, 1)) for P in blocks], pos,
+                       fused_front=fused)
     loss = sr.step(rn.to_dev(x, "f32"), rn.to_dev(tgt, cfg.resid_dtype))
     torch.cuda.synchronize()
     out = orc.step(x, emb, agg, blocks, tgt, cfg.p, cfg.heads, cfg.ln_eps, pos)
     errs = {}
-    errs["tok"] = check("tok", sr.front.tok, out["tok"], tol)
+    if not fused:
+        errs["tok"] = check("tok", sr.front.tok, out["tok"], tol)
     errs["agg"] = check("agg", sr.front.out, out["agg"], tol)
     errs["y"] = check("y", sr.blocks[-1].y, out["y"], tol)
     assert abs(float(loss.item()) - out["loss"]) <= 5 * tol * abs(out["loss"])
@@ -164,7 +168,8 @@ def run_and_compare_step(rn, cfg, seed, tol, with_pos=True):
         for k in br.SHARD:
             errs[f"b{i}.{k}"] = check(f"b{i}.d{k}", br.gshards[0][k], G[k], tol)
     errs["dagg"] = check("dagg", sr.blocks[0].dx, out["dagg"], tol)
-    errs["dtok"] = check("dtok", sr.front.dtok, out["dtok"], tol)
+    if not fused:
+        errs["dtok"] = check("dtok", sr.front.dtok, out["dtok"], tol)
     for k, g in out["agg_grads"].items():
         if k == "bk":   # analytically zero: compare absolutely against the scale of its siblings
             got = rn.to_np(sr.front.gagg[k])
@@ -197,6 +202,54 @@ def test_front_end_v91_ragged(rn):
     cfg = syn.Config("S3", B=1, V=91, Hg=16, Wg=24, p=4, D=128, heads=16, F=256, depth=1, dtype="bf16",
                      resid_dtype="bf16")
     run_and_compare_step(rn, cfg, 43, 1e-2, with_pos=False)
+
+
+def test_c1_full_step_fp32_fused_front(rn):
+    """C1 with the pixel-space fused front end (orbit_embed_fused), fp32: <= 1e-4 against the two-step oracle."""
+    errs = run_and_compare_step(rn, syn.CONFIGS["C1"], syn.seed_of("C1"), 1e-4, fused=True)
+    print("C1 fused max err", max(errs.values()))
+
+
+@pytest.mark.parametrize("with_pos", [True, False])
+def test_small_bf16_full_step_fused_front(rn, with_pos):
+    cfg = syn.Config("S2", B=2, V=7, Hg=16, Wg=32, p=2, D=256, heads=4, F=1024, depth=2, dtype="bf16",
+                     resid_dtype="f32")
+    errs = run_and_compare_step(rn, cfg, 42, 1e-2, with_pos=with_pos, fused=True)
+    print("S2 fused errs", {k: f"{v:.2e}" for k, v in errs.items()})
+
+
+@pytest.mark.parametrize("case", [
+    dict(B=1, V=91, Hg=16, Wg=24, p=4, D=128, heads=16, rd="bf16"),     # V odd and > 64 (two variable pairs per lane)
+    dict(B=3, V=48, Hg=12, Wg=20, p=2, D=256, heads=16, rd="bf16"),     # C2-like V, ragged patch count (BL = 180)
+    dict(B=2, V=5, Hg=6, Wg=10, p=1, D=64, heads=8, rd="f32"),          # patch 1, tiny
+    dict(B=1, V=128, Hg=8, Wg=8, p=4, D=128, heads=2, rd="f32"),        # V at the limit
+])
+def test_front_end_fused_shapes(rn, case):
+    cfg = syn.Config("SF", B=case["B"], V=case["V"], Hg=case["Hg"], Wg=case["Wg"], p=case["p"], D=case["D"],
+                     heads=case["heads"], F=2 * case["D"], depth=1, dtype="bf16", resid_dtype=case["rd"])
+    errs = run_and_compare_step(rn, cfg, 44, 1e-2, with_pos=False, fused=True)
+    print("fused front", case, {k: f"{v:.2e}" for k, v in errs.items() if not k.startswith("b0")})
+
+
+def test_front_end_fused_fp32_shapes(rn):
+    """fp32 storage (SIMT GEMMs, strided batch over heads) on an odd shape: <= 1e-4."""
+    cfg = syn.Config("SF32", B=2, V=9, Hg=8, Wg=12, p=2, D=64, heads=4, F=128, depth=1, dtype="f32", resid_dtype="f32")
+    run_and_compare_step(rn, cfg, 45, 1e-4, fused=True)
+
+
+def test_fused_front_error_codes(ob, rn):
+    cfg = syn.Config("SE", B=1, V=4, Hg=8, Wg=8, p=2, D=64, heads=4, F=128, depth=1, dtype="bf16", resid_dtype="bf16")
+    emb, agg, blocks, x, tgt, pos = make_step_case(cfg, 3)
+    fr = rn.FusedFrontRunner(1, 4, 8, 8, 2, 64, 4, "bf16", "bf16", emb, agg)
+    fr.fd.V = 129                                    # above the V <= 128 limit
+    with pytest.raises(ob.OrbitError) as e:
+        fr.fwd_keep(rn.to_dev(x, "f32"))
+    assert e.value.status == 2                      # ORBIT_ERR_SHAPE
+    fr.fd.V = 4
+    fr.fd.p = 3                                      # Hg % p != 0 and unsupported patch size
+    with pytest.raises(ob.OrbitError) as e:
+        fr.fwd_keep(rn.to_dev(x, "f32"))
+    assert e.value.status == 2
 
 
 # ---------------------------------------------------------------------------------------------------------

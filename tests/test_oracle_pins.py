@@ -380,6 +380,58 @@ def test_aggregate_closed_forms():
     assert orc.rel_fro(o @ P["Wo"] + P["bo"], agg) < 1e-13
 
 
+def test_pixel_space_fused_form_equals_definition():
+    """The pixel-space form behind orbit_embed_fused restated here in
+    numpy -- G = Wpb Ut, H = Wpb Wv, A_a = alpha_a * pixext, o_a = A_a H_a + bv_a, and the backward chain
+    dH, dA, ds, dG, dWpb = dH Wv^T + dG Ut^T -- equals tokenize -> var_aggregate (the definition) and its
+    backward to ~1e-13, so a CUDA path built on it is held to the same oracle."""
+    B, V, Hg, Wg, p, D, h = 2, 5, 4, 6, 2, 8, 2
+    P2, R, da = p * p, p * p + 1, D // h
+    x = rnd(B, V, Hg, Wg)
+    Wp, bp = rnd(V, P2, D) * 0.5, 0.1 * rnd(V, D)
+    P = rand_agg_params(D)
+    tok = orc.tokenize(x, Wp, bp, p)
+    agg, cache = orc.var_aggregate(tok, P, h)
+    dagg = rnd(*agg.shape)
+    dtok, Gd, _ = orc.var_aggregate_bwd(dagg, P, cache)
+    dWp, dbp = orc.tokenize_bwd(x, dtok, p)
+    # ---- fused form ----
+    L = (Hg // p) * (Wg // p)
+    pix = orc.patches(x, p).transpose(0, 2, 1, 3).reshape(B * L, V, P2)          # [BL, V, p^2]
+    pixext = np.concatenate([pix, np.ones((B * L, V, 1))], axis=2)               # [BL, V, R]
+    Wpb = np.concatenate([Wp, bp[:, None, :]], axis=1)                           # [V, R, D]
+    qt = P["q"] @ P["Wq"] + P["bq"]
+    Ut = np.stack([P["Wk"][:, a * da:(a + 1) * da] @ qt[a * da:(a + 1) * da] / math.sqrt(da) for a in range(h)], axis=1)
+    Gm = np.einsum("vrd,da->vra", Wpb, Ut)
+    H = np.einsum("vrd,dc->vrc", Wpb, P["Wv"])
+    s = np.einsum("nvr,vra->nav", pixext, Gm)
+    alpha = orc.softmax_lastdim(s)                                               # [BL, h, V]
+    assert np.allclose(alpha.reshape(B, L, h, V), cache["alpha"], atol=1e-13)
+    A = np.einsum("nav,nvr->navr", alpha, pixext)                                # [BL, h, V, R]
+    o = np.concatenate([np.einsum("nvr,vrc->nc", A[:, a], H[:, :, a * da:(a + 1) * da]) for a in range(h)], axis=1) + P["bv"]
+    agg2 = (o @ P["Wo"] + P["bo"]).reshape(B, L, D)
+    assert orc.rel_fro(agg2, agg) < 1e-13
+    # ---- backward ----
+    g2 = dagg.reshape(B * L, D)
+    do = g2 @ P["Wo"].T
+    dH = np.zeros_like(H)
+    dA = np.zeros_like(A)
+    for a in range(h):
+        c = slice(a * da, (a + 1) * da)
+        dH[:, :, c] = np.einsum("nvr,nc->vrc", A[:, a], do[:, c])
+        dA[:, a] = np.einsum("nc,vrc->nvr", do[:, c], H[:, :, c])
+    dalpha = np.einsum("navr,nvr->nav", dA, pixext)
+    ds = alpha * (dalpha - (alpha * dalpha).sum(-1, keepdims=True))
+    dG = np.einsum("nav,nvr->vra", ds, pixext)
+    dWpb = np.einsum("vrc,dc->vrd", dH, P["Wv"]) + np.einsum("vra,da->vrd", dG, Ut)
+    assert orc.rel_fro(dWpb[:, :P2], dWp) < 1e-12 and orc.rel_fro(dWpb[:, P2], dbp) < 1e-12
+    assert orc.rel_fro(np.einsum("vrd,vrc->dc", Wpb, dH), Gd["Wv"]) < 1e-12
+    dUt = np.einsum("vrd,vra->da", Wpb, dG)
+    dWk = np.concatenate([np.outer(dUt[:, a], qt[a * da:(a + 1) * da]) / math.sqrt(da) for a in range(h)], axis=1)
+    assert orc.rel_fro(dWk, Gd["Wk"]) < 1e-12
+    assert orc.rel_fro(do.sum(0), Gd["bv"]) < 1e-12
+
+
 # ------------------------------------------------------------------ whole step -----------------
 def test_whole_step_fd_through_everything():
     B, V, Hg, Wg, p, D, h, F = 1, 3, 8, 8, 2, 8, 2, 16     # SURVEY.md §8(c): "B1 V3 8x8 p2 D8 h2 F16"

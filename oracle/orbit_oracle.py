@@ -14,7 +14,9 @@ Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): central finite diff
 fwd/bwd pair; softmax rows sum to 1 / shift invariance; LayerNorm zero-mean unit-variance; attention
 over identical keys = mean of values; Eq. (2)/(3) shard sums = unsharded product; tokeniser = strided
 convolution (torch conv2d, float64); whole block fwd+bwd = torch float64 autograd of textbook ops;
-aggregation V=1 closed form, permutation invariance, dbk == 0, dbv == sum(do).
+aggregation V=1 closed form, permutation invariance, dbk == 0, dbv == sum(do); QK-LayerNorm: torch
+float64 autograd with F.layer_norm on the per-head q / k, finite differences, logits bounded by
+sqrt(d_h) for gamma = 1, beta = 0, invariance to rescaling the pre-norm queries (eps = 0).
 Parity unpinned: none.
 
 Layout conventions (same as include/orbit.h): row-major, weights [in, out] so y = x A exactly as in
@@ -250,14 +252,45 @@ def attention_bwd(dO, Q, K, V, Pm, heads):
     return dQ, dK, dV
 
 
+def qk_layernorm(Z, heads, gamma, beta, eps):
+    """QK-LayerNorm ("additional layer normalization to the queries ... and keys ... before
+    computing the self-attention scaled dot product", after [8]; reading 9): LayerNorm over the d_h entries
+    of every head's query (resp. key) vector, gamma / beta in R^{d_h} shared by all heads.
+    Z: [B, N, heads*d_h] -> (normalised [B, N, heads*d_h], zhat [B, N, heads, d_h], rstd)."""
+    B, N, Dz = Z.shape
+    dh = Dz // heads
+    out, zhat, rstd = layernorm(Z.reshape(B, N, heads, dh), gamma, beta, eps)
+    return out.reshape(B, N, Dz), zhat, rstd
+
+
+def qk_layernorm_bwd(dZn, heads, zhat, rstd, gamma):
+    """Backward of qk_layernorm: (dZ [B, N, heads*d_h], dgamma [d_h], dbeta [d_h]) -- gamma / beta gradients
+    sum over tokens AND heads (the parameters are shared by the heads)."""
+    B, N, Dz = dZn.shape
+    dh = Dz // heads
+    dz, dgamma, dbeta = layernorm_bwd(_f64(dZn).reshape(B, N, heads, dh), zhat, rstd, gamma)
+    return dz.reshape(B, N, Dz), dgamma, dbeta
+
+
+def has_qk_norm(P):
+    """A block uses QK-LayerNorm iff its parameter dict carries qn_g, qn_b, kn_g, kn_b (all [d_h])."""
+    return "qn_g" in P
+
+
 def block_fwd(x, P, heads, eps=1e-5):
-    """a = LN1(x); [Q|K|V] = a Wqkv + bqkv; O = attention; x1 = x + O Wproj + bproj;
+    """a = LN1(x); [Q|K|V] = a Wqkv + bqkv; (Q, K <- QK-LayerNorm per head when P has qn_g.. : PAPER.md:114);
+    O = attention; x1 = x + O Wproj + bproj;
     m = LN2(x1); u = m Wfc1 + bfc1; g = GELU(u); y = x1 + g Wfc2 + bfc2.    x: [B, N, D]."""
     x = _f64(x)
     B, N, D = x.shape
     a, xhat, rstd1 = layernorm(x, P["ln1_g"], P["ln1_b"], eps)
     qkv = a @ _f64(P["Wqkv"]) + _f64(P["bqkv"])
     Q, K, V = qkv[..., 0:D], qkv[..., D:2 * D], qkv[..., 2 * D:3 * D]
+    qkn = None
+    if has_qk_norm(P):
+        Q, qhat, qrstd = qk_layernorm(Q, heads, P["qn_g"], P["qn_b"], eps)
+        K, khat, krstd = qk_layernorm(K, heads, P["kn_g"], P["kn_b"], eps)
+        qkn = dict(qhat=qhat, qrstd=qrstd, khat=khat, krstd=krstd)
     O, Pm = attention(Q, K, V, heads)
     x1 = x + O @ _f64(P["Wproj"]) + _f64(P["bproj"])
     m, x1hat, rstd2 = layernorm(x1, P["ln2_g"], P["ln2_b"], eps)
@@ -265,7 +298,7 @@ def block_fwd(x, P, heads, eps=1e-5):
     g = gelu(u)
     y = x1 + g @ _f64(P["Wfc2"]) + _f64(P["bfc2"])
     cache = dict(xhat=xhat, rstd1=rstd1, a=a, Q=Q, K=K, V=V, Pm=Pm, O=O, x1=x1, x1hat=x1hat,
-                 rstd2=rstd2, m=m, u=u, g=g, heads=heads)
+                 rstd2=rstd2, m=m, u=u, g=g, heads=heads, qkn=qkn)
     return y, cache
 
 
@@ -294,6 +327,10 @@ def block_bwd(dy, P, cache):
     G["Wproj"] = c["O"].reshape(M, D).T @ dx12
     dO = dx1 @ _f64(P["Wproj"]).T
     dQ, dK, dV = attention_bwd(dO, c["Q"], c["K"], c["V"], c["Pm"], heads)
+    if c.get("qkn") is not None:
+        n = c["qkn"]
+        dQ, G["qn_g"], G["qn_b"] = qk_layernorm_bwd(dQ, heads, n["qhat"], n["qrstd"], P["qn_g"])
+        dK, G["kn_g"], G["kn_b"] = qk_layernorm_bwd(dK, heads, n["khat"], n["krstd"], P["kn_g"])
     dqkv = np.concatenate([dQ, dK, dV], axis=-1)
     dqkv2 = dqkv.reshape(M, 3 * D)
     G["bqkv"] = dqkv2.sum(axis=0)
@@ -345,9 +382,14 @@ def block_fwd_sharded(x, Pc, shards, heads, eps=1e-5):
     for S in shards:
         qkv = a @ _f64(S["Wqkv"]) + _f64(S["bqkv"])
         Q, K, V = qkv[..., 0:dc], qkv[..., dc:2 * dc], qkv[..., 2 * dc:3 * dc]
+        qkn = None
+        if has_qk_norm(Pc):          # gamma / beta in R^{d_h} are shared by the heads, hence by the shards
+            Q, qhat, qrstd = qk_layernorm(Q, hk, Pc["qn_g"], Pc["qn_b"], eps)
+            K, khat, krstd = qk_layernorm(K, hk, Pc["kn_g"], Pc["kn_b"], eps)
+            qkn = dict(qhat=qhat, qrstd=qrstd, khat=khat, krstd=krstd)
         O, Pm = attention(Q, K, V, hk)
         acc = acc + O @ _f64(S["Wproj"])
-        per.append(dict(Q=Q, K=K, V=V, Pm=Pm, O=O))
+        per.append(dict(Q=Q, K=K, V=V, Pm=Pm, O=O, qkn=qkn))
     x1 = x + acc + _f64(Pc["bproj"])
     m, x1hat, rstd2 = layernorm(x1, Pc["ln2_g"], Pc["ln2_b"], eps)
     acc2 = np.zeros_like(x)
@@ -393,6 +435,12 @@ def block_bwd_sharded(dy, Pc, shards, cache):
         G["Wproj"] = c["O"].reshape(M, dc).T @ dx12
         dO = dx1 @ _f64(S["Wproj"]).T
         dQ, dK, dV = attention_bwd(dO, c["Q"], c["K"], c["V"], c["Pm"], hk)
+        if c.get("qkn") is not None:
+            n = c["qkn"]
+            dQ, gqg, gqb = qk_layernorm_bwd(dQ, hk, n["qhat"], n["qrstd"], Pc["qn_g"])
+            dK, gkg, gkb = qk_layernorm_bwd(dK, hk, n["khat"], n["krstd"], Pc["kn_g"])
+            for name, g in (("qn_g", gqg), ("qn_b", gqb), ("kn_g", gkg), ("kn_b", gkb)):
+                Gc[name] = Gc.get(name, 0.0) + g          # shared parameters: sum over the shards
         dqkv = np.concatenate([dQ, dK, dV], axis=-1)
         G["bqkv"] = dqkv.reshape(M, 3 * dc).sum(axis=0)
         G["Wqkv"] = cache["a"].reshape(M, D).T @ dqkv.reshape(M, 3 * dc)

@@ -269,16 +269,16 @@ int orbit_block_bwd(const orbit_block_desc* d, const void* dy, const orbit_block
   ORBIT_TRY(layernorm_bwd(w.da, ORBIT_F32, sv.x, rt, sv.mean1, sv.rstd1, P->ln1_g, dt, w.dx1f, ORBIT_F32,
                           nullptr, dx, rt, acc_ln1g, acc_ln1b, M, D, s));
   // fp32 accumulators -> gradient dtype
-  ORBIT_TRY(cast_copy(acc_bfc2, ORBIT_F32, G->bfc2, dt, D, s));
-  ORBIT_TRY(cast_copy(acc_bproj, ORBIT_F32, G->bproj, dt, D, s));
-  ORBIT_TRY(cast_copy(acc_ln2g, ORBIT_F32, G->ln2_g, dt, D, s));
-  ORBIT_TRY(cast_copy(acc_ln2b, ORBIT_F32, G->ln2_b, dt, D, s));
-  ORBIT_TRY(cast_copy(acc_ln1g, ORBIT_F32, G->ln1_g, dt, D, s));
-  ORBIT_TRY(cast_copy(acc_ln1b, ORBIT_F32, G->ln1_b, dt, D, s));
+  CastSegs cs;
+  cs.add(acc_bfc2, G->bfc2, D); cs.add(acc_bproj, G->bproj, D);
+  cs.add(acc_ln2g, G->ln2_g, D); cs.add(acc_ln2b, G->ln2_b, D);
+  cs.add(acc_ln1g, G->ln1_g, D); cs.add(acc_ln1b, G->ln1_b, D);
   for (int k = 0; k < T; k++) {
-    ORBIT_TRY(cast_copy(acc_bfc1 + (size_t)k * fc, ORBIT_F32, G->shards[k].bfc1, dt, fc, s));
-    ORBIT_TRY(cast_copy(acc_bqkv + (size_t)k * 3 * dc, ORBIT_F32, G->shards[k].bqkv, dt, 3 * dc, s));
+    if (cs.count > 14) { ORBIT_TRY(cast_multi(cs, dt, s)); cs.count = 0; }
+    cs.add(acc_bfc1 + (size_t)k * fc, G->shards[k].bfc1, fc);
+    cs.add(acc_bqkv + (size_t)k * 3 * dc, G->shards[k].bqkv, 3 * dc);
   }
+  ORBIT_TRY(cast_multi(cs, dt, s));
   return ORBIT_OK;
 }
 

@@ -212,7 +212,7 @@ int orbit_embed_fused_bwd(const orbit_front_desc* d, const float* x, const void*
   }
   // score path: ds per patch, dG = sum_bl pixext ds, dUt = Wpb^T dG
   ORBIT_TRY(fe_patch_bwd(x, sv.alpha, w.dA, dt, w.dsT, d->V, f.Vp, d->Hg, d->Wg, d->p, h, BL, s));
-  ORBIT_TRY(fe_dg(x, w.dsT, w.dG, d->V, f.Vp, d->Hg, d->Wg, d->p, BL, s));
+  ORBIT_TRY(fe_dg(x, w.dsT, w.dG, d->B, d->V, f.Vp, d->Hg, d->Wg, d->p, s));
   ORBIT_TRY(fe_dut(sv.Wpb, dt, w.dG, acc_dUt, f.KVp, D, h, s));
   ORBIT_TRY(fe_finish_dwp(w.accW, w.dG, sv.Ut, dWp, dbp, dt, d->V, f.Vp, f.P2, D, h, s));
   ORBIT_TRY(agg_param_bwd(acc_dUt, sv.qt, P->q, P->Wq, P->Wk, dt, G->Wk, G->bk, G->bq, G->Wq, G->q, dqt, D, h, s));

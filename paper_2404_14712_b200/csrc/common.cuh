@@ -130,6 +130,13 @@ int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const 
 int colsum(const void* in, int in_dt, long long ld, int M, int N, float* acc, void* copy_out, int copy_dt,
            long long ld_copy, cudaStream_t s);
 int cast_copy(const void* in, int in_dt, void* out, int out_dt, size_t n, cudaStream_t s);
+// up to 16 fp32 -> out_dt casts in one launch
+struct CastSeg { const float* src; void* dst; size_t n; };
+struct CastSegs {
+  CastSeg s[16]; int count = 0;
+  void add(const float* src, void* dst, size_t n) { s[count].src = src; s[count].dst = dst; s[count].n = n; count++; }
+};
+int cast_multi(const CastSegs& segs, int out_dt, cudaStream_t s);
 int fill_zero(void* p, size_t bytes, cudaStream_t s);
 // out = a (a_dt) + b_f32 + bias (p_dt)  (combine of fp32 Hybrid-STOP partials)
 int add_partial(const void* a, int a_dt, const float* part, const void* bias, int p_dt, void* out, int out_dt,

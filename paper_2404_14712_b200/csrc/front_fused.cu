@@ -84,11 +84,24 @@ __global__ void fe_make_g_kernel(const T* __restrict__ Wpb, const float* __restr
   float acc[HP];
 #pragma unroll
   for (int a = 0; a < HP; a++) acc[a] = 0.f;
-  for (int d = lane; d < D; d += 32) {
-    const float w = to_f<T>(Wpb[(size_t)k * D + d]);
+  if (h == HP) {                       // rows of Ut are 64 bytes: four 16-byte loads
+    for (int d = lane; d < D; d += 32) {
+      const float w = to_f<T>(Wpb[(size_t)k * D + d]);
+      const float4* u4 = reinterpret_cast<const float4*>(Ut + (size_t)d * HP);
 #pragma unroll
-    for (int a = 0; a < HP; a++)
-      if (a < h) acc[a] = fmaf(w, Ut[(size_t)d * h + a], acc[a]);
+      for (int q = 0; q < HP / 4; q++) {
+        const float4 u = __ldg(u4 + q);
+        acc[4 * q] = fmaf(w, u.x, acc[4 * q]); acc[4 * q + 1] = fmaf(w, u.y, acc[4 * q + 1]);
+        acc[4 * q + 2] = fmaf(w, u.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(w, u.w, acc[4 * q + 3]);
+      }
+    }
+  } else {
+    for (int d = lane; d < D; d += 32) {
+      const float w = to_f<T>(Wpb[(size_t)k * D + d]);
+#pragma unroll
+      for (int a = 0; a < HP; a++)
+        if (a < h) acc[a] = fmaf(w, Ut[(size_t)d * h + a], acc[a]);
+    }
   }
 #pragma unroll
   for (int a = 0; a < HP; a++) acc[a] = warp_sum(acc[a]);
@@ -247,69 +260,76 @@ __global__ void __launch_bounds__(256) fe_patch_bwd_kernel(const float* __restri
   }
 }
 
-// dG[(r, v), a] += sum_{bl in this split} pixext[bl, v, r] dsT[v][bl][a]; block = (v, split), thread = (r, a)
+// dG[(r, v), a] += sum_{bl in this split} pixext[bl, v, r] dsT[v][bl][a]; block = (v, a range of patch rows),
+// thread = (r, a).  A patch row (b, i) is gw consecutive patches: its pixels for (v, r) are x[row + j*P] and its
+// ds values dsT[v][bl0 + j][a], so the inner loop has no index arithmetic beyond two strides.
 template <int P>
 __global__ void fe_dg_kernel(const float* __restrict__ x, const float* __restrict__ dsT, float* __restrict__ dG, int V, int Vp,
-                             int Hg, int Wg, int BL, int per_split) {
+                             int Hg, int Wg, int B, int rows_per_split) {
   constexpr int P2 = P * P, R = P2 + 1;
   const int v = blockIdx.x, t = threadIdx.x;
   if (t >= R * HP) return;
   const int r = t / HP, a = t - r * HP;
-  const int gw = Wg / P, L = (Hg / P) * gw;
+  const int gh = Hg / P, gw = Wg / P, BL = B * gh * gw;
   const int di = r / P, dj = r - di * P;
-  const int bl0 = blockIdx.y * per_split, bl1 = min(BL, bl0 + per_split);
+  const int pr0 = blockIdx.y * rows_per_split, pr1 = min(B * gh, pr0 + rows_per_split);
   float acc = 0.f;
   const float* dsv = dsT + (size_t)v * BL * HP + a;
-#pragma unroll 4
-  for (int bl = bl0; bl < bl1; bl++) {
-    float pv = 1.f;
+  for (int pr = pr0; pr < pr1; pr++) {
+    const int b = pr / gh, i = pr - b * gh;
+    const float* ds = dsv + (size_t)pr * gw * HP;
     if (r < P2) {
-      const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
-      pv = __ldg(x + (((size_t)b * V + v) * Hg + (size_t)i * P + di) * Wg + (size_t)j * P + dj);
+      const float* px = x + (((size_t)b * V + v) * Hg + (size_t)i * P + di) * Wg + dj;
+#pragma unroll 8
+      for (int j = 0; j < gw; j++) acc = fmaf(__ldg(px + j * P), ds[(size_t)j * HP], acc);
+    } else {
+#pragma unroll 8
+      for (int j = 0; j < gw; j++) acc += ds[(size_t)j * HP];
     }
-    acc = fmaf(pv, dsv[(size_t)bl * HP], acc);
   }
   atomicAdd(dG + ((size_t)r * Vp + v) * HP + a, acc);
 }
 
-// dUt[d, a] += sum_{k in split} Wpb[k, d] dG[k, a]
+// dUt[d, a] += sum_{k in split} Wpb[k, d] dG[k, a]; block = 32 d x 16 a (thread t <-> (d, a), a fastest: the
+// atomics of a warp cover consecutive floats of dUt [D, h] when h == HP), blockIdx.y = k split
 template <typename T>
-__global__ void fe_dut_kernel(const T* __restrict__ Wpb, const float* __restrict__ dG, float* __restrict__ dUt, int KVp, int D,
-                              int h, int per_split) {
-  const int d = blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(512) fe_dut_kernel(const T* __restrict__ Wpb, const float* __restrict__ dG,
+                                                     float* __restrict__ dUt, int KVp, int D, int h, int per_split) {
+  const int a = threadIdx.x & (HP - 1), d = blockIdx.x * 32 + (threadIdx.x >> 4);
   if (d >= D) return;
   const int k0 = blockIdx.y * per_split, k1 = min(KVp, k0 + per_split);
-  float acc[HP];
-#pragma unroll
-  for (int a = 0; a < HP; a++) acc[a] = 0.f;
-  for (int k = k0; k < k1; k++) {
-    const float w = to_f<T>(Wpb[(size_t)k * D + d]);
-    const float4* g4 = reinterpret_cast<const float4*>(dG + (size_t)k * HP);
-#pragma unroll
-    for (int q = 0; q < HP / 4; q++) {
-      const float4 g = __ldg(g4 + q);
-      acc[4 * q] = fmaf(w, g.x, acc[4 * q]); acc[4 * q + 1] = fmaf(w, g.y, acc[4 * q + 1]);
-      acc[4 * q + 2] = fmaf(w, g.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(w, g.w, acc[4 * q + 3]);
-    }
-  }
-#pragma unroll
-  for (int a = 0; a < HP; a++)
-    if (a < h) atomicAdd(dUt + (size_t)d * h + a, acc[a]);
+  float acc = 0.f;
+#pragma unroll 4
+  for (int k = k0; k < k1; k++) acc = fmaf(to_f<T>(Wpb[(size_t)k * D + d]), __ldg(dG + (size_t)k * HP + a), acc);
+  if (a < h) atomicAdd(dUt + (size_t)d * h + a, acc);
 }
 
-// dWp[v, r, d] / dbp[v, d] = accW[(r, v), d] + sum_a dG[(r, v), a] Ut[d, a]
+// dWp[v, r, d] / dbp[v, d] = accW[(r, v), d] + sum_a dG[(r, v), a] Ut[d, a]; blockIdx.y = (r, v), threads over d
 template <typename T>
 __global__ void fe_finish_dwp_kernel(const float* __restrict__ accW, const float* __restrict__ dG, const float* __restrict__ Ut,
                                      T* __restrict__ dWp, T* __restrict__ dbp, int V, int Vp, int P2, int D, int h) {
-  const size_t n = (size_t)(P2 + 1) * V * D;
-  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
-    const int d = (int)(idx % D);
-    const int rv = (int)(idx / D), r = rv / V, v = rv - r * V;
-    const size_t k = (size_t)r * Vp + v;
+  const int rv = blockIdx.y, r = rv / V, v = rv - r * V;
+  const size_t k = (size_t)r * Vp + v;
+  float g[HP];
+#pragma unroll
+  for (int a = 0; a < HP; a++) g[a] = a < h ? dG[k * HP + a] : 0.f;
+  T* out = r < P2 ? dWp + ((size_t)v * P2 + r) * D : dbp + (size_t)v * D;
+  for (int d = blockIdx.x * blockDim.x + threadIdx.x; d < D; d += gridDim.x * blockDim.x) {
     float val = accW[k * D + d];
-    for (int a = 0; a < h; a++) val = fmaf(dG[k * HP + a], Ut[(size_t)d * h + a], val);
-    if (r < P2) dWp[((size_t)v * P2 + r) * D + d] = from_f<T>(val);
-    else dbp[(size_t)v * D + d] = from_f<T>(val);
+    if (h == HP) {
+      const float4* u4 = reinterpret_cast<const float4*>(Ut + (size_t)d * HP);
+#pragma unroll
+      for (int q = 0; q < HP / 4; q++) {
+        const float4 u = __ldg(u4 + q);
+        val = fmaf(g[4 * q], u.x, val); val = fmaf(g[4 * q + 1], u.y, val);
+        val = fmaf(g[4 * q + 2], u.z, val); val = fmaf(g[4 * q + 3], u.w, val);
+      }
+    } else {
+#pragma unroll
+      for (int a = 0; a < HP; a++)
+        if (a < h) val = fmaf(g[a], Ut[(size_t)d * h + a], val);
+    }
+    out[d] = from_f<T>(val);
   }
 }
 
@@ -379,34 +399,37 @@ int fe_patch_bwd(const float* x, const float* alpha, const void* dA, int dt, flo
   return ORBIT_OK;
 }
 
-int fe_dg(const float* x, const float* dsT, float* dG, int V, int Vp, int Hg, int Wg, int p, int BL, cudaStream_t s) {
-  const int P2 = p * p, R = P2 + 1;
-  int splits = cdiv(148 * 4, V);
-  if (splits > cdiv(BL, 64)) splits = cdiv(BL, 64);
-  const int per = cdiv(BL, splits);
-  dim3 grid(V, cdiv(BL, per));
+int fe_dg(const float* x, const float* dsT, float* dG, int B, int V, int Vp, int Hg, int Wg, int p, cudaStream_t s) {
+  const int P2 = p * p, R = P2 + 1, prows = B * (Hg / p);
+  int splits = cdiv(148 * 8, V);
+  if (splits > prows) splits = prows;
+  const int per = cdiv(prows, splits);
+  dim3 grid(V, cdiv(prows, per));
   const int nt = ((R * HP + 31) / 32) * 32;
-  if (p == 4) fe_dg_kernel<4><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, BL, per);
-  else if (p == 2) fe_dg_kernel<2><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, BL, per);
-  else fe_dg_kernel<1><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, BL, per);
+  if (p == 4) fe_dg_kernel<4><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, B, per);
+  else if (p == 2) fe_dg_kernel<2><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, B, per);
+  else fe_dg_kernel<1><<<grid, nt, 0, s>>>(x, dsT, dG, V, Vp, Hg, Wg, B, per);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
 
 int fe_dut(const void* Wpb, int dt, const float* dG, float* dUt, int KVp, int D, int h, cudaStream_t s) {
-  const int splits = KVp >= 256 ? 16 : 1, per = cdiv(KVp, splits);
-  dim3 grid(cdiv(D, 128), cdiv(KVp, per));
-  if (dt == ORBIT_BF16) fe_dut_kernel<bf16><<<grid, 128, 0, s>>>((const bf16*)Wpb, dG, dUt, KVp, D, h, per);
-  else fe_dut_kernel<float><<<grid, 128, 0, s>>>((const float*)Wpb, dG, dUt, KVp, D, h, per);
+  const int gx = cdiv(D, 32);
+  int splits = cdiv(148 * 4, gx);
+  if (splits > cdiv(KVp, 16)) splits = cdiv(KVp, 16);
+  const int per = cdiv(KVp, splits);
+  dim3 grid(gx, cdiv(KVp, per));
+  if (dt == ORBIT_BF16) fe_dut_kernel<bf16><<<grid, 512, 0, s>>>((const bf16*)Wpb, dG, dUt, KVp, D, h, per);
+  else fe_dut_kernel<float><<<grid, 512, 0, s>>>((const float*)Wpb, dG, dUt, KVp, D, h, per);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
 
 int fe_finish_dwp(const float* accW, const float* dG, const float* Ut, void* dWp, void* dbp, int dt, int V, int Vp, int P2,
                   int D, int h, cudaStream_t s) {
-  const size_t n = (size_t)(P2 + 1) * V * D;
-  if (dt == ORBIT_BF16) fe_finish_dwp_kernel<bf16><<<grid_for(n, 256), 256, 0, s>>>(accW, dG, Ut, (bf16*)dWp, (bf16*)dbp, V, Vp, P2, D, h);
-  else fe_finish_dwp_kernel<float><<<grid_for(n, 256), 256, 0, s>>>(accW, dG, Ut, (float*)dWp, (float*)dbp, V, Vp, P2, D, h);
+  dim3 grid(cdiv(D, 256), (P2 + 1) * V);
+  if (dt == ORBIT_BF16) fe_finish_dwp_kernel<bf16><<<grid, 256, 0, s>>>(accW, dG, Ut, (bf16*)dWp, (bf16*)dbp, V, Vp, P2, D, h);
+  else fe_finish_dwp_kernel<float><<<grid, 256, 0, s>>>(accW, dG, Ut, (float*)dWp, (float*)dbp, V, Vp, P2, D, h);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

@@ -18,7 +18,7 @@ int fe_patch_fwd(const float* x, const float* G, float* alpha, void* A, int dt, 
 int fe_patch_bwd(const float* x, const float* alpha, const void* dA, int dt, float* dsT, int V, int Vp, int Hg, int Wg, int p,
                  int h, int BL, cudaStream_t s);
 // dG[(r, v), a] += sum_bl pixext[bl, v, r] dsT[v][bl][a]   (dG zeroed by the caller)
-int fe_dg(const float* x, const float* dsT, float* dG, int V, int Vp, int Hg, int Wg, int p, int BL, cudaStream_t s);
+int fe_dg(const float* x, const float* dsT, float* dG, int B, int V, int Vp, int Hg, int Wg, int p, cudaStream_t s);
 // dUt[d, a] += sum_k Wpb[k, d] dG[k, a]                    (dUt zeroed by the caller)
 int fe_dut(const void* Wpb, int dt, const float* dG, float* dUt, int KVp, int D, int h, cudaStream_t s);
 // dWp[v, r, :] / dbp[v, :] = accW[(r, v), :] + sum_a dG[(r, v), a] Ut[:, a]

@@ -97,8 +97,12 @@ __global__ void __launch_bounds__(1024) ln_fwd_kernel(const void* __restrict__ x
 }
 
 // ---- LayerNorm backward ------------------------------------------------------------------------------
-template <int MAXCH>
-__global__ void __launch_bounds__(MAXCH == 1 ? 1024 : 512) ln_bwd_kernel(const void* __restrict__ dout, int dout_dt,
+// One block per row (persistent over rows); a thread owns MAXCH 8-column chunks and keeps their dgamma / dbeta
+// sums in registers across rows.  With MAXCH == 1 the next row's x / dout / add chunks are requested before
+// the block-wide reduction of the current row (software prefetch: the two barriers of the reduction otherwise
+// expose a full HBM round trip per row).
+template <int MAXCH, int TMAX>
+__global__ void __launch_bounds__(TMAX) ln_bwd_kernel(const void* __restrict__ dout, int dout_dt,
     const void* __restrict__ x, int x_dt, const float* __restrict__ mean, const float* __restrict__ rstd,
     const void* __restrict__ gamma, int p_dt, const void* __restrict__ add, int add_dt,
     float* __restrict__ dx_f32, void* __restrict__ dx_out, int out_dt,
@@ -113,58 +117,113 @@ __global__ void __launch_bounds__(MAXCH == 1 ? 1024 : 512) ln_bwd_kernel(const v
     for (int j = 0; j < 8; j++) { dg[c][j] = 0.f; db[c][j] = 0.f; gm[c][j] = 0.f; }
     if (ch < nch) ld8(gamma, (size_t)ch * 8, p_dt, gm[c]);
   }
-  for (int row = blockIdx.x; row < M; row += gridDim.x) {
-    const float mu = mean[row], rs = rstd[row];
-    float zh[MAXCH][8], gh[MAXCH][8];
-    float s1 = 0.f, s2 = 0.f;
+  if (MAXCH == 1) {
+    const int ch = threadIdx.x;
+    const bool act = ch < nch;
+    float xn[8], dn[8], an[8];
 #pragma unroll
-    for (int c = 0; c < MAXCH; c++) {
-      int ch = threadIdx.x + c * blockDim.x;
-      if (ch < nch) {
-        float xv[8], dv[8];
-        ld8(x, (size_t)row * D + (size_t)ch * 8, x_dt, xv);
-        ld8(dout, (size_t)row * D + (size_t)ch * 8, dout_dt, dv);
-#pragma unroll
-        for (int j = 0; j < 8; j++) {
-          float z = (xv[j] - mu) * rs;
-          zh[c][j] = z;
-          dg[c][j] += dv[j] * z;
-          db[c][j] += dv[j];
-          float g = dv[j] * gm[c][j];
-          gh[c][j] = g;
-          s1 += g; s2 += g * z;
-        }
-      }
+    for (int j = 0; j < 8; j++) { xn[j] = 0.f; dn[j] = 0.f; an[j] = 0.f; }
+    int row = blockIdx.x;
+    if (row < M && act) {
+      const size_t off = (size_t)row * D + (size_t)ch * 8;
+      ld8(x, off, x_dt, xn); ld8(dout, off, dout_dt, dn);
+      if (add) ld8(add, off, add_dt, an);
     }
-    float2 r = block_sum2(make_float2(s1, s2), sh);
-    const float m1 = r.x / D, m2 = r.y / D;
+    for (; row < M; row += gridDim.x) {
+      const float mu = mean[row], rs = rstd[row];
+      float zh[8], gh[8], av[8];
+      float s1 = 0.f, s2 = 0.f;
 #pragma unroll
-    for (int c = 0; c < MAXCH; c++) {
-      int ch = threadIdx.x + c * blockDim.x;
-      if (ch < nch) {
+      for (int j = 0; j < 8; j++) {
+        const float z = (xn[j] - mu) * rs;
+        zh[j] = z; av[j] = an[j];
+        dg[0][j] += dn[j] * z;
+        db[0][j] += dn[j];
+        const float g = dn[j] * gm[0][j];
+        gh[j] = g;
+        s1 += g; s2 += g * z;
+      }
+      const int nrow = row + gridDim.x;
+      if (nrow < M && act) {                       // prefetch the next row before the reduction barriers
+        const size_t off = (size_t)nrow * D + (size_t)ch * 8;
+        ld8(x, off, x_dt, xn); ld8(dout, off, dout_dt, dn);
+        if (add) ld8(add, off, add_dt, an);
+      }
+      const float2 r = block_sum2(make_float2(s1, s2), sh);
+      const float m1 = r.x / D, m2 = r.y / D;
+      if (act) {
         float o[8];
-        size_t off = (size_t)row * D + (size_t)ch * 8;
-        if (add) ld8(add, off, add_dt, o);
-        else {
+        const size_t off = (size_t)row * D + (size_t)ch * 8;
 #pragma unroll
-          for (int j = 0; j < 8; j++) o[j] = 0.f;
-        }
-#pragma unroll
-        for (int j = 0; j < 8; j++) o[j] += (gh[c][j] - m1 - zh[c][j] * m2) * rs;
+        for (int j = 0; j < 8; j++) o[j] = av[j] + (gh[j] - m1 - zh[j] * m2) * rs;
         if (dx_f32) st8(dx_f32, off, ORBIT_F32, o);
         if (dx_out) st8(dx_out, off, out_dt, o);
       }
     }
+  } else {
+    for (int row = blockIdx.x; row < M; row += gridDim.x) {
+      const float mu = mean[row], rs = rstd[row];
+      float zh[MAXCH][8], gh[MAXCH][8];
+      float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+      for (int c = 0; c < MAXCH; c++) {
+        int ch = threadIdx.x + c * blockDim.x;
+        if (ch < nch) {
+          float xv[8], dv[8];
+          ld8(x, (size_t)row * D + (size_t)ch * 8, x_dt, xv);
+          ld8(dout, (size_t)row * D + (size_t)ch * 8, dout_dt, dv);
+#pragma unroll
+          for (int j = 0; j < 8; j++) {
+            float z = (xv[j] - mu) * rs;
+            zh[c][j] = z;
+            dg[c][j] += dv[j] * z;
+            db[c][j] += dv[j];
+            float g = dv[j] * gm[c][j];
+            gh[c][j] = g;
+            s1 += g; s2 += g * z;
+          }
+        }
+      }
+      float2 r = block_sum2(make_float2(s1, s2), sh);
+      const float m1 = r.x / D, m2 = r.y / D;
+#pragma unroll
+      for (int c = 0; c < MAXCH; c++) {
+        int ch = threadIdx.x + c * blockDim.x;
+        if (ch < nch) {
+          float o[8];
+          size_t off = (size_t)row * D + (size_t)ch * 8;
+          if (add) ld8(add, off, add_dt, o);
+          else {
+#pragma unroll
+            for (int j = 0; j < 8; j++) o[j] = 0.f;
+          }
+#pragma unroll
+          for (int j = 0; j < 8; j++) o[j] += (gh[c][j] - m1 - zh[c][j] * m2) * rs;
+          if (dx_f32) st8(dx_f32, off, ORBIT_F32, o);
+          if (dx_out) st8(dx_out, off, out_dt, o);
+        }
+      }
+    }
   }
+  // dgamma / dbeta: a thread's 8 consecutive columns are transposed through a per-warp shared-memory strip so that
+  // every atomic instruction of a warp covers 32 consecutive floats (one 128-byte line instead of eight)
+  __shared__ float tr[TMAX / 32][256];
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
   for (int c = 0; c < MAXCH; c++) {
-    int ch = threadIdx.x + c * blockDim.x;
-    if (ch < nch) {
+    const int col0 = (w * 32 + c * blockDim.x) * 8;          // first column of this warp's 256-column strip
 #pragma unroll
-      for (int j = 0; j < 8; j++) {
-        atomicAdd(dgamma_acc + (size_t)ch * 8 + j, dg[c][j]);
-        atomicAdd(dbeta_acc + (size_t)ch * 8 + j, db[c][j]);
+    for (int which = 0; which < 2; which++) {
+#pragma unroll
+      for (int j = 0; j < 8; j++) tr[w][lane * 8 + j] = which ? db[c][j] : dg[c][j];
+      __syncwarp();
+      float* acc = which ? dbeta_acc : dgamma_acc;
+#pragma unroll
+      for (int i = 0; i < 8; i++) {
+        const int col = col0 + i * 32 + lane;
+        if (col < D) atomicAdd(acc + col, tr[w][i * 32 + lane]);
       }
+      __syncwarp();
     }
   }
 }
@@ -193,13 +252,14 @@ __global__ void __launch_bounds__(256) colsum_kernel(const void* __restrict__ in
 #pragma unroll
   for (int j = 0; j < 8; j++) sh[ry][cx][j] = s[j];
   __syncthreads();
-  if (ry == 0 && col < N) {
+  {  // thread t <-> column t of the block's 256: a warp's atomics cover 32 consecutive floats (one line)
+    const int t = threadIdx.x, c2 = t >> 3, j = t & 7;
+    const int colt = blockIdx.x * 256 + t;
+    if (colt < N) {
+      float tot = 0.f;
 #pragma unroll
-    for (int j = 0; j < 8; j++) {
-      float t = 0.f;
-#pragma unroll
-      for (int y = 0; y < 8; y++) t += sh[y][cx][j];
-      atomicAdd(acc + col + j, t);
+      for (int y = 0; y < 8; y++) tot += sh[y][c2][j];
+      atomicAdd(acc + colt, tot);
     }
   }
 }
@@ -214,6 +274,13 @@ __global__ void cast_kernel(const void* __restrict__ in, int in_dt, void* __rest
   }
   for (size_t i = (nv << 3) + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
     stf(out, i, ldf(in, i, in_dt), out_dt);
+}
+
+// several fp32 -> out_dt casts in one launch (the small parameter-gradient accumulators of a block backward)
+__global__ void cast_multi_kernel(CastSegs segs, int out_dt) {
+  const CastSeg sg = segs.s[blockIdx.y];
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < sg.n; i += (size_t)gridDim.x * blockDim.x)
+    stf(sg.dst, i, sg.src[i], out_dt);
 }
 
 __global__ void add_partial_kernel(const void* __restrict__ a, int a_dt, const float* __restrict__ part,
@@ -280,12 +347,16 @@ int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const 
     thr = ((cdiv(nch, maxch) + 31) / 32) * 32;
   }
   int grid = M < 148 * 4 ? M : 148 * 4;
-#define LNB(C) ln_bwd_kernel<C><<<grid, thr, 0, s>>>(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, \
-                                                     dx_f32, dx_out, out_dt, dgamma_acc, dbeta_acc, M, D)
-  if (maxch <= 1) LNB(1);
-  else if (maxch <= 2) LNB(2);
-  else if (maxch <= 3) LNB(3);
-  else if (maxch <= 4) LNB(4);
+#define LNB(C, T) ln_bwd_kernel<C, T><<<grid, thr, 0, s>>>(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, \
+                                                           dx_f32, dx_out, out_dt, dgamma_acc, dbeta_acc, M, D)
+  if (maxch <= 1) {                      // register budget follows the block size (no spills up to 512 threads)
+    if (thr <= 256) LNB(1, 256);
+    else if (thr <= 512) LNB(1, 512);
+    else LNB(1, 1024);
+  }
+  else if (maxch <= 2) LNB(2, 512);
+  else if (maxch <= 3) LNB(3, 512);
+  else if (maxch <= 4) LNB(4, 512);
   else { set_error("layernorm_bwd: D=%d too large", D); return ORBIT_ERR_SHAPE; }
 #undef LNB
   ORBIT_LAUNCH_CHECK();
@@ -311,6 +382,18 @@ int cast_copy(const void* in, int in_dt, void* out, int out_dt, size_t n, cudaSt
   if (blocks < 1) blocks = 1;
   if (blocks > 148 * 8) blocks = 148 * 8;
   cast_kernel<<<(int)blocks, 256, 0, s>>>(in, in_dt, out, out_dt, n);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int cast_multi(const CastSegs& segs, int out_dt, cudaStream_t s) {
+  if (segs.count <= 0) return ORBIT_OK;
+  size_t mx = 0;
+  for (int i = 0; i < segs.count; i++) mx = segs.s[i].n > mx ? segs.s[i].n : mx;
+  int gx = (int)((mx + 255) / 256);
+  if (gx > 148) gx = 148;
+  if (gx < 1) gx = 1;
+  cast_multi_kernel<<<dim3(gx, segs.count), 256, 0, s>>>(segs, out_dt);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

@@ -291,6 +291,106 @@ def test_sharded_block_equals_unsharded(T):
         assert orc.rel_fro(Gc[k], G[k]) < 1e-12, k
 
 
+# ------------------------------------------------------------------ QK-LayerNorm -
+def add_qk_norm_params(P, dh):
+    P.update(qn_g=1 + 0.2 * rnd(dh), qn_b=0.1 * rnd(dh), kn_g=1 + 0.2 * rnd(dh), kn_b=0.1 * rnd(dh))
+    return P
+
+
+def torch_block_qknorm(x, P, heads, eps):
+    """Textbook block with layer_norm over d_h applied to every head's q and k before the scaled dot product
+    (after ref. [8]) from torch library ops in float64 -- test-only cross-check."""
+    F_ = torch.nn.functional
+    B, N, D = x.shape
+    dh = D // heads
+    a = F_.layer_norm(x, (D,), P["ln1_g"], P["ln1_b"], eps)
+    qkv = a @ P["Wqkv"] + P["bqkv"]
+    q, k, v = qkv.split(D, dim=-1)
+    sp = lambda t: t.reshape(B, N, heads, dh).transpose(1, 2)
+    qn = F_.layer_norm(sp(q), (dh,), P["qn_g"], P["qn_b"], eps)
+    kn = F_.layer_norm(sp(k), (dh,), P["kn_g"], P["kn_b"], eps)
+    o = F_.scaled_dot_product_attention(qn, kn, sp(v)).transpose(1, 2).reshape(B, N, D)
+    x1 = x + o @ P["Wproj"] + P["bproj"]
+    m = F_.layer_norm(x1, (D,), P["ln2_g"], P["ln2_b"], eps)
+    return x1 + F_.gelu(m @ P["Wfc1"] + P["bfc1"]) @ P["Wfc2"] + P["bfc2"]
+
+
+def test_qk_norm_block_matches_torch_autograd():
+    B, N, D, h, F = 2, 10, 16, 4, 40
+    P = add_qk_norm_params(rand_block_params(D, F), D // h)
+    x, dy = rnd(B, N, D), rnd(B, N, D)
+    y, cache = orc.block_fwd(x, P, h, 1e-5)
+    dx, G = orc.block_bwd(dy, P, cache)
+    Pt = {k: torch.tensor(v, requires_grad=True) for k, v in P.items()}
+    xt = torch.tensor(x, requires_grad=True)
+    yt = torch_block_qknorm(xt, Pt, h, 1e-5)
+    yt.backward(torch.tensor(dy))
+    assert orc.rel_fro(y, yt.detach().numpy()) < 1e-13
+    assert orc.rel_fro(dx, xt.grad.numpy()) < 1e-12
+    assert set(G) == set(P)
+    for k in P:
+        if k == "kn_b":     # a bias on the keys shifts every logit of a query row equally: softmax-invariant, so
+            assert np.abs(G[k]).max() < 1e-12 and np.abs(Pt[k].grad.numpy()).max() < 1e-12   # d kn_b == 0
+        else:
+            assert orc.rel_fro(G[k], Pt[k].grad.numpy()) < 1e-12, k
+    # and it is not the plain block: dropping the four parameters changes the output
+    y0, _ = orc.block_fwd(x, {k: v for k, v in P.items() if k[1:3] != "n_"}, h, 1e-5)
+    assert orc.rel_fro(y0, y) > 1e-3
+
+
+def test_qk_norm_fd_and_invariants():
+    B, N, D, h, F = 1, 5, 8, 2, 16
+    dh = D // h
+    P = add_qk_norm_params(rand_block_params(D, F), dh)
+    prm = dict(P)
+    prm["x"] = rnd(B, N, D)
+    up = rnd(B, N, D)
+    f = lambda: float((orc.block_fwd(prm["x"], prm, h, 1e-5)[0] * up).sum())
+    y, cache = orc.block_fwd(prm["x"], prm, h, 1e-5)
+    dx, G = orc.block_bwd(up, prm, cache)
+    ana = dict(G)
+    ana["x"] = dx
+    fd_check(f, prm, list(ana.keys()), ana)
+    # gamma = 1, beta = 0: every normalised q / k has squared norm d_h var/(var+eps) <= d_h, so the scaled
+    # logits are bounded by sqrt(d_h) whatever the weights ("the attention logit growth is contained", :114)
+    Pb = dict(P)
+    Pb["Wqkv"] = P["Wqkv"] * 50.0
+    Pb.update(qn_g=np.ones(dh), qn_b=np.zeros(dh), kn_g=np.ones(dh), kn_b=np.zeros(dh))
+    _, c = orc.block_fwd(prm["x"], Pb, h, 1e-5)
+    Qh, Kh = c["Q"].reshape(B, N, h, dh), c["K"].reshape(B, N, h, dh)
+    logits = np.einsum("bnhd,bmhd->bhnm", Qh, Kh) / math.sqrt(dh)
+    assert np.abs(logits).max() <= math.sqrt(dh) + 1e-9
+    assert np.allclose(Qh.mean(-1), 0, atol=1e-12) and np.all((Qh ** 2).sum(-1) <= dh + 1e-9)
+    # eps = 0: rescaling the pre-norm queries (Q columns of Wqkv and bqkv) by c > 0 leaves y unchanged
+    P2 = dict(P)
+    Wq2, bq2 = P["Wqkv"].copy(), P["bqkv"].copy()
+    Wq2[:, :D] *= 7.0
+    bq2[:D] *= 7.0
+    P2["Wqkv"], P2["bqkv"] = Wq2, bq2
+    ya, _ = orc.block_fwd(prm["x"], P, h, 0.0)
+    yb, _ = orc.block_fwd(prm["x"], P2, h, 0.0)
+    assert orc.rel_fro(yb, ya) < 1e-12
+
+
+@pytest.mark.parametrize("T", [2, 4])
+def test_qk_norm_sharded_block_equals_unsharded(T):
+    B, N, D, h, F = 2, 9, 32, 4, 64
+    P = add_qk_norm_params(rand_block_params(D, F), D // h)
+    shards = syn.shard_block_params(P, h, T)
+    x, dy = rnd(B, N, D), rnd(B, N, D)
+    y, c = orc.block_fwd(x, P, h)
+    dx, G = orc.block_bwd(dy, P, c)
+    ys, cs = orc.block_fwd_sharded(x, P, shards, h)
+    dxs, Gc, Gs = orc.block_bwd_sharded(dy, P, shards, cs)
+    assert orc.rel_fro(ys, y) < 1e-13 and orc.rel_fro(dxs, dx) < 1e-13
+    for k in ("qn_g", "qn_b", "kn_g"):
+        assert orc.rel_fro(Gc[k], G[k]) < 1e-12, k
+    assert np.abs(Gc["kn_b"]).max() < 1e-12 and np.abs(G["kn_b"]).max() < 1e-12      # analytically zero
+    Gu = syn.unshard_block_grads(Gs, T)
+    for k in Gu:
+        assert orc.rel_fro(Gu[k], G[k]) < 1e-12, k
+
+
 # ------------------------------------------------------------------ aggregation ----------------
 def torch_aggregate(tok, P, heads, pos=None):
     """Library cross-check: torch's own multi-head attention with one query token per patch."""

@@ -293,7 +293,7 @@ def run_ours(args, cfg):
                     traffic = float(row["dram_bytes_per_launch"])
         except Exception:
             traffic = None
-    roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (tcgen05 bf16 GEMM, all 12 GEMMs of the block)",
+    roofline = {"bound": "tensor", "kernel": "gemm_tc2_kernel / gemm_tc_kernel (tcgen05 bf16 GEMM; every GEMM launch of the step)",
                 "achieved": achieved, "peak": peaks["bf16"], "unit": "TFLOP/s", "frac": achieved / peaks["bf16"],
                 "peak_source": f"{peaks['src']} burst bf16 (MEASURED_PEAKS.json bf16_tflops)",
                 "frac_of_sustained": (achieved / peaks["bf16_sustained"]) if peaks["bf16_sustained"] else None,

@@ -22,6 +22,14 @@ constexpr int NTH = 192;
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 
+// one MUFU.EX2 (ex2.approx.ftz): exp2f() adds a range fix-up of ~5 instructions per element, which made the softmax
+// warps issue-bound; the arguments here are <= 8 and results below 2^-126 may flush to zero
+__device__ __forceinline__ float fast_ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 template <int DH>
 struct Cfg {
   static constexpr int NBLK = DH / 64;                  // 64-column blocks per tile row
@@ -174,8 +182,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         uint32_t pk[4];
 #pragma unroll
         for (int i = 0; i < 4; i++) {
-          const float p0 = exp2f(__uint_as_float(s[c * 8 + 2 * i]) * sl2 - m_used);
-          const float p1 = exp2f(__uint_as_float(s[c * 8 + 2 * i + 1]) * sl2 - m_used);
+          const float p0 = fast_ex2(__uint_as_float(s[c * 8 + 2 * i]) * sl2 - m_used);
+          const float p1 = fast_ex2(__uint_as_float(s[c * 8 + 2 * i + 1]) * sl2 - m_used);
           sum += p0 + p1;
           __nv_bfloat162 v = __floats2bfloat162_rn(p0, p1);
           pk[i] = *reinterpret_cast<uint32_t*>(&v);
@@ -231,6 +239,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
 // and as an MN-major B operand (contraction over its 64 rows).
 // =====================================================================================================
 constexpr int BT = 64;
+constexpr int NTHB = 320;   // warp 0 TMA, warp 1 MMA, warps 2..9 softmax: two warps per TMEM lane quarter, 32 columns each
 
 template <int DH>
 struct CfgB {
@@ -238,8 +247,11 @@ struct CfgB {
   static constexpr int BIG = 128 * DH * 2;        // stationary [128 x DH] tile
   static constexpr int SMALL = BT * DH * 2;       // streamed [64 x DH] tile
   static constexpr int PT = 128 * BT * 2;         // [128 x 64] bf16 operand tile written by the softmax threads
-  static constexpr int SMEM_DKV = 2 * BIG + 4 * SMALL + 2 * PT + 1024 /*stats*/ + 1024 + 256;
-  static constexpr int SMEM_DQ = 2 * BIG + 4 * SMALL + PT + 1024 + 256;
+  // stages of the streamed (two-tile) ring: hide the TMA round trip.  The operand tiles written by the softmax warps
+  // (P^T, dS^T resp. dS) are double buffered so that tile j+1 is written while the MMAs of tile j still read tile j.
+  static constexpr int NST_DKV = 3, NST_DQ = 4;
+  static constexpr int SMEM_DKV = 2 * BIG + 2 * NST_DKV * SMALL + 4 * PT + 1024 /*stats*/ + 1024 + 256;
+  static constexpr int SMEM_DQ = 2 * BIG + 2 * NST_DQ * SMALL + 2 * PT + 1024 + 256;
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
@@ -256,6 +268,20 @@ __device__ __forceinline__ void write_row64(uint32_t tile, int r, const float* v
       pk[i] = *reinterpret_cast<uint32_t*>(&t2);
     }
     const uint32_t addr = tile + r * 128 + ((c ^ (r & 7)) << 4);
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+  }
+}
+// same for 32 of the 64 columns (chunks 4*half .. 4*half + 3): two warps share a row (backward softmax warps)
+__device__ __forceinline__ void write_row32(uint32_t tile, int r, const float* v, int half) {
+#pragma unroll
+  for (int c = 0; c < 4; c++) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      __nv_bfloat162 t2 = __floats2bfloat162_rn(v[c * 8 + 2 * i], v[c * 8 + 2 * i + 1]);
+      pk[i] = *reinterpret_cast<uint32_t*>(&t2);
+    }
+    const uint32_t addr = tile + r * 128 + (((half * 4 + c) ^ (r & 7)) << 4);
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
   }
 }
@@ -285,19 +311,20 @@ __device__ __forceinline__ void store_acc_row(uint32_t taddr, bf16* dst, float s
 
 // ---------------------------------------------------------------- dK, dV : rows = keys -------------------
 template <int DH>
-__global__ void __launch_bounds__(NTH, 1)
+__global__ void __launch_bounds__(NTHB, 1)
 attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
                         const __grid_constant__ CUtensorMap tmdO, AttnArgs a, float scale, float sl2) {
   using C = CfgB<DH>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sK = base, sV = sK + C::BIG, sRing = sV + C::BIG, sPt = sRing + 4 * C::SMALL, sdSt = sPt + C::PT,
-                 sStat = sdSt + C::PT, bar = sStat + 1024;
+  const uint32_t sK = base, sV = sK + C::BIG, sRing = sV + C::BIG, sPt0 = sRing + 2 * C::NST_DKV * C::SMALL,
+                 sStat = sPt0 + 4 * C::PT, bar = sStat + 1024;
   auto sQ = [&](int st) { return sRing + st * 2 * C::SMALL; };
   auto sdO = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
   float* stat = reinterpret_cast<float*>(smem_raw + (sStat - ptx::smem_u32(smem_raw)));   // [2][2][64]
-  const uint32_t kv_full = bar, qdo_full0 = bar + 8, qdo_empty0 = bar + 24, st_full0 = bar + 40, st_empty0 = bar + 56,
-                 p_full = bar + 72, p_done = bar + 80, tmem_slot = bar + 88;
+  constexpr int NST = C::NST_DKV;
+  const uint32_t kv_full = bar, qdo_full0 = bar + 8, qdo_empty0 = qdo_full0 + 8 * NST, st_full0 = qdo_empty0 + 8 * NST,
+                 st_empty0 = st_full0 + 16, p_full0 = st_empty0 + 16, p_done0 = p_full0 + 16, tmem_slot = p_done0 + 16;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int k0 = blockIdx.x * 128;
@@ -308,12 +335,9 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdO);
     ptx::mbar_init(kv_full, 1);
-    for (int i = 0; i < 2; i++) {
-      ptx::mbar_init(qdo_full0 + 8 * i, 1); ptx::mbar_init(qdo_empty0 + 8 * i, 1);
-      ptx::mbar_init(st_full0 + 8 * i, 1);  ptx::mbar_init(st_empty0 + 8 * i, 4);
-    }
-    ptx::mbar_init(p_full, 4);
-    ptx::mbar_init(p_done, 1);
+    for (int i = 0; i < NST; i++) { ptx::mbar_init(qdo_full0 + 8 * i, 1); ptx::mbar_init(qdo_empty0 + 8 * i, 1); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(st_full0 + 8 * i, 1);  ptx::mbar_init(st_empty0 + 8 * i, 8); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
   if (warp == 1) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
@@ -333,8 +357,8 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         ptx::tma_load_2d(sV + bk * 16384, &tmBig, kv_full, vc + bk * 64, row0 + k0);
       }
       for (int j = 0; j < ntiles; j++) {
-        const int st = j & 1;
-        ptx::mbar_wait(qdo_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        const int st = j % NST;
+        ptx::mbar_wait(qdo_empty0 + 8 * st, ((j / NST) & 1) ^ 1);
         ptx::mbar_expect_tx(qdo_full0 + 8 * st, 2 * C::SMALL);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) {
@@ -348,29 +372,31 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
       auto issue_s = [&](int j) {
-        const int st = j & 1;
-        ptx::mbar_wait(qdo_full0 + 8 * st, (j >> 1) & 1);
-        ptx::mbar_wait(st_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        const int st = j % NST, tb = j & 1;
+        ptx::mbar_wait(qdo_full0 + 8 * st, (j / NST) & 1);
+        ptx::mbar_wait(st_empty0 + 8 * tb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tSt + st * BT, ptx::make_smem_desc(sK + ob, 16, 1024), ptx::make_smem_desc(sQ(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tSt + tb * BT, ptx::make_smem_desc(sK + ob, 16, 1024), ptx::make_smem_desc(sQ(st) + os, 16, 1024), idesc_s, ks != 0);
         }
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tdPt + st * BT, ptx::make_smem_desc(sV + ob, 16, 1024), ptx::make_smem_desc(sdO(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tdPt + tb * BT, ptx::make_smem_desc(sV + ob, 16, 1024), ptx::make_smem_desc(sdO(st) + os, 16, 1024), idesc_s, ks != 0);
         }
-        ptx::mma_commit(st_full0 + 8 * st);
+        ptx::mma_commit(st_full0 + 8 * tb);
       };
       ptx::mbar_wait(kv_full, 0);
       issue_s(0);
       for (int j = 0; j < ntiles; j++) {
         if (j + 1 < ntiles) issue_s(j + 1);
-        ptx::mbar_wait(p_full, j & 1);
+        const int pb = j & 1;
+        const uint32_t sPt = sPt0 + pb * 2 * C::PT, sdSt = sPt + C::PT;
+        ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
         ptx::tc_fence_after();
-        const int st = j & 1;
+        const int st = j % NST;
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dV += P^T dO_j   (contraction over the tile's 64 queries)
           ptx::mma_f16_ss(tdV, ptx::make_smem_desc(sPt + ks * 32, 16, 1024), ptx::make_smem_desc(sdO(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
@@ -378,58 +404,62 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         for (int ks = 0; ks < BT / 16; ks++)      // dK += dS^T Q_j
           ptx::mma_f16_ss(tdK, ptx::make_smem_desc(sdSt + ks * 32, 16, 1024), ptx::make_smem_desc(sQ(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
         ptx::mma_commit(qdo_empty0 + 8 * st);
-        ptx::mma_commit(p_done);
+        ptx::mma_commit(p_done0 + 8 * pb);
       }
     }
   } else {
-    const int quarter = warp & 3;
+    const int quarter = warp & 3, half = (warp - 2) >> 2;     // this warp: 32 key rows x 32 of the tile's 64 query columns
     const int r = quarter * 32 + lane;                       // key row within the CTA tile = TMEM lane
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
-    const int gi = threadIdx.x - 64;                         // 0..127: stats loader index
+    const int gi = threadIdx.x - 64;                         // 0..255: the first 128 load the statistics
     auto load_stat = [&](int j) -> float {
       const int q = j * BT + (gi & 63);
-      if (j >= ntiles || q >= N) return 0.f;
+      if (gi >= 128 || j >= ntiles || q >= N) return 0.f;
       return (gi >> 6) ? a.delta[(size_t)bh * N + q] : a.lse[(size_t)bh * N + q] * LOG2E;
     };
     float nxt = load_stat(0);
     for (int j = 0; j < ntiles; j++) {
       const int st = j & 1;
-      stat[st * 128 + gi] = nxt;                             // [st][0][c] = lse2, [st][1][c] = delta
-      named_bar_sync(1, 128);
+      if (gi < 128) stat[st * 128 + gi] = nxt;               // [st][0][c] = lse2, [st][1][c] = delta
+      named_bar_sync(1, 256);
       nxt = load_stat(j + 1);
-      const float* lse2 = stat + st * 128;
+      const float* lse2 = stat + st * 128 + half * 32;
       const float* dl = lse2 + 64;
       ptx::mbar_wait(st_full0 + 8 * st, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[64], dp[64];
-      ptx::tmem_ld_32x32(tSt + st * BT + lane_off, s);
-      ptx::tmem_ld_32x32(tSt + st * BT + 32 + lane_off, s + 32);
-      ptx::tmem_ld_32x32(tdPt + st * BT + lane_off, dp);
-      ptx::tmem_ld_32x32(tdPt + st * BT + 32 + lane_off, dp + 32);
+      uint32_t s[32], dp[32];
+      ptx::tmem_ld_32x32(tSt + st * BT + half * 32 + lane_off, s);
+      ptx::tmem_ld_32x32(tdPt + st * BT + half * 32 + lane_off, dp);
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(st_empty0 + 8 * st);
-      float p[64];
-      const int nvalid = N - j * BT;                         // queries (columns) >= N are masked
+      float p[32];
+      const int nvalid = N - j * BT - half * 32;             // queries (columns) >= N are masked
+      if (nvalid >= 32) {                                   // masking only in the ragged last tile (warp-uniform branch)
 #pragma unroll
-      for (int c = 0; c < 64; c++) p[c] = (c < nvalid) ? exp2f(__uint_as_float(s[c]) * sl2 - lse2[c]) : 0.f;
-      if (j > 0) ptx::mbar_wait(p_done, (j - 1) & 1);        // P^T / dS^T tiles are free again
-      write_row64(sPt, r, p);
+        for (int c = 0; c < 32; c++) p[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]);
+      } else {
 #pragma unroll
-      for (int c = 0; c < 64; c++) p[c] *= __uint_as_float(dp[c]) - dl[c];
-      write_row64(sdSt, r, p);
+        for (int c = 0; c < 32; c++) p[c] = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]) : 0.f;
+      }
+      const uint32_t sPt = sPt0 + st * 2 * C::PT, sdSt = sPt + C::PT;
+      if (j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);   // this buffer's P^T / dS^T tiles are free again
+      write_row32(sPt, r, p, half);
+#pragma unroll
+      for (int c = 0; c < 32; c++) p[c] *= __uint_as_float(dp[c]) - dl[c];
+      write_row32(sdSt, r, p, half);
       ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full);
+      if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);
     }
-    ptx::mbar_wait(p_done, (ntiles - 1) & 1);
+    ptx::mbar_wait(p_done0 + 8 * ((ntiles - 1) & 1), ((ntiles - 1) >> 1) & 1);
     ptx::tc_fence_after();
     const int krow = k0 + r;
-    bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld;
-    store_acc_row<DH>(tdV + lane_off, out + vc, 1.f, krow < N);
-    store_acc_row<DH>(tdK + lane_off, out + kc, scale, krow < N);
+    bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld + half * (DH / 2);
+    store_acc_row<DH / 2>(tdV + half * (DH / 2) + lane_off, out + vc, 1.f, krow < N);
+    store_acc_row<DH / 2>(tdK + half * (DH / 2) + lane_off, out + kc, scale, krow < N);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -438,17 +468,18 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
 
 // ---------------------------------------------------------------- dQ : rows = queries -------------------
 template <int DH>
-__global__ void __launch_bounds__(NTH, 1)
+__global__ void __launch_bounds__(NTHB, 1)
 attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
                        const __grid_constant__ CUtensorMap tmdOBig, AttnArgs a, float scale, float sl2) {
   using C = CfgB<DH>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sQ = base, sdO = sQ + C::BIG, sRing = sdO + C::BIG, sdS = sRing + 4 * C::SMALL, bar = sdS + C::PT;
+  const uint32_t sQ = base, sdO = sQ + C::BIG, sRing = sdO + C::BIG, sdS0 = sRing + 2 * C::NST_DQ * C::SMALL, bar = sdS0 + 2 * C::PT;
   auto sK = [&](int st) { return sRing + st * 2 * C::SMALL; };
   auto sV = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
-  const uint32_t q_full = bar, kv_full0 = bar + 8, kv_empty0 = bar + 24, s_full0 = bar + 40, s_empty0 = bar + 56,
-                 p_full = bar + 72, p_done = bar + 80, tmem_slot = bar + 88;
+  constexpr int NST = C::NST_DQ;
+  const uint32_t q_full = bar, kv_full0 = bar + 8, kv_empty0 = kv_full0 + 8 * NST, s_full0 = kv_empty0 + 8 * NST,
+                 s_empty0 = s_full0 + 16, p_full0 = s_empty0 + 16, p_done0 = p_full0 + 16, tmem_slot = p_done0 + 16;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int q0 = blockIdx.x * 128;
@@ -459,12 +490,9 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdOBig);
     ptx::mbar_init(q_full, 1);
-    for (int i = 0; i < 2; i++) {
-      ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1);
-      ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 4);
-    }
-    ptx::mbar_init(p_full, 4);
-    ptx::mbar_init(p_done, 1);
+    for (int i = 0; i < NST; i++) { ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 8); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
   if (warp == 1) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
@@ -484,8 +512,8 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::tma_load_2d(sdO + bk * 16384, &tmdOBig, q_full, h * DH + bk * 64, row0 + q0);
       }
       for (int j = 0; j < ntiles; j++) {
-        const int st = j & 1;
-        ptx::mbar_wait(kv_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        const int st = j % NST;
+        ptx::mbar_wait(kv_empty0 + 8 * st, ((j / NST) & 1) ^ 1);
         ptx::mbar_expect_tx(kv_full0 + 8 * st, 2 * C::SMALL);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) {
@@ -499,38 +527,40 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
       auto issue_s = [&](int j) {
-        const int st = j & 1;
-        ptx::mbar_wait(kv_full0 + 8 * st, (j >> 1) & 1);
-        ptx::mbar_wait(s_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        const int st = j % NST, tb = j & 1;
+        ptx::mbar_wait(kv_full0 + 8 * st, (j / NST) & 1);
+        ptx::mbar_wait(s_empty0 + 8 * tb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tS + st * BT, ptx::make_smem_desc(sQ + ob, 16, 1024), ptx::make_smem_desc(sK(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tS + tb * BT, ptx::make_smem_desc(sQ + ob, 16, 1024), ptx::make_smem_desc(sK(st) + os, 16, 1024), idesc_s, ks != 0);
         }
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tdP + st * BT, ptx::make_smem_desc(sdO + ob, 16, 1024), ptx::make_smem_desc(sV(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tdP + tb * BT, ptx::make_smem_desc(sdO + ob, 16, 1024), ptx::make_smem_desc(sV(st) + os, 16, 1024), idesc_s, ks != 0);
         }
-        ptx::mma_commit(s_full0 + 8 * st);
+        ptx::mma_commit(s_full0 + 8 * tb);
       };
       ptx::mbar_wait(q_full, 0);
       issue_s(0);
       for (int j = 0; j < ntiles; j++) {
         if (j + 1 < ntiles) issue_s(j + 1);
-        ptx::mbar_wait(p_full, j & 1);
+        const int pb = j & 1;
+        const uint32_t sdS = sdS0 + pb * C::PT;
+        ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
         ptx::tc_fence_after();
-        const int st = j & 1;
+        const int st = j % NST;
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dQ += dS K_j   (contraction over the tile's 64 keys)
           ptx::mma_f16_ss(tdQ, ptx::make_smem_desc(sdS + ks * 32, 16, 1024), ptx::make_smem_desc(sK(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
         ptx::mma_commit(kv_empty0 + 8 * st);
-        ptx::mma_commit(p_done);
+        ptx::mma_commit(p_done0 + 8 * pb);
       }
     }
   } else {
-    const int quarter = warp & 3;
+    const int quarter = warp & 3, half = (warp - 2) >> 2;     // 32 query rows x 32 of the tile's 64 key columns
     const int r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     const int qrow = q0 + r;
@@ -540,32 +570,36 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
       const int st = j & 1;
       ptx::mbar_wait(s_full0 + 8 * st, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[64], dp[64];
-      ptx::tmem_ld_32x32(tS + st * BT + lane_off, s);
-      ptx::tmem_ld_32x32(tS + st * BT + 32 + lane_off, s + 32);
-      ptx::tmem_ld_32x32(tdP + st * BT + lane_off, dp);
-      ptx::tmem_ld_32x32(tdP + st * BT + 32 + lane_off, dp + 32);
+      uint32_t s[32], dp[32];
+      ptx::tmem_ld_32x32(tS + st * BT + half * 32 + lane_off, s);
+      ptx::tmem_ld_32x32(tdP + st * BT + half * 32 + lane_off, dp);
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
-      float ds[64];
-      const int nvalid = N - j * BT;                         // keys (columns) >= N are masked
+      float ds[32];
+      const int nvalid = N - j * BT - half * 32;             // keys (columns) >= N are masked
+      if (nvalid >= 32) {                                   // masking only in the ragged last tile (warp-uniform branch)
 #pragma unroll
-      for (int c = 0; c < 64; c++) {
-        const float p = (c < nvalid) ? exp2f(__uint_as_float(s[c]) * sl2 - lse2) : 0.f;
-        ds[c] = p * (__uint_as_float(dp[c]) - dl);
+        for (int c = 0; c < 32; c++) ds[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) * (__uint_as_float(dp[c]) - dl);
+      } else {
+#pragma unroll
+        for (int c = 0; c < 32; c++) {
+          const float p = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) : 0.f;
+          ds[c] = p * (__uint_as_float(dp[c]) - dl);
+        }
       }
-      if (j > 0) ptx::mbar_wait(p_done, (j - 1) & 1);
-      write_row64(sdS, r, ds);
+      if (j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
+      write_row32(sdS0 + st * C::PT, r, ds, half);
       ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full);
+      if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);
     }
-    ptx::mbar_wait(p_done, (ntiles - 1) & 1);
+    ptx::mbar_wait(p_done0 + 8 * ((ntiles - 1) & 1), ((ntiles - 1) >> 1) & 1);
     ptx::tc_fence_after();
-    store_acc_row<DH>(tdQ + lane_off, (bf16*)a.dqkv + (size_t)(row0 + qrow) * a.ld + qc, scale, qrow < N);
+    store_acc_row<DH / 2>(tdQ + half * (DH / 2) + lane_off,
+                          (bf16*)a.dqkv + (size_t)(row0 + qrow) * a.ld + qc + half * (DH / 2), scale, qrow < N);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -662,9 +696,9 @@ int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_LAUNCH_CHECK();
   dim3 grid(cdiv(a.N, 128), a.B * a.heads);
   const float scale = 1.0f / sqrtf((float)DH);
-  attn_bwd_dq_tc5_kernel<DH><<<grid, NTH, CfgB<DH>::SMEM_DQ, s>>>(tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E);
+  attn_bwd_dq_tc5_kernel<DH><<<grid, NTHB, CfgB<DH>::SMEM_DQ, s>>>(tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E);
   ORBIT_LAUNCH_CHECK();
-  attn_bwd_dkv_tc5_kernel<DH><<<grid, NTH, CfgB<DH>::SMEM_DKV, s>>>(tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E);
+  attn_bwd_dkv_tc5_kernel<DH><<<grid, NTHB, CfgB<DH>::SMEM_DKV, s>>>(tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

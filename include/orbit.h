@@ -44,9 +44,12 @@ typedef enum {
 
 typedef enum { ORBIT_F32 = 0, ORBIT_BF16 = 1 } orbit_dtype;
 
-/* flags of orbit_block_desc (reserved: setting one returns ORBIT_ERR_UNSUPPORTED) */
-#define ORBIT_QK_NORM   1u   /* QK-LayerNorm, PAPER.md:114 -- SURVEY NEXT-2 */
-#define ORBIT_RECOMPUTE 2u   /* activation checkpointing, PAPER.md:124 -- SURVEY NEXT-2 */
+/* flags of orbit_block_desc (any other bit returns ORBIT_ERR_UNSUPPORTED) */
+#define ORBIT_QK_NORM   1u   /* QK-LayerNorm (R9): LayerNorm over d_h of every head's q and k before the
+                                scaled dot product, gamma / beta in R^{d_h} shared by the heads (qn_g, qn_b, kn_g, kn_b of
+                                orbit_block_params); needs d_h in {32, 64, 128, 256} */
+#define ORBIT_RECOMPUTE 2u   /* activation checkpointing: orbit_block_fwd keeps only the block input in
+                                `saved`; orbit_block_bwd re-runs the forward into its workspace first.  Same results. */
 
 /* ---- a1 / a1': per-variable patch tokenisation (R1, R2) --------------------------- */
 typedef struct {
@@ -125,10 +128,14 @@ typedef struct {
 typedef struct { const void *Wqkv /*[D,3D/T]*/, *bqkv /*[3D/T]*/, *Wproj /*[D/T,D]*/, *Wfc1 /*[D,F/T]*/,
                  *bfc1 /*[F/T]*/, *Wfc2 /*[F/T,D]*/; } orbit_block_shard;
 typedef struct { const void *ln1_g, *ln1_b, *ln2_g, *ln2_b, *bproj, *bfc2 /* all [D] */;
-                 const orbit_block_shard* shards /* T of them, host array */; } orbit_block_params;
+                 const orbit_block_shard* shards /* T of them, host array */;
+                 const void *qn_g, *qn_b, *kn_g, *kn_b /* [d_h]; read only with ORBIT_QK_NORM, else may be NULL */;
+               } orbit_block_params;
 typedef struct { void *Wqkv, *bqkv, *Wproj, *Wfc1, *bfc1, *Wfc2; } orbit_block_shard_grads;
 typedef struct { void *ln1_g, *ln1_b, *ln2_g, *ln2_b, *bproj, *bfc2;
-                 const orbit_block_shard_grads* shards; } orbit_block_grads;
+                 const orbit_block_shard_grads* shards;
+                 void *qn_g, *qn_b, *kn_g, *kn_b /* written only with ORBIT_QK_NORM (d kn_b is analytically 0) */;
+               } orbit_block_grads;
 
 int orbit_block_fwd(const orbit_block_desc* d, const void* x /* [B,N,D] */, const orbit_block_params* P,
                     void* y, void* saved, void* ws, size_t ws_bytes, void* stream);

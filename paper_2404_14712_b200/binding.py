@@ -68,6 +68,8 @@ class orbit_block_desc(C.Structure):
 
 _SHARD_NAMES = ("Wqkv", "bqkv", "Wproj", "Wfc1", "bfc1", "Wfc2")
 _COMMON_NAMES = ("ln1_g", "ln1_b", "ln2_g", "ln2_b", "bproj", "bfc2")
+_QKN_NAMES = ("qn_g", "qn_b", "kn_g", "kn_b")      # QK-LayerNorm parameters [d_h], only with ORBIT_QK_NORM
+ORBIT_QK_NORM, ORBIT_RECOMPUTE = 1, 2
 
 
 class orbit_block_shard(C.Structure):
@@ -75,11 +77,13 @@ class orbit_block_shard(C.Structure):
 
 
 class orbit_block_params(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in _COMMON_NAMES] + [("shards", C.POINTER(orbit_block_shard))]
+    _fields_ = ([(n, C.c_void_p) for n in _COMMON_NAMES] + [("shards", C.POINTER(orbit_block_shard))] +
+                [(n, C.c_void_p) for n in _QKN_NAMES])
 
 
 class orbit_block_grads(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in _COMMON_NAMES] + [("shards", C.POINTER(orbit_block_shard))]
+    _fields_ = ([(n, C.c_void_p) for n in _COMMON_NAMES] + [("shards", C.POINTER(orbit_block_shard))] +
+                [(n, C.c_void_p) for n in _QKN_NAMES])
 
 
 # ---- prototypes ---------------------------------------------------------------------------------------------
@@ -185,7 +189,7 @@ def _agg_struct(cls, P):
 
 def _block_struct(cls, common, shards):
     arr = (orbit_block_shard * len(shards))(*[orbit_block_shard(*[_ptr(S[n]) for n in _SHARD_NAMES]) for S in shards])
-    st = cls(*[_ptr(common[n]) for n in _COMMON_NAMES], arr)
+    st = cls(*[_ptr(common[n]) for n in _COMMON_NAMES], arr, *[_ptr(common.get(n)) for n in _QKN_NAMES])
     st._keep = arr
     return st
 

@@ -142,6 +142,14 @@ int fill_zero(void* p, size_t bytes, cudaStream_t s);
 int add_partial(const void* a, int a_dt, const float* part, const void* bias, int p_dt, void* out, int out_dt,
                 int M, int D, cudaStream_t s);
 
+// ---- QK-LayerNorm (qknorm.cu): buffer layout [M, ld] with columns [Q | K | V | Q' | K'], dc each -------
+bool qknorm_supported(int dh);
+int qknorm_fwd(void* qkv, long long ld, int M, int hk, int dh, int dc, const void* qg, const void* qb, const void* kg,
+               const void* kb, int p_dt, int dt, float eps, cudaStream_t s);
+// dqkv holds dQ', dK' (columns 3dc, 4dc) on entry; dQ, dK are written to columns 0, dc; acc [4][dh] += dgamma/dbeta
+int qknorm_bwd(const void* qkv, void* dqkv, long long ld, int M, int hk, int dh, int dc, const void* qg, const void* kg,
+               int p_dt, int dt, float eps, float* acc, cudaStream_t s);
+
 int mse_loss_grad(const void* y, const void* t, int dt, void* dy, float* loss, size_t n, cudaStream_t s);
 
 // ---- attention (attention_simt.cu / attention_tc.cu) ------------------------------------------------

@@ -166,6 +166,16 @@ def block_params(seed: int, D: int, F: int, dtype: str, tag: str = "blk0") -> di
     return P
 
 
+def qk_norm_params(seed: int, dh: int, dtype: str, tag: str = "blk0") -> dict:
+    """QK-LayerNorm parameters (R9, R23): gains 1 + 0.1 N(0,1), biases 0.1 N(0,1), all [d_h]."""
+    return {
+        "qn_g": round_storage(1.0 + normal(seed, tag + ".qn_g", (dh,), 0.1), dtype),
+        "qn_b": normal(seed, tag + ".qn_b", (dh,), 0.1, dtype=dtype),
+        "kn_g": round_storage(1.0 + normal(seed, tag + ".kn_g", (dh,), 0.1), dtype),
+        "kn_b": normal(seed, tag + ".kn_b", (dh,), 0.1, dtype=dtype),
+    }
+
+
 def shard_block_params(P: dict, heads: int, T: int) -> list[dict]:
     """Split unsharded block parameters into T Hybrid-STOP shards (Eq. 1-2):
     Wqkv, Wfc1 by columns (head-aligned; shard k's Wqkv is [Q_k | K_k | V_k]); Wproj, Wfc2 by rows.

@@ -37,11 +37,16 @@ class BlockRunner:
     SHARD = ob._SHARD_NAMES
 
     def __init__(self, B, N, D, heads, F, T, dtype, resid_dtype, common: dict, shards: list, ln_eps=1e-5,
-                 device="cuda"):
-        self.desc = ob.block_desc(B, N, D, heads, F, T, ln_eps, dtype, resid_dtype)
+                 device="cuda", recompute=False):
+        """QK-LayerNorm (ORBIT_QK_NORM) is switched on by the presence of qn_g, qn_b, kn_g, kn_b in `common`;
+        recompute=True sets ORBIT_RECOMPUTE (activation checkpointing)."""
+        self.qk_norm = "qn_g" in common
+        flags = (ob.ORBIT_QK_NORM if self.qk_norm else 0) | (ob.ORBIT_RECOMPUTE if recompute else 0)
+        self.desc = ob.block_desc(B, N, D, heads, F, T, ln_eps, dtype, resid_dtype, flags)
         self.B, self.N, self.D, self.heads, self.F, self.T = B, N, D, heads, F, T
         self.dtype, self.resid_dtype, self.device = dtype, resid_dtype, device
-        self.common = {k: to_dev(common[k], dtype, device) for k in self.COMMON}
+        names = self.COMMON + (ob._QKN_NAMES if self.qk_norm else ())
+        self.common = {k: to_dev(common[k], dtype, device) for k in names}
         self.shards = [{k: to_dev(S[k], dtype, device) for k in self.SHARD} for S in shards]
         self.gcommon = {k: torch.empty_like(v) for k, v in self.common.items()}
         self.gshards = [{k: torch.empty_like(v) for k, v in S.items()} for S in self.shards]

@@ -50,8 +50,18 @@ def test_size_queries_and_validation_without_gpu(lib):
     assert lib.orbit_block_fwd(ctypes.byref(ok), None, None, None, None, None, 0, None) == 1    # ERR_NULL
     lib.orbit_last_error.restype = ctypes.c_char_p
     assert b"NULL" in lib.orbit_last_error()
-    ok.flags = 1
+    ok.flags = 8                                     # unknown flag bit
     assert lib.orbit_block_fwd(ctypes.byref(ok), None, None, None, None, None, 0, None) == 6    # ERR_UNSUPPORTED
+    # ORBIT_RECOMPUTE keeps only the block input in `saved` and moves the forward state into the workspaces
+    rc = ob.block_desc(1, 2048, 12288, 96, 49152, 1, 1e-5, "bf16", "bf16", ob.ORBIT_RECOMPUTE)
+    assert ob.orbit_block_saved_bytes(rc) == 2048 * 12288 * 2
+    assert ob.orbit_block_fwd_workspace_bytes(rc) >= ob.orbit_block_fwd_workspace_bytes(d) + sv
+    assert ob.orbit_block_bwd_workspace_bytes(rc) >= ob.orbit_block_bwd_workspace_bytes(d) + sv
+    # ORBIT_QK_NORM widens the qkv buffer by the normalised Q', K' copies and rejects unsupported head widths
+    qn = ob.block_desc(1, 2048, 12288, 96, 49152, 1, 1e-5, "bf16", "bf16", ob.ORBIT_QK_NORM)
+    assert ob.orbit_block_saved_bytes(qn) >= sv + 2 * 2048 * 12288 * 2
+    odd = ob.block_desc(1, 16, 96, 2, 192, 1, 1e-5, "bf16", "bf16", ob.ORBIT_QK_NORM)     # d_h = 48
+    assert lib.orbit_block_fwd(ctypes.byref(odd), None, None, None, None, None, 0, None) == 2   # ERR_SHAPE
 
 
 def test_sass_is_sm100a(lib):

@@ -44,8 +44,8 @@ def make_block_case(seed, B, N, D, heads, F, T, dtype, resid_dtype):
     return P, shards, x, dy
 
 
-def run_block(rn, B, N, D, heads, F, T, dtype, resid_dtype, P, shards, x, dy):
-    br = rn.BlockRunner(B, N, D, heads, F, T, dtype, resid_dtype, P, shards)
+def run_block(rn, B, N, D, heads, F, T, dtype, resid_dtype, P, shards, x, dy, recompute=False):
+    br = rn.BlockRunner(B, N, D, heads, F, T, dtype, resid_dtype, P, shards, recompute=recompute)
     xd, dyd = rn.to_dev(x, resid_dtype), rn.to_dev(dy, resid_dtype)
     y = br.fwd(xd)
     dx = br.bwd(dyd)
@@ -59,6 +59,11 @@ def compare_block(br, y, dx, P, x, dy, heads, T, tol, eps=1e-5):
     errs = {"y": check("y", y, yo, tol), "dx": check("dx", dx, dxo, tol)}
     for k in br.COMMON:
         errs[k] = check("d" + k, br.gcommon[k], G[k], tol)
+    if br.qk_norm:
+        for k in ("qn_g", "qn_b", "kn_g"):
+            errs[k] = check("d" + k, br.gcommon[k], G[k], tol)
+        got = br.gcommon["kn_b"].detach().to(torch.float32).cpu().numpy()        # analytically zero (softmax shift invariance)
+        assert np.abs(got).max() <= tol * max(1e-6, np.abs(G["qn_b"]).max()), "d kn_b must vanish"
     gs = [{k: v.detach().to(torch.float32).cpu().numpy() for k, v in S.items()} for S in br.gshards]
     Gu = syn.unshard_block_grads(gs, T)
     for k in Gu:
@@ -107,6 +112,45 @@ def test_block_bf16_vs_oracle(rn, shape):
     br, y, dx = run_block(rn, B, N, D, heads, F, T, "bf16", rdt, P, shards, x, dy)
     errs = compare_block(br, y, dx, P, x, dy, heads, T, 1e-2)
     print("bf16 block errs", {k: f"{v:.2e}" for k, v in errs.items()})
+
+
+@pytest.mark.parametrize("T", [1, 2])
+def test_block_qk_norm_fp32(rn, T):
+    """QK-LayerNorm (ORBIT_QK_NORM) in fp32, d_h = 32, also sharded: <= 1e-4 vs the unsharded oracle."""
+    B, N, D, heads, F = 2, 100, 128, 4, 256
+    P, shards, x, dy = make_block_case(14, B, N, D, heads, F, T, "f32", "f32")
+    P.update(syn.qk_norm_params(14, D // heads, "f32"))
+    br, y, dx = run_block(rn, B, N, D, heads, F, T, "f32", "f32", P, shards, x, dy)
+    compare_block(br, y, dx, P, x, dy, heads, T, 1e-4)
+
+
+@pytest.mark.parametrize("shape", [
+    (2, 384, 512, 8, 1024, 1, "bf16"),      # d_h = 64 on the tcgen05 attention path
+    (1, 200, 256, 2, 512, 1, "f32"),        # d_h = 128, ragged N
+    (2, 256, 512, 4, 1024, 2, "bf16"),      # Hybrid-STOP T = 2, d_h = 128: gamma / beta grads summed over shards
+])
+@pytest.mark.parametrize("recompute", [False, True])
+def test_block_qk_norm_bf16(rn, shape, recompute):
+    B, N, D, heads, F, T, rdt = shape
+    P, shards, x, dy = make_block_case(22, B, N, D, heads, F, T, "bf16", rdt)
+    P.update(syn.qk_norm_params(22, D // heads, "bf16"))
+    br, y, dx = run_block(rn, B, N, D, heads, F, T, "bf16", rdt, P, shards, x, dy, recompute=recompute)
+    errs = compare_block(br, y, dx, P, x, dy, heads, T, 1e-2)
+    print("qk-norm bf16 errs", {k: f"{v:.2e}" for k, v in errs.items()})
+
+
+def test_block_recompute_matches_and_saves_memory(ob, rn):
+    """ORBIT_RECOMPUTE (activation checkpointing): same outputs / gradients as the stored-activation
+    path within tolerance of the oracle, with `saved` reduced to the block input."""
+    B, N, D, heads, F, T = 2, 320, 512, 8, 2048, 1
+    P, shards, x, dy = make_block_case(23, B, N, D, heads, F, T, "bf16", "bf16")
+    br, y, dx = run_block(rn, B, N, D, heads, F, T, "bf16", "bf16", P, shards, x, dy, recompute=True)
+    compare_block(br, y, dx, P, x, dy, heads, T, 1e-2)
+    d0 = ob.block_desc(B, N, D, heads, F, T, 1e-5, "bf16", "bf16", 0)
+    assert ob.orbit_block_saved_bytes(br.desc) == B * N * D * 2
+    assert ob.orbit_block_saved_bytes(br.desc) * 8 < ob.orbit_block_saved_bytes(d0)
+    br0, y0, dx0 = run_block(rn, B, N, D, heads, F, T, "bf16", "bf16", P, shards, x, dy)
+    assert torch.equal(y, y0) and torch.equal(br.gshards[0]["Wfc1"], br0.gshards[0]["Wfc1"])
 
 
 def test_chain_eq2_eq3(ob, rn):
@@ -261,10 +305,14 @@ def test_error_codes(ob, rn):
     assert e.value.status == 2                      # ORBIT_ERR_SHAPE
     P = syn.block_params(1, 64, 128, "bf16")
     br = rn.BlockRunner(1, 16, 64, 2, 128, 1, "bf16", "bf16", P, syn.shard_block_params(P, 2, 1))
-    br.desc.flags = 1                               # reserved QK-norm flag
+    br.desc.flags = 4                               # unknown flag bit
     with pytest.raises(ob.OrbitError) as e:
         br.fwd(torch.zeros(1, 16, 64, device="cuda", dtype=torch.bfloat16))
     assert e.value.status == 6                      # ORBIT_ERR_UNSUPPORTED
+    br.desc.flags = 1                               # QK-LayerNorm without its parameters
+    with pytest.raises(ob.OrbitError) as e:
+        br.fwd(torch.zeros(1, 16, 64, device="cuda", dtype=torch.bfloat16))
+    assert e.value.status == 1                      # ORBIT_ERR_NULL
     br.desc.flags = 0
     br.ws_f = torch.empty(16, dtype=torch.uint8, device="cuda")
     with pytest.raises(ob.OrbitError) as e:

@@ -43,7 +43,8 @@ def run_gemm(ob, M, N, K, a_major, b_major, dtype, simt=False):
     return np.linalg.norm(got - ref) / np.linalg.norm(ref)
 
 
-SHAPES = [(128, 256, 64), (256, 512, 256), (200, 264, 136), (1024, 768, 520), (2048, 1024, 2048), (64, 64, 32)]
+SHAPES = [(128, 256, 64), (256, 512, 256), (200, 264, 136), (1024, 768, 520), (2048, 1024, 2048), (64, 64, 32),
+          (2048, 3072, 512), (1800, 2904, 264)]     # two rounds of 256 x 256 CTA-pair tiles, ragged N tail
 
 
 @pytest.mark.parametrize("a_major", ["K", "M"])

@@ -16,7 +16,9 @@ over identical keys = mean of values; Eq. (2)/(3) shard sums = unsharded product
 convolution (torch conv2d, float64); whole block fwd+bwd = torch float64 autograd of textbook ops;
 aggregation V=1 closed form, permutation invariance, dbk == 0, dbv == sum(do); QK-LayerNorm: torch
 float64 autograd with F.layer_norm on the per-head q / k, finite differences, logits bounded by
-sqrt(d_h) for gamma = 1, beta = 0, invariance to rescaling the pre-norm queries (eps = 0).
+sqrt(d_h) for gamma = 1, beta = 0, invariance to rescaling the pre-norm queries (eps = 0); head + wMSE: torch
+float64 autograd (layer_norm, linear, permute, weighted mean), finite differences, unpatchify = inverse of
+`patches`, weights with mean 1 / equator-symmetric / uniform weights = plain MSE, sum_i cos closed form.
 Parity unpinned: none.
 
 Layout conventions (same as include/orbit.h): row-major, weights [in, out] so y = x A exactly as in
@@ -504,6 +506,87 @@ def mse_loss(y, t):
     y, t = _f64(y), _f64(t)
     d = y - t
     return float((d * d).mean()), 2.0 * d / d.size
+
+
+# ---------------------------------------------------------------------------------------------
+# HEAD -- final LayerNorm, projection "from the feature space to the image space" and the
+# latitude-weighted MSE the paper trains with ("training loss computed as the latitude-weighted
+# Mean Squared Error (wMSE)"); readings R26-R28 of DESIGN.md.
+# ---------------------------------------------------------------------------------------------
+def lat_weights(Hg):
+    """w_i = cos(lat_i) / mean_i cos(lat_i) at the cell centres lat_i = -90 + (i + 1/2) 180/Hg (reading R27:
+    the paper only says "latitude-weighted"; PAPER.md:171 gives the reason: cell areas shrink towards the poles)."""
+    lat = -90.0 + (np.arange(Hg, dtype=F64) + 0.5) * 180.0 / Hg
+    w = np.cos(np.deg2rad(lat))
+    return w / w.mean()
+
+
+def unpatchify(P, V, Hg, Wg, p):
+    """P[b, l, v*p^2 + r] -> img[b, v, i*p+di, j*p+dj] with l = i*(Wg/p)+j, r = di*p+dj: the inverse of `patches`
+    per variable (reading R26: head columns are variable-major, pixels row-major inside a patch)."""
+    B, L, _ = P.shape
+    gh, gw = Hg // p, Wg // p
+    return P.reshape(B, gh, gw, V, p, p).transpose(0, 3, 1, 4, 2, 5).reshape(B, V, Hg, Wg)
+
+
+def patchify_img(img, p):
+    """Inverse of unpatchify: img[b, v, y, x] -> [b, l, v*p^2 + r]."""
+    B, V, Hg, Wg = img.shape
+    gh, gw = Hg // p, Wg // p
+    return img.reshape(B, V, gh, p, gw, p).transpose(0, 2, 4, 1, 3, 5).reshape(B, gh * gw, V * p * p)
+
+
+def head_loss(z, Ph, target, p, eps=1e-5, latw=None):
+    """zn = LN_f(z); P = zn Wh + bh ([B, L, V p^2]); pred = unpatchify(P) ([B, V, Hg, Wg]);
+    loss = mean_{b,v,y,x} w_y (pred - target)^2.  Ph: lnf_g, lnf_b [D], Wh [D, V p^2], bh [V p^2]."""
+    z, target = _f64(z), _f64(target)
+    B, V, Hg, Wg = target.shape
+    w = lat_weights(Hg) if latw is None else _f64(latw)
+    zn, zhat, rstd = layernorm(z, Ph["lnf_g"], Ph["lnf_b"], eps)
+    P = zn @ _f64(Ph["Wh"]) + _f64(Ph["bh"])
+    pred = unpatchify(P, V, Hg, Wg, p)
+    diff = pred - target
+    loss = float((w[None, None, :, None] * diff * diff).mean())
+    cache = dict(zn=zn, zhat=zhat, rstd=rstd, diff=diff, w=w, p=p)
+    return loss, pred, cache
+
+
+def head_loss_bwd(Ph, cache):
+    """dpred = 2 w_y (pred - target) / (B V Hg Wg); dP = patchify(dpred); dbh = sum dP; dWh = zn^T dP;
+    dzn = dP Wh^T; dz, dlnf_g, dlnf_b = LayerNorm backward."""
+    diff, w, p = cache["diff"], cache["w"], cache["p"]
+    dpred = 2.0 * w[None, None, :, None] * diff / diff.size
+    dP = patchify_img(dpred, p)
+    B, L, C = dP.shape
+    D = cache["zn"].shape[-1]
+    G = {}
+    G["bh"] = dP.reshape(B * L, C).sum(axis=0)
+    G["Wh"] = cache["zn"].reshape(B * L, D).T @ dP.reshape(B * L, C)
+    dzn = dP @ _f64(Ph["Wh"]).T
+    dz, G["lnf_g"], G["lnf_b"] = layernorm_bwd(dzn, cache["zhat"], cache["rstd"], Ph["lnf_g"])
+    return dz, G
+
+
+def step_head(x, emb, agg, blocks, head, target_img, p, heads, eps=1e-5, pos=None):
+    """Whole training step with the paper's loss: tokenise -> aggregate -> blocks -> head -> wMSE, and backward."""
+    tok = tokenize(x, emb["Wp"], emb["bp"], p)
+    z, acache = var_aggregate(tok, agg, heads, pos)
+    caches = []
+    h = z
+    for P in blocks:
+        h, c = block_fwd(h, P, heads, eps)
+        caches.append(c)
+    loss, pred, hc = head_loss(h, head, target_img, p, eps)
+    dh, Gh = head_loss_bwd(head, hc)
+    out = dict(agg=z, y=h, loss=loss, pred=pred, dy=dh, head_grads=Gh, block_grads=[None] * len(blocks))
+    for i in reversed(range(len(blocks))):
+        dh, G = block_bwd(dh, blocks[i], caches[i])
+        out["block_grads"][i] = G
+    out["dagg"] = dh
+    dtok, Ga, dpos = var_aggregate_bwd(dh, agg, acache, want_dpos=pos is not None)
+    out["agg_grads"], out["dpos"] = Ga, dpos
+    out["dWp"], out["dbp"] = tokenize_bwd(x, dtok, p)
+    return out
 
 
 # ---------------------------------------------------------------------------------------------

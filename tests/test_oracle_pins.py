@@ -532,6 +532,71 @@ def test_pixel_space_fused_form_equals_definition():
     assert orc.rel_fro(do.sum(0), Gd["bv"]) < 1e-12
 
 
+# ------------------------------------------------------------------ head + wMSE
+def rand_head_params(D, C):
+    return dict(lnf_g=1 + 0.1 * rnd(D), lnf_b=0.1 * rnd(D), Wh=rnd(D, C) / math.sqrt(D), bh=0.1 * rnd(C))
+
+
+def test_lat_weights_and_unpatchify():
+    for Hg in (4, 32, 128):
+        w = orc.lat_weights(Hg)
+        assert abs(w.mean() - 1) < 1e-14 and np.allclose(w, w[::-1], atol=1e-14) and w.argmax() in (Hg // 2 - 1, Hg // 2)
+        # closed form: sum_i cos((i + 1/2) pi/H - pi/2) = 1 / sin(pi / (2H))  (Dirichlet-kernel sum)
+        lat = -90.0 + (np.arange(Hg) + 0.5) * 180.0 / Hg
+        assert abs(np.cos(np.deg2rad(lat)).sum() - 1 / math.sin(math.pi / (2 * Hg))) < 1e-9
+    # unpatchify is the inverse of `patches` variable by variable, and of patchify_img
+    B, V, Hg, Wg, p = 2, 3, 8, 12, 4
+    img = rnd(B, V, Hg, Wg)
+    P = orc.patchify_img(img, p)
+    assert np.array_equal(orc.unpatchify(P, V, Hg, Wg, p), img)
+    pix = orc.patches(img, p)                                   # [B, V, L, p^2]
+    assert np.array_equal(P.reshape(B, -1, V, p * p), pix.transpose(0, 2, 1, 3))
+
+
+def test_head_loss_matches_torch_autograd_and_special_cases():
+    B, V, Hg, Wg, p, D = 2, 3, 8, 12, 2, 16
+    L, C = (Hg // p) * (Wg // p), V * p * p
+    Ph = rand_head_params(D, C)
+    z, tgt = rnd(B, L, D), rnd(B, V, Hg, Wg)
+    loss, pred, cache = orc.head_loss(z, Ph, tgt, p)
+    dz, G = orc.head_loss_bwd(Ph, cache)
+    F_ = torch.nn.functional
+    Pt = {k: torch.tensor(v, requires_grad=True) for k, v in Ph.items()}
+    zt = torch.tensor(z, requires_grad=True)
+    zn = F_.layer_norm(zt, (D,), Pt["lnf_g"], Pt["lnf_b"], 1e-5)
+    Pm = F_.linear(zn, Pt["Wh"].t(), Pt["bh"])
+    predt = Pm.reshape(B, Hg // p, Wg // p, V, p, p).permute(0, 3, 1, 4, 2, 5).reshape(B, V, Hg, Wg)
+    lat = torch.deg2rad(-90.0 + (torch.arange(Hg, dtype=torch.float64) + 0.5) * 180.0 / Hg)
+    w = torch.cos(lat) / torch.cos(lat).mean()
+    lt = (w[None, None, :, None] * (predt - torch.tensor(tgt)) ** 2).mean()
+    lt.backward()
+    assert abs(loss - lt.item()) < 1e-13 * abs(lt.item()) and orc.rel_fro(pred, predt.detach().numpy()) < 1e-13
+    assert orc.rel_fro(dz, zt.grad.numpy()) < 1e-12
+    for k in Ph:
+        assert orc.rel_fro(G[k], Pt[k].grad.numpy()) < 1e-12, k
+    # uniform weights: the plain MSE of the harness loss
+    l1, pred1, _ = orc.head_loss(z, Ph, tgt, p, latw=np.ones(Hg))
+    assert abs(l1 - orc.mse_loss(pred1, tgt)[0]) < 1e-14
+    # a perfect prediction has zero loss and zero gradients
+    l0, _, c0 = orc.head_loss(z, Ph, pred, p)
+    dz0, G0 = orc.head_loss_bwd(Ph, c0)
+    assert l0 == 0.0 and np.abs(dz0).max() == 0.0 and all(np.abs(g).max() == 0.0 for g in G0.values())
+
+
+def test_head_loss_fd():
+    B, V, Hg, Wg, p, D = 1, 2, 4, 4, 2, 8
+    L, C = (Hg // p) * (Wg // p), V * p * p
+    prm = rand_head_params(D, C)
+    prm["z"] = rnd(B, L, D)
+    tgt = rnd(B, V, Hg, Wg)
+    f = lambda: orc.head_loss(prm["z"], prm, tgt, p)[0]
+    _, _, cache = orc.head_loss(prm["z"], prm, tgt, p)
+    dz, G = orc.head_loss_bwd(prm, cache)
+    ana = dict(G)
+    ana["z"] = dz
+    fd_check(f, prm, list(ana.keys()), ana)
+
+
 # ------------------------------------------------------------------ whole step -----------------
 def test_whole_step_fd_through_everything():
     B, V, Hg, Wg, p, D, h, F = 1, 3, 8, 8, 2, 8, 2, 16     # "B1 V3 8x8 p2 D8 h2 F16"

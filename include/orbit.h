@@ -145,6 +145,30 @@ size_t orbit_block_fwd_workspace_bytes(const orbit_block_desc* d);
 size_t orbit_block_bwd_workspace_bytes(const orbit_block_desc* d);
 size_t orbit_block_saved_bytes(const orbit_block_desc* d);
 
+/* ---- head + loss: "predictions are computed by projecting the embedding output from the
+ * feature space to the image space" and the latitude-weighted MSE the paper trains with;
+ * readings R26-R28:  zn = LN_f(z);  P = zn Wh + bh  ([B*L, V p^2], column c = v p^2 + di p + dj);
+ *   pred[b, v, i p + di, j p + dj] = P[b, l = i (Wg/p) + j, c];
+ *   loss = mean_{b,v,y,x} w_y (pred - target)^2,  w_y = cos(lat_y) / mean cos,  lat_y = -90 + (y + 1/2) 180 / Hg.
+ * z [B,L,D] (resid_dtype); lnf_g, lnf_b [D]; Wh [D, V p^2]; bh [V p^2] (dtype); target, pred [B,V,Hg,Wg] fp32 (pred
+ * nullable); latw [Hg] fp32 device weights or NULL for the cosine weights above; loss: fp32 scalar on the device. */
+typedef struct {
+  int B, V, Hg, Wg, p, D;
+  float ln_eps;
+  orbit_dtype dtype;           /* parameters, parameter grads, internal operands */
+  orbit_dtype resid_dtype;     /* z, dz */
+} orbit_head_desc;
+int orbit_head_loss(const orbit_head_desc* d, const void* z, const void* lnf_g, const void* lnf_b, const void* Wh,
+                    const void* bh, const float* target, const float* latw, float* pred, float* loss, void* saved,
+                    void* ws, size_t ws_bytes, void* stream);
+/* dz [B,L,D] and the gradients of lnf_g, lnf_b, Wh, bh for the loss of the matching orbit_head_loss call. */
+int orbit_head_loss_bwd(const orbit_head_desc* d, const void* z, const void* lnf_g, const void* Wh, const void* saved,
+                        void* dz, void* dlnf_g, void* dlnf_b, void* dWh, void* dbh, void* ws, size_t ws_bytes,
+                        void* stream);
+size_t orbit_head_loss_workspace_bytes(const orbit_head_desc* d);
+size_t orbit_head_loss_bwd_workspace_bytes(const orbit_head_desc* d);
+size_t orbit_head_loss_saved_bytes(const orbit_head_desc* d);
+
 /* ---- bare Eq. (2)/(3) chain, used by the fp32 shard-recombination check (R15):
  *   y = sum_k (x A_k) B_k   with A_k [d, n/T] column shards and B_k [n/T, e] row shards;
  *   dx = sum_k (dy B_k^T) A_k^T.  x [m,d], y [m,e]; fp32 partials combined on device.

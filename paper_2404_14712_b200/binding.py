@@ -61,6 +61,11 @@ class orbit_front_desc(C.Structure):
                 ("heads", C.c_int), ("dtype", C.c_int), ("resid_dtype", C.c_int)]
 
 
+class orbit_head_desc(C.Structure):
+    _fields_ = [("B", C.c_int), ("V", C.c_int), ("Hg", C.c_int), ("Wg", C.c_int), ("p", C.c_int), ("D", C.c_int),
+                ("ln_eps", C.c_float), ("dtype", C.c_int), ("resid_dtype", C.c_int)]
+
+
 class orbit_block_desc(C.Structure):
     _fields_ = [("B", C.c_int), ("N", C.c_int), ("D", C.c_int), ("heads", C.c_int), ("F", C.c_int), ("T", C.c_int),
                 ("ln_eps", C.c_float), ("dtype", C.c_int), ("resid_dtype", C.c_int), ("flags", C.c_uint)]
@@ -118,6 +123,10 @@ _proto("orbit_embed_fused_bwd", C.c_int,
         C.POINTER(orbit_agg_grads), _vp, _vp, _sz, _vp])
 for _n in ("orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes", "orbit_embed_fused_saved_bytes"):
     _proto(_n, _sz, [C.POINTER(orbit_front_desc)])
+_proto("orbit_head_loss", C.c_int, [C.POINTER(orbit_head_desc)] + [_vp] * 11 + [_sz, _vp])
+_proto("orbit_head_loss_bwd", C.c_int, [C.POINTER(orbit_head_desc)] + [_vp] * 10 + [_sz, _vp])
+for _n in ("orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes"):
+    _proto(_n, _sz, [C.POINTER(orbit_head_desc)])
 _proto("orbit_block_fwd", C.c_int,
        [C.POINTER(orbit_block_desc), _vp, C.POINTER(orbit_block_params), _vp, _vp, _vp, _sz, _vp])
 _proto("orbit_block_bwd", C.c_int,
@@ -144,7 +153,8 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_set_debug_force_simt", "orbit_debug_gemm", "orbit_profile_gemm",
            "orbit_profile_gemm_collect", "orbit_embed_fused", "orbit_embed_fused_bwd",
            "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
-           "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched"]
+           "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched", "orbit_head_loss", "orbit_head_loss_bwd",
+           "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -177,6 +187,10 @@ def agg_desc(B, L, V, D, heads, dtype, resid_dtype):
 
 def front_desc(B, V, Hg, Wg, p, D, heads, dtype, resid_dtype):
     return orbit_front_desc(B, V, Hg, Wg, p, D, heads, DTYPES[dtype], DTYPES[resid_dtype])
+
+
+def head_desc(B, V, Hg, Wg, p, D, ln_eps, dtype, resid_dtype):
+    return orbit_head_desc(B, V, Hg, Wg, p, D, ln_eps, DTYPES[dtype], DTYPES[resid_dtype])
 
 
 def block_desc(B, N, D, heads, F, T=1, ln_eps=1e-5, dtype="bf16", resid_dtype="bf16", flags=0):
@@ -258,6 +272,30 @@ def orbit_embed_fused_bwd(d, x, Wp, bp, P, dagg, saved, dWp, dbp, G, dpos, ws, s
     _check(lib.orbit_embed_fused_bwd(C.byref(d), _ptr(x), _ptr(Wp), _ptr(bp), C.byref(ps), _ptr(dagg), _ptr(saved),
                                      _ptr(dWp), _ptr(dbp), C.byref(gs), _ptr(dpos), _ptr(ws),
                                      ws.numel() * ws.element_size(), _stream(stream)), "orbit_embed_fused_bwd")
+
+
+def orbit_head_loss_saved_bytes(d):
+    return lib.orbit_head_loss_saved_bytes(C.byref(d))
+
+
+def orbit_head_loss_workspace_bytes(d):
+    return lib.orbit_head_loss_workspace_bytes(C.byref(d))
+
+
+def orbit_head_loss_bwd_workspace_bytes(d):
+    return lib.orbit_head_loss_bwd_workspace_bytes(C.byref(d))
+
+
+def orbit_head_loss(d, z, lnf_g, lnf_b, Wh, bh, target, latw, pred, loss, saved, ws, stream=None):
+    _check(lib.orbit_head_loss(C.byref(d), _ptr(z), _ptr(lnf_g), _ptr(lnf_b), _ptr(Wh), _ptr(bh), _ptr(target), _ptr(latw),
+                               _ptr(pred), _ptr(loss), _ptr(saved), _ptr(ws), ws.numel() * ws.element_size(),
+                               _stream(stream)), "orbit_head_loss")
+
+
+def orbit_head_loss_bwd(d, z, lnf_g, Wh, saved, dz, dlnf_g, dlnf_b, dWh, dbh, ws, stream=None):
+    _check(lib.orbit_head_loss_bwd(C.byref(d), _ptr(z), _ptr(lnf_g), _ptr(Wh), _ptr(saved), _ptr(dz), _ptr(dlnf_g),
+                                   _ptr(dlnf_b), _ptr(dWh), _ptr(dbh), _ptr(ws), ws.numel() * ws.element_size(),
+                                   _stream(stream)), "orbit_head_loss_bwd")
 
 
 def orbit_block_saved_bytes(d):

@@ -166,6 +166,17 @@ def block_params(seed: int, D: int, F: int, dtype: str, tag: str = "blk0") -> di
     return P
 
 
+def head_params(seed: int, D: int, V: int, p: int, dtype: str) -> dict:
+    """Final LayerNorm and image-space head (R23, R26): Wh [D, V p^2] Xavier-uniform."""
+    C = V * p * p
+    return {
+        "lnf_g": round_storage(1.0 + normal(seed, "head.lnf_g", (D,), 0.1), dtype),
+        "lnf_b": normal(seed, "head.lnf_b", (D,), 0.1, dtype=dtype),
+        "Wh": xavier_uniform(seed, "head.Wh", (D, C), D, C, dtype),
+        "bh": normal(seed, "head.bh", (C,), 0.02, dtype=dtype),
+    }
+
+
 def qk_norm_params(seed: int, dh: int, dtype: str, tag: str = "blk0") -> dict:
     """QK-LayerNorm parameters (R9, R23): gains 1 + 0.1 N(0,1), biases 0.1 N(0,1), all [d_h]."""
     return {

@@ -141,12 +141,42 @@ class FusedFrontRunner:
                                  self.gagg, self.dpos, self.ws_b)
 
 
+class HeadRunner:
+    """orbit_head_loss / orbit_head_loss_bwd: final LayerNorm, image-space head, latitude-weighted MSE."""
+
+    NAMES = ("lnf_g", "lnf_b", "Wh", "bh")
+
+    def __init__(self, B, V, Hg, Wg, p, D, dtype, resid_dtype, head: dict, ln_eps=1e-5, device="cuda", keep_pred=True):
+        self.hd = ob.head_desc(B, V, Hg, Wg, p, D, ln_eps, dtype, resid_dtype)
+        L = (Hg // p) * (Wg // p)
+        self.P = {k: to_dev(head[k], dtype, device) for k in self.NAMES}
+        self.G = {k: torch.empty_like(v) for k, v in self.P.items()}
+        self.saved = _bytes(ob.orbit_head_loss_saved_bytes(self.hd), device)
+        self.ws_f = _bytes(ob.orbit_head_loss_workspace_bytes(self.hd), device)
+        self.ws_b = _bytes(ob.orbit_head_loss_bwd_workspace_bytes(self.hd), device)
+        self.pred = torch.empty(B, V, Hg, Wg, dtype=torch.float32, device=device) if keep_pred else None
+        self.loss = torch.zeros(1, dtype=torch.float32, device=device)
+        self.dz = torch.empty(B, L, D, dtype=TD[resid_dtype], device=device)
+
+    def loss_and_grad(self, z, target_img, latw=None):
+        ob.orbit_head_loss(self.hd, z, self.P["lnf_g"], self.P["lnf_b"], self.P["Wh"], self.P["bh"], target_img, latw,
+                           self.pred, self.loss, self.saved, self.ws_f)
+        ob.orbit_head_loss_bwd(self.hd, z, self.P["lnf_g"], self.P["Wh"], self.saved, self.dz, self.G["lnf_g"],
+                               self.G["lnf_b"], self.G["Wh"], self.G["bh"], self.ws_b)
+        return self.loss, self.dz
+
+
 class StepRunner:
     """Whole hot path for a Config: tokenise -> aggregate -> depth x block, forward + backward, MSE loss."""
 
-    def __init__(self, cfg: Config, emb=None, agg=None, blocks=None, pos=None, device="cuda", fused_front=False):
+    def __init__(self, cfg: Config, emb=None, agg=None, blocks=None, pos=None, device="cuda", fused_front=False,
+                 head=None):
         self.cfg = cfg
         self.front = None
+        self.head = None
+        if head is not None:
+            self.head = HeadRunner(cfg.B, cfg.V, cfg.Hg, cfg.Wg, cfg.p, cfg.D, cfg.dtype, cfg.resid_dtype, head, cfg.ln_eps,
+                                   device)
         if cfg.V is not None:
             self.front = (FusedFrontRunner if fused_front else FrontRunner)(cfg.B, cfg.V, cfg.Hg, cfg.Wg, cfg.p, cfg.D, cfg.heads, cfg.dtype, cfg.resid_dtype,
                                      emb, agg, pos, device)
@@ -175,6 +205,14 @@ class StepRunner:
         if self.front is not None:
             self.front.bwd(g)
         return g
+
+    def step_head(self, x, target_img):
+        """The paper's training step: ... -> blocks -> final LN + head -> latitude-weighted MSE and
+        backward.  x, target_img: [B,V,Hg,Wg] fp32."""
+        y = self.forward(x)
+        loss, dz = self.head.loss_and_grad(y, target_img)
+        self.backward(dz)
+        return loss
 
     def step(self, x, target):
         """x: fields [B,V,Hg,Wg] fp32 (or block input [B,N,D] for block-only configs); target [B,L,D]."""

@@ -281,6 +281,59 @@ def test_front_end_fused_fp32_shapes(rn):
     run_and_compare_step(rn, cfg, 45, 1e-4, fused=True)
 
 
+@pytest.mark.parametrize("case", [
+    dict(name="C1", fused=False, tol=1e-4),
+    dict(name="C1", fused=True, tol=1e-4),
+    dict(name="S2", fused=True, tol=1e-2),
+])
+def test_full_step_with_head_and_wmse(rn, case):
+    """The paper's training step (NEXT-3): ... -> blocks -> final LayerNorm -> image-space head -> latitude-weighted MSE
+    (PAPER.md:46, :169), forward + backward through everything, against orc.step_head."""
+    if case["name"] == "C1":
+        cfg, seed = syn.CONFIGS["C1"], syn.seed_of("C1")
+    else:
+        cfg, seed = syn.Config("S2", B=2, V=6, Hg=16, Wg=32, p=2, D=256, heads=4, F=1024, depth=2, dtype="bf16",
+                               resid_dtype="f32"), 46
+    tol = case["tol"]
+    emb, agg, blocks, x, _, pos = make_step_case(cfg, seed)
+    head = syn.head_params(seed, cfg.D, cfg.V, cfg.p, cfg.dtype)
+    timg = syn.fields(seed + 7, cfg.B, cfg.V, cfg.Hg, cfg.Wg, per_variable_scale=False)
+    sr = rn.StepRunner(cfg, emb, agg, [(P, syn.shard_block_params(P, cfg.heads, 1)) for P in blocks], pos,
+                       fused_front=case["fused"], head=head)
+    loss = sr.step_head(rn.to_dev(x, "f32"), rn.to_dev(timg, "f32"))
+    torch.cuda.synchronize()
+    out = orc.step_head(x, emb, agg, blocks, head, timg, cfg.p, cfg.heads, cfg.ln_eps, pos)
+    assert abs(float(loss.item()) - out["loss"]) <= 5 * tol * abs(out["loss"])
+    errs = {"pred": check("pred", sr.head.pred, out["pred"], tol), "dy": check("dy", sr.head.dz, out["dy"], tol)}
+    for k in ("lnf_g", "lnf_b", "Wh", "bh"):
+        errs["head." + k] = check("head.d" + k, sr.head.G[k], out["head_grads"][k], tol)
+    errs["dagg"] = check("dagg", sr.blocks[0].dx, out["dagg"], tol)
+    errs["dWp"] = check("dWp", sr.front.dWp, out["dWp"], tol)
+    errs["dbp"] = check("dbp", sr.front.dbp, out["dbp"], tol)
+    errs["dWqkv0"] = check("dWqkv0", sr.blocks[0].gshards[0]["Wqkv"], out["block_grads"][0]["Wqkv"], tol)
+    print("head step errs", case, {k: f"{v:.2e}" for k, v in errs.items()})
+
+
+def test_head_loss_user_weights_and_errors(ob, rn):
+    """Explicit weights (uniform = plain MSE) and argument checks of orbit_head_loss."""
+    B, V, Hg, Wg, p, D = 2, 4, 8, 16, 2, 64
+    head = syn.head_params(5, D, V, p, "f32")
+    z = syn.normal(5, "z", (B, (Hg // p) * (Wg // p), D))
+    timg = syn.fields(6, B, V, Hg, Wg, per_variable_scale=False)
+    hr = rn.HeadRunner(B, V, Hg, Wg, p, D, "f32", "f32", head)
+    ones = torch.ones(Hg, device="cuda")
+    hr.loss_and_grad(rn.to_dev(z, "f32"), rn.to_dev(timg, "f32"), ones)
+    torch.cuda.synchronize()
+    l, pred, c = orc.head_loss(z, head, timg, p, latw=np.ones(Hg))
+    dz, G = orc.head_loss_bwd(head, c)
+    assert abs(float(hr.loss.item()) - l) <= 1e-5 * l
+    check("pred", hr.pred, pred, 1e-4); check("dz", hr.dz, dz, 1e-4); check("dWh", hr.G["Wh"], G["Wh"], 1e-4)
+    hr.hd.V = 3                                      # V p^2 = 12 is not a multiple of 8
+    with pytest.raises(ob.OrbitError) as e:
+        hr.loss_and_grad(rn.to_dev(z, "f32"), rn.to_dev(timg, "f32"))
+    assert e.value.status == 2
+
+
 def test_fused_front_error_codes(ob, rn):
     cfg = syn.Config("SE", B=1, V=4, Hg=8, Wg=8, p=2, D=64, heads=4, F=128, depth=1, dtype="bf16", resid_dtype="bf16")
     emb, agg, blocks, x, tgt, pos = make_step_case(cfg, 3)

@@ -35,7 +35,11 @@ struct Cfg {
   static constexpr int NBLK = DH / 64;                  // 64-column blocks per tile row
   static constexpr int TILE = 128 * DH * 2;             // bytes of a [128 x DH] bf16 tile
   static constexpr int P_BYTES = 128 * BKV * 2;         // 32 KB
-  static constexpr int SMEM = TILE /*Q*/ + 2 * 2 * TILE /*K,V x 2 stages*/ + P_BYTES + 1024 + 256;
+  // K and V stream through separate rings: a K stage is free as soon as S_j = Q K_j^T has been computed, a V stage
+  // only after O += P_j V_j; with 3 + 2 stages the TMA round trip of K_{j+1} no longer sits between PV_{j-1} and S_{j+1}
+  // (measured with clock64 stamps: the MMA thread waited ~2000 of 2750 cycles per tile for K/V with a shared 2-stage ring)
+  static constexpr int KST = 3, VST = 2;
+  static constexpr int SMEM = TILE /*Q*/ + (KST + VST) * TILE + P_BYTES + 1024 + 256;
 };
 
 template <int DH>
@@ -44,11 +48,13 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   using C = Cfg<DH>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sQ = base, sKV = sQ + C::TILE, sP = sKV + 4 * C::TILE, bar = sP + C::P_BYTES;
-  auto sK = [&](int st) { return sKV + st * 2 * C::TILE; };
-  auto sV = [&](int st) { return sKV + st * 2 * C::TILE + C::TILE; };
-  const uint32_t q_full = bar, kv_full0 = bar + 8, kv_empty0 = bar + 24, s_full0 = bar + 40, s_empty0 = bar + 56,
-                 p_full = bar + 72, o_done = bar + 80, tmem_slot = bar + 88;
+  constexpr int KST = C::KST, VST = C::VST;
+  const uint32_t sQ = base, sK0 = sQ + C::TILE, sV0 = sK0 + KST * C::TILE, sP = sV0 + VST * C::TILE, bar = sP + C::P_BYTES;
+  auto sK = [&](int st) { return sK0 + st * C::TILE; };
+  auto sV = [&](int st) { return sV0 + st * C::TILE; };
+  const uint32_t q_full = bar, k_full0 = bar + 8, k_empty0 = k_full0 + 8 * KST, v_full0 = k_empty0 + 8 * KST,
+                 v_empty0 = v_full0 + 8 * VST, s_full0 = v_empty0 + 8 * VST, s_empty0 = s_full0 + 16, p_full = s_empty0 + 16,
+                 o_done = p_full + 8, tmem_slot = o_done + 8;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int q0 = blockIdx.x * BQ;
@@ -59,10 +65,9 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmQKV);
     ptx::mbar_init(q_full, 1);
-    for (int i = 0; i < 2; i++) {
-      ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1);
-      ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 4);
-    }
+    for (int i = 0; i < KST; i++) { ptx::mbar_init(k_full0 + 8 * i, 1); ptx::mbar_init(k_empty0 + 8 * i, 1); }
+    for (int i = 0; i < VST; i++) { ptx::mbar_init(v_full0 + 8 * i, 1); ptx::mbar_init(v_empty0 + 8 * i, 1); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 4); }
     ptx::mbar_init(p_full, 4);
     ptx::mbar_init(o_done, 1);
     ptx::fence_barrier_init();
@@ -80,15 +85,21 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
       ptx::mbar_expect_tx(q_full, C::TILE);
 #pragma unroll
       for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sQ + bk * 16384, &tmQKV, q_full, qc + bk * 64, row0 + q0);
-      for (int j = 0; j < ntiles; j++) {
-        const int st = j & 1;
-        ptx::mbar_wait(kv_empty0 + 8 * st, ((j >> 1) & 1) ^ 1);
-        ptx::mbar_expect_tx(kv_full0 + 8 * st, 2 * C::TILE);
+      auto load_k = [&](int j) {
+        const int st = j % KST;
+        ptx::mbar_wait(k_empty0 + 8 * st, ((j / KST) & 1) ^ 1);
+        ptx::mbar_expect_tx(k_full0 + 8 * st, C::TILE);
 #pragma unroll
-        for (int bk = 0; bk < C::NBLK; bk++) {
-          ptx::tma_load_2d(sK(st) + bk * 16384, &tmQKV, kv_full0 + 8 * st, kc + bk * 64, row0 + j * BKV);
-          ptx::tma_load_2d(sV(st) + bk * 16384, &tmQKV, kv_full0 + 8 * st, vc + bk * 64, row0 + j * BKV);
-        }
+        for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sK(st) + bk * 16384, &tmQKV, k_full0 + 8 * st, kc + bk * 64, row0 + j * BKV);
+      };
+      load_k(0);
+      for (int j = 0; j < ntiles; j++) {                      // K runs one tile ahead of V
+        if (j + 1 < ntiles) load_k(j + 1);
+        const int st = j % VST;
+        ptx::mbar_wait(v_empty0 + 8 * st, ((j / VST) & 1) ^ 1);
+        ptx::mbar_expect_tx(v_full0 + 8 * st, C::TILE);
+#pragma unroll
+        for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sV(st) + bk * 16384, &tmQKV, v_full0 + 8 * st, vc + bk * 64, row0 + j * BKV);
       }
     }
   } else if (warp == 1) {
@@ -96,8 +107,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(BQ, BKV, 0, 0);     // S = Q K^T: both K-major
       constexpr uint32_t idesc_o = ptx::make_idesc_bf16(BQ, DH, 0, 1);      // O += P V: V is MN-major
       auto issue_s = [&](int j) {
-        const int st = j & 1, sb = j & 1;
-        ptx::mbar_wait(kv_full0 + 8 * st, (j >> 1) & 1);
+        const int st = j % KST, sb = j & 1;
+        ptx::mbar_wait(k_full0 + 8 * st, (j / KST) & 1);
         ptx::mbar_wait(s_empty0 + 8 * sb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
 #pragma unroll
@@ -106,22 +117,24 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
           ptx::mma_f16_ss(tS0 + sb * 128, ptx::make_smem_desc(sQ + off, 16, 1024), ptx::make_smem_desc(sK(st) + off, 16, 1024),
                           idesc_s, ks != 0);
         }
+        ptx::mma_commit(k_empty0 + 8 * st);          // K stage free once these MMAs have read it
         ptx::mma_commit(s_full0 + 8 * sb);
       };
       ptx::mbar_wait(q_full, 0);
       issue_s(0);
       for (int j = 0; j < ntiles; j++) {
         if (j + 1 < ntiles) issue_s(j + 1);
+        const int st = j % VST;
+        ptx::mbar_wait(v_full0 + 8 * st, (j / VST) & 1);
         ptx::mbar_wait(p_full, j & 1);
         ptx::tc_fence_after();
-        const int st = j & 1;
 #pragma unroll
         for (int ks = 0; ks < BKV / 16; ks++) {
           const uint32_t aoff = (ks >> 2) * 16384 + (ks & 3) * 32;          // P: K-major, two 64-key blocks
           ptx::mma_f16_ss(tO, ptx::make_smem_desc(sP + aoff, 16, 1024),
                           ptx::make_smem_desc(sV(st) + ks * 2048, 16384, 1024), idesc_o, (j | ks) != 0);
         }
-        ptx::mma_commit(kv_empty0 + 8 * st);
+        ptx::mma_commit(v_empty0 + 8 * st);
         ptx::mma_commit(o_done);
       }
     }

@@ -18,7 +18,7 @@ namespace orbit {
 namespace {
 
 constexpr int BQ = 128, BKV = 128;
-constexpr int NTH = 192;
+constexpr int NTH = 192;   // forward: warp 0 TMA, warp 1 MMA issuer, warps 2..5 softmax
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 
@@ -29,6 +29,11 @@ __device__ __forceinline__ float fast_ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+
+// descriptor of the same tile `bytes` further on: the start-address field (bits [0,14), in 16-byte units) never carries
+// out for shared-memory addresses, so this is one 64-bit add instead of rebuilding the descriptor (the single MMA-issuing
+// thread is latency-bound: ~13 dependent uniform-datapath instructions per tcgen05.mma otherwise)
+__device__ __forceinline__ uint64_t desc_adv(uint64_t d, uint32_t bytes) { return d + (uint64_t)(bytes >> 4); }
 
 template <int DH>
 struct Cfg {
@@ -106,16 +111,17 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(BQ, BKV, 0, 0);     // S = Q K^T: both K-major
       constexpr uint32_t idesc_o = ptx::make_idesc_bf16(BQ, DH, 0, 1);      // O += P V: V is MN-major
+      const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024), dP0 = ptx::make_smem_desc(sP, 16, 1024);
       auto issue_s = [&](int j) {
         const int st = j % KST, sb = j & 1;
         ptx::mbar_wait(k_full0 + 8 * st, (j / KST) & 1);
         ptx::mbar_wait(s_empty0 + 8 * sb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
+        const uint64_t dK0 = ptx::make_smem_desc(sK(st), 16, 1024);
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t off = (ks >> 2) * 16384 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tS0 + sb * 128, ptx::make_smem_desc(sQ + off, 16, 1024), ptx::make_smem_desc(sK(st) + off, 16, 1024),
-                          idesc_s, ks != 0);
+          ptx::mma_f16_ss(tS0 + sb * 128, desc_adv(dQ0, off), desc_adv(dK0, off), idesc_s, ks != 0);
         }
         ptx::mma_commit(k_empty0 + 8 * st);          // K stage free once these MMAs have read it
         ptx::mma_commit(s_full0 + 8 * sb);
@@ -128,11 +134,11 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         ptx::mbar_wait(v_full0 + 8 * st, (j / VST) & 1);
         ptx::mbar_wait(p_full, j & 1);
         ptx::tc_fence_after();
+        const uint64_t dV0 = ptx::make_smem_desc(sV(st), 16384, 1024);
 #pragma unroll
         for (int ks = 0; ks < BKV / 16; ks++) {
           const uint32_t aoff = (ks >> 2) * 16384 + (ks & 3) * 32;          // P: K-major, two 64-key blocks
-          ptx::mma_f16_ss(tO, ptx::make_smem_desc(sP + aoff, 16, 1024),
-                          ptx::make_smem_desc(sV(st) + ks * 2048, 16384, 1024), idesc_o, (j | ks) != 0);
+          ptx::mma_f16_ss(tO, desc_adv(dP0, aoff), desc_adv(dV0, ks * 2048), idesc_o, (j | ks) != 0);
         }
         ptx::mma_commit(v_empty0 + 8 * st);
         ptx::mma_commit(o_done);
@@ -140,7 +146,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
     }
   } else {
     // ===================== softmax / correction / epilogue =====================
-    const int quarter = warp & 3;
+    const int quarter = warp & 3;            // warps 2..5
     const int r = quarter * 32 + lane;                       // query row within the tile = TMEM lane
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     float m_used = -INFINITY, l = 0.f;
@@ -252,7 +258,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
 // and as an MN-major B operand (contraction over its 64 rows).
 // =====================================================================================================
 constexpr int BT = 64;
-constexpr int NTHB = 320;   // warp 0 TMA, warp 1 MMA, warps 2..9 softmax: two warps per TMEM lane quarter, 32 columns each
+constexpr int NTHB = 352;   // warp 0 TMA, warp 1 gradient MMAs, warps 2..9 softmax (two per TMEM lane quarter, 32 columns each), warp 10 S/dP MMAs
 
 template <int DH>
 struct CfgB {
@@ -380,7 +386,7 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         }
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == 1 || warp == NTHB / 32 - 1) {   // warp 1: gradient MMAs; last warp: S^T / dP^T MMAs (issue-bound otherwise)
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
@@ -389,33 +395,39 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         ptx::mbar_wait(qdo_full0 + 8 * st, (j / NST) & 1);
         ptx::mbar_wait(st_empty0 + 8 * tb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
+        const uint64_t dK0 = ptx::make_smem_desc(sK, 16, 1024), dV0 = ptx::make_smem_desc(sV, 16, 1024);
+        const uint64_t dQs = ptx::make_smem_desc(sQ(st), 16, 1024), dOs = ptx::make_smem_desc(sdO(st), 16, 1024);
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tSt + tb * BT, ptx::make_smem_desc(sK + ob, 16, 1024), ptx::make_smem_desc(sQ(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tSt + tb * BT, desc_adv(dK0, ob), desc_adv(dQs, os), idesc_s, ks != 0);
         }
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tdPt + tb * BT, ptx::make_smem_desc(sV + ob, 16, 1024), ptx::make_smem_desc(sdO(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tdPt + tb * BT, desc_adv(dV0, ob), desc_adv(dOs, os), idesc_s, ks != 0);
         }
         ptx::mma_commit(st_full0 + 8 * tb);
       };
       ptx::mbar_wait(kv_full, 0);
-      issue_s(0);
+      if (warp != 1) {
+        for (int j = 0; j < ntiles; j++) issue_s(j);
+      } else
       for (int j = 0; j < ntiles; j++) {
-        if (j + 1 < ntiles) issue_s(j + 1);
+        ptx::mbar_wait(qdo_full0 + 8 * (j % NST), (j / NST) & 1);
         const int pb = j & 1;
         const uint32_t sPt = sPt0 + pb * 2 * C::PT, sdSt = sPt + C::PT;
         ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
         ptx::tc_fence_after();
         const int st = j % NST;
+        const uint64_t dPt = ptx::make_smem_desc(sPt, 16, 1024), dSt = ptx::make_smem_desc(sdSt, 16, 1024);
+        const uint64_t dOm = ptx::make_smem_desc(sdO(st), 8192, 1024), dQm = ptx::make_smem_desc(sQ(st), 8192, 1024);
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dV += P^T dO_j   (contraction over the tile's 64 queries)
-          ptx::mma_f16_ss(tdV, ptx::make_smem_desc(sPt + ks * 32, 16, 1024), ptx::make_smem_desc(sdO(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
+          ptx::mma_f16_ss(tdV, desc_adv(dPt, ks * 32), desc_adv(dOm, ks * 2048), idesc_g, (j | ks) != 0);
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dK += dS^T Q_j
-          ptx::mma_f16_ss(tdK, ptx::make_smem_desc(sdSt + ks * 32, 16, 1024), ptx::make_smem_desc(sQ(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
+          ptx::mma_f16_ss(tdK, desc_adv(dSt, ks * 32), desc_adv(dQm, ks * 2048), idesc_g, (j | ks) != 0);
         ptx::mma_commit(qdo_empty0 + 8 * st);
         ptx::mma_commit(p_done0 + 8 * pb);
       }
@@ -535,7 +547,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         }
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == 1 || warp == NTHB / 32 - 1) {   // warp 1: dQ MMAs; last warp: S / dP MMAs
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
@@ -544,30 +556,35 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::mbar_wait(kv_full0 + 8 * st, (j / NST) & 1);
         ptx::mbar_wait(s_empty0 + 8 * tb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
+        const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024), dO0 = ptx::make_smem_desc(sdO, 16, 1024);
+        const uint64_t dKs = ptx::make_smem_desc(sK(st), 16, 1024), dVs = ptx::make_smem_desc(sV(st), 16, 1024);
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tS + tb * BT, ptx::make_smem_desc(sQ + ob, 16, 1024), ptx::make_smem_desc(sK(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tS + tb * BT, desc_adv(dQ0, ob), desc_adv(dKs, os), idesc_s, ks != 0);
         }
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
           const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tdP + tb * BT, ptx::make_smem_desc(sdO + ob, 16, 1024), ptx::make_smem_desc(sV(st) + os, 16, 1024), idesc_s, ks != 0);
+          ptx::mma_f16_ss(tdP + tb * BT, desc_adv(dO0, ob), desc_adv(dVs, os), idesc_s, ks != 0);
         }
         ptx::mma_commit(s_full0 + 8 * tb);
       };
       ptx::mbar_wait(q_full, 0);
-      issue_s(0);
+      if (warp != 1) {
+        for (int j = 0; j < ntiles; j++) issue_s(j);
+      } else
       for (int j = 0; j < ntiles; j++) {
-        if (j + 1 < ntiles) issue_s(j + 1);
+        ptx::mbar_wait(kv_full0 + 8 * (j % NST), (j / NST) & 1);
         const int pb = j & 1;
         const uint32_t sdS = sdS0 + pb * C::PT;
         ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
         ptx::tc_fence_after();
         const int st = j % NST;
+        const uint64_t dSd = ptx::make_smem_desc(sdS, 16, 1024), dKm = ptx::make_smem_desc(sK(st), 8192, 1024);
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dQ += dS K_j   (contraction over the tile's 64 keys)
-          ptx::mma_f16_ss(tdQ, ptx::make_smem_desc(sdS + ks * 32, 16, 1024), ptx::make_smem_desc(sK(st) + ks * 2048, 8192, 1024), idesc_g, (j | ks) != 0);
+          ptx::mma_f16_ss(tdQ, desc_adv(dSd, ks * 32), desc_adv(dKm, ks * 2048), idesc_g, (j | ks) != 0);
         ptx::mma_commit(kv_empty0 + 8 * st);
         ptx::mma_commit(p_done0 + 8 * pb);
       }

@@ -258,7 +258,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
 // and as an MN-major B operand (contraction over its 64 rows).
 // =====================================================================================================
 constexpr int BT = 64;
-constexpr int NTHB = 352;   // warp 0 TMA, warp 1 gradient MMAs, warps 2..9 softmax (two per TMEM lane quarter, 32 columns each), warp 10 S/dP MMAs
+constexpr int NTHB = 384;   // warp 0 TMA, warp 1 gradient MMAs, warps 2..9 softmax (two per TMEM lane quarter, 32 columns each), warp 10 dP MMAs, warp 11 S MMAs
 
 template <int DH>
 struct CfgB {
@@ -355,7 +355,7 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdO);
     ptx::mbar_init(kv_full, 1);
     for (int i = 0; i < NST; i++) { ptx::mbar_init(qdo_full0 + 8 * i, 1); ptx::mbar_init(qdo_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(st_full0 + 8 * i, 1);  ptx::mbar_init(st_empty0 + 8 * i, 8); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(st_full0 + 8 * i, 2);  ptx::mbar_init(st_empty0 + 8 * i, 8); }
     for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
@@ -386,7 +386,7 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         }
       }
     }
-  } else if (warp == 1 || warp == NTHB / 32 - 1) {   // warp 1: gradient MMAs; last warp: S^T / dP^T MMAs (issue-bound otherwise)
+  } else if (warp == 1 || warp >= NTHB / 32 - 2) {   // warp 1: gradient MMAs; last warp: S^T / dP^T MMAs (issue-bound otherwise)
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
@@ -397,15 +397,18 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         ptx::tc_fence_after();
         const uint64_t dK0 = ptx::make_smem_desc(sK, 16, 1024), dV0 = ptx::make_smem_desc(sV, 16, 1024);
         const uint64_t dQs = ptx::make_smem_desc(sQ(st), 16, 1024), dOs = ptx::make_smem_desc(sdO(st), 16, 1024);
+        if (warp == NTHB / 32 - 1) {
 #pragma unroll
-        for (int ks = 0; ks < DH / 16; ks++) {
-          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tSt + tb * BT, desc_adv(dK0, ob), desc_adv(dQs, os), idesc_s, ks != 0);
-        }
+          for (int ks = 0; ks < DH / 16; ks++) {
+            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            ptx::mma_f16_ss(tSt + tb * BT, desc_adv(dK0, ob), desc_adv(dQs, os), idesc_s, ks != 0);
+          }
+        } else {
 #pragma unroll
-        for (int ks = 0; ks < DH / 16; ks++) {
-          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tdPt + tb * BT, desc_adv(dV0, ob), desc_adv(dOs, os), idesc_s, ks != 0);
+          for (int ks = 0; ks < DH / 16; ks++) {
+            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            ptx::mma_f16_ss(tdPt + tb * BT, desc_adv(dV0, ob), desc_adv(dOs, os), idesc_s, ks != 0);
+          }
         }
         ptx::mma_commit(st_full0 + 8 * tb);
       };
@@ -516,7 +519,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdOBig);
     ptx::mbar_init(q_full, 1);
     for (int i = 0; i < NST; i++) { ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 8); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 2);  ptx::mbar_init(s_empty0 + 8 * i, 8); }
     for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
@@ -547,7 +550,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         }
       }
     }
-  } else if (warp == 1 || warp == NTHB / 32 - 1) {   // warp 1: dQ MMAs; last warp: S / dP MMAs
+  } else if (warp == 1 || warp >= NTHB / 32 - 2) {   // warp 1: dQ MMAs; last warp: S / dP MMAs
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
@@ -558,15 +561,18 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::tc_fence_after();
         const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024), dO0 = ptx::make_smem_desc(sdO, 16, 1024);
         const uint64_t dKs = ptx::make_smem_desc(sK(st), 16, 1024), dVs = ptx::make_smem_desc(sV(st), 16, 1024);
+        if (warp == NTHB / 32 - 1) {
 #pragma unroll
-        for (int ks = 0; ks < DH / 16; ks++) {
-          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tS + tb * BT, desc_adv(dQ0, ob), desc_adv(dKs, os), idesc_s, ks != 0);
-        }
+          for (int ks = 0; ks < DH / 16; ks++) {
+            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            ptx::mma_f16_ss(tS + tb * BT, desc_adv(dQ0, ob), desc_adv(dKs, os), idesc_s, ks != 0);
+          }
+        } else {
 #pragma unroll
-        for (int ks = 0; ks < DH / 16; ks++) {
-          const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tdP + tb * BT, desc_adv(dO0, ob), desc_adv(dVs, os), idesc_s, ks != 0);
+          for (int ks = 0; ks < DH / 16; ks++) {
+            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            ptx::mma_f16_ss(tdP + tb * BT, desc_adv(dO0, ob), desc_adv(dVs, os), idesc_s, ks != 0);
+          }
         }
         ptx::mma_commit(s_full0 + 8 * tb);
       };

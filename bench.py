@@ -166,6 +166,17 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(ms, world, device):
+    """Replicas-only scaling: the step time of the job is the slowest rank's; every rank gets it."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
@@ -247,12 +258,7 @@ def run_ours(args, cfg):
             fn()
         e1.record()
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
 
     for _ in range(max(args.warmup, 3)):
         step()

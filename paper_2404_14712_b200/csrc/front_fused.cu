@@ -28,6 +28,7 @@ namespace orbit {
 namespace {
 
 constexpr int HP = FE_HP;
+constexpr int HG = 8;     // heads per pass of fe_patch_fwd
 
 template <typename T> struct Pair;
 template <> struct Pair<float> {
@@ -123,69 +124,82 @@ __global__ void __launch_bounds__(256) fe_patch_fwd_kernel(const float* __restri
   const int gw = Wg / P, L = (Hg / P) * gw, KVp = R * Vp;
   for (int bl = warp0; bl < BL; bl += nwarps) {
     const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
-    float pix[E][P2], s[E][HP];
+    float pix[E][P2];
 #pragma unroll
     for (int e = 0; e < E; e++) {
       const int v = 64 * (e >> 1) + 2 * lane + (e & 1);
-      if (v < V) {
-        load_pix<P>(x, V, Hg, Wg, b, v, i, j, pix[e]);
-        const float4* g4 = reinterpret_cast<const float4*>(G + ((size_t)P2 * Vp + v) * HP);
-#pragma unroll
-        for (int q = 0; q < HP / 4; q++) {
-          const float4 g = __ldg(g4 + q);
-          s[e][4 * q] = g.x; s[e][4 * q + 1] = g.y; s[e][4 * q + 2] = g.z; s[e][4 * q + 3] = g.w;
-        }
-#pragma unroll
-        for (int r = 0; r < P2; r++) {
-          const float4* gr = reinterpret_cast<const float4*>(G + ((size_t)r * Vp + v) * HP);
-#pragma unroll
-          for (int q = 0; q < HP / 4; q++) {
-            const float4 g = __ldg(gr + q);
-            s[e][4 * q] = fmaf(pix[e][r], g.x, s[e][4 * q]);
-            s[e][4 * q + 1] = fmaf(pix[e][r], g.y, s[e][4 * q + 1]);
-            s[e][4 * q + 2] = fmaf(pix[e][r], g.z, s[e][4 * q + 2]);
-            s[e][4 * q + 3] = fmaf(pix[e][r], g.w, s[e][4 * q + 3]);
-          }
-        }
-      } else {
+      if (v < V) load_pix<P>(x, V, Hg, Wg, b, v, i, j, pix[e]);
+      else {
 #pragma unroll
         for (int r = 0; r < P2; r++) pix[e][r] = 0.f;
-#pragma unroll
-        for (int a = 0; a < HP; a++) s[e][a] = -INFINITY;
       }
     }
-    // softmax over the variables, per head (R3): alpha replaces s
+    // heads in groups of HG = 8: 16 score accumulators per variable pair at a time keep the kernel at ~128 registers
+    // (all 16 heads at once needed 255 registers and left 12 % occupancy on a purely HBM-bound kernel)
+#pragma unroll 1
+    for (int a0 = 0; a0 < h; a0 += HG) {
+      float s[E][HG];
 #pragma unroll
-    for (int a = 0; a < HP; a++) {
-      if (a < h) {
-        float m = s[0][a];
+      for (int e = 0; e < E; e++) {
+        const int v = 64 * (e >> 1) + 2 * lane + (e & 1);
+        if (v < V) {
+          const float4* g4 = reinterpret_cast<const float4*>(G + ((size_t)P2 * Vp + v) * HP + a0);
 #pragma unroll
-        for (int e = 1; e < E; e++) m = fmaxf(m, s[e][a]);
-        m = warp_max(m);
-        float sum = 0.f;
+          for (int q = 0; q < HG / 4; q++) {
+            const float4 g = __ldg(g4 + q);
+            s[e][4 * q] = g.x; s[e][4 * q + 1] = g.y; s[e][4 * q + 2] = g.z; s[e][4 * q + 3] = g.w;
+          }
 #pragma unroll
-        for (int e = 0; e < E; e++) { s[e][a] = __expf(s[e][a] - m); sum += s[e][a]; }
-        sum = warp_sum(sum);
-        const float inv = 1.f / sum;
+          for (int r = 0; r < P2; r++) {
+            const float4* gr = reinterpret_cast<const float4*>(G + ((size_t)r * Vp + v) * HP + a0);
 #pragma unroll
-        for (int e = 0; e < E; e++) s[e][a] *= inv;
+            for (int q = 0; q < HG / 4; q++) {
+              const float4 g = __ldg(gr + q);
+              s[e][4 * q] = fmaf(pix[e][r], g.x, s[e][4 * q]);
+              s[e][4 * q + 1] = fmaf(pix[e][r], g.y, s[e][4 * q + 1]);
+              s[e][4 * q + 2] = fmaf(pix[e][r], g.z, s[e][4 * q + 2]);
+              s[e][4 * q + 3] = fmaf(pix[e][r], g.w, s[e][4 * q + 3]);
+            }
+          }
+        } else {
+#pragma unroll
+          for (int aa = 0; aa < HG; aa++) s[e][aa] = -INFINITY;
+        }
       }
-    }
-    // alpha [BL, h, Vp] fp32 and A [BL, h, R*Vp] (k = r*Vp + v); padded variables get exact zeros
+      // softmax over the variables, per head (R3): alpha replaces s
 #pragma unroll
-    for (int a = 0; a < HP; a++) {
-      if (a < h) {
+      for (int aa = 0; aa < HG; aa++) {
+        if (a0 + aa < h) {
+          float m = s[0][aa];
 #pragma unroll
-        for (int n = 0; n < NV; n++) {
-          const int v0 = 64 * n + 2 * lane;
-          if (v0 < Vp) {
-            const float a0 = s[2 * n][a], a1 = s[2 * n + 1][a];
-            *reinterpret_cast<float2*>(alpha + ((size_t)bl * h + a) * Vp + v0) = make_float2(a0, a1);
-            T* row = A + ((size_t)bl * h + a) * KVp + v0;
+          for (int e = 1; e < E; e++) m = fmaxf(m, s[e][aa]);
+          m = warp_max(m);
+          float sum = 0.f;
 #pragma unroll
-            for (int r = 0; r < P2; r++)
-              *reinterpret_cast<pair_t*>(row + (size_t)r * Vp) = Pair<T>::make(a0 * pix[2 * n][r], a1 * pix[2 * n + 1][r]);
-            *reinterpret_cast<pair_t*>(row + (size_t)P2 * Vp) = Pair<T>::make(a0, a1);
+          for (int e = 0; e < E; e++) { s[e][aa] = __expf(s[e][aa] - m); sum += s[e][aa]; }
+          sum = warp_sum(sum);
+          const float inv = 1.f / sum;
+#pragma unroll
+          for (int e = 0; e < E; e++) s[e][aa] *= inv;
+        }
+      }
+      // alpha [BL, h, Vp] fp32 and A [BL, h, R*Vp] (k = r*Vp + v); padded variables get exact zeros
+#pragma unroll
+      for (int aa = 0; aa < HG; aa++) {
+        if (a0 + aa < h) {
+          const int a = a0 + aa;
+#pragma unroll
+          for (int n = 0; n < NV; n++) {
+            const int v0 = 64 * n + 2 * lane;
+            if (v0 < Vp) {
+              const float w0 = s[2 * n][aa], w1 = s[2 * n + 1][aa];
+              *reinterpret_cast<float2*>(alpha + ((size_t)bl * h + a) * Vp + v0) = make_float2(w0, w1);
+              T* row = A + ((size_t)bl * h + a) * KVp + v0;
+#pragma unroll
+              for (int r = 0; r < P2; r++)
+                *reinterpret_cast<pair_t*>(row + (size_t)r * Vp) = Pair<T>::make(w0 * pix[2 * n][r], w1 * pix[2 * n + 1][r]);
+              *reinterpret_cast<pair_t*>(row + (size_t)P2 * Vp) = Pair<T>::make(w0, w1);
+            }
           }
         }
       }

@@ -126,6 +126,13 @@ int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, 
 int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
                   const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
                   int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s);
+// TMA-staged variants (layernorm_tma.cu), same contracts; used whenever two row stages fit in shared memory
+bool layernorm_tma_supported(int D, int x_dt, int dout_dt /* -1: forward */, int add_dt, bool has_add);
+int layernorm_fwd_tma(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,
+                     float* mean, float* rstd, int M, int D, float eps, void* x_copy, cudaStream_t s);
+int layernorm_bwd_tma(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
+                     const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
+                     int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s);
 // out[n] = sum_m in[m*ld + n]  (fp32 atomics into acc, caller zeroes) ; optional bf16/f32 copy of `in`
 int colsum(const void* in, int in_dt, long long ld, int M, int N, float* acc, void* copy_out, int copy_dt,
            long long ld_copy, cudaStream_t s);

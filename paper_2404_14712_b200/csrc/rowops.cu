@@ -1,40 +1,12 @@
 // rowops.cu -- HBM-bound row-wise kernels: LayerNorm fwd/bwd, column sums (bias grads), casts, combines.
 // All are one pass over their inputs with 16-byte vector accesses; statistics and sums in fp32.
 #include "common.cuh"
+#include "vec8.cuh"
+#include <stdlib.h>
 
 namespace orbit {
 
 namespace {
-
-// 8 consecutive elements starting at element index i (i % 8 == 0, base 16B aligned)
-__device__ __forceinline__ void ld8(const void* p, size_t i, int dt, float* v) {
-  if (dt == ORBIT_BF16) {
-    uint4 raw = *reinterpret_cast<const uint4*>((const bf16*)p + i);
-    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&raw);
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-      float2 f = __bfloat1622float2(h[j]);
-      v[2 * j] = f.x; v[2 * j + 1] = f.y;
-    }
-  } else {
-    const float4* q = reinterpret_cast<const float4*>((const float*)p + i);
-    float4 a = q[0], b = q[1];
-    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-  }
-}
-__device__ __forceinline__ void st8(void* p, size_t i, int dt, const float* v) {
-  if (dt == ORBIT_BF16) {
-    uint4 raw;
-    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&raw);
-#pragma unroll
-    for (int j = 0; j < 4; j++) h[j] = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
-    *reinterpret_cast<uint4*>((bf16*)p + i) = raw;
-  } else {
-    float4* q = reinterpret_cast<float4*>((float*)p + i);
-    q[0] = make_float4(v[0], v[1], v[2], v[3]);
-    q[1] = make_float4(v[4], v[5], v[6], v[7]);
-  }
-}
 
 __device__ __forceinline__ float2 block_sum2(float2 v, float2* sh) {
   int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
@@ -313,6 +285,12 @@ __global__ void mse_kernel(const void* __restrict__ y, const void* __restrict__ 
   if (threadIdx.x == 0) atomicAdd(loss, acc * inv);
 }
 
+// TMA-staged kernels (layernorm_tma.cu) unless the row does not fit two stages or ORBIT_LN_ONEBLOCK=1 (A/B timing)
+bool ln_use_tma(int D, int x_dt, int dout_dt, int add_dt, bool has_add) {
+  static int forced = -1;
+  if (forced < 0) { const char* e = getenv("ORBIT_LN_ONEBLOCK"); forced = (e && e[0] == '1') ? 1 : 0; }
+  return !forced && layernorm_tma_supported(D, x_dt, dout_dt, add_dt, has_add);
+}
 int ln_threads(int D) {
   int nch = D / 8;
   int t = ((nch + 31) / 32) * 32;
@@ -322,6 +300,7 @@ int ln_threads(int D) {
 
 int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,
                   float* mean, float* rstd, int M, int D, float eps, void* x_copy, cudaStream_t s) {
+  if (ln_use_tma(D, x_dt, -1, 0, false)) return layernorm_fwd_tma(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy, s);
   int thr = ln_threads(D);
   int maxch = cdiv(D / 8, thr);
   int grid = M < 148 * 4 ? M : 148 * 4;
@@ -337,6 +316,9 @@ int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, 
 int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
                   const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
                   int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s) {
+  if (ln_use_tma(D, x_dt, dout_dt, add_dt, add != nullptr))
+    return layernorm_bwd_tma(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, dx_f32, dx_out, out_dt, dgamma_acc,
+                            dbeta_acc, M, D, s);
   // <= 512 threads once a thread owns more than one 8-column chunk: the per-column dgamma/dbeta accumulators
   // (16 registers per chunk) then fit without spills
   const int nch = D / 8;

@@ -212,6 +212,20 @@ int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long
 int orbit_debug_gemm_batched(int M, int N, int K, int batch, orbit_dtype dtype, const void* A, long long a_rs,
                              long long a_cs, long long a_bs, const void* B, long long b_rs, long long b_cs,
                              long long b_bs, float* C, long long ldc, long long c_bs, void* stream);
+/* Kernel-level diagnostic: the LayerNorm kernels of orbit_block_fwd / orbit_block_bwd on their own (the
+ * pre-LN sub-layers; SURVEY.md 8(c) BLK / BLK').  Row-major [M, D], D % 8 == 0, all pointers device memory.
+ * fwd: out = (x - mean) * rstd * gamma + beta with biased variance; mean, rstd [M] fp32 are written.
+ * bwd: dx = add (nullable) + dz(dout; x, mean, rstd, gamma), written as fp32 to dx_f32 (nullable) and as out_dtype to
+ *      dx_out (nullable); dgamma_acc / dbeta_acc [D] fp32 are ACCUMULATED into (the caller zeroes them).
+ * Errors: ORBIT_ERR_NULL, ORBIT_ERR_DTYPE, ORBIT_ERR_SHAPE (M <= 0, D % 8 != 0), ORBIT_ERR_CUDA. */
+int orbit_debug_layernorm_fwd(int M, int D, orbit_dtype x_dtype, orbit_dtype p_dtype, orbit_dtype out_dtype, float eps,
+                              const void* x, const void* gamma, const void* beta, void* out, float* mean, float* rstd,
+                              void* stream);
+int orbit_debug_layernorm_bwd(int M, int D, orbit_dtype dout_dtype, orbit_dtype x_dtype, orbit_dtype p_dtype,
+                              orbit_dtype add_dtype, orbit_dtype out_dtype, const void* dout, const void* x,
+                              const float* mean, const float* rstd, const void* gamma, const void* add /*nullable*/,
+                              float* dx_f32 /*nullable*/, void* dx_out /*nullable*/, float* dgamma_acc, float* dbeta_acc,
+                              void* stream);
 
 #ifdef __cplusplus
 }

@@ -143,6 +143,8 @@ _proto("orbit_profile_gemm_collect", C.c_int, [C.POINTER(C.c_double), C.POINTER(
 _proto("orbit_debug_gemm", C.c_int, [C.c_int] * 4 + [_vp, C.c_longlong, C.c_longlong, _vp, C.c_longlong, C.c_longlong, _vp, _vp])
 _ll = C.c_longlong
 _proto("orbit_debug_gemm_batched", C.c_int, [C.c_int] * 5 + [_vp, _ll, _ll, _ll, _vp, _ll, _ll, _ll, _vp, _ll, _ll, _vp])
+_proto("orbit_debug_layernorm_fwd", C.c_int, [C.c_int] * 5 + [C.c_float] + [_vp] * 7)
+_proto("orbit_debug_layernorm_bwd", C.c_int, [C.c_int] * 7 + [_vp] * 11)
 
 EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace_bytes", "orbit_var_aggregate",
            "orbit_var_aggregate_bwd", "orbit_var_aggregate_workspace_bytes",
@@ -154,7 +156,8 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_profile_gemm_collect", "orbit_embed_fused", "orbit_embed_fused_bwd",
            "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
            "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched", "orbit_head_loss", "orbit_head_loss_bwd",
-           "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes"]
+           "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes",
+           "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -355,6 +358,20 @@ def orbit_debug_gemm(M, N, K, dtype, A, a_rs, a_cs, B, b_rs, b_cs, Cout, stream=
 def orbit_debug_gemm_batched(M, N, K, batch, dtype, A, a_rs, a_cs, a_bs, B, b_rs, b_cs, b_bs, Cout, ldc, c_bs, stream=None):
     _check(lib.orbit_debug_gemm_batched(M, N, K, batch, DTYPES[dtype], _ptr(A), a_rs, a_cs, a_bs, _ptr(B), b_rs, b_cs, b_bs,
                                         _ptr(Cout), ldc, c_bs, _stream(stream)), "orbit_debug_gemm_batched")
+
+
+def orbit_debug_layernorm_fwd(M, D, x_dt, p_dt, out_dt, eps, x, gamma, beta, out, mean, rstd, stream=None):
+    _check(lib.orbit_debug_layernorm_fwd(M, D, DTYPES[x_dt], DTYPES[p_dt], DTYPES[out_dt], eps, _ptr(x), _ptr(gamma),
+                                         _ptr(beta), _ptr(out), _ptr(mean), _ptr(rstd), _stream(stream)),
+           "orbit_debug_layernorm_fwd")
+
+
+def orbit_debug_layernorm_bwd(M, D, dout_dt, x_dt, p_dt, add_dt, out_dt, dout, x, mean, rstd, gamma, add, dx_f32, dx_out,
+                              dgamma_acc, dbeta_acc, stream=None):
+    _check(lib.orbit_debug_layernorm_bwd(M, D, DTYPES[dout_dt], DTYPES[x_dt], DTYPES[p_dt], DTYPES[add_dt], DTYPES[out_dt],
+                                         _ptr(dout), _ptr(x), _ptr(mean), _ptr(rstd), _ptr(gamma), _ptr(add), _ptr(dx_f32),
+                                         _ptr(dx_out), _ptr(dgamma_acc), _ptr(dbeta_acc), _stream(stream)),
+           "orbit_debug_layernorm_bwd")
 
 
 def orbit_profile_gemm(on: bool):

@@ -116,6 +116,32 @@ int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long
   return gemm(g, (cudaStream_t)stream);
 }
 
+int orbit_debug_layernorm_fwd(int M, int D, orbit_dtype x_dtype, orbit_dtype p_dtype, orbit_dtype out_dtype, float eps,
+                              const void* x, const void* gamma, const void* beta, void* out, float* mean, float* rstd,
+                              void* stream) {
+  if (!x || !gamma || !beta || !out || !mean || !rstd) { set_error("debug_layernorm_fwd: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!valid_dtype(x_dtype) || !valid_dtype(p_dtype) || !valid_dtype(out_dtype)) { set_error("debug_layernorm_fwd: bad dtype"); return ORBIT_ERR_DTYPE; }
+  if (M <= 0 || D <= 0 || D % 8) { set_error("debug_layernorm_fwd: bad shape M=%d D=%d", M, D); return ORBIT_ERR_SHAPE; }
+  ORBIT_TRY(check_device());
+  return layernorm_fwd(x, x_dtype, gamma, beta, p_dtype, out, out_dtype, mean, rstd, M, D, eps, nullptr, (cudaStream_t)stream);
+}
+
+int orbit_debug_layernorm_bwd(int M, int D, orbit_dtype dout_dtype, orbit_dtype x_dtype, orbit_dtype p_dtype,
+                              orbit_dtype add_dtype, orbit_dtype out_dtype, const void* dout, const void* x,
+                              const float* mean, const float* rstd, const void* gamma, const void* add, float* dx_f32,
+                              void* dx_out, float* dgamma_acc, float* dbeta_acc, void* stream) {
+  if (!dout || !x || !mean || !rstd || !gamma || !dgamma_acc || !dbeta_acc || (!dx_f32 && !dx_out)) {
+    set_error("debug_layernorm_bwd: NULL pointer"); return ORBIT_ERR_NULL;
+  }
+  if (!valid_dtype(dout_dtype) || !valid_dtype(x_dtype) || !valid_dtype(p_dtype) || !valid_dtype(add_dtype) || !valid_dtype(out_dtype)) {
+    set_error("debug_layernorm_bwd: bad dtype"); return ORBIT_ERR_DTYPE;
+  }
+  if (M <= 0 || D <= 0 || D % 8) { set_error("debug_layernorm_bwd: bad shape M=%d D=%d", M, D); return ORBIT_ERR_SHAPE; }
+  ORBIT_TRY(check_device());
+  return layernorm_bwd(dout, dout_dtype, x, x_dtype, mean, rstd, gamma, p_dtype, add, add_dtype, dx_f32, dx_out, out_dtype,
+                       dgamma_acc, dbeta_acc, M, D, (cudaStream_t)stream);
+}
+
 int orbit_mse_loss_grad(orbit_dtype dtype, size_t n, const void* y, const void* t, void* dy, float* loss, void* stream) {
   if (!y || !t || !dy || !loss) { set_error("mse: NULL pointer"); return ORBIT_ERR_NULL; }
   if (!valid_dtype(dtype)) { set_error("mse: bad dtype"); return ORBIT_ERR_DTYPE; }

@@ -57,17 +57,17 @@ def step_flops(cfg):
 # ------------------------------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle on a bounded sample
 # ------------------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, n_tokens):
-    """Block fwd+bwd of the oracle at cfg's widths on n_tokens tokens (B=1).  Returns a closure running one
+def oracle_sample(cfg, n_tokens, batch=1):
+    """Block fwd+bwd of the oracle at cfg's widths on `batch` samples of n_tokens tokens.  Returns a closure running one
     sample step and the sample's model FLOPs.  Weights are widened to float64 outside the timed call (input
     preparation, not arithmetic of the method)."""
     from oracle import orbit_oracle as orc
     seed = syn.seed_of(cfg.name)
     P = syn.block_params(seed, cfg.D, cfg.F, cfg.dtype)
     P = {k: np.asarray(v, dtype=np.float64) for k, v in P.items()}
-    x = np.asarray(syn.normal(seed, "blk.x", (1, n_tokens, cfg.D), dtype=cfg.resid_dtype), dtype=np.float64)
-    dy = np.asarray(syn.normal(seed, "blk.dy", (1, n_tokens, cfg.D), dtype=cfg.resid_dtype), dtype=np.float64)
-    flops = 3.0 * (2.0 * n_tokens * cfg.D * (4 * cfg.D + 2 * cfg.F) + 4.0 * n_tokens * n_tokens * cfg.D)
+    x = np.asarray(syn.normal(seed, "blk.x", (batch, n_tokens, cfg.D), dtype=cfg.resid_dtype), dtype=np.float64)
+    dy = np.asarray(syn.normal(seed, "blk.dy", (batch, n_tokens, cfg.D), dtype=cfg.resid_dtype), dtype=np.float64)
+    flops = batch * 3.0 * (2.0 * n_tokens * cfg.D * (4 * cfg.D + 2 * cfg.F) + 4.0 * n_tokens * n_tokens * cfg.D)
 
     def run():
         y, cache = orc.block_fwd(x, P, cfg.heads, cfg.ln_eps)
@@ -166,6 +166,63 @@ class ClockSampler:
         return out
 
 
+class HostPipeline:
+    """The end-to-end leg's input / output plumbing: every step copies its inputs from pinned host memory and its
+    results back to pinned host memory, as a training loop with a prefetching loader does -- the copies run on their
+    own streams and overlap the neighbouring steps' kernels.  Inputs are double buffered on the device (step i+1's
+    batch lands while step i computes); results are snapshotted device-to-device on the compute stream (so the next
+    step may overwrite them) and drained to the host on the read-back stream.  Every copy of every step is inside
+    the timed region: finish() makes the compute stream wait for the last read-back before the closing event."""
+
+    def __init__(self, host_in, host_out):
+        import torch
+        self.torch = torch
+        self.host_in, self.host_out = host_in, host_out
+        self.h2d, self.d2h = torch.cuda.Stream(), torch.cuda.Stream()
+        self.slots = [[torch.empty(h.shape, dtype=h.dtype, device="cuda") for h in host_in] for _ in range(2)]
+        self.stage = [torch.empty(h.shape, dtype=h.dtype, device="cuda") for h in host_out]
+        self.slot_free = [None, None]
+        self.drained = None
+        self.i = 0
+
+    def inputs(self):
+        torch = self.torch
+        cur = torch.cuda.current_stream()
+        k = self.i % 2
+        self.k = k
+        with torch.cuda.stream(self.h2d):
+            if self.slot_free[k] is not None:
+                self.h2d.wait_event(self.slot_free[k])          # the step that last read this slot has finished
+            for d, h in zip(self.slots[k], self.host_in):
+                d.copy_(h, non_blocking=True)
+            ready = torch.cuda.Event()
+            ready.record(self.h2d)
+        cur.wait_event(ready)
+        return self.slots[k]
+
+    def outputs(self, dev_out):
+        torch = self.torch
+        cur = torch.cuda.current_stream()
+        if self.drained is not None:
+            cur.wait_event(self.drained)                        # previous read-back has left the snapshot buffers
+        for st, d in zip(self.stage, dev_out):
+            st.copy_(d.view(st.shape), non_blocking=True)
+        done = torch.cuda.Event()
+        done.record(cur)
+        self.slot_free[self.k] = done
+        with torch.cuda.stream(self.d2h):
+            self.d2h.wait_event(done)
+            for h, st in zip(self.host_out, self.stage):
+                h.copy_(st, non_blocking=True)
+            self.drained = torch.cuda.Event()
+            self.drained.record(self.d2h)
+        self.i += 1
+
+    def finish(self):
+        if self.drained is not None:
+            self.torch.cuda.current_stream().wait_event(self.drained)
+
+
 def max_over_ranks(ms, world, device):
     """Replicas-only scaling: the step time of the job is the slowest rank's; every rank gets it."""
     if world <= 1:
@@ -211,13 +268,13 @@ def run_ours(args, cfg):
         h2d = hx.numel() * hx.element_size() * 2
         d2h = h2d
 
+        pipe = HostPipeline([hx, hdy], [hy, hdx])
+
         def step_e2e():
-            x_d.copy_(hx, non_blocking=True)
-            dy_d.copy_(hdy, non_blocking=True)
-            sr.forward(x_d)
-            sr.backward(dy_d)
-            hy.copy_(sr.blocks[-1].y, non_blocking=True)
-            hdx.copy_(sr.blocks[0].dx, non_blocking=True)
+            xs, dys = pipe.inputs()
+            sr.forward(xs)
+            sr.backward(dys)
+            pipe.outputs([sr.blocks[-1].y, sr.blocks[0].dx])
     else:
         emb = syn.embed_params(seed, cfg.V, cfg.p, cfg.D, cfg.dtype)
         agg = syn.agg_params(seed, cfg.D, cfg.dtype)
@@ -239,23 +296,26 @@ def run_ours(args, cfg):
         h2d = hx.numel() * 4 + ht.numel() * ht.element_size()
         d2h = 4
 
+        pipe = HostPipeline([hx, ht], [hloss])
+
         def step_e2e():
-            x_d.copy_(hx, non_blocking=True)
-            t_d.copy_(ht, non_blocking=True)
-            sr.step(x_d, t_d)
-            hloss.copy_(sr.loss, non_blocking=True)
+            xs, ts = pipe.inputs()
+            sr.step(xs, ts)
+            pipe.outputs([sr.loss])
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(fn, steps):
+    def timed(fn, steps, finish=None):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record()
         for _ in range(steps):
             fn()
+        if finish:
+            finish()
         e1.record()
         barrier()
         return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
@@ -275,7 +335,7 @@ def run_ours(args, cfg):
     # ---- end to end through the public API with host buffers ----
     for _ in range(2):
         step_e2e()
-    ms_e2e = timed(step_e2e, args.steps)
+    ms_e2e = timed(step_e2e, args.steps, pipe.finish)
 
     flops = step_flops(cfg)
     ms_step = ms / args.steps
@@ -308,13 +368,15 @@ def run_ours(args, cfg):
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only) ----
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        n_tok = 64 if cfg.D >= 8192 else 256
-        run, sflops = oracle_sample(cfg, n_tok)
+        # about 10-30 s of CPU work: C5 1024 tokens, C4 one whole sample, C3 two samples, C2 the whole batch
+        n_tok = 1024 if cfg.D >= 8192 else cfg.L
+        nb = 1 if cfg.D >= 4096 else min(cfg.B, 2 if cfg.D >= 2048 else cfg.B)
+        run, sflops = oracle_sample(cfg, n_tok, nb)
         t0 = time.perf_counter()
         run()
         dt = time.perf_counter() - t0
         cpu = {"value": sflops / dt / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
-               "sample": f"oracle block fwd+bwd at {cfg.name} widths on {n_tok} of {cfg.L} tokens (B=1), fp64 "
+               "sample": f"oracle block fwd+bwd at {cfg.name} widths on {nb} x {n_tok} of {cfg.B} x {cfg.L} tokens, fp64 "
                          f"numpy/OpenBLAS, {dt:.1f} s"}
     line = {
         "metric": METRIC, "value": tflops, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -330,7 +392,8 @@ def run_ours(args, cfg):
         "frac_of_peak_nominal_2250": tflops / world / 2250.0,
         "clocks": clocks,
         "e2e": {"value": tflops_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": ms_e2e / args.steps},
+                "ms_per_step": ms_e2e / args.steps,
+                "overlap": "every step's H2D / D2H runs on copy streams (double-buffered inputs, snapshotted results) inside the timed region"},
         "gpu_launches": int(launches),
         "roofline": roofline,
         "cpu_baseline": cpu,

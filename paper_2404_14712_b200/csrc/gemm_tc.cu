@@ -194,7 +194,7 @@ EncodeTiledFn get_encode() {
 // bf16 tensor map over `batch` 2-D problems `bstride` elements apart: `inner` contiguous elements, `outer` rows `ld`
 // elements apart; 128B swizzle; box = box_inner x box_outer x 1 (out-of-bounds elements read as zero per problem)
 int make_map(CUtensorMap* m, const void* base, long long inner, long long outer, long long ld, int box_inner,
-             int box_outer, int batch, long long bstride) {
+             int box_outer, int batch, long long bstride, CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_128B) {
   EncodeTiledFn enc = get_encode();
   if (!enc) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
   if (batch <= 1) { batch = 1; bstride = ld * outer; }
@@ -204,7 +204,7 @@ int make_map(CUtensorMap* m, const void* base, long long inner, long long outer,
   cuuint32_t box[3] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer, 1};
   cuuint32_t es[3] = {1, 1, 1};
   CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     set_error("cuTensorMapEncodeTiled failed (%d): inner=%lld outer=%lld ld=%lld box=%dx%d batch=%d bstride=%lld", (int)r,
@@ -260,8 +260,8 @@ int launch_bn(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, b
 }
 }  // namespace
 
-int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, bool a_mn, bool b_mn, int sms,
-                    cudaStream_t s);   // gemm_tc2.cu
+int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const GemmArgs& g, bool a_mn, bool b_mn,
+                    int sms, cudaStream_t s);   // gemm_tc2.cu
 
 int gemm_profile_enable(int on) {
   if (on && !g_prof.ev) {
@@ -320,9 +320,15 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   else      ORBIT_TRY(make_map(&ma, g.A, g.K, g.M, g.a_rs, 64, BM, g.batch, g.a_bs));   // [M rows, K contiguous]
   if (b_mn) ORBIT_TRY(make_map(&mb, g.B, g.N, g.K, g.b_rs, 64, 64, g.batch, g.b_bs));   // [K rows, N contiguous]
   else      ORBIT_TRY(make_map(&mb, g.B, g.K, g.N, g.b_cs, 64, bn, g.batch, g.b_bs));   // [N rows, K contiguous]
+  // plain bf16 outputs (weight gradients, QKV, dO) leave the CTA-pair kernel through TMA stores; g_force_simt == 5
+  // keeps the direct row-per-thread stores (A/B comparison)
+  CUtensorMap mc;
+  const bool store_map = pair && g_force_simt != 5 && g.out_dtype == ORBIT_BF16 && !g.resid && !g.accumulate &&
+                         g.act == ACT_NONE && !g.aux_out && !g.aux_in;
+  if (store_map) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 32, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B));
   const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
   if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
-  if (pair) ORBIT_TRY(gemm_tc2_launch(ma, mb, g, a_mn, b_mn, num_sms(), s));
+  if (pair) ORBIT_TRY(gemm_tc2_launch(ma, mb, store_map ? &mc : nullptr, g, a_mn, b_mn, num_sms(), s));
   else if (bn == 128) ORBIT_TRY(launch_bn<128>(ma, mb, g, a_mn, b_mn, s));
   else ORBIT_TRY(launch_bn<256>(ma, mb, g, a_mn, b_mn, s));
   if (rec) {

@@ -24,7 +24,19 @@ constexpr int B_BYTES = 128 * BK * 2;           // this CTA's half of B
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
 constexpr int NTHREADS = 320;                   // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (2 per TMEM lane quarter)
 constexpr int TMEM_COLS = 512;
-constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 + 256;
+// epilogue staging for the TMA-store path: per epilogue warp two [32 rows x 32 bf16] boxes (64-byte rows, 64B swizzle)
+constexpr int EPI_BOX_BYTES = 32 * 32 * 2;
+constexpr int EPI_BYTES = 8 * 2 * EPI_BOX_BYTES;    // 32 KB
+constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + EPI_BYTES + 1024 + 256;
+
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(m), "r"(src), "r"(c0),
+               "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 __device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, int& mb, int& nb) {
   constexpr int GROUP = 8;                      // 8 x 256 rows of A shared through L2 by concurrent clusters
@@ -38,11 +50,13 @@ __device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, in
 
 template <int A_MN, int B_MN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
-gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, epi::Args e0, int M, int N, int K,
+gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                const __grid_constant__ CUtensorMap tmC, int tma_store, epi::Args e0, int M, int N, int K,
                 int batch, long long c_bs, long long bias_bs) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+  const uint32_t epi_base = smem_base + STAGES * STAGE_BYTES;
+  const uint32_t bar_base = epi_base + EPI_BYTES;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
   auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * STAGES + a); };
@@ -61,6 +75,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmA);
     ptx::prefetch_tmap(&tmB);
+    if (tma_store) ptx::prefetch_tmap(&tmC);
     for (int s = 0; s < STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
     for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 16); }
     ptx::fence_barrier_init();
@@ -140,6 +155,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int quarter = warp & 3;                // TMEM lanes [32*quarter, +32)
     const int chalf = (warp - 2) >> 2;           // which 128 of the 256 accumulator columns
     int acc = 0; uint32_t aph = 0;
+    uint32_t ebuf = 0;
     for (int t = cluster_id; t < num_tiles; t += num_clusters) {
       const int bi = t / tiles_per_batch;
       int mb, nb;
@@ -152,6 +168,46 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + acc * BN2 + ((uint32_t)(quarter * 32) << 16);
       const int rrow = e.resid_row_mod > 0 ? (row % e.resid_row_mod) : row;
+      if (tma_store) {
+        // plain bf16 output (+ bias): 32 x 32 boxes through shared memory, written back by TMA as full 64-byte row
+        // segments (the row-per-thread direct stores below touch 32 different lines per instruction, which made the
+        // K = 2048 weight-gradient GEMMs epilogue-bound)
+        const int wrow0 = mb * BM2 + (int)rank * 128 + quarter * 32;
+#pragma unroll 1
+        for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
+          uint32_t r[32];
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          const int col0 = n0 + c * 32;
+          if (lane == 0) bulk_wait_read<1>();            // the store issued two chunks ago has left this buffer
+          __syncwarp();
+          const uint32_t buf = epi_base + (uint32_t)(warp - 2) * (2 * EPI_BOX_BYTES) + ebuf * EPI_BOX_BYTES;
+#pragma unroll
+          for (int g8 = 0; g8 < 4; g8++) {
+            float v[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = __uint_as_float(r[g8 * 8 + j]);
+            if (e.bias && col0 + g8 * 8 < N) {
+              float b[8];
+              epi::load8(e.bias, col0 + g8 * 8, e.bias_dt, b);
+#pragma unroll
+              for (int j = 0; j < 8; j++) v[j] += b[j];
+            }
+            uint32_t pk[4];
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+              __nv_bfloat162 t2 = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+              pk[j] = *reinterpret_cast<uint32_t*>(&t2);
+            }
+            const uint32_t addr = buf + lane * 64 + ((g8 ^ ((lane >> 1) & 3)) << 4);
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+          }
+          ptx::fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) { tma_store_3d(&tmC, buf, col0, wrow0, bi); bulk_commit(); }
+          ebuf ^= 1;
+        }
+      } else {
 #pragma unroll 1
       for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
         uint32_t r[32];
@@ -159,11 +215,13 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         ptx::tmem_ld_wait();
         if (row < M) epi::chunk32(e, r, row, rrow, n0 + c * 32, N);
       }
+      }
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), 0));
       if (++acc == 2) { acc = 0; aph ^= 1; }
     }
+    if (tma_store && lane == 0) bulk_wait_all();   // the staging buffers (and the writes) outlive the last store
   }
   ptx::tc_fence_before();
   ptx::cluster_sync_all();                       // peer smem / barriers stay alive until both CTAs are done
@@ -174,7 +232,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 }
 
 template <int A_MN, int B_MN>
-int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, int sms, cudaStream_t s) {
+int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const GemmArgs& g, int sms, cudaStream_t s) {
   const epi::Args e = epi::from_gemm(g);
   const int M = g.M, N = g.N, K = g.K, batch = g.batch > 1 ? g.batch : 1;
   static bool attr_set = false;
@@ -186,19 +244,21 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, int
   const long long tiles = (long long)cdiv(M, BM2) * cdiv(N, BN2) * batch;
   int clusters = sms / 2;
   if (tiles < clusters) clusters = (int)tiles;
-  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, e, M, N, K, batch, g.c_bs, g.bias_bs);
+  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, mc ? *mc : ma, mc ? 1 : 0, e, M, N, K, batch,
+                                                                         g.c_bs, g.bias_bs);
   return ORBIT_OK;
 }
 }  // namespace
 
 // called by gemm_tc() (gemm_tc.cu), which builds the tensor maps: A boxes as in the 1-CTA kernel, B boxes with
 // 128 rows (K-major) or 64 x 64 (N-major)
-int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, bool a_mn, bool b_mn, int sms,
-                    cudaStream_t s) {
-  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, g, sms, s);
-  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, g, sms, s);
-  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, g, sms, s);
-  return launch2<1, 0>(ma, mb, g, sms, s);
+// mc: tensor map of C for the TMA-store epilogue (32 x 32 bf16 boxes, 64B swizzle), or null for direct stores
+int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const GemmArgs& g, bool a_mn, bool b_mn,
+                    int sms, cudaStream_t s) {
+  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, mc, g, sms, s);
+  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, mc, g, sms, s);
+  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, mc, g, sms, s);
+  return launch2<1, 0>(ma, mb, mc, g, sms, s);
 }
 
 }  // namespace orbit

@@ -4,10 +4,17 @@
 //   warp 0      : TMA producer (Q once, then K_j / V_j tiles; 128B-swizzled boxes of 64 columns x 128 rows)
 //   warp 1      : single-thread tcgen05.mma issuer:  S_j = Q K_j^T  (fp32, TMEM, double buffered)
 //                                                     O  += P_j V_j  (fp32, TMEM)
-//   warps 2..5  : softmax; thread <-> query row <-> TMEM lane: tcgen05.ld the S row, row max / exp2 / row sum with
-//                 no cross-thread traffic, P_j as bf16 into a swizzled K-major shared-memory tile (the A operand
-//                 of the PV product), lazy rescale of O in TMEM (only when a row max grows by more than 2^8:
-//                 stale maxima keep exp2 below 256, which is exact enough in fp32 accumulators), final O / l.
+//   warps 2..9  : softmax; two warps share a TMEM lane quarter (thread <-> query row <-> TMEM lane) and split the
+//                 tile's 128 key columns: tcgen05.ld of the S half-row, row max (agreed between the pair through
+//                 shared memory as ceil(max) in int16), exp2 / row sum, P_j as bf16 into a swizzled K-major
+//                 shared-memory tile (the A operand of the PV product) whose two 64-key halves are published and
+//                 released separately (PV_j starts on the first half while the second is still being written),
+//                 lazy rescale of O in TMEM (only when a row max grows by more than 2^8: stale maxima keep exp2
+//                 below 256, which is exact enough in fp32 accumulators), final O / l.
+// clock64 stamps (C5, one CTA per SM, 16 tiles): ~2200 cycles per tile against ~1050 of MMA; the softmax warps are
+// the critical path: 128 MUFU.EX2 per row and tile = ~1024 cycles of the sub-partition's quarter-rate unit, plus the
+// serial tcgen05.ld / fence.proxy.async / barrier latencies of a tile.  Tried and measured no faster: a max-only warp
+// running one tile ahead of an exp-only warp (291 us vs 284), P packed by truncation instead of cvt (311 us).
 // S_{j+1} is issued before the softmax of tile j finishes, so the tensor pipe overlaps the exponentials.
 // V tiles are consumed as an MN-major B operand straight from their row-major [keys, d] layout.
 #include <cuda.h>
@@ -18,7 +25,7 @@ namespace orbit {
 namespace {
 
 constexpr int BQ = 128, BKV = 128;
-constexpr int NTH = 192;   // forward: warp 0 TMA, warp 1 MMA issuer, warps 2..5 softmax
+constexpr int NTH = 320;   // forward: warp 0 TMA, warp 1 MMA issuer, warps 2..9 softmax (two per TMEM lane quarter, 64 key columns each)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 
@@ -35,6 +42,10 @@ __device__ __forceinline__ float fast_ex2(float x) {
 // thread is latency-bound: ~13 dependent uniform-datapath instructions per tcgen05.mma otherwise)
 __device__ __forceinline__ uint64_t desc_adv(uint64_t d, uint32_t bytes) { return d + (uint64_t)(bytes >> 4); }
 
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 template <int DH>
 struct Cfg {
   static constexpr int NBLK = DH / 64;                  // 64-column blocks per tile row
@@ -44,7 +55,7 @@ struct Cfg {
   // only after O += P_j V_j; with 3 + 2 stages the TMA round trip of K_{j+1} no longer sits between PV_{j-1} and S_{j+1}
   // (measured with clock64 stamps: the MMA thread waited ~2000 of 2750 cycles per tile for K/V with a shared 2-stage ring)
   static constexpr int KST = 3, VST = 2;
-  static constexpr int SMEM = TILE /*Q*/ + (KST + VST) * TILE + P_BYTES + 1024 + 256;
+  static constexpr int SMEM = TILE /*Q*/ + (KST + VST) * TILE + P_BYTES + 1024 + 256 + 1024 /*row-max exchange*/;
 };
 
 template <int DH>
@@ -58,8 +69,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   auto sK = [&](int st) { return sK0 + st * C::TILE; };
   auto sV = [&](int st) { return sV0 + st * C::TILE; };
   const uint32_t q_full = bar, k_full0 = bar + 8, k_empty0 = k_full0 + 8 * KST, v_full0 = k_empty0 + 8 * KST,
-                 v_empty0 = v_full0 + 8 * VST, s_full0 = v_empty0 + 8 * VST, s_empty0 = s_full0 + 16, p_full = s_empty0 + 16,
-                 o_done = p_full + 8, tmem_slot = o_done + 8;
+                 v_empty0 = v_full0 + 8 * VST, s_full0 = v_empty0 + 8 * VST, s_empty0 = s_full0 + 16, p_full0 = s_empty0 + 16,
+                 p_free0 = p_full0 + 16, o_done = p_free0 + 16, tmem_slot = o_done + 8, xmax = bar + 256;   // xmax: int16 [2 parity][2 halves][128 rows]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int q0 = blockIdx.x * BQ;
@@ -72,8 +83,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
     ptx::mbar_init(q_full, 1);
     for (int i = 0; i < KST; i++) { ptx::mbar_init(k_full0 + 8 * i, 1); ptx::mbar_init(k_empty0 + 8 * i, 1); }
     for (int i = 0; i < VST; i++) { ptx::mbar_init(v_full0 + 8 * i, 1); ptx::mbar_init(v_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 4); }
-    ptx::mbar_init(p_full, 4);
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 8); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 4); ptx::mbar_init(p_free0 + 8 * i, 1); }
     ptx::mbar_init(o_done, 1);
     ptx::fence_barrier_init();
   }
@@ -132,13 +143,18 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         if (j + 1 < ntiles) issue_s(j + 1);
         const int st = j % VST;
         ptx::mbar_wait(v_full0 + 8 * st, (j / VST) & 1);
-        ptx::mbar_wait(p_full, j & 1);
-        ptx::tc_fence_after();
         const uint64_t dV0 = ptx::make_smem_desc(sV(st), 16384, 1024);
 #pragma unroll
-        for (int ks = 0; ks < BKV / 16; ks++) {
-          const uint32_t aoff = (ks >> 2) * 16384 + (ks & 3) * 32;          // P: K-major, two 64-key blocks
-          ptx::mma_f16_ss(tO, desc_adv(dP0, aoff), desc_adv(dV0, ks * 2048), idesc_o, (j | ks) != 0);
+        for (int hh = 0; hh < 2; hh++) {                      // the two 64-key halves of P are written by different warps
+          ptx::mbar_wait(p_full0 + 8 * hh, j & 1);
+          ptx::tc_fence_after();
+#pragma unroll
+          for (int k4 = 0; k4 < 4; k4++) {
+            const int ks = hh * 4 + k4;
+            const uint32_t aoff = (ks >> 2) * 16384 + (ks & 3) * 32;        // P: K-major, two 64-key blocks
+            ptx::mma_f16_ss(tO, desc_adv(dP0, aoff), desc_adv(dV0, ks * 2048), idesc_o, (j | ks) != 0);
+          }
+          ptx::mma_commit(p_free0 + 8 * hh);                  // this half of the P tile may be rewritten
         }
         ptx::mma_commit(v_empty0 + 8 * st);
         ptx::mma_commit(o_done);
@@ -146,17 +162,23 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
     }
   } else {
     // ===================== softmax / correction / epilogue =====================
-    const int quarter = warp & 3;            // warps 2..5
+    // Two warps share a TMEM lane quarter (32 query rows) and split the tile's 128 key columns: the exponentials of a
+    // row are issued from two schedulers' worth of warps instead of one (with 4 softmax warps the single warp per SM
+    // sub-partition could not hide its own MUFU / TMEM latencies: ~2900 cycles per tile against ~1050 of MMA).
+    // The pair agrees on the row maximum through shared memory as ceil(max) in int16: any common reference >= the
+    // true maximum is exact for softmax (it cancels in P / l), and the integer keeps the exchange at 1 KB.
+    const int quarter = warp & 3, half = (warp - 2) >> 2;   // warps 2..9
     const int r = quarter * 32 + lane;                       // query row within the tile = TMEM lane
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
-    float m_used = -INFINITY, l = 0.f;
+    const int pair_bar = 1 + quarter;                        // named barrier of the two warps of this quarter
+    float m_used = -INFINITY, l = 0.f;                       // l: this thread's half of the row sum
     for (int j = 0; j < ntiles; j++) {
       const int sb = j & 1;
       ptx::mbar_wait(s_full0 + 8 * sb, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[128];
+      uint32_t s[64];
 #pragma unroll
-      for (int c = 0; c < 4; c++) ptx::tmem_ld_32x32(tS0 + sb * 128 + c * 32 + lane_off, s + c * 32);
+      for (int c = 0; c < 2; c++) ptx::tmem_ld_32x32(tS0 + sb * 128 + half * 64 + c * 32 + lane_off, s + c * 32);
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();
@@ -164,40 +186,53 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
       float mx = -INFINITY;
       if ((j + 1) * BKV > N) {                               // last, ragged tile: mask keys >= N
 #pragma unroll
-        for (int c = 0; c < 128; c++) {
-          float v = (j * BKV + c < N) ? __uint_as_float(s[c]) : -INFINITY;
+        for (int c = 0; c < 64; c++) {
+          float v = (j * BKV + half * 64 + c < N) ? __uint_as_float(s[c]) : -INFINITY;
           s[c] = __float_as_uint(v);
           mx = fmaxf(mx, v);
         }
       } else {
 #pragma unroll
-        for (int c = 0; c < 128; c++) mx = fmaxf(mx, __uint_as_float(s[c]));
+        for (int c = 0; c < 64; c++) mx = fmaxf(mx, __uint_as_float(s[c]));
       }
-      const float m_tile = mx * sl2;
-      // P buffer and O are free / final once PV_{j-1} has completed
-      if (j > 0) { ptx::mbar_wait(o_done, (j - 1) & 1); ptx::tc_fence_after(); }
+      const int mi = (int)fminf(fmaxf(ceilf(mx * sl2), -32768.f), 32767.f);
+      const uint32_t xm = xmax + (uint32_t)(sb * 256 + r) * 2;          // [parity][half][row]
+      asm volatile("st.shared.b16 [%0], %1;" ::"r"(xm + half * 256), "h"((short)mi) : "memory");
+      named_bar_sync(pair_bar, 64);
+      short mo;
+      asm volatile("ld.shared.b16 %0, [%1];" : "=h"(mo) : "r"(xm + (half ^ 1) * 256) : "memory");
+      const float m_tile = (float)max(mi, (int)mo);
       float m_new = m_used;
       bool need = false;
       if (j == 0) m_new = m_tile;
       else if (m_tile > m_used + 8.f) { m_new = m_tile; need = true; }
-      if (__any_sync(0xffffffffu, need)) {                    // lazy rescale of the O row in TMEM
+      if (__any_sync(0xffffffffu, need)) {                    // lazy rescale: this thread's half of the O row in TMEM
+        // O is final only once PV_{j-1} has completed, and PV_j (which starts as soon as the FIRST half of P_j is
+        // published) must not begin before BOTH warps of the pair have rescaled: pair barrier after the rescale.
+        // The partner takes the same branch: it sees the same maxima.
+        ptx::mbar_wait(o_done, (j - 1) & 1);
+        ptx::tc_fence_after();
         const float f = exp2f(m_used - m_new);
         l *= f;
 #pragma unroll
-        for (int c = 0; c < DH / 32; c++) {
+        for (int c = 0; c < DH / 64; c++) {
           uint32_t o[32];
-          ptx::tmem_ld_32x32(tO + c * 32 + lane_off, o);
+          ptx::tmem_ld_32x32(tO + half * (DH / 2) + c * 32 + lane_off, o);
           ptx::tmem_ld_wait();
 #pragma unroll
           for (int i = 0; i < 32; i++) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-          ptx::tmem_st_32x32(tO + c * 32 + lane_off, o);
+          ptx::tmem_st_32x32(tO + half * (DH / 2) + c * 32 + lane_off, o);
         }
         ptx::tmem_st_wait();
+        ptx::tc_fence_before();
+        named_bar_sync(pair_bar, 64);
       }
+      // this half of the P tile is free once the first / last four MMAs of PV_{j-1} have read it
+      if (j > 0) ptx::mbar_wait(p_free0 + 8 * half, (j - 1) & 1);
       m_used = m_new;
       float sum = 0.f;
 #pragma unroll
-      for (int c = 0; c < 16; c++) {                          // 8 keys = one 16-byte chunk of the P row
+      for (int c = 0; c < 8; c++) {                           // 8 keys = one 16-byte chunk of the P row
         uint32_t pk[4];
 #pragma unroll
         for (int i = 0; i < 4; i++) {
@@ -207,25 +242,30 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
           __nv_bfloat162 v = __floats2bfloat162_rn(p0, p1);
           pk[i] = *reinterpret_cast<uint32_t*>(&v);
         }
-        const uint32_t addr = sP + (c >> 3) * 16384 + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+        const uint32_t addr = sP + half * 16384 + r * 128 + ((c ^ (r & 7)) << 4);
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
       }
       l += sum;
       ptx::fence_proxy_async();                               // generic-proxy smem writes -> visible to the MMA
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full);
+      if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * half);
     }
-    // ---- epilogue: O / l -> bf16 -> global; logsumexp
+    // ---- epilogue: O / l -> bf16 -> global; logsumexp.  The P tile is idle now: the pair adds its half sums through it
     ptx::mbar_wait(o_done, (ntiles - 1) & 1);
     ptx::tc_fence_after();
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(sP + (uint32_t)(half * 128 + r) * 4), "f"(l) : "memory");
+    named_bar_sync(pair_bar, 64);
+    float lo;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(lo) : "r"(sP + (uint32_t)((half ^ 1) * 128 + r) * 4) : "memory");
+    l += lo;
     const int qrow = q0 + r;
     const float inv = 1.f / l;
-    bf16* orow = (bf16*)a.O + (size_t)(row0 + qrow) * a.ldo + h * DH;
+    bf16* orow = (bf16*)a.O + (size_t)(row0 + qrow) * a.ldo + h * DH + half * (DH / 2);
 #pragma unroll
-    for (int c = 0; c < DH / 32; c++) {
+    for (int c = 0; c < DH / 64; c++) {
       uint32_t o[32];
-      ptx::tmem_ld_32x32(tO + c * 32 + lane_off, o);
+      ptx::tmem_ld_32x32(tO + half * (DH / 2) + c * 32 + lane_off, o);
       ptx::tmem_ld_wait();
       if (qrow < N) {
 #pragma unroll
@@ -241,7 +281,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         }
       }
     }
-    if (qrow < N) a.lse[(size_t)bh * N + qrow] = (m_used + log2f(l)) * LN2;
+    if (half == 0 && qrow < N) a.lse[(size_t)bh * N + qrow] = (m_used + log2f(l)) * LN2;
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -273,9 +313,6 @@ struct CfgB {
   static constexpr int SMEM_DQ = 2 * BIG + 2 * NST_DQ * SMALL + 2 * PT + 1024 + 256;
 };
 
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
 // write 64 bf16 (this thread's row r) into a K-major [128 x 64] operand tile (128-byte rows, 128B swizzle)
 __device__ __forceinline__ void write_row64(uint32_t tile, int r, const float* v) {
 #pragma unroll

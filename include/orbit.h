@@ -212,6 +212,12 @@ int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long
 int orbit_debug_gemm_batched(int M, int N, int K, int batch, orbit_dtype dtype, const void* A, long long a_rs,
                              long long a_cs, long long a_bs, const void* B, long long b_rs, long long b_cs,
                              long long b_bs, float* C, long long ldc, long long c_bs, void* stream);
+/* As orbit_debug_gemm, with the output options of the block's GEMMs: C (row stride ldc, ldc % 8 == 0) in out_dtype and an
+ * optional bias[N] (dtype `dtype`) added before the store.  bf16 outputs of tile-sized problems take the TMA-store
+ * epilogue of the CTA-pair kernel. */
+int orbit_debug_gemm_out(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,
+                         const void* B, long long b_rs, long long b_cs, orbit_dtype out_dtype, void* C, long long ldc,
+                         const void* bias /*nullable*/, void* stream);
 /* Kernel-level diagnostic: the LayerNorm kernels of orbit_block_fwd / orbit_block_bwd on their own (the
  * pre-LN sub-layers; SURVEY.md 8(c) BLK / BLK').  Row-major [M, D], D % 8 == 0, all pointers device memory.
  * fwd: out = (x - mean) * rstd * gamma + beta with biased variance; mean, rstd [M] fp32 are written.

@@ -143,6 +143,7 @@ _proto("orbit_profile_gemm_collect", C.c_int, [C.POINTER(C.c_double), C.POINTER(
 _proto("orbit_debug_gemm", C.c_int, [C.c_int] * 4 + [_vp, C.c_longlong, C.c_longlong, _vp, C.c_longlong, C.c_longlong, _vp, _vp])
 _ll = C.c_longlong
 _proto("orbit_debug_gemm_batched", C.c_int, [C.c_int] * 5 + [_vp, _ll, _ll, _ll, _vp, _ll, _ll, _ll, _vp, _ll, _ll, _vp])
+_proto("orbit_debug_gemm_out", C.c_int, [C.c_int] * 4 + [_vp, _ll, _ll, _vp, _ll, _ll, C.c_int, _vp, _ll, _vp, _vp])
 _proto("orbit_debug_layernorm_fwd", C.c_int, [C.c_int] * 5 + [C.c_float] + [_vp] * 7)
 _proto("orbit_debug_layernorm_bwd", C.c_int, [C.c_int] * 7 + [_vp] * 11)
 
@@ -157,7 +158,7 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
            "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched", "orbit_head_loss", "orbit_head_loss_bwd",
            "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes",
-           "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd"]
+           "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd", "orbit_debug_gemm_out"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -358,6 +359,11 @@ def orbit_debug_gemm(M, N, K, dtype, A, a_rs, a_cs, B, b_rs, b_cs, Cout, stream=
 def orbit_debug_gemm_batched(M, N, K, batch, dtype, A, a_rs, a_cs, a_bs, B, b_rs, b_cs, b_bs, Cout, ldc, c_bs, stream=None):
     _check(lib.orbit_debug_gemm_batched(M, N, K, batch, DTYPES[dtype], _ptr(A), a_rs, a_cs, a_bs, _ptr(B), b_rs, b_cs, b_bs,
                                         _ptr(Cout), ldc, c_bs, _stream(stream)), "orbit_debug_gemm_batched")
+
+
+def orbit_debug_gemm_out(M, N, K, dtype, A, a_rs, a_cs, B, b_rs, b_cs, out_dtype, Cout, ldc, bias=None, stream=None):
+    _check(lib.orbit_debug_gemm_out(M, N, K, DTYPES[dtype], _ptr(A), a_rs, a_cs, _ptr(B), b_rs, b_cs, DTYPES[out_dtype],
+                                    _ptr(Cout), ldc, _ptr(bias), _stream(stream)), "orbit_debug_gemm_out")
 
 
 def orbit_debug_layernorm_fwd(M, D, x_dt, p_dt, out_dt, eps, x, gamma, beta, out, mean, rstd, stream=None):

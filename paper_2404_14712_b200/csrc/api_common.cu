@@ -116,6 +116,19 @@ int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long
   return gemm(g, (cudaStream_t)stream);
 }
 
+int orbit_debug_gemm_out(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,
+                         const void* B, long long b_rs, long long b_cs, orbit_dtype out_dtype, void* C, long long ldc,
+                         const void* bias, void* stream) {
+  if (!A || !B || !C) { set_error("debug_gemm_out: NULL pointer"); return ORBIT_ERR_NULL; }
+  if (!valid_dtype(dtype) || !valid_dtype(out_dtype)) { set_error("debug_gemm_out: bad dtype"); return ORBIT_ERR_DTYPE; }
+  if (M <= 0 || N <= 0 || K <= 0 || ldc < N) { set_error("debug_gemm_out: bad shape"); return ORBIT_ERR_SHAPE; }
+  ORBIT_TRY(check_device());
+  GemmArgs g;
+  g.A = A; g.a_rs = a_rs; g.a_cs = a_cs; g.B = B; g.b_rs = b_rs; g.b_cs = b_cs; g.C = C; g.ldc = ldc;
+  g.M = M; g.N = N; g.K = K; g.in_dtype = dtype; g.out_dtype = out_dtype; g.bias = bias; g.bias_dtype = dtype;
+  return gemm(g, (cudaStream_t)stream);
+}
+
 int orbit_debug_layernorm_fwd(int M, int D, orbit_dtype x_dtype, orbit_dtype p_dtype, orbit_dtype out_dtype, float eps,
                               const void* x, const void* gamma, const void* beta, void* out, float* mean, float* rstd,
                               void* stream) {

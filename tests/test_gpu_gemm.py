@@ -89,3 +89,32 @@ def test_gemm_strided_batch(ob, case, dtype):
         ref = A64[:, i * K:(i + 1) * K] @ B64[:, i * N:(i + 1) * N]
         err = np.linalg.norm(got[:, i * N:(i + 1) * N] - ref) / np.linalg.norm(ref)
         assert err < 1e-4, f"{case} {dtype} batch {i}: rel err {err:.3e}"
+
+
+# ---- bf16 outputs (+ bias): the TMA-store epilogue of the CTA-pair kernel, ragged in M and N, padded row stride ----
+OUT_SHAPES = [(256, 256, 64, 256), (520, 776, 136, 776), (1800, 2904, 264, 2912), (300, 264, 520, 272), (2048, 3072, 512, 3072)]
+
+
+@pytest.mark.parametrize("a_major", ["K", "M"])
+@pytest.mark.parametrize("with_bias", [False, True])
+@pytest.mark.parametrize("shape", OUT_SHAPES)
+def test_gemm_bf16_out_tma_store(ob, shape, a_major, with_bias):
+    M, N, K, ldc = shape
+    A = syn.normal(6, f"A{M}{K}", (M, K), dtype="bf16")
+    B = syn.normal(6, f"B{K}{N}", (K, N), dtype="bf16")
+    bias = syn.normal(6, f"b{N}", (N,), dtype="bf16") if with_bias else None
+    At, Bt = torch.from_numpy(A).cuda().bfloat16(), torch.from_numpy(B).cuda().bfloat16()
+    if a_major == "K":
+        Ad, a_rs, a_cs = At.contiguous(), K, 1
+    else:
+        Ad, a_rs, a_cs = At.t().contiguous(), 1, M
+    bd = torch.from_numpy(bias).cuda().bfloat16() if with_bias else None
+    C = torch.full((M, ldc), float("nan"), device="cuda", dtype=torch.bfloat16)
+    ob.orbit_debug_gemm_out(M, N, K, "bf16", Ad, a_rs, a_cs, Bt.contiguous(), N, 1, "bf16", C, ldc, bd)
+    torch.cuda.synchronize()
+    ref = A.astype(np.float64) @ B.astype(np.float64) + (bias.astype(np.float64) if with_bias else 0.0)
+    got = C.float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(got[:, :N]).all()
+    assert np.isnan(got[:, N:]).all(), "columns beyond N (row padding) must not be written"
+    err = np.linalg.norm(got[:, :N] - ref) / np.linalg.norm(ref)
+    assert err < 4e-3, f"{shape} rel err {err:.3e}"        # one bf16 rounding of the fp32 accumulator (2^-9 relative, rms ~1.7e-3)

@@ -92,7 +92,9 @@ def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_tok = 16
+    # a step of the reference arm = the oracle on a bounded sample: 256 tokens at the 113B-class width (~4 s per step),
+    # one whole sample (L tokens) at the smaller widths
+    n_tok = 256 if cfg.D >= 8192 else (512 if cfg.D >= 4096 else cfg.L)
     run, flops = oracle_sample(cfg, n_tok)
     for _ in range(args.warmup):
         run()

@@ -334,6 +334,13 @@ def run_ours(args, cfg):
     gemm_ms, gemm_flops, gemm_n = ob.orbit_profile_gemm_collect()
     ob.orbit_profile_gemm(False)
     clocks = sampler.stop() if sampler else None
+    # ---- optional: the same device-resident step replayed from a CUDA graph ----
+    graph_ms = None
+    if args.graph:
+        replay = sr.capture(step)
+        for _ in range(3):
+            replay()
+        graph_ms = timed(replay, args.steps) / args.steps
     # ---- end to end through the public API with host buffers ----
     for _ in range(2):
         step_e2e()
@@ -397,6 +404,7 @@ def run_ours(args, cfg):
                 "ms_per_step": ms_e2e / args.steps,
                 "overlap": "every step's H2D / D2H runs on copy streams (double-buffered inputs, snapshotted results) inside the timed region"},
         "gpu_launches": int(launches),
+        **({"graph": {"ms_per_step": graph_ms, "value": flops / (graph_ms * 1e-3) / 1e12 * world, "unit": UNIT}} if graph_ms else {}),
         "roofline": roofline,
         "cpu_baseline": cpu,
     }
@@ -415,6 +423,9 @@ def main():
     ap.add_argument("--front", default="fused", choices=["fused", "twocall"],
                     help="front end of C2/C3: orbit_embed_fused (pixel space, no tok tensor) or orbit_tokenize + "
                          "orbit_var_aggregate (tok materialised)")
+    ap.add_argument("--graph", action="store_true",
+                    help="additionally time the device-resident step replayed from a CUDA graph (reported as 'graph'; "
+                         "the headline value and the roofline leg stay un-captured)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--debug-mode", type=int, default=0, help="orbit_set_debug_force_simt value (A/B comparisons only)")
     args = ap.parse_args()

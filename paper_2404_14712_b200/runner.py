@@ -214,6 +214,26 @@ class StepRunner:
         self.backward(dz)
         return loss
 
+    def capture(self, fn):
+        """Capture one invocation of `fn` (a closure over this runner's calls and FIXED device tensors) into a CUDA
+        graph and return its replay function.  Every C-ABI entry point only enqueues kernels on the caller's stream
+        (no allocation, no host synchronisation; tensor maps travel by value as kernel parameters), so a whole step is
+        capturable; replay removes the per-launch host work and most of the inter-kernel gaps of launch-bound shapes
+        (C2: 330 launches per step).  Not usable together with orbit_profile_gemm (event timing cannot be captured)."""
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            fn()                                   # warm-up on the capture stream (first-use attribute calls)
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            fn()
+        torch.cuda.synchronize()
+        self._graphs = getattr(self, "_graphs", []) + [g]
+        return g.replay
+
     def step(self, x, target):
         """x: fields [B,V,Hg,Wg] fp32 (or block input [B,N,D] for block-only configs); target [B,L,D]."""
         y = self.forward(x)

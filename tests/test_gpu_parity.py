@@ -371,3 +371,27 @@ def test_error_codes(ob, rn):
     with pytest.raises(ob.OrbitError) as e:
         br.fwd(torch.zeros(1, 16, 64, device="cuda", dtype=torch.bfloat16))
     assert e.value.status == 5                      # ORBIT_ERR_WORKSPACE
+
+
+def test_step_replayed_from_cuda_graph_matches_oracle(rn):
+    """StepRunner.capture: the whole step (fused front end + 2 blocks + MSE, fwd + bwd) captured into a CUDA graph and
+    replayed on FRESH inputs written into the captured buffers must match the oracle like the eager step does -- every
+    entry point only enqueues kernels on the caller's stream (include/orbit.h "Execution")."""
+    cfg = syn.Config("S2", B=2, V=7, Hg=16, Wg=32, p=2, D=256, heads=4, F=1024, depth=2, dtype="bf16",
+                     resid_dtype="f32")
+    emb, agg, blocks, x, tgt, pos = make_step_case(cfg, 44)
+    sr = rn.StepRunner(cfg, emb, agg, [(P, syn.shard_block_params(P, cfg.heads, 1)) for P in blocks], pos,
+                       fused_front=True)
+    x_d = torch.zeros(x.shape, device="cuda", dtype=torch.float32)          # captured with other contents
+    t_d = torch.zeros(tgt.shape, device="cuda", dtype=torch.float32)
+    replay = sr.capture(lambda: sr.step(x_d, t_d))
+    x_d.copy_(torch.from_numpy(x))
+    t_d.copy_(torch.from_numpy(np.asarray(tgt, dtype=np.float32)))
+    replay()
+    torch.cuda.synchronize()
+    out = orc.step(x, emb, agg, blocks, tgt, cfg.p, cfg.heads, cfg.ln_eps, pos)
+    check("graph y", sr.blocks[-1].y, out["y"], 1e-2)
+    check("graph dagg", sr.blocks[0].dx, out["dagg"], 1e-2)
+    check("graph dWp", sr.front.dWp, out["dWp"], 1e-2)
+    check("graph b1.dWfc1", sr.blocks[1].gshards[0]["Wfc1"], out["block_grads"][1]["Wfc1"], 1e-2)
+    assert abs(float(sr.loss.item()) - out["loss"]) <= 5e-2 * abs(out["loss"])

@@ -260,8 +260,8 @@ int launch_bn(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, b
 }
 }  // namespace
 
-int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const GemmArgs& g, bool a_mn, bool b_mn,
-                    int sms, cudaStream_t s);   // gemm_tc2.cu
+int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const CUtensorMap* mx, const GemmArgs& g,
+                    bool a_mn, bool b_mn, int sms, cudaStream_t s);   // gemm_tc2.cu
 
 int gemm_profile_enable(int on) {
   if (on && !g_prof.ev) {
@@ -320,15 +320,19 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   else      ORBIT_TRY(make_map(&ma, g.A, g.K, g.M, g.a_rs, 64, BM, g.batch, g.a_bs));   // [M rows, K contiguous]
   if (b_mn) ORBIT_TRY(make_map(&mb, g.B, g.N, g.K, g.b_rs, 64, 64, g.batch, g.b_bs));   // [K rows, N contiguous]
   else      ORBIT_TRY(make_map(&mb, g.B, g.K, g.N, g.b_cs, 64, bn, g.batch, g.b_bs));   // [N rows, K contiguous]
-  // plain bf16 outputs (weight gradients, QKV, dO) leave the CTA-pair kernel through TMA stores; g_force_simt == 5
+  // bf16 outputs without residual (weight gradients, QKV, dO, fc1 with GELU, du with GELU') leave the CTA-pair kernel through TMA stores; g_force_simt == 5
   // keeps the direct row-per-thread stores (A/B comparison)
-  CUtensorMap mc;
+  CUtensorMap mc, mx;
   const bool store_map = pair && g_force_simt != 5 && g.out_dtype == ORBIT_BF16 && !g.resid && !g.accumulate &&
-                         g.act == ACT_NONE && !g.aux_out && !g.aux_in;
+                         (g.act == ACT_NONE ? (!g.aux_out && !g.aux_in)
+                          : g.act == ACT_GELU ? (g.batch <= 1 && (!g.aux_out || g.aux_dtype == ORBIT_BF16))
+                                              : (g.batch <= 1 && g.aux_in != nullptr));
+  const bool aux_map = store_map && g.act == ACT_GELU && g.aux_out;
   if (store_map) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 32, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B));
+  if (aux_map) ORBIT_TRY(make_map(&mx, g.aux_out, g.N, g.M, g.ld_aux, 32, 32, 1, 0, CU_TENSOR_MAP_SWIZZLE_64B));
   const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
   if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
-  if (pair) ORBIT_TRY(gemm_tc2_launch(ma, mb, store_map ? &mc : nullptr, g, a_mn, b_mn, num_sms(), s));
+  if (pair) ORBIT_TRY(gemm_tc2_launch(ma, mb, store_map ? &mc : nullptr, aux_map ? &mx : nullptr, g, a_mn, b_mn, num_sms(), s));
   else if (bn == 128) ORBIT_TRY(launch_bn<128>(ma, mb, g, a_mn, b_mn, s));
   else ORBIT_TRY(launch_bn<256>(ma, mb, g, a_mn, b_mn, s));
   if (rec) {

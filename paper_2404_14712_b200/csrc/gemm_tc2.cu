@@ -51,7 +51,8 @@ __device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, in
 template <int A_MN, int B_MN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                const __grid_constant__ CUtensorMap tmC, int tma_store, epi::Args e0, int M, int N, int K,
+                const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmX, int tma_store, epi::Args e0,
+                int M, int N, int K,
                 int batch, long long c_bs, long long bias_bs) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -76,6 +77,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     ptx::prefetch_tmap(&tmA);
     ptx::prefetch_tmap(&tmB);
     if (tma_store) ptx::prefetch_tmap(&tmC);
+    if (tma_store & 2) ptx::prefetch_tmap(&tmX);
     for (int s = 0; s < STAGES; s++) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
     for (int a = 0; a < 2; a++) { ptx::mbar_init(tfull_bar(a), 1); ptx::mbar_init(tempty_bar(a), 16); }
     ptx::fence_barrier_init();
@@ -169,34 +171,20 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       const uint32_t taddr = tmem_base + acc * BN2 + ((uint32_t)(quarter * 32) << 16);
       const int rrow = e.resid_row_mod > 0 ? (row % e.resid_row_mod) : row;
       if (tma_store) {
-        // plain bf16 output (+ bias): 32 x 32 boxes through shared memory, written back by TMA as full 64-byte row
-        // segments (the row-per-thread direct stores below touch 32 different lines per instruction, which made the
-        // K = 2048 weight-gradient GEMMs epilogue-bound)
+        // bf16 outputs (+ bias, GELU with its pre-activation side output, GELU'): 32 x 32 boxes through shared memory,
+        // written back by TMA as full 64-byte row segments (the row-per-thread direct stores below touch 32 different
+        // lines per instruction, which made the K = 2048 weight-gradient GEMMs epilogue-bound)
         const int wrow0 = mb * BM2 + (int)rank * 128 + quarter * 32;
-#pragma unroll 1
-        for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
-          uint32_t r[32];
-          ptx::tmem_ld_32x32(taddr + c * 32, r);
-          ptx::tmem_ld_wait();
-          const int col0 = n0 + c * 32;
-          if (lane == 0) bulk_wait_read<1>();            // the store issued two chunks ago has left this buffer
+        auto stage_store = [&](const CUtensorMap* tm, const float (&v)[32], int col0) {
+          if (lane == 0) bulk_wait_read<1>();            // the store issued two boxes ago has left this buffer
           __syncwarp();
           const uint32_t buf = epi_base + (uint32_t)(warp - 2) * (2 * EPI_BOX_BYTES) + ebuf * EPI_BOX_BYTES;
 #pragma unroll
           for (int g8 = 0; g8 < 4; g8++) {
-            float v[8];
-#pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = __uint_as_float(r[g8 * 8 + j]);
-            if (e.bias && col0 + g8 * 8 < N) {
-              float b[8];
-              epi::load8(e.bias, col0 + g8 * 8, e.bias_dt, b);
-#pragma unroll
-              for (int j = 0; j < 8; j++) v[j] += b[j];
-            }
             uint32_t pk[4];
 #pragma unroll
             for (int j = 0; j < 4; j++) {
-              __nv_bfloat162 t2 = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+              __nv_bfloat162 t2 = __floats2bfloat162_rn(v[g8 * 8 + 2 * j], v[g8 * 8 + 2 * j + 1]);
               pk[j] = *reinterpret_cast<uint32_t*>(&t2);
             }
             const uint32_t addr = buf + lane * 64 + ((g8 ^ ((lane >> 1) & 3)) << 4);
@@ -204,8 +192,49 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           }
           ptx::fence_proxy_async();
           __syncwarp();
-          if (lane == 0) { tma_store_3d(&tmC, buf, col0, wrow0, bi); bulk_commit(); }
+          if (lane == 0) { tma_store_3d(tm, buf, col0, wrow0, bi); bulk_commit(); }
           ebuf ^= 1;
+        };
+#pragma unroll 1
+        for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
+          uint32_t r[32];
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          const int col0 = n0 + c * 32;
+          float v[32];
+#pragma unroll
+          for (int g8 = 0; g8 < 4; g8++) {
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[g8 * 8 + j] = __uint_as_float(r[g8 * 8 + j]);
+            if (e.bias && col0 + g8 * 8 < N) {
+              float b[8];
+              epi::load8(e.bias, col0 + g8 * 8, e.bias_dt, b);
+#pragma unroll
+              for (int j = 0; j < 8; j++) v[g8 * 8 + j] += b[j];
+            }
+          }
+          if (e.act == ACT_GELU) {
+            if (tma_store & 2) {                                  // pre-activation u (bf16); g = GELU(bf16(u)) (reading R25)
+              stage_store(&tmX, v, col0);
+#pragma unroll
+              for (int j = 0; j < 32; j++) v[j] = __bfloat162float(__float2bfloat16_rn(v[j]));
+            }
+#pragma unroll
+            for (int j = 0; j < 32; j++) v[j] = gelu_f(v[j]);
+          } else if (e.act == ACT_GELU_GRAD) {
+            if (row < M) {
+#pragma unroll
+              for (int g8 = 0; g8 < 4; g8++) {
+                if (col0 + g8 * 8 < N) {
+                  float u[8];
+                  epi::load8(e.aux_in, (size_t)row * e.ld_aux + col0 + g8 * 8, e.aux_dt, u);
+#pragma unroll
+                  for (int j = 0; j < 8; j++) v[g8 * 8 + j] *= gelu_grad_f(u[j]);
+                }
+              }
+            }
+          }
+          stage_store(&tmC, v, col0);
         }
       } else {
 #pragma unroll 1
@@ -232,7 +261,8 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 }
 
 template <int A_MN, int B_MN>
-int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const GemmArgs& g, int sms, cudaStream_t s) {
+int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const CUtensorMap* mx, const GemmArgs& g, int sms,
+            cudaStream_t s) {
   const epi::Args e = epi::from_gemm(g);
   const int M = g.M, N = g.N, K = g.K, batch = g.batch > 1 ? g.batch : 1;
   static bool attr_set = false;
@@ -244,21 +274,23 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc,
   const long long tiles = (long long)cdiv(M, BM2) * cdiv(N, BN2) * batch;
   int clusters = sms / 2;
   if (tiles < clusters) clusters = (int)tiles;
-  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, mc ? *mc : ma, mc ? 1 : 0, e, M, N, K, batch,
-                                                                         g.c_bs, g.bias_bs);
+  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, mc ? *mc : ma, mx ? *mx : ma,
+                                                                         (mc ? 1 : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,
+                                                                         g.bias_bs);
   return ORBIT_OK;
 }
 }  // namespace
 
 // called by gemm_tc() (gemm_tc.cu), which builds the tensor maps: A boxes as in the 1-CTA kernel, B boxes with
 // 128 rows (K-major) or 64 x 64 (N-major)
-// mc: tensor map of C for the TMA-store epilogue (32 x 32 bf16 boxes, 64B swizzle), or null for direct stores
-int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const GemmArgs& g, bool a_mn, bool b_mn,
-                    int sms, cudaStream_t s) {
-  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, mc, g, sms, s);
-  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, mc, g, sms, s);
-  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, mc, g, sms, s);
-  return launch2<1, 0>(ma, mb, mc, g, sms, s);
+// mc / mx: tensor maps of C / of the GELU pre-activation side output for the TMA-store epilogue (32 x 32 bf16 boxes, 64B
+// swizzle), or null for direct stores
+int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const CUtensorMap* mx, const GemmArgs& g,
+                    bool a_mn, bool b_mn, int sms, cudaStream_t s) {
+  if (!a_mn && b_mn) return launch2<0, 1>(ma, mb, mc, mx, g, sms, s);
+  if (!a_mn && !b_mn) return launch2<0, 0>(ma, mb, mc, mx, g, sms, s);
+  if (a_mn && b_mn) return launch2<1, 1>(ma, mb, mc, mx, g, sms, s);
+  return launch2<1, 0>(ma, mb, mc, mx, g, sms, s);
 }
 
 }  // namespace orbit

@@ -369,9 +369,13 @@ def run_ours(args, cfg):
         except Exception:
             traffic = None
     roofline = {"bound": "tensor", "kernel": "gemm_tc2_kernel / gemm_tc_kernel (tcgen05 bf16 GEMM; every GEMM launch of the step)",
-                "achieved": achieved, "peak": peaks["bf16"], "unit": "TFLOP/s", "frac": achieved / peaks["bf16"],
-                "peak_source": f"{peaks['src']} burst bf16 (MEASURED_PEAKS.json bf16_tflops)",
-                "frac_of_sustained": (achieved / peaks["bf16_sustained"]) if peaks["bf16_sustained"] else None,
+                # the GEMM launches are timed inside the long timed step (the power-capped regime), so the peak is the
+                # SUSTAINED measured bf16 figure; the burst figure (a kernel timed alone) is given beside it
+                "achieved": achieved, "peak": peaks["bf16_sustained"] or peaks["bf16"], "unit": "TFLOP/s",
+                "frac": achieved / (peaks["bf16_sustained"] or peaks["bf16"]),
+                "peak_source": f"{peaks['src']} sustained bf16 (MEASURED_PEAKS.json bf16_tflops_sustained: torch.matmul back to "
+                               f"back for 4 s; kernels here are timed inside a long step)",
+                "peak_burst": peaks["bf16"], "frac_of_burst": achieved / peaks["bf16"],
                 "launches": gemm_n, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
                 "share_of_step": gemm_ms / ms if ms > 0 else None, "traffic": traffic}
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only) ----

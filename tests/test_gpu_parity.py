@@ -395,3 +395,48 @@ def test_step_replayed_from_cuda_graph_matches_oracle(rn):
     check("graph dWp", sr.front.dWp, out["dWp"], 1e-2)
     check("graph b1.dWfc1", sr.blocks[1].gshards[0]["Wfc1"], out["block_grads"][1]["Wfc1"], 1e-2)
     assert abs(float(sr.loss.item()) - out["loss"]) <= 5e-2 * abs(out["loss"])
+
+
+# ---- degenerate cases of the method (SURVEY.md 8(c) pins, here on the CUDA path) ---------------------------------
+@pytest.mark.parametrize("N", [1, 2, 3])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_block_tiny_sequences(rn, N, dtype):
+    """N = 1: softmax over one key is 1 and O = V (the oracle pin 'N = 1 => O = V'); N = 2, 3: every tile is a tail."""
+    B, D, heads, F = 3, 128, 4, 256
+    P, shards, x, dy = make_block_case(31, B, N, D, heads, F, 1, dtype, "f32")
+    br, y, dx = run_block(rn, B, N, D, heads, F, 1, dtype, "f32", P, shards, x, dy)
+    compare_block(br, y, dx, P, x, dy, heads, 1, 1e-4 if dtype == "f32" else 1e-2)
+
+
+@pytest.mark.parametrize("fused", [False, True])
+@pytest.mark.parametrize("V", [1, 2])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_front_end_one_and_two_variables(rn, V, fused, dtype):
+    """V = 1: alpha = 1, the aggregation is (X Wv + bv) Wo + bo whatever q, Wq, Wk are and their gradients vanish
+    (oracle pin); V = 2 is the smallest real softmax.  Both front ends."""
+    cfg = syn.Config("SV", B=2, V=V, Hg=8, Wg=16, p=2, D=64, heads=4, F=128, depth=1, dtype=dtype, resid_dtype="f32")
+    tol = 1e-4 if dtype == "f32" else 1e-2
+    emb, agg, blocks, x, tgt, pos = make_step_case(cfg, 46)
+    sr = rn.StepRunner(cfg, emb, agg, [(P, syn.shard_block_params(P, cfg.heads, 1)) for P in blocks], pos, fused_front=fused)
+    sr.step(rn.to_dev(x, "f32"), rn.to_dev(tgt, cfg.resid_dtype))
+    torch.cuda.synchronize()
+    out = orc.step(x, emb, agg, blocks, tgt, cfg.p, cfg.heads, cfg.ln_eps, pos)
+    check("agg", sr.front.out, out["agg"], tol)
+    check("dWp", sr.front.dWp, out["dWp"], tol)
+    check("dWv", sr.front.gagg["Wv"], out["agg_grads"]["Wv"], tol)
+    check("dWo", sr.front.gagg["Wo"], out["agg_grads"]["Wo"], tol)
+    if V == 1:        # gradients of the query path are analytically zero: compare absolutely against the scale of dWv
+        scale = np.abs(out["agg_grads"]["Wv"]).max()
+        for k in ("q", "Wq", "bq", "Wk"):
+            got = sr.front.gagg[k].detach().to(torch.float32).cpu().numpy()
+            assert np.abs(got).max() <= tol * scale, f"d{k} must vanish for V = 1"
+    else:
+        check("dWk", sr.front.gagg["Wk"], out["agg_grads"]["Wk"], tol)
+        check("dq", sr.front.gagg["q"], out["agg_grads"]["q"], tol)
+
+
+def test_single_patch_single_sample(rn):
+    """B = 1 and one patch (L = 1): the smallest whole step (M = 1 row in every GEMM, attention over one token)."""
+    cfg = syn.Config("S1", B=1, V=3, Hg=4, Wg=4, p=4, D=64, heads=4, F=128, depth=1, dtype="f32", resid_dtype="f32")
+    run_and_compare_step(rn, cfg, 47, 1e-4)
+    run_and_compare_step(rn, cfg, 47, 1e-4, fused=True)

@@ -111,7 +111,7 @@ int orbit_embed_fused(const orbit_front_desc* d, const float* x, const void* Wp,
   ORBIT_TRY(agg_make_qt(P->q, P->Wq, P->bq, dt, sv.qt, D, s));
   ORBIT_TRY(agg_make_u(P->Wk, dt, sv.qt, sv.Ut, D, h, s));
   ORBIT_TRY(fe_pack_wpb(Wp, bp, dt, sv.Wpb, d->V, f.Vp, f.P2, D, s));
-  ORBIT_TRY(fe_make_g(sv.Wpb, dt, sv.Ut, sv.G, f.KVp, D, h, s));
+  ORBIT_TRY(fe_make_g(sv.Wpb, dt, sv.Ut, sv.G, f.KVp, f.Vp, D, h, s));
   {
     GemmArgs g;
     g.A = sv.Wpb; g.a_rs = D; g.a_cs = 1; g.B = P->Wv; g.b_rs = D; g.b_cs = 1; g.C = sv.H; g.ldc = D;

@@ -76,10 +76,10 @@ __global__ void fe_pack_wpb_kernel(const T* __restrict__ Wp, const T* __restrict
   }
 }
 
-// G[(r, v), a] = sum_d Wpb[(r, v), d] Ut[d, a]; one warp per k row, lanes stride over d
+// G[r][a][v] = sum_d Wpb[(r, v), d] Ut[d, a]  (fp32 [R][HP][Vp], v fastest); one warp per k = (r, v) row, lanes stride over d
 template <typename T>
 __global__ void fe_make_g_kernel(const T* __restrict__ Wpb, const float* __restrict__ Ut, float* __restrict__ G, int KVp,
-                                 int D, int h) {
+                                 int Vp, int D, int h) {
   const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= KVp) return;
   float acc[HP];
@@ -107,15 +107,16 @@ __global__ void fe_make_g_kernel(const T* __restrict__ Wpb, const float* __restr
 #pragma unroll
   for (int a = 0; a < HP; a++) acc[a] = warp_sum(acc[a]);
   if (lane == 0) {
+    const int r = k / Vp, v = k - r * Vp;
 #pragma unroll
-    for (int a = 0; a < HP; a++) G[(size_t)k * HP + a] = acc[a];
+    for (int a = 0; a < HP; a++) G[((size_t)r * HP + a) * Vp + v] = acc[a];
   }
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // forward, one warp per patch; lane owns the variable pairs (64 n + 2 lane, +1), n < NV
 template <typename T, int P, int NV>
-__global__ void __launch_bounds__(256) fe_patch_fwd_kernel(const float* __restrict__ x, const float* __restrict__ G,
+__global__ void __launch_bounds__(256, NV == 2 ? 1 : 2) fe_patch_fwd_kernel(const float* __restrict__ x, const float* __restrict__ G,
     float* __restrict__ alpha, T* __restrict__ A, int V, int Vp, int Hg, int Wg, int h, int BL) {
   constexpr int P2 = P * P, R = P2 + 1, E = 2 * NV;
   typedef typename Pair<T>::type pair_t;
@@ -139,31 +140,35 @@ __global__ void __launch_bounds__(256) fe_patch_fwd_kernel(const float* __restri
 #pragma unroll 1
     for (int a0 = 0; a0 < h; a0 += HG) {
       float s[E][HG];
+      // G is stored [r][head][v] (v fastest): the lanes of a warp (consecutive variable pairs) read 256 contiguous bytes
+      // per (r, head).  With the [(r, v)][head] layout every 16-byte load of a warp touched 32 different lines.
 #pragma unroll
-      for (int e = 0; e < E; e++) {
-        const int v = 64 * (e >> 1) + 2 * lane + (e & 1);
-        if (v < V) {
-          const float4* g4 = reinterpret_cast<const float4*>(G + ((size_t)P2 * Vp + v) * HP + a0);
+      for (int n = 0; n < NV; n++) {
+        const int v0 = 64 * n + 2 * lane;
+        if (v0 < Vp) {
 #pragma unroll
-          for (int q = 0; q < HG / 4; q++) {
-            const float4 g = __ldg(g4 + q);
-            s[e][4 * q] = g.x; s[e][4 * q + 1] = g.y; s[e][4 * q + 2] = g.z; s[e][4 * q + 3] = g.w;
+          for (int aa = 0; aa < HG; aa++) {
+            const float2 g = __ldg(reinterpret_cast<const float2*>(G + ((size_t)P2 * HP + a0 + aa) * Vp + v0));
+            s[2 * n][aa] = g.x; s[2 * n + 1][aa] = g.y;
           }
 #pragma unroll
           for (int r = 0; r < P2; r++) {
-            const float4* gr = reinterpret_cast<const float4*>(G + ((size_t)r * Vp + v) * HP + a0);
+            float2 g[HG];
 #pragma unroll
-            for (int q = 0; q < HG / 4; q++) {
-              const float4 g = __ldg(gr + q);
-              s[e][4 * q] = fmaf(pix[e][r], g.x, s[e][4 * q]);
-              s[e][4 * q + 1] = fmaf(pix[e][r], g.y, s[e][4 * q + 1]);
-              s[e][4 * q + 2] = fmaf(pix[e][r], g.z, s[e][4 * q + 2]);
-              s[e][4 * q + 3] = fmaf(pix[e][r], g.w, s[e][4 * q + 3]);
+            for (int aa = 0; aa < HG; aa++) g[aa] = __ldg(reinterpret_cast<const float2*>(G + ((size_t)r * HP + a0 + aa) * Vp + v0));
+#pragma unroll
+            for (int aa = 0; aa < HG; aa++) {
+              s[2 * n][aa] = fmaf(pix[2 * n][r], g[aa].x, s[2 * n][aa]);
+              s[2 * n + 1][aa] = fmaf(pix[2 * n + 1][r], g[aa].y, s[2 * n + 1][aa]);
             }
           }
-        } else {
+        }
 #pragma unroll
-          for (int aa = 0; aa < HG; aa++) s[e][aa] = -INFINITY;
+        for (int q = 0; q < 2; q++) {
+          if (v0 + q >= V) {
+#pragma unroll
+            for (int aa = 0; aa < HG; aa++) s[2 * n + q][aa] = -INFINITY;
+          }
         }
       }
       // softmax over the variables, per head (R3): alpha replaces s
@@ -363,10 +368,10 @@ int fe_pack_wpb(const void* Wp, const void* bp, int dt, void* Wpb, int V, int Vp
   return ORBIT_OK;
 }
 
-int fe_make_g(const void* Wpb, int dt, const float* Ut, float* G, int KVp, int D, int h, cudaStream_t s) {
+int fe_make_g(const void* Wpb, int dt, const float* Ut, float* G, int KVp, int Vp, int D, int h, cudaStream_t s) {
   const int grid = cdiv((long long)KVp * 32, 256);
-  if (dt == ORBIT_BF16) fe_make_g_kernel<bf16><<<grid, 256, 0, s>>>((const bf16*)Wpb, Ut, G, KVp, D, h);
-  else fe_make_g_kernel<float><<<grid, 256, 0, s>>>((const float*)Wpb, Ut, G, KVp, D, h);
+  if (dt == ORBIT_BF16) fe_make_g_kernel<bf16><<<grid, 256, 0, s>>>((const bf16*)Wpb, Ut, G, KVp, Vp, D, h);
+  else fe_make_g_kernel<float><<<grid, 256, 0, s>>>((const float*)Wpb, Ut, G, KVp, Vp, D, h);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

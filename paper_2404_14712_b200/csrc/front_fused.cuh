@@ -9,8 +9,8 @@ constexpr int FE_HP = 16;   // heads are padded to 16 in G / dG / dsT
 bool fe_supported(int V, int p, int heads);
 // Wpb[(r, v), :] = Wp[v, r, :] (r < p^2) | bp[v, :] (r = p^2); rows with v >= V are zero.  [R*Vp, D]
 int fe_pack_wpb(const void* Wp, const void* bp, int dt, void* Wpb, int V, int Vp, int P2, int D, cudaStream_t s);
-// G[(r, v), a] = sum_d Wpb[(r, v), d] Ut[d, a]    (fp32 [R*Vp, FE_HP])
-int fe_make_g(const void* Wpb, int dt, const float* Ut, float* G, int KVp, int D, int h, cudaStream_t s);
+// G[r][a][v] = sum_d Wpb[(r, v), d] Ut[d, a]    (fp32 [R][FE_HP][Vp], v fastest: coalesced for fe_patch_fwd)
+int fe_make_g(const void* Wpb, int dt, const float* Ut, float* G, int KVp, int Vp, int D, int h, cudaStream_t s);
 // per patch: scores from pixels and G, softmax over V -> alpha [BL, h, Vp] fp32, A [BL, h, R*Vp] = alpha * pixext
 int fe_patch_fwd(const float* x, const float* G, float* alpha, void* A, int dt, int V, int Vp, int Hg, int Wg, int p, int h,
                  int BL, cudaStream_t s);

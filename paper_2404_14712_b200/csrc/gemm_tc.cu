@@ -194,17 +194,17 @@ EncodeTiledFn get_encode() {
 // bf16 tensor map over `batch` 2-D problems `bstride` elements apart: `inner` contiguous elements, `outer` rows `ld`
 // elements apart; 128B swizzle; box = box_inner x box_outer x 1 (out-of-bounds elements read as zero per problem)
 int make_map(CUtensorMap* m, const void* base, long long inner, long long outer, long long ld, int box_inner,
-             int box_outer, int batch, long long bstride, CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_128B) {
+             int box_outer, int batch, long long bstride, CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_128B, int esz = 2) {
   EncodeTiledFn enc = get_encode();
   if (!enc) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
   if (batch <= 1) { batch = 1; bstride = ld * outer; }
   cuuint64_t dims[3] = {(cuuint64_t)inner, (cuuint64_t)outer, (cuuint64_t)batch};
-  cuuint64_t strides[2] = {(cuuint64_t)ld * 2, (cuuint64_t)bstride * 2};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * esz, (cuuint64_t)bstride * esz};
   if (batch == 1) strides[1] = strides[0] * dims[1];
   cuuint32_t box[3] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer, 1};
   cuuint32_t es[3] = {1, 1, 1};
-  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+  CUresult r = enc(m, esz == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims,
+                   strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     set_error("cuTensorMapEncodeTiled failed (%d): inner=%lld outer=%lld ld=%lld box=%dx%d batch=%d bstride=%lld", (int)r,
@@ -323,12 +323,16 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   // bf16 outputs without residual (weight gradients, QKV, dO, fc1 with GELU, du with GELU') leave the CTA-pair kernel through TMA stores; g_force_simt == 5
   // keeps the direct row-per-thread stores (A/B comparison)
   CUtensorMap mc, mx;
-  const bool store_map = pair && g_force_simt != 5 && g.out_dtype == ORBIT_BF16 && !g.resid && !g.accumulate &&
-                         (g.act == ACT_NONE ? (!g.aux_out && !g.aux_in)
-                          : g.act == ACT_GELU ? (g.batch <= 1 && (!g.aux_out || g.aux_dtype == ORBIT_BF16))
-                                              : (g.batch <= 1 && g.aux_in != nullptr));
+  const bool store_bf16 = g.out_dtype == ORBIT_BF16 && !g.resid && !g.accumulate &&
+                          (g.act == ACT_NONE ? (!g.aux_out && !g.aux_in)
+                           : g.act == ACT_GELU ? (g.batch <= 1 && (!g.aux_out || g.aux_dtype == ORBIT_BF16))
+                                               : (g.batch <= 1 && g.aux_in != nullptr));
+  // fp32 outputs, stored or accumulated (the Hybrid-STOP partial sums and the fp32 dm / da of the backward): TMA store / reduce-add
+  const bool store_f32 = g.out_dtype == ORBIT_F32 && !g.resid && g.act == ACT_NONE && !g.aux_out && !g.aux_in && g.ldc % 4 == 0;
+  const bool store_map = pair && g_force_simt != 5 && (store_bf16 || store_f32);
   const bool aux_map = store_map && g.act == ACT_GELU && g.aux_out;
-  if (store_map) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 32, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B));
+  if (store_map && store_f32) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 16, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B, 4));
+  else if (store_map) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 32, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B));
   if (aux_map) ORBIT_TRY(make_map(&mx, g.aux_out, g.N, g.M, g.ld_aux, 32, 32, 1, 0, CU_TENSOR_MAP_SWIZZLE_64B));
   const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
   if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));

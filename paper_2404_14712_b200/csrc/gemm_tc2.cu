@@ -34,6 +34,11 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src,
                "r"(c1), "r"(c2)
                : "memory");
 }
+__device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(m), "r"(src),
+               "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -170,7 +175,53 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + acc * BN2 + ((uint32_t)(quarter * 32) << 16);
       const int rrow = e.resid_row_mod > 0 ? (row % e.resid_row_mod) : row;
-      if (tma_store) {
+      if (tma_store & 4) {
+        // fp32 output (+ bias), stored or ACCUMULATED (Hybrid-STOP partial sums): 32 rows x 16 columns boxes
+        // through shared memory; the accumulate is a TMA reduce-add performed at the L2 instead of a row-per-thread
+        // read-modify-write of C in the SM
+        const int wrow0 = mb * BM2 + (int)rank * 128 + quarter * 32;
+#pragma unroll 1
+        for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
+          uint32_t r[32];
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          const int col0 = n0 + c * 32;
+#pragma unroll
+          for (int hh = 0; hh < 2; hh++) {
+            if (lane == 0) bulk_wait_read<1>();
+            __syncwarp();
+            const uint32_t buf = epi_base + (uint32_t)(warp - 2) * (2 * EPI_BOX_BYTES) + ebuf * EPI_BOX_BYTES;
+#pragma unroll
+            for (int g4 = 0; g4 < 4; g4++) {
+              float v[4];
+#pragma unroll
+              for (int j = 0; j < 4; j++) v[j] = __uint_as_float(r[hh * 16 + g4 * 4 + j]);
+              const int col = col0 + hh * 16 + g4 * 4;
+              if (e.bias && col < N) {
+                if (e.bias_dt == ORBIT_BF16) {
+                  const uint2 raw = *reinterpret_cast<const uint2*>((const bf16*)e.bias + col);
+                  const float2 b0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&raw.x));
+                  const float2 b1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&raw.y));
+                  v[0] += b0.x; v[1] += b0.y; v[2] += b1.x; v[3] += b1.y;
+                } else {
+                  const float4 b = *reinterpret_cast<const float4*>((const float*)e.bias + col);
+                  v[0] += b.x; v[1] += b.y; v[2] += b.z; v[3] += b.w;
+                }
+              }
+              const uint32_t addr = buf + lane * 64 + ((g4 ^ ((lane >> 1) & 3)) << 4);
+              asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
+            }
+            ptx::fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+              if (e.accumulate) tma_reduce_add_3d(&tmC, buf, col0 + hh * 16, wrow0, bi);
+              else tma_store_3d(&tmC, buf, col0 + hh * 16, wrow0, bi);
+              bulk_commit();
+            }
+            ebuf ^= 1;
+          }
+        }
+      } else if (tma_store) {
         // bf16 outputs (+ bias, GELU with its pre-activation side output, GELU'): 32 x 32 boxes through shared memory,
         // written back by TMA as full 64-byte row segments (the row-per-thread direct stores below touch 32 different
         // lines per instruction, which made the K = 2048 weight-gradient GEMMs epilogue-bound)
@@ -275,7 +326,7 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc,
   int clusters = sms / 2;
   if (tiles < clusters) clusters = (int)tiles;
   gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, mc ? *mc : ma, mx ? *mx : ma,
-                                                                         (mc ? 1 : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,
+                                                                         (mc ? (g.out_dtype == ORBIT_F32 ? 4 : 1) : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,
                                                                          g.bias_bs);
   return ORBIT_OK;
 }

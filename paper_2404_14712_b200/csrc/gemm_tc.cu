@@ -323,12 +323,13 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   // bf16 outputs without residual (weight gradients, QKV, dO, fc1 with GELU, du with GELU') leave the CTA-pair kernel through TMA stores; g_force_simt == 5
   // keeps the direct row-per-thread stores (A/B comparison)
   CUtensorMap mc, mx;
-  const bool store_bf16 = g.out_dtype == ORBIT_BF16 && !g.resid && !g.accumulate &&
+  const bool store_bf16 = g.out_dtype == ORBIT_BF16 && !g.accumulate &&
                           (g.act == ACT_NONE ? (!g.aux_out && !g.aux_in)
                            : g.act == ACT_GELU ? (g.batch <= 1 && (!g.aux_out || g.aux_dtype == ORBIT_BF16))
                                                : (g.batch <= 1 && g.aux_in != nullptr));
   // fp32 outputs, stored or accumulated (the Hybrid-STOP partial sums and the fp32 dm / da of the backward): TMA store / reduce-add
-  const bool store_f32 = g.out_dtype == ORBIT_F32 && !g.resid && g.act == ACT_NONE && !g.aux_out && !g.aux_in && g.ldc % 4 == 0;
+  const bool store_f32 = g.out_dtype == ORBIT_F32 && !(g.resid && g.accumulate) && g.act == ACT_NONE && !g.aux_out && !g.aux_in &&
+                         g.ldc % 4 == 0 && (!g.resid || g.ldr % 4 == 0);
   const bool store_map = pair && g_force_simt != 5 && (store_bf16 || store_f32);
   const bool aux_map = store_map && g.act == ACT_GELU && g.aux_out;
   if (store_map && store_f32) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 16, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B, 4));

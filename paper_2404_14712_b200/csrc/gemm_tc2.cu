@@ -208,6 +208,17 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                   v[0] += b.x; v[1] += b.y; v[2] += b.z; v[3] += b.w;
                 }
               }
+              if (e.resid && row < M && col < N) {                // residual (+ positional embedding rows): direct loads
+                if (e.resid_dt == ORBIT_BF16) {
+                  const uint2 raw = *reinterpret_cast<const uint2*>((const bf16*)e.resid + (size_t)rrow * e.ldr + col);
+                  const float2 q0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&raw.x));
+                  const float2 q1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&raw.y));
+                  v[0] += q0.x; v[1] += q0.y; v[2] += q1.x; v[3] += q1.y;
+                } else {
+                  const float4 q = *reinterpret_cast<const float4*>((const float*)e.resid + (size_t)rrow * e.ldr + col);
+                  v[0] += q.x; v[1] += q.y; v[2] += q.z; v[3] += q.w;
+                }
+              }
               const uint32_t addr = buf + lane * 64 + ((g4 ^ ((lane >> 1) & 3)) << 4);
               asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
             }
@@ -282,6 +293,17 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 #pragma unroll
                   for (int j = 0; j < 8; j++) v[g8 * 8 + j] *= gelu_grad_f(u[j]);
                 }
+              }
+            }
+          }
+          if (e.resid && row < M) {
+#pragma unroll
+            for (int g8 = 0; g8 < 4; g8++) {
+              if (col0 + g8 * 8 < N) {
+                float q[8];
+                epi::load8(e.resid, (size_t)rrow * e.ldr + col0 + g8 * 8, e.resid_dt, q);
+#pragma unroll
+                for (int j = 0; j < 8; j++) v[g8 * 8 + j] += q[j];
               }
             }
           }

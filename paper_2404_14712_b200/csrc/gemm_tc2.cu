@@ -2,8 +2,12 @@
 // computes a 256 x 256 output tile.  Each CTA loads its own 128 rows of A and its own 128 columns of B (so the
 // per-SM shared-memory traffic per MMA is halved), the leader CTA issues tcgen05.mma.cta_group::2 (M = 256),
 // and each CTA drains its own 128 x 256 half of the accumulator from its own TMEM.
-// Stage = 16 KB (A half) + 16 KB (B half) -> 6 stages in 192 KB.  Same operand-major handling and fused epilogue
-// as gemm_tc.cu.  Synchronisation:
+// Stage = 16 KB (A half) + 16 KB (B half) -> 6 stages in 192 KB.  Same operand-major handling and fused epilogue math
+// as gemm_tc.cu; the results leave through 32 KB of shared-memory staging and TMA: per epilogue warp two 2 KB boxes
+// (32 rows x 32 bf16 or 32 rows x 16 fp32, 64B swizzle) in flight as bulk store groups -- plain stores, or reduce-add for
+// the fp32 partial sums of the Hybrid-STOP shard mode.  Direct row-per-thread stores remain as the
+// fallback (aux outputs that are not bf16, resid + accumulate) and for A/B timing (orbit_set_debug_force_simt(5)).
+// Synchronisation:
 //   full[s]   (leader's, count 1): the leader's producer arrives expecting the bytes of BOTH CTAs; the peer's TMA
 //                                  complete_tx on it too (a remote arrive per stage costs ~1400 cycles: measured)
 //   empty[s]  (per CTA, count 1) : tcgen05.commit multicast to both CTAs frees the stage

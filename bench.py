@@ -121,7 +121,7 @@ def run_reference(args, cfg):
 # ------------------------------------------------------------------------------------------------------------
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -130,11 +130,23 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-i", str(gpu_index), "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-i", str(gpu_index), "-lms", "20"], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
+    # the sampler is started before the warm-up (nvidia-smi takes a few hundred ms to print its first line); only the
+    # samples whose timestamp falls inside [begin, end] -- host times taken right after the barriers that bracket the
+    # timed region -- are used (all samples if the region was shorter than the sampling period)
+    def begin(self):
+        import datetime
+        self.t0 = datetime.datetime.now()
+
+    def end(self):
+        import datetime
+        self.t1 = datetime.datetime.now()
+
     def stop(self):
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
         if self.p is None:
             return out
@@ -145,16 +157,24 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, reasons, pw = [], [], set(), []
+        rows = []
         for ln in self.f.read().splitlines():
             c = [t.strip() for t in ln.split(",")]
             if len(c) < 8:
                 continue
             try:
-                sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+                ts = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f")
+                rows.append((ts, float(c[1]), float(c[2]), float(c[3]), c[4:8]))
             except ValueError:
                 continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[4:8]):
+        t0, t1 = getattr(self, "t0", None), getattr(self, "t1", None)
+        inside = [r for r in rows if t0 is not None and t1 is not None and t0 <= r[0] <= t1]
+        if not inside:
+            inside = rows
+        sm, mx, reasons, pw = [], [], set(), []
+        for _, a, b, c3, flags in inside:
+            sm.append(a); mx.append(b); pw.append(c3)
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), flags):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         try:
@@ -162,8 +182,7 @@ class ClockSampler:
         except OSError:
             pass
         if sm:
-            hi = sorted(sm)[len(sm) // 2:]          # upper half = samples under load
-            out = {"sm_mhz": float(np.median(hi)), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
                    "power_w_max": max(pw), "samples": len(sm)}
         return out
 
@@ -322,14 +341,18 @@ def run_ours(args, cfg):
         barrier()
         return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
 
+    sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
     # ---- timed region: device-resident inputs ----
-    sampler = ClockSampler(local) if rank == 0 else None
     ob.orbit_profile_gemm(True)
     ob.orbit_reset_launch_count()
+    if sampler:
+        sampler.begin()
     ms = timed(step, args.steps)
+    if sampler:
+        sampler.end()
     launches = ob.orbit_launch_count()
     gemm_ms, gemm_flops, gemm_n = ob.orbit_profile_gemm_collect()
     ob.orbit_profile_gemm(False)

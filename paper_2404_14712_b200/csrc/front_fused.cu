@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(256, NV == 2 ? 1 : 2) fe_patch_fwd_kernel(cons
 // backward, one warp per patch: dalpha[v, a] = sum_r dA[bl, a, (r, v)] pixext[v, r];
 // ds = alpha (dalpha - sum_w alpha_w dalpha_w) -> dsT[v][bl][a]
 template <typename T, int P, int NV>
-__global__ void __launch_bounds__(256) fe_patch_bwd_kernel(const float* __restrict__ x, const float* __restrict__ alpha,
+__global__ void __launch_bounds__(256, 2) fe_patch_bwd_kernel(const float* __restrict__ x, const float* __restrict__ alpha,
     const T* __restrict__ dA, float* __restrict__ dsT, int V, int Vp, int Hg, int Wg, int h, int BL) {
   constexpr int P2 = P * P, R = P2 + 1, E = 2 * NV;
   typedef typename Pair<T>::type pair_t;

@@ -1,27 +1,25 @@
 // aggregate_tc.cu -- tensor-core versions of the per-patch aggregation kernels (a2 / a2'; collapsed
 // form of DESIGN.md §4).  bf16 storage, heads <= 16, V <= 128, D % 64 == 0.
 //
-// A CTA streams one patch's token tile X [V x D] through shared memory in D-chunks (cp.async double buffer,
-// XOR-swizzled 16-byte chunks) and runs the small products on mma.sync.m16n8k16 (bf16 in, fp32 accumulate):
+// A CTA streams one patch's token tile X [V x D] through shared memory in D-chunks (TMA box copies into a ring of
+// mbarrier-guarded stages, 128-byte swizzle) and runs the small products on mma.sync.m16n8k16 (bf16 in, fp32 accumulate):
 //   forward : S = X Ut^T  (scores, [V x h])  -> warp softmax over V -> Xbar = alpha^T X  ([h x D])
 //   backward: dA = X dXbar^T ([V x h]) -> ds -> dX = [alpha | ds] [dXbar ; Ut]  ([V x D]),  dUt^T += ds^T X
 // X is read twice per direction (second pass mostly from L2); everything else is tiny.  This makes the kernels
 // HBM/L2-bound instead of fp32-ALU-bound (2*heads .. 4*heads FMA per token element on CUDA cores).
+#include <cuda.h>
 #include "frontend.cuh"
+#include "ptx.cuh"
 
 namespace orbit {
 namespace {
+using namespace ptx;
 
 constexpr int NT = 256;            // 8 warps
 constexpr int VP_MAX = 128;
 constexpr int HP = 16;             // heads padded to 16
 
 __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int bytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void ldsm4(uint32_t addr, uint32_t* r) {
   asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
@@ -48,14 +46,11 @@ struct Tl {
   __device__ static __forceinline__ uint32_t addr(uint32_t base, int row, int chunk) {
     return base + row * ROWB + ((chunk ^ (row & 7)) << 4);
   }
-  // rows [0, nrows_tile) <- g[(row) * ld + col0 ...]; rows >= nvalid zero-filled
-  __device__ static __forceinline__ void load_async(uint32_t base, const bf16* g, long long ld, int nrows_tile, int nvalid,
-                                                     int col0) {
-    for (int idx = threadIdx.x; idx < nrows_tile * CH; idx += NT) {
-      int r = idx / CH, c = idx - r * CH;
-      bool ok = r < nvalid;
-      cp_async16(addr(base, r, c), g + (size_t)(ok ? r : 0) * ld + col0 + c * 8, ok ? 16 : 0);
-    }
+  // B(k, n) = T[k][n]: 16 k from k0, 8 n from n0 -> r[0..1]
+  __device__ static __forceinline__ void ldB_nmajor8(uint32_t base, int k0, int n0, uint32_t* r) {
+    int lane = threadIdx.x & 31;
+    asm volatile("ldmatrix.sync.aligned.m8n8.x2.trans.shared.b16 {%0,%1}, [%2];"
+                 : "=r"(r[0]), "=r"(r[1]) : "r"(addr(base, k0 + (lane & 7) + ((lane >> 3) & 1) * 8, n0 >> 3)));
   }
   __device__ static __forceinline__ void ldA(uint32_t base, int r0, int k0, uint32_t* a) {
     int lane = threadIdx.x & 31;
@@ -94,38 +89,77 @@ __device__ __forceinline__ void chunk_scores(float (*acc)[4], uint32_t xc, int r
 
 constexpr int SROW = HP + 1;   // fp32 score matrix row stride (floats)
 
+// Both kernels stream their operands with TMA (cp.async.bulk.tensor, 128-byte swizzle = the XOR layout of Tl<64>): one
+// thread issues a few box copies per step instead of every thread issuing ~10 cp.async with their address arithmetic
+// (which was ~2/3 of the instructions of the cp.async versions; ncu: issue-bound at 2 warps per scheduler, not
+// HBM-bound).  The chunks of all patches of a CTA form ONE stream (n = patch_iter * 2 nch + i) through an STG-deep ring
+// of mbarrier-guarded stages, so the ring stays full across the softmax phase and across patch boundaries.
+// Box rows = V exactly (the next patch's rows must not land in the tile); tile rows V..Vp-1 are zeroed once.
+constexpr int TB = 64;                       // columns per TMA box / smem sub-tile (128 bytes: one swizzle span)
+constexpr int XT = VP_MAX * TB * 2;          // bytes of an X sub-tile   (16 KB)
+constexpr int UT = HP * TB * 2;              // bytes of a [16 x 64] sub-tile (2 KB)
+
+__device__ __forceinline__ void zero_tail_rows(uint8_t* tile, int r0, int r1, int nthreads) {
+  for (int i = r0 * 8 + threadIdx.x; i < r1 * 8; i += nthreads) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+}
+
 // ============================================ forward ============================================
-template <int DC>
-__global__ void __launch_bounds__(NT) agg_fwd_tc_kernel(const bf16* __restrict__ tok, const bf16* __restrict__ Utb /* [HP, D] */,
-    float* __restrict__ alpha, bf16* __restrict__ Xbar, int BL, int V, int D, int h) {
-  extern __shared__ __align__(1024) uint8_t smem[];
+// A step is NSUB = 2 sub-tiles (128 columns).  Pass 1: warp w < mtiles accumulates its 16 rows of scores.  Pass 2: warp w
+// owns 16 columns of the step (sub-tile w / 4, columns (w % 4) * 16).
+template <int STG>
+__global__ void __launch_bounds__(NT) agg_fwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
+    const __grid_constant__ CUtensorMap tmU, float* __restrict__ alpha, bf16* __restrict__ Xbar, int BL, int V, int D, int h) {
+  constexpr int NSUB = 2;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
   const int Vp = (V + 15) & ~15;
-  const int XB = VP_MAX * Tl<DC>::ROWB, UB = HP * Tl<DC>::ROWB;
-  const uint32_t sX = s_u32(smem), sU = sX + 2 * XB;
-  float* sS = reinterpret_cast<float*>(smem + 2 * XB + 2 * UB);            // [VP_MAX][SROW]
+  const uint32_t sX = s_u32(smem), sU = sX + STG * NSUB * XT;               // [STG][NSUB] tiles each
+  uint8_t* rest = smem + STG * NSUB * (XT + UT);
+  float* sS = reinterpret_cast<float*>(rest);                               // [VP_MAX][SROW]
   bf16* sAT = reinterpret_cast<bf16*>(sS + VP_MAX * SROW);                  // alpha^T [HP][ATROW]
   constexpr int ATROW = VP_MAX + 8;
   const uint32_t sATu = s_u32(sAT);
+  const uint32_t bar0 = s_u32(sAT + HP * ATROW);                            // full[STG]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const int nch = D / DC, mtiles = Vp / 16;
+  const int nch = D / (TB * NSUB), mtiles = Vp / 16;
 
-  for (int bl = blockIdx.x; bl < BL; bl += gridDim.x) {
-    const bf16* X = tok + (size_t)bl * V * D;
-    auto load = [&](int i) {            // i in [0, 2*nch): pass 1 (scores) then pass 2 (Xbar)
-      const int c = i % nch, buf = i & 1;
-      Tl<DC>::load_async(sX + buf * XB, X, D, Vp, V, c * DC);
-      if (i < nch) Tl<DC>::load_async(sU + buf * UB, Utb, D, HP, HP, c * DC);
-      cp_commit();
-    };
+  for (int j = 0; j < STG * NSUB; j++) zero_tail_rows(smem + j * XT, V, Vp, NT);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < STG; i++) mbar_init(bar0 + 8 * i, 1);
+    fence_barrier_init();
+  }
+  fence_proxy_async();
+  __syncthreads();
+
+  const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+  const int per = 2 * nch, total = npat * per;
+  auto issue = [&](int n) {             // thread 0: n-th step of this CTA: pass 1 (scores) then pass 2 (Xbar) of each patch
+    if (n >= total) return;
+    const int pi = n / per, i = n - pi * per, c = i % nch, st = n % STG;
+    const int row0 = (blockIdx.x + pi * gridDim.x) * V;
+    const uint32_t bar = bar0 + 8 * st;
+    mbar_expect_tx(bar, NSUB * (V * TB * 2 + (i < nch ? UT : 0)));
+#pragma unroll
+    for (int j = 0; j < NSUB; j++) {
+      tma_load_2d(sX + (st * NSUB + j) * XT, &tmX, bar, (c * NSUB + j) * TB, row0);
+      if (i < nch) tma_load_2d(sU + (st * NSUB + j) * UT, &tmU, bar, (c * NSUB + j) * TB, 0);
+    }
+  };
+  if (threadIdx.x == 0) for (int n = 0; n < STG - 1; n++) issue(n);
+
+  for (int pi = 0; pi < npat; pi++) {
+    const int bl = blockIdx.x + pi * gridDim.x, n0 = pi * per;
     float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-    __syncthreads();                    // previous patch finished with every buffer
-    load(0);
     // ---- pass 1: S[v, a] = X_v . Ut[a, :]
     for (int i = 0; i < nch; i++) {
-      cp_wait<0>();
-      __syncthreads();
-      load(i + 1);                      // i + 1 == nch starts pass 2's first chunk
-      if (warp < mtiles) chunk_scores<DC>(acc, sX + (i & 1) * XB, warp * 16, sU + (i & 1) * UB);
+      const int n = n0 + i, st = n % STG;
+      mbar_wait(bar0 + 8 * st, (n / STG) & 1);
+      __syncthreads();                  // step n - 1 is finished everywhere: its stage is free (and sS / sAT of the previous patch)
+      if (threadIdx.x == 0) issue(n + STG - 1);
+      if (warp < mtiles) {
+#pragma unroll
+        for (int j = 0; j < NSUB; j++) chunk_scores<TB>(acc, sX + (st * NSUB + j) * XT, warp * 16, sU + (st * NSUB + j) * UT);
+      }
     }
     if (warp < mtiles) {
 #pragma unroll
@@ -156,31 +190,31 @@ __global__ void __launch_bounds__(NT) agg_fwd_tc_kernel(const bf16* __restrict__
       }
     }
     __syncthreads();
-    // ---- pass 2: Xbar[a, d] = sum_v alpha[v, a] X[v, d]; warp w owns DC/8 columns of the chunk
+    // ---- pass 2: Xbar[a, d] = sum_v alpha[v, a] X[v, d]
     uint32_t af[VP_MAX / 16][4];
 #pragma unroll
     for (int ks = 0; ks < VP_MAX / 16; ks++)
       if (ks < mtiles) ldA_plain(sATu, ATROW * 2, 0, ks * 16, af[ks]);
-    constexpr int WN = DC / 8;          // columns per warp per chunk (16 for DC = 128, 8 for DC = 64)
     for (int i = nch; i < 2 * nch; i++) {
-      cp_wait<0>();
+      const int n = n0 + i, st = n % STG;
+      mbar_wait(bar0 + 8 * st, (n / STG) & 1);
       __syncthreads();
-      if (i + 1 < 2 * nch) load(i + 1);
-      const uint32_t xc = sX + (i & 1) * XB;
+      if (threadIdx.x == 0) issue(n + STG - 1);
+      const uint32_t xc = sX + (st * NSUB + (warp >> 2)) * XT;
+      const int cg = (warp & 3) * 16;
       float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-      const int n0 = (warp * WN) & ~15;  // 16-column group holding this warp's columns
 #pragma unroll
       for (int ks = 0; ks < VP_MAX / 16; ks++) {
         if (ks < mtiles) {
           uint32_t b[4];
-          Tl<DC>::ldB_nmajor(xc, ks * 16, n0, b);
-          if (WN == 16) { mma16816(o[0], af[ks], b[0], b[1]); mma16816(o[1], af[ks], b[2], b[3]); }
-          else { if (warp & 1) mma16816(o[0], af[ks], b[2], b[3]); else mma16816(o[0], af[ks], b[0], b[1]); }
+          Tl<TB>::ldB_nmajor(xc, ks * 16, cg, b);
+          mma16816(o[0], af[ks], b[0], b[1]);
+          mma16816(o[1], af[ks], b[2], b[3]);
         }
       }
-      const int c = (i - nch) * DC + warp * WN;
+      const int c = (i - nch) * (TB * NSUB) + (warp >> 2) * TB + cg;
 #pragma unroll
-      for (int nt = 0; nt < WN / 8; nt++) {
+      for (int nt = 0; nt < 2; nt++) {
         const int d = c + nt * 8 + 2 * t;
         if (g < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g) * D + d) = pack_bf16(o[nt][0], o[nt][1]);
         if (g + 8 < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g + 8) * D + d) = pack_bf16(o[nt][2], o[nt][3]);
@@ -190,62 +224,109 @@ __global__ void __launch_bounds__(NT) agg_fwd_tc_kernel(const bf16* __restrict__
 }
 
 // ============================================ backward ============================================
-template <int DC>
-__global__ void __launch_bounds__(NT) agg_bwd_tc_kernel(const bf16* __restrict__ tok, const bf16* __restrict__ Utb,
-    const float* __restrict__ alpha, const bf16* __restrict__ dXbar, bf16* __restrict__ dtok, float* __restrict__ dUt_acc,
-    int BL, int V, int D, int h) {
-  extern __shared__ __align__(1024) uint8_t smem[];
+// 16 warps, one 64-column sub-tile per step (the [HP][D] fp32 dUt accumulator takes most of the shared memory).  Pass 1:
+// warp w takes row tile (w & 7) and k half (w >> 3) of the chunk; pass 2: warps 0-7 produce dX (one 16-row tile each)
+// while warps 8-15 accumulate dUt^T (one 8-column group of the chunk each).  dX leaves through a per-warp XOR-swizzled
+// staging tile (aliasing the dalpha / alpha score buffers, dead in pass 2) as 16-byte pieces, 128 contiguous bytes of a
+// token row per 8 lanes, instead of 4-byte pieces of 16 rows.
+constexpr int NTB = 512;
+constexpr int BT = 2 * UT;                   // B tile: rows 0-15 dXbar chunk, 16-31 Ut chunk
+template <int STG>
+__global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
+    const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmU,
+    const float* __restrict__ alpha, bf16* __restrict__ dtok, float* __restrict__ dUt_acc, int BL, int V, int D, int h) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
   const int Vp = (V + 15) & ~15;
-  const int XB = VP_MAX * Tl<DC>::ROWB, BB = 2 * HP * Tl<DC>::ROWB;          // B tile: rows 0-15 dXbar chunk, 16-31 Ut chunk
-  const uint32_t sX = s_u32(smem), sB = sX + 2 * XB;
-  float* sS = reinterpret_cast<float*>(smem + 2 * XB + 2 * BB);              // [VP_MAX][SROW] dalpha
+  const uint32_t sX = s_u32(smem), sB = sX + STG * XT;
+  float* sS = reinterpret_cast<float*>(smem + STG * (XT + BT));              // [VP_MAX][SROW] dalpha
   float* sAl = sS + VP_MAX * SROW;                                            // [VP_MAX][SROW] alpha
   bf16* sAD = reinterpret_cast<bf16*>(sAl + VP_MAX * SROW);                  // [VP_MAX][ADROW]  (alpha | ds)
   constexpr int ADROW = 2 * HP + 8;
   bf16* sDT = sAD + VP_MAX * ADROW;                                          // ds^T [HP][DTROW]
   constexpr int DTROW = VP_MAX + 8;
-  float* sAcc = reinterpret_cast<float*>(sDT + HP * DTROW);                  // [HP][D] block-private dUt^T accumulator
+  float* sAcc = reinterpret_cast<float*>(sDT + HP * DTROW);                  // [HP][D + 8] block-private dUt^T accumulator
+  const int AR = D + 8;                                                       // padded: rows g, g + 1 are 8 banks apart
+  const uint32_t bar0 = s_u32(sAcc + HP * AR);                               // full[STG]
   const uint32_t sADu = s_u32(sAD), sDTu = s_u32(sDT);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const int nch = D / DC, mtiles = Vp / 16;
+  const int wt = warp & 7, wh = warp >> 3;
+  const int nch = D / TB, mtiles = Vp / 16;
+  uint8_t* sO = reinterpret_cast<uint8_t*>(sS) + wt * (16 * 128);            // [16][64] bf16, swizzled (2 KB per dX warp <= sS + sAl)
+  static_assert(8 * 16 * 128 <= 2 * VP_MAX * SROW * 4, "staging tiles must fit in the score buffers");
 
-  for (int i = threadIdx.x; i < HP * D; i += NT) sAcc[i] = 0.f;
+  for (int i = threadIdx.x; i < HP * AR; i += NTB) sAcc[i] = 0.f;
+  for (int j = 0; j < STG; j++) {
+    zero_tail_rows(smem + j * XT, V, Vp, NTB);
+    zero_tail_rows(smem + STG * XT + j * BT, h, HP, NTB);
+  }
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < STG; i++) mbar_init(bar0 + 8 * i, 1);
+    fence_barrier_init();
+  }
+  fence_proxy_async();
+  __syncthreads();
 
-  for (int bl = blockIdx.x; bl < BL; bl += gridDim.x) {
-    const bf16* X = tok + (size_t)bl * V * D;
-    const bf16* dXb = dXbar + (size_t)bl * h * D;
-    auto load = [&](int i) {
-      const int c = i % nch, buf = i & 1;
-      Tl<DC>::load_async(sX + buf * XB, X, D, Vp, V, c * DC);
-      Tl<DC>::load_async(sB + buf * BB, dXb, D, HP, h, c * DC);
-      if (i >= nch) Tl<DC>::load_async(sB + buf * BB + HP * Tl<DC>::ROWB, Utb, D, HP, HP, c * DC);
-      cp_commit();
-    };
+  const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+  const int per = 2 * nch, total = npat * per;
+  auto issue = [&](int n) {             // thread 0
+    if (n >= total) return;
+    const int pi = n / per, i = n - pi * per, c = i % nch, st = n % STG;
+    const int bl = blockIdx.x + pi * gridDim.x;
+    const uint32_t bar = bar0 + 8 * st;
+    mbar_expect_tx(bar, (V + h) * TB * 2 + (i >= nch ? UT : 0));
+    tma_load_2d(sX + st * XT, &tmX, bar, c * TB, bl * V);
+    tma_load_2d(sB + st * BT, &tmG, bar, c * TB, bl * h);
+    if (i >= nch) tma_load_2d(sB + st * BT + UT, &tmU, bar, c * TB, 0);
+  };
+  if (threadIdx.x == 0) for (int n = 0; n < STG - 1; n++) issue(n);
+
+  for (int pi = 0; pi < npat; pi++) {
+    const int bl = blockIdx.x + pi * gridDim.x, n0 = pi * per;
     float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-    __syncthreads();
-    load(0);
-    for (int i = threadIdx.x; i < Vp * HP; i += NT) {
+    __syncthreads();                    // previous patch finished with the score / staging buffers
+    for (int i = threadIdx.x; i < Vp * HP; i += NTB) {
       int v = i / HP, a = i - v * HP;
       sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
     }
-    // ---- pass 1: dalpha[v, a] = X_v . dXbar[a, :]
+    // ---- pass 1: dalpha[v, a] = X_v . dXbar[a, :]   (k half wh of every chunk)
     for (int i = 0; i < nch; i++) {
-      cp_wait<0>();
+      const int n = n0 + i, st = n % STG;
+      mbar_wait(bar0 + 8 * st, (n / STG) & 1);
       __syncthreads();
-      load(i + 1);
-      if (warp < mtiles) chunk_scores<DC>(acc, sX + (i & 1) * XB, warp * 16, sB + (i & 1) * BB);
+      if (threadIdx.x == 0) issue(n + STG - 1);
+      if (wt < mtiles) {
+        const uint32_t xc = sX + st * XT, bc = sB + st * BT;
+#pragma unroll
+        for (int ks = 0; ks < TB / 32; ks++) {
+          uint32_t a[4], b[4];
+          Tl<TB>::ldA(xc, wt * 16, (wh * (TB / 32) + ks) * 16, a);
+          Tl<TB>::ldB_kmajor(bc, 0, (wh * (TB / 32) + ks) * 16, b);
+          mma16816(acc[0], a, b[0], b[1]);
+          mma16816(acc[1], a, b[2], b[3]);
+        }
+      }
     }
-    if (warp < mtiles) {
+    if (wt < mtiles && wh == 0) {
 #pragma unroll
       for (int nt = 0; nt < 2; nt++) {
-        int r = warp * 16 + g, c = nt * 8 + 2 * t;
+        int r = wt * 16 + g, c = nt * 8 + 2 * t;
         sS[r * SROW + c] = acc[nt][0]; sS[r * SROW + c + 1] = acc[nt][1];
         sS[(r + 8) * SROW + c] = acc[nt][2]; sS[(r + 8) * SROW + c + 1] = acc[nt][3];
       }
     }
     __syncthreads();
+    if (wt < mtiles && wh == 1) {
+#pragma unroll
+      for (int nt = 0; nt < 2; nt++) {
+        int r = wt * 16 + g, c = nt * 8 + 2 * t;
+        sS[r * SROW + c] += acc[nt][0]; sS[r * SROW + c + 1] += acc[nt][1];
+        sS[(r + 8) * SROW + c] += acc[nt][2]; sS[(r + 8) * SROW + c + 1] += acc[nt][3];
+      }
+    }
+    __syncthreads();
     // ---- ds[v, a] = alpha (dalpha - sum_w alpha_w dalpha_w); A operands (alpha | ds) and ds^T in bf16
-    for (int a = warp; a < HP; a += NT / 32) {
+    for (int a = warp; a < HP; a += NTB / 32) {
       float dot = 0.f;
       for (int v = lane; v < V; v += 32) dot += sAl[v * SROW + a] * sS[v * SROW + a];
       dot = warp_sum(dot);
@@ -259,63 +340,71 @@ __global__ void __launch_bounds__(NT) agg_bwd_tc_kernel(const bf16* __restrict__
     }
     __syncthreads();
     uint32_t adf[2][4];                 // this warp's 16 rows of (alpha | ds): K = 32 -> 2 k-steps
-    if (warp < mtiles) {
-      ldA_plain(sADu, ADROW * 2, warp * 16, 0, adf[0]);
-      ldA_plain(sADu, ADROW * 2, warp * 16, 16, adf[1]);
+    if (wh == 0 && wt < mtiles) {
+      ldA_plain(sADu, ADROW * 2, wt * 16, 0, adf[0]);
+      ldA_plain(sADu, ADROW * 2, wt * 16, 16, adf[1]);
     }
     // ---- pass 2: dX chunk = (alpha | ds) [dXbar ; Ut] chunk;  dUt^T chunk += ds^T X chunk
     for (int i = nch; i < 2 * nch; i++) {
-      cp_wait<0>();
+      const int n = n0 + i, st = n % STG;
+      mbar_wait(bar0 + 8 * st, (n / STG) & 1);
       __syncthreads();
-      if (i + 1 < 2 * nch) load(i + 1);
-      const uint32_t xc = sX + (i & 1) * XB, bc = sB + (i & 1) * BB;
-      const int c0 = (i - nch) * DC;
-      if (warp < mtiles) {
+      if (threadIdx.x == 0) issue(n + STG - 1);
+      const uint32_t xc = sX + st * XT, bc = sB + st * BT;
+      const int c0 = (i - nch) * TB;
+      if (wh == 0) {
+        if (wt < mtiles) {
 #pragma unroll
-        for (int np = 0; np < DC / 16; np++) {
-          float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+          for (int np = 0; np < TB / 16; np++) {
+            float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
 #pragma unroll
-          for (int ks = 0; ks < 2; ks++) {
-            uint32_t b[4];
-            Tl<DC>::ldB_nmajor(bc, ks * 16, np * 16, b);
-            mma16816(o[0], adf[ks], b[0], b[1]);
-            mma16816(o[1], adf[ks], b[2], b[3]);
+            for (int ks = 0; ks < 2; ks++) {
+              uint32_t b[4];
+              Tl<TB>::ldB_nmajor(bc, ks * 16, np * 16, b);
+              mma16816(o[0], adf[ks], b[0], b[1]);
+              mma16816(o[1], adf[ks], b[2], b[3]);
+            }
+#pragma unroll
+            for (int nt = 0; nt < 2; nt++) {
+              const int ch = np * 2 + nt;                 // 16-byte chunk of the 128-byte staging row
+              *reinterpret_cast<uint32_t*>(sO + g * 128 + ((ch ^ g) << 4) + t * 4) = pack_bf16(o[nt][0], o[nt][1]);
+              *reinterpret_cast<uint32_t*>(sO + (g + 8) * 128 + ((ch ^ g) << 4) + t * 4) = pack_bf16(o[nt][2], o[nt][3]);
+            }
           }
-          const int r = warp * 16 + g;
+          __syncwarp();
 #pragma unroll
-          for (int nt = 0; nt < 2; nt++) {
-            const int d = c0 + np * 16 + nt * 8 + 2 * t;
-            if (r < V) *reinterpret_cast<uint32_t*>(dtok + ((size_t)bl * V + r) * D + d) = pack_bf16(o[nt][0], o[nt][1]);
-            if (r + 8 < V) *reinterpret_cast<uint32_t*>(dtok + ((size_t)bl * V + r + 8) * D + d) = pack_bf16(o[nt][2], o[nt][3]);
+          for (int q = 0; q < 4; q++) {
+            const int row = q * 4 + (lane >> 3), ch = lane & 7, r = wt * 16 + row;
+            if (r < V)
+              *reinterpret_cast<uint4*>(dtok + ((size_t)bl * V + r) * D + c0 + ch * 8) =
+                  *reinterpret_cast<const uint4*>(sO + row * 128 + ((ch ^ (row & 7)) << 4));
           }
         }
-      }
-      // dUt^T[a, c0 + ...] += sum_v ds[v, a] X[v, ...]: 16-column groups over the warps
-      for (int np = (warp + 4) & 7; np < DC / 16; np += NT / 32) {   // warps 4..7 (the dX warps are 0..mtiles-1)
-        float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+      } else {
+        // dUt^T[a, c0 + 8 wt ...] += sum_v ds[v, a] X[v, ...]
+        float o[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int ks = 0; ks < VP_MAX / 16; ks++) {
           if (ks < mtiles) {
-            uint32_t a[4], b[4];
+            uint32_t a[4], b[2];
             ldA_plain(sDTu, DTROW * 2, 0, ks * 16, a);
-            Tl<DC>::ldB_nmajor(xc, ks * 16, np * 16, b);
-            mma16816(o[0], a, b[0], b[1]);
-            mma16816(o[1], a, b[2], b[3]);
+            Tl<TB>::ldB_nmajor8(xc, ks * 16, wt * 8, b);
+            mma16816(o, a, b[0], b[1]);
           }
         }
-#pragma unroll
-        for (int nt = 0; nt < 2; nt++) {
-          const int d = c0 + np * 16 + nt * 8 + 2 * t;
-          sAcc[g * D + d] += o[nt][0]; sAcc[g * D + d + 1] += o[nt][1];
-          sAcc[(g + 8) * D + d] += o[nt][2]; sAcc[(g + 8) * D + d + 1] += o[nt][3];
-        }
+        const int d = c0 + wt * 8 + 2 * t;
+        float2* p0 = reinterpret_cast<float2*>(sAcc + g * AR + d);
+        float2* p1 = reinterpret_cast<float2*>(sAcc + (g + 8) * AR + d);
+        float2 v0 = *p0, v1 = *p1;
+        v0.x += o[0]; v0.y += o[1]; v1.x += o[2]; v1.y += o[3];
+        *p0 = v0; *p1 = v1;
       }
     }
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < h * D; i += NT) {
+  for (int i = threadIdx.x; i < h * D; i += NTB) {
     int a = i / D, d = i - a * D;
-    atomicAdd(dUt_acc + (size_t)d * h + a, sAcc[i]);
+    atomicAdd(dUt_acc + (size_t)d * h + a, sAcc[a * AR + d]);
   }
 }
 
@@ -327,17 +416,42 @@ __global__ void agg_ut_to_bf16_kernel(const float* __restrict__ Ut, bf16* __rest
   Utb[i] = __float2bfloat16_rn(a < h ? Ut[(size_t)d * h + a] : 0.f);
 }
 
-template <int DC> size_t fwd_smem() {
-  return 2 * (size_t)VP_MAX * Tl<DC>::ROWB + 2 * (size_t)HP * Tl<DC>::ROWB + (size_t)VP_MAX * SROW * 4 + (size_t)HP * (VP_MAX + 8) * 2;
+size_t fwd_smem(int stg) {
+  return 1024 + (size_t)stg * 2 * (XT + UT) + (size_t)VP_MAX * SROW * 4 + (size_t)HP * (VP_MAX + 8) * 2 + 8 * stg;
 }
-template <int DC> size_t bwd_smem(int D) {
-  return 2 * (size_t)VP_MAX * Tl<DC>::ROWB + 2 * (size_t)2 * HP * Tl<DC>::ROWB + 2 * (size_t)VP_MAX * SROW * 4 +
-         (size_t)VP_MAX * (2 * HP + 8) * 2 + (size_t)HP * (VP_MAX + 8) * 2 + (size_t)HP * D * 4;
+size_t bwd_smem(int D, int stg) {
+  return 1024 + (size_t)stg * (XT + BT) + 2 * (size_t)VP_MAX * SROW * 4 + (size_t)VP_MAX * (2 * HP + 8) * 2 +
+         (size_t)HP * (VP_MAX + 8) * 2 + (size_t)HP * (D + 8) * 4 + 8 * stg;
+}
+constexpr size_t SMEM_MAX = 227 * 1024;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+// bf16 matrix [rows, D] row-major -> boxes of [box_rows x 64 columns], 128-byte swizzle
+int make_map(CUtensorMap* tm, const void* base, long long rows, int D, int box_rows) {
+  static EncodeTiledFn enc = nullptr;
+  if (!enc) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
+    enc = (EncodeTiledFn)p;
+  }
+  cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)D * 2};
+  cuuint32_t box[2] = {(cuuint32_t)TB, (cuuint32_t)box_rows};
+  cuuint32_t es[2] = {1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("aggregate: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
+  return ORBIT_OK;
 }
 }  // namespace
 
 bool agg_tc_supported(int dt, int V, int D, int heads) {
-  return dt == ORBIT_BF16 && heads <= HP && V <= VP_MAX && D % 128 == 0 && bwd_smem<64>(D) <= 225 * 1024;
+  return dt == ORBIT_BF16 && heads <= HP && V <= VP_MAX && D % 128 == 0 && bwd_smem(D, 2) <= SMEM_MAX;
 }
 size_t agg_tc_utb_bytes(int D) { return (size_t)HP * D * sizeof(bf16); }
 
@@ -345,23 +459,35 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
                      cudaStream_t s) {
   agg_ut_to_bf16_kernel<<<cdiv((long long)HP * D, 256), 256, 0, s>>>(Ut, (bf16*)Utb, D, heads);
   ORBIT_LAUNCH_CHECK();
-  constexpr int DC = 128;
+  CUtensorMap tmX, tmU;
+  ORBIT_TRY(make_map(&tmX, tok, (long long)BL * V, D, V));
+  ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
+  constexpr int STG = 3;                // 3 x 36 KB stages + 13 KB: one or two CTAs per SM
+  const size_t smb = fwd_smem(STG);
   static bool set = false;
-  if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_fwd_tc_kernel<DC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fwd_smem<DC>())); set = true; }
-  int grid = BL < 148 * 2 ? BL : 148 * 2;
-  agg_fwd_tc_kernel<DC><<<grid, NT, fwd_smem<DC>(), s>>>((const bf16*)tok, (const bf16*)Utb, alpha, (bf16*)Xbar, BL, V, D, heads);
+  if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_fwd_tma_kernel<STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }
+  const int grid = BL < 148 ? BL : 148;
+  agg_fwd_tma_kernel<STG><<<grid, NT, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
 
 int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const void* dXbar, void* dtok, float* dUt_acc,
                      int BL, int V, int D, int heads, cudaStream_t s) {
-  constexpr int DC = 64;
-  const size_t smb = bwd_smem<DC>(D);
-  ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_bwd_tc_kernel<DC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));
-  int grid = BL < 148 ? BL : 148;
-  agg_bwd_tc_kernel<DC><<<grid, NT, smb, s>>>((const bf16*)tok, (const bf16*)Utb, alpha, (const bf16*)dXbar, (bf16*)dtok, dUt_acc,
-                                              BL, V, D, heads);
+  CUtensorMap tmX, tmG, tmU;
+  ORBIT_TRY(make_map(&tmX, tok, (long long)BL * V, D, V));
+  ORBIT_TRY(make_map(&tmG, dXbar, (long long)BL * heads, D, heads));
+  ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
+  const int grid = BL < 148 ? BL : 148;
+  int stg = 4;                          // deepest ring that fits beside the [HP][D] fp32 dUt accumulator
+  while (stg > 2 && bwd_smem(D, stg) > SMEM_MAX) stg--;
+  const size_t smb = bwd_smem(D, stg);
+#define AB(S) do {                                                                                            \
+    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_bwd_tma_kernel<S>,                                \
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));            \
+    agg_bwd_tma_kernel<S><<<grid, NTB, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads); } while (0)
+  if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
+#undef AB
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

@@ -15,6 +15,7 @@ namespace {
 constexpr int NT = 256;
 constexpr int DCH = 512;                 // columns per CTA
 constexpr int BROW = (DCH + 8) * 2;      // padded smem row of the B tiles (bytes): conflict-free ldmatrix
+constexpr int OROW = (64 + 8) * 2;       // padded row of a warp's output staging tile (bytes)
 
 __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
@@ -63,8 +64,11 @@ __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, cons
   extern __shared__ __align__(128) uint8_t smem[];
   uint8_t* sA = smem;                                     // [PT][KP + 8] bf16
   uint8_t* sB = smem + PT * AROW;                         // [KP][DCH + 8] bf16
-  const int v = blockIdx.y, c0 = blockIdx.z * DCH;
-  const int BL = d.B * L, bl0 = blockIdx.x * PT;
+  // blockIdx.x = (v, column chunk): CTAs that run together write neighbouring 1 KB pieces of the same token rows
+  // ([V x D] of a patch is contiguous), instead of pieces V*D*2 bytes apart.
+  const int nz = gridDim.x / d.V;
+  const int v = blockIdx.x / nz, c0 = (blockIdx.x - v * nz) * DCH;
+  const int BL = d.B * L, bl0 = blockIdx.y * PT;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int ncol = min(DCH, d.D - c0);
   // A: [hi | lo | 0] of the pixels
@@ -92,29 +96,45 @@ __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, cons
 #pragma unroll
     for (int ks = 0; ks < KP / 16; ks++) ldsm4(s_u32(sA) + row * AROW + (ks * 16 + (lane >> 4) * 8) * 2, af[ks]);
   }
-  const int r_lo = bl0 + warp * 16 + g, r_hi = r_lo + 8;
-  bf16* o_lo = tok + ((size_t)r_lo * d.V + v) * d.D + c0;
-  bf16* o_hi = tok + ((size_t)r_hi * d.V + v) * d.D + c0;
+  // Epilogue: the m16n8 accumulator layout gives a thread 4-byte pieces of 16 different rows, so direct stores fill
+  // half a 32-byte sector per instruction.  Each warp stages 16 rows x 64 columns (+ bias) in shared memory and
+  // writes them back as 16-byte pieces: 8 lanes cover 128 contiguous bytes of one token row.
+  uint8_t* sO = sB + KP * BROW + warp * (16 * OROW);      // [16][64 + 8] bf16 per warp
+  const int r0 = bl0 + warp * 16;
   const bf16* bias = bp + (size_t)v * d.D + c0;
   const uint32_t sBu = s_u32(sB);
-#pragma unroll 2
-  for (int np = 0; np < DCH / 16; np++) {
-    if (np * 16 >= ncol) break;
-    float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+  for (int ng = 0; ng < DCH / 64; ng++) {
+    if (ng * 64 >= ncol) break;
 #pragma unroll
-    for (int ks = 0; ks < KP / 16; ks++) {
-      uint32_t b[4];
-      ldB(sBu, ks * 16, np * 16, b);
-      mma16816(acc[0], af[ks], b[0], b[1]);
-      mma16816(acc[1], af[ks], b[2], b[3]);
-    }
+    for (int j = 0; j < 4; j++) {
+      const int np = ng * 4 + j;
+      float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
 #pragma unroll
-    for (int nt = 0; nt < 2; nt++) {
-      const int col = np * 16 + nt * 8 + 2 * t;
-      const float2 bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + col));
-      if (r_lo < BL) *reinterpret_cast<uint32_t*>(o_lo + col) = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
-      if (r_hi < BL) *reinterpret_cast<uint32_t*>(o_hi + col) = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
+      for (int ks = 0; ks < KP / 16; ks++) {
+        uint32_t b[4];
+        ldB(sBu, ks * 16, np * 16, b);
+        mma16816(acc[0], af[ks], b[0], b[1]);
+        mma16816(acc[1], af[ks], b[2], b[3]);
+      }
+#pragma unroll
+      for (int nt = 0; nt < 2; nt++) {
+        const int cl = j * 16 + nt * 8 + 2 * t;           // column inside the 64-column group
+        float2 bb = make_float2(0.f, 0.f);
+        if (ng * 64 + cl < ncol) bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + ng * 64 + cl));
+        *reinterpret_cast<uint32_t*>(sO + g * OROW + cl * 2) = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
+        *reinterpret_cast<uint32_t*>(sO + (g + 8) * OROW + cl * 2) = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
+      }
     }
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+      const int row = q * 4 + (lane >> 3), ch = lane & 7;
+      const int col = ng * 64 + ch * 8;
+      if (r0 + row < BL && col < ncol)
+        *reinterpret_cast<uint4*>(tok + ((size_t)(r0 + row) * d.V + v) * d.D + c0 + col) =
+            *reinterpret_cast<const uint4*>(sO + row * OROW + ch * 16);
+    }
+    __syncwarp();
   }
 }
 
@@ -215,9 +235,9 @@ bool tokenize_tc_supported(const orbit_embed_desc& d) {
 
 int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, const void* bp, void* tok, cudaStream_t s) {
   const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
-  dim3 grid(cdiv((long long)d.B * L, 128), d.V, cdiv(d.D, DCH));
+  dim3 grid(d.V * cdiv(d.D, DCH), cdiv((long long)d.B * L, 128));
 #define TF(P, K) do {                                                                                         \
-    const size_t smb = (size_t)128 * (K + 8) * 2 + (size_t)K * BROW;                                          \
+    const size_t smb = (size_t)128 * (K + 8) * 2 + (size_t)K * BROW + (size_t)(NT / 32) * 16 * OROW;                                        \
     static bool set = false;                                                                                  \
     if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)tok_fwd_tc_kernel<P, K>,                  \
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }       \

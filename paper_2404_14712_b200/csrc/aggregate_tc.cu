@@ -104,10 +104,12 @@ __device__ __forceinline__ void zero_tail_rows(uint8_t* tile, int r0, int r1, in
 }
 
 // ============================================ forward ============================================
-// A step is NSUB = 2 sub-tiles (128 columns).  Pass 1: warp w < mtiles accumulates its 16 rows of scores.  Pass 2: warp w
-// owns 16 columns of the step (sub-tile w / 4, columns (w % 4) * 16).
+// A step is NSUB = 2 sub-tiles (128 columns); 16 warps = two groups of 8, group wh works on sub-tile wh.  Pass 1: warp
+// (wh, wt < mtiles) accumulates the scores of its 16 rows over its sub-tiles (the two groups' halves are summed through
+// shared memory).  Pass 2: warp (wh, wt) owns 8 columns of sub-tile wh.
+constexpr int NTF = 512;
 template <int STG>
-__global__ void __launch_bounds__(NT) agg_fwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
+__global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
     const __grid_constant__ CUtensorMap tmU, float* __restrict__ alpha, bf16* __restrict__ Xbar, int BL, int V, int D, int h) {
   constexpr int NSUB = 2;
   extern __shared__ uint8_t smem_raw[];
@@ -121,9 +123,10 @@ __global__ void __launch_bounds__(NT) agg_fwd_tma_kernel(const __grid_constant__
   const uint32_t sATu = s_u32(sAT);
   const uint32_t bar0 = s_u32(sAT + HP * ATROW);                            // full[STG]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int wt = warp & 7, wh = warp >> 3;
   const int nch = D / (TB * NSUB), mtiles = Vp / 16;
 
-  for (int j = 0; j < STG * NSUB; j++) zero_tail_rows(smem + j * XT, V, Vp, NT);
+  for (int j = 0; j < STG * NSUB; j++) zero_tail_rows(smem + j * XT, V, Vp, NTF);
   if (threadIdx.x == 0) {
     for (int i = 0; i < STG; i++) mbar_init(bar0 + 8 * i, 1);
     fence_barrier_init();
@@ -135,7 +138,7 @@ __global__ void __launch_bounds__(NT) agg_fwd_tma_kernel(const __grid_constant__
   const int per = 2 * nch, total = npat * per;
   auto issue = [&](int n) {             // thread 0: n-th step of this CTA: pass 1 (scores) then pass 2 (Xbar) of each patch
     if (n >= total) return;
-    const int pi = n / per, i = n - pi * per, c = i % nch, st = n % STG;
+    const int pi = n / per, i = n - pi * per, c = i < nch ? i : per - 1 - i, st = n % STG;   // pass 2 walks back
     const int row0 = (blockIdx.x + pi * gridDim.x) * V;
     const uint32_t bar = bar0 + 8 * st;
     mbar_expect_tx(bar, NSUB * (V * TB * 2 + (i < nch ? UT : 0)));
@@ -156,22 +159,28 @@ __global__ void __launch_bounds__(NT) agg_fwd_tma_kernel(const __grid_constant__
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
       __syncthreads();                  // step n - 1 is finished everywhere: its stage is free (and sS / sAT of the previous patch)
       if (threadIdx.x == 0) issue(n + STG - 1);
-      if (warp < mtiles) {
-#pragma unroll
-        for (int j = 0; j < NSUB; j++) chunk_scores<TB>(acc, sX + (st * NSUB + j) * XT, warp * 16, sU + (st * NSUB + j) * UT);
-      }
+      if (wt < mtiles) chunk_scores<TB>(acc, sX + (st * NSUB + wh) * XT, wt * 16, sU + (st * NSUB + wh) * UT);
     }
-    if (warp < mtiles) {
+    if (wt < mtiles && wh == 0) {
 #pragma unroll
       for (int nt = 0; nt < 2; nt++) {
-        int r = warp * 16 + g, c = nt * 8 + 2 * t;
+        int r = wt * 16 + g, c = nt * 8 + 2 * t;
         sS[r * SROW + c] = acc[nt][0]; sS[r * SROW + c + 1] = acc[nt][1];
         sS[(r + 8) * SROW + c] = acc[nt][2]; sS[(r + 8) * SROW + c + 1] = acc[nt][3];
       }
     }
     __syncthreads();
+    if (wt < mtiles && wh == 1) {
+#pragma unroll
+      for (int nt = 0; nt < 2; nt++) {
+        int r = wt * 16 + g, c = nt * 8 + 2 * t;
+        sS[r * SROW + c] += acc[nt][0]; sS[r * SROW + c + 1] += acc[nt][1];
+        sS[(r + 8) * SROW + c] += acc[nt][2]; sS[(r + 8) * SROW + c + 1] += acc[nt][3];
+      }
+    }
+    __syncthreads();
     // ---- softmax over v per head; alpha -> global (fp32) and alpha^T (bf16) -> smem
-    for (int a = warp; a < HP; a += NT / 32) {
+    for (int a = warp; a < HP; a += NTF / 32) {
       if (a < h) {
         float m = -INFINITY;
         for (int v = lane; v < V; v += 32) m = fmaxf(m, sS[v * SROW + a]);
@@ -200,25 +209,19 @@ __global__ void __launch_bounds__(NT) agg_fwd_tma_kernel(const __grid_constant__
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
       __syncthreads();
       if (threadIdx.x == 0) issue(n + STG - 1);
-      const uint32_t xc = sX + (st * NSUB + (warp >> 2)) * XT;
-      const int cg = (warp & 3) * 16;
-      float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+      const uint32_t xc = sX + (st * NSUB + wh) * XT;
+      float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};      // two accumulation chains (even / odd k-steps)
 #pragma unroll
       for (int ks = 0; ks < VP_MAX / 16; ks++) {
         if (ks < mtiles) {
-          uint32_t b[4];
-          Tl<TB>::ldB_nmajor(xc, ks * 16, cg, b);
-          mma16816(o[0], af[ks], b[0], b[1]);
-          mma16816(o[1], af[ks], b[2], b[3]);
+          uint32_t b[2];
+          Tl<TB>::ldB_nmajor8(xc, ks * 16, wt * 8, b);
+          mma16816(o[ks & 1], af[ks], b[0], b[1]);
         }
       }
-      const int c = (i - nch) * (TB * NSUB) + (warp >> 2) * TB + cg;
-#pragma unroll
-      for (int nt = 0; nt < 2; nt++) {
-        const int d = c + nt * 8 + 2 * t;
-        if (g < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g) * D + d) = pack_bf16(o[nt][0], o[nt][1]);
-        if (g + 8 < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g + 8) * D + d) = pack_bf16(o[nt][2], o[nt][3]);
-      }
+      const int d = (per - 1 - i) * (TB * NSUB) + wh * TB + wt * 8 + 2 * t;   // pass 2 runs from the last chunk back (L2 reuse distance)
+      if (g < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g) * D + d) = pack_bf16(o[0][0] + o[1][0], o[0][1] + o[1][1]);
+      if (g + 8 < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g + 8) * D + d) = pack_bf16(o[0][2] + o[1][2], o[0][3] + o[1][3]);
     }
   }
 }
@@ -238,12 +241,13 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
   const int Vp = (V + 15) & ~15;
-  const uint32_t sX = s_u32(smem), sB = sX + STG * XT;
-  float* sS = reinterpret_cast<float*>(smem + STG * (XT + BT));              // [VP_MAX][SROW] dalpha
-  float* sAl = sS + VP_MAX * SROW;                                            // [VP_MAX][SROW] alpha
-  bf16* sAD = reinterpret_cast<bf16*>(sAl + VP_MAX * SROW);                  // [VP_MAX][ADROW]  (alpha | ds)
+  const int XTb = Vp * TB * 2;                                                // X tile sized for this V: more stages fit
+  const uint32_t sX = s_u32(smem), sB = sX + STG * XTb;
+  float* sS = reinterpret_cast<float*>(smem + STG * (XTb + BT));             // [Vp][SROW] dalpha
+  float* sAl = sS + Vp * SROW;                                                // [Vp][SROW] alpha
+  bf16* sAD = reinterpret_cast<bf16*>(sAl + Vp * SROW);                      // [Vp][ADROW]  (alpha | ds)
   constexpr int ADROW = 2 * HP + 8;
-  bf16* sDT = sAD + VP_MAX * ADROW;                                          // ds^T [HP][DTROW]
+  bf16* sDT = sAD + Vp * ADROW;                                              // ds^T [HP][DTROW]
   constexpr int DTROW = VP_MAX + 8;
   float* sAcc = reinterpret_cast<float*>(sDT + HP * DTROW);                  // [HP][D + 8] block-private dUt^T accumulator
   const int AR = D + 8;                                                       // padded: rows g, g + 1 are 8 banks apart
@@ -252,13 +256,13 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int wt = warp & 7, wh = warp >> 3;
   const int nch = D / TB, mtiles = Vp / 16;
-  uint8_t* sO = reinterpret_cast<uint8_t*>(sS) + wt * (16 * 128);            // [16][64] bf16, swizzled (2 KB per dX warp <= sS + sAl)
-  static_assert(8 * 16 * 128 <= 2 * VP_MAX * SROW * 4, "staging tiles must fit in the score buffers");
+  uint8_t* sO = reinterpret_cast<uint8_t*>(sS) + wt * (16 * 128);            // [16][64] bf16, swizzled: 2 KB per dX warp (wt < mtiles)
+  static_assert(16 * 128 <= 2 * 16 * SROW * 4, "staging tiles (2 KB per 16 rows) must fit in the score buffers (2 x 16 x SROW floats)");
 
   for (int i = threadIdx.x; i < HP * AR; i += NTB) sAcc[i] = 0.f;
   for (int j = 0; j < STG; j++) {
-    zero_tail_rows(smem + j * XT, V, Vp, NTB);
-    zero_tail_rows(smem + STG * XT + j * BT, h, HP, NTB);
+    zero_tail_rows(smem + j * XTb, V, Vp, NTB);
+    zero_tail_rows(smem + STG * XTb + j * BT, h, HP, NTB);
   }
   if (threadIdx.x == 0) {
     for (int i = 0; i < STG; i++) mbar_init(bar0 + 8 * i, 1);
@@ -271,11 +275,11 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
   const int per = 2 * nch, total = npat * per;
   auto issue = [&](int n) {             // thread 0
     if (n >= total) return;
-    const int pi = n / per, i = n - pi * per, c = i % nch, st = n % STG;
+    const int pi = n / per, i = n - pi * per, c = i < nch ? i : per - 1 - i, st = n % STG;
     const int bl = blockIdx.x + pi * gridDim.x;
     const uint32_t bar = bar0 + 8 * st;
     mbar_expect_tx(bar, (V + h) * TB * 2 + (i >= nch ? UT : 0));
-    tma_load_2d(sX + st * XT, &tmX, bar, c * TB, bl * V);
+    tma_load_2d(sX + st * XTb, &tmX, bar, c * TB, bl * V);
     tma_load_2d(sB + st * BT, &tmG, bar, c * TB, bl * h);
     if (i >= nch) tma_load_2d(sB + st * BT + UT, &tmU, bar, c * TB, 0);
   };
@@ -296,7 +300,7 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
       __syncthreads();
       if (threadIdx.x == 0) issue(n + STG - 1);
       if (wt < mtiles) {
-        const uint32_t xc = sX + st * XT, bc = sB + st * BT;
+        const uint32_t xc = sX + st * XTb, bc = sB + st * BT;
 #pragma unroll
         for (int ks = 0; ks < TB / 32; ks++) {
           uint32_t a[4], b[4];
@@ -350,8 +354,8 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
       __syncthreads();
       if (threadIdx.x == 0) issue(n + STG - 1);
-      const uint32_t xc = sX + st * XT, bc = sB + st * BT;
-      const int c0 = (i - nch) * TB;
+      const uint32_t xc = sX + st * XTb, bc = sB + st * BT;
+      const int c0 = (per - 1 - i) * TB;   // pass 2 runs from the last chunk back: most recently read lines first (L2)
       if (wh == 0) {
         if (wt < mtiles) {
 #pragma unroll
@@ -419,8 +423,9 @@ __global__ void agg_ut_to_bf16_kernel(const float* __restrict__ Ut, bf16* __rest
 size_t fwd_smem(int stg) {
   return 1024 + (size_t)stg * 2 * (XT + UT) + (size_t)VP_MAX * SROW * 4 + (size_t)HP * (VP_MAX + 8) * 2 + 8 * stg;
 }
-size_t bwd_smem(int D, int stg) {
-  return 1024 + (size_t)stg * (XT + BT) + 2 * (size_t)VP_MAX * SROW * 4 + (size_t)VP_MAX * (2 * HP + 8) * 2 +
+size_t bwd_smem(int V, int D, int stg) {
+  const size_t Vp = (V + 15) & ~15;
+  return 1024 + (size_t)stg * (Vp * TB * 2 + BT) + 2 * Vp * SROW * 4 + Vp * (2 * HP + 8) * 2 +
          (size_t)HP * (VP_MAX + 8) * 2 + (size_t)HP * (D + 8) * 4 + 8 * stg;
 }
 constexpr size_t SMEM_MAX = 227 * 1024;
@@ -451,7 +456,7 @@ int make_map(CUtensorMap* tm, const void* base, long long rows, int D, int box_r
 }  // namespace
 
 bool agg_tc_supported(int dt, int V, int D, int heads) {
-  return dt == ORBIT_BF16 && heads <= HP && V <= VP_MAX && D % 128 == 0 && bwd_smem(D, 2) <= SMEM_MAX;
+  return dt == ORBIT_BF16 && heads <= HP && V <= VP_MAX && D % 128 == 0 && bwd_smem(V, D, 2) <= SMEM_MAX;
 }
 size_t agg_tc_utb_bytes(int D) { return (size_t)HP * D * sizeof(bf16); }
 
@@ -467,7 +472,7 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
   static bool set = false;
   if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_fwd_tma_kernel<STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }
   const int grid = BL < 148 ? BL : 148;
-  agg_fwd_tma_kernel<STG><<<grid, NT, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads);
+  agg_fwd_tma_kernel<STG><<<grid, NTF, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
@@ -479,14 +484,14 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
   ORBIT_TRY(make_map(&tmG, dXbar, (long long)BL * heads, D, heads));
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
   const int grid = BL < 148 ? BL : 148;
-  int stg = 4;                          // deepest ring that fits beside the [HP][D] fp32 dUt accumulator
-  while (stg > 2 && bwd_smem(D, stg) > SMEM_MAX) stg--;
-  const size_t smb = bwd_smem(D, stg);
+  int stg = 6;                          // deepest ring that fits beside the [HP][D] fp32 dUt accumulator
+  while (stg > 2 && bwd_smem(V, D, stg) > SMEM_MAX) stg--;
+  const size_t smb = bwd_smem(V, D, stg);
 #define AB(S) do {                                                                                            \
     ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_bwd_tma_kernel<S>,                                \
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));            \
     agg_bwd_tma_kernel<S><<<grid, NTB, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads); } while (0)
-  if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
+  if (stg == 6) AB(6); else if (stg == 5) AB(5); else if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
 #undef AB
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;

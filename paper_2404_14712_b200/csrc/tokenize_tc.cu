@@ -71,16 +71,36 @@ __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, cons
   const int BL = d.B * L, bl0 = blockIdx.y * PT;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int ncol = min(DCH, d.D - c0);
-  // A: [hi | lo | 0] of the pixels
-  for (int idx = threadIdx.x; idx < PT * KP; idx += NT) {
-    const int pr = idx / KP, k = idx - pr * KP;
-    bf16 val = __float2bfloat16_rn(0.f);
-    if (k < 2 * P2 && bl0 + pr < BL) {
-      bf16 hi, lo;
-      split_bf16(pixel(x, d.V, d.Hg, d.Wg, d.p, bl0 + pr, L, v, k % P2), hi, lo);
-      val = k < P2 ? hi : lo;
+  // A: [hi | lo | 0] of the pixels.  One thread per (patch, patch row): the (b, i, j) arithmetic is done once per p
+  // pixels and the row is one vector load (the per-element version spent half of the kernel's instructions here).
+  constexpr int P = P2 == 16 ? 4 : (P2 == 4 ? 2 : 1);
+  if (2 * P2 < KP) {
+    constexpr int PAD = KP - 2 * P2 > 0 ? KP - 2 * P2 : 1;
+    for (int idx = threadIdx.x; idx < PT * PAD; idx += NT)
+      *reinterpret_cast<bf16*>(sA + (idx / PAD) * AROW + (2 * P2 + idx % PAD) * 2) = __float2bfloat16_rn(0.f);
+  }
+  {
+    const int gw = d.Wg / P;
+    for (int idx = threadIdx.x; idx < PT * P; idx += NT) {
+      const int pr = idx / P, di = idx % P, bl = bl0 + pr;
+      float px[P];
+#pragma unroll
+      for (int dj = 0; dj < P; dj++) px[dj] = 0.f;
+      if (bl < BL) {
+        const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
+        const float* src = x + (((size_t)b * d.V + v) * d.Hg + i * P + di) * d.Wg + j * P;
+        if (P == 4) { const float4 q = *reinterpret_cast<const float4*>(src); px[0] = q.x; px[1 % P] = q.y; px[2 % P] = q.z; px[3 % P] = q.w; }
+        else if (P == 2) { const float2 q = *reinterpret_cast<const float2*>(src); px[0] = q.x; px[1 % P] = q.y; }
+        else px[0] = *src;
+      }
+#pragma unroll
+      for (int dj = 0; dj < P; dj++) {
+        bf16 hi, lo;
+        split_bf16(px[dj], hi, lo);
+        *reinterpret_cast<bf16*>(sA + pr * AROW + (di * P + dj) * 2) = hi;
+        *reinterpret_cast<bf16*>(sA + pr * AROW + (P2 + di * P + dj) * 2) = lo;
+      }
     }
-    *reinterpret_cast<bf16*>(sA + pr * AROW + k * 2) = val;
   }
   // B: [Wp[v]; Wp[v]; 0] columns c0..c0+ncol
   for (int idx = threadIdx.x; idx < KP * (DCH / 8); idx += NT) {

@@ -21,6 +21,10 @@ __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cv
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
+// 4-byte copy, zero-filled when bytes == 0
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, int bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void ldsm4(uint32_t addr, uint32_t* r) {
@@ -167,9 +171,11 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
   extern __shared__ __align__(128) uint8_t smem[];
   uint8_t* sB = smem;                                     // [STG][KC][DCH + 8] bf16
   float* sP = reinterpret_cast<float*>(smem + STG * KC * BROW);   // [STG][KC][16] pixels (fp32)
-  const int v = blockIdx.y, c0 = blockIdx.z * DCH;
+  // blockIdx.x = (v, column chunk): CTAs that run together read neighbouring 1 KB pieces of the same token rows
+  const int nz = gridDim.x / d.V;
+  const int v = blockIdx.x / nz, c0 = (blockIdx.x - v * nz) * DCH;
   const int BL = d.B * L;
-  const int p0 = blockIdx.x * patches_per_cta, p1 = min(BL, p0 + patches_per_cta);
+  const int p0 = blockIdx.y * patches_per_cta, p1 = min(BL, p0 + patches_per_cta);
   const int nchunks = (p1 - p0 + KC - 1) / KC;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int ncol = min(DCH, d.D - c0);
@@ -183,10 +189,17 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
       else *reinterpret_cast<uint4*>(sB + (st * KC + k) * BROW + ch * 16) = make_uint4(0, 0, 0, 0);
     }
     {
-      const int k = threadIdx.x >> 4, r = threadIdx.x & 15;     // 16 x 16 pixels per chunk
-      float pv = 0.f;
-      if (r < P2 && base + k < p1) pv = pixel(x, d.V, d.Hg, d.Wg, d.p, base + k, L, v, r);
-      sP[(st * KC + k) * 16 + r] = pv;
+      // 16 x 16 pixels per chunk, asynchronously like the dtok rows (a plain load + st.shared stalled every warp for a
+      // full memory latency per chunk: the ring never ran ahead)
+      const int k = threadIdx.x >> 4, r = threadIdx.x & 15;
+      const bool ok = r < P2 && base + k < p1;
+      const float* src = x;
+      if (ok) {
+        const int bl = base + k, b = bl / L, l = bl - b * L, gw = d.Wg / d.p;
+        const int i = l / gw, j = l - i * gw, di = r / d.p, dj = r - di * d.p;
+        src = x + (((size_t)b * d.V + v) * d.Hg + i * d.p + di) * d.Wg + j * d.p + dj;
+      }
+      cp_async4(s_u32(sP + (st * KC + k) * 16 + r), src, ok ? 4 : 0);
     }
     cp_commit();
   };
@@ -278,7 +291,7 @@ int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* d
   int ppc = cdiv(BL, splits);
   ppc = ((ppc + 15) / 16) * 16;
   if (ppc < 64) ppc = 64;
-  dim3 grid(cdiv(BL, ppc), d.V, nz);
+  dim3 grid(d.V * nz, cdiv(BL, ppc));
   const size_t smb = (size_t)4 * 16 * BROW + (size_t)4 * 16 * 16 * sizeof(float);
 #define TB(P) do {                                                                                            \
     static bool set = false;                                                                                  \

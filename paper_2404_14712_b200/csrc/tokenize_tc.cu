@@ -287,7 +287,18 @@ int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* d
   const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
   const long long BL = (long long)d.B * L;
   const int nz = cdiv(d.D, DCH);
-  int splits = cdiv(148 * 6, d.V * nz);
+  // patch splits: the first count whose grid fills whole waves of 2 CTAs per SM to >= 95 % (else the fullest)
+  int splits = 1;
+  {
+    const long long slots = 148 * 2, per = (long long)d.V * nz;
+    double best = 0.0;
+    for (int sp = 1; sp <= 16; sp++) {
+      const long long n = per * sp, waves = (n + slots - 1) / slots;
+      const double eff = (double)n / (double)(waves * slots);
+      if (eff > best + 1e-9) { best = eff; splits = sp; }
+      if (n >= slots * 2 && eff >= 0.95) { splits = sp; break; }
+    }
+  }
   int ppc = cdiv(BL, splits);
   ppc = ((ppc + 15) / 16) * 16;
   if (ppc < 64) ppc = 64;

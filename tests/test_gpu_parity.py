@@ -275,6 +275,20 @@ def test_front_end_fused_shapes(rn, case):
     print("fused front", case, {k: f"{v:.2e}" for k, v in errs.items() if not k.startswith("b0")})
 
 
+@pytest.mark.parametrize("case", [
+    dict(B=1, V=128, Hg=8, Wg=8, p=4, D=128, heads=2, rd="f32"),        # V at the limit of the TMA-fed kernels, 2 heads of 16
+    dict(B=3, V=48, Hg=24, Wg=20, p=2, D=256, heads=16, rd="bf16"),     # BL = 360: 2-3 patches per CTA through one ring
+    dict(B=2, V=5, Hg=6, Wg=10, p=1, D=128, heads=8, rd="f32"),         # patch 1, V < 16 (one row tile, 11 zero rows)
+    dict(B=5, V=17, Hg=16, Wg=16, p=2, D=384, heads=12, rd="bf16"),     # odd chunk count (D = 6 x 64), V = 16 + 1, BL = 320
+])
+def test_front_end_twocall_shapes(rn, case):
+    """orbit_tokenize + orbit_var_aggregate (+ backward) on the tensor-core / TMA kernels over edge shapes, <= 1e-2."""
+    cfg = syn.Config("ST", B=case["B"], V=case["V"], Hg=case["Hg"], Wg=case["Wg"], p=case["p"], D=case["D"],
+                     heads=case["heads"], F=2 * case["D"], depth=1, dtype="bf16", resid_dtype=case["rd"])
+    errs = run_and_compare_step(rn, cfg, 47, 1e-2, with_pos=False, fused=False)
+    print("two-call front", case, {k: f"{v:.2e}" for k, v in errs.items() if not k.startswith("b0")})
+
+
 def test_front_end_fused_fp32_shapes(rn):
     """fp32 storage (SIMT GEMMs, strided batch over heads) on an odd shape: <= 1e-4."""
     cfg = syn.Config("SF32", B=2, V=9, Hg=8, Wg=12, p=2, D=64, heads=4, F=128, depth=1, dtype="f32", resid_dtype="f32")

@@ -232,10 +232,11 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
 // while warps 8-15 accumulate dUt^T (one 8-column group of the chunk each).  dX leaves through a per-warp XOR-swizzled
 // staging tile (aliasing the dalpha / alpha score buffers, dead in pass 2) as 16-byte pieces, 128 contiguous bytes of a
 // token row per 8 lanes, instead of 4-byte pieces of 16 rows.
-constexpr int NTB = 512;
+constexpr int NTB = 512;                    // consumer threads; warp 16 is the TMA producer
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 constexpr int BT = 2 * UT;                   // B tile: rows 0-15 dXbar chunk, 16-31 Ut chunk
 template <int STG>
-__global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
+__global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
     const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmU,
     const float* __restrict__ alpha, bf16* __restrict__ dtok, float* __restrict__ dUt_acc, int BL, int V, int D, int h) {
   extern __shared__ uint8_t smem_raw[];
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
   constexpr int DTROW = VP_MAX + 8;
   float* sAcc = reinterpret_cast<float*>(sDT + HP * DTROW);                  // [HP][D + 8] block-private dUt^T accumulator
   const int AR = D + 8;                                                       // padded: rows g, g + 1 are 8 banks apart
-  const uint32_t bar0 = s_u32(sAcc + HP * AR);                               // full[STG]
+  const uint32_t bar0 = s_u32(sAcc + HP * AR), ebar0 = bar0 + 8 * STG;       // full[STG], empty[STG]
   const uint32_t sADu = s_u32(sAD), sDTu = s_u32(sDT);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int wt = warp & 7, wh = warp >> 3;
@@ -259,13 +260,13 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
   uint8_t* sO = reinterpret_cast<uint8_t*>(sS) + wt * (16 * 128);            // [16][64] bf16, swizzled: 2 KB per dX warp (wt < mtiles)
   static_assert(16 * 128 <= 2 * 16 * SROW * 4, "staging tiles (2 KB per 16 rows) must fit in the score buffers (2 x 16 x SROW floats)");
 
-  for (int i = threadIdx.x; i < HP * AR; i += NTB) sAcc[i] = 0.f;
+  for (int i = threadIdx.x; i < HP * AR; i += NTB + 32) sAcc[i] = 0.f;
   for (int j = 0; j < STG; j++) {
-    zero_tail_rows(smem + j * XTb, V, Vp, NTB);
-    zero_tail_rows(smem + STG * XTb + j * BT, h, HP, NTB);
+    zero_tail_rows(smem + j * XTb, V, Vp, NTB + 32);
+    zero_tail_rows(smem + STG * XTb + j * BT, h, HP, NTB + 32);
   }
   if (threadIdx.x == 0) {
-    for (int i = 0; i < STG; i++) mbar_init(bar0 + 8 * i, 1);
+    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(ebar0 + 8 * i, NTB / 32); }
     fence_barrier_init();
   }
   fence_proxy_async();
@@ -273,8 +274,7 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   const int per = 2 * nch, total = npat * per;
-  auto issue = [&](int n) {             // thread 0
-    if (n >= total) return;
+  auto issue = [&](int n) {             // producer lane
     const int pi = n / per, i = n - pi * per, c = i < nch ? i : per - 1 - i, st = n % STG;
     const int bl = blockIdx.x + pi * gridDim.x;
     const uint32_t bar = bar0 + 8 * st;
@@ -283,12 +283,21 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
     tma_load_2d(sB + st * BT, &tmG, bar, c * TB, bl * h);
     if (i >= nch) tma_load_2d(sB + st * BT + UT, &tmU, bar, c * TB, 0);
   };
-  if (threadIdx.x == 0) for (int n = 0; n < STG - 1; n++) issue(n);
+  // Producer warp: refills a stage as soon as all 16 consumer warps have released it (empty[st]); the consumers never
+  // synchronise with each other inside a pass, so warps drift apart and the per-step CTA barrier is gone.
+  if (warp == NTB / 32) {
+    if (lane == 0)
+      for (int n = 0; n < total; n++) {
+        if (n >= STG) mbar_wait(ebar0 + 8 * (n % STG), ((n / STG) + 1) & 1);
+        issue(n);
+      }
+    return;
+  }
 
   for (int pi = 0; pi < npat; pi++) {
     const int bl = blockIdx.x + pi * gridDim.x, n0 = pi * per;
     float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-    __syncthreads();                    // previous patch finished with the score / staging buffers
+    consumer_sync();                    // previous patch finished with the score / staging buffers
     for (int i = threadIdx.x; i < Vp * HP; i += NTB) {
       int v = i / HP, a = i - v * HP;
       sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
@@ -297,8 +306,6 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
     for (int i = 0; i < nch; i++) {
       const int n = n0 + i, st = n % STG;
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
-      __syncthreads();
-      if (threadIdx.x == 0) issue(n + STG - 1);
       if (wt < mtiles) {
         const uint32_t xc = sX + st * XTb, bc = sB + st * BT;
 #pragma unroll
@@ -310,6 +317,8 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
           mma16816(acc[1], a, b[2], b[3]);
         }
       }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ebar0 + 8 * st);
     }
     if (wt < mtiles && wh == 0) {
 #pragma unroll
@@ -319,7 +328,7 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
         sS[(r + 8) * SROW + c] = acc[nt][2]; sS[(r + 8) * SROW + c + 1] = acc[nt][3];
       }
     }
-    __syncthreads();
+    consumer_sync();
     if (wt < mtiles && wh == 1) {
 #pragma unroll
       for (int nt = 0; nt < 2; nt++) {
@@ -328,7 +337,7 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
         sS[(r + 8) * SROW + c] += acc[nt][2]; sS[(r + 8) * SROW + c + 1] += acc[nt][3];
       }
     }
-    __syncthreads();
+    consumer_sync();
     // ---- ds[v, a] = alpha (dalpha - sum_w alpha_w dalpha_w); A operands (alpha | ds) and ds^T in bf16
     for (int a = warp; a < HP; a += NTB / 32) {
       float dot = 0.f;
@@ -342,7 +351,7 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
         sDT[a * DTROW + v] = __float2bfloat16_rn(ds);
       }
     }
-    __syncthreads();
+    consumer_sync();
     uint32_t adf[2][4];                 // this warp's 16 rows of (alpha | ds): K = 32 -> 2 k-steps
     if (wh == 0 && wt < mtiles) {
       ldA_plain(sADu, ADROW * 2, wt * 16, 0, adf[0]);
@@ -352,8 +361,6 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
     for (int i = nch; i < 2 * nch; i++) {
       const int n = n0 + i, st = n % STG;
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
-      __syncthreads();
-      if (threadIdx.x == 0) issue(n + STG - 1);
       const uint32_t xc = sX + st * XTb, bc = sB + st * BT;
       const int c0 = (per - 1 - i) * TB;   // pass 2 runs from the last chunk back: most recently read lines first (L2)
       if (wh == 0) {
@@ -403,9 +410,11 @@ __global__ void __launch_bounds__(NTB) agg_bwd_tma_kernel(const __grid_constant_
         v0.x += o[0]; v0.y += o[1]; v1.x += o[2]; v1.y += o[3];
         *p0 = v0; *p1 = v1;
       }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ebar0 + 8 * st);
     }
   }
-  __syncthreads();
+  consumer_sync();
   for (int i = threadIdx.x; i < h * D; i += NTB) {
     int a = i / D, d = i - a * D;
     atomicAdd(dUt_acc + (size_t)d * h + a, sAcc[a * AR + d]);
@@ -426,7 +435,7 @@ size_t fwd_smem(int stg) {
 size_t bwd_smem(int V, int D, int stg) {
   const size_t Vp = (V + 15) & ~15;
   return 1024 + (size_t)stg * (Vp * TB * 2 + BT) + 2 * Vp * SROW * 4 + Vp * (2 * HP + 8) * 2 +
-         (size_t)HP * (VP_MAX + 8) * 2 + (size_t)HP * (D + 8) * 4 + 8 * stg;
+         (size_t)HP * (VP_MAX + 8) * 2 + (size_t)HP * (D + 8) * 4 + 16 * stg;
 }
 constexpr size_t SMEM_MAX = 227 * 1024;
 
@@ -490,7 +499,7 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
 #define AB(S) do {                                                                                            \
     ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_bwd_tma_kernel<S>,                                \
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));            \
-    agg_bwd_tma_kernel<S><<<grid, NTB, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads); } while (0)
+    agg_bwd_tma_kernel<S><<<grid, NTB + 32, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads); } while (0)
   if (stg == 6) AB(6); else if (stg == 5) AB(5); else if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
 #undef AB
   ORBIT_LAUNCH_CHECK();

@@ -107,9 +107,10 @@ __device__ __forceinline__ void zero_tail_rows(uint8_t* tile, int r0, int r1, in
 // A step is NSUB = 2 sub-tiles (128 columns); 16 warps = two groups of 8, group wh works on sub-tile wh.  Pass 1: warp
 // (wh, wt < mtiles) accumulates the scores of its 16 rows over its sub-tiles (the two groups' halves are summed through
 // shared memory).  Pass 2: warp (wh, wt) owns 8 columns of sub-tile wh.
-constexpr int NTF = 512;
+constexpr int NTF = 512;                    // consumer threads; warp 16 is the TMA producer
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 template <int STG>
-__global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
+__global__ void __launch_bounds__(NTF + 32) agg_fwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
     const __grid_constant__ CUtensorMap tmU, float* __restrict__ alpha, bf16* __restrict__ Xbar, int BL, int V, int D, int h) {
   constexpr int NSUB = 2;
   extern __shared__ uint8_t smem_raw[];
@@ -121,14 +122,14 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
   bf16* sAT = reinterpret_cast<bf16*>(sS + VP_MAX * SROW);                  // alpha^T [HP][ATROW]
   constexpr int ATROW = VP_MAX + 8;
   const uint32_t sATu = s_u32(sAT);
-  const uint32_t bar0 = s_u32(sAT + HP * ATROW);                            // full[STG]
+  const uint32_t bar0 = s_u32(sAT + HP * ATROW), ebar0 = bar0 + 8 * STG;    // full[STG], empty[STG]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int wt = warp & 7, wh = warp >> 3;
   const int nch = D / (TB * NSUB), mtiles = Vp / 16;
 
-  for (int j = 0; j < STG * NSUB; j++) zero_tail_rows(smem + j * XT, V, Vp, NTF);
+  for (int j = 0; j < STG * NSUB; j++) zero_tail_rows(smem + j * XT, V, Vp, NTF + 32);
   if (threadIdx.x == 0) {
-    for (int i = 0; i < STG; i++) mbar_init(bar0 + 8 * i, 1);
+    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(ebar0 + 8 * i, NTF / 32); }
     fence_barrier_init();
   }
   fence_proxy_async();
@@ -136,8 +137,7 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   const int per = 2 * nch, total = npat * per;
-  auto issue = [&](int n) {             // thread 0: n-th step of this CTA: pass 1 (scores) then pass 2 (Xbar) of each patch
-    if (n >= total) return;
+  auto issue = [&](int n) {             // producer lane: n-th step of this CTA: pass 1 (scores) then pass 2 (Xbar) of each patch
     const int pi = n / per, i = n - pi * per, c = i < nch ? i : per - 1 - i, st = n % STG;   // pass 2 walks back
     const int row0 = (blockIdx.x + pi * gridDim.x) * V;
     const uint32_t bar = bar0 + 8 * st;
@@ -148,7 +148,16 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
       if (i < nch) tma_load_2d(sU + (st * NSUB + j) * UT, &tmU, bar, (c * NSUB + j) * TB, 0);
     }
   };
-  if (threadIdx.x == 0) for (int n = 0; n < STG - 1; n++) issue(n);
+  // Producer warp: refills a stage as soon as all 16 consumer warps have released it (empty[st]); inside a pass the
+  // consumer warps never meet at a CTA barrier.
+  if (warp == NTF / 32) {
+    if (lane == 0)
+      for (int n = 0; n < total; n++) {
+        if (n >= STG) mbar_wait(ebar0 + 8 * (n % STG), ((n / STG) + 1) & 1);
+        issue(n);
+      }
+    return;
+  }
 
   for (int pi = 0; pi < npat; pi++) {
     const int bl = blockIdx.x + pi * gridDim.x, n0 = pi * per;
@@ -157,10 +166,11 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
     for (int i = 0; i < nch; i++) {
       const int n = n0 + i, st = n % STG;
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
-      __syncthreads();                  // step n - 1 is finished everywhere: its stage is free (and sS / sAT of the previous patch)
-      if (threadIdx.x == 0) issue(n + STG - 1);
       if (wt < mtiles) chunk_scores<TB>(acc, sX + (st * NSUB + wh) * XT, wt * 16, sU + (st * NSUB + wh) * UT);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ebar0 + 8 * st);
     }
+    consumer_sync();                    // the previous patch's pass 2 is finished everywhere: sS / sAT may be rewritten
     if (wt < mtiles && wh == 0) {
 #pragma unroll
       for (int nt = 0; nt < 2; nt++) {
@@ -169,7 +179,7 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
         sS[(r + 8) * SROW + c] = acc[nt][2]; sS[(r + 8) * SROW + c + 1] = acc[nt][3];
       }
     }
-    __syncthreads();
+    consumer_sync();
     if (wt < mtiles && wh == 1) {
 #pragma unroll
       for (int nt = 0; nt < 2; nt++) {
@@ -178,7 +188,7 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
         sS[(r + 8) * SROW + c] += acc[nt][2]; sS[(r + 8) * SROW + c + 1] += acc[nt][3];
       }
     }
-    __syncthreads();
+    consumer_sync();
     // ---- softmax over v per head; alpha -> global (fp32) and alpha^T (bf16) -> smem
     for (int a = warp; a < HP; a += NTF / 32) {
       if (a < h) {
@@ -198,7 +208,7 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
         for (int v = lane; v < Vp; v += 32) sAT[a * ATROW + v] = __float2bfloat16_rn(0.f);
       }
     }
-    __syncthreads();
+    consumer_sync();
     // ---- pass 2: Xbar[a, d] = sum_v alpha[v, a] X[v, d]
     uint32_t af[VP_MAX / 16][4];
 #pragma unroll
@@ -207,8 +217,6 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
     for (int i = nch; i < 2 * nch; i++) {
       const int n = n0 + i, st = n % STG;
       mbar_wait(bar0 + 8 * st, (n / STG) & 1);
-      __syncthreads();
-      if (threadIdx.x == 0) issue(n + STG - 1);
       const uint32_t xc = sX + (st * NSUB + wh) * XT;
       float o[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};      // two accumulation chains (even / odd k-steps)
 #pragma unroll
@@ -222,6 +230,8 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
       const int d = (per - 1 - i) * (TB * NSUB) + wh * TB + wt * 8 + 2 * t;   // pass 2 runs from the last chunk back (L2 reuse distance)
       if (g < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g) * D + d) = pack_bf16(o[0][0] + o[1][0], o[0][1] + o[1][1]);
       if (g + 8 < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g + 8) * D + d) = pack_bf16(o[0][2] + o[1][2], o[0][3] + o[1][3]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ebar0 + 8 * st);
     }
   }
 }
@@ -233,7 +243,6 @@ __global__ void __launch_bounds__(NTF) agg_fwd_tma_kernel(const __grid_constant_
 // staging tile (aliasing the dalpha / alpha score buffers, dead in pass 2) as 16-byte pieces, 128 contiguous bytes of a
 // token row per 8 lanes, instead of 4-byte pieces of 16 rows.
 constexpr int NTB = 512;                    // consumer threads; warp 16 is the TMA producer
-__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 constexpr int BT = 2 * UT;                   // B tile: rows 0-15 dXbar chunk, 16-31 Ut chunk
 template <int STG>
 __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
@@ -430,7 +439,7 @@ __global__ void agg_ut_to_bf16_kernel(const float* __restrict__ Ut, bf16* __rest
 }
 
 size_t fwd_smem(int stg) {
-  return 1024 + (size_t)stg * 2 * (XT + UT) + (size_t)VP_MAX * SROW * 4 + (size_t)HP * (VP_MAX + 8) * 2 + 8 * stg;
+  return 1024 + (size_t)stg * 2 * (XT + UT) + (size_t)VP_MAX * SROW * 4 + (size_t)HP * (VP_MAX + 8) * 2 + 16 * stg;
 }
 size_t bwd_smem(int V, int D, int stg) {
   const size_t Vp = (V + 15) & ~15;
@@ -481,7 +490,7 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
   static bool set = false;
   if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_fwd_tma_kernel<STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }
   const int grid = BL < 148 ? BL : 148;
-  agg_fwd_tma_kernel<STG><<<grid, NTF, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads);
+  agg_fwd_tma_kernel<STG><<<grid, NTF + 32, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

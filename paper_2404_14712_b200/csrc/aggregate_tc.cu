@@ -485,7 +485,7 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
   CUtensorMap tmX, tmU;
   ORBIT_TRY(make_map(&tmX, tok, (long long)BL * V, D, V));
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
-  constexpr int STG = 3;                // 3 x 36 KB stages + 13 KB: one or two CTAs per SM
+  constexpr int STG = 5;                // 5 x 36 KB stages + 13 KB, one CTA per SM
   const size_t smb = fwd_smem(STG);
   static bool set = false;
   if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_fwd_tma_kernel<STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }

@@ -180,6 +180,16 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int ncol = min(DCH, d.D - c0);
 
+  // patch grid position of this thread's pixel for the next chunk to be loaded (load() is called with ci = 0, 1, 2, ...)
+  constexpr int P = P2 == 16 ? 4 : (P2 == 4 ? 2 : 1);
+  const int gw = d.Wg / P, gh = d.Hg / P;
+  int pb, pi, pj;
+  {
+    const int bl = p0 + (threadIdx.x >> 4);
+    pb = bl / L;
+    const int l = bl - pb * L;
+    pi = l / gw; pj = l - pi * gw;
+  }
   auto load = [&](int ci) {
     const int st = ci % STG, base = p0 + ci * KC;
     for (int idx = threadIdx.x; idx < KC * (DCH / 8); idx += NT) {
@@ -194,11 +204,11 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
       const int k = threadIdx.x >> 4, r = threadIdx.x & 15;
       const bool ok = r < P2 && base + k < p1;
       const float* src = x;
-      if (ok) {
-        const int bl = base + k, b = bl / L, l = bl - b * L, gw = d.Wg / d.p;
-        const int i = l / gw, j = l - i * gw, di = r / d.p, dj = r - di * d.p;
-        src = x + (((size_t)b * d.V + v) * d.Hg + i * d.p + di) * d.Wg + j * d.p + dj;
-      }
+      if (ok) src = x + (((size_t)pb * d.V + v) * d.Hg + pi * P + r / P) * d.Wg + pj * P + r % P;
+      // this thread's patch of the next chunk: (b, i, j) advanced by KC patches without divisions
+      pj += KC;
+      while (pj >= gw) { pj -= gw; pi++; }
+      while (pi >= gh) { pi -= gh; pb++; }
       cp_async4(s_u32(sP + (st * KC + k) * 16 + r), src, ok ? 4 : 0);
     }
     cp_commit();

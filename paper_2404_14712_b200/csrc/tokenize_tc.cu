@@ -48,6 +48,11 @@ __device__ __forceinline__ void split_bf16(float x, bf16& hi, bf16& lo) {
   hi = __float2bfloat16_rn(x);
   lo = __float2bfloat16_rn(x - __bfloat162float(hi));
 }
+// two fp32 values -> packed bf16 (hi, hi) and packed residuals (lo, lo): a = hi_a + lo_a + O(2^-17 |a|)
+__device__ __forceinline__ void split_pair(float a, float b, uint32_t& hi, uint32_t& lo) {
+  hi = pack_bf16(a, b);
+  lo = pack_bf16(a - __uint_as_float(hi << 16), b - __uint_as_float(hi & 0xffff0000u));
+}
 // B fragments of an N-major tile with padded rows: 16 k from k0, 16 n from n0
 __device__ __forceinline__ void ldB(uint32_t base, int k0, int n0, uint32_t* r) {
   int lane = threadIdx.x & 31;
@@ -230,17 +235,10 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
     // A fragments (rows = pixel index r, cols = patch k) straight from the pixel tile, split hi / lo
     const float* pt = sP + st * KC * 16;
     uint32_t ah[4], al[4];
-    {
-      bf16 h0, l0, h1, l1;
-      split_bf16(pt[(2 * t) * 16 + g], h0, l0); split_bf16(pt[(2 * t + 1) * 16 + g], h1, l1);
-      ah[0] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[0] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
-      split_bf16(pt[(2 * t) * 16 + g + 8], h0, l0); split_bf16(pt[(2 * t + 1) * 16 + g + 8], h1, l1);
-      ah[1] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[1] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
-      split_bf16(pt[(2 * t + 8) * 16 + g], h0, l0); split_bf16(pt[(2 * t + 9) * 16 + g], h1, l1);
-      ah[2] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[2] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
-      split_bf16(pt[(2 * t + 8) * 16 + g + 8], h0, l0); split_bf16(pt[(2 * t + 9) * 16 + g + 8], h1, l1);
-      ah[3] = pack_bf16(__bfloat162float(h0), __bfloat162float(h1)); al[3] = pack_bf16(__bfloat162float(l0), __bfloat162float(l1));
-    }
+    split_pair(pt[(2 * t) * 16 + g], pt[(2 * t + 1) * 16 + g], ah[0], al[0]);
+    split_pair(pt[(2 * t) * 16 + g + 8], pt[(2 * t + 1) * 16 + g + 8], ah[1], al[1]);
+    split_pair(pt[(2 * t + 8) * 16 + g], pt[(2 * t + 9) * 16 + g], ah[2], al[2]);
+    split_pair(pt[(2 * t + 8) * 16 + g + 8], pt[(2 * t + 9) * 16 + g + 8], ah[3], al[3]);
     const uint32_t bt = s_u32(sB + st * KC * BROW);
 #pragma unroll
     for (int np = 0; np < 4; np++) {                       // this warp's 64 columns = 4 pairs of n-tiles

@@ -228,8 +228,8 @@ __global__ void __launch_bounds__(NTF + 32) agg_fwd_tma_kernel(const __grid_cons
         }
       }
       const int d = (per - 1 - i) * (TB * NSUB) + wh * TB + wt * 8 + 2 * t;   // pass 2 runs from the last chunk back (L2 reuse distance)
-      if (g < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g) * D + d) = pack_bf16(o[0][0] + o[1][0], o[0][1] + o[1][1]);
-      if (g + 8 < h) *reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g + 8) * D + d) = pack_bf16(o[0][2] + o[1][2], o[0][3] + o[1][3]);
+      if (g < h) __stcs(reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g) * D + d), pack_bf16(o[0][0] + o[1][0], o[0][1] + o[1][1]));
+      if (g + 8 < h) __stcs(reinterpret_cast<uint32_t*>(Xbar + ((size_t)bl * h + g + 8) * D + d), pack_bf16(o[0][2] + o[1][2], o[0][3] + o[1][3]));
       __syncwarp();
       if (lane == 0) mbar_arrive(ebar0 + 8 * st);
     }
@@ -396,8 +396,8 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
           for (int q = 0; q < 4; q++) {
             const int row = q * 4 + (lane >> 3), ch = lane & 7, r = wt * 16 + row;
             if (r < V)
-              *reinterpret_cast<uint4*>(dtok + ((size_t)bl * V + r) * D + c0 + ch * 8) =
-                  *reinterpret_cast<const uint4*>(sO + row * 128 + ((ch ^ (row & 7)) << 4));
+              __stcs(reinterpret_cast<uint4*>(dtok + ((size_t)bl * V + r) * D + c0 + ch * 8),   // streaming: keep X in L2
+                     *reinterpret_cast<const uint4*>(sO + row * 128 + ((ch ^ (row & 7)) << 4)));
           }
         }
       } else {

@@ -268,7 +268,7 @@ def run_ours(args, cfg):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     seed = syn.seed_of(cfg.name)
     if args.debug_mode:
-        ob.lib.orbit_set_debug_force_simt(args.debug_mode)
+        ob.orbit_set_debug_force_simt(args.debug_mode)      # needs the A/B build: ORBIT_LIB=dbg
 
     # ---- build the workload (inputs resident in HBM) ----
     if cfg.V is None:
@@ -454,7 +454,7 @@ def main():
                     help="additionally time the device-resident step replayed from a CUDA graph (reported as 'graph'; "
                          "the headline value and the roofline leg stay un-captured)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--debug-mode", type=int, default=0, help="orbit_set_debug_force_simt value (A/B comparisons only)")
+    ap.add_argument("--debug-mode", type=int, default=0, help="kernel-variant switch of the A/B build (ORBIT_DEBUG_SWITCH=1 build, ORBIT_LIB=dbg); never set by the default run")
     args = ap.parse_args()
     cfg = syn.CONFIGS[args.workload]
     if args.impl == "reference":

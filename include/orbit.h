@@ -193,13 +193,6 @@ int orbit_version(void);
  * gpu_launches claim). */
 long long orbit_launch_count(void);
 void orbit_reset_launch_count(void);
-/* Debug / A-B switch (process-wide; never set by bench.py's default run):
- *   0 = automatic (tcgen05 tensor-core kernels for bf16 where shapes allow),
- *   1 = force the SIMT fp32-FMA kernels everywhere (cross-check),
- *   2 = single-CTA tcgen05 GEMM instead of the CTA-pair kernel,
- *   3 = mma.sync attention instead of the tcgen05 attention (forward and backward), 4 = backward only,
- *   5 = direct row-per-thread stores in the CTA-pair GEMM epilogue instead of the TMA store / reduce-add path. */
-void orbit_set_debug_force_simt(int on);
 /* Per-launch CUDA-event timing of the tensor-core GEMM kernel (the dominant kernel; bench.py's roofline leg).
  * orbit_profile_gemm(1) starts recording an event pair around every tcgen05 GEMM launch on its stream;
  * orbit_profile_gemm_collect() waits for them, returns the summed kernel milliseconds, the summed algorithmic

@@ -14,7 +14,9 @@ Parity pins (tests/test_oracle_pins.py, all `-m "not gpu"`): central finite diff
 fwd/bwd pair; softmax rows sum to 1 / shift invariance; LayerNorm zero-mean unit-variance; attention
 over identical keys = mean of values; Eq. (2)/(3) shard sums = unsharded product; tokeniser = strided
 convolution (torch conv2d, float64); whole block fwd+bwd = torch float64 autograd of textbook ops;
-aggregation V=1 closed form, permutation invariance, dbk == 0, dbv == sum(do); QK-LayerNorm: torch
+aggregation V=1 closed form, permutation invariance, dbk == 0, dbv == sum(do); patch-chunked front end
+(tokenize_patches / var_aggregate / var_aggregate_bwd / tokenize_bwd_patches over a partition of the patches) = the
+whole-tensor functions; QK-LayerNorm: torch
 float64 autograd with F.layer_norm on the per-head q / k, finite differences, logits bounded by
 sqrt(d_h) for gamma = 1, beta = 0, invariance to rescaling the pre-norm queries (eps = 0); head + wMSE: torch
 float64 autograd (layer_norm, linear, permute, weighted mean), finite differences, unpatchify = inverse of
@@ -466,6 +468,22 @@ def tokenize_patches(x, Wp, bp, p, ls):
     for v in range(V):
         tok[:, :, v, :] = pix[:, v] @ Wp[v] + bp[v]
     return tok
+
+
+def tokenize_bwd_patches(x, dtok_s, p, ls):
+    """Contribution of the sampled patches `ls` to tokenize_bwd(): dWp[v, r, :] = sum_{b, l in ls} pix dtok_s,
+    dbp[v, :] = sum_{b, l in ls} dtok_s, with dtok_s = dtok[:, ls] ([B, S, V, D]).  The gradients are sums over
+    (b, l), so the contributions of a partition of the patches add up to tokenize_bwd() exactly."""
+    pix = patches(x, p)[:, :, ls, :]                                  # [B, V, S, p^2]
+    dtok_s = _f64(dtok_s)
+    B, V, S, P2 = pix.shape
+    D = dtok_s.shape[3]
+    dWp = np.empty((V, P2, D), dtype=F64)
+    dbp = np.empty((V, D), dtype=F64)
+    for v in range(V):
+        dWp[v] = pix[:, v].reshape(B * S, P2).T @ dtok_s[:, :, v, :].reshape(B * S, D)
+        dbp[v] = dtok_s[:, :, v, :].reshape(B * S, D).sum(axis=0)
+    return dWp, dbp
 
 
 def block_sampled(x, dy, P, heads, eps, rows, fcols):

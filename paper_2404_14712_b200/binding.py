@@ -12,7 +12,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "liborbit.so")
+# ORBIT_LIB=dbg selects the A/B build (liborbit_dbg.so, `ORBIT_DEBUG_SWITCH=1 python -m paper_2404_14712_b200.build`)
+LIB_PATH = os.path.join(_HERE, "liborbit_dbg.so" if os.environ.get("ORBIT_LIB") == "dbg" else "liborbit.so")
 if not os.path.exists(LIB_PATH):
     raise ImportError(
         f"{LIB_PATH} not found: build it with `python -m paper_2404_14712_b200.build` "
@@ -104,7 +105,9 @@ _proto("orbit_last_error", C.c_char_p, [])
 _proto("orbit_version", C.c_int, [])
 _proto("orbit_launch_count", C.c_longlong, [])
 _proto("orbit_reset_launch_count", None, [])
-_proto("orbit_set_debug_force_simt", None, [C.c_int])
+HAS_DEBUG_SWITCH = hasattr(lib, "orbit_set_debug_force_simt")      # only the A/B build exports it (csrc/orbit_debug.h)
+if HAS_DEBUG_SWITCH:
+    _proto("orbit_set_debug_force_simt", None, [C.c_int])
 _proto("orbit_tokenize", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp])
 _proto("orbit_tokenize_bwd", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp, _sz, _vp])
 _proto("orbit_tokenize_bwd_workspace_bytes", _sz, [C.POINTER(orbit_embed_desc)])
@@ -153,7 +156,7 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_block_bwd", "orbit_block_fwd_workspace_bytes", "orbit_block_bwd_workspace_bytes",
            "orbit_block_saved_bytes", "orbit_mse_loss_grad", "orbit_chain_fwd", "orbit_chain_bwd", "orbit_chain_workspace_bytes",
            "orbit_last_error", "orbit_version", "orbit_launch_count", "orbit_reset_launch_count",
-           "orbit_set_debug_force_simt", "orbit_debug_gemm", "orbit_profile_gemm",
+           "orbit_debug_gemm", "orbit_profile_gemm",
            "orbit_profile_gemm_collect", "orbit_embed_fused", "orbit_embed_fused_bwd",
            "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
            "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched", "orbit_head_loss", "orbit_head_loss_bwd",
@@ -402,5 +405,9 @@ def orbit_reset_launch_count():
     lib.orbit_reset_launch_count()
 
 
-def orbit_set_debug_force_simt(on: bool):
-    lib.orbit_set_debug_force_simt(1 if on else 0)
+def orbit_set_debug_force_simt(mode: int):
+    """A/B switch of the debug build only (ORBIT_LIB=dbg); the product library has a single dispatch."""
+    if not HAS_DEBUG_SWITCH:
+        raise RuntimeError("orbit_set_debug_force_simt: not in this build; build with ORBIT_DEBUG_SWITCH=1 and run with "
+                           "ORBIT_LIB=dbg (A/B comparisons only)")
+    lib.orbit_set_debug_force_simt(int(mode))

@@ -487,8 +487,7 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
   constexpr int STG = 5;                // 5 x 36 KB stages + 13 KB, one CTA per SM
   const size_t smb = fwd_smem(STG);
-  static bool set = false;
-  if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_fwd_tma_kernel<STG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }
+  ORBIT_SMEM_ATTR(agg_fwd_tma_kernel<STG>, smb);
   const int grid = BL < 148 ? BL : 148;
   agg_fwd_tma_kernel<STG><<<grid, NTF + 32, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads);
   ORBIT_LAUNCH_CHECK();
@@ -506,8 +505,7 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
   while (stg > 2 && bwd_smem(V, D, stg) > SMEM_MAX) stg--;
   const size_t smb = bwd_smem(V, D, stg);
 #define AB(S) do {                                                                                            \
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)agg_bwd_tma_kernel<S>,                                \
-                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));            \
+    ORBIT_SMEM_ATTR(agg_bwd_tma_kernel<S>, smb);                                                              \
     agg_bwd_tma_kernel<S><<<grid, NTB + 32, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads); } while (0)
   if (stg == 6) AB(6); else if (stg == 5) AB(5); else if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
 #undef AB

@@ -44,7 +44,7 @@ AggBwdWs carve_agg_bwd(const orbit_agg_desc& d, void* base) {
   return w;
 }
 
-int check_agg(const orbit_agg_desc* d) {
+int check_agg(const orbit_agg_desc* d, bool bwd) {
   if (!d) { set_error("agg desc is NULL"); return ORBIT_ERR_NULL; }
   if (!valid_dtype(d->dtype) || !valid_dtype(d->resid_dtype)) { set_error("agg: bad dtype"); return ORBIT_ERR_DTYPE; }
   if (d->dtype == ORBIT_F32 && d->resid_dtype != ORBIT_F32) { set_error("agg: resid_dtype must be F32 when dtype is F32"); return ORBIT_ERR_DTYPE; }
@@ -53,7 +53,15 @@ int check_agg(const orbit_agg_desc* d) {
     set_error("agg: bad shape B=%d L=%d V=%d D=%d heads=%d (need D%%heads==0, D%%8==0, (D/heads)%%8==0, heads<=32)", d->B, d->L, d->V, d->D, d->heads);
     return ORBIT_ERR_SHAPE;
   }
-  if (agg_patch_bwd_smem(d->V, d->D, d->heads) > 220 * 1024) { set_error("agg: heads*D too large for the per-patch kernels"); return ORBIT_ERR_SHAPE; }
+  // shared-memory bounds of the per-patch kernel that will actually run: the bf16 TMA kernels carry their own bound
+  // (agg_tc_supported); the SIMT forward keeps only the [V, heads] scores, the SIMT backward a [heads, D] fp32 accumulator
+  const bool tc = g_force_simt != 1 && agg_tc_supported(d->dtype, d->V, d->D, d->heads);
+  if (!tc && (size_t)d->V * d->heads * sizeof(float) > 220 * 1024) { set_error("agg: V*heads too large for the per-patch forward kernel"); return ORBIT_ERR_SHAPE; }
+  if (bwd && !tc && agg_patch_bwd_smem(d->V, d->D, d->heads) > 220 * 1024) {
+    set_error("agg_bwd: (2 V heads + heads D) * 4 bytes = %zu exceeds 220 KB of shared memory for the per-patch backward kernel",
+              agg_patch_bwd_smem(d->V, d->D, d->heads));
+    return ORBIT_ERR_SHAPE;
+  }
   return ORBIT_OK;
 }
 int check_agg_params(const orbit_agg_params* P) {
@@ -78,7 +86,7 @@ size_t orbit_var_aggregate_bwd_workspace_bytes(const orbit_agg_desc* d) { return
 
 int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_agg_params* P, const void* pos, void* agg,
                         void* saved, void* ws, size_t ws_bytes, void* stream) {
-  ORBIT_TRY(check_agg(d));
+  ORBIT_TRY(check_agg(d, false));
   ORBIT_TRY(check_agg_params(P));
   if (!tok || !agg || !saved || !ws) { set_error("var_aggregate: NULL pointer"); return ORBIT_ERR_NULL; }
   if (!aligned16(tok) || !aligned16(agg) || !aligned16(saved) || !aligned16(ws) || (pos && !aligned16(pos))) { set_error("var_aggregate: pointer not 16B aligned"); return ORBIT_ERR_ALIGN; }
@@ -113,7 +121,7 @@ int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_ag
 int orbit_var_aggregate_bwd(const orbit_agg_desc* d, const void* tok, const orbit_agg_params* P, const void* dagg,
                             const void* saved, void* dtok, orbit_agg_grads* G, void* dpos, void* ws, size_t ws_bytes,
                             void* stream) {
-  ORBIT_TRY(check_agg(d));
+  ORBIT_TRY(check_agg(d, true));
   ORBIT_TRY(check_agg_params(P));
   if (!tok || !dagg || !saved || !dtok || !G || !ws) { set_error("var_aggregate_bwd: NULL pointer"); return ORBIT_ERR_NULL; }
   {

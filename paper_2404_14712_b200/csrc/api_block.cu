@@ -79,9 +79,9 @@ int check_block(const orbit_block_desc* d) {
   if (d->dtype == ORBIT_F32 && d->resid_dtype != ORBIT_F32) { set_error("block: resid_dtype must be F32 when dtype is F32"); return ORBIT_ERR_DTYPE; }
   if (d->flags & ~(ORBIT_QK_NORM | ORBIT_RECOMPUTE)) { set_error("block: unknown flag bits 0x%x", d->flags); return ORBIT_ERR_UNSUPPORTED; }
   if (d->B <= 0 || d->N <= 0 || d->D <= 0 || d->heads <= 0 || d->F <= 0 || d->T <= 0 || d->D % d->heads || d->heads % d->T ||
-      d->F % d->T || d->D % 8 || (d->F / d->T) % 8 || (d->D / d->T) % 8 || (d->D / d->heads) > 256) {
+      d->F % d->T || d->D % 8 || (d->F / d->T) % 8 || (d->D / d->T) % 8 || (d->D / d->heads) > 256 || d->D > ORBIT_LN_MAX_D) {
     set_error("block: bad shape B=%d N=%d D=%d heads=%d F=%d T=%d (need D%%heads==0, heads%%T==0, F%%T==0, D%%8==0, "
-              "(F/T)%%8==0, (D/T)%%8==0, d_h<=256)", d->B, d->N, d->D, d->heads, d->F, d->T);
+              "(F/T)%%8==0, (D/T)%%8==0, d_h<=256, D<=16384)", d->B, d->N, d->D, d->heads, d->F, d->T);
     return ORBIT_ERR_SHAPE;
   }
   if ((d->flags & ORBIT_QK_NORM) && !qknorm_supported(d->D / d->heads)) {
@@ -231,6 +231,11 @@ int orbit_block_bwd(const orbit_block_desc* d, const void* dy, const orbit_block
     if (!S.Wqkv || !S.bqkv || !S.Wproj || !S.Wfc1 || !S.bfc1 || !S.Wfc2) { set_error("block_bwd: NULL shard gradient pointer"); return ORBIT_ERR_NULL; }
     if (!aligned16(S.Wqkv) || !aligned16(S.bqkv) || !aligned16(S.Wproj) || !aligned16(S.Wfc1) || !aligned16(S.bfc1) || !aligned16(S.Wfc2)) { set_error("block_bwd: shard gradient not 16B aligned"); return ORBIT_ERR_ALIGN; }
   }
+  if (qk_norm(*d)) {   // checked before the first launch (the ORBIT_RECOMPUTE forward below already enqueues kernels)
+    if (!G->qn_g || !G->qn_b || !G->kn_g || !G->kn_b) { set_error("block_bwd: NULL QK-LayerNorm gradient pointer"); return ORBIT_ERR_NULL; }
+    if (!aligned16(G->qn_g) || !aligned16(G->qn_b) || !aligned16(G->kn_g) || !aligned16(G->kn_b)) { set_error("block_bwd: QK-LayerNorm gradient not 16B aligned"); return ORBIT_ERR_ALIGN; }
+  }
+  if (!aligned16(G->ln1_g) || !aligned16(G->ln1_b) || !aligned16(G->ln2_g) || !aligned16(G->ln2_b) || !aligned16(G->bproj) || !aligned16(G->bfc2)) { set_error("block_bwd: gradient not 16B aligned"); return ORBIT_ERR_ALIGN; }
   if (dx == dy) { set_error("block_bwd: in-place (dx == dy) not allowed"); return ORBIT_ERR_UNSUPPORTED; }
   if (!aligned16(dy) || !aligned16(dx) || !aligned16(saved) || !aligned16(ws)) { set_error("block_bwd: pointer not 16B aligned"); return ORBIT_ERR_ALIGN; }
   if (ws_bytes < orbit_block_bwd_workspace_bytes(d)) { set_error("block_bwd: workspace too small"); return ORBIT_ERR_WORKSPACE; }
@@ -243,9 +248,6 @@ int orbit_block_bwd(const orbit_block_desc* d, const void* dy, const orbit_block
   if (recompute(*d)) {   // "the needed activation outputs are recomputed by rerunning the forward pass segment"
     sv.x = const_cast<void*>(saved);
     ORBIT_TRY(block_fwd_impl(d, saved, P, w.re_y, sv, (float*)w.re_part, false, s));
-  }
-  if (qk_norm(*d)) {
-    if (!G->qn_g || !G->qn_b || !G->kn_g || !G->kn_b) { set_error("block_bwd: NULL QK-LayerNorm gradient pointer"); return ORBIT_ERR_NULL; }
   }
   const int nc = qkv_cols(*d), dh = D / d->heads;
   float* acc_bfc2 = w.acc;

@@ -3,12 +3,15 @@
 #include <string.h>
 #include "api_util.cuh"
 #include "frontend.cuh"
+#include "orbit_debug.h"
 
 namespace orbit {
 
 static thread_local char g_err[512] = "";
 thread_local long long g_launches = 0;
+#ifdef ORBIT_DEBUG_SWITCH
 int g_force_simt = 0;
+#endif
 
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -18,22 +21,56 @@ void set_error(const char* fmt, ...) {
 }
 
 int check_device() {
-  static thread_local int cached = -1;
-  if (cached >= 0) return cached;
+  // cached per device ordinal: 0 = unknown, 1 = sm_100-class, 2 = other architecture
+  static std::atomic<int> cached[ORBIT_MAX_DEV];
   int dev = 0;
-  cudaDeviceProp prop;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+  if (cudaGetDevice(&dev) != cudaSuccess) {
     cudaGetLastError();
     set_error("no usable CUDA device");
     return ORBIT_ERR_ARCH;
   }
-  if (prop.major != 10) {
-    set_error("device '%s' is sm_%d%d; liborbit is built for sm_100a only (no fallback)", prop.name, prop.major,
-              prop.minor);
+  const bool cacheable = dev >= 0 && dev < ORBIT_MAX_DEV;
+  if (cacheable && cached[dev].load(std::memory_order_relaxed) == 1) return ORBIT_OK;
+  int major = 0, minor = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess) {
+    cudaGetLastError();
+    set_error("no usable CUDA device");
     return ORBIT_ERR_ARCH;
   }
-  cached = ORBIT_OK;
-  return cached;
+  if (major != 10) {
+    set_error("device %d is sm_%d%d; liborbit is built for sm_100a only (no fallback)", dev, major, minor);
+    return ORBIT_ERR_ARCH;
+  }
+  if (cacheable) cached[dev].store(1, std::memory_order_relaxed);
+  return ORBIT_OK;
+}
+
+int device_ordinal() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 0; }
+  return dev;
+}
+int smem_attr_once(SmemAttrOnce& st, const void* fn, int bytes) {
+  const int dev = device_ordinal();
+  if (dev >= 0 && dev < ORBIT_MAX_DEV && st.bytes[dev].load(std::memory_order_acquire) >= bytes) return ORBIT_OK;
+  ORBIT_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  if (dev >= 0 && dev < ORBIT_MAX_DEV) {
+    int cur = st.bytes[dev].load(std::memory_order_relaxed);
+    while (cur < bytes && !st.bytes[dev].compare_exchange_weak(cur, bytes, std::memory_order_release)) {}
+  }
+  return ORBIT_OK;
+}
+int num_sms() {
+  static std::atomic<int> n[ORBIT_MAX_DEV];
+  const int dev = device_ordinal();
+  const bool cacheable = dev >= 0 && dev < ORBIT_MAX_DEV;
+  int v = cacheable ? n[dev].load(std::memory_order_relaxed) : 0;
+  if (!v) {
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) { cudaGetLastError(); v = 148; }
+    if (cacheable) n[dev].store(v, std::memory_order_relaxed);
+  }
+  return v;
 }
 
 bool valid_dtype(int dt) { return dt == ORBIT_F32 || dt == ORBIT_BF16; }
@@ -49,7 +86,9 @@ const char* orbit_last_error(void) { return g_err; }
 int orbit_version(void) { return ORBIT_VERSION; }
 long long orbit_launch_count(void) { return g_launches; }
 void orbit_reset_launch_count(void) { g_launches = 0; }
-void orbit_set_debug_force_simt(int on) { g_force_simt = on; }
+#ifdef ORBIT_DEBUG_SWITCH
+void orbit_set_debug_force_simt(int on) { g_force_simt = on; }   // csrc/orbit_debug.h; not part of include/orbit.h
+#endif
 
 // ------------------------------------------------------------------------------------------------------
 // a1 / a1'
@@ -134,7 +173,7 @@ int orbit_debug_layernorm_fwd(int M, int D, orbit_dtype x_dtype, orbit_dtype p_d
                               void* stream) {
   if (!x || !gamma || !beta || !out || !mean || !rstd) { set_error("debug_layernorm_fwd: NULL pointer"); return ORBIT_ERR_NULL; }
   if (!valid_dtype(x_dtype) || !valid_dtype(p_dtype) || !valid_dtype(out_dtype)) { set_error("debug_layernorm_fwd: bad dtype"); return ORBIT_ERR_DTYPE; }
-  if (M <= 0 || D <= 0 || D % 8) { set_error("debug_layernorm_fwd: bad shape M=%d D=%d", M, D); return ORBIT_ERR_SHAPE; }
+  if (M <= 0 || D <= 0 || D % 8 || D > 65536) { set_error("debug_layernorm_fwd: bad shape M=%d D=%d (D <= 65536)", M, D); return ORBIT_ERR_SHAPE; }
   ORBIT_TRY(check_device());
   return layernorm_fwd(x, x_dtype, gamma, beta, p_dtype, out, out_dtype, mean, rstd, M, D, eps, nullptr, (cudaStream_t)stream);
 }
@@ -149,7 +188,7 @@ int orbit_debug_layernorm_bwd(int M, int D, orbit_dtype dout_dtype, orbit_dtype 
   if (!valid_dtype(dout_dtype) || !valid_dtype(x_dtype) || !valid_dtype(p_dtype) || !valid_dtype(add_dtype) || !valid_dtype(out_dtype)) {
     set_error("debug_layernorm_bwd: bad dtype"); return ORBIT_ERR_DTYPE;
   }
-  if (M <= 0 || D <= 0 || D % 8) { set_error("debug_layernorm_bwd: bad shape M=%d D=%d", M, D); return ORBIT_ERR_SHAPE; }
+  if (M <= 0 || D <= 0 || D % 8 || D > ORBIT_LN_MAX_D) { set_error("debug_layernorm_bwd: bad shape M=%d D=%d (D <= 16384)", M, D); return ORBIT_ERR_SHAPE; }
   ORBIT_TRY(check_device());
   return layernorm_bwd(dout, dout_dtype, x, x_dtype, mean, rstd, gamma, p_dtype, add, add_dtype, dx_f32, dx_out, out_dtype,
                        dgamma_acc, dbeta_acc, M, D, (cudaStream_t)stream);

@@ -97,8 +97,8 @@ int check_head(const orbit_head_desc* d) {
   if (!valid_dtype(d->dtype) || !valid_dtype(d->resid_dtype)) { set_error("head: bad dtype"); return ORBIT_ERR_DTYPE; }
   if (d->dtype == ORBIT_F32 && d->resid_dtype != ORBIT_F32) { set_error("head: resid_dtype must be F32 when dtype is F32"); return ORBIT_ERR_DTYPE; }
   if (d->B <= 0 || d->V <= 0 || d->Hg <= 0 || d->Wg <= 0 || d->p <= 0 || d->D <= 0 || d->Hg % d->p || d->Wg % d->p || d->D % 8 ||
-      (d->V * d->p * d->p) % 8) {
-    set_error("head: bad shape B=%d V=%d grid=%dx%d p=%d D=%d (need Hg%%p==0, Wg%%p==0, D%%8==0, (V p^2)%%8==0)", d->B, d->V,
+      (d->V * d->p * d->p) % 8 || d->D > ORBIT_LN_MAX_D) {
+    set_error("head: bad shape B=%d V=%d grid=%dx%d p=%d D=%d (need Hg%%p==0, Wg%%p==0, D%%8==0, (V p^2)%%8==0, D<=16384)", d->B, d->V,
               d->Hg, d->Wg, d->p, d->D);
     return ORBIT_ERR_SHAPE;
   }

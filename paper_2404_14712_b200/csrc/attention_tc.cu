@@ -405,8 +405,7 @@ template <int DH> size_t dkv_smem() { return 6 * Tile<DH>::BYTES + 4 * BC * size
 
 template <int DH>
 int launch_fwd(const AttnArgs& a, cudaStream_t s) {
-  static bool set = false;
-  if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_fwd_tc_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fwd_smem<DH>())); set = true; }
+  ORBIT_SMEM_ATTR(attn_fwd_tc_kernel<DH>, fwd_smem<DH>());
   dim3 grid(cdiv(a.N, BR), a.B * a.heads);
   attn_fwd_tc_kernel<DH><<<grid, NT, fwd_smem<DH>(), s>>>(a, LOG2E / sqrtf((float)DH));
   ORBIT_LAUNCH_CHECK();
@@ -414,12 +413,8 @@ int launch_fwd(const AttnArgs& a, cudaStream_t s) {
 }
 template <int DH>
 int launch_bwd(const AttnArgs& a, cudaStream_t s) {
-  static bool set = false;
-  if (!set) {
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_bwd_dq_tc_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dq_smem<DH>()));
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_bwd_dkv_tc_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dkv_smem<DH>()));
-    set = true;
-  }
+  ORBIT_SMEM_ATTR(attn_bwd_dq_tc_kernel<DH>, dq_smem<DH>());
+  ORBIT_SMEM_ATTR(attn_bwd_dkv_tc_kernel<DH>, dkv_smem<DH>());
   const int total_w = a.B * a.heads * a.N;
   attn_delta_tc_kernel<<<cdiv((long long)total_w * 32, 256), 256, 0, s>>>(a);
   ORBIT_LAUNCH_CHECK();

@@ -6,7 +6,7 @@
 //                                                     O  += P_j V_j  (fp32, TMEM)
 //   warps 2..9  : softmax; two warps share a TMEM lane quarter (thread <-> query row <-> TMEM lane) and split the
 //                 tile's 128 key columns: tcgen05.ld of the S half-row, row max (agreed between the pair through
-//                 shared memory as ceil(max) in int16), exp2 / row sum, P_j as bf16 into a swizzled K-major
+//                 shared memory as ceil(max), a float), exp2 / row sum, P_j as bf16 into a swizzled K-major
 //                 shared-memory tile (the A operand of the PV product) whose two 64-key halves are published and
 //                 released separately (PV_j starts on the first half while the second is still being written),
 //                 lazy rescale of O in TMEM (only when a row max grows by more than 2^8: stale maxima keep exp2
@@ -55,22 +55,26 @@ struct Cfg {
   // only after O += P_j V_j; with 3 + 2 stages the TMA round trip of K_{j+1} no longer sits between PV_{j-1} and S_{j+1}
   // (measured with clock64 stamps: the MMA thread waited ~2000 of 2750 cycles per tile for K/V with a shared 2-stage ring)
   static constexpr int KST = 3, VST = 2;
-  static constexpr int SMEM = TILE /*Q*/ + (KST + VST) * TILE + P_BYTES + 1024 + 256 + 1024 /*row-max exchange*/;
+  static constexpr int SMEM = TILE /*Q*/ + (KST + VST) * TILE + P_BYTES + 256 /*alignment slack, see the kernel*/ + 256 + 2048 /*row-max exchange*/;
 };
 
 template <int DH>
 __global__ void __launch_bounds__(NTH, 1)
 attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float sl2) {
   using C = Cfg<DH>;
-  extern __shared__ uint8_t smem_raw[];
+  // the 128B-swizzled tiles need 1024-byte aligned shared addresses: the alignment is requested on the declaration
+  // (dynamic shared memory starts at the window's 1 KB-aligned base when the kernel has no static shared memory) and
+  // the budget keeps only 256 bytes of slack, so a base that is further off fails loudly instead of overrunning
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  if (base - ptx::smem_u32(smem_raw) > 256u) __trap();
   constexpr int KST = C::KST, VST = C::VST;
   const uint32_t sQ = base, sK0 = sQ + C::TILE, sV0 = sK0 + KST * C::TILE, sP = sV0 + VST * C::TILE, bar = sP + C::P_BYTES;
   auto sK = [&](int st) { return sK0 + st * C::TILE; };
   auto sV = [&](int st) { return sV0 + st * C::TILE; };
   const uint32_t q_full = bar, k_full0 = bar + 8, k_empty0 = k_full0 + 8 * KST, v_full0 = k_empty0 + 8 * KST,
                  v_empty0 = v_full0 + 8 * VST, s_full0 = v_empty0 + 8 * VST, s_empty0 = s_full0 + 16, p_full0 = s_empty0 + 16,
-                 p_free0 = p_full0 + 16, o_done = p_free0 + 16, tmem_slot = o_done + 8, xmax = bar + 256;   // xmax: int16 [2 parity][2 halves][128 rows]
+                 p_free0 = p_full0 + 16, o_done = p_free0 + 16, tmem_slot = o_done + 8, xmax = bar + 256;   // xmax: fp32 [2 parity][2 halves][128 rows]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int q0 = blockIdx.x * BQ;
@@ -165,8 +169,9 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
     // Two warps share a TMEM lane quarter (32 query rows) and split the tile's 128 key columns: the exponentials of a
     // row are issued from two schedulers' worth of warps instead of one (with 4 softmax warps the single warp per SM
     // sub-partition could not hide its own MUFU / TMEM latencies: ~2900 cycles per tile against ~1050 of MMA).
-    // The pair agrees on the row maximum through shared memory as ceil(max) in int16: any common reference >= the
-    // true maximum is exact for softmax (it cancels in P / l), and the integer keeps the exchange at 1 KB.
+    // The pair agrees on the row maximum through shared memory as ceil(max): any common reference >= the true
+    // maximum is exact for softmax (it cancels in P / l); exchanged as fp32 so runaway logits (the regime QK-LayerNorm
+    // targets) do not saturate the reference.
     const int quarter = warp & 3, half = (warp - 2) >> 2;   // warps 2..9
     const int r = quarter * 32 + lane;                       // query row within the tile = TMEM lane
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
@@ -195,13 +200,13 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
 #pragma unroll
         for (int c = 0; c < 64; c++) mx = fmaxf(mx, __uint_as_float(s[c]));
       }
-      const int mi = (int)fminf(fmaxf(ceilf(mx * sl2), -32768.f), 32767.f);
-      const uint32_t xm = xmax + (uint32_t)(sb * 256 + r) * 2;          // [parity][half][row]
-      asm volatile("st.shared.b16 [%0], %1;" ::"r"(xm + half * 256), "h"((short)mi) : "memory");
+      const float mi = ceilf(mx * sl2);                                  // -inf when this half of a ragged tile is fully masked
+      const uint32_t xm = xmax + (uint32_t)(sb * 256 + r) * 4;          // [parity][half][row] fp32 (no range limit on the logits)
+      asm volatile("st.shared.f32 [%0], %1;" ::"r"(xm + half * 512), "f"(mi) : "memory");
       named_bar_sync(pair_bar, 64);
-      short mo;
-      asm volatile("ld.shared.b16 %0, [%1];" : "=h"(mo) : "r"(xm + (half ^ 1) * 256) : "memory");
-      const float m_tile = (float)max(mi, (int)mo);
+      float mo;
+      asm volatile("ld.shared.f32 %0, [%1];" : "=f"(mo) : "r"(xm + (half ^ 1) * 512) : "memory");
+      const float m_tile = fmaxf(mi, mo);
       float m_new = m_used;
       bool need = false;
       if (j == 0) m_new = m_tile;
@@ -726,11 +731,7 @@ int launch_fwd5(const AttnArgs& a, cudaStream_t s) {
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { set_error("attention: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
-  static bool set = false;
-  if (!set) {
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_fwd_tc5_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<DH>::SMEM));
-    set = true;
-  }
+  ORBIT_SMEM_ATTR(attn_fwd_tc5_kernel<DH>, Cfg<DH>::SMEM);
   dim3 grid(cdiv(a.N, BQ), a.B * a.heads);
   attn_fwd_tc5_kernel<DH><<<grid, NTH, Cfg<DH>::SMEM, s>>>(tm, a, LOG2E / sqrtf((float)DH));
   ORBIT_LAUNCH_CHECK();
@@ -758,12 +759,8 @@ int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_TRY(make_map5(&tmSmall, a.qkv, a.ld, rows, 64));
   ORBIT_TRY(make_map5(&tmdOBig, a.dO, a.lddo, rows, 128));
   ORBIT_TRY(make_map5(&tmdOSmall, a.dO, a.lddo, rows, 64));
-  static bool set = false;
-  if (!set) {
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_bwd_dkv_tc5_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, CfgB<DH>::SMEM_DKV));
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)attn_bwd_dq_tc5_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, CfgB<DH>::SMEM_DQ));
-    set = true;
-  }
+  ORBIT_SMEM_ATTR(attn_bwd_dkv_tc5_kernel<DH>, CfgB<DH>::SMEM_DKV);
+  ORBIT_SMEM_ATTR(attn_bwd_dq_tc5_kernel<DH>, CfgB<DH>::SMEM_DQ);
   const int total_w = a.B * a.heads * a.N;
   attn_delta5_kernel<<<cdiv((long long)total_w * 32, 256), 256, 0, s>>>(a);
   ORBIT_LAUNCH_CHECK();

@@ -4,6 +4,7 @@
 #include <cuda_bf16.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <atomic>
 #include "../../include/orbit.h"
 
 namespace orbit {
@@ -13,7 +14,15 @@ typedef __nv_bfloat16 bf16;
 // ---- error state (thread-local) --------------------------------------------------------------
 void set_error(const char* fmt, ...);
 extern thread_local long long g_launches;
+// A/B switch between kernel variants (0 = the product dispatch).  Compiled in only with -DORBIT_DEBUG_SWITCH
+// (`ORBIT_DEBUG_SWITCH=1 python -m paper_2404_14712_b200.build` -> liborbit_dbg.so, which also exports
+// orbit_set_debug_force_simt, declared in csrc/orbit_debug.h); in the shipped liborbit.so it is the constant 0, so the
+// alternative branches fold away and no process-wide dispatch state exists.
+#ifdef ORBIT_DEBUG_SWITCH
 extern int g_force_simt;
+#else
+constexpr int g_force_simt = 0;
+#endif
 inline void count_launch(int n = 1) { g_launches += n; }
 
 #define ORBIT_CUDA_CHECK(expr)                                                                   \
@@ -33,6 +42,21 @@ inline void count_launch(int n = 1) { g_launches += n; }
       orbit::set_error("%s:%d launch -> %s", __FILE__, __LINE__, cudaGetErrorString(_e));        \
       return ORBIT_ERR_CUDA;                                                                     \
     }                                                                                            \
+  } while (0)
+
+// ---- per-device one-time launch setup --------------------------------------------------------------
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the (function, device) pair, not to the process: the record is
+// kept per device ordinal (atomics: two host threads may race, both then set the same value, which is harmless) and
+// remembers the largest size requested so far, so call sites whose size depends on the shape stay correct.
+constexpr int ORBIT_MAX_DEV = 64;
+struct SmemAttrOnce { std::atomic<int> bytes[ORBIT_MAX_DEV]; };
+int smem_attr_once(SmemAttrOnce& st, const void* fn, int bytes);
+int device_ordinal();            // cudaGetDevice (0 when it fails; the launch that follows reports the error)
+int num_sms();                   // multiprocessor count of the current device (cached per device)
+#define ORBIT_SMEM_ATTR(fn, nbytes)                                                              \
+  do {                                                                                           \
+    static orbit::SmemAttrOnce _once;                                                            \
+    ORBIT_TRY(orbit::smem_attr_once(_once, (const void*)(fn), (int)(nbytes)));                   \
   } while (0)
 
 #define ORBIT_TRY(expr)                                                                          \
@@ -117,6 +141,10 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s);        // tcgen05 + TMA, bf16 in
 bool gemm_tc_supported(const GemmArgs& g);
 int gemm_profile_enable(int on);
 int gemm_profile_collect(double* ms, double* flops, long long* launches);
+
+// widest row the LayerNorm kernels take (backward: 4 chunks of 8 columns per thread, 512 threads); entry points reject
+// wider models with ORBIT_ERR_SHAPE before the first launch
+constexpr int ORBIT_LN_MAX_D = 16384;
 
 // ---- row-wise / reduction kernels (rowops.cu) -----------------------------------------------------
 int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,

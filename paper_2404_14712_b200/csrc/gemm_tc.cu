@@ -214,17 +214,6 @@ int make_map(CUtensorMap* m, const void* base, long long inner, long long outer,
   return ORBIT_OK;
 }
 
-int num_sms() {
-  static int n = 0;
-  if (!n) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    if (n <= 0) n = 148;
-  }
-  return n;
-}
-
 // ---- optional per-launch CUDA-event timing of the tensor-core GEMM (bench.py's roofline leg) ----------------
 struct Prof {
   bool on = false;
@@ -238,12 +227,7 @@ Prof g_prof;
 template <int A_MN, int B_MN, int BN>
 int launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, cudaStream_t s) {
   using Cf = TcCfg<BN>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)gemm_tc_kernel<A_MN, B_MN, BN>,
-                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cf::SMEM_BYTES));
-    attr_set = true;
-  }
+  ORBIT_SMEM_ATTR((gemm_tc_kernel<A_MN, B_MN, BN>), Cf::SMEM_BYTES);
   const int batch = g.batch > 1 ? g.batch : 1;
   const long long tiles = (long long)cdiv(g.M, BM) * cdiv(g.N, BN) * batch;
   const int grid = tiles < num_sms() ? (int)tiles : num_sms();

@@ -342,12 +342,7 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc,
             cudaStream_t s) {
   const epi::Args e = epi::from_gemm(g);
   const int M = g.M, N = g.N, K = g.K, batch = g.batch > 1 ? g.batch : 1;
-  static bool attr_set = false;
-  if (!attr_set) {
-    ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)gemm_tc2_kernel<A_MN, B_MN>,
-                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-    attr_set = true;
-  }
+  ORBIT_SMEM_ATTR((gemm_tc2_kernel<A_MN, B_MN>), SMEM_BYTES);
   const long long tiles = (long long)cdiv(M, BM2) * cdiv(N, BN2) * batch;
   int clusters = sms / 2;
   if (tiles < clusters) clusters = (int)tiles;

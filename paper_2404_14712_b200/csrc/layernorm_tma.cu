@@ -548,13 +548,15 @@ int layernorm_fwd_tma(const void* x, int x_dt, const void* gamma, const void* be
   int per_sm, NS; size_t smem;
 #define LNF(C)                                                                                                       \
   do {                                                                                                               \
-    static int regs = 0;                                                                                             \
+    static std::atomic<int> regs_c{0};   /* registers per thread: a property of the binary, not of the device */          \
+    int regs = regs_c.load(std::memory_order_relaxed);                                                               \
     if (!regs) {                                                                                                     \
       cudaFuncAttributes fa;                                                                                         \
-      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_fwd_tma_kernel<C>));                               \
-      ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)ln_fwd_tma_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX)); \
+      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_fwd_tma_kernel<C>));\
       regs = fa.numRegs;                                                                                             \
+      regs_c.store(regs, std::memory_order_relaxed);                                                                 \
     }                                                                                                                \
+    ORBIT_SMEM_ATTR(ln_fwd_tma_kernel<C>, SMEM_MAX);                                                                  \
     shape(T, regs, (size_t)D * dsize(x_dt), 8, &per_sm, &NS, &smem);                                                 \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > M) grid = M;                                                                                          \
@@ -562,13 +564,15 @@ int layernorm_fwd_tma(const void* x, int x_dt, const void* gamma, const void* be
   } while (0)
 #define LNFR(RR)                                                                                                     \
   do {                                                                                                               \
-    static int regs = 0;                                                                                             \
+    static std::atomic<int> regs_c{0};   /* registers per thread: a property of the binary, not of the device */          \
+    int regs = regs_c.load(std::memory_order_relaxed);                                                               \
     if (!regs) {                                                                                                     \
       cudaFuncAttributes fa;                                                                                         \
-      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_fwd_tma_rows_kernel<RR>));                         \
-      ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)ln_fwd_tma_rows_kernel<RR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX)); \
+      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_fwd_tma_rows_kernel<RR>));\
       regs = fa.numRegs;                                                                                             \
+      regs_c.store(regs, std::memory_order_relaxed);                                                                 \
     }                                                                                                                \
+    ORBIT_SMEM_ATTR(ln_fwd_tma_rows_kernel<RR>, SMEM_MAX);                                                                  \
     shape(T, regs, (size_t)RR * D * dsize(x_dt), 8, &per_sm, &NS, &smem);                                            \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > cdiv(M, RR)) grid = cdiv(M, RR);                                                                      \
@@ -596,13 +600,15 @@ int layernorm_bwd_tma(const void* dout, int dout_dt, const void* x, int x_dt, co
   if (2 * stage > (size_t)SMEM_MAX) { add_direct = 1; stage = (size_t)D * (dsize(x_dt) + dsize(dout_dt)); }
 #define LNB(C)                                                                                                       \
   do {                                                                                                               \
-    static int regs = 0;                                                                                             \
+    static std::atomic<int> regs_c{0};   /* registers per thread: a property of the binary, not of the device */          \
+    int regs = regs_c.load(std::memory_order_relaxed);                                                               \
     if (!regs) {                                                                                                     \
       cudaFuncAttributes fa;                                                                                         \
-      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_bwd_tma_kernel<C>));                               \
-      ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)ln_bwd_tma_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX)); \
+      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_bwd_tma_kernel<C>));\
       regs = fa.numRegs;                                                                                             \
+      regs_c.store(regs, std::memory_order_relaxed);                                                                 \
     }                                                                                                                \
+    ORBIT_SMEM_ATTR(ln_bwd_tma_kernel<C>, SMEM_MAX);                                                                  \
     shape(T, regs, stage, 4, &per_sm, &NS, &smem);                                                                   \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > M) grid = M;                                                                                          \
@@ -611,13 +617,15 @@ int layernorm_bwd_tma(const void* dout, int dout_dt, const void* x, int x_dt, co
   } while (0)
 #define LNBR(RR)                                                                                                     \
   do {                                                                                                               \
-    static int regs = 0;                                                                                             \
+    static std::atomic<int> regs_c{0};   /* registers per thread: a property of the binary, not of the device */          \
+    int regs = regs_c.load(std::memory_order_relaxed);                                                               \
     if (!regs) {                                                                                                     \
       cudaFuncAttributes fa;                                                                                         \
-      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_bwd_tma_rows_kernel<RR>));                         \
-      ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)ln_bwd_tma_rows_kernel<RR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX)); \
+      ORBIT_CUDA_CHECK(cudaFuncGetAttributes(&fa, (const void*)ln_bwd_tma_rows_kernel<RR>));\
       regs = fa.numRegs;                                                                                             \
+      regs_c.store(regs, std::memory_order_relaxed);                                                                 \
     }                                                                                                                \
+    ORBIT_SMEM_ATTR(ln_bwd_tma_rows_kernel<RR>, SMEM_MAX);                                                                  \
     shape(T, regs, (size_t)RR * stage, 4, &per_sm, &NS, &smem);                                                      \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > cdiv(M, RR)) grid = cdiv(M, RR);                                                                      \

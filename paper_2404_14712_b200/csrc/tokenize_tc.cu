@@ -279,9 +279,7 @@ int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, c
   dim3 grid(d.V * cdiv(d.D, DCH), cdiv((long long)d.B * L, 128));
 #define TF(P, K) do {                                                                                         \
     const size_t smb = (size_t)128 * (K + 8) * 2 + (size_t)K * BROW + (size_t)(NT / 32) * 16 * OROW;                                        \
-    static bool set = false;                                                                                  \
-    if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)tok_fwd_tc_kernel<P, K>,                  \
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }       \
+    ORBIT_SMEM_ATTR((tok_fwd_tc_kernel<P, K>), smb);                                                           \
     tok_fwd_tc_kernel<P, K><<<grid, NT, smb, s>>>(d, x, (const bf16*)Wp, (const bf16*)bp, (bf16*)tok, L); } while (0)
   if (P2 == 16) TF(16, 32);
   else if (P2 == 4) TF(4, 16);
@@ -313,9 +311,7 @@ int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* d
   dim3 grid(d.V * nz, cdiv(BL, ppc));
   const size_t smb = (size_t)4 * 16 * BROW + (size_t)4 * 16 * 16 * sizeof(float);
 #define TB(P) do {                                                                                            \
-    static bool set = false;                                                                                  \
-    if (!set) { ORBIT_CUDA_CHECK(cudaFuncSetAttribute((const void*)tok_bwd_tc_kernel<P>,                     \
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb)); set = true; }       \
+    ORBIT_SMEM_ATTR(tok_bwd_tc_kernel<P>, smb);                                                               \
     tok_bwd_tc_kernel<P><<<grid, NT, smb, s>>>(d, x, (const bf16*)dtok, accW, accB, L, ppc); } while (0)
   if (P2 == 16) TB(16);
   else if (P2 == 4) TB(4);

@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 import torch
 
+import parity
 from oracle import orbit_oracle as orc
 from paper_2404_14712_b200 import inputs as syn
 
@@ -29,11 +30,8 @@ def rn():
 
 
 def check(name, got, ref, tol):
-    got = got.detach().to(torch.float32).cpu().numpy() if isinstance(got, torch.Tensor) else got
-    err = orc.rel_fro(got.reshape(ref.shape), ref)
-    assert np.isfinite(got).all(), f"{name}: non-finite values"
-    assert err <= tol, f"{name}: rel Frobenius error {err:.3e} > {tol:.1e}"
-    return err
+    """relative Frobenius error <= tol AND the element-wise bound of tests/parity.py."""
+    return parity.check(name, got, ref, tol)
 
 
 def make_block_case(seed, B, N, D, heads, F, T, dtype, resid_dtype):
@@ -98,6 +96,30 @@ def test_block_softmax_stress_logits_x30(rn):
     shards = syn.shard_block_params(P, heads, 1)
     br, y, dx = run_block(rn, B, N, D, heads, F, 1, "f32", "f32", P, shards, x, dy)
     compare_block(br, y, dx, P, x, dy, heads, 1, 2e-4)
+
+
+@pytest.mark.parametrize("dh", [64, 128])
+def test_block_bf16_runaway_logits_stay_finite(rn, dh):
+    """Runaway attention logits (the regime QK-LayerNorm targets) on the tcgen05 attention path: logits of
+    order 1e5 (beyond an int16 row-max reference in log2 units) must give finite y / dx / gradients, as on every other
+    path.  No oracle comparison: at this magnitude the softmax is an arg-max decided by the bf16 rounding of q and k
+    (one ulp of a logit is ~4e2), so only the property is checked."""
+    B, N, heads, F = 1, 256, 2, 256
+    D = heads * dh
+    P, shards, x, dy = make_block_case(15, B, N, D, heads, F, 1, "bf16", "bf16")
+    def max_logit(Wm):          # harness-side magnitude estimate (LN1 keeps the rows at unit scale)
+        qkv = x.reshape(-1, D).astype(np.float64) @ Wm.astype(np.float64)
+        return np.abs(qkv[:, :dh] @ qkv[:, D:D + dh].T).max() / math.sqrt(dh)
+    W = P["Wqkv"].copy()
+    W[:, :2 * D] *= np.float32(math.sqrt(1e5 / max_logit(W)))                             # |q.k| / sqrt(d_h) ~ 1e5
+    P["Wqkv"] = syn.round_storage(W, "bf16")
+    shards = syn.shard_block_params(P, heads, 1)
+    br, y, dx = run_block(rn, B, N, D, heads, F, 1, "bf16", "bf16", P, shards, x, dy)
+    big = max_logit(P["Wqkv"])
+    assert big > 4e4, big                                 # log2 units: > 5.7e4, past the int16 range
+    assert torch.isfinite(y.float()).all() and torch.isfinite(dx.float()).all()
+    for k in br.SHARD:
+        assert torch.isfinite(br.gshards[0][k].float()).all(), k
 
 
 @pytest.mark.parametrize("shape", [

@@ -646,3 +646,34 @@ def test_sampled_helpers_equal_slices_of_full_functions():
     Wp, bp = rnd(3, 4, 5), rnd(3, 5)
     ls = np.array([0, 7, 23])
     assert np.array_equal(orc.tokenize_patches(xf, Wp, bp, 2, ls), orc.tokenize(xf, Wp, bp, 2)[:, ls])
+
+
+def test_patch_chunked_front_end_equals_whole_tensor_functions():
+    """tests/parity.front_oracle_chunked (the full-size C3 GPU tests: oracle front end accumulated over chunks of
+    patches, oracle/ functions only) equals tokenize -> var_aggregate -> var_aggregate_bwd -> tokenize_bwd on the
+    whole tensors: agg, dpos assembled by patch, every parameter gradient summed over the chunks (ragged last chunk)."""
+    import parity
+    B, V, Hg, Wg, p, D, h = 2, 3, 8, 12, 2, 8, 2
+    L = (Hg // p) * (Wg // p)
+    x = rnd(B, V, Hg, Wg)
+    emb = {"Wp": rnd(V, p * p, D), "bp": rnd(V, D)}
+    A = rand_agg_params(D)
+    pos, dagg = rnd(L, D), rnd(B, L, D)
+    tok = orc.tokenize(x, emb["Wp"], emb["bp"], p)
+    agg, cache = orc.var_aggregate(tok, A, h, pos)
+    dtok, G, dpos = orc.var_aggregate_bwd(dagg, A, cache, want_dpos=True)
+    dWp, dbp = orc.tokenize_bwd(x, dtok, p)
+    agg_c, dWp_c, dbp_c, G_c, dpos_c = parity.front_oracle_chunked(orc, x, emb, A, dagg, p, h, 5, pos=pos)
+    assert orc.rel_fro(agg_c, agg) < 1e-14 and orc.rel_fro(dpos_c, dpos) < 1e-14
+    assert orc.rel_fro(dWp_c, dWp) < 1e-13 and orc.rel_fro(dbp_c, dbp) < 1e-13
+    for k in G:
+        if k == "bk":
+            assert np.abs(G_c[k]).max() < 1e-12
+        else:
+            assert orc.rel_fro(G_c[k], G[k]) < 1e-13, k
+    # tokenize_bwd_patches over one chunk is the restriction of tokenize_bwd's sums to those patches
+    ls = np.array([1, 4, 9])
+    w, b = orc.tokenize_bwd_patches(x, dtok[:, ls], p, ls)
+    pix = orc.patches(x, p)
+    assert np.allclose(b, dtok[:, ls].sum(axis=(0, 1)), atol=1e-13)
+    assert np.allclose(w[1, 2], np.einsum("bs,bsd->d", pix[:, 1, ls, 2], dtok[:, ls, 1, :]), atol=1e-13)

@@ -145,6 +145,43 @@ size_t orbit_block_fwd_workspace_bytes(const orbit_block_desc* d);
 size_t orbit_block_bwd_workspace_bytes(const orbit_block_desc* d);
 size_t orbit_block_saved_bytes(const orbit_block_desc* d);
 
+/* ---- the rank-local Hybrid-STOP program (Fig. 3): what ONE rank of a
+ * tensor-parallel group of size d->T computes between the collectives.  Rank k holds the column shards Wqkv^k [D, 3D/T]
+ * (= [Q_k | K_k | V_k], head aligned), Wfc1^k [D, F/T] with bqkv^k, bfc1^k and the row shards Wproj^k [D/T, D],
+ * Wfc2^k [F/T, D]: P->shards[0] / G->shards[0] are THIS rank's shard (one element); LayerNorm parameters, bproj, bfc2 are
+ * replicated.  One block is six calls; between them the CALLER all-reduces (sum) `part`, an fp32 [B, N, D] buffer, over
+ * the group -- "GPUs in each tensor-parallel group add their individual activations together", "add their
+ * activation gradients together through all-reduce".  The library holds no communicator.
+ *   orbit_rank_fwd_attn : a = LN1(x); qkv^k = a Wqkv^k + bqkv^k; attention on this rank's heads/T heads;
+ *                         part <- O^k Wproj^k                                             -- all-reduce(part) --
+ *   orbit_rank_fwd_mlp  : x1 = x + part + bproj; m = LN2(x1); g^k = GELU(m Wfc1^k + bfc1^k);
+ *                         part <- g^k Wfc2^k                                              -- all-reduce(part) --
+ *   orbit_rank_fwd_out  : y = x1 + part + bfc2
+ *   orbit_rank_bwd_mlp  : dbfc2, dWfc2^k, du^k, dbfc1^k, dWfc1^k; part <- du^k Wfc1^k^T   -- all-reduce(part) --
+ *   orbit_rank_bwd_attn : dx1 = dy + LN2'(part); d ln2, dbproj, dWproj^k, dO^k, attention backward, dbqkv^k, dWqkv^k;
+ *                         part <- dqkv^k Wqkv^k^T                                         -- all-reduce(part) --
+ *   orbit_rank_bwd_out  : dx = dx1 + LN1'(part); d ln1; gradients cast to `dtype`.
+ * y, dx and the gradients of the replicated parameters come out identical on every rank, except the QK-LayerNorm
+ * gradients (ORBIT_QK_NORM), which are the sums over THIS rank's heads and must be summed over the group by the caller
+ * with its other gradient reductions.  ORBIT_RECOMPUTE -> ORBIT_ERR_UNSUPPORTED.  `saved` (orbit_rank_saved_bytes) is
+ * written by the forward calls and read by the backward calls; `ws` (orbit_rank_bwd_workspace_bytes) must be the SAME
+ * buffer, untouched, through the three backward calls (it carries dx1 and the fp32 gradient accumulators).  Precision:
+ * the partials are fp32 (R15).  Same checks / error codes as orbit_block_*. */
+int orbit_rank_fwd_attn(const orbit_block_desc* d, const void* x /* [B,N,D] */, const orbit_block_params* P,
+                        float* part /* out */, void* saved, void* stream);
+int orbit_rank_fwd_mlp(const orbit_block_desc* d, const orbit_block_params* P, float* part /* in: summed; out */,
+                       void* saved, void* stream);
+int orbit_rank_fwd_out(const orbit_block_desc* d, const orbit_block_params* P, const float* part /* in: summed */,
+                       void* y, const void* saved, void* stream);
+int orbit_rank_bwd_mlp(const orbit_block_desc* d, const void* dy, const orbit_block_params* P, const void* saved,
+                       orbit_block_grads* G, float* part /* out */, void* ws, size_t ws_bytes, void* stream);
+int orbit_rank_bwd_attn(const orbit_block_desc* d, const void* dy, const orbit_block_params* P, const void* saved,
+                        orbit_block_grads* G, float* part /* in: summed; out */, void* ws, size_t ws_bytes, void* stream);
+int orbit_rank_bwd_out(const orbit_block_desc* d, const orbit_block_params* P, const void* saved, orbit_block_grads* G,
+                       const float* part /* in: summed */, void* dx, void* ws, size_t ws_bytes, void* stream);
+size_t orbit_rank_saved_bytes(const orbit_block_desc* d);
+size_t orbit_rank_bwd_workspace_bytes(const orbit_block_desc* d);
+
 /* ---- head + loss: "predictions are computed by projecting the embedding output from the
  * feature space to the image space" and the latitude-weighted MSE the paper trains with;
  * readings R26-R28:  zn = LN_f(z);  P = zn Wh + bh  ([B*L, V p^2], column c = v p^2 + di p + dj);

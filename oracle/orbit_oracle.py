@@ -21,6 +21,8 @@ float64 autograd with F.layer_norm on the per-head q / k, finite differences, lo
 sqrt(d_h) for gamma = 1, beta = 0, invariance to rescaling the pre-norm queries (eps = 0); head + wMSE: torch
 float64 autograd (layer_norm, linear, permute, weighted mean), finite differences, unpatchify = inverse of
 `patches`, weights with mean 1 / equator-symmetric / uniform weights = plain MSE, sum_i cos closed form.
+Rank-local Hybrid-STOP program (rank_block_fwd / rank_block_bwd): world-size-2 gloo run with a real all-reduce
+= the unsharded block (tests/test_multiproc.py), and a plain-sum run for T in {1, 2, 4} (tests/test_oracle_pins.py).
 Parity unpinned: none.
 
 Layout conventions (same as include/orbit.h): row-major, weights [in, out] so y = x A exactly as in
@@ -452,6 +454,87 @@ def block_bwd_sharded(dy, Pc, shards, cache):
     dz1, Gc["ln1_g"], Gc["ln1_b"] = layernorm_bwd(da, cache["xhat"], cache["rstd1"], Pc["ln1_g"])
     dx = dx1 + dz1
     return dx, Gc, Gs
+
+
+# ---------------------------------------------------------------------------------------------
+# RANK -- the rank-local Hybrid-STOP program (Fig. 3): what ONE rank of a tensor-parallel group
+# computes between the collectives.  Rank k holds the column shards Wqkv^k, Wfc1^k (with bqkv^k, bfc1^k) and the row
+# shards Wproj^k, Wfc2^k; the replicated parameters (LayerNorm gains / offsets, bproj, bfc2) live on every rank.
+# "GPUs in each tensor-parallel group add their individual activations together" after the row-sharded
+# products, and "add their activation gradients together through all-reduce" after the transposed
+# column-sharded products: four all-reduce(sum) of an [B, N, D] partial per block.  `allreduce` is passed in (a
+# function partial -> sum over the ranks), so the same code runs under torch.distributed (tests/test_multiproc.py,
+# world size 2, gloo) and with a plain Python sum.  Written separately from BLK / SHARD; pinned against BLK.
+# ---------------------------------------------------------------------------------------------
+def rank_block_fwd(x, Pc, S, heads_local, allreduce, eps=1e-5):
+    """Forward of rank k.  x: the replicated block input [B, N, D]; Pc: replicated parameters; S: this rank's shard
+    (Wqkv [D, 3D/T] = [Q_k | K_k | V_k], bqkv, Wproj [D/T, D], Wfc1 [D, F/T], bfc1, Wfc2 [F/T, D]); heads_local =
+    heads / T.  Returns (y, cache, partials): y is identical on every rank; `partials` are this rank's two
+    pre-all-reduce partial products (what the collective sees)."""
+    x = _f64(x)
+    D = x.shape[-1]
+    dc = _f64(S["Wproj"]).shape[0]
+    a, xhat, rstd1 = layernorm(x, Pc["ln1_g"], Pc["ln1_b"], eps)
+    qkv = a @ _f64(S["Wqkv"]) + _f64(S["bqkv"])
+    Q, K, V = qkv[..., 0:dc], qkv[..., dc:2 * dc], qkv[..., 2 * dc:3 * dc]
+    qkn = None
+    if has_qk_norm(Pc):
+        Q, qhat, qrstd = qk_layernorm(Q, heads_local, Pc["qn_g"], Pc["qn_b"], eps)
+        K, khat, krstd = qk_layernorm(K, heads_local, Pc["kn_g"], Pc["kn_b"], eps)
+        qkn = dict(qhat=qhat, qrstd=qrstd, khat=khat, krstd=krstd)
+    O, Pm = attention(Q, K, V, heads_local)
+    part_proj = O @ _f64(S["Wproj"])                       # row shard: a partial of the full product (Eq. 2)
+    x1 = x + allreduce(part_proj) + _f64(Pc["bproj"])     # PAPER.md:98; bias and residual once, after the sum (R14)
+    m, x1hat, rstd2 = layernorm(x1, Pc["ln2_g"], Pc["ln2_b"], eps)
+    u = m @ _f64(S["Wfc1"]) + _f64(S["bfc1"])
+    g = gelu(u)
+    part_fc2 = g @ _f64(S["Wfc2"])
+    y = x1 + allreduce(part_fc2) + _f64(Pc["bfc2"])
+    cache = dict(xhat=xhat, rstd1=rstd1, a=a, Q=Q, K=K, V=V, Pm=Pm, O=O, qkn=qkn, x1hat=x1hat, rstd2=rstd2, m=m, u=u,
+                 g=g, heads_local=heads_local)
+    return y, cache, dict(proj=part_proj, fc2=part_fc2)
+
+
+def rank_block_bwd(dy, Pc, S, cache, allreduce):
+    """Backward of rank k (Eq. 3).  Returns (dx, Gc, Gs, partials): dx and the gradients Gc of the
+    replicated parameters are identical on every rank EXCEPT the QK-LayerNorm ones (qn_g, qn_b, kn_g, kn_b), which are
+    this rank's sum over its own heads and still have to be summed over the group; Gs are the gradients of this rank's
+    shard; `partials` are the two pre-all-reduce activation-gradient partials."""
+    dy = _f64(dy)
+    B, N, D = dy.shape
+    M = B * N
+    c = cache
+    hk = c["heads_local"]
+    Fk = c["u"].shape[-1]
+    dc = c["O"].shape[-1]
+    Gc, Gs = {}, {}
+    dy2 = dy.reshape(M, D)
+    Gc["bfc2"] = dy2.sum(axis=0)
+    Gs["Wfc2"] = c["g"].reshape(M, Fk).T @ dy2
+    du = (dy @ _f64(S["Wfc2"]).T) * gelu_grad(c["u"])
+    Gs["bfc1"] = du.reshape(M, Fk).sum(axis=0)
+    Gs["Wfc1"] = c["m"].reshape(M, D).T @ du.reshape(M, Fk)
+    part_dm = du @ _f64(S["Wfc1"]).T
+    dm = allreduce(part_dm)                                # PAPER.md:102
+    dz2, Gc["ln2_g"], Gc["ln2_b"] = layernorm_bwd(dm, c["x1hat"], c["rstd2"], Pc["ln2_g"])
+    dx1 = dy + dz2
+    dx12 = dx1.reshape(M, D)
+    Gc["bproj"] = dx12.sum(axis=0)
+    Gs["Wproj"] = c["O"].reshape(M, dc).T @ dx12
+    dO = dx1 @ _f64(S["Wproj"]).T
+    dQ, dK, dV = attention_bwd(dO, c["Q"], c["K"], c["V"], c["Pm"], hk)
+    if c.get("qkn") is not None:
+        n = c["qkn"]
+        dQ, Gc["qn_g"], Gc["qn_b"] = qk_layernorm_bwd(dQ, hk, n["qhat"], n["qrstd"], Pc["qn_g"])
+        dK, Gc["kn_g"], Gc["kn_b"] = qk_layernorm_bwd(dK, hk, n["khat"], n["krstd"], Pc["kn_g"])
+    dqkv = np.concatenate([dQ, dK, dV], axis=-1)
+    Gs["bqkv"] = dqkv.reshape(M, 3 * dc).sum(axis=0)
+    Gs["Wqkv"] = c["a"].reshape(M, D).T @ dqkv.reshape(M, 3 * dc)
+    part_da = dqkv @ _f64(S["Wqkv"]).T
+    da = allreduce(part_da)
+    dz1, Gc["ln1_g"], Gc["ln1_b"] = layernorm_bwd(da, c["xhat"], c["rstd1"], Pc["ln1_g"])
+    dx = dx1 + dz1
+    return dx, Gc, Gs, dict(dm=part_dm, da=part_da)
 
 
 # ---------------------------------------------------------------------------------------------

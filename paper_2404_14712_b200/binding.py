@@ -105,6 +105,15 @@ _proto("orbit_last_error", C.c_char_p, [])
 _proto("orbit_version", C.c_int, [])
 _proto("orbit_launch_count", C.c_longlong, [])
 _proto("orbit_reset_launch_count", None, [])
+_bd, _bp, _bg = C.POINTER(orbit_block_desc), C.POINTER(orbit_block_params), C.POINTER(orbit_block_grads)
+_proto("orbit_rank_fwd_attn", C.c_int, [_bd, _vp, _bp, _vp, _vp, _vp])
+_proto("orbit_rank_fwd_mlp", C.c_int, [_bd, _bp, _vp, _vp, _vp])
+_proto("orbit_rank_fwd_out", C.c_int, [_bd, _bp, _vp, _vp, _vp, _vp])
+_proto("orbit_rank_bwd_mlp", C.c_int, [_bd, _vp, _bp, _vp, _bg, _vp, _vp, _sz, _vp])
+_proto("orbit_rank_bwd_attn", C.c_int, [_bd, _vp, _bp, _vp, _bg, _vp, _vp, _sz, _vp])
+_proto("orbit_rank_bwd_out", C.c_int, [_bd, _bp, _vp, _bg, _vp, _vp, _vp, _sz, _vp])
+_proto("orbit_rank_saved_bytes", _sz, [_bd])
+_proto("orbit_rank_bwd_workspace_bytes", _sz, [_bd])
 HAS_DEBUG_SWITCH = hasattr(lib, "orbit_set_debug_force_simt")      # only the A/B build exports it (csrc/orbit_debug.h)
 if HAS_DEBUG_SWITCH:
     _proto("orbit_set_debug_force_simt", None, [C.c_int])
@@ -161,7 +170,9 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
            "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched", "orbit_head_loss", "orbit_head_loss_bwd",
            "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes",
-           "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd", "orbit_debug_gemm_out"]
+           "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd", "orbit_debug_gemm_out",
+           "orbit_rank_fwd_attn", "orbit_rank_fwd_mlp", "orbit_rank_fwd_out", "orbit_rank_bwd_mlp", "orbit_rank_bwd_attn",
+           "orbit_rank_bwd_out", "orbit_rank_saved_bytes", "orbit_rank_bwd_workspace_bytes"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -329,6 +340,54 @@ def orbit_block_bwd(d, dy, common, shards, saved, dx, gcommon, gshards, ws, stre
     gs = _block_struct(orbit_block_grads, gcommon, gshards)
     _check(lib.orbit_block_bwd(C.byref(d), _ptr(dy), C.byref(ps), _ptr(saved), _ptr(dx), C.byref(gs), _ptr(ws),
                                ws.numel() * ws.element_size(), _stream(stream)), "orbit_block_bwd")
+
+
+# ---- rank-local Hybrid-STOP program: `shard` / `gshard` are THIS rank's shard dicts, `part` the fp32 [B,N,D] partial the
+# caller all-reduces between the calls (include/orbit.h)
+def orbit_rank_saved_bytes(d):
+    return lib.orbit_rank_saved_bytes(C.byref(d))
+
+
+def orbit_rank_bwd_workspace_bytes(d):
+    return lib.orbit_rank_bwd_workspace_bytes(C.byref(d))
+
+
+def orbit_rank_fwd_attn(d, x, common, shard, part, saved, stream=None):
+    ps = _block_struct(orbit_block_params, common, [shard])
+    _check(lib.orbit_rank_fwd_attn(C.byref(d), _ptr(x), C.byref(ps), _ptr(part), _ptr(saved), _stream(stream)),
+           "orbit_rank_fwd_attn")
+
+
+def orbit_rank_fwd_mlp(d, common, shard, part, saved, stream=None):
+    ps = _block_struct(orbit_block_params, common, [shard])
+    _check(lib.orbit_rank_fwd_mlp(C.byref(d), C.byref(ps), _ptr(part), _ptr(saved), _stream(stream)), "orbit_rank_fwd_mlp")
+
+
+def orbit_rank_fwd_out(d, common, shard, part, y, saved, stream=None):
+    ps = _block_struct(orbit_block_params, common, [shard])
+    _check(lib.orbit_rank_fwd_out(C.byref(d), C.byref(ps), _ptr(part), _ptr(y), _ptr(saved), _stream(stream)),
+           "orbit_rank_fwd_out")
+
+
+def orbit_rank_bwd_mlp(d, dy, common, shard, saved, gcommon, gshard, part, ws, stream=None):
+    ps = _block_struct(orbit_block_params, common, [shard])
+    gs = _block_struct(orbit_block_grads, gcommon, [gshard])
+    _check(lib.orbit_rank_bwd_mlp(C.byref(d), _ptr(dy), C.byref(ps), _ptr(saved), C.byref(gs), _ptr(part), _ptr(ws),
+                                  ws.numel() * ws.element_size(), _stream(stream)), "orbit_rank_bwd_mlp")
+
+
+def orbit_rank_bwd_attn(d, dy, common, shard, saved, gcommon, gshard, part, ws, stream=None):
+    ps = _block_struct(orbit_block_params, common, [shard])
+    gs = _block_struct(orbit_block_grads, gcommon, [gshard])
+    _check(lib.orbit_rank_bwd_attn(C.byref(d), _ptr(dy), C.byref(ps), _ptr(saved), C.byref(gs), _ptr(part), _ptr(ws),
+                                   ws.numel() * ws.element_size(), _stream(stream)), "orbit_rank_bwd_attn")
+
+
+def orbit_rank_bwd_out(d, common, shard, saved, gcommon, gshard, part, dx, ws, stream=None):
+    ps = _block_struct(orbit_block_params, common, [shard])
+    gs = _block_struct(orbit_block_grads, gcommon, [gshard])
+    _check(lib.orbit_rank_bwd_out(C.byref(d), C.byref(ps), _ptr(saved), C.byref(gs), _ptr(part), _ptr(dx), _ptr(ws),
+                                  ws.numel() * ws.element_size(), _stream(stream)), "orbit_rank_bwd_out")
 
 
 def _ptr_array(ts):

@@ -73,6 +73,8 @@ BlockBwdWs carve_bwd(const orbit_block_desc& d, void* base) {
   return w;
 }
 
+}  // namespace
+
 int check_block(const orbit_block_desc* d) {
   if (!d) { set_error("block desc is NULL"); return ORBIT_ERR_NULL; }
   if (!valid_dtype(d->dtype) || !valid_dtype(d->resid_dtype)) { set_error("block: bad dtype"); return ORBIT_ERR_DTYPE; }
@@ -90,9 +92,9 @@ int check_block(const orbit_block_desc* d) {
   }
   return ORBIT_OK;
 }
-int check_block_params(const orbit_block_desc* d, const orbit_block_params* P) {
+static int check_params_n(const orbit_block_desc* d, const orbit_block_params* P, int nshards) {
   if (!P || !P->ln1_g || !P->ln1_b || !P->ln2_g || !P->ln2_b || !P->bproj || !P->bfc2 || !P->shards) { set_error("block: NULL parameter"); return ORBIT_ERR_NULL; }
-  for (int k = 0; k < d->T; k++) {
+  for (int k = 0; k < nshards; k++) {
     const orbit_block_shard& S = P->shards[k];
     if (!S.Wqkv || !S.bqkv || !S.Wproj || !S.Wfc1 || !S.bfc1 || !S.Wfc2) { set_error("block: NULL shard parameter (shard %d)", k); return ORBIT_ERR_NULL; }
     if (!aligned16(S.Wqkv) || !aligned16(S.bqkv) || !aligned16(S.Wproj) || !aligned16(S.Wfc1) || !aligned16(S.bfc1) || !aligned16(S.Wfc2)) { set_error("block: shard parameter not 16B aligned"); return ORBIT_ERR_ALIGN; }
@@ -105,6 +107,10 @@ int check_block_params(const orbit_block_desc* d, const orbit_block_params* P) {
   return ORBIT_OK;
 }
 
+int check_block_params(const orbit_block_desc* d, const orbit_block_params* P) { return check_params_n(d, P, d->T); }
+int check_shard_params(const orbit_block_desc* d, const orbit_block_params* P) { return check_params_n(d, P, 1); }
+
+namespace {
 AttnArgs attn_args(const orbit_block_desc& d, const BlockSaved& sv, int k) {
   const int dc = d.D / d.T, hk = d.heads / d.T, dh = d.D / d.heads;
   const size_t M = (size_t)d.B * d.N;

@@ -21,6 +21,11 @@ struct Carver {
   template <typename T> T* take_n(size_t n) { return (T*)take(n * sizeof(T)); }
 };
 
+// shape / dtype / flag checks shared by orbit_block_* (api_block.cu) and the rank-local orbit_rank_* calls (api_shard.cu)
+int check_block(const orbit_block_desc* d);
+int check_block_params(const orbit_block_desc* d, const orbit_block_params* P);   // reads P->shards[0 .. T)
+int check_shard_params(const orbit_block_desc* d, const orbit_block_params* P);   // reads P->shards[0] only
+
 inline const void* offs(const void* p, size_t elems, int dt) { return (const char*)p + elems * dsize(dt); }
 inline void* offs(void* p, size_t elems, int dt) { return (char*)p + elems * dsize(dt); }
 

@@ -71,6 +71,57 @@ class BlockRunner:
         return self.dx
 
 
+class RankBlockRunner:
+    """One rank of a tensor-parallel group running the rank-local Hybrid-STOP program (orbit_rank_*):
+    six C-ABI calls with four all-reduce(sum) of the fp32 [B, N, D] partial in between.  `allreduce(t)` sums the tensor
+    `t` in place over the group (default: torch.distributed.all_reduce on the default group -- NCCL over NVLink on a
+    multi-GPU node, gloo in the tests).  `shard` is THIS rank's shard dict."""
+
+    COMMON = ob._COMMON_NAMES
+    SHARD = ob._SHARD_NAMES
+
+    def __init__(self, B, N, D, heads, F, T, dtype, resid_dtype, common: dict, shard: dict, allreduce=None, ln_eps=1e-5,
+                 device="cuda"):
+        self.qk_norm = "qn_g" in common
+        self.desc = ob.block_desc(B, N, D, heads, F, T, ln_eps, dtype, resid_dtype, ob.ORBIT_QK_NORM if self.qk_norm else 0)
+        names = self.COMMON + (ob._QKN_NAMES if self.qk_norm else ())
+        self.common = {k: to_dev(common[k], dtype, device) for k in names}
+        self.shard = {k: to_dev(shard[k], dtype, device) for k in self.SHARD}
+        self.gcommon = {k: torch.empty_like(v) for k, v in self.common.items()}
+        self.gshard = {k: torch.empty_like(v) for k, v in self.shard.items()}
+        self.saved = _bytes(ob.orbit_rank_saved_bytes(self.desc), device)
+        self.ws = _bytes(ob.orbit_rank_bwd_workspace_bytes(self.desc), device)
+        self.part = torch.empty(B, N, D, dtype=torch.float32, device=device)
+        self.y = torch.empty(B, N, D, dtype=TD[resid_dtype], device=device)
+        self.dx = torch.empty(B, N, D, dtype=TD[resid_dtype], device=device)
+        if allreduce is None:
+            import torch.distributed as dist
+            allreduce = dist.all_reduce
+        self.allreduce = allreduce
+        self.partials = None          # optional dict: copies of this rank's pre-all-reduce partials (tests)
+
+    def _reduce(self, name):
+        if self.partials is not None:
+            self.partials[name] = self.part.clone()
+        self.allreduce(self.part)
+
+    def fwd(self, x):
+        ob.orbit_rank_fwd_attn(self.desc, x, self.common, self.shard, self.part, self.saved)
+        self._reduce("proj")
+        ob.orbit_rank_fwd_mlp(self.desc, self.common, self.shard, self.part, self.saved)
+        self._reduce("fc2")
+        ob.orbit_rank_fwd_out(self.desc, self.common, self.shard, self.part, self.y, self.saved)
+        return self.y
+
+    def bwd(self, dy):
+        ob.orbit_rank_bwd_mlp(self.desc, dy, self.common, self.shard, self.saved, self.gcommon, self.gshard, self.part, self.ws)
+        self._reduce("dm")
+        ob.orbit_rank_bwd_attn(self.desc, dy, self.common, self.shard, self.saved, self.gcommon, self.gshard, self.part, self.ws)
+        self._reduce("da")
+        ob.orbit_rank_bwd_out(self.desc, self.common, self.shard, self.saved, self.gcommon, self.gshard, self.part, self.dx, self.ws)
+        return self.dx
+
+
 class FrontRunner:
     """orbit_tokenize + orbit_var_aggregate and their backward."""
 

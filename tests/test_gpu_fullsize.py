@@ -124,6 +124,22 @@ def test_c4_fullsize_hybrid_stop_vs_unsharded_oracle(rn):
         errs[k] = rel(Gu[k], G[k])
     print("C4 errs", {k: f"{v:.2e}" for k, v in errs.items()})
     assert max(errs.values()) <= TOL, errs
+    # the same block as the rank-local program (orbit_rank_*): 4 ranks in lock step on this GPU, the fp32 partials summed
+    # between the calls as an all-reduce would, against the same unsharded oracle
+    del br
+    from test_gpu_rank import run_ranks
+    runners, _ = run_ranks(rn, (cfg.B, cfg.L, cfg.D, cfg.heads, cfg.F), cfg.T, cfg.dtype, cfg.resid_dtype, P, x, dy)
+    errs = {}
+    for k, r in enumerate(runners):
+        errs[f"r{k}.y"] = rel(r.y, yo, f"rank{k}.y")
+        errs[f"r{k}.dx"] = rel(r.dx, dxo, f"rank{k}.dx")
+        for name in r.COMMON:
+            errs[f"r{k}.{name}"] = rel(r.gcommon[name], G[name], f"rank{k}.d{name}")
+    Gu = syn.unshard_block_grads([{n: parity.to_np(v) for n, v in r.gshard.items()} for r in runners], cfg.T)
+    for name in Gu:
+        errs["rank." + name] = rel(Gu[name], G[name], "rank-local d" + name)
+    print("C4 rank-local errs", {k: f"{v:.2e}" for k, v in errs.items() if not k.startswith(("r1", "r2", "r3"))})
+    assert max(errs.values()) <= TOL, errs
 
 
 def test_c3_front_end_fullsize_sampled_patches(rn):

@@ -677,3 +677,63 @@ def test_patch_chunked_front_end_equals_whole_tensor_functions():
     pix = orc.patches(x, p)
     assert np.allclose(b, dtok[:, ls].sum(axis=(0, 1)), atol=1e-13)
     assert np.allclose(w[1, 2], np.einsum("bs,bsd->d", pix[:, 1, ls, 2], dtok[:, ls, 1, :]), atol=1e-13)
+
+
+class _LockstepGroup:
+    """Plain-Python stand-in for an all-reduce over T ranks run as T threads: every rank deposits its partial, a barrier,
+    every rank reads the sum (ranks added in rank order)."""
+
+    def __init__(self, T):
+        import threading
+        self.T, self.slots, self.bar = T, [None] * T, threading.Barrier(T)
+
+    def allreduce(self, rank):
+        def f(part):
+            self.slots[rank] = part
+            self.bar.wait()
+            total = sum(self.slots[1:], self.slots[0])
+            self.bar.wait()
+            return total
+        return f
+
+
+@pytest.mark.parametrize("T", [1, 2, 4])
+@pytest.mark.parametrize("qk_norm", [False, True])
+def test_rank_local_program_equals_unsharded_block(T, qk_norm):
+    """RANK (oracle rank_block_fwd / rank_block_bwd: one rank's program between the four all-reduces)
+    run for all T ranks in lock step = the unsharded BLK oracle: y, dx, replicated-parameter gradients identical on every
+    rank, shard gradients = the column / row slices of the unsharded gradients, partials sum to the combined products."""
+    import threading
+    B, N, D, h, F = 2, 6, 16, 4, 32
+    P = rand_block_params(D, F)
+    if qk_norm:
+        dh = D // h
+        P.update(qn_g=1 + 0.1 * rnd(dh), qn_b=0.1 * rnd(dh), kn_g=1 + 0.1 * rnd(dh), kn_b=0.1 * rnd(dh))
+    x, dy = rnd(B, N, D), rnd(B, N, D)
+    y, cache = orc.block_fwd(x, P, h, 1e-5)
+    dx, G = orc.block_bwd(dy, P, cache)
+    shards = syn.shard_block_params(P, h, T)
+    grp = _LockstepGroup(T)
+    res = [None] * T
+
+    def run(k):
+        yk, ck, pf = orc.rank_block_fwd(x, P, shards[k], h // T, grp.allreduce(k), 1e-5)
+        dxk, Gc, Gs, pb = orc.rank_block_bwd(dy, P, shards[k], ck, grp.allreduce(k))
+        res[k] = (yk, dxk, Gc, Gs, pf, pb)
+    ts = [threading.Thread(target=run, args=(k,)) for k in range(T)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    for k in range(T):
+        yk, dxk, Gc, Gs, pf, pb = res[k]
+        assert orc.rel_fro(yk, y) < 1e-13 and orc.rel_fro(dxk, dx) < 1e-12
+        for name in ("ln1_g", "ln1_b", "ln2_g", "ln2_b", "bproj", "bfc2"):
+            assert orc.rel_fro(Gc[name], G[name]) < 1e-12, name
+    Gu = syn.unshard_block_grads([r[3] for r in res], T)
+    for name in Gu:
+        assert orc.rel_fro(Gu[name], G[name]) < 1e-12, name
+    if qk_norm:      # shared by the heads: each rank holds the sum over ITS heads
+        for name in ("qn_g", "qn_b", "kn_g"):
+            assert orc.rel_fro(sum(r[2][name] for r in res), G[name]) < 1e-12, name
+    # what the collectives see: the partials add up to the unsharded products (Eq. 2 forward, Eq. 3 backward)
+    assert orc.rel_fro(sum(r[4]["proj"] for r in res), cache["O"] @ P["Wproj"]) < 1e-13
+    assert orc.rel_fro(sum(r[4]["fc2"] for r in res), cache["g"] @ P["Wfc2"]) < 1e-13

@@ -206,6 +206,30 @@ size_t orbit_head_loss_workspace_bytes(const orbit_head_desc* d);
 size_t orbit_head_loss_bwd_workspace_bytes(const orbit_head_desc* d);
 size_t orbit_head_loss_saved_bytes(const orbit_head_desc* d);
 
+/* ---- dynamic gradient scaling and fp32 gradient accumulation ("the PyTorch dynamic
+ * gradient scaling mechanism [24] ... detects the value range of the computed gradient magnitude ... scale the gradient
+ * magnitudes to the proper value range representable in BFLOAT16, and then reverse the scaling during the parameters
+ * update").  The caller scales its loss gradient (dy) by S; after the backward calls:
+ *   orbit_grads_unscale_check: every element of the n gradient tensors (device pointers grads[i], counts[i] elements of
+ *     `dtype`) is multiplied in place by 1 / *scale (fp32 arithmetic, one rounding to `dtype`); *found_inf is set to 1.0f
+ *     when any gradient element is Inf / NaN (it is never cleared here: zero it once per step).  scale == NULL means S = 1
+ *     (check only).
+ *   orbit_grads_accumulate: acc[i][j] += grads[i][j] / *scale in fp32 (gradient accumulation across micro-steps without
+ *     the per-step rounding of the `dtype` gradients); found_inf nullable.
+ *   orbit_grad_scale_update: the scale schedule of [24]: if *found_inf != 0: S <- S * backoff_factor, tracker <- 0 (the
+ *     caller skips the parameter update); else tracker += 1 and, when it reaches growth_interval, S <- S * growth_factor,
+ *     tracker <- 0.  The paper names no values; the caller supplies them (ORBIT_ERR_SHAPE unless growth_factor > 1,
+ *     0 < backoff_factor < 1, growth_interval >= 1).
+ * grads / acc / counts are HOST arrays of n entries; the tensors, scale, found_inf and growth_tracker are DEVICE memory
+ * (no host synchronisation).  Tensors must be 16-byte aligned; counts[i] == 0 entries are skipped.  No optimizer is
+ * part of this library (the paper names none). */
+int orbit_grads_unscale_check(int n, void* const* grads, const size_t* counts, orbit_dtype dtype, const float* scale,
+                              float* found_inf, void* stream);
+int orbit_grads_accumulate(int n, const void* const* grads, float* const* acc, const size_t* counts, orbit_dtype dtype,
+                           const float* scale /* nullable */, float* found_inf /* nullable */, void* stream);
+int orbit_grad_scale_update(float* scale, int* growth_tracker, const float* found_inf, float growth_factor,
+                            float backoff_factor, int growth_interval, void* stream);
+
 /* ---- bare Eq. (2)/(3) chain, used by the fp32 shard-recombination check (R15):
  *   y = sum_k (x A_k) B_k   with A_k [d, n/T] column shards and B_k [n/T, e] row shards;
  *   dx = sum_k (dy B_k^T) A_k^T.  x [m,d], y [m,e]; fp32 partials combined on device.

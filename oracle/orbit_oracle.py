@@ -21,6 +21,9 @@ float64 autograd with F.layer_norm on the per-head q / k, finite differences, lo
 sqrt(d_h) for gamma = 1, beta = 0, invariance to rescaling the pre-norm queries (eps = 0); head + wMSE: torch
 float64 autograd (layer_norm, linear, permute, weighted mean), finite differences, unpatchify = inverse of
 `patches`, weights with mean 1 / equator-symmetric / uniform weights = plain MSE, sum_i cos closed form.
+Gradient scaling (grads_unscale_check / grads_accumulate / grad_scale_update): torch's own CPU implementation of the
+mechanism the paper cites (torch._amp_foreach_non_finite_check_and_unscale_, torch._amp_update_scale_), exact
+power-of-two closed forms, and a hand-worked schedule trace (tests/golden/grad_scale_trace.json).
 Rank-local Hybrid-STOP program (rank_block_fwd / rank_block_bwd): world-size-2 gloo run with a real all-reduce
 = the unsharded block (tests/test_multiproc.py), and a plain-sum run for T in {1, 2, 4} (tests/test_oracle_pins.py).
 Parity unpinned: none.
@@ -712,6 +715,44 @@ def step(x, emb, agg, blocks, target, p, heads, eps=1e-5, pos=None):
     out["dtok"], out["agg_grads"], out["dpos"] = dtok, Ga, dpos
     out["dWp"], out["dbp"] = tokenize_bwd(x, dtok, p)
     return out
+
+
+# ---------------------------------------------------------------------------------------------
+# SCALE -- dynamic gradient scaling and fp32 gradient accumulation ("we applied the PyTorch dynamic
+# gradient scaling mechanism [24] ... detects the value range of the computed gradient magnitude ... scale the gradient
+# magnitudes to the proper value range representable in BFLOAT16, and then reverse the scaling during the parameters
+# update").  The loss gradient is multiplied by S before the backward pass; afterwards:
+# ---------------------------------------------------------------------------------------------
+def grads_unscale_check(grads, scale):
+    """Reverse the scaling: g / S for every gradient tensor, and detect overflow: found_inf = 1.0 iff any gradient
+    element is Inf or NaN (as [24] does: the test is on the computed gradient, before it is unscaled; the step is then
+    skipped).  Returns (list of unscaled fp64 arrays, found_inf)."""
+    inv = 1.0 / float(scale)
+    found = 0.0
+    for g in grads:
+        if not np.isfinite(_f64(g)).all():
+            found = 1.0
+    with np.errstate(invalid="ignore"):
+        out = [_f64(g) * inv for g in grads]
+    return out, found
+
+
+def grads_accumulate(acc, grads, scale=1.0):
+    """Gradient accumulation across micro-steps: acc_i + g_i / S, per tensor (new list)."""
+    inv = 1.0 / float(scale)
+    return [_f64(a) + _f64(g) * inv for a, g in zip(acc, grads)]
+
+
+def grad_scale_update(scale, tracker, found_inf, growth_factor, backoff_factor, growth_interval):
+    """The scale schedule of [24]: on overflow S <- S * backoff_factor and the count of clean steps restarts; otherwise
+    the count grows by one and, when it reaches growth_interval, S <- S * growth_factor and the count restarts.
+    Returns (scale, tracker).  The paper gives no values for the three constants: they are arguments."""
+    if found_inf != 0.0:
+        return float(scale) * backoff_factor, 0
+    tracker = int(tracker) + 1
+    if tracker >= growth_interval:
+        return float(scale) * growth_factor, 0
+    return float(scale), tracker
 
 
 def rel_fro(got, ref):

@@ -114,6 +114,9 @@ _proto("orbit_rank_bwd_attn", C.c_int, [_bd, _vp, _bp, _vp, _bg, _vp, _vp, _sz, 
 _proto("orbit_rank_bwd_out", C.c_int, [_bd, _bp, _vp, _bg, _vp, _vp, _vp, _sz, _vp])
 _proto("orbit_rank_saved_bytes", _sz, [_bd])
 _proto("orbit_rank_bwd_workspace_bytes", _sz, [_bd])
+_proto("orbit_grads_unscale_check", C.c_int, [C.c_int, C.POINTER(_vp), C.POINTER(_sz), C.c_int, _vp, _vp, _vp])
+_proto("orbit_grads_accumulate", C.c_int, [C.c_int, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_sz), C.c_int, _vp, _vp, _vp])
+_proto("orbit_grad_scale_update", C.c_int, [_vp, _vp, _vp, C.c_float, C.c_float, C.c_int, _vp])
 HAS_DEBUG_SWITCH = hasattr(lib, "orbit_set_debug_force_simt")      # only the A/B build exports it (csrc/orbit_debug.h)
 if HAS_DEBUG_SWITCH:
     _proto("orbit_set_debug_force_simt", None, [C.c_int])
@@ -172,7 +175,8 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes",
            "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd", "orbit_debug_gemm_out",
            "orbit_rank_fwd_attn", "orbit_rank_fwd_mlp", "orbit_rank_fwd_out", "orbit_rank_bwd_mlp", "orbit_rank_bwd_attn",
-           "orbit_rank_bwd_out", "orbit_rank_saved_bytes", "orbit_rank_bwd_workspace_bytes"]
+           "orbit_rank_bwd_out", "orbit_rank_saved_bytes", "orbit_rank_bwd_workspace_bytes",
+           "orbit_grads_unscale_check", "orbit_grads_accumulate", "orbit_grad_scale_update"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -388,6 +392,28 @@ def orbit_rank_bwd_out(d, common, shard, saved, gcommon, gshard, part, dx, ws, s
     gs = _block_struct(orbit_block_grads, gcommon, [gshard])
     _check(lib.orbit_rank_bwd_out(C.byref(d), C.byref(ps), _ptr(saved), C.byref(gs), _ptr(part), _ptr(dx), _ptr(ws),
                                   ws.numel() * ws.element_size(), _stream(stream)), "orbit_rank_bwd_out")
+
+
+# ---- dynamic gradient scaling / fp32 accumulation: lists of gradient tensors of one dtype
+def _counts(ts):
+    return (_sz * len(ts))(*[t.numel() for t in ts])
+
+
+def orbit_grads_unscale_check(grads, dtype, scale, found_inf, stream=None):
+    """grads: list of device tensors of `dtype`, unscaled in place by 1 / scale[0]; found_inf[0] <- 1.0 on Inf / NaN."""
+    _check(lib.orbit_grads_unscale_check(len(grads), _ptr_array(grads), _counts(grads), DTYPES[dtype], _ptr(scale),
+                                         _ptr(found_inf), _stream(stream)), "orbit_grads_unscale_check")
+
+
+def orbit_grads_accumulate(grads, acc, dtype, scale=None, found_inf=None, stream=None):
+    """acc[i] (fp32) += grads[i] / scale[0]."""
+    _check(lib.orbit_grads_accumulate(len(grads), _ptr_array(grads), _ptr_array(acc), _counts(grads), DTYPES[dtype],
+                                      _ptr(scale), _ptr(found_inf), _stream(stream)), "orbit_grads_accumulate")
+
+
+def orbit_grad_scale_update(scale, growth_tracker, found_inf, growth_factor, backoff_factor, growth_interval, stream=None):
+    _check(lib.orbit_grad_scale_update(_ptr(scale), _ptr(growth_tracker), _ptr(found_inf), growth_factor, backoff_factor,
+                                       growth_interval, _stream(stream)), "orbit_grad_scale_update")
 
 
 def _ptr_array(ts):

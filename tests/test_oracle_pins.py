@@ -737,3 +737,47 @@ def test_rank_local_program_equals_unsharded_block(T, qk_norm):
     # what the collectives see: the partials add up to the unsharded products (Eq. 2 forward, Eq. 3 backward)
     assert orc.rel_fro(sum(r[4]["proj"] for r in res), cache["O"] @ P["Wproj"]) < 1e-13
     assert orc.rel_fro(sum(r[4]["fc2"] for r in res), cache["g"] @ P["Wfc2"]) < 1e-13
+
+
+# ------------------------------------------------------------------ dynamic gradient scaling -----
+def test_grad_scale_schedule_golden_trace_and_torch():
+    """grad_scale_update against the hand-worked trace (tests/golden/grad_scale_trace.json) and against torch's CPU
+    implementation of the mechanism the paper cites (torch._amp_update_scale_)."""
+    tr = json.load(open(os.path.join(GOLD, "grad_scale_trace.json")))
+    s, t = tr["scale0"], 0
+    ts, tt = torch.tensor([tr["scale0"]], dtype=torch.float32), torch.zeros(1, dtype=torch.int32)
+    for f, s_want, t_want in zip(tr["found_inf"], tr["scale_after"], tr["tracker_after"]):
+        s, t = orc.grad_scale_update(s, t, float(f), tr["growth_factor"], tr["backoff_factor"], tr["growth_interval"])
+        assert s == s_want and t == t_want
+        torch._amp_update_scale_(ts, tt, torch.tensor([float(f)]), tr["growth_factor"], tr["backoff_factor"], tr["growth_interval"])
+        assert float(ts) == s and int(tt) == t
+
+
+def test_grads_unscale_check_and_accumulate():
+    """Unscaling by a power of two is exact (= ldexp); overflow detection fires on Inf and NaN only; equals torch's
+    _amp_foreach_non_finite_check_and_unscale_ on CPU; accumulation of k micro-steps of g with scale S = k g / S."""
+    gs = [rnd(5, 7) * 1e3, rnd(11) * 1e-3, rnd(2, 3, 4)]
+    out, found = orc.grads_unscale_check(gs, 1024.0)
+    assert found == 0.0
+    for o, g in zip(out, gs):
+        assert np.array_equal(o, np.ldexp(g, -10))
+    tg = [torch.tensor(g, dtype=torch.float64) for g in gs]
+    tf = torch.zeros(1, dtype=torch.float32)
+    torch._amp_foreach_non_finite_check_and_unscale_(tg, tf, torch.tensor([1.0 / 1024.0], dtype=torch.float32))
+    assert float(tf) == 0.0
+    for o, g in zip(out, tg):
+        assert np.array_equal(o, g.numpy())
+    for bad in (np.inf, -np.inf, np.nan):
+        g2 = [g.copy() for g in gs]
+        g2[1][3] = bad
+        _, found = orc.grads_unscale_check(g2, 3.0)
+        assert found == 1.0
+        tg = [torch.tensor(g, dtype=torch.float64) for g in g2]
+        tf = torch.zeros(1, dtype=torch.float32)
+        torch._amp_foreach_non_finite_check_and_unscale_(tg, tf, torch.tensor([1.0 / 3.0], dtype=torch.float32))
+        assert float(tf) == 1.0
+    acc = [np.zeros_like(g) for g in gs]
+    for _ in range(4):
+        acc = orc.grads_accumulate(acc, gs, 8.0)
+    for a, g in zip(acc, gs):
+        assert np.allclose(a, 4 * g / 8.0, rtol=1e-15)

@@ -446,7 +446,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C5", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C5", choices=["C2", "C3", "C4", "C5", "P113", "P10B"],
+                    help="C2..C5: BASELINE.json configs (default C5, the one the metric is quoted on); P113 / P10B: one block "
+                         "of the paper's own 113B / 10B shapes (PAPER.md:140: d_h 192 / 256)")
     ap.add_argument("--front", default="fused", choices=["fused", "twocall"],
                     help="front end of C2/C3: orbit_embed_fused (pixel space, no tok tensor) or orbit_tokenize + "
                          "orbit_var_aggregate (tok materialised)")

@@ -47,7 +47,7 @@ typedef enum { ORBIT_F32 = 0, ORBIT_BF16 = 1 } orbit_dtype;
 /* flags of orbit_block_desc (any other bit returns ORBIT_ERR_UNSUPPORTED) */
 #define ORBIT_QK_NORM   1u   /* QK-LayerNorm (R9): LayerNorm over d_h of every head's q and k before the
                                 scaled dot product, gamma / beta in R^{d_h} shared by the heads (qn_g, qn_b, kn_g, kn_b of
-                                orbit_block_params); needs d_h in {32, 64, 128, 256} */
+                                orbit_block_params); needs d_h in {32, 64, 128, 192, 256} */
 #define ORBIT_RECOMPUTE 2u   /* activation checkpointing: orbit_block_fwd keeps only the block input in
                                 `saved`; orbit_block_bwd re-runs the forward into its workspace first.  Same results. */
 

@@ -87,7 +87,7 @@ int check_block(const orbit_block_desc* d) {
     return ORBIT_ERR_SHAPE;
   }
   if ((d->flags & ORBIT_QK_NORM) && !qknorm_supported(d->D / d->heads)) {
-    set_error("block: QK-LayerNorm needs d_h in {32, 64, 128, 256} (d_h = %d)", d->D / d->heads);
+    set_error("block: QK-LayerNorm needs d_h in {32, 64, 128, 192, 256} (d_h = %d)", d->D / d->heads);
     return ORBIT_ERR_SHAPE;
   }
   return ORBIT_OK;

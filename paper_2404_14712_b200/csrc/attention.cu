@@ -1,6 +1,8 @@
 // attention.cu -- dispatch between the attention kernels:
-//   tcgen05/TMEM flash kernels (attention_tc5.cu), forward and backward, for bf16, d_h in {64, 128}, N >= 128;
-//   mma.sync flash kernels (attention_tc.cu) otherwise for bf16 d_h in {64, 128}; fp32-FMA kernels else.
+//   tcgen05/TMEM flash kernels (attention_tc5.cu), forward and backward, for bf16, d_h in {64, 128, 192, 256} (192 and
+//   256 are the paper's own head widths), N >= 128;
+//   mma.sync flash kernels (attention_tc.cu) otherwise for bf16 d_h in {64, 128}; fp32-FMA kernels else (fp32 storage,
+//   other head widths, bf16 d_h 192 / 256 with N < 128).
 // orbit_set_debug_force_simt: 1 = fp32-FMA kernels everywhere, 3 = skip the tcgen05 attention (A/B comparison),
 // 4 = tcgen05 forward only (mma.sync backward).
 #include "common.cuh"

@@ -24,7 +24,7 @@
 namespace orbit {
 namespace {
 
-constexpr int BQ = 128, BKV = 128;
+constexpr int BQ = 128;
 constexpr int NTH = 320;   // forward: warp 0 TMA, warp 1 MMA issuer, warps 2..9 softmax (two per TMEM lane quarter, 64 key columns each)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
@@ -48,19 +48,28 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 
 template <int DH>
 struct Cfg {
+  // head widths up to 128 stream key / value tiles of 128 rows; 192 and 256 (the paper's 113B / 1B / 10B shapes,
+  // PAPER.md:140) stream 64-row tiles so that Q + the K / V rings + P still fit 227 KB and S (double buffered) + O fit
+  // the 512 TMEM columns (2 * 64 + 256)
+  static constexpr int BKV = DH <= 128 ? 128 : 64;
   static constexpr int NBLK = DH / 64;                  // 64-column blocks per tile row
-  static constexpr int TILE = 128 * DH * 2;             // bytes of a [128 x DH] bf16 tile
-  static constexpr int P_BYTES = 128 * BKV * 2;         // 32 KB
+  static constexpr int QBLK = 128 * 128;                // bytes of one 64-column block of the Q tile (128 rows)
+  static constexpr int KBLK = BKV * 128;                // ... of a K / V tile (BKV rows)
+  static constexpr int QTILE = 128 * DH * 2;            // bytes of the [128 x DH] bf16 query tile
+  static constexpr int TILE = BKV * DH * 2;             // bytes of a [BKV x DH] bf16 key / value tile
+  static constexpr int P_BYTES = 128 * BKV * 2;         // P tile: BKV / 64 blocks of [128 rows x 64 keys]
   // K and V stream through separate rings: a K stage is free as soon as S_j = Q K_j^T has been computed, a V stage
   // only after O += P_j V_j; with 3 + 2 stages the TMA round trip of K_{j+1} no longer sits between PV_{j-1} and S_{j+1}
   // (measured with clock64 stamps: the MMA thread waited ~2000 of 2750 cycles per tile for K/V with a shared 2-stage ring)
-  static constexpr int KST = 3, VST = 2;
-  static constexpr int SMEM = TILE /*Q*/ + (KST + VST) * TILE + P_BYTES + 256 /*alignment slack, see the kernel*/ + 256 + 2048 /*row-max exchange*/;
+  static constexpr int KST = DH == 256 ? 2 : 3, VST = DH == 192 ? 3 : 2;
+  static constexpr int SMEM = QTILE + (KST + VST) * TILE + P_BYTES + 256 /*alignment slack, see the kernel*/ + 256 + 2048 /*row-max exchange*/;
+  static_assert(SMEM <= 227 * 1024, "attention forward: shared memory budget");
+  static_assert(2 * BKV + DH <= 512, "attention forward: TMEM budget");
 };
 
 template <int DH>
 __global__ void __launch_bounds__(NTH, 1)
-attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float sl2) {
+attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_constant__ CUtensorMap tmKV, AttnArgs a, float sl2) {
   using C = Cfg<DH>;
   // the 128B-swizzled tiles need 1024-byte aligned shared addresses: the alignment is requested on the declaration
   // (dynamic shared memory starts at the window's 1 KB-aligned base when the kernel has no static shared memory) and
@@ -68,8 +77,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   if (base - ptx::smem_u32(smem_raw) > 256u) __trap();
-  constexpr int KST = C::KST, VST = C::VST;
-  const uint32_t sQ = base, sK0 = sQ + C::TILE, sV0 = sK0 + KST * C::TILE, sP = sV0 + VST * C::TILE, bar = sP + C::P_BYTES;
+  constexpr int KST = C::KST, VST = C::VST, BKV = C::BKV;
+  const uint32_t sQ = base, sK0 = sQ + C::QTILE, sV0 = sK0 + KST * C::TILE, sP = sV0 + VST * C::TILE, bar = sP + C::P_BYTES;
   auto sK = [&](int st) { return sK0 + st * C::TILE; };
   auto sV = [&](int st) { return sV0 + st * C::TILE; };
   const uint32_t q_full = bar, k_full0 = bar + 8, k_empty0 = k_full0 + 8 * KST, v_full0 = k_empty0 + 8 * KST,
@@ -83,7 +92,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   const int qc = a.q_off + h * DH, kc = a.k_off + h * DH, vc = a.v_off + h * DH;
 
   if (warp == 0 && lane == 0) {
-    ptx::prefetch_tmap(&tmQKV);
+    ptx::prefetch_tmap(&tmQKV); ptx::prefetch_tmap(&tmKV);
     ptx::mbar_init(q_full, 1);
     for (int i = 0; i < KST; i++) { ptx::mbar_init(k_full0 + 8 * i, 1); ptx::mbar_init(k_empty0 + 8 * i, 1); }
     for (int i = 0; i < VST; i++) { ptx::mbar_init(v_full0 + 8 * i, 1); ptx::mbar_init(v_empty0 + 8 * i, 1); }
@@ -98,19 +107,19 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
   ptx::tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
-  const uint32_t tS0 = tmem, tO = tmem + 256;
+  const uint32_t tS0 = tmem, tO = tmem + 2 * BKV;
 
   if (warp == 0) {
     if (lane == 0) {
-      ptx::mbar_expect_tx(q_full, C::TILE);
+      ptx::mbar_expect_tx(q_full, C::QTILE);
 #pragma unroll
-      for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sQ + bk * 16384, &tmQKV, q_full, qc + bk * 64, row0 + q0);
+      for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sQ + bk * C::QBLK, &tmQKV, q_full, qc + bk * 64, row0 + q0);
       auto load_k = [&](int j) {
         const int st = j % KST;
         ptx::mbar_wait(k_empty0 + 8 * st, ((j / KST) & 1) ^ 1);
         ptx::mbar_expect_tx(k_full0 + 8 * st, C::TILE);
 #pragma unroll
-        for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sK(st) + bk * 16384, &tmQKV, k_full0 + 8 * st, kc + bk * 64, row0 + j * BKV);
+        for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sK(st) + bk * C::KBLK, &tmKV, k_full0 + 8 * st, kc + bk * 64, row0 + j * BKV);
       };
       load_k(0);
       for (int j = 0; j < ntiles; j++) {                      // K runs one tile ahead of V
@@ -119,7 +128,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         ptx::mbar_wait(v_empty0 + 8 * st, ((j / VST) & 1) ^ 1);
         ptx::mbar_expect_tx(v_full0 + 8 * st, C::TILE);
 #pragma unroll
-        for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sV(st) + bk * 16384, &tmQKV, v_full0 + 8 * st, vc + bk * 64, row0 + j * BKV);
+        for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sV(st) + bk * C::KBLK, &tmKV, v_full0 + 8 * st, vc + bk * 64, row0 + j * BKV);
       }
     }
   } else if (warp == 1) {
@@ -135,8 +144,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         const uint64_t dK0 = ptx::make_smem_desc(sK(st), 16, 1024);
 #pragma unroll
         for (int ks = 0; ks < DH / 16; ks++) {
-          const uint32_t off = (ks >> 2) * 16384 + (ks & 3) * 32;
-          ptx::mma_f16_ss(tS0 + sb * 128, desc_adv(dQ0, off), desc_adv(dK0, off), idesc_s, ks != 0);
+          const uint32_t qoff = (ks >> 2) * C::QBLK + (ks & 3) * 32, koff = (ks >> 2) * C::KBLK + (ks & 3) * 32;
+          ptx::mma_f16_ss(tS0 + sb * BKV, desc_adv(dQ0, qoff), desc_adv(dK0, koff), idesc_s, ks != 0);
         }
         ptx::mma_commit(k_empty0 + 8 * st);          // K stage free once these MMAs have read it
         ptx::mma_commit(s_full0 + 8 * sb);
@@ -147,14 +156,14 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
         if (j + 1 < ntiles) issue_s(j + 1);
         const int st = j % VST;
         ptx::mbar_wait(v_full0 + 8 * st, (j / VST) & 1);
-        const uint64_t dV0 = ptx::make_smem_desc(sV(st), 16384, 1024);
+        const uint64_t dV0 = ptx::make_smem_desc(sV(st), C::KBLK, 1024);
 #pragma unroll
-        for (int hh = 0; hh < 2; hh++) {                      // the two 64-key halves of P are written by different warps
+        for (int hh = 0; hh < 2; hh++) {                      // the two key halves of P are written by different warps
           ptx::mbar_wait(p_full0 + 8 * hh, j & 1);
           ptx::tc_fence_after();
 #pragma unroll
-          for (int k4 = 0; k4 < 4; k4++) {
-            const int ks = hh * 4 + k4;
+          for (int k4 = 0; k4 < BKV / 32; k4++) {
+            const int ks = hh * (BKV / 32) + k4;
             const uint32_t aoff = (ks >> 2) * 16384 + (ks & 3) * 32;        // P: K-major, two 64-key blocks
             ptx::mma_f16_ss(tO, desc_adv(dP0, aoff), desc_adv(dV0, ks * 2048), idesc_o, (j | ks) != 0);
           }
@@ -181,9 +190,10 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
       const int sb = j & 1;
       ptx::mbar_wait(s_full0 + 8 * sb, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[64];
+      constexpr int HC = BKV / 2;                             // key columns of this warp
+      uint32_t s[HC];
 #pragma unroll
-      for (int c = 0; c < 2; c++) ptx::tmem_ld_32x32(tS0 + sb * 128 + half * 64 + c * 32 + lane_off, s + c * 32);
+      for (int c = 0; c < HC / 32; c++) ptx::tmem_ld_32x32(tS0 + sb * BKV + half * HC + c * 32 + lane_off, s + c * 32);
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();
@@ -191,14 +201,14 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
       float mx = -INFINITY;
       if ((j + 1) * BKV > N) {                               // last, ragged tile: mask keys >= N
 #pragma unroll
-        for (int c = 0; c < 64; c++) {
-          float v = (j * BKV + half * 64 + c < N) ? __uint_as_float(s[c]) : -INFINITY;
+        for (int c = 0; c < HC; c++) {
+          float v = (j * BKV + half * HC + c < N) ? __uint_as_float(s[c]) : -INFINITY;
           s[c] = __float_as_uint(v);
           mx = fmaxf(mx, v);
         }
       } else {
 #pragma unroll
-        for (int c = 0; c < 64; c++) mx = fmaxf(mx, __uint_as_float(s[c]));
+        for (int c = 0; c < HC; c++) mx = fmaxf(mx, __uint_as_float(s[c]));
       }
       const float mi = ceilf(mx * sl2);                                  // -inf when this half of a ragged tile is fully masked
       const uint32_t xm = xmax + (uint32_t)(sb * 256 + r) * 4;          // [parity][half][row] fp32 (no range limit on the logits)
@@ -237,7 +247,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
       m_used = m_new;
       float sum = 0.f;
 #pragma unroll
-      for (int c = 0; c < 8; c++) {                           // 8 keys = one 16-byte chunk of the P row
+      for (int c = 0; c < HC / 8; c++) {                      // 8 keys = one 16-byte chunk of the P row
         uint32_t pk[4];
 #pragma unroll
         for (int i = 0; i < 4; i++) {
@@ -247,7 +257,9 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
           __nv_bfloat162 v = __floats2bfloat162_rn(p0, p1);
           pk[i] = *reinterpret_cast<uint32_t*>(&v);
         }
-        const uint32_t addr = sP + half * 16384 + r * 128 + ((c ^ (r & 7)) << 4);
+        // BKV = 128: this warp owns the 64-key block `half`; BKV = 64: chunks 4 half .. 4 half + 3 of the one block
+        const uint32_t addr = BKV == 128 ? sP + half * 16384 + r * 128 + ((c ^ (r & 7)) << 4)
+                                         : sP + r * 128 + (((half * 4 + c) ^ (r & 7)) << 4);
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
       }
       l += sum;
@@ -302,20 +314,31 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, AttnArgs a, float
 // A streamed [64 x d_h] tile is used twice from the same bytes: as a K-major B operand (contraction over d_h)
 // and as an MN-major B operand (contraction over its 64 rows).
 // =====================================================================================================
-constexpr int BT = 64;
-constexpr int NTHB = 384;   // warp 0 TMA, warp 1 gradient MMAs, warps 2..9 softmax (two per TMEM lane quarter, 32 columns each), warp 10 dP MMAs, warp 11 S MMAs
+constexpr int NTHB = 384;   // warp 0 TMA, warp 1 gradient MMAs, warps 2..9 softmax (two per TMEM lane quarter, BT / 2 columns each), warp 10 dP MMAs, warp 11 S MMAs
 
 template <int DH>
 struct CfgB {
+  // streamed tile rows: 64 up to d_h = 128; 32 for d_h = 192 / 256 (PAPER.md:140 shapes) so that S / dP (double
+  // buffered, 4 BT columns) + the gradient accumulators fit the 512 TMEM columns and two stationary [128 x DH] tiles +
+  // the ring fit 227 KB.  d_h = 256: dK + dV alone would fill TMEM, so the dK/dV kernel computes one 128-column slice
+  // of both per CTA (grid z = NSPLIT; S^T and dP^T are recomputed per slice: 6 tile products instead of 4).
+  static constexpr int BT = DH <= 128 ? 64 : 32;
   static constexpr int NBLK = DH / 64;
+  static constexpr int BBLK = 128 * 128;          // bytes of one 64-column block of a stationary [128 x DH] tile
+  static constexpr int SBLK = BT * 128;           // ... of a streamed [BT x DH] tile
   static constexpr int BIG = 128 * DH * 2;        // stationary [128 x DH] tile
-  static constexpr int SMALL = BT * DH * 2;       // streamed [64 x DH] tile
-  static constexpr int PT = 128 * BT * 2;         // [128 x 64] bf16 operand tile written by the softmax threads
+  static constexpr int SMALL = BT * DH * 2;       // streamed [BT x DH] tile
+  static constexpr int PT = 128 * BT * 2;         // [128 x BT] bf16 operand tile written by the softmax threads (rows of 2 BT bytes:
+                                                  // 128B swizzle at BT = 64, 64B swizzle at BT = 32)
+  static constexpr int NSPLIT = DH == 256 ? 2 : 1;
+  static constexpr int DHO = DH / NSPLIT;         // dK / dV columns per CTA
   // stages of the streamed (two-tile) ring: hide the TMA round trip.  The operand tiles written by the softmax warps
   // (P^T, dS^T resp. dS) are double buffered so that tile j+1 is written while the MMAs of tile j still read tile j.
-  static constexpr int NST_DKV = 3, NST_DQ = 4;
+  static constexpr int NST_DKV = DH == 256 ? 2 : 3, NST_DQ = DH == 256 ? 2 : 4;
   static constexpr int SMEM_DKV = 2 * BIG + 2 * NST_DKV * SMALL + 4 * PT + 1024 /*stats*/ + 1024 + 256;
   static constexpr int SMEM_DQ = 2 * BIG + 2 * NST_DQ * SMALL + 2 * PT + 1024 + 256;
+  static_assert(SMEM_DKV <= 227 * 1024 && SMEM_DQ <= 227 * 1024, "attention backward: shared memory budget");
+  static_assert(4 * BT + 2 * DHO <= 512 && 4 * BT + DH <= 512, "attention backward: TMEM budget");
 };
 
 // write 64 bf16 (this thread's row r) into a K-major [128 x 64] operand tile (128-byte rows, 128B swizzle)
@@ -345,6 +368,34 @@ __device__ __forceinline__ void write_row32(uint32_t tile, int r, const float* v
     const uint32_t addr = tile + r * 128 + (((half * 4 + c) ^ (r & 7)) << 4);
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
   }
+}
+// 16 of the 32 columns of a [128 x 32] K-major operand tile with 64-byte rows (64B swizzle: 16-byte chunk index ^ ((row >> 1) & 3))
+__device__ __forceinline__ void write_row16_sw64(uint32_t tile, int r, const float* v, int half) {
+#pragma unroll
+  for (int c = 0; c < 2; c++) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      __nv_bfloat162 t2 = __floats2bfloat162_rn(v[c * 8 + 2 * i], v[c * 8 + 2 * i + 1]);
+      pk[i] = *reinterpret_cast<uint32_t*>(&t2);
+    }
+    const uint32_t addr = tile + r * 64 + (((half * 2 + c) ^ ((r >> 1) & 3)) << 4);
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+  }
+}
+// this warp's CW = BT / 2 columns of a row into the [128 x BT] operand tile
+template <int CW>
+__device__ __forceinline__ void write_row_half(uint32_t tile, int r, const float* v, int half) {
+  if (CW == 32) write_row32(tile, r, v, half); else write_row16_sw64(tile, r, v, half);
+}
+template <int CW>
+__device__ __forceinline__ void tmem_ld_cw(uint32_t taddr, uint32_t* v) {
+  if (CW == 32) ptx::tmem_ld_32x32(taddr, v); else ptx::tmem_ld_32x16(taddr, v);
+}
+// K-major descriptor of a [128 x BT] operand tile
+template <int BT>
+__device__ __forceinline__ uint64_t optile_desc(uint32_t saddr) {
+  return BT == 64 ? ptx::make_smem_desc(saddr, 16, 1024) : ptx::make_smem_desc_sw64(saddr, 16, 512);
 }
 // TMEM accumulator row (DH fp32 columns of this thread's lane) * scale -> bf16 -> global row
 template <int DH>
@@ -376,13 +427,15 @@ __global__ void __launch_bounds__(NTHB, 1)
 attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
                         const __grid_constant__ CUtensorMap tmdO, AttnArgs a, float scale, float sl2) {
   using C = CfgB<DH>;
+  constexpr int BT = C::BT, CW = BT / 2, DHO = C::DHO;       // streamed rows; columns per softmax warp; dK / dV columns of this CTA
+  const int slice = blockIdx.z;                              // which DHO-column slice of dK / dV (d_h = 256: two)
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sK = base, sV = sK + C::BIG, sRing = sV + C::BIG, sPt0 = sRing + 2 * C::NST_DKV * C::SMALL,
                  sStat = sPt0 + 4 * C::PT, bar = sStat + 1024;
   auto sQ = [&](int st) { return sRing + st * 2 * C::SMALL; };
   auto sdO = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
-  float* stat = reinterpret_cast<float*>(smem_raw + (sStat - ptx::smem_u32(smem_raw)));   // [2][2][64]
+  float* stat = reinterpret_cast<float*>(smem_raw + (sStat - ptx::smem_u32(smem_raw)));   // [2][2][BT]
   constexpr int NST = C::NST_DKV;
   const uint32_t kv_full = bar, qdo_full0 = bar + 8, qdo_empty0 = qdo_full0 + 8 * NST, st_full0 = qdo_empty0 + 8 * NST,
                  st_empty0 = st_full0 + 16, p_full0 = st_empty0 + 16, p_done0 = p_full0 + 16, tmem_slot = p_done0 + 16;
@@ -407,15 +460,15 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
   ptx::tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
-  const uint32_t tSt = tmem, tdPt = tmem + 128, tdV = tmem + 256, tdK = tmem + 256 + DH;
+  const uint32_t tSt = tmem, tdPt = tmem + 2 * BT, tdV = tmem + 4 * BT, tdK = tdV + DHO;
 
   if (warp == 0) {
     if (lane == 0) {
       ptx::mbar_expect_tx(kv_full, 2 * C::BIG);
 #pragma unroll
       for (int bk = 0; bk < C::NBLK; bk++) {
-        ptx::tma_load_2d(sK + bk * 16384, &tmBig, kv_full, kc + bk * 64, row0 + k0);
-        ptx::tma_load_2d(sV + bk * 16384, &tmBig, kv_full, vc + bk * 64, row0 + k0);
+        ptx::tma_load_2d(sK + bk * C::BBLK, &tmBig, kv_full, kc + bk * 64, row0 + k0);
+        ptx::tma_load_2d(sV + bk * C::BBLK, &tmBig, kv_full, vc + bk * 64, row0 + k0);
       }
       for (int j = 0; j < ntiles; j++) {
         const int st = j % NST;
@@ -423,15 +476,15 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         ptx::mbar_expect_tx(qdo_full0 + 8 * st, 2 * C::SMALL);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) {
-          ptx::tma_load_2d(sQ(st) + bk * 8192, &tmSmall, qdo_full0 + 8 * st, qc + bk * 64, row0 + j * BT);
-          ptx::tma_load_2d(sdO(st) + bk * 8192, &tmdO, qdo_full0 + 8 * st, h * DH + bk * 64, row0 + j * BT);
+          ptx::tma_load_2d(sQ(st) + bk * C::SBLK, &tmSmall, qdo_full0 + 8 * st, qc + bk * 64, row0 + j * BT);
+          ptx::tma_load_2d(sdO(st) + bk * C::SBLK, &tmdO, qdo_full0 + 8 * st, h * DH + bk * 64, row0 + j * BT);
         }
       }
     }
   } else if (warp == 1 || warp >= NTHB / 32 - 2) {   // warp 1: gradient MMAs; last warp: S^T / dP^T MMAs (issue-bound otherwise)
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
-      constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
+      constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DHO, 0, 1);
       auto issue_s = [&](int j) {
         const int st = j % NST, tb = j & 1;
         ptx::mbar_wait(qdo_full0 + 8 * st, (j / NST) & 1);
@@ -442,13 +495,13 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         if (warp == NTHB / 32 - 1) {
 #pragma unroll
           for (int ks = 0; ks < DH / 16; ks++) {
-            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            const uint32_t ob = (ks >> 2) * C::BBLK + (ks & 3) * 32, os = (ks >> 2) * C::SBLK + (ks & 3) * 32;
             ptx::mma_f16_ss(tSt + tb * BT, desc_adv(dK0, ob), desc_adv(dQs, os), idesc_s, ks != 0);
           }
         } else {
 #pragma unroll
           for (int ks = 0; ks < DH / 16; ks++) {
-            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            const uint32_t ob = (ks >> 2) * C::BBLK + (ks & 3) * 32, os = (ks >> 2) * C::SBLK + (ks & 3) * 32;
             ptx::mma_f16_ss(tdPt + tb * BT, desc_adv(dV0, ob), desc_adv(dOs, os), idesc_s, ks != 0);
           }
         }
@@ -465,8 +518,10 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
         ptx::tc_fence_after();
         const int st = j % NST;
-        const uint64_t dPt = ptx::make_smem_desc(sPt, 16, 1024), dSt = ptx::make_smem_desc(sdSt, 16, 1024);
-        const uint64_t dOm = ptx::make_smem_desc(sdO(st), 8192, 1024), dQm = ptx::make_smem_desc(sQ(st), 8192, 1024);
+        const uint64_t dPt = optile_desc<BT>(sPt), dSt = optile_desc<BT>(sdSt);
+        // streamed tiles as MN-major B operands: this CTA's DHO columns start (slice * DHO / 64) blocks in
+        const uint32_t so = slice * (DHO / 64) * C::SBLK;
+        const uint64_t dOm = ptx::make_smem_desc(sdO(st) + so, C::SBLK, 1024), dQm = ptx::make_smem_desc(sQ(st) + so, C::SBLK, 1024);
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dV += P^T dO_j   (contraction over the tile's 64 queries)
           ptx::mma_f16_ss(tdV, desc_adv(dPt, ks * 32), desc_adv(dOm, ks * 2048), idesc_g, (j | ks) != 0);
@@ -478,47 +533,47 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
       }
     }
   } else {
-    const int quarter = warp & 3, half = (warp - 2) >> 2;     // this warp: 32 key rows x 32 of the tile's 64 query columns
+    const int quarter = warp & 3, half = (warp - 2) >> 2;     // this warp: 32 key rows x CW of the tile's BT query columns
     const int r = quarter * 32 + lane;                       // key row within the CTA tile = TMEM lane
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     const int gi = threadIdx.x - 64;                         // 0..255: the first 128 load the statistics
     auto load_stat = [&](int j) -> float {
-      const int q = j * BT + (gi & 63);
-      if (gi >= 128 || j >= ntiles || q >= N) return 0.f;
-      return (gi >> 6) ? a.delta[(size_t)bh * N + q] : a.lse[(size_t)bh * N + q] * LOG2E;
+      const int q = j * BT + (gi % BT);
+      if (gi >= 2 * BT || j >= ntiles || q >= N) return 0.f;
+      return (gi / BT) ? a.delta[(size_t)bh * N + q] : a.lse[(size_t)bh * N + q] * LOG2E;
     };
     float nxt = load_stat(0);
     for (int j = 0; j < ntiles; j++) {
       const int st = j & 1;
-      if (gi < 128) stat[st * 128 + gi] = nxt;               // [st][0][c] = lse2, [st][1][c] = delta
+      if (gi < 2 * BT) stat[st * 2 * BT + gi] = nxt;         // [st][0][c] = lse2, [st][1][c] = delta
       named_bar_sync(1, 256);
       nxt = load_stat(j + 1);
-      const float* lse2 = stat + st * 128 + half * 32;
-      const float* dl = lse2 + 64;
+      const float* lse2 = stat + st * 2 * BT + half * CW;
+      const float* dl = lse2 + BT;
       ptx::mbar_wait(st_full0 + 8 * st, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[32], dp[32];
-      ptx::tmem_ld_32x32(tSt + st * BT + half * 32 + lane_off, s);
-      ptx::tmem_ld_32x32(tdPt + st * BT + half * 32 + lane_off, dp);
+      uint32_t s[CW], dp[CW];
+      tmem_ld_cw<CW>(tSt + st * BT + half * CW + lane_off, s);
+      tmem_ld_cw<CW>(tdPt + st * BT + half * CW + lane_off, dp);
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(st_empty0 + 8 * st);
-      float p[32];
-      const int nvalid = N - j * BT - half * 32;             // queries (columns) >= N are masked
-      if (nvalid >= 32) {                                   // masking only in the ragged last tile (warp-uniform branch)
+      float p[CW];
+      const int nvalid = N - j * BT - half * CW;             // queries (columns) >= N are masked
+      if (nvalid >= CW) {                                   // masking only in the ragged last tile (warp-uniform branch)
 #pragma unroll
-        for (int c = 0; c < 32; c++) p[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]);
+        for (int c = 0; c < CW; c++) p[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]);
       } else {
 #pragma unroll
-        for (int c = 0; c < 32; c++) p[c] = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]) : 0.f;
+        for (int c = 0; c < CW; c++) p[c] = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]) : 0.f;
       }
       const uint32_t sPt = sPt0 + st * 2 * C::PT, sdSt = sPt + C::PT;
       if (j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);   // this buffer's P^T / dS^T tiles are free again
-      write_row32(sPt, r, p, half);
+      write_row_half<CW>(sPt, r, p, half);
 #pragma unroll
-      for (int c = 0; c < 32; c++) p[c] *= __uint_as_float(dp[c]) - dl[c];
-      write_row32(sdSt, r, p, half);
+      for (int c = 0; c < CW; c++) p[c] *= __uint_as_float(dp[c]) - dl[c];
+      write_row_half<CW>(sdSt, r, p, half);
       ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
@@ -527,9 +582,9 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
     ptx::mbar_wait(p_done0 + 8 * ((ntiles - 1) & 1), ((ntiles - 1) >> 1) & 1);
     ptx::tc_fence_after();
     const int krow = k0 + r;
-    bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld + half * (DH / 2);
-    store_acc_row<DH / 2>(tdV + half * (DH / 2) + lane_off, out + vc, 1.f, krow < N);
-    store_acc_row<DH / 2>(tdK + half * (DH / 2) + lane_off, out + kc, scale, krow < N);
+    bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld + slice * DHO + half * (DHO / 2);
+    store_acc_row<DHO / 2>(tdV + half * (DHO / 2) + lane_off, out + vc, 1.f, krow < N);
+    store_acc_row<DHO / 2>(tdK + half * (DHO / 2) + lane_off, out + kc, scale, krow < N);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -542,6 +597,7 @@ __global__ void __launch_bounds__(NTHB, 1)
 attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
                        const __grid_constant__ CUtensorMap tmdOBig, AttnArgs a, float scale, float sl2) {
   using C = CfgB<DH>;
+  constexpr int BT = C::BT, CW = BT / 2;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = base, sdO = sQ + C::BIG, sRing = sdO + C::BIG, sdS0 = sRing + 2 * C::NST_DQ * C::SMALL, bar = sdS0 + 2 * C::PT;
@@ -571,15 +627,15 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   ptx::tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
-  const uint32_t tS = tmem, tdP = tmem + 128, tdQ = tmem + 256;
+  const uint32_t tS = tmem, tdP = tmem + 2 * BT, tdQ = tmem + 4 * BT;
 
   if (warp == 0) {
     if (lane == 0) {
       ptx::mbar_expect_tx(q_full, 2 * C::BIG);
 #pragma unroll
       for (int bk = 0; bk < C::NBLK; bk++) {
-        ptx::tma_load_2d(sQ + bk * 16384, &tmBig, q_full, qc + bk * 64, row0 + q0);
-        ptx::tma_load_2d(sdO + bk * 16384, &tmdOBig, q_full, h * DH + bk * 64, row0 + q0);
+        ptx::tma_load_2d(sQ + bk * C::BBLK, &tmBig, q_full, qc + bk * 64, row0 + q0);
+        ptx::tma_load_2d(sdO + bk * C::BBLK, &tmdOBig, q_full, h * DH + bk * 64, row0 + q0);
       }
       for (int j = 0; j < ntiles; j++) {
         const int st = j % NST;
@@ -587,8 +643,8 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::mbar_expect_tx(kv_full0 + 8 * st, 2 * C::SMALL);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) {
-          ptx::tma_load_2d(sK(st) + bk * 8192, &tmSmall, kv_full0 + 8 * st, kc + bk * 64, row0 + j * BT);
-          ptx::tma_load_2d(sV(st) + bk * 8192, &tmSmall, kv_full0 + 8 * st, vc + bk * 64, row0 + j * BT);
+          ptx::tma_load_2d(sK(st) + bk * C::SBLK, &tmSmall, kv_full0 + 8 * st, kc + bk * 64, row0 + j * BT);
+          ptx::tma_load_2d(sV(st) + bk * C::SBLK, &tmSmall, kv_full0 + 8 * st, vc + bk * 64, row0 + j * BT);
         }
       }
     }
@@ -606,13 +662,13 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         if (warp == NTHB / 32 - 1) {
 #pragma unroll
           for (int ks = 0; ks < DH / 16; ks++) {
-            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            const uint32_t ob = (ks >> 2) * C::BBLK + (ks & 3) * 32, os = (ks >> 2) * C::SBLK + (ks & 3) * 32;
             ptx::mma_f16_ss(tS + tb * BT, desc_adv(dQ0, ob), desc_adv(dKs, os), idesc_s, ks != 0);
           }
         } else {
 #pragma unroll
           for (int ks = 0; ks < DH / 16; ks++) {
-            const uint32_t ob = (ks >> 2) * 16384 + (ks & 3) * 32, os = (ks >> 2) * 8192 + (ks & 3) * 32;
+            const uint32_t ob = (ks >> 2) * C::BBLK + (ks & 3) * 32, os = (ks >> 2) * C::SBLK + (ks & 3) * 32;
             ptx::mma_f16_ss(tdP + tb * BT, desc_adv(dO0, ob), desc_adv(dVs, os), idesc_s, ks != 0);
           }
         }
@@ -629,7 +685,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
         ptx::tc_fence_after();
         const int st = j % NST;
-        const uint64_t dSd = ptx::make_smem_desc(sdS, 16, 1024), dKm = ptx::make_smem_desc(sK(st), 8192, 1024);
+        const uint64_t dSd = optile_desc<BT>(sdS), dKm = ptx::make_smem_desc(sK(st), C::SBLK, 1024);
 #pragma unroll
         for (int ks = 0; ks < BT / 16; ks++)      // dQ += dS K_j   (contraction over the tile's 64 keys)
           ptx::mma_f16_ss(tdQ, desc_adv(dSd, ks * 32), desc_adv(dKm, ks * 2048), idesc_g, (j | ks) != 0);
@@ -638,7 +694,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
       }
     }
   } else {
-    const int quarter = warp & 3, half = (warp - 2) >> 2;     // 32 query rows x 32 of the tile's 64 key columns
+    const int quarter = warp & 3, half = (warp - 2) >> 2;     // 32 query rows x CW of the tile's BT key columns
     const int r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     const int qrow = q0 + r;
@@ -648,27 +704,27 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
       const int st = j & 1;
       ptx::mbar_wait(s_full0 + 8 * st, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[32], dp[32];
-      ptx::tmem_ld_32x32(tS + st * BT + half * 32 + lane_off, s);
-      ptx::tmem_ld_32x32(tdP + st * BT + half * 32 + lane_off, dp);
+      uint32_t s[CW], dp[CW];
+      tmem_ld_cw<CW>(tS + st * BT + half * CW + lane_off, s);
+      tmem_ld_cw<CW>(tdP + st * BT + half * CW + lane_off, dp);
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
-      float ds[32];
-      const int nvalid = N - j * BT - half * 32;             // keys (columns) >= N are masked
-      if (nvalid >= 32) {                                   // masking only in the ragged last tile (warp-uniform branch)
+      float ds[CW];
+      const int nvalid = N - j * BT - half * CW;             // keys (columns) >= N are masked
+      if (nvalid >= CW) {                                   // masking only in the ragged last tile (warp-uniform branch)
 #pragma unroll
-        for (int c = 0; c < 32; c++) ds[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) * (__uint_as_float(dp[c]) - dl);
+        for (int c = 0; c < CW; c++) ds[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) * (__uint_as_float(dp[c]) - dl);
       } else {
 #pragma unroll
-        for (int c = 0; c < 32; c++) {
+        for (int c = 0; c < CW; c++) {
           const float p = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) : 0.f;
           ds[c] = p * (__uint_as_float(dp[c]) - dl);
         }
       }
       if (j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
-      write_row32(sdS0 + st * C::PT, r, ds, half);
+      write_row_half<CW>(sdS0 + st * C::PT, r, ds, half);
       ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
@@ -718,25 +774,6 @@ EncodeTiledFn get_encode5() {
   return fn;
 }
 
-template <int DH>
-int launch_fwd5(const AttnArgs& a, cudaStream_t s) {
-  EncodeTiledFn enc = get_encode5();
-  if (!enc) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
-  CUtensorMap tm;
-  cuuint64_t dims[2] = {(cuuint64_t)a.ld, (cuuint64_t)a.B * a.N};
-  cuuint64_t strides[1] = {(cuuint64_t)a.ld * 2};
-  cuuint32_t box[2] = {64, 128};
-  cuuint32_t es[2] = {1, 1};
-  CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(a.qkv), dims, strides, box, es,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) { set_error("attention: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
-  ORBIT_SMEM_ATTR(attn_fwd_tc5_kernel<DH>, Cfg<DH>::SMEM);
-  dim3 grid(cdiv(a.N, BQ), a.B * a.heads);
-  attn_fwd_tc5_kernel<DH><<<grid, NTH, Cfg<DH>::SMEM, s>>>(tm, a, LOG2E / sqrtf((float)DH));
-  ORBIT_LAUNCH_CHECK();
-  return ORBIT_OK;
-}
 int make_map5(CUtensorMap* tm, const void* basep, long long ld, long long rows, int box_rows) {
   EncodeTiledFn enc = get_encode5();
   if (!enc) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
@@ -752,30 +789,50 @@ int make_map5(CUtensorMap* tm, const void* basep, long long ld, long long rows, 
 }
 
 template <int DH>
+int launch_fwd5(const AttnArgs& a, cudaStream_t s) {
+  const long long rows = (long long)a.B * a.N;
+  CUtensorMap tmQ, tmKV;                                   // boxes of 64 columns x 128 (query) / Cfg::BKV (key, value) rows
+  ORBIT_TRY(make_map5(&tmQ, a.qkv, a.ld, rows, 128));
+  ORBIT_TRY(make_map5(&tmKV, a.qkv, a.ld, rows, Cfg<DH>::BKV));
+  ORBIT_SMEM_ATTR(attn_fwd_tc5_kernel<DH>, Cfg<DH>::SMEM);
+  dim3 grid(cdiv(a.N, BQ), a.B * a.heads);
+  attn_fwd_tc5_kernel<DH><<<grid, NTH, Cfg<DH>::SMEM, s>>>(tmQ, tmKV, a, LOG2E / sqrtf((float)DH));
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+template <int DH>
 int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
+  using C = CfgB<DH>;
   const long long rows = (long long)a.B * a.N;
   CUtensorMap tmBig, tmSmall, tmdOBig, tmdOSmall;
   ORBIT_TRY(make_map5(&tmBig, a.qkv, a.ld, rows, 128));
-  ORBIT_TRY(make_map5(&tmSmall, a.qkv, a.ld, rows, 64));
+  ORBIT_TRY(make_map5(&tmSmall, a.qkv, a.ld, rows, C::BT));
   ORBIT_TRY(make_map5(&tmdOBig, a.dO, a.lddo, rows, 128));
-  ORBIT_TRY(make_map5(&tmdOSmall, a.dO, a.lddo, rows, 64));
-  ORBIT_SMEM_ATTR(attn_bwd_dkv_tc5_kernel<DH>, CfgB<DH>::SMEM_DKV);
-  ORBIT_SMEM_ATTR(attn_bwd_dq_tc5_kernel<DH>, CfgB<DH>::SMEM_DQ);
+  ORBIT_TRY(make_map5(&tmdOSmall, a.dO, a.lddo, rows, C::BT));
+  ORBIT_SMEM_ATTR(attn_bwd_dkv_tc5_kernel<DH>, C::SMEM_DKV);
+  ORBIT_SMEM_ATTR(attn_bwd_dq_tc5_kernel<DH>, C::SMEM_DQ);
   const int total_w = a.B * a.heads * a.N;
   attn_delta5_kernel<<<cdiv((long long)total_w * 32, 256), 256, 0, s>>>(a);
   ORBIT_LAUNCH_CHECK();
   dim3 grid(cdiv(a.N, 128), a.B * a.heads);
   const float scale = 1.0f / sqrtf((float)DH);
-  attn_bwd_dq_tc5_kernel<DH><<<grid, NTHB, CfgB<DH>::SMEM_DQ, s>>>(tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E);
+  attn_bwd_dq_tc5_kernel<DH><<<grid, NTHB, C::SMEM_DQ, s>>>(tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E);
   ORBIT_LAUNCH_CHECK();
-  attn_bwd_dkv_tc5_kernel<DH><<<grid, NTHB, CfgB<DH>::SMEM_DKV, s>>>(tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E);
+  dim3 grid_kv(cdiv(a.N, 128), a.B * a.heads, C::NSPLIT);
+  attn_bwd_dkv_tc5_kernel<DH><<<grid_kv, NTHB, C::SMEM_DKV, s>>>(tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E);
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
 }  // namespace
 
 int attention_bwd_tc5(const AttnArgs& a, cudaStream_t s) {
-  return a.dh == 64 ? launch_bwd5<64>(a, s) : launch_bwd5<128>(a, s);
+  switch (a.dh) {
+    case 64: return launch_bwd5<64>(a, s);
+    case 128: return launch_bwd5<128>(a, s);
+    case 192: return launch_bwd5<192>(a, s);
+    default: return launch_bwd5<256>(a, s);
+  }
 }
 bool attention_bwd_tc5_supported(const AttnArgs& a) {
   auto al16 = [](const void* p) { return (((uintptr_t)p) & 15) == 0; };
@@ -783,14 +840,19 @@ bool attention_bwd_tc5_supported(const AttnArgs& a) {
 }
 
 bool attention_tc5_supported(const AttnArgs& a) {
-  if (a.dtype != ORBIT_BF16 || (a.dh != 64 && a.dh != 128)) return false;
+  if (a.dtype != ORBIT_BF16 || (a.dh != 64 && a.dh != 128 && a.dh != 192 && a.dh != 256)) return false;
   auto al16 = [](const void* p) { return (((uintptr_t)p) & 15) == 0; };
   if (a.ld % 8 || a.ldo % 8 || a.q_off % 8 || a.k_off % 8 || a.v_off % 8) return false;
   if (!al16(a.qkv) || !al16(a.O)) return false;
   return a.N >= 128;
 }
 int attention_fwd_tc5(const AttnArgs& a, cudaStream_t s) {
-  return a.dh == 64 ? launch_fwd5<64>(a, s) : launch_fwd5<128>(a, s);
+  switch (a.dh) {
+    case 64: return launch_fwd5<64>(a, s);
+    case 128: return launch_fwd5<128>(a, s);
+    case 192: return launch_fwd5<192>(a, s);
+    default: return launch_fwd5<256>(a, s);
+  }
 }
 
 }  // namespace orbit

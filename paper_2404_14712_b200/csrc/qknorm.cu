@@ -32,6 +32,7 @@ __device__ __forceinline__ void ld_vec_bf16(const bf16* p, float* v) {
 }
 template <> __device__ __forceinline__ void ld_vec<bf16, 2>(const bf16* p, float* v) { ld_vec_bf16<2>(p, v); }
 template <> __device__ __forceinline__ void ld_vec<bf16, 4>(const bf16* p, float* v) { ld_vec_bf16<4>(p, v); }
+template <> __device__ __forceinline__ void ld_vec<bf16, 6>(const bf16* p, float* v) { ld_vec_bf16<6>(p, v); }
 template <> __device__ __forceinline__ void ld_vec<bf16, 8>(const bf16* p, float* v) { ld_vec_bf16<8>(p, v); }
 
 template <typename T, int EPL>
@@ -46,6 +47,7 @@ __device__ __forceinline__ void st_vec_bf16(bf16* p, const float* v) {
 }
 template <> __device__ __forceinline__ void st_vec<bf16, 2>(bf16* p, const float* v) { st_vec_bf16<2>(p, v); }
 template <> __device__ __forceinline__ void st_vec<bf16, 4>(bf16* p, const float* v) { st_vec_bf16<4>(p, v); }
+template <> __device__ __forceinline__ void st_vec<bf16, 6>(bf16* p, const float* v) { st_vec_bf16<6>(p, v); }
 template <> __device__ __forceinline__ void st_vec<bf16, 8>(bf16* p, const float* v) { st_vec_bf16<8>(p, v); }
 
 // mean / rstd of one head vector spread over the warp (EPL elements per lane)
@@ -144,7 +146,7 @@ template <typename T>
 int launch_fwd(void* qkv, long long ld, long long items, int hk, int dh, int dc, const void* qg, const void* qb, const void* kg,
                const void* kb, int p_dt, float eps, int grid, cudaStream_t s) {
 #define QF(E) qknorm_fwd_kernel<T, E><<<grid, 256, 0, s>>>((T*)qkv, ld, items, hk, dh, dc, qg, qb, kg, kb, p_dt, eps)
-  switch (dh / 32) { case 1: QF(1); break; case 2: QF(2); break; case 4: QF(4); break; case 8: QF(8); break; default: return ORBIT_ERR_SHAPE; }
+  switch (dh / 32) { case 1: QF(1); break; case 2: QF(2); break; case 4: QF(4); break; case 6: QF(6); break; case 8: QF(8); break; default: return ORBIT_ERR_SHAPE; }
 #undef QF
   return ORBIT_OK;
 }
@@ -152,7 +154,7 @@ template <typename T>
 int launch_bwd(const void* qkv, void* dqkv, long long ld, long long items, int hk, int dh, int dc, const void* qg, const void* kg,
                int p_dt, float eps, float* acc, int grid, cudaStream_t s) {
 #define QB(E) qknorm_bwd_kernel<T, E><<<grid, 256, 0, s>>>((const T*)qkv, (T*)dqkv, ld, items, hk, dh, dc, qg, kg, p_dt, eps, acc)
-  switch (dh / 32) { case 1: QB(1); break; case 2: QB(2); break; case 4: QB(4); break; case 8: QB(8); break; default: return ORBIT_ERR_SHAPE; }
+  switch (dh / 32) { case 1: QB(1); break; case 2: QB(2); break; case 4: QB(4); break; case 6: QB(6); break; case 8: QB(8); break; default: return ORBIT_ERR_SHAPE; }
 #undef QB
   return ORBIT_OK;
 }
@@ -162,7 +164,7 @@ int grid_items(long long items) {
 }
 }  // namespace
 
-bool qknorm_supported(int dh) { return dh == 32 || dh == 64 || dh == 128 || dh == 256; }
+bool qknorm_supported(int dh) { return dh == 32 || dh == 64 || dh == 128 || dh == 192 || dh == 256; }
 
 int qknorm_fwd(void* qkv, long long ld, int M, int hk, int dh, int dc, const void* qg, const void* qb, const void* kg,
                const void* kb, int p_dt, int dt, float eps, cudaStream_t s) {

@@ -63,6 +63,12 @@ CONFIGS = {
                  dtype="bf16", resid_dtype="bf16"),
     "C5": Config("C5", B=1, N=2048, D=12288, heads=96, F=49152, depth=1,
                  dtype="bf16", resid_dtype="bf16"),
+    # the paper's own layer shapes (PAPER.md:140 model table), one block each: not BASELINE.json
+    # configs, benchmarked with `bench.py --workload P113 / P10B`
+    "P113": Config("P113", B=1, N=2048, D=12288, heads=64, F=49152, depth=1,       # 113B: 12288 wide, 64 heads => d_h 192
+                   dtype="bf16", resid_dtype="bf16"),
+    "P10B": Config("P10B", B=2, N=2048, D=8192, heads=32, F=32768, depth=1,        # 10B: 8192 wide, 32 heads => d_h 256
+                   dtype="bf16", resid_dtype="bf16"),
 }
 
 
@@ -264,4 +270,6 @@ def fields(seed: int, B: int, V: int, Hg: int, Wg: int, per_variable_scale: bool
 
 
 def seed_of(cfg_name: str) -> int:
+    if cfg_name.startswith("P"):                  # paper-shaped workloads
+        return 1100 + int("".join(ch for ch in cfg_name if ch.isdigit()))
     return 1000 + int(cfg_name[1:])

@@ -7,15 +7,17 @@ also held, element by element, to
     |got - ref|  <=  C_ELEM * tol * max(rms(ref), rms(ref row))  +  eps_store * |ref|
 
 (DESIGN.md §7): eps_store |ref| is the one rounding of the element's own stored value (bf16: 2^-8, fp32: 2^-23);
-the first term bounds the error inherited from upstream roundings, which behaves like noise of standard deviation
-<= tol * rms(ref) (that is what the Frobenius tolerance says) whose maximum over n <= 2e9 elements stays below 6.4
-standard deviations; C_ELEM = 8 leaves a margin.  A wrongly placed tile differs from the reference by ~sqrt(2) rms(ref),
-i.e. >= 17x this bound at tol = 1e-2, so a single misplaced element fails.
+the first term bounds the error inherited from upstream roundings, whose standard deviation is <= tol * rms(ref) (that
+is what the Frobenius tolerance says).  Were it Gaussian its maximum over n <= 2e9 elements would stay below 6.4
+standard deviations; it is heavier-tailed than that (an element that is a short, cancelling sum of large rounded terms
+-- e.g. a tokeniser weight gradient summed over 4 patches -- inherits the error of its terms, not of its value:
+11.6 standard deviations observed), so C_ELEM = 16.  A wrongly placed tile differs from the reference by ~sqrt(2) rms(ref),
+i.e. ~9x this bound at tol = 1e-2 over a whole 32 x 32 box, so a single misplaced box fails.
 """
 import numpy as np
 import torch
 
-C_ELEM = 8.0
+C_ELEM = 16.0
 EPS_STORE = {"bf16": 2.0 ** -8, "f32": 2.0 ** -23}
 
 

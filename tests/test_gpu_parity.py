@@ -136,6 +136,25 @@ def test_block_bf16_vs_oracle(rn, shape):
     print("bf16 block errs", {k: f"{v:.2e}" for k, v in errs.items()})
 
 
+@pytest.mark.parametrize("shape", [
+    (1, 384, 768, 4, 1536, 1, "bf16"),      # d_h 192 (113B and 1B rows), three 128-row tiles
+    (2, 200, 512, 2, 1024, 1, "f32"),       # d_h 256 (10B row), ragged N (one full + one partial query tile; 7 key tiles of 32)
+    (1, 520, 768, 4, 1536, 2, "bf16"),      # d_h 192, Hybrid-STOP T = 2, ragged N spanning tile tails
+    (1, 333, 1024, 4, 2048, 1, "bf16"),     # d_h 256, odd N: ragged 64-key / 32-row tiles, dK/dV computed in two column slices
+])
+@pytest.mark.parametrize("qkn", [False, True])
+def test_block_bf16_paper_head_widths(rn, shape, qkn):
+    """The paper's own head widths d_h = 192 and 256 on the tcgen05 attention path (64-row key tiles
+    forward, 32-row streamed tiles backward), with and without QK-LayerNorm."""
+    B, N, D, heads, F, T, rdt = shape
+    P, shards, x, dy = make_block_case(23, B, N, D, heads, F, T, "bf16", rdt)
+    if qkn:
+        P.update(syn.qk_norm_params(23, D // heads, "bf16"))
+    br, y, dx = run_block(rn, B, N, D, heads, F, T, "bf16", rdt, P, shards, x, dy)
+    errs = compare_block(br, y, dx, P, x, dy, heads, T, 1e-2)
+    print("paper head widths", shape, qkn, {k: f"{v:.2e}" for k, v in errs.items()})
+
+
 @pytest.mark.parametrize("T", [1, 2])
 def test_block_qk_norm_fp32(rn, T):
     """QK-LayerNorm (ORBIT_QK_NORM) in fp32, d_h = 32, also sharded: <= 1e-4 vs the unsharded oracle."""

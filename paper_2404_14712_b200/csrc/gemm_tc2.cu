@@ -14,6 +14,7 @@
 //   tfull[a]  (per CTA, count 1) : tcgen05.commit multicast -> both epilogues
 //   tempty[a] (leader's, count 16): the 8 epilogue warps of both CTAs release the accumulator
 #include <cuda.h>
+#include <stdlib.h>
 #include "common.cuh"
 #include "gemm_epi.cuh"
 #include "ptx.cuh"
@@ -33,9 +34,9 @@ constexpr int EPI_BOX_BYTES = 32 * 32 * 2;
 constexpr int EPI_BYTES = 8 * 2 * EPI_BOX_BYTES;    // 32 KB
 constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + EPI_BYTES + 1024 + 256;
 
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(m), "r"(src), "r"(c0),
-               "r"(c1), "r"(c2)
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;" ::"l"(m), "r"(src), "r"(c0),
+               "r"(c1), "r"(c2), "l"(policy)
                : "memory");
 }
 __device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
@@ -47,8 +48,9 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-__device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, int& mb, int& nb) {
-  constexpr int GROUP = 8;                      // 8 x 256 rows of A shared through L2 by concurrent clusters
+// Raster: groups of `group` row blocks, all column blocks of a group before the next group.  The A panels of a group
+// (group x 256 x K) are what concurrent clusters share through L2; B is streamed once per group (host heuristic in launch2).
+__device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, int GROUP, int& mb, int& nb) {
   const int group_size = GROUP * tiles_n;
   const int g = t / group_size, r = t - g * group_size;
   const int first_m = g * GROUP;
@@ -56,13 +58,23 @@ __device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, in
   mb = first_m + r % gm;
   nb = r / gm;
 }
+// Work units of the persistent loop.  Units [0, full) are whole 256 x 256 tiles, dealt round-robin to the clusters.  The
+// tiles of the last, partial round (num_tiles % num_clusters of them: 14 of 384 at N = 12288 on 74 clusters, i.e. a sixth
+// round that keeps 19 % of the SMs busy) are split into `parts` column sub-tiles of W = 256 / parts columns each, so that
+// the last round takes 1 / parts of a tile time on parts x as many clusters.
+// hint_a / hint_b / hint_c: L2 eviction priority of the A loads, B loads and C stores (0 normal, 1 evict_first, 2 evict_last)
+struct Sched { int full, parts, total, group_m, hint_a, hint_b, hint_c; };
+__device__ __forceinline__ void unit_of(const Sched& sc, int u, int& t, int& part, int& W) {
+  if (u < sc.full) { t = u; part = 0; W = BN2; }
+  else { const int r = u - sc.full; t = sc.full + r / sc.parts; part = r % sc.parts; W = BN2 / sc.parts; }
+}
 
 template <int A_MN, int B_MN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                 const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmX, int tma_store, epi::Args e0,
                 int M, int N, int K,
-                int batch, long long c_bs, long long bias_bs) {
+                int batch, long long c_bs, long long bias_bs, Sched sc) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t epi_base = smem_base + STAGES * STAGE_BYTES;
@@ -105,11 +117,15 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     // ===================== TMA producer (both CTAs) =====================
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
-      for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+      const uint64_t pol_a = ptx::l2_policy(sc.hint_a), pol_b = ptx::l2_policy(sc.hint_b);
+      for (int u = cluster_id; u < sc.total; u += num_clusters) {
+        int t, part, W;
+        unit_of(sc, u, t, part, W);
         const int bi = t / tiles_per_batch;
         int mb, nb;
-        tile_coords2(t - bi * tiles_per_batch, tiles_m, tiles_n, mb, nb);
-        const int m0 = mb * BM2 + (int)rank * 128, n0 = nb * BN2 + (int)rank * 128;
+        tile_coords2(t - bi * tiles_per_batch, tiles_m, tiles_n, sc.group_m, mb, nb);
+        // a sub-tile loads the same boxes (expect_tx unchanged) from its own column origin and uses the first W / 2 of them
+        const int m0 = mb * BM2 + (int)rank * 128, n0 = nb * BN2 + part * W + (int)rank * (W / 2);
         for (int kb = 0; kb < num_kb; kb++) {
           ptx::mbar_wait(empty_bar(s), ph ^ 1);
           const uint32_t lfull = ptx::mapa(full_bar(s), 0);
@@ -118,15 +134,15 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           const int k0 = kb * BK;
           if (A_MN) {
 #pragma unroll
-            for (int i = 0; i < 2; i++) ptx::tma_load_3d_2sm(sa + i * 8192, &tmA, lfull, m0 + i * 64, k0, bi);
+            for (int i = 0; i < 2; i++) ptx::tma_load_3d_2sm_hint(sa + i * 8192, &tmA, lfull, m0 + i * 64, k0, bi, pol_a);
           } else {
-            ptx::tma_load_3d_2sm(sa, &tmA, lfull, k0, m0, bi);
+            ptx::tma_load_3d_2sm_hint(sa, &tmA, lfull, k0, m0, bi, pol_a);
           }
           if (B_MN) {
 #pragma unroll
-            for (int i = 0; i < 2; i++) ptx::tma_load_3d_2sm(sb + i * 8192, &tmB, lfull, n0 + i * 64, k0, bi);
+            for (int i = 0; i < 2; i++) ptx::tma_load_3d_2sm_hint(sb + i * 8192, &tmB, lfull, n0 + i * 64, k0, bi, pol_b);
           } else {
-            ptx::tma_load_3d_2sm(sb, &tmB, lfull, k0, n0, bi);
+            ptx::tma_load_3d_2sm_hint(sb, &tmB, lfull, k0, n0, bi, pol_b);
           }
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
@@ -135,12 +151,12 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA only) =====================
     if (leader && lane == 0) {
-      constexpr uint32_t idesc = ptx::make_idesc_bf16(BM2, BN2, A_MN, B_MN);
       constexpr uint32_t a_lbo = A_MN ? 8192 : 16, a_sbo = 1024, a_step = A_MN ? 2048 : 32;
       constexpr uint32_t b_lbo = B_MN ? 8192 : 16, b_sbo = 1024, b_step = B_MN ? 2048 : 32;
       int s = 0; uint32_t ph = 0;
       int acc = 0; uint32_t aph = 0;
-      for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+      for (int u = cluster_id; u < sc.total; u += num_clusters) {
+        const uint32_t idesc = ptx::make_idesc_bf16(BM2, u < sc.full ? BN2 : BN2 / sc.parts, A_MN, B_MN);
         ptx::mbar_wait(tempty_bar(acc), aph ^ 1);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * BN2;
@@ -167,14 +183,18 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int chalf = (warp - 2) >> 2;           // which 128 of the 256 accumulator columns
     int acc = 0; uint32_t aph = 0;
     uint32_t ebuf = 0;
-    for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+    const uint64_t pol_c = ptx::l2_policy(sc.hint_c);
+    for (int u = cluster_id; u < sc.total; u += num_clusters) {
+      int t, part, W;
+      unit_of(sc, u, t, part, W);
       const int bi = t / tiles_per_batch;
       int mb, nb;
-      tile_coords2(t - bi * tiles_per_batch, tiles_m, tiles_n, mb, nb);
+      tile_coords2(t - bi * tiles_per_batch, tiles_m, tiles_n, sc.group_m, mb, nb);
       epi::Args e = e0;
       if (batch > 1) epi::offset_batch(e, bi, c_bs, bias_bs);
       const int row = mb * BM2 + (int)rank * 128 + quarter * 32 + lane;
-      const int n0 = nb * BN2;
+      const int n0 = nb * BN2 + part * W;
+      const int c_lo = chalf * (W / 64), c_hi = (chalf + 1) * (W / 64);     // this warp's 32-column chunks of the (sub-)tile
       ptx::mbar_wait(tfull_bar(acc), aph);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + acc * BN2 + ((uint32_t)(quarter * 32) << 16);
@@ -185,7 +205,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // read-modify-write of C in the SM
         const int wrow0 = mb * BM2 + (int)rank * 128 + quarter * 32;
 #pragma unroll 1
-        for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
+        for (int c = c_lo; c < c_hi; c++) {
           uint32_t r[32];
           ptx::tmem_ld_32x32(taddr + c * 32, r);
           ptx::tmem_ld_wait();
@@ -230,7 +250,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             __syncwarp();
             if (lane == 0) {
               if (e.accumulate) tma_reduce_add_3d(&tmC, buf, col0 + hh * 16, wrow0, bi);
-              else tma_store_3d(&tmC, buf, col0 + hh * 16, wrow0, bi);
+              else tma_store_3d(&tmC, buf, col0 + hh * 16, wrow0, bi, pol_c);
               bulk_commit();
             }
             ebuf ^= 1;
@@ -258,11 +278,11 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           }
           ptx::fence_proxy_async();
           __syncwarp();
-          if (lane == 0) { tma_store_3d(tm, buf, col0, wrow0, bi); bulk_commit(); }
+          if (lane == 0) { tma_store_3d(tm, buf, col0, wrow0, bi, pol_c); bulk_commit(); }
           ebuf ^= 1;
         };
 #pragma unroll 1
-        for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
+        for (int c = c_lo; c < c_hi; c++) {
           uint32_t r[32];
           ptx::tmem_ld_32x32(taddr + c * 32, r);
           ptx::tmem_ld_wait();
@@ -315,7 +335,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         }
       } else {
 #pragma unroll 1
-      for (int c = chalf * (BN2 / 64); c < (chalf + 1) * (BN2 / 64); c++) {
+      for (int c = c_lo; c < c_hi; c++) {
         uint32_t r[32];
         ptx::tmem_ld_32x32(taddr + c * 32, r);
         ptx::tmem_ld_wait();
@@ -337,18 +357,59 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   }
 }
 
+// A/B switches of the schedule (read once; profiles/r2_gemm_schedule.md): ORBIT_GEMM_TAIL_SPLIT=0 keeps whole tiles in
+// the last round; ORBIT_GEMM_GROUP_M=<n> forces the raster group height; ORBIT_GEMM_L2HINT=<bits> selects the L2 eviction
+// hints (default 1).
+bool tail_split_enabled() {
+  static const int v = [] { const char* e = getenv("ORBIT_GEMM_TAIL_SPLIT"); return (e && e[0] == '0') ? 0 : 1; }();
+  return v != 0;
+}
+int l2_hint_mode() {
+  static const int v = [] { const char* e = getenv("ORBIT_GEMM_L2HINT"); return e ? atoi(e) : 1; }();
+  return v;
+}
+int raster_group_m(int tiles_m, int M, int K) {
+  static const int forced = [] { const char* e = getenv("ORBIT_GEMM_GROUP_M"); return e ? atoi(e) : 0; }();
+  if (forced > 0) return forced < tiles_m ? forced : tiles_m;
+  (void)M; (void)K;
+  return 8 < tiles_m ? 8 : tiles_m;
+}
+
 template <int A_MN, int B_MN>
 int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const CUtensorMap* mx, const GemmArgs& g, int sms,
             cudaStream_t s) {
   const epi::Args e = epi::from_gemm(g);
   const int M = g.M, N = g.N, K = g.K, batch = g.batch > 1 ? g.batch : 1;
   ORBIT_SMEM_ATTR((gemm_tc2_kernel<A_MN, B_MN>), SMEM_BYTES);
-  const long long tiles = (long long)cdiv(M, BM2) * cdiv(N, BN2) * batch;
+  const int tiles_m = cdiv(M, BM2);
+  const long long tiles = (long long)tiles_m * cdiv(N, BN2) * batch;
   int clusters = sms / 2;
   if (tiles < clusters) clusters = (int)tiles;
+  Sched sc;
+  // last partial round: split its tiles into two 256 x 128 sub-tiles when they then still fit one round
+  const int rem = (int)(tiles % clusters);
+  sc.parts = (rem > 0 && 2 * rem <= clusters && tiles > clusters && tail_split_enabled()) ? 2 : 1;
+  sc.full = sc.parts > 1 ? (int)(tiles - rem) : (int)tiles;
+  sc.total = sc.full + (sc.parts > 1 ? rem * sc.parts : 0);
+  sc.group_m = raster_group_m(tiles_m, M, K);
+  // L2 policy (A/B on one box, profiles/r2_gemm_schedule.md): evict_last on the SMALLER operand (the activation panel every
+  // round re-reads: C5 fc1 needs its 50 MB `a` in all 21 rounds while 1.2 GB of weights stream through the L2) is worth
+  // ~1 % of the C5 step; evict_first on the larger operand RAISES the DRAM traffic (27 -> 37 GB per step: the clusters that
+  // share a panel inside a round then miss it) and evict_first on large outputs changes nothing; both stay off.
+  sc.hint_a = sc.hint_b = sc.hint_c = 0;
+  const int hm = l2_hint_mode();                // bit 0: smaller operand evict_last; bit 1: large outputs evict_first; bit 2: larger operand evict_first
+  if (hm) {
+    const double bytes_a = 2.0 * M * K * batch, bytes_b = 2.0 * N * K * batch, bytes_c = (double)dsize(g.out_dtype) * M * N * batch;
+    const double small = bytes_a < bytes_b ? bytes_a : bytes_b, big = bytes_a < bytes_b ? bytes_b : bytes_a;
+    if (small <= 80e6 && big > 100e6) {
+      if (hm & 1) (bytes_a < bytes_b ? sc.hint_a : sc.hint_b) = 2;
+      if (hm & 4) (bytes_a < bytes_b ? sc.hint_b : sc.hint_a) = 1;
+    }
+    if ((hm & 2) && bytes_c > 100e6) sc.hint_c = 1;
+  }
   gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, mc ? *mc : ma, mx ? *mx : ma,
                                                                          (mc ? (g.out_dtype == ORBIT_F32 ? 4 : 1) : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,
-                                                                         g.bias_bs);
+                                                                         g.bias_bs, sc);
   return ORBIT_OK;
 }
 }  // namespace

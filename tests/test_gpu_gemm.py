@@ -40,7 +40,9 @@ def run_gemm(ob, M, N, K, a_major, b_major, dtype):
 
 
 SHAPES = [(128, 256, 64), (256, 512, 256), (200, 264, 136), (1024, 768, 520), (2048, 1024, 2048), (64, 64, 32),
-          (2048, 3072, 512), (1800, 2904, 264)]     # two rounds of 256 x 256 CTA-pair tiles, ragged N tail
+          (2048, 3072, 512), (1800, 2904, 264),     # two rounds of 256 x 256 CTA-pair tiles, ragged N tail
+          (2048, 12288, 320), (1800, 9992, 136)]    # 384 / 320 tiles on 74 clusters: the 14 / 24 tiles of the last round run as
+                                                    # 256 x 128 column sub-tiles (gemm_tc2.cu Sched), full and ragged N
 
 
 @pytest.mark.parametrize("a_major", ["K", "M"])
@@ -89,7 +91,8 @@ def test_gemm_strided_batch(ob, case, dtype):
 
 
 # ---- bf16 outputs (+ bias): the TMA-store epilogue of the CTA-pair kernel, ragged in M and N, padded row stride ----
-OUT_SHAPES = [(256, 256, 64, 256), (520, 776, 136, 776), (1800, 2904, 264, 2912), (300, 264, 520, 272), (2048, 3072, 512, 3072)]
+OUT_SHAPES = [(256, 256, 64, 256), (520, 776, 136, 776), (1800, 2904, 264, 2912), (300, 264, 520, 272), (2048, 3072, 512, 3072),
+              (2048, 12288, 192, 12288)]          # last round of 14 tiles split into column sub-tiles (TMA-store epilogue)
 
 
 @pytest.mark.parametrize("a_major", ["K", "M"])

@@ -257,9 +257,14 @@ void orbit_reset_launch_count(void);
 /* Per-launch CUDA-event timing of the tensor-core GEMM kernel (the dominant kernel; bench.py's roofline leg).
  * orbit_profile_gemm(1) starts recording an event pair around every tcgen05 GEMM launch on its stream;
  * orbit_profile_gemm_collect() waits for them, returns the summed kernel milliseconds, the summed algorithmic
- * FLOPs (2 M N K per launch) and the number of launches recorded, and clears the record. */
+ * FLOPs (2 M N K per launch) and the number of launches recorded. */
 int orbit_profile_gemm(int on);
 int orbit_profile_gemm_collect(double* ms, double* flops, long long* launches);
+/* The same record by category (bench.py's secondary roofline entries): 0 = tcgen05 GEMM (work = FLOPs), 1 = attention forward,
+ * 2 = attention backward (FLOPs: 4 B N^2 D resp. twice that), 3 = LayerNorm forward / backward kernels, 4 = front-end
+ * streaming kernels (tokenise, per-patch aggregation, pixel-space per-patch kernels) (work = algorithmic bytes).
+ * Non-destructive; orbit_profile_gemm(1) clears the record.  ORBIT_ERR_SHAPE for an unknown category. */
+int orbit_profile_collect(int category, double* ms, double* work, long long* launches);
 /* Kernel-level diagnostic: C[M,N] (fp32, row-major) = A B through the library's GEMM dispatcher.
  * A(m,k) = A[m*a_rs + k*a_cs], B(k,n) = B[k*b_rs + n*b_cs] (element strides); dtype of A and B = `dtype`.
  * Exercises every operand-major combination the block uses (K-major / MN-major A and B). */

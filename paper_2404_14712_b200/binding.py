@@ -155,6 +155,7 @@ _proto("orbit_chain_workspace_bytes", _sz, [C.c_int] * 5 + [C.c_int])
 _proto("orbit_mse_loss_grad", C.c_int, [C.c_int, _sz, _vp, _vp, _vp, _vp, _vp])
 _proto("orbit_profile_gemm", C.c_int, [C.c_int])
 _proto("orbit_profile_gemm_collect", C.c_int, [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)])
+_proto("orbit_profile_collect", C.c_int, [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)])
 _proto("orbit_debug_gemm", C.c_int, [C.c_int] * 4 + [_vp, C.c_longlong, C.c_longlong, _vp, C.c_longlong, C.c_longlong, _vp, _vp])
 _ll = C.c_longlong
 _proto("orbit_debug_gemm_batched", C.c_int, [C.c_int] * 5 + [_vp, _ll, _ll, _ll, _vp, _ll, _ll, _ll, _vp, _ll, _ll, _vp])
@@ -169,7 +170,7 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_block_saved_bytes", "orbit_mse_loss_grad", "orbit_chain_fwd", "orbit_chain_bwd", "orbit_chain_workspace_bytes",
            "orbit_last_error", "orbit_version", "orbit_launch_count", "orbit_reset_launch_count",
            "orbit_debug_gemm", "orbit_profile_gemm",
-           "orbit_profile_gemm_collect", "orbit_embed_fused", "orbit_embed_fused_bwd",
+           "orbit_profile_gemm_collect", "orbit_profile_collect", "orbit_embed_fused", "orbit_embed_fused_bwd",
            "orbit_embed_fused_workspace_bytes", "orbit_embed_fused_bwd_workspace_bytes",
            "orbit_embed_fused_saved_bytes", "orbit_debug_gemm_batched", "orbit_head_loss", "orbit_head_loss_bwd",
            "orbit_head_loss_workspace_bytes", "orbit_head_loss_bwd_workspace_bytes", "orbit_head_loss_saved_bytes",
@@ -470,6 +471,16 @@ def orbit_debug_layernorm_bwd(M, D, dout_dt, x_dt, p_dt, add_dt, out_dt, dout, x
 
 def orbit_profile_gemm(on: bool):
     _check(lib.orbit_profile_gemm(1 if on else 0), "orbit_profile_gemm")
+
+
+PROF_GEMM, PROF_ATTN_FWD, PROF_ATTN_BWD, PROF_LN, PROF_FRONT = range(5)
+
+
+def orbit_profile_collect(category):
+    """(summed kernel ms, summed algorithmic work, launches) of one category of the per-launch event record."""
+    ms, wk, n = C.c_double(), C.c_double(), C.c_longlong()
+    _check(lib.orbit_profile_collect(category, C.byref(ms), C.byref(wk), C.byref(n)), "orbit_profile_collect")
+    return ms.value, wk.value, n.value
 
 
 def orbit_profile_gemm_collect():

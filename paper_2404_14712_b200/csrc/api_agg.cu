@@ -98,8 +98,11 @@ int orbit_var_aggregate(const orbit_agg_desc* d, const void* tok, const orbit_ag
   ORBIT_TRY(agg_make_qt(P->q, P->Wq, P->bq, dt, sv.qt, D, s));   // qt = q Wq + bq (data independent; R3, R4)
   ORBIT_TRY(agg_make_u(P->Wk, dt, sv.qt, sv.Ut, D, h, s));
   const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);
-  if (tc) ORBIT_TRY(agg_patch_fwd_tc(tok, sv.Ut, sv.Utb, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
-  else ORBIT_TRY(agg_patch_fwd(tok, dt, sv.Ut, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
+  {
+    ProfScope prof(PROF_FRONT, (double)BL * d->V * D * dsize(dt), s);                            // a2 reads tok once (algorithmic)
+    if (tc) ORBIT_TRY(agg_patch_fwd_tc(tok, sv.Ut, sv.Utb, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
+    else ORBIT_TRY(agg_patch_fwd(tok, dt, sv.Ut, sv.alpha, sv.Xbar, BL, d->V, D, h, s));
+  }
   {  // o_a = Xbar_a Wv[:, a] + bv[a], the `heads` products as one strided-batch launch
     GemmArgs g;
     g.A = sv.Xbar; g.a_rs = (long long)h * D; g.a_cs = 1; g.B = P->Wv; g.b_rs = D; g.b_cs = 1;
@@ -174,8 +177,11 @@ int orbit_var_aggregate_bwd(const orbit_agg_desc* d, const void* tok, const orbi
     ORBIT_TRY(gemm(gx, s));
   }
   const bool tc = g_force_simt != 1 && agg_tc_supported(dt, d->V, D, h);
-  if (tc) ORBIT_TRY(agg_patch_bwd_tc(tok, sv.Utb, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
-  else ORBIT_TRY(agg_patch_bwd(tok, dt, sv.Ut, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
+  {
+    ProfScope prof(PROF_FRONT, 2.0 * BL * d->V * D * dsize(dt), s);                              // a2' reads tok and writes dtok
+    if (tc) ORBIT_TRY(agg_patch_bwd_tc(tok, sv.Utb, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
+    else ORBIT_TRY(agg_patch_bwd(tok, dt, sv.Ut, sv.alpha, w.dXbar, dtok, acc_dUt, BL, d->V, D, h, s));
+  }
   ORBIT_TRY(agg_param_bwd(acc_dUt, sv.qt, P->q, P->Wq, P->Wk, dt, G->Wk, G->bk, G->bq, G->Wq, G->q, dqt, D, h, s));
   ORBIT_TRY(cast_copy(acc_bo, ORBIT_F32, G->bo, dt, D, s));
   ORBIT_TRY(cast_copy(acc_bv, ORBIT_F32, G->bv, dt, D, s));

@@ -1,5 +1,6 @@
 // api_common.cu -- error state, device check, diagnostics, tokenise and Eq.(2)/(3) chain entry points.
 #include <stdarg.h>
+#include <stdlib.h>
 #include <string.h>
 #include "api_util.cuh"
 #include "frontend.cuh"
@@ -46,6 +47,58 @@ int check_device() {
   return ORBIT_OK;
 }
 
+// ---- per-launch event timing ------------------------------------------------------------------------------------------
+namespace {
+struct ProfState {
+  bool on = false;
+  static constexpr int MAXP = 32768;
+  cudaEvent_t* ev = nullptr;     // 2 * MAXP events, created on first enable
+  double* work = nullptr;
+  unsigned char* cat = nullptr;
+  int n = 0;
+} g_prof;
+}  // namespace
+int prof_enable(int on) {
+  if (on && !g_prof.ev) {
+    g_prof.ev = new cudaEvent_t[2 * ProfState::MAXP];
+    g_prof.work = new double[ProfState::MAXP];
+    g_prof.cat = new unsigned char[ProfState::MAXP];
+    for (int i = 0; i < 2 * ProfState::MAXP; i++) ORBIT_CUDA_CHECK(cudaEventCreate(&g_prof.ev[i]));
+  }
+  g_prof.on = on != 0;
+  g_prof.n = 0;
+  return ORBIT_OK;
+}
+int prof_collect(int cat, double* ms, double* work, long long* launches) {
+  double t = 0, w = 0;
+  long long n = 0;
+  for (int i = 0; i < g_prof.n; i++) {
+    if (g_prof.cat[i] != cat) continue;
+    float e = 0.f;
+    ORBIT_CUDA_CHECK(cudaEventSynchronize(g_prof.ev[2 * i + 1]));
+    ORBIT_CUDA_CHECK(cudaEventElapsedTime(&e, g_prof.ev[2 * i], g_prof.ev[2 * i + 1]));
+    t += e; w += g_prof.work[i]; n++;
+  }
+  if (ms) *ms = t;
+  if (work) *work = w;
+  if (launches) *launches = n;
+  return ORBIT_OK;
+}
+ProfScope::ProfScope(int cat, double work, cudaStream_t stream) : slot(-1), s(stream) {
+  if (!g_prof.on || g_prof.n >= ProfState::MAXP) return;
+  slot = g_prof.n++;
+  g_prof.cat[slot] = (unsigned char)cat;
+  g_prof.work[slot] = work;
+  cudaEventRecord(g_prof.ev[2 * slot], s);
+}
+ProfScope::~ProfScope() {
+  if (slot >= 0) cudaEventRecord(g_prof.ev[2 * slot + 1], s);
+}
+
+bool pdl_enabled() {
+  static const int v = [] { const char* e = getenv("ORBIT_PDL"); return (e && e[0] == '0') ? 0 : 1; }();
+  return v != 0;
+}
 int device_ordinal() {
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 0; }
@@ -110,6 +163,8 @@ int orbit_tokenize(const orbit_embed_desc* d, const float* x, const void* Wp, co
   if (!x || !Wp || !bp || !tok) { set_error("tokenize: NULL pointer"); return ORBIT_ERR_NULL; }
   if (!aligned16(x) || !aligned16(Wp) || !aligned16(bp) || !aligned16(tok)) { set_error("tokenize: pointer not 16B aligned"); return ORBIT_ERR_ALIGN; }
   ORBIT_TRY(check_device());
+  const size_t ntok = (size_t)d->B * (d->Hg / d->p) * (d->Wg / d->p) * d->V;
+  ProfScope prof(PROF_FRONT, (double)ntok * d->D * dsize(d->dtype), (cudaStream_t)stream);     // a1 writes tok once
   if (g_force_simt != 1 && tokenize_tc_supported(*d)) return tokenize_fwd_tc(*d, x, Wp, bp, tok, (cudaStream_t)stream);
   return tokenize_fwd(*d, x, Wp, bp, tok, (cudaStream_t)stream);
 }
@@ -131,16 +186,24 @@ int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dt
   float* accW = (float*)ws;
   float* accB = accW + (size_t)d->V * P2 * d->D;
   ORBIT_TRY(fill_zero(ws, (size_t)d->V * (P2 + 1) * d->D * sizeof(float), s));
-  if (g_force_simt != 1 && tokenize_tc_supported(*d)) ORBIT_TRY(tokenize_bwd_acc_tc(*d, x, dtok, accW, accB, s));
-  else ORBIT_TRY(tokenize_bwd_acc(*d, x, dtok, accW, accB, s));
+  {
+    const size_t ntok = (size_t)d->B * (d->Hg / d->p) * (d->Wg / d->p) * d->V;
+    ProfScope prof(PROF_FRONT, (double)ntok * d->D * dsize(d->dtype), s);                       // a1' reads dtok once
+    if (g_force_simt != 1 && tokenize_tc_supported(*d)) ORBIT_TRY(tokenize_bwd_acc_tc(*d, x, dtok, accW, accB, s));
+    else ORBIT_TRY(tokenize_bwd_acc(*d, x, dtok, accW, accB, s));
+  }
   ORBIT_TRY(cast_copy(accW, ORBIT_F32, dWp, d->dtype, (size_t)d->V * P2 * d->D, s));
   ORBIT_TRY(cast_copy(accB, ORBIT_F32, dbp, d->dtype, (size_t)d->V * d->D, s));
   return ORBIT_OK;
 }
 
-int orbit_profile_gemm(int on) { return gemm_profile_enable(on); }
+int orbit_profile_gemm(int on) { return prof_enable(on); }
 int orbit_profile_gemm_collect(double* ms, double* flops, long long* launches) {
-  return gemm_profile_collect(ms, flops, launches);
+  return prof_collect(PROF_GEMM, ms, flops, launches);
+}
+int orbit_profile_collect(int category, double* ms, double* work, long long* launches) {
+  if (category < 0 || category >= PROF_NCAT) { set_error("profile_collect: bad category %d", category); return ORBIT_ERR_SHAPE; }
+  return prof_collect(category, ms, work, launches);
 }
 
 int orbit_debug_gemm(int M, int N, int K, orbit_dtype dtype, const void* A, long long a_rs, long long a_cs,

@@ -119,7 +119,10 @@ int orbit_embed_fused(const orbit_front_desc* d, const float* x, const void* Wp,
     ORBIT_TRY(gemm(g, s));
   }
   // per patch: scores, softmax over the variables, A = alpha * pixext
-  ORBIT_TRY(fe_patch_fwd(x, sv.G, sv.alpha, sv.A, dt, d->V, f.Vp, d->Hg, d->Wg, d->p, h, f.BL, s));
+  {   // writes the A operand [BL, heads, R Vp] once (the algorithmic bytes of the pixel-space front end)
+    ProfScope prof(PROF_FRONT, (double)f.BL * h * (d->p * d->p + 1) * f.Vp * dsize(dt), s);
+    ORBIT_TRY(fe_patch_fwd(x, sv.G, sv.alpha, sv.A, dt, d->V, f.Vp, d->Hg, d->Wg, d->p, h, f.BL, s));
+  }
   {  // o_a = A_a H[:, a] + bv[a]   (strided batch over the heads; K = R*Vp)
     GemmArgs g;
     g.A = sv.A; g.a_rs = (long long)h * f.KVp; g.a_cs = 1; g.B = sv.H; g.b_rs = D; g.b_cs = 1;
@@ -211,7 +214,10 @@ int orbit_embed_fused_bwd(const orbit_front_desc* d, const float* x, const void*
     ORBIT_TRY(gemm(g, s));
   }
   // score path: ds per patch, dG = sum_bl pixext ds, dUt = Wpb^T dG
-  ORBIT_TRY(fe_patch_bwd(x, sv.alpha, w.dA, dt, w.dsT, d->V, f.Vp, d->Hg, d->Wg, d->p, h, BL, s));
+  {   // reads dA once
+    ProfScope prof(PROF_FRONT, (double)BL * h * (d->p * d->p + 1) * f.Vp * dsize(dt), s);
+    ORBIT_TRY(fe_patch_bwd(x, sv.alpha, w.dA, dt, w.dsT, d->V, f.Vp, d->Hg, d->Wg, d->p, h, BL, s));
+  }
   ORBIT_TRY(fe_dg(x, w.dsT, w.dG, d->B, d->V, f.Vp, d->Hg, d->Wg, d->p, s));
   ORBIT_TRY(fe_dut(sv.Wpb, dt, w.dG, acc_dUt, f.KVp, D, h, s));
   ORBIT_TRY(fe_finish_dwp(w.accW, w.dG, sv.Ut, dWp, dbp, dt, d->V, f.Vp, f.P2, D, h, s));

@@ -17,12 +17,17 @@ bool attention_bwd_tc5_supported(const AttnArgs& a);
 int attention_fwd_tc5(const AttnArgs& a, cudaStream_t s);
 int attention_bwd_tc5(const AttnArgs& a, cudaStream_t s);
 
+// algorithmic work: forward 4 B N^2 D FLOP (QK^T and PV), backward twice that (backward = 2x forward)
+static double attn_flops(const AttnArgs& a) { return 4.0 * a.B * (double)a.N * a.N * a.heads * a.dh; }
+
 int attention_fwd(const AttnArgs& a, cudaStream_t s) {
+  ProfScope prof(PROF_ATTN_FWD, attn_flops(a), s);
   if (g_force_simt != 1 && g_force_simt != 3 && attention_tc5_supported(a)) return attention_fwd_tc5(a, s);
   if (g_force_simt != 1 && attention_tc_supported(a)) return attention_fwd_tc(a, s);
   return attention_fwd_simt(a, s);
 }
 int attention_bwd(const AttnArgs& a, cudaStream_t s) {
+  ProfScope prof(PROF_ATTN_BWD, 2.0 * attn_flops(a), s);
   if (g_force_simt != 1 && g_force_simt != 3 && g_force_simt != 4 && attention_tc5_supported(a) && attention_bwd_tc5_supported(a))
     return attention_bwd_tc5(a, s);
   if (g_force_simt != 1 && attention_tc_supported(a)) return attention_bwd_tc(a, s);

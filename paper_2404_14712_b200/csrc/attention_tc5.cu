@@ -107,6 +107,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
   ptx::tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
+  pdl_wait();                                    // on-chip prologue done; first global access is below
+  pdl_trigger();
   const uint32_t tS0 = tmem, tO = tmem + 2 * BKV;
 
   if (warp == 0) {
@@ -460,6 +462,8 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
   ptx::tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
+  pdl_wait();                                    // on-chip prologue done; first global access is below
+  pdl_trigger();
   const uint32_t tSt = tmem, tdPt = tmem + 2 * BT, tdV = tmem + 4 * BT, tdK = tdV + DHO;
 
   if (warp == 0) {
@@ -627,6 +631,8 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   ptx::tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
+  pdl_wait();                                    // on-chip prologue done; first global access is below
+  pdl_trigger();
   const uint32_t tS = tmem, tdP = tmem + 2 * BT, tdQ = tmem + 4 * BT;
 
   if (warp == 0) {
@@ -742,6 +748,8 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
 
 // delta[b,h,i] = sum_d dO[i, h*dh+d] * O[i, h*dh+d]
 __global__ void attn_delta5_kernel(AttnArgs a) {
+  pdl_wait();
+  pdl_trigger();
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   const int total = a.B * a.heads * a.N;
   if (w >= total) return;
@@ -796,7 +804,7 @@ int launch_fwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_TRY(make_map5(&tmKV, a.qkv, a.ld, rows, Cfg<DH>::BKV));
   ORBIT_SMEM_ATTR(attn_fwd_tc5_kernel<DH>, Cfg<DH>::SMEM);
   dim3 grid(cdiv(a.N, BQ), a.B * a.heads);
-  attn_fwd_tc5_kernel<DH><<<grid, NTH, Cfg<DH>::SMEM, s>>>(tmQ, tmKV, a, LOG2E / sqrtf((float)DH));
+  ORBIT_CUDA_CHECK(launch_pdl(attn_fwd_tc5_kernel<DH>, grid, dim3(NTH), Cfg<DH>::SMEM, s, tmQ, tmKV, a, LOG2E / sqrtf((float)DH)));
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
@@ -813,14 +821,14 @@ int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_SMEM_ATTR(attn_bwd_dkv_tc5_kernel<DH>, C::SMEM_DKV);
   ORBIT_SMEM_ATTR(attn_bwd_dq_tc5_kernel<DH>, C::SMEM_DQ);
   const int total_w = a.B * a.heads * a.N;
-  attn_delta5_kernel<<<cdiv((long long)total_w * 32, 256), 256, 0, s>>>(a);
+  ORBIT_CUDA_CHECK(launch_pdl(attn_delta5_kernel, dim3(cdiv((long long)total_w * 32, 256)), dim3(256), 0, s, a));
   ORBIT_LAUNCH_CHECK();
   dim3 grid(cdiv(a.N, 128), a.B * a.heads);
   const float scale = 1.0f / sqrtf((float)DH);
-  attn_bwd_dq_tc5_kernel<DH><<<grid, NTHB, C::SMEM_DQ, s>>>(tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E);
+  ORBIT_CUDA_CHECK(launch_pdl(attn_bwd_dq_tc5_kernel<DH>, grid, dim3(NTHB), C::SMEM_DQ, s, tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E));
   ORBIT_LAUNCH_CHECK();
   dim3 grid_kv(cdiv(a.N, 128), a.B * a.heads, C::NSPLIT);
-  attn_bwd_dkv_tc5_kernel<DH><<<grid_kv, NTHB, C::SMEM_DKV, s>>>(tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E);
+  ORBIT_CUDA_CHECK(launch_pdl(attn_bwd_dkv_tc5_kernel<DH>, grid_kv, dim3(NTHB), C::SMEM_DKV, s, tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E));
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

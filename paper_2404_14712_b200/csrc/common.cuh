@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <atomic>
+#include <utility>
 #include "../../include/orbit.h"
 
 namespace orbit {
@@ -58,6 +59,28 @@ int num_sms();                   // multiprocessor count of the current device (
     static orbit::SmemAttrOnce _once;                                                            \
     ORBIT_TRY(orbit::smem_attr_once(_once, (const void*)(fn), (int)(nbytes)));                   \
   } while (0)
+
+// ---- programmatic dependent launch (PDL) -------------------------------------------------------------------
+// The block is a chain of 25-80 short dependent kernels; at C2 / C4 sizes the drain of one kernel plus the launch latency
+// and on-chip prologue (barrier init, TMEM allocation, tensor-map fetch) of the next is a few microseconds per link.  Kernels
+// launched through launch_pdl() may start while their predecessor is still running; they run their prologue, then
+// pdl_wait() (griddepcontrol.wait: returns once every prerequisite grid has completed and its writes are visible) BEFORE
+// their first global-memory access, then pdl_trigger() so that their own successor may be scheduled as soon as all their
+// CTAs are resident.  A kernel launched without the attribute (or after a memset) behaves as usual: the two
+// instructions are no-ops there.  ORBIT_PDL=0 disables the attribute (A/B).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+bool pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 
 #define ORBIT_TRY(expr)                                                                          \
   do {                                                                                           \
@@ -139,8 +162,19 @@ int gemm(const GemmArgs& g, cudaStream_t s);           // dispatcher (tensor-cor
 int gemm_simt(const GemmArgs& g, cudaStream_t s);      // fp32-FMA kernels, any dtype/stride
 int gemm_tc(const GemmArgs& g, cudaStream_t s);        // tcgen05 + TMA, bf16 in / fp32 accumulate
 bool gemm_tc_supported(const GemmArgs& g);
-int gemm_profile_enable(int on);
-int gemm_profile_collect(double* ms, double* flops, long long* launches);
+
+// ---- optional per-launch CUDA-event timing (bench.py's roofline legs) ------------------------------------------------
+// When switched on, a ProfScope records an event pair on the launching stream around the kernel(s) issued inside it, tagged
+// with a category and the algorithmic work of those launches (FLOPs for the tensor-bound categories, bytes for the
+// HBM-bound ones).  Single-threaded use (bench.py); off by default: the scope then costs one load.
+enum { PROF_GEMM = 0, PROF_ATTN_FWD = 1, PROF_ATTN_BWD = 2, PROF_LN = 3, PROF_FRONT = 4, PROF_NCAT = 5 };
+int prof_enable(int on);
+int prof_collect(int cat, double* ms, double* work, long long* launches);     // sums over the category; clears it
+struct ProfScope {
+  int slot; cudaStream_t s;
+  ProfScope(int cat, double work, cudaStream_t stream);
+  ~ProfScope();
+};
 
 // widest row the LayerNorm kernels take (backward: 4 chunks of 8 columns per thread, 512 threads); entry points reject
 // wider models with ORBIT_ERR_SHAPE before the first launch

@@ -76,6 +76,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  pdl_wait();                                    // only on-chip state and kernel parameters were touched above
+  pdl_trigger();
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -214,16 +216,6 @@ int make_map(CUtensorMap* m, const void* base, long long inner, long long outer,
   return ORBIT_OK;
 }
 
-// ---- optional per-launch CUDA-event timing of the tensor-core GEMM (bench.py's roofline leg) ----------------
-struct Prof {
-  bool on = false;
-  static constexpr int MAXP = 16384;
-  cudaEvent_t* ev = nullptr;     // 2 * MAXP events, created lazily
-  double* flops = nullptr;
-  int n = 0;
-};
-Prof g_prof;
-
 template <int A_MN, int B_MN, int BN>
 int launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, cudaStream_t s) {
   using Cf = TcCfg<BN>;
@@ -231,8 +223,8 @@ int launch(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, cuda
   const int batch = g.batch > 1 ? g.batch : 1;
   const long long tiles = (long long)cdiv(g.M, BM) * cdiv(g.N, BN) * batch;
   const int grid = tiles < num_sms() ? (int)tiles : num_sms();
-  gemm_tc_kernel<A_MN, B_MN, BN><<<grid, NTHREADS, Cf::SMEM_BYTES, s>>>(ma, mb, epi::from_gemm(g), g.M, g.N, g.K, batch,
-                                                                       g.c_bs, g.bias_bs);
+  ORBIT_CUDA_CHECK(launch_pdl(gemm_tc_kernel<A_MN, B_MN, BN>, dim3(grid), dim3(NTHREADS), Cf::SMEM_BYTES, s, ma, mb, epi::from_gemm(g),
+                              g.M, g.N, g.K, batch, g.c_bs, g.bias_bs));
   return ORBIT_OK;
 }
 template <int BN>
@@ -246,31 +238,6 @@ int launch_bn(const CUtensorMap& ma, const CUtensorMap& mb, const GemmArgs& g, b
 
 int gemm_tc2_launch(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc, const CUtensorMap* mx, const GemmArgs& g,
                     bool a_mn, bool b_mn, int sms, cudaStream_t s);   // gemm_tc2.cu
-
-int gemm_profile_enable(int on) {
-  if (on && !g_prof.ev) {
-    g_prof.ev = new cudaEvent_t[2 * Prof::MAXP];
-    g_prof.flops = new double[Prof::MAXP];
-    for (int i = 0; i < 2 * Prof::MAXP; i++) ORBIT_CUDA_CHECK(cudaEventCreate(&g_prof.ev[i]));
-  }
-  g_prof.on = on != 0;
-  g_prof.n = 0;
-  return ORBIT_OK;
-}
-int gemm_profile_collect(double* ms, double* flops, long long* launches) {
-  double t = 0, f = 0;
-  for (int i = 0; i < g_prof.n; i++) {
-    float e = 0.f;
-    ORBIT_CUDA_CHECK(cudaEventSynchronize(g_prof.ev[2 * i + 1]));
-    ORBIT_CUDA_CHECK(cudaEventElapsedTime(&e, g_prof.ev[2 * i], g_prof.ev[2 * i + 1]));
-    t += e; f += g_prof.flops[i];
-  }
-  if (ms) *ms = t;
-  if (flops) *flops = f;
-  if (launches) *launches = g_prof.n;
-  g_prof.n = 0;
-  return ORBIT_OK;
-}
 
 bool gemm_tc_supported(const GemmArgs& g) {
   if (g.in_dtype != ORBIT_BF16 || g.alpha != 1.f) return false;
@@ -319,15 +286,10 @@ int gemm_tc(const GemmArgs& g, cudaStream_t s) {
   if (store_map && store_f32) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 16, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B, 4));
   else if (store_map) ORBIT_TRY(make_map(&mc, g.C, g.N, g.M, g.ldc, 32, 32, g.batch, g.c_bs, CU_TENSOR_MAP_SWIZZLE_64B));
   if (aux_map) ORBIT_TRY(make_map(&mx, g.aux_out, g.N, g.M, g.ld_aux, 32, 32, 1, 0, CU_TENSOR_MAP_SWIZZLE_64B));
-  const bool rec = g_prof.on && g_prof.n < Prof::MAXP;
-  if (rec) ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n], s));
+  ProfScope prof(PROF_GEMM, 2.0 * g.M * g.N * g.K * (g.batch > 1 ? g.batch : 1), s);
   if (pair) ORBIT_TRY(gemm_tc2_launch(ma, mb, store_map ? &mc : nullptr, aux_map ? &mx : nullptr, g, a_mn, b_mn, num_sms(), s));
   else if (bn == 128) ORBIT_TRY(launch_bn<128>(ma, mb, g, a_mn, b_mn, s));
   else ORBIT_TRY(launch_bn<256>(ma, mb, g, a_mn, b_mn, s));
-  if (rec) {
-    ORBIT_CUDA_CHECK(cudaEventRecord(g_prof.ev[2 * g_prof.n + 1], s));
-    g_prof.flops[g_prof.n++] = 2.0 * g.M * g.N * g.K * (g.batch > 1 ? g.batch : 1);
-  }
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

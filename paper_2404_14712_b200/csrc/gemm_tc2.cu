@@ -112,6 +112,8 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  pdl_wait();                                    // everything above touched only on-chip state and kernel parameters
+  pdl_trigger();
 
   if (warp == 0) {
     // ===================== TMA producer (both CTAs) =====================
@@ -407,9 +409,9 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc,
     }
     if ((hm & 2) && bytes_c > 100e6) sc.hint_c = 1;
   }
-  gemm_tc2_kernel<A_MN, B_MN><<<2 * clusters, NTHREADS, SMEM_BYTES, s>>>(ma, mb, mc ? *mc : ma, mx ? *mx : ma,
-                                                                         (mc ? (g.out_dtype == ORBIT_F32 ? 4 : 1) : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,
-                                                                         g.bias_bs, sc);
+  ORBIT_CUDA_CHECK(launch_pdl(gemm_tc2_kernel<A_MN, B_MN>, dim3(2 * clusters), dim3(NTHREADS), SMEM_BYTES, s, ma, mb, mc ? *mc : ma,
+                              mx ? *mx : ma, (mc ? (g.out_dtype == ORBIT_F32 ? 4 : 1) : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,
+                              g.bias_bs, sc));
   return ORBIT_OK;
 }
 }  // namespace

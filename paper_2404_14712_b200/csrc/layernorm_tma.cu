@@ -38,6 +38,8 @@ template <int MAXCH>
 __global__ void __launch_bounds__(512, MAXCH >= 3 ? 2 : 1) ln_fwd_tma_kernel(const void* __restrict__ x, int x_dt, const void* __restrict__ gamma,
     const void* __restrict__ beta, int p_dt, void* __restrict__ out, int out_dt, float* __restrict__ mean,
     float* __restrict__ rstd, int M, int D, float eps, void* __restrict__ x_copy, int NS) {
+  pdl_wait();          // PDL (common.cuh): nothing above touches global memory
+  pdl_trigger();
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float slots[2][3 * SLOTS];
   __shared__ __align__(8) uint64_t full_bar[8];
@@ -133,6 +135,8 @@ __global__ void __launch_bounds__(512) ln_bwd_tma_kernel(const void* __restrict_
     const void* __restrict__ gamma, int p_dt, const void* __restrict__ add, int add_dt,
     float* __restrict__ dx_f32, void* __restrict__ dx_out, int out_dt,
     float* __restrict__ dgamma_acc, float* __restrict__ dbeta_acc, int M, int D, int NS, int add_direct) {
+  pdl_wait();          // PDL (common.cuh): nothing above touches global memory
+  pdl_trigger();
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float slots[2][2 * SLOTS];
   __shared__ __align__(8) uint64_t full_bar[8];
@@ -258,6 +262,8 @@ template <int R>
 __global__ void __launch_bounds__(512) ln_fwd_tma_rows_kernel(const void* __restrict__ x, int x_dt,
     const void* __restrict__ gamma, const void* __restrict__ beta, int p_dt, void* __restrict__ out, int out_dt,
     float* __restrict__ mean, float* __restrict__ rstd, int M, int D, float eps, void* __restrict__ x_copy, int NS) {
+  pdl_wait();          // PDL (common.cuh): nothing above touches global memory
+  pdl_trigger();
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float slots[2][R][3 * SLOTS];
   __shared__ __align__(8) uint64_t full_bar[8];
@@ -366,6 +372,8 @@ __global__ void __launch_bounds__(512) ln_bwd_tma_rows_kernel(const void* __rest
     const void* __restrict__ gamma, int p_dt, const void* __restrict__ add, int add_dt,
     float* __restrict__ dx_f32, void* __restrict__ dx_out, int out_dt,
     float* __restrict__ dgamma_acc, float* __restrict__ dbeta_acc, int M, int D, int NS) {
+  pdl_wait();          // PDL (common.cuh): nothing above touches global memory
+  pdl_trigger();
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float slots[2][R][2 * SLOTS];
   __shared__ __align__(8) uint64_t full_bar[8];
@@ -560,7 +568,7 @@ int layernorm_fwd_tma(const void* x, int x_dt, const void* gamma, const void* be
     shape(T, regs, (size_t)D * dsize(x_dt), 8, &per_sm, &NS, &smem);                                                 \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > M) grid = M;                                                                                          \
-    ln_fwd_tma_kernel<C><<<grid, T, smem, s>>>(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy, NS); \
+    ORBIT_CUDA_CHECK(launch_pdl(ln_fwd_tma_kernel<C>, dim3(grid), dim3(T), smem, s, x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy, NS)); \
   } while (0)
 #define LNFR(RR)                                                                                                     \
   do {                                                                                                               \
@@ -576,7 +584,7 @@ int layernorm_fwd_tma(const void* x, int x_dt, const void* gamma, const void* be
     shape(T, regs, (size_t)RR * D * dsize(x_dt), 8, &per_sm, &NS, &smem);                                            \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > cdiv(M, RR)) grid = cdiv(M, RR);                                                                      \
-    ln_fwd_tma_rows_kernel<RR><<<grid, T, smem, s>>>(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy, NS); \
+    ORBIT_CUDA_CHECK(launch_pdl(ln_fwd_tma_rows_kernel<RR>, dim3(grid), dim3(T), smem, s, x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy, NS)); \
   } while (0)
   if (MC == 1) {
     const int R = rows_per_stage((size_t)D * dsize(x_dt), M);
@@ -612,8 +620,8 @@ int layernorm_bwd_tma(const void* dout, int dout_dt, const void* x, int x_dt, co
     shape(T, regs, stage, 4, &per_sm, &NS, &smem);                                                                   \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > M) grid = M;                                                                                          \
-    ln_bwd_tma_kernel<C><<<grid, T, smem, s>>>(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, dx_f32, dx_out, \
-                                               out_dt, dgamma_acc, dbeta_acc, M, D, NS, add_direct);                 \
+    ORBIT_CUDA_CHECK(launch_pdl(ln_bwd_tma_kernel<C>, dim3(grid), dim3(T), smem, s, dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, \
+                                add_dt, dx_f32, dx_out, out_dt, dgamma_acc, dbeta_acc, M, D, NS, add_direct));        \
   } while (0)
 #define LNBR(RR)                                                                                                     \
   do {                                                                                                               \
@@ -629,8 +637,8 @@ int layernorm_bwd_tma(const void* dout, int dout_dt, const void* x, int x_dt, co
     shape(T, regs, (size_t)RR * stage, 4, &per_sm, &NS, &smem);                                                      \
     int grid = 148 * per_sm;                                                                                         \
     if (grid > cdiv(M, RR)) grid = cdiv(M, RR);                                                                      \
-    ln_bwd_tma_rows_kernel<RR><<<grid, T, smem, s>>>(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, dx_f32, dx_out, \
-                                                    out_dt, dgamma_acc, dbeta_acc, M, D, NS);                        \
+    ORBIT_CUDA_CHECK(launch_pdl(ln_bwd_tma_rows_kernel<RR>, dim3(grid), dim3(T), smem, s, dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, \
+                                add, add_dt, dx_f32, dx_out, out_dt, dgamma_acc, dbeta_acc, M, D, NS));               \
   } while (0)
   if (MC == 1) {
     const int R = rows_per_stage(stage, M);

@@ -204,6 +204,8 @@ __global__ void __launch_bounds__(TMAX) ln_bwd_kernel(const void* __restrict__ d
 __global__ void __launch_bounds__(256) colsum_kernel(const void* __restrict__ in, int in_dt, long long ld, int M,
     int N, float* __restrict__ acc, void* __restrict__ copy_out, int copy_dt, long long ld_copy,
     int rows_per_block) {
+  pdl_wait();
+  pdl_trigger();
   __shared__ float sh[8][32][9];
   const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
   const int col = (blockIdx.x * 32 + cx) * 8;
@@ -250,6 +252,8 @@ __global__ void cast_kernel(const void* __restrict__ in, int in_dt, void* __rest
 
 // several fp32 -> out_dt casts in one launch (the small parameter-gradient accumulators of a block backward)
 __global__ void cast_multi_kernel(CastSegs segs, int out_dt) {
+  pdl_wait();
+  pdl_trigger();
   const CastSeg sg = segs.s[blockIdx.y];
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < sg.n; i += (size_t)gridDim.x * blockDim.x)
     stf(sg.dst, i, sg.src[i], out_dt);
@@ -257,6 +261,8 @@ __global__ void cast_multi_kernel(CastSegs segs, int out_dt) {
 
 __global__ void add_partial_kernel(const void* __restrict__ a, int a_dt, const float* __restrict__ part,
     const void* __restrict__ bias, int p_dt, void* __restrict__ out, int out_dt, size_t n8, int D8) {
+  pdl_wait();
+  pdl_trigger();
   size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += stride) {
     float va[8], vp[8], vb[8], o[8];
@@ -300,6 +306,8 @@ int ln_threads(int D) {
 
 int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, int p_dt, void* out, int out_dt,
                   float* mean, float* rstd, int M, int D, float eps, void* x_copy, cudaStream_t s) {
+  // algorithmic bytes: read x, write out (+ the copy of x the backward needs)
+  ProfScope prof(PROF_LN, (double)M * D * (dsize(x_dt) + dsize(out_dt) + (x_copy ? dsize(x_dt) : 0)), s);
   if (ln_use_tma(D, x_dt, -1, 0, false)) return layernorm_fwd_tma(x, x_dt, gamma, beta, p_dt, out, out_dt, mean, rstd, M, D, eps, x_copy, s);
   int thr = ln_threads(D);
   int maxch = cdiv(D / 8, thr);
@@ -316,6 +324,9 @@ int layernorm_fwd(const void* x, int x_dt, const void* gamma, const void* beta, 
 int layernorm_bwd(const void* dout, int dout_dt, const void* x, int x_dt, const float* mean, const float* rstd,
                   const void* gamma, int p_dt, const void* add, int add_dt, float* dx_f32, void* dx_out,
                   int out_dt, float* dgamma_acc, float* dbeta_acc, int M, int D, cudaStream_t s) {
+  // algorithmic bytes: read dout, x (+ add), write dx in the requested forms
+  ProfScope prof(PROF_LN, (double)M * D * (dsize(dout_dt) + dsize(x_dt) + (add ? dsize(add_dt) : 0) + (dx_f32 ? 4 : 0) +
+                                           (dx_out ? dsize(out_dt) : 0)), s);
   if (ln_use_tma(D, x_dt, dout_dt, add_dt, add != nullptr))
     return layernorm_bwd_tma(dout, dout_dt, x, x_dt, mean, rstd, gamma, p_dt, add, add_dt, dx_f32, dx_out, out_dt, dgamma_acc,
                             dbeta_acc, M, D, s);
@@ -353,7 +364,7 @@ int colsum(const void* in, int in_dt, long long ld, int M, int N, float* acc, vo
   rows_per_block = ((rows_per_block + 7) / 8) * 8;
   if (rows_per_block < 8) rows_per_block = 8;
   dim3 grid(gx, cdiv(M, rows_per_block));
-  colsum_kernel<<<grid, 256, 0, s>>>(in, in_dt, ld, M, N, acc, copy_out, copy_dt, ld_copy, rows_per_block);
+  ORBIT_CUDA_CHECK(launch_pdl(colsum_kernel, grid, dim3(256), 0, s, in, in_dt, ld, M, N, acc, copy_out, copy_dt, ld_copy, rows_per_block));
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
@@ -375,7 +386,7 @@ int cast_multi(const CastSegs& segs, int out_dt, cudaStream_t s) {
   int gx = (int)((mx + 255) / 256);
   if (gx > 148) gx = 148;
   if (gx < 1) gx = 1;
-  cast_multi_kernel<<<dim3(gx, segs.count), 256, 0, s>>>(segs, out_dt);
+  ORBIT_CUDA_CHECK(launch_pdl(cast_multi_kernel, dim3(gx, segs.count), dim3(256), 0, s, segs, out_dt));
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }
@@ -400,7 +411,7 @@ int add_partial(const void* a, int a_dt, const float* part, const void* bias, in
   size_t n8 = (size_t)M * D / 8;
   size_t blocks = (n8 + 255) / 256;
   if (blocks > 148 * 8) blocks = 148 * 8;
-  add_partial_kernel<<<(int)blocks, 256, 0, s>>>(a, a_dt, part, bias, p_dt, out, out_dt, n8, D / 8);
+  ORBIT_CUDA_CHECK(launch_pdl(add_partial_kernel, dim3((int)blocks), dim3(256), 0, s, a, a_dt, part, bias, p_dt, out, out_dt, n8, D / 8));
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

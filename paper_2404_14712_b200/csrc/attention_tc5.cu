@@ -316,7 +316,14 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
 // A streamed [64 x d_h] tile is used twice from the same bytes: as a K-major B operand (contraction over d_h)
 // and as an MN-major B operand (contraction over its 64 rows).
 // =====================================================================================================
-constexpr int NTHB = 384;   // warp 0 TMA, warp 1 gradient MMAs, warps 2..9 softmax (two per TMEM lane quarter, BT / 2 columns each), warp 10 dP MMAs, warp 11 S MMAs
+// warp 0 TMA, warp 1 gradient MMAs, warps 2..17 softmax, warp 18 dP MMAs, warp 19 S MMAs.  The 16 softmax warps form two
+// groups of 8 (two per TMEM lane quarter, BT / 2 columns each); group g owns the tiles of parity g, i.e. the S / dP
+// accumulator buffer g and the operand-tile buffer g.  A tile's softmax is a serial chain (tcgen05.ld latency -> exponentials
+// -> shared-memory stores -> proxy fence -> barrier) of about a tile's MMA time; with one group that chain sat between the
+// S^T / dP^T products and the gradient products of every tile (tensor pipe 47-53 % active, profiles/r1_full_ncu.md); with
+// two groups the chains of consecutive tiles overlap.  The backward has no running maximum (logsumexp is saved), so tiles
+// are independent and the groups never exchange anything.
+constexpr int NTHB = 640;
 
 template <int DH>
 struct CfgB {
@@ -337,8 +344,9 @@ struct CfgB {
   // stages of the streamed (two-tile) ring: hide the TMA round trip.  The operand tiles written by the softmax warps
   // (P^T, dS^T resp. dS) are double buffered so that tile j+1 is written while the MMAs of tile j still read tile j.
   static constexpr int NST_DKV = DH == 256 ? 2 : 3, NST_DQ = DH == 256 ? 2 : 4;
-  static constexpr int SMEM_DKV = 2 * BIG + 2 * NST_DKV * SMALL + 4 * PT + 1024 /*stats*/ + 1024 + 256;
-  static constexpr int SMEM_DQ = 2 * BIG + 2 * NST_DQ * SMALL + 2 * PT + 1024 + 256;
+  // + statistics [2 groups][2 buffers][lse2 | delta][BT] floats, 256 bytes of alignment slack (see the kernels), barriers
+  static constexpr int SMEM_DKV = 2 * BIG + 2 * NST_DKV * SMALL + 4 * PT + 2048 /*stats*/ + 256 + 256;
+  static constexpr int SMEM_DQ = 2 * BIG + 2 * NST_DQ * SMALL + 2 * PT + 256 + 256;
   static_assert(SMEM_DKV <= 227 * 1024 && SMEM_DQ <= 227 * 1024, "attention backward: shared memory budget");
   static_assert(4 * BT + 2 * DHO <= 512 && 4 * BT + DH <= 512, "attention backward: TMEM budget");
 };
@@ -385,14 +393,22 @@ __device__ __forceinline__ void write_row16_sw64(uint32_t tile, int r, const flo
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
   }
 }
-// this warp's CW = BT / 2 columns of a row into the [128 x BT] operand tile
-template <int CW>
-__device__ __forceinline__ void write_row_half(uint32_t tile, int r, const float* v, int half) {
-  if (CW == 32) write_row32(tile, r, v, half); else write_row16_sw64(tile, r, v, half);
-}
-template <int CW>
-__device__ __forceinline__ void tmem_ld_cw(uint32_t taddr, uint32_t* v) {
-  if (CW == 32) ptx::tmem_ld_32x32(taddr, v); else ptx::tmem_ld_32x16(taddr, v);
+// 16 columns (two 16-byte chunks, column group g16 of the row) of a [128 x BT] K-major operand tile: 128-byte rows with 128B
+// swizzle at BT = 64, 64-byte rows with 64B swizzle at BT = 32
+template <int BT>
+__device__ __forceinline__ void write_cols16(uint32_t tile, int r, const float* v, int g16) {
+#pragma unroll
+  for (int c = 0; c < 2; c++) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      __nv_bfloat162 t2 = __floats2bfloat162_rn(v[c * 8 + 2 * i], v[c * 8 + 2 * i + 1]);
+      pk[i] = *reinterpret_cast<uint32_t*>(&t2);
+    }
+    const uint32_t addr = BT == 64 ? tile + r * 128 + (((g16 * 2 + c) ^ (r & 7)) << 4)
+                                   : tile + r * 64 + (((g16 * 2 + c) ^ ((r >> 1) & 3)) << 4);
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+  }
 }
 // K-major descriptor of a [128 x BT] operand tile
 template <int BT>
@@ -431,13 +447,14 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
   using C = CfgB<DH>;
   constexpr int BT = C::BT, CW = BT / 2, DHO = C::DHO;       // streamed rows; columns per softmax warp; dK / dV columns of this CTA
   const int slice = blockIdx.z;                              // which DHO-column slice of dK / dV (d_h = 256: two)
-  extern __shared__ uint8_t smem_raw[];
+  extern __shared__ __align__(1024) uint8_t smem_raw[];     // see attn_fwd_tc5_kernel: 256 bytes of slack budgeted, fail loudly beyond
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  if (base - ptx::smem_u32(smem_raw) > 256u) __trap();
   const uint32_t sK = base, sV = sK + C::BIG, sRing = sV + C::BIG, sPt0 = sRing + 2 * C::NST_DKV * C::SMALL,
-                 sStat = sPt0 + 4 * C::PT, bar = sStat + 1024;
+                 sStat = sPt0 + 4 * C::PT, bar = sStat + 2048;
   auto sQ = [&](int st) { return sRing + st * 2 * C::SMALL; };
   auto sdO = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
-  float* stat = reinterpret_cast<float*>(smem_raw + (sStat - ptx::smem_u32(smem_raw)));   // [2][2][BT]
+  float* stat = reinterpret_cast<float*>(smem_raw + (sStat - ptx::smem_u32(smem_raw)));   // [2 groups][2 uses][lse2 | delta][BT]
   constexpr int NST = C::NST_DKV;
   const uint32_t kv_full = bar, qdo_full0 = bar + 8, qdo_empty0 = qdo_full0 + 8 * NST, st_full0 = qdo_empty0 + 8 * NST,
                  st_empty0 = st_full0 + 16, p_full0 = st_empty0 + 16, p_done0 = p_full0 + 16, tmem_slot = p_done0 + 16;
@@ -537,58 +554,69 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
       }
     }
   } else {
-    const int quarter = warp & 3, half = (warp - 2) >> 2;     // this warp: 32 key rows x CW of the tile's BT query columns
+    const int sw = warp - 2, grp = sw >> 3;                  // softmax warp 0..15; group = parity of the tiles it works on
+    const int quarter = warp & 3, half = (sw & 7) >> 2;      // this warp: 32 key rows x CW of the tile's BT query columns
     const int r = quarter * 32 + lane;                       // key row within the CTA tile = TMEM lane
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
-    const int gi = threadIdx.x - 64;                         // 0..255: the first 128 load the statistics
+    const int gi = (sw & 7) * 32 + lane;                     // 0..255 within the group: the first 2 BT load the statistics
     auto load_stat = [&](int j) -> float {
       const int q = j * BT + (gi % BT);
       if (gi >= 2 * BT || j >= ntiles || q >= N) return 0.f;
       return (gi / BT) ? a.delta[(size_t)bh * N + q] : a.lse[(size_t)bh * N + q] * LOG2E;
     };
-    float nxt = load_stat(0);
-    for (int j = 0; j < ntiles; j++) {
-      const int st = j & 1;
-      if (gi < 2 * BT) stat[st * 2 * BT + gi] = nxt;         // [st][0][c] = lse2, [st][1][c] = delta
-      named_bar_sync(1, 256);
-      nxt = load_stat(j + 1);
-      const float* lse2 = stat + st * 2 * BT + half * CW;
+    float nxt = load_stat(grp);
+    for (int j = grp; j < ntiles; j += 2) {
+      const int st = grp;                                    // accumulator / operand-tile buffer of this group (= j & 1)
+      float* sbuf = stat + (grp * 2 + ((j >> 1) & 1)) * 2 * BT;   // [group][use parity][0][c] = lse2, [..][1][c] = delta
+      if (gi < 2 * BT) sbuf[gi] = nxt;
+      named_bar_sync(1 + grp, 256);                          // a buffer is rewritten two barriers of the group later
+      nxt = load_stat(j + 2);
+      const float* lse2 = sbuf + half * CW;
       const float* dl = lse2 + BT;
       ptx::mbar_wait(st_full0 + 8 * st, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[CW], dp[CW];
-      tmem_ld_cw<CW>(tSt + st * BT + half * CW + lane_off, s);
-      tmem_ld_cw<CW>(tdPt + st * BT + half * CW + lane_off, dp);
-      ptx::tmem_ld_wait();
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(st_empty0 + 8 * st);
-      float p[CW];
-      const int nvalid = N - j * BT - half * CW;             // queries (columns) >= N are masked
-      if (nvalid >= CW) {                                   // masking only in the ragged last tile (warp-uniform branch)
-#pragma unroll
-        for (int c = 0; c < CW; c++) p[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]);
-      } else {
-#pragma unroll
-        for (int c = 0; c < CW; c++) p[c] = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[c]) : 0.f;
-      }
       const uint32_t sPt = sPt0 + st * 2 * C::PT, sdSt = sPt + C::PT;
-      if (j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);   // this buffer's P^T / dS^T tiles are free again
-      write_row_half<CW>(sPt, r, p, half);
+      const int nvalid = N - j * BT - half * CW;             // queries (columns) >= N are masked (ragged last tile only)
 #pragma unroll
-      for (int c = 0; c < CW; c++) p[c] *= __uint_as_float(dp[c]) - dl[c];
-      write_row_half<CW>(sdSt, r, p, half);
+      for (int g = 0; g < CW / 16; g++) {                    // 16 columns at a time: 48 live values instead of 96
+        uint32_t s[16], dp[16];
+        ptx::tmem_ld_32x16(tSt + st * BT + half * CW + g * 16 + lane_off, s);
+        ptx::tmem_ld_32x16(tdPt + st * BT + half * CW + g * 16 + lane_off, dp);
+        ptx::tmem_ld_wait();
+        if (g == CW / 16 - 1) {                              // both accumulators of this tile are in registers
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(st_empty0 + 8 * st);
+        }
+        float p[16];
+#pragma unroll
+        for (int c = 0; c < 16; c++) {
+          const float e = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[g * 16 + c]);
+          p[c] = (g * 16 + c < nvalid) ? e : 0.f;
+        }
+        if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);   // this buffer's P^T / dS^T tiles are free again
+        write_cols16<BT>(sPt, r, p, half * (CW / 16) + g);
+#pragma unroll
+        for (int c = 0; c < 16; c++) p[c] *= __uint_as_float(dp[c]) - dl[g * 16 + c];
+        write_cols16<BT>(sdSt, r, p, half * (CW / 16) + g);
+      }
       ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);
     }
-    ptx::mbar_wait(p_done0 + 8 * ((ntiles - 1) & 1), ((ntiles - 1) >> 1) & 1);
-    ptx::tc_fence_after();
-    const int krow = k0 + r;
-    bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld + slice * DHO + half * (DHO / 2);
-    store_acc_row<DHO / 2>(tdV + half * (DHO / 2) + lane_off, out + vc, 1.f, krow < N);
-    store_acc_row<DHO / 2>(tdK + half * (DHO / 2) + lane_off, out + kc, scale, krow < N);
+    // every group waits for the gradient MMAs of ITS OWN last tile (a barrier whose phases it has followed one by one:
+    // a group that never waited on the other buffer's barrier could not tell its phase k from phase k - 2), then the two
+    // groups meet, and the first one drains the accumulators
+    if (ntiles > grp) { const int jl = ((ntiles - 1 - grp) & ~1) + grp; ptx::mbar_wait(p_done0 + 8 * grp, (jl >> 1) & 1); }
+    named_bar_sync(3, 512);
+    if (grp == 0) {                                          // epilogue: DHO / 2 columns of both gradients per warp
+      ptx::tc_fence_after();
+      const int krow = k0 + r;
+      bf16* out = (bf16*)a.dqkv + (size_t)(row0 + krow) * a.ld + slice * DHO + half * (DHO / 2);
+      store_acc_row<DHO / 2>(tdV + half * (DHO / 2) + lane_off, out + vc, 1.f, krow < N);
+      store_acc_row<DHO / 2>(tdK + half * (DHO / 2) + lane_off, out + kc, scale, krow < N);
+    }
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -602,8 +630,9 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
                        const __grid_constant__ CUtensorMap tmdOBig, AttnArgs a, float scale, float sl2) {
   using C = CfgB<DH>;
   constexpr int BT = C::BT, CW = BT / 2;
-  extern __shared__ uint8_t smem_raw[];
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  if (base - ptx::smem_u32(smem_raw) > 256u) __trap();
   const uint32_t sQ = base, sdO = sQ + C::BIG, sRing = sdO + C::BIG, sdS0 = sRing + 2 * C::NST_DQ * C::SMALL, bar = sdS0 + 2 * C::PT;
   auto sK = [&](int st) { return sRing + st * 2 * C::SMALL; };
   auto sV = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
@@ -700,46 +729,50 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
       }
     }
   } else {
-    const int quarter = warp & 3, half = (warp - 2) >> 2;     // 32 query rows x CW of the tile's BT key columns
+    const int sw = warp - 2, grp = sw >> 3;                  // two groups of 8 warps alternate over the tiles (see NTHB)
+    const int quarter = warp & 3, half = (sw & 7) >> 2;      // 32 query rows x CW of the tile's BT key columns
     const int r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     const int qrow = q0 + r;
     const float lse2 = qrow < N ? a.lse[(size_t)bh * N + qrow] * LOG2E : 0.f;
     const float dl = qrow < N ? a.delta[(size_t)bh * N + qrow] : 0.f;
-    for (int j = 0; j < ntiles; j++) {
-      const int st = j & 1;
+    for (int j = grp; j < ntiles; j += 2) {
+      const int st = grp;
       ptx::mbar_wait(s_full0 + 8 * st, (j >> 1) & 1);
       ptx::tc_fence_after();
-      uint32_t s[CW], dp[CW];
-      tmem_ld_cw<CW>(tS + st * BT + half * CW + lane_off, s);
-      tmem_ld_cw<CW>(tdP + st * BT + half * CW + lane_off, dp);
-      ptx::tmem_ld_wait();
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
-      float ds[CW];
-      const int nvalid = N - j * BT - half * CW;             // keys (columns) >= N are masked
-      if (nvalid >= CW) {                                   // masking only in the ragged last tile (warp-uniform branch)
+      const int nvalid = N - j * BT - half * CW;             // keys (columns) >= N are masked (ragged last tile only)
 #pragma unroll
-        for (int c = 0; c < CW; c++) ds[c] = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) * (__uint_as_float(dp[c]) - dl);
-      } else {
-#pragma unroll
-        for (int c = 0; c < CW; c++) {
-          const float p = (c < nvalid) ? fast_ex2(__uint_as_float(s[c]) * sl2 - lse2) : 0.f;
-          ds[c] = p * (__uint_as_float(dp[c]) - dl);
+      for (int g = 0; g < CW / 16; g++) {
+        uint32_t s[16], dp[16];
+        ptx::tmem_ld_32x16(tS + st * BT + half * CW + g * 16 + lane_off, s);
+        ptx::tmem_ld_32x16(tdP + st * BT + half * CW + g * 16 + lane_off, dp);
+        ptx::tmem_ld_wait();
+        if (g == CW / 16 - 1) {
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
         }
+        float ds[16];
+#pragma unroll
+        for (int c = 0; c < 16; c++) {
+          const float pv = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2);
+          ds[c] = (g * 16 + c < nvalid) ? pv * (__uint_as_float(dp[c]) - dl) : 0.f;
+        }
+        if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
+        write_cols16<BT>(sdS0 + st * C::PT, r, ds, half * (CW / 16) + g);
       }
-      if (j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
-      write_row_half<CW>(sdS0 + st * C::PT, r, ds, half);
       ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);
     }
-    ptx::mbar_wait(p_done0 + 8 * ((ntiles - 1) & 1), ((ntiles - 1) >> 1) & 1);
-    ptx::tc_fence_after();
-    store_acc_row<DH / 2>(tdQ + half * (DH / 2) + lane_off,
-                          (bf16*)a.dqkv + (size_t)(row0 + qrow) * a.ld + qc + half * (DH / 2), scale, qrow < N);
+    if (ntiles > grp) { const int jl = ((ntiles - 1 - grp) & ~1) + grp; ptx::mbar_wait(p_done0 + 8 * grp, (jl >> 1) & 1); }
+    named_bar_sync(3, 512);                                  // see the dK / dV kernel
+    if (grp == 0) {
+      ptx::tc_fence_after();
+      store_acc_row<DH / 2>(tdQ + half * (DH / 2) + lane_off,
+                            (bf16*)a.dqkv + (size_t)(row0 + qrow) * a.ld + qc + half * (DH / 2), scale, qrow < N);
+    }
   }
   ptx::tc_fence_before();
   __syncthreads();

@@ -324,6 +324,16 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
 // two groups the chains of consecutive tiles overlap.  The backward has no running maximum (logsumexp is saved), so tiles
 // are independent and the groups never exchange anything.
 constexpr int NTHB = 640;
+// TS_DKV: in the dK / dV kernel the operand tiles P^T and dS^T stay in TENSOR MEMORY (tcgen05.mma with the A operand in
+// TMEM), written by the softmax threads with tcgen05.st over the S^T / dP^T columns they have just read (16 fp32 columns
+// -> 8 columns of packed bf16 pairs, in place).  The kernels were shared-memory-bandwidth bound: per 64-query tile the
+// MMAs read 160 KB of operands from shared memory, the softmax warps wrote 32 KB of operand tiles and TMA 32 KB of Q / dO,
+// i.e. 224 KB = 1750 cycles at 128 B/clk against 1024 cycles of MMA; without the operand tiles (written and read once
+// each) it is 160 KB.  A buffer of S^T / dP^T is then free only once the gradient MMAs that read it have completed.
+constexpr bool TS_DKV = true;
+// the same for dS in the dQ kernel measured no gain (C5: attention backward 417 vs 423-429 TFLOP/s of model FLOPs): that
+// kernel has one operand tile, not two, and releasing its S / dP buffer only after the dQ product costs the overlap back
+constexpr bool TS_DQ = false;
 
 template <int DH>
 struct CfgB {
@@ -469,7 +479,9 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdO);
     ptx::mbar_init(kv_full, 1);
     for (int i = 0; i < NST; i++) { ptx::mbar_init(qdo_full0 + 8 * i, 1); ptx::mbar_init(qdo_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(st_full0 + 8 * i, 2);  ptx::mbar_init(st_empty0 + 8 * i, 8); }
+    // st_empty: released by the 8 softmax warps once S^T / dP^T are in registers, or (TS_DKV: the operands live in those
+    // columns) by the commit of the gradient MMAs that read them
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(st_full0 + 8 * i, 2);  ptx::mbar_init(st_empty0 + 8 * i, TS_DKV ? 1 : 8); }
     for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
@@ -543,12 +555,22 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         // streamed tiles as MN-major B operands: this CTA's DHO columns start (slice * DHO / 64) blocks in
         const uint32_t so = slice * (DHO / 64) * C::SBLK;
         const uint64_t dOm = ptx::make_smem_desc(sdO(st) + so, C::SBLK, 1024), dQm = ptx::make_smem_desc(sQ(st) + so, C::SBLK, 1024);
+        if (TS_DKV) {                             // A operands in TMEM: k-step ks (16 queries) = 8 columns at offset 16 ks of the buffer
 #pragma unroll
-        for (int ks = 0; ks < BT / 16; ks++)      // dV += P^T dO_j   (contraction over the tile's 64 queries)
-          ptx::mma_f16_ss(tdV, desc_adv(dPt, ks * 32), desc_adv(dOm, ks * 2048), idesc_g, (j | ks) != 0);
+          for (int ks = 0; ks < BT / 16; ks++)    // dV += P^T dO_j   (contraction over the tile's queries)
+            ptx::mma_f16_ts(tdV, tSt + pb * BT + ks * 16, desc_adv(dOm, ks * 2048), idesc_g, (j | ks) != 0);
 #pragma unroll
-        for (int ks = 0; ks < BT / 16; ks++)      // dK += dS^T Q_j
-          ptx::mma_f16_ss(tdK, desc_adv(dSt, ks * 32), desc_adv(dQm, ks * 2048), idesc_g, (j | ks) != 0);
+          for (int ks = 0; ks < BT / 16; ks++)    // dK += dS^T Q_j
+            ptx::mma_f16_ts(tdK, tdPt + pb * BT + ks * 16, desc_adv(dQm, ks * 2048), idesc_g, (j | ks) != 0);
+          ptx::mma_commit(st_empty0 + 8 * pb);    // the S^T / dP^T columns of this buffer may be overwritten
+        } else {
+#pragma unroll
+          for (int ks = 0; ks < BT / 16; ks++)    // dV += P^T dO_j   (contraction over the tile's 64 queries)
+            ptx::mma_f16_ss(tdV, desc_adv(dPt, ks * 32), desc_adv(dOm, ks * 2048), idesc_g, (j | ks) != 0);
+#pragma unroll
+          for (int ks = 0; ks < BT / 16; ks++)    // dK += dS^T Q_j
+            ptx::mma_f16_ss(tdK, desc_adv(dSt, ks * 32), desc_adv(dQm, ks * 2048), idesc_g, (j | ks) != 0);
+        }
         ptx::mma_commit(qdo_empty0 + 8 * st);
         ptx::mma_commit(p_done0 + 8 * pb);
       }
@@ -583,7 +605,7 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
         ptx::tmem_ld_32x16(tSt + st * BT + half * CW + g * 16 + lane_off, s);
         ptx::tmem_ld_32x16(tdPt + st * BT + half * CW + g * 16 + lane_off, dp);
         ptx::tmem_ld_wait();
-        if (g == CW / 16 - 1) {                              // both accumulators of this tile are in registers
+        if (!TS_DKV && g == CW / 16 - 1) {                   // both accumulators of this tile are in registers
           ptx::tc_fence_before();
           __syncwarp();
           if (lane == 0) ptx::mbar_arrive(st_empty0 + 8 * st);
@@ -594,13 +616,28 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
           const float e = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2[g * 16 + c]);
           p[c] = (g * 16 + c < nvalid) ? e : 0.f;
         }
-        if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);   // this buffer's P^T / dS^T tiles are free again
-        write_cols16<BT>(sPt, r, p, half * (CW / 16) + g);
+        if (TS_DKV) {
+          // P^T / dS^T of these 16 queries as 8 columns of packed bf16 pairs over the first half of the 16 fp32 columns
+          // just read (this thread's own lane and columns: no other thread reads or writes them)
+          const uint32_t c0 = st * BT + half * CW + g * 16 + lane_off;
+          uint32_t pk[8];
 #pragma unroll
-        for (int c = 0; c < 16; c++) p[c] *= __uint_as_float(dp[c]) - dl[g * 16 + c];
-        write_cols16<BT>(sdSt, r, p, half * (CW / 16) + g);
+          for (int i = 0; i < 8; i++) { __nv_bfloat162 t2 = __floats2bfloat162_rn(p[2 * i], p[2 * i + 1]); pk[i] = *reinterpret_cast<uint32_t*>(&t2); }
+          ptx::tmem_st_32x8(tSt + c0, pk);
+#pragma unroll
+          for (int c = 0; c < 16; c++) p[c] *= __uint_as_float(dp[c]) - dl[g * 16 + c];
+#pragma unroll
+          for (int i = 0; i < 8; i++) { __nv_bfloat162 t2 = __floats2bfloat162_rn(p[2 * i], p[2 * i + 1]); pk[i] = *reinterpret_cast<uint32_t*>(&t2); }
+          ptx::tmem_st_32x8(tdPt + c0, pk);
+        } else {
+          if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);   // this buffer's P^T / dS^T tiles are free again
+          write_cols16<BT>(sPt, r, p, half * (CW / 16) + g);
+#pragma unroll
+          for (int c = 0; c < 16; c++) p[c] *= __uint_as_float(dp[c]) - dl[g * 16 + c];
+          write_cols16<BT>(sdSt, r, p, half * (CW / 16) + g);
+        }
       }
-      ptx::fence_proxy_async();
+      if (TS_DKV) ptx::tmem_st_wait(); else ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);
@@ -650,7 +687,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdOBig);
     ptx::mbar_init(q_full, 1);
     for (int i = 0; i < NST; i++) { ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 2);  ptx::mbar_init(s_empty0 + 8 * i, 8); }
+    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 2);  ptx::mbar_init(s_empty0 + 8 * i, TS_DQ ? 1 : 8); }   // as in the dK / dV kernel
     for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
@@ -721,9 +758,16 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::tc_fence_after();
         const int st = j % NST;
         const uint64_t dSd = optile_desc<BT>(sdS), dKm = ptx::make_smem_desc(sK(st), C::SBLK, 1024);
+        if (TS_DQ) {                             // dS stays in TMEM over the dP columns (A operand from tensor memory)
 #pragma unroll
-        for (int ks = 0; ks < BT / 16; ks++)      // dQ += dS K_j   (contraction over the tile's 64 keys)
-          ptx::mma_f16_ss(tdQ, desc_adv(dSd, ks * 32), desc_adv(dKm, ks * 2048), idesc_g, (j | ks) != 0);
+          for (int ks = 0; ks < BT / 16; ks++)    // dQ += dS K_j   (contraction over the tile's keys)
+            ptx::mma_f16_ts(tdQ, tdP + pb * BT + ks * 16, desc_adv(dKm, ks * 2048), idesc_g, (j | ks) != 0);
+          ptx::mma_commit(s_empty0 + 8 * pb);
+        } else {
+#pragma unroll
+          for (int ks = 0; ks < BT / 16; ks++)    // dQ += dS K_j   (contraction over the tile's 64 keys)
+            ptx::mma_f16_ss(tdQ, desc_adv(dSd, ks * 32), desc_adv(dKm, ks * 2048), idesc_g, (j | ks) != 0);
+        }
         ptx::mma_commit(kv_empty0 + 8 * st);
         ptx::mma_commit(p_done0 + 8 * pb);
       }
@@ -747,7 +791,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         ptx::tmem_ld_32x16(tS + st * BT + half * CW + g * 16 + lane_off, s);
         ptx::tmem_ld_32x16(tdP + st * BT + half * CW + g * 16 + lane_off, dp);
         ptx::tmem_ld_wait();
-        if (g == CW / 16 - 1) {
+        if (!TS_DQ && g == CW / 16 - 1) {
           ptx::tc_fence_before();
           __syncwarp();
           if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
@@ -758,10 +802,17 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
           const float pv = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2);
           ds[c] = (g * 16 + c < nvalid) ? pv * (__uint_as_float(dp[c]) - dl) : 0.f;
         }
-        if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
-        write_cols16<BT>(sdS0 + st * C::PT, r, ds, half * (CW / 16) + g);
+        if (TS_DQ) {
+          uint32_t pk[8];
+#pragma unroll
+          for (int i = 0; i < 8; i++) { __nv_bfloat162 t2 = __floats2bfloat162_rn(ds[2 * i], ds[2 * i + 1]); pk[i] = *reinterpret_cast<uint32_t*>(&t2); }
+          ptx::tmem_st_32x8(tdP + st * BT + half * CW + g * 16 + lane_off, pk);
+        } else {
+          if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
+          write_cols16<BT>(sdS0 + st * C::PT, r, ds, half * (CW / 16) + g);
+        }
       }
-      ptx::fence_proxy_async();
+      if (TS_DQ) ptx::tmem_st_wait(); else ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);

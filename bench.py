@@ -472,6 +472,37 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+def run_hbm_probe():
+    """Write-only, read-only and copy bandwidth of this GPU's HBM (torch fills / reductions / copies of 3 GiB buffers, best of
+    10, CUDA events): the ceilings of kernels that only write (orbit_tokenize) or only read (orbit_tokenize_bwd) a large
+    tensor.  MEASURED_PEAKS.json's hbm_gbs is the COPY figure (read + write bytes).  profiles/r2_hbm_probe.md."""
+    import torch
+    torch.cuda.set_device(0)
+    n = 3 << 28                                               # 3 Gi bf16 elements... as int32: 3 GiB
+    a = torch.empty(n, dtype=torch.int32, device="cuda")
+    b = torch.empty(n, dtype=torch.int32, device="cuda")
+    nbytes = n * 4
+
+    def best(fn, moved):
+        ts = []
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return moved / (min(ts) * 1e-3) / 1e9
+    a.zero_(); b.zero_(); torch.cuda.synchronize()
+    out = {"probe": "hbm", "buffer_bytes": nbytes,
+           "write_only_gbs": best(lambda: a.zero_(), nbytes),
+           "write_only_fill_gbs": best(lambda: a.fill_(7), nbytes),
+           "read_only_gbs": best(lambda: a.sum(), nbytes),
+           "copy_gbs": best(lambda: b.copy_(a), 2 * nbytes),
+           "how": "torch zero_ / fill_ / sum / copy_ on 3 GiB int32 buffers, best of 10, CUDA events; copy counts read + write bytes"}
+    pk = measured_peaks()
+    out["measured_peaks_hbm_gbs"] = pk["hbm"]
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -489,7 +520,12 @@ def main():
                          "the headline value and the roofline leg stay un-captured)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--debug-mode", type=int, default=0, help="kernel-variant switch of the A/B build (ORBIT_DEBUG_SWITCH=1 build, ORBIT_LIB=dbg); never set by the default run")
+    ap.add_argument("--hbm-probe", action="store_true",
+                    help="print the write-only / read-only / copy HBM bandwidth of cuda:0 (JSON) and exit")
     args = ap.parse_args()
+    if args.hbm_probe:
+        run_hbm_probe()
+        return
     cfg = syn.CONFIGS[args.workload]
     if args.impl == "reference":
         run_reference(args, cfg)

@@ -49,6 +49,8 @@ def build(force: bool = False, verbose: bool = True, debug_switch: bool | None =
     bdir = os.path.join(CSRC, "build_dbg" if debug_switch else "build")
     out = os.path.join(HERE, "liborbit_dbg.so") if debug_switch else OUT
     extra = ["-DORBIT_DEBUG_SWITCH"] if debug_switch else []
+    if debug_switch:                               # measurement probes of the A/B build only, e.g. ORBIT_NVCC_EXTRA=-DORBIT_PROBE_NOEXP
+        extra += os.environ.get("ORBIT_NVCC_EXTRA", "").split()
     os.makedirs(bdir, exist_ok=True)
     hm = _headers_mtime()
     todo, objs = [], []

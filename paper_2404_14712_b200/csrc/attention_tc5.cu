@@ -15,6 +15,11 @@
 // the critical path: 128 MUFU.EX2 per row and tile = ~1024 cycles of the sub-partition's quarter-rate unit, plus the
 // serial tcgen05.ld / fence.proxy.async / barrier latencies of a tile.  Tried and measured no faster: a max-only warp
 // running one tile ahead of an exp-only warp (291 us vs 284), P packed by truncation instead of cvt (311 us).
+// Round-2 probes (A/B build, C4, per-launch CUDA events): with the exponentials removed (ORBIT_PROBE_NOEXP) 54.0 -> 54.7 us, with
+// half of the tcgen05.ld traffic removed (ORBIT_PROBE_HALFLD) 52.0 us, with the K / V tiles TMA-multicast across a cluster of two
+// query tiles (half the L2 -> SM traffic) 54 -> 58 us: none of MUFU, TMEM reads or L2 bandwidth bounds the kernel; what is
+// left is the serial per-tile chain of barrier hand-offs between the three agents and the per-CTA prologue / epilogue (one CTA
+// per SM, ~5 us of a 27 us CTA at C5).
 // S_{j+1} is issued before the softmax of tile j finishes, so the tensor pipe overlaps the exponentials.
 // V tiles are consumed as an MN-major B operand straight from their row-major [keys, d] layout.
 #include <cuda.h>
@@ -32,9 +37,13 @@ constexpr float LN2 = 0.6931471805599453f;
 // one MUFU.EX2 (ex2.approx.ftz): exp2f() adds a range fix-up of ~5 instructions per element, which made the softmax
 // warps issue-bound; the arguments here are <= 8 and results below 2^-126 may flush to zero
 __device__ __forceinline__ float fast_ex2(float x) {
+#ifdef ORBIT_PROBE_NOEXP       // measurement probe (A/B build only, ORBIT_NVCC_EXTRA): no MUFU work, wrong results
+  return x * 0.001f;
+#else
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+#endif
 }
 
 // descriptor of the same tile `bytes` further on: the start-address field (bits [0,14), in 16-byte units) never carries
@@ -195,7 +204,12 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       constexpr int HC = BKV / 2;                             // key columns of this warp
       uint32_t s[HC];
 #pragma unroll
+#ifdef ORBIT_PROBE_HALFLD      // measurement probe (A/B build only): half of the tcgen05.ld traffic, wrong results
+      ptx::tmem_ld_32x32(tS0 + sb * BKV + half * HC + lane_off, s);
+      if (HC == 64) { ptx::tmem_ld_wait(); for (int c = 0; c < 32; c++) s[32 + c] = s[c]; }
+#else
       for (int c = 0; c < HC / 32; c++) ptx::tmem_ld_32x32(tS0 + sb * BKV + half * HC + c * 32 + lane_off, s + c * 32);
+#endif
       ptx::tmem_ld_wait();
       ptx::tc_fence_before();
       __syncwarp();

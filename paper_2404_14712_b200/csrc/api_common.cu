@@ -7,6 +7,7 @@
 #include "orbit_debug.h"
 
 namespace orbit {
+int attention_probe_read(unsigned long long* out, int n, int reset);   // attention_tc5.cu (probe build only)
 
 static thread_local char g_err[512] = "";
 thread_local long long g_launches = 0;
@@ -141,6 +142,9 @@ long long orbit_launch_count(void) { return g_launches; }
 void orbit_reset_launch_count(void) { g_launches = 0; }
 #ifdef ORBIT_DEBUG_SWITCH
 void orbit_set_debug_force_simt(int on) { g_force_simt = on; }   // csrc/orbit_debug.h; not part of include/orbit.h
+#ifdef ORBIT_PROBE_TIMELINE
+int orbit_debug_read_probe(unsigned long long* out, int n, int reset) { return orbit::attention_probe_read(out, n, reset); }
+#endif
 #endif
 
 // ------------------------------------------------------------------------------------------------------

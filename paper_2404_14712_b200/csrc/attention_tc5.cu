@@ -30,6 +30,24 @@ namespace orbit {
 namespace {
 
 constexpr int BQ = 128;
+
+// ---- timeline probe of the forward kernel (A/B build with ORBIT_NVCC_EXTRA=-DORBIT_PROBE_TIMELINE only) ---------------------
+// Cycles the three agents of CTA (0, 0) spend in each mbarrier wait, summed over its tiles, read back with
+// orbit_debug_read_probe (csrc/orbit_debug.h).  Slots: 0 producer k_empty, 1 producer v_empty, 2 mma k_full, 3 mma s_empty,
+// 4 mma v_full, 5 mma p_full[0], 6 mma p_full[1], 7 softmax s_full, 8 softmax o_done (rescale), 9 softmax p_free, 10 softmax
+// loop total, 11 mma loop total, 12 tiles, 13 producer loop total, 14 softmax pair barrier, 15 softmax final o_done wait.
+#ifdef ORBIT_PROBE_TIMELINE
+__device__ unsigned long long g_attn_probe[32];
+#define PROBE_DECL long long pw_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}; const bool pon_ = blockIdx.x == 0 && blockIdx.y == 0
+#define PWAIT(slot, bar, par) do { long long t0_ = clock64(); ptx::mbar_wait(bar, par); pw_[slot] += clock64() - t0_; } while (0)
+#define PTIME(slot, stmt) do { long long t0_ = clock64(); stmt; pw_[slot] += clock64() - t0_; } while (0)
+#define PFLUSH(a, b) do { if (pon_) for (int i_ = a; i_ <= b; i_++) atomicAdd(&g_attn_probe[i_], (unsigned long long)pw_[i_]); } while (0)
+#else
+#define PROBE_DECL
+#define PWAIT(slot, bar, par) ptx::mbar_wait(bar, par)
+#define PTIME(slot, stmt) stmt
+#define PFLUSH(a, b)
+#endif
 constexpr int NTH = 320;   // forward: warp 0 TMA, warp 1 MMA issuer, warps 2..9 softmax (two per TMEM lane quarter, 64 key columns each)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
@@ -120,6 +138,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
   pdl_trigger();
   const uint32_t tS0 = tmem, tO = tmem + 2 * BKV;
 
+  PROBE_DECL;
   if (warp == 0) {
     if (lane == 0) {
       ptx::mbar_expect_tx(q_full, C::QTILE);
@@ -127,7 +146,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sQ + bk * C::QBLK, &tmQKV, q_full, qc + bk * 64, row0 + q0);
       auto load_k = [&](int j) {
         const int st = j % KST;
-        ptx::mbar_wait(k_empty0 + 8 * st, ((j / KST) & 1) ^ 1);
+        PWAIT(0, k_empty0 + 8 * st, ((j / KST) & 1) ^ 1);
         ptx::mbar_expect_tx(k_full0 + 8 * st, C::TILE);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sK(st) + bk * C::KBLK, &tmKV, k_full0 + 8 * st, kc + bk * 64, row0 + j * BKV);
@@ -136,11 +155,12 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       for (int j = 0; j < ntiles; j++) {                      // K runs one tile ahead of V
         if (j + 1 < ntiles) load_k(j + 1);
         const int st = j % VST;
-        ptx::mbar_wait(v_empty0 + 8 * st, ((j / VST) & 1) ^ 1);
+        PWAIT(1, v_empty0 + 8 * st, ((j / VST) & 1) ^ 1);
         ptx::mbar_expect_tx(v_full0 + 8 * st, C::TILE);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) ptx::tma_load_2d(sV(st) + bk * C::KBLK, &tmKV, v_full0 + 8 * st, vc + bk * 64, row0 + j * BKV);
       }
+      PFLUSH(0, 1);
     }
   } else if (warp == 1) {
     if (lane == 0) {
@@ -149,8 +169,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024), dP0 = ptx::make_smem_desc(sP, 16, 1024);
       auto issue_s = [&](int j) {
         const int st = j % KST, sb = j & 1;
-        ptx::mbar_wait(k_full0 + 8 * st, (j / KST) & 1);
-        ptx::mbar_wait(s_empty0 + 8 * sb, ((j >> 1) & 1) ^ 1);
+        PWAIT(2, k_full0 + 8 * st, (j / KST) & 1);
+        PWAIT(3, s_empty0 + 8 * sb, ((j >> 1) & 1) ^ 1);
         ptx::tc_fence_after();
         const uint64_t dK0 = ptx::make_smem_desc(sK(st), 16, 1024);
 #pragma unroll
@@ -162,15 +182,18 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         ptx::mma_commit(s_full0 + 8 * sb);
       };
       ptx::mbar_wait(q_full, 0);
+#ifdef ORBIT_PROBE_TIMELINE
+      const long long pt_m0 = clock64();
+#endif
       issue_s(0);
       for (int j = 0; j < ntiles; j++) {
         if (j + 1 < ntiles) issue_s(j + 1);
         const int st = j % VST;
-        ptx::mbar_wait(v_full0 + 8 * st, (j / VST) & 1);
+        PWAIT(4, v_full0 + 8 * st, (j / VST) & 1);
         const uint64_t dV0 = ptx::make_smem_desc(sV(st), C::KBLK, 1024);
 #pragma unroll
         for (int hh = 0; hh < 2; hh++) {                      // the two key halves of P are written by different warps
-          ptx::mbar_wait(p_full0 + 8 * hh, j & 1);
+          PWAIT(5 + hh, p_full0 + 8 * hh, j & 1);
           ptx::tc_fence_after();
 #pragma unroll
           for (int k4 = 0; k4 < BKV / 32; k4++) {
@@ -183,6 +206,10 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         ptx::mma_commit(v_empty0 + 8 * st);
         ptx::mma_commit(o_done);
       }
+#ifdef ORBIT_PROBE_TIMELINE
+      pw_[11] = clock64() - pt_m0;
+      PFLUSH(2, 6); PFLUSH(11, 11);
+#endif
     }
   } else {
     // ===================== softmax / correction / epilogue =====================
@@ -197,9 +224,12 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     const int pair_bar = 1 + quarter;                        // named barrier of the two warps of this quarter
     float m_used = -INFINITY, l = 0.f;                       // l: this thread's half of the row sum
+#ifdef ORBIT_PROBE_TIMELINE
+    const long long pt_sm0 = clock64();
+#endif
     for (int j = 0; j < ntiles; j++) {
       const int sb = j & 1;
-      ptx::mbar_wait(s_full0 + 8 * sb, (j >> 1) & 1);
+      PWAIT(7, s_full0 + 8 * sb, (j >> 1) & 1);
       ptx::tc_fence_after();
       constexpr int HC = BKV / 2;                             // key columns of this warp
       uint32_t s[HC];
@@ -229,7 +259,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       const float mi = ceilf(mx * sl2);                                  // -inf when this half of a ragged tile is fully masked
       const uint32_t xm = xmax + (uint32_t)(sb * 256 + r) * 4;          // [parity][half][row] fp32 (no range limit on the logits)
       asm volatile("st.shared.f32 [%0], %1;" ::"r"(xm + half * 512), "f"(mi) : "memory");
-      named_bar_sync(pair_bar, 64);
+      PTIME(14, named_bar_sync(pair_bar, 64));
       float mo;
       asm volatile("ld.shared.f32 %0, [%1];" : "=f"(mo) : "r"(xm + (half ^ 1) * 512) : "memory");
       const float m_tile = fmaxf(mi, mo);
@@ -241,7 +271,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         // O is final only once PV_{j-1} has completed, and PV_j (which starts as soon as the FIRST half of P_j is
         // published) must not begin before BOTH warps of the pair have rescaled: pair barrier after the rescale.
         // The partner takes the same branch: it sees the same maxima.
-        ptx::mbar_wait(o_done, (j - 1) & 1);
+        PWAIT(8, o_done, (j - 1) & 1);
         ptx::tc_fence_after();
         const float f = exp2f(m_used - m_new);
         l *= f;
@@ -259,7 +289,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         named_bar_sync(pair_bar, 64);
       }
       // this half of the P tile is free once the first / last four MMAs of PV_{j-1} have read it
-      if (j > 0) ptx::mbar_wait(p_free0 + 8 * half, (j - 1) & 1);
+      if (j > 0) PWAIT(9, p_free0 + 8 * half, (j - 1) & 1);
       m_used = m_new;
       float sum = 0.f;
 #pragma unroll
@@ -285,7 +315,11 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * half);
     }
     // ---- epilogue: O / l -> bf16 -> global; logsumexp.  The P tile is idle now: the pair adds its half sums through it
-    ptx::mbar_wait(o_done, (ntiles - 1) & 1);
+    PWAIT(15, o_done, (ntiles - 1) & 1);
+#ifdef ORBIT_PROBE_TIMELINE
+    pw_[10] = clock64() - pt_sm0; pw_[12] = ntiles;
+    if (warp == 2 && lane == 0) { PFLUSH(7, 10); PFLUSH(12, 12); PFLUSH(14, 15); }
+#endif
     ptx::tc_fence_after();
     asm volatile("st.shared.f32 [%0], %1;" ::"r"(sP + (uint32_t)(half * 128 + r) * 4), "f"(l) : "memory");
     named_bar_sync(pair_bar, 64);
@@ -952,6 +986,15 @@ bool attention_tc5_supported(const AttnArgs& a) {
   if (!al16(a.qkv) || !al16(a.O)) return false;
   return a.N >= 128;
 }
+#ifdef ORBIT_PROBE_TIMELINE
+int attention_probe_read(unsigned long long* out, int n, int reset) {
+  unsigned long long h[32] = {0};
+  if (cudaMemcpyFromSymbol(h, g_attn_probe, sizeof(h)) != cudaSuccess) return ORBIT_ERR_CUDA;
+  for (int i = 0; i < n && i < 32; i++) out[i] = h[i];
+  if (reset) { unsigned long long z[32] = {0}; cudaMemcpyToSymbol(g_attn_probe, z, sizeof(z)); }
+  return ORBIT_OK;
+}
+#endif
 int attention_fwd_tc5(const AttnArgs& a, cudaStream_t s) {
   switch (a.dh) {
     case 64: return launch_fwd5<64>(a, s);

@@ -13,6 +13,9 @@
 extern "C" {
 #endif
 void orbit_set_debug_force_simt(int mode);
+/* only with -DORBIT_PROBE_TIMELINE: the forward-attention wait-cycle counters of CTA (0, 0) (attention_tc5.cu), summed over the
+ * launches since the last reset */
+int orbit_debug_read_probe(unsigned long long* out, int n, int reset);
 #ifdef __cplusplus
 }
 #endif

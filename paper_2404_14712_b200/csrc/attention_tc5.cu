@@ -6,20 +6,23 @@
 //                                                     O  += P_j V_j  (fp32, TMEM)
 //   warps 2..9  : softmax; two warps share a TMEM lane quarter (thread <-> query row <-> TMEM lane) and split the
 //                 tile's 128 key columns: tcgen05.ld of the S half-row, row max (agreed between the pair through
-//                 shared memory as ceil(max), a float), exp2 / row sum, P_j as bf16 into a swizzled K-major
-//                 shared-memory tile (the A operand of the PV product) whose two 64-key halves are published and
-//                 released separately (PV_j starts on the first half while the second is still being written),
+//                 shared memory as ceil(max), a float), exp2 / row sum, P_j as packed bf16 pairs written with tcgen05.st
+//                 over the S columns just read (the A operand of the PV product, read from TENSOR MEMORY); the two key
+//                 halves are published separately (PV_j starts on the first half while the second is still being written),
 //                 lazy rescale of O in TMEM (only when a row max grows by more than 2^8: stale maxima keep exp2
 //                 below 256, which is exact enough in fp32 accumulators), final O / l.
 // clock64 stamps (C5, one CTA per SM, 16 tiles): ~2200 cycles per tile against ~1050 of MMA; the softmax warps are
 // the critical path: 128 MUFU.EX2 per row and tile = ~1024 cycles of the sub-partition's quarter-rate unit, plus the
 // serial tcgen05.ld / fence.proxy.async / barrier latencies of a tile.  Tried and measured no faster: a max-only warp
 // running one tile ahead of an exp-only warp (291 us vs 284), P packed by truncation instead of cvt (311 us).
-// Round-2 probes (A/B build, C4, per-launch CUDA events): with the exponentials removed (ORBIT_PROBE_NOEXP) 54.0 -> 54.7 us, with
-// half of the tcgen05.ld traffic removed (ORBIT_PROBE_HALFLD) 52.0 us, with the K / V tiles TMA-multicast across a cluster of two
-// query tiles (half the L2 -> SM traffic) 54 -> 58 us: none of MUFU, TMEM reads or L2 bandwidth bounds the kernel; what is
-// left is the serial per-tile chain of barrier hand-offs between the three agents and the per-CTA prologue / epilogue (one CTA
-// per SM, ~5 us of a 27 us CTA at C5).
+// Round-2 probes (A/B build, C4, per-launch CUDA events) of the version that kept P in shared memory: with the exponentials removed
+// (ORBIT_PROBE_NOEXP) 54.0 -> 54.7 us, with half of the tcgen05.ld traffic removed (ORBIT_PROBE_HALFLD) 52.0 us, with the K / V
+// tiles TMA-multicast across a cluster of two query tiles (half the L2 -> SM traffic) 54 -> 58 us: none of MUFU, TMEM reads or L2
+// bandwidth bounded it.  The timeline probe (ORBIT_PROBE_TIMELINE: cycles per mbarrier wait of each agent) then showed the
+// MMA-issuing thread busy ~1850 of 2350 cycles per tile OUTSIDE its waits while the softmax warps waited 550 cycles per tile for
+// S: the tensor pipe was starved by shared-memory bandwidth (Cfg above).  With P in tensor memory: 2090 cycles per tile, MMA thread
+// 1540 busy, softmax wait for S 240; same-box A/B of the kernel: 53.3 -> 48.0 us at C4 (644 -> 715 TFLOP/s), 370 -> 344 us at C5,
+// 195 -> 180 us at C3.  Both agents are now about equally loaded (softmax ~1850 busy cycles per tile).
 // S_{j+1} is issued before the softmax of tile j finishes, so the tensor pipe overlaps the exponentials.
 // V tiles are consumed as an MN-major B operand straight from their row-major [keys, d] layout.
 #include <cuda.h>
@@ -84,14 +87,20 @@ struct Cfg {
   static constexpr int KBLK = BKV * 128;                // ... of a K / V tile (BKV rows)
   static constexpr int QTILE = 128 * DH * 2;            // bytes of the [128 x DH] bf16 query tile
   static constexpr int TILE = BKV * DH * 2;             // bytes of a [BKV x DH] bf16 key / value tile
-  static constexpr int P_BYTES = 128 * BKV * 2;         // P tile: BKV / 64 blocks of [128 rows x 64 keys]
+  // P never touches shared memory: the softmax threads write it (packed bf16 pairs, tcgen05.st) over the S columns they have
+  // just read and O += P V is a tcgen05.mma with the A operand in tensor memory.  The timeline probe (below) showed the
+  // MMA-issuing thread busy ~1850 of 2350 cycles per tile with the softmax warps WAITING for S: the tensor pipe was starved by
+  // shared-memory bandwidth -- per 128-key tile the MMAs read 128 KB of operands (8 KB per 64-cycle instruction = the whole
+  // 128 B/clk of the SM), the softmax warps wrote 32 KB of P and TMA 64 KB of K / V: 224 KB = 1750 cycles against 1024 cycles
+  // of MMA.  Without the P tile it is 160 KB.  S is then free only after PV has read P, hence THREE S buffers (S_{j+1} is
+  // issued before PV_j, S_{j+2} must not wait for it): 3 BKV + DH <= 512 TMEM columns.
+  static constexpr int NSB = 3;
   // K and V stream through separate rings: a K stage is free as soon as S_j = Q K_j^T has been computed, a V stage
-  // only after O += P_j V_j; with 3 + 2 stages the TMA round trip of K_{j+1} no longer sits between PV_{j-1} and S_{j+1}
-  // (measured with clock64 stamps: the MMA thread waited ~2000 of 2750 cycles per tile for K/V with a shared 2-stage ring)
-  static constexpr int KST = DH == 256 ? 2 : 3, VST = DH == 192 ? 3 : 2;
-  static constexpr int SMEM = QTILE + (KST + VST) * TILE + P_BYTES + 256 /*alignment slack, see the kernel*/ + 256 + 2048 /*row-max exchange*/;
+  // only after O += P_j V_j
+  static constexpr int KST = DH == 256 ? 2 : 3, VST = DH == 256 ? 2 : 3;
+  static constexpr int SMEM = QTILE + (KST + VST) * TILE + 256 /*alignment slack, see the kernel*/ + 256 + 2048 /*row-max exchange*/;
   static_assert(SMEM <= 227 * 1024, "attention forward: shared memory budget");
-  static_assert(2 * BKV + DH <= 512, "attention forward: TMEM budget");
+  static_assert(NSB * BKV + DH <= 512, "attention forward: TMEM budget");
 };
 
 template <int DH>
@@ -105,12 +114,13 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   if (base - ptx::smem_u32(smem_raw) > 256u) __trap();
   constexpr int KST = C::KST, VST = C::VST, BKV = C::BKV;
-  const uint32_t sQ = base, sK0 = sQ + C::QTILE, sV0 = sK0 + KST * C::TILE, sP = sV0 + VST * C::TILE, bar = sP + C::P_BYTES;
+  constexpr int NSB = C::NSB;
+  const uint32_t sQ = base, sK0 = sQ + C::QTILE, sV0 = sK0 + KST * C::TILE, bar = sV0 + VST * C::TILE;
   auto sK = [&](int st) { return sK0 + st * C::TILE; };
   auto sV = [&](int st) { return sV0 + st * C::TILE; };
   const uint32_t q_full = bar, k_full0 = bar + 8, k_empty0 = k_full0 + 8 * KST, v_full0 = k_empty0 + 8 * KST,
-                 v_empty0 = v_full0 + 8 * VST, s_full0 = v_empty0 + 8 * VST, s_empty0 = s_full0 + 16, p_full0 = s_empty0 + 16,
-                 p_free0 = p_full0 + 16, o_done = p_free0 + 16, tmem_slot = o_done + 8, xmax = bar + 256;   // xmax: fp32 [2 parity][2 halves][128 rows]
+                 v_empty0 = v_full0 + 8 * VST, s_full0 = v_empty0 + 8 * VST, s_empty0 = s_full0 + 8 * NSB, p_full0 = s_empty0 + 8 * NSB,
+                 o_done = p_full0 + 16, tmem_slot = o_done + 8, xmax = bar + 256;   // xmax: fp32 [2 parity][2 halves][128 rows]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int q0 = blockIdx.x * BQ;
@@ -123,8 +133,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
     ptx::mbar_init(q_full, 1);
     for (int i = 0; i < KST; i++) { ptx::mbar_init(k_full0 + 8 * i, 1); ptx::mbar_init(k_empty0 + 8 * i, 1); }
     for (int i = 0; i < VST; i++) { ptx::mbar_init(v_full0 + 8 * i, 1); ptx::mbar_init(v_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 8); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 4); ptx::mbar_init(p_free0 + 8 * i, 1); }
+    for (int i = 0; i < NSB; i++) { ptx::mbar_init(s_full0 + 8 * i, 1);  ptx::mbar_init(s_empty0 + 8 * i, 1); }   // empty: commit of the PV that read P
+    for (int i = 0; i < 2; i++) ptx::mbar_init(p_full0 + 8 * i, 4);
     ptx::mbar_init(o_done, 1);
     ptx::fence_barrier_init();
   }
@@ -136,7 +146,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
   pdl_wait();                                    // on-chip prologue done; first global access is below
   pdl_trigger();
-  const uint32_t tS0 = tmem, tO = tmem + 2 * BKV;
+  const uint32_t tS0 = tmem, tO = tmem + NSB * BKV;
 
   PROBE_DECL;
   if (warp == 0) {
@@ -166,11 +176,11 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(BQ, BKV, 0, 0);     // S = Q K^T: both K-major
       constexpr uint32_t idesc_o = ptx::make_idesc_bf16(BQ, DH, 0, 1);      // O += P V: V is MN-major
-      const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024), dP0 = ptx::make_smem_desc(sP, 16, 1024);
+      const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024);
       auto issue_s = [&](int j) {
-        const int st = j % KST, sb = j & 1;
+        const int st = j % KST, sb = j % NSB;
         PWAIT(2, k_full0 + 8 * st, (j / KST) & 1);
-        PWAIT(3, s_empty0 + 8 * sb, ((j >> 1) & 1) ^ 1);
+        PWAIT(3, s_empty0 + 8 * sb, ((j / NSB) & 1) ^ 1);
         ptx::tc_fence_after();
         const uint64_t dK0 = ptx::make_smem_desc(sK(st), 16, 1024);
 #pragma unroll
@@ -191,18 +201,18 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         const int st = j % VST;
         PWAIT(4, v_full0 + 8 * st, (j / VST) & 1);
         const uint64_t dV0 = ptx::make_smem_desc(sV(st), C::KBLK, 1024);
+        const uint32_t tP = tS0 + (j % NSB) * BKV;            // P_j lives in the columns of S_j
 #pragma unroll
         for (int hh = 0; hh < 2; hh++) {                      // the two key halves of P are written by different warps
           PWAIT(5 + hh, p_full0 + 8 * hh, j & 1);
           ptx::tc_fence_after();
 #pragma unroll
-          for (int k4 = 0; k4 < BKV / 32; k4++) {
+          for (int k4 = 0; k4 < BKV / 32; k4++) {             // k-step (16 keys) k4 of half hh: 8 columns of packed bf16 pairs
             const int ks = hh * (BKV / 32) + k4;
-            const uint32_t aoff = (ks >> 2) * 16384 + (ks & 3) * 32;        // P: K-major, two 64-key blocks
-            ptx::mma_f16_ss(tO, desc_adv(dP0, aoff), desc_adv(dV0, ks * 2048), idesc_o, (j | ks) != 0);
+            ptx::mma_f16_ts(tO, tP + hh * (BKV / 2) + k4 * 8, desc_adv(dV0, ks * 2048), idesc_o, (j | ks) != 0);
           }
-          ptx::mma_commit(p_free0 + 8 * hh);                  // this half of the P tile may be rewritten
         }
+        ptx::mma_commit(s_empty0 + 8 * (j % NSB));            // S_j / P_j columns may be overwritten by S_{j+3}
         ptx::mma_commit(v_empty0 + 8 * st);
         ptx::mma_commit(o_done);
       }
@@ -228,8 +238,8 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
     const long long pt_sm0 = clock64();
 #endif
     for (int j = 0; j < ntiles; j++) {
-      const int sb = j & 1;
-      PWAIT(7, s_full0 + 8 * sb, (j >> 1) & 1);
+      const int sb = j % NSB;
+      PWAIT(7, s_full0 + 8 * sb, (j / NSB) & 1);
       ptx::tc_fence_after();
       constexpr int HC = BKV / 2;                             // key columns of this warp
       uint32_t s[HC];
@@ -241,9 +251,6 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
       for (int c = 0; c < HC / 32; c++) ptx::tmem_ld_32x32(tS0 + sb * BKV + half * HC + c * 32 + lane_off, s + c * 32);
 #endif
       ptx::tmem_ld_wait();
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * sb);   // S buffer may be overwritten by S_{j+2}
       float mx = -INFINITY;
       if ((j + 1) * BKV > N) {                               // last, ragged tile: mask keys >= N
 #pragma unroll
@@ -257,7 +264,7 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         for (int c = 0; c < HC; c++) mx = fmaxf(mx, __uint_as_float(s[c]));
       }
       const float mi = ceilf(mx * sl2);                                  // -inf when this half of a ragged tile is fully masked
-      const uint32_t xm = xmax + (uint32_t)(sb * 256 + r) * 4;          // [parity][half][row] fp32 (no range limit on the logits)
+      const uint32_t xm = xmax + (uint32_t)((j & 1) * 256 + r) * 4;     // [parity][half][row] fp32 (no range limit on the logits)
       asm volatile("st.shared.f32 [%0], %1;" ::"r"(xm + half * 512), "f"(mi) : "memory");
       PTIME(14, named_bar_sync(pair_bar, 64));
       float mo;
@@ -288,43 +295,41 @@ attn_fwd_tc5_kernel(const __grid_constant__ CUtensorMap tmQKV, const __grid_cons
         ptx::tc_fence_before();
         named_bar_sync(pair_bar, 64);
       }
-      // this half of the P tile is free once the first / last four MMAs of PV_{j-1} have read it
-      if (j > 0) PWAIT(9, p_free0 + 8 * half, (j - 1) & 1);
       m_used = m_new;
       float sum = 0.f;
+      // P_j: packed bf16 pairs over the first half of this thread's own S columns (k-step of 16 keys = 8 columns); nobody else
+      // reads or writes this lane's columns [half HC, half HC + HC) of the buffer until PV_j has consumed them
+      const uint32_t tPh = tS0 + sb * BKV + half * HC + lane_off;
 #pragma unroll
-      for (int c = 0; c < HC / 8; c++) {                      // 8 keys = one 16-byte chunk of the P row
-        uint32_t pk[4];
+      for (int c = 0; c < HC / 16; c++) {
+        uint32_t pk[8];
 #pragma unroll
-        for (int i = 0; i < 4; i++) {
-          const float p0 = fast_ex2(__uint_as_float(s[c * 8 + 2 * i]) * sl2 - m_used);
-          const float p1 = fast_ex2(__uint_as_float(s[c * 8 + 2 * i + 1]) * sl2 - m_used);
+        for (int i = 0; i < 8; i++) {
+          const float p0 = fast_ex2(__uint_as_float(s[c * 16 + 2 * i]) * sl2 - m_used);
+          const float p1 = fast_ex2(__uint_as_float(s[c * 16 + 2 * i + 1]) * sl2 - m_used);
           sum += p0 + p1;
           __nv_bfloat162 v = __floats2bfloat162_rn(p0, p1);
           pk[i] = *reinterpret_cast<uint32_t*>(&v);
         }
-        // BKV = 128: this warp owns the 64-key block `half`; BKV = 64: chunks 4 half .. 4 half + 3 of the one block
-        const uint32_t addr = BKV == 128 ? sP + half * 16384 + r * 128 + ((c ^ (r & 7)) << 4)
-                                         : sP + r * 128 + (((half * 4 + c) ^ (r & 7)) << 4);
-        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+        ptx::tmem_st_32x8(tPh + c * 8, pk);
       }
       l += sum;
-      ptx::fence_proxy_async();                               // generic-proxy smem writes -> visible to the MMA
+      ptx::tmem_st_wait();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * half);
     }
-    // ---- epilogue: O / l -> bf16 -> global; logsumexp.  The P tile is idle now: the pair adds its half sums through it
+    // ---- epilogue: O / l -> bf16 -> global; logsumexp.  All MMAs and TMA loads are done: the pair adds its half sums through K stage 0
     PWAIT(15, o_done, (ntiles - 1) & 1);
 #ifdef ORBIT_PROBE_TIMELINE
     pw_[10] = clock64() - pt_sm0; pw_[12] = ntiles;
     if (warp == 2 && lane == 0) { PFLUSH(7, 10); PFLUSH(12, 12); PFLUSH(14, 15); }
 #endif
     ptx::tc_fence_after();
-    asm volatile("st.shared.f32 [%0], %1;" ::"r"(sP + (uint32_t)(half * 128 + r) * 4), "f"(l) : "memory");
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(sK0 + (uint32_t)(half * 128 + r) * 4), "f"(l) : "memory");
     named_bar_sync(pair_bar, 64);
     float lo;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(lo) : "r"(sP + (uint32_t)((half ^ 1) * 128 + r) * 4) : "memory");
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(lo) : "r"(sK0 + (uint32_t)((half ^ 1) * 128 + r) * 4) : "memory");
     l += lo;
     const int qrow = q0 + r;
     const float inv = 1.f / l;

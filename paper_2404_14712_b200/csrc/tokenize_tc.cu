@@ -7,7 +7,10 @@
 //   forward : tok[b, l, v, c0:c0+512] for 128 patches of one (b, v) per CTA; B = [Wp[v]; Wp[v]] chunk in smem.
 //   backward: dWp[v] (p^2 x D) and dbp[v] = sum over patches of pix^T dtok / dtok: CTA = (v, 512 columns, a range
 //             of patches); dtok rows stream through a 4-stage cp.async ring; A fragments are built from pixels.
+#include <cuda.h>
+#include <string.h>
 #include "frontend.cuh"
+#include "ptx.cuh"
 
 namespace orbit {
 namespace {
@@ -64,15 +67,30 @@ __device__ __forceinline__ float pixel(const float* x, int V, int Hg, int Wg, in
   return x[(((size_t)b * V + v) * Hg + i * p + di) * Wg + j * p + dj];
 }
 
+__device__ __forceinline__ void stsm4(uint32_t addr, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3) {
+  asm volatile("stmatrix.sync.aligned.m8n8.x4.shared.b16 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(r0), "r"(r1), "r"(r2), "r"(r3) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, uint32_t src, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(m), "r"(src), "r"(c0), "r"(c1) : "memory");
+}
+
 // ---------------------------------------------------------------- forward ----------------------------------
 // KP = contraction length after the hi/lo split, padded to a multiple of 16 (p = 4: 32; p = 2: 16; p = 1: 16)
-template <int P2, int KP>
+// TMA_OUT (D % 64 == 0): a warp's 16 x 64 output tile is written to a 128B-swizzled staging tile with four stmatrix.x4 (the
+// m16n8 accumulator fragments are exactly the 8 x 8 matrices stmatrix stores) and leaves as ONE TMA box store over tok seen as a
+// [B L, V D] matrix, two staging tiles per warp in flight.  The kernel is ISSUE-bound, not HBM-bound (445 M warp instructions for
+// 3 GB at 47 % issue-active, profiles/r1_twocall_front.md): per 64-column group this drops 16 st.shared + 4 ld.shared + 4
+// st.global and their address arithmetic.
+template <int P2, int KP, bool TMA_OUT>
 __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, const float* __restrict__ x,
-    const bf16* __restrict__ Wp, const bf16* __restrict__ bp, bf16* __restrict__ tok, int L) {
+    const bf16* __restrict__ Wp, const bf16* __restrict__ bp, bf16* __restrict__ tok, int L,
+    const __grid_constant__ CUtensorMap tmTok) {
   constexpr int PT = 128, AROW = (KP + 8) * 2;          // patches per CTA; padded A row (bytes)
-  extern __shared__ __align__(128) uint8_t smem[];
-  uint8_t* sA = smem;                                     // [PT][KP + 8] bf16
-  uint8_t* sB = smem + PT * AROW;                         // [KP][DCH + 8] bf16
+  extern __shared__ __align__(1024) uint8_t smem[];
+  // TMA_OUT: the first 32 KB are the staging tiles (8 warps x 2 x [16 rows x 128 B], 1024-byte aligned for the 128B swizzle)
+  constexpr int STAGE_BYTES = TMA_OUT ? (NT / 32) * 2 * 2048 : 0;
+  uint8_t* sA = smem + STAGE_BYTES;                       // [PT][KP + 8] bf16
+  uint8_t* sB = sA + PT * AROW;                           // [KP][DCH + 8] bf16
   // blockIdx.x = (v, column chunk): CTAs that run together write neighbouring 1 KB pieces of the same token rows
   // ([V x D] of a patch is contiguous), instead of pieces V*D*2 bytes apart.
   const int nz = gridDim.x / d.V;
@@ -128,10 +146,53 @@ __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, cons
   // Epilogue: the m16n8 accumulator layout gives a thread 4-byte pieces of 16 different rows, so direct stores fill
   // half a 32-byte sector per instruction.  Each warp stages 16 rows x 64 columns (+ bias) in shared memory and
   // writes them back as 16-byte pieces: 8 lanes cover 128 contiguous bytes of one token row.
-  uint8_t* sO = sB + KP * BROW + warp * (16 * OROW);      // [16][64 + 8] bf16 per warp
   const int r0 = bl0 + warp * 16;
   const bf16* bias = bp + (size_t)v * d.D + c0;
   const uint32_t sBu = s_u32(sB);
+  if (TMA_OUT) {
+    if (s_u32(smem) & 1023u) __trap();                        // the swizzled staging tiles need the 1024-byte aligned base requested above
+    const uint32_t stg0 = s_u32(smem) + warp * 4096;
+    // stmatrix row address of this lane: matrix (lane >> 3) = (rows 8 (m & 1) .., n-tile 2 q + (m >> 1)), row lane & 7
+    const int mrow = (lane & 7) + ((lane >> 3) & 1) * 8, mnt = lane >> 4;
+    for (int ng = 0; ng < DCH / 64; ng++) {
+      if (ng * 64 >= ncol) break;
+      const uint32_t buf = stg0 + (ng & 1) * 2048;
+      if (ng >= 2) {                                          // the store issued from this buffer two groups ago has read it
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+        __syncwarp();
+      }
+#pragma unroll
+      for (int j = 0; j < 4; j++) {
+        const int np = ng * 4 + j;
+        float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+        for (int ks = 0; ks < KP / 16; ks++) {
+          uint32_t b[4];
+          ldB(sBu, ks * 16, np * 16, b);
+          mma16816(acc[0], af[ks], b[0], b[1]);
+          mma16816(acc[1], af[ks], b[2], b[3]);
+        }
+        uint32_t pk[4];                                       // (rows 0-7, n-tile 2j), (rows 8-15, 2j), (rows 0-7, 2j+1), (rows 8-15, 2j+1)
+#pragma unroll
+        for (int nt = 0; nt < 2; nt++) {
+          const float2 bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + ng * 64 + j * 16 + nt * 8 + 2 * t));
+          pk[nt * 2] = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
+          pk[nt * 2 + 1] = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
+        }
+        const int chunk = j * 2 + mnt;                        // 16-byte chunk (n-tile) of the 128-byte staging row
+        stsm4(buf + mrow * 128 + ((chunk ^ (mrow & 7)) << 4), pk[0], pk[1], pk[2], pk[3]);
+      }
+      ptx::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) {
+        tma_store_2d(&tmTok, buf, v * d.D + c0 + ng * 64, r0);      // rows >= B L are clipped by the map
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      }
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the staging tiles outlive the stores
+    return;
+  }
+  uint8_t* sO = sB + KP * BROW + warp * (16 * OROW);      // [16][64 + 8] bf16 per warp
   for (int ng = 0; ng < DCH / 64; ng++) {
     if (ng * 64 >= ncol) break;
 #pragma unroll
@@ -274,13 +335,48 @@ bool tokenize_tc_supported(const orbit_embed_desc& d) {
   return d.dtype == ORBIT_BF16 && (d.p == 1 || d.p == 2 || d.p == 4) && d.D % 16 == 0;
 }
 
+// tok seen as a bf16 matrix [B L rows, V D columns]: boxes of 16 rows x 64 columns, 128-byte swizzle
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long cols) {
+  static std::atomic<EncodeTiledFn> enc_c{nullptr};
+  EncodeTiledFn enc = enc_c.load(std::memory_order_relaxed);
+  if (!enc) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
+    enc = (EncodeTiledFn)p;
+    enc_c.store(enc, std::memory_order_relaxed);
+  }
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)cols * 2};
+  cuuint32_t box[2] = {64, 16};
+  cuuint32_t es[2] = {1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, tok, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("tokenize: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
+  return ORBIT_OK;
+}
+
 int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, const void* bp, void* tok, cudaStream_t s) {
   const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
   dim3 grid(d.V * cdiv(d.D, DCH), cdiv((long long)d.B * L, 128));
+  const bool tma_out = d.D % 64 == 0 && (long long)d.V * d.D < (1ll << 31);
+  CUtensorMap tm;
+  memset(&tm, 0, sizeof(tm));
+  if (tma_out) ORBIT_TRY(make_tok_map(&tm, tok, (long long)d.B * L, (long long)d.V * d.D));
 #define TF(P, K) do {                                                                                         \
-    const size_t smb = (size_t)128 * (K + 8) * 2 + (size_t)K * BROW + (size_t)(NT / 32) * 16 * OROW;                                        \
-    ORBIT_SMEM_ATTR((tok_fwd_tc_kernel<P, K>), smb);                                                           \
-    tok_fwd_tc_kernel<P, K><<<grid, NT, smb, s>>>(d, x, (const bf16*)Wp, (const bf16*)bp, (bf16*)tok, L); } while (0)
+    if (tma_out) {                                                                                            \
+      const size_t smb = (size_t)(NT / 32) * 4096 + (size_t)128 * (K + 8) * 2 + (size_t)K * BROW;              \
+      ORBIT_SMEM_ATTR((tok_fwd_tc_kernel<P, K, true>), smb);                                                  \
+      tok_fwd_tc_kernel<P, K, true><<<grid, NT, smb, s>>>(d, x, (const bf16*)Wp, (const bf16*)bp, (bf16*)tok, L, tm); \
+    } else {                                                                                                  \
+      const size_t smb = (size_t)128 * (K + 8) * 2 + (size_t)K * BROW + (size_t)(NT / 32) * 16 * OROW;         \
+      ORBIT_SMEM_ATTR((tok_fwd_tc_kernel<P, K, false>), smb);                                                 \
+      tok_fwd_tc_kernel<P, K, false><<<grid, NT, smb, s>>>(d, x, (const bf16*)Wp, (const bf16*)bp, (bf16*)tok, L, tm); \
+    } } while (0)
   if (P2 == 16) TF(16, 32);
   else if (P2 == 4) TF(4, 16);
   else TF(1, 16);

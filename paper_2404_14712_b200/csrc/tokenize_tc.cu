@@ -95,137 +95,153 @@ __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, cons
   // ([V x D] of a patch is contiguous), instead of pieces V*D*2 bytes apart.
   const int nz = gridDim.x / d.V;
   const int v = blockIdx.x / nz, c0 = (blockIdx.x - v * nz) * DCH;
-  const int BL = d.B * L, bl0 = blockIdx.y * PT;
+  const int BL = d.B * L, npb = (BL + PT - 1) / PT;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int ncol = min(DCH, d.D - c0);
-  // A: [hi | lo | 0] of the pixels.  One thread per (patch, patch row): the (b, i, j) arithmetic is done once per p
-  // pixels and the row is one vector load (the per-element version spent half of the kernel's instructions here).
   constexpr int P = P2 == 16 ? 4 : (P2 == 4 ? 2 : 1);
-  if (2 * P2 < KP) {
-    constexpr int PAD = KP - 2 * P2 > 0 ? KP - 2 * P2 : 1;
-    for (int idx = threadIdx.x; idx < PT * PAD; idx += NT)
-      *reinterpret_cast<bf16*>(sA + (idx / PAD) * AROW + (2 * P2 + idx % PAD) * 2) = __float2bfloat16_rn(0.f);
-  }
-  {
-    const int gw = d.Wg / P;
-    for (int idx = threadIdx.x; idx < PT * P; idx += NT) {
-      const int pr = idx / P, di = idx % P, bl = bl0 + pr;
-      float px[P];
-#pragma unroll
-      for (int dj = 0; dj < P; dj++) px[dj] = 0.f;
-      if (bl < BL) {
-        const int b = bl / L, l = bl - b * L, i = l / gw, j = l - i * gw;
-        const float* src = x + (((size_t)b * d.V + v) * d.Hg + i * P + di) * d.Wg + j * P;
-        if (P == 4) { const float4 q = *reinterpret_cast<const float4*>(src); px[0] = q.x; px[1 % P] = q.y; px[2 % P] = q.z; px[3 % P] = q.w; }
-        else if (P == 2) { const float2 q = *reinterpret_cast<const float2*>(src); px[0] = q.x; px[1 % P] = q.y; }
-        else px[0] = *src;
-      }
-#pragma unroll
-      for (int dj = 0; dj < P; dj++) {
-        bf16 hi, lo;
-        split_bf16(px[dj], hi, lo);
-        *reinterpret_cast<bf16*>(sA + pr * AROW + (di * P + dj) * 2) = hi;
-        *reinterpret_cast<bf16*>(sA + pr * AROW + (P2 + di * P + dj) * 2) = lo;
-      }
-    }
-  }
-  // B: [Wp[v]; Wp[v]; 0] columns c0..c0+ncol
+  // B: [Wp[v]; Wp[v]; 0] columns c0..c0+ncol -- ONCE per CTA: the CTA is persistent over the patch blocks blockIdx.y,
+  // blockIdx.y + gridDim.y, ... of its (variable, column chunk).  One CTA per patch block spent ~2 us of its ~5.5 us in this
+  // load and in the drain of its last stores with nothing else of its own in flight (3 CTAs per SM): 0.87 ms for 3 GB.
   for (int idx = threadIdx.x; idx < KP * (DCH / 8); idx += NT) {
     const int k = idx / (DCH / 8), ch = idx - k * (DCH / 8);
     uint4 val = make_uint4(0, 0, 0, 0);
     if (k < 2 * P2 && ch * 8 < ncol) val = *reinterpret_cast<const uint4*>(Wp + ((size_t)v * P2 + (k % P2)) * d.D + c0 + ch * 8);
     *reinterpret_cast<uint4*>(sB + k * BROW + ch * 16) = val;
   }
-  __syncthreads();
-  uint32_t af[KP / 16][4];
-  {
-    const int row = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
-#pragma unroll
-    for (int ks = 0; ks < KP / 16; ks++) ldsm4(s_u32(sA) + row * AROW + (ks * 16 + (lane >> 4) * 8) * 2, af[ks]);
+  if (2 * P2 < KP) {
+    constexpr int PAD = KP - 2 * P2 > 0 ? KP - 2 * P2 : 1;
+    for (int idx = threadIdx.x; idx < PT * PAD; idx += NT)
+      *reinterpret_cast<bf16*>(sA + (idx / PAD) * AROW + (2 * P2 + idx % PAD) * 2) = __float2bfloat16_rn(0.f);
   }
-  // Epilogue: the m16n8 accumulator layout gives a thread 4-byte pieces of 16 different rows, so direct stores fill
-  // half a 32-byte sector per instruction.  Each warp stages 16 rows x 64 columns (+ bias) in shared memory and
-  // writes them back as 16-byte pieces: 8 lanes cover 128 contiguous bytes of one token row.
-  const int r0 = bl0 + warp * 16;
+  // A: [hi | lo | 0] of the pixels.  One thread per (patch, patch row): the (b, i, j) arithmetic is done once per p pixels and
+  // the row is one vector load; the rows of the NEXT patch block are requested before the current block is computed.
+  constexpr int ITEMS = PT * P / NT > 0 ? PT * P / NT : 1;     // (patch, row) items per thread (PT * P is a multiple of NT or below it)
+  float px[ITEMS][P];
+  const int gw = d.Wg / P;
+  auto fetch = [&](int pb) {
+#pragma unroll
+    for (int it = 0; it < ITEMS; it++) {
+      const int idx = threadIdx.x + it * NT;
+#pragma unroll
+      for (int dj = 0; dj < P; dj++) px[it][dj] = 0.f;
+      const int pr = idx / P, di = idx % P, bl = pb * PT + pr;
+      if (idx < PT * P && pb < npb && bl < BL) {
+        const int b = bl / L, l = bl - b * L, i = l / gw, jj = l - i * gw;
+        const float* src = x + (((size_t)b * d.V + v) * d.Hg + i * P + di) * d.Wg + jj * P;
+        if (P == 4) { const float4 q = *reinterpret_cast<const float4*>(src); px[it][0] = q.x; px[it][1 % P] = q.y; px[it][2 % P] = q.z; px[it][3 % P] = q.w; }
+        else if (P == 2) { const float2 q = *reinterpret_cast<const float2*>(src); px[it][0] = q.x; px[it][1 % P] = q.y; }
+        else px[it][0] = *src;
+      }
+    }
+  };
   const bf16* bias = bp + (size_t)v * d.D + c0;
   const uint32_t sBu = s_u32(sB);
-  if (TMA_OUT) {
-    if (s_u32(smem) & 1023u) __trap();                        // the swizzled staging tiles need the 1024-byte aligned base requested above
-    const uint32_t stg0 = s_u32(smem) + warp * 4096;
-    // stmatrix row address of this lane: matrix (lane >> 3) = (rows 8 (m & 1) .., n-tile 2 q + (m >> 1)), row lane & 7
-    const int mrow = (lane & 7) + ((lane >> 3) & 1) * 8, mnt = lane >> 4;
+  const uint32_t stg0 = s_u32(smem) + warp * 4096;
+  if (TMA_OUT && (s_u32(smem) & 1023u)) __trap();            // the swizzled staging tiles need the 1024-byte aligned base requested above
+  // stmatrix row address of this lane: matrix (lane >> 3) = (rows 8 (m & 1) .., n-tile 2 q + (m >> 1)), row lane & 7
+  const int mrow = (lane & 7) + ((lane >> 3) & 1) * 8, mnt = lane >> 4;
+  uint8_t* sO = sB + KP * BROW + warp * (16 * OROW);        // !TMA_OUT: [16][64 + 8] bf16 per warp
+  int nstore = 0;                                            // TMA stores issued by this warp
+  fetch(blockIdx.y);
+  for (int pb = blockIdx.y; pb < npb; pb += gridDim.y) {
+    const int bl0 = pb * PT;
+#pragma unroll
+    for (int it = 0; it < ITEMS; it++) {
+      const int idx = threadIdx.x + it * NT;
+      if (idx < PT * P) {
+        const int pr = idx / P, di = idx % P;
+#pragma unroll
+        for (int dj = 0; dj < P; dj++) {
+          bf16 hi, lo;
+          split_bf16(px[it][dj], hi, lo);
+          *reinterpret_cast<bf16*>(sA + pr * AROW + (di * P + dj) * 2) = hi;
+          *reinterpret_cast<bf16*>(sA + pr * AROW + (P2 + di * P + dj) * 2) = lo;
+        }
+      }
+    }
+    __syncthreads();
+    uint32_t af[KP / 16][4];
+    {
+      const int row = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+#pragma unroll
+      for (int ks = 0; ks < KP / 16; ks++) ldsm4(s_u32(sA) + row * AROW + (ks * 16 + (lane >> 4) * 8) * 2, af[ks]);
+    }
+    __syncthreads();                                         // sA may be rewritten for the next patch block
+    fetch(pb + gridDim.y);                                   // in flight while this block is computed and stored
+    const int r0 = bl0 + warp * 16;
     for (int ng = 0; ng < DCH / 64; ng++) {
       if (ng * 64 >= ncol) break;
-      const uint32_t buf = stg0 + (ng & 1) * 2048;
-      if (ng >= 2) {                                          // the store issued from this buffer two groups ago has read it
-        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+      if (TMA_OUT) {
+        const uint32_t buf = stg0 + (nstore & 1) * 2048;
+        if (nstore >= 2) {                                    // the store issued from this buffer two groups ago has read it
+          if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+          __syncwarp();
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          const int np = ng * 4 + j;
+          float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+          for (int ks = 0; ks < KP / 16; ks++) {
+            uint32_t b[4];
+            ldB(sBu, ks * 16, np * 16, b);
+            mma16816(acc[0], af[ks], b[0], b[1]);
+            mma16816(acc[1], af[ks], b[2], b[3]);
+          }
+          uint32_t pk[4];                                     // (rows 0-7, n-tile 2j), (rows 8-15, 2j), (rows 0-7, 2j+1), (rows 8-15, 2j+1)
+#pragma unroll
+          for (int nt = 0; nt < 2; nt++) {
+            const float2 bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + ng * 64 + j * 16 + nt * 8 + 2 * t));
+            pk[nt * 2] = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
+            pk[nt * 2 + 1] = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
+          }
+          const int chunk = j * 2 + mnt;                      // 16-byte chunk (n-tile) of the 128-byte staging row
+          stsm4(buf + mrow * 128 + ((chunk ^ (mrow & 7)) << 4), pk[0], pk[1], pk[2], pk[3]);
+        }
+        ptx::fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          tma_store_2d(&tmTok, buf, v * d.D + c0 + ng * 64, r0);    // rows >= B L are clipped by the map
+          asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        nstore++;
+      } else {
+        // The m16n8 accumulator layout gives a thread 4-byte pieces of 16 different rows: each warp stages 16 rows x 64 columns
+        // (+ bias) in shared memory and writes them back as 16-byte pieces, 8 lanes covering 128 contiguous bytes of a token row.
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          const int np = ng * 4 + j;
+          float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+          for (int ks = 0; ks < KP / 16; ks++) {
+            uint32_t b[4];
+            ldB(sBu, ks * 16, np * 16, b);
+            mma16816(acc[0], af[ks], b[0], b[1]);
+            mma16816(acc[1], af[ks], b[2], b[3]);
+          }
+#pragma unroll
+          for (int nt = 0; nt < 2; nt++) {
+            const int cl = j * 16 + nt * 8 + 2 * t;           // column inside the 64-column group
+            float2 bb = make_float2(0.f, 0.f);
+            if (ng * 64 + cl < ncol) bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + ng * 64 + cl));
+            *reinterpret_cast<uint32_t*>(sO + g * OROW + cl * 2) = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
+            *reinterpret_cast<uint32_t*>(sO + (g + 8) * OROW + cl * 2) = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
+          }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+          const int row = q * 4 + (lane >> 3), ch = lane & 7;
+          const int col = ng * 64 + ch * 8;
+          if (r0 + row < BL && col < ncol)
+            *reinterpret_cast<uint4*>(tok + ((size_t)(r0 + row) * d.V + v) * d.D + c0 + col) =
+                *reinterpret_cast<const uint4*>(sO + row * OROW + ch * 16);
+        }
         __syncwarp();
       }
-#pragma unroll
-      for (int j = 0; j < 4; j++) {
-        const int np = ng * 4 + j;
-        float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-#pragma unroll
-        for (int ks = 0; ks < KP / 16; ks++) {
-          uint32_t b[4];
-          ldB(sBu, ks * 16, np * 16, b);
-          mma16816(acc[0], af[ks], b[0], b[1]);
-          mma16816(acc[1], af[ks], b[2], b[3]);
-        }
-        uint32_t pk[4];                                       // (rows 0-7, n-tile 2j), (rows 8-15, 2j), (rows 0-7, 2j+1), (rows 8-15, 2j+1)
-#pragma unroll
-        for (int nt = 0; nt < 2; nt++) {
-          const float2 bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + ng * 64 + j * 16 + nt * 8 + 2 * t));
-          pk[nt * 2] = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
-          pk[nt * 2 + 1] = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
-        }
-        const int chunk = j * 2 + mnt;                        // 16-byte chunk (n-tile) of the 128-byte staging row
-        stsm4(buf + mrow * 128 + ((chunk ^ (mrow & 7)) << 4), pk[0], pk[1], pk[2], pk[3]);
-      }
-      ptx::fence_proxy_async();
-      __syncwarp();
-      if (lane == 0) {
-        tma_store_2d(&tmTok, buf, v * d.D + c0 + ng * 64, r0);      // rows >= B L are clipped by the map
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      }
     }
-    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the staging tiles outlive the stores
-    return;
   }
-  uint8_t* sO = sB + KP * BROW + warp * (16 * OROW);      // [16][64 + 8] bf16 per warp
-  for (int ng = 0; ng < DCH / 64; ng++) {
-    if (ng * 64 >= ncol) break;
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-      const int np = ng * 4 + j;
-      float acc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-#pragma unroll
-      for (int ks = 0; ks < KP / 16; ks++) {
-        uint32_t b[4];
-        ldB(sBu, ks * 16, np * 16, b);
-        mma16816(acc[0], af[ks], b[0], b[1]);
-        mma16816(acc[1], af[ks], b[2], b[3]);
-      }
-#pragma unroll
-      for (int nt = 0; nt < 2; nt++) {
-        const int cl = j * 16 + nt * 8 + 2 * t;           // column inside the 64-column group
-        float2 bb = make_float2(0.f, 0.f);
-        if (ng * 64 + cl < ncol) bb = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(bias + ng * 64 + cl));
-        *reinterpret_cast<uint32_t*>(sO + g * OROW + cl * 2) = pack_bf16(acc[nt][0] + bb.x, acc[nt][1] + bb.y);
-        *reinterpret_cast<uint32_t*>(sO + (g + 8) * OROW + cl * 2) = pack_bf16(acc[nt][2] + bb.x, acc[nt][3] + bb.y);
-      }
-    }
-    __syncwarp();
-#pragma unroll
-    for (int q = 0; q < 4; q++) {
-      const int row = q * 4 + (lane >> 3), ch = lane & 7;
-      const int col = ng * 64 + ch * 8;
-      if (r0 + row < BL && col < ncol)
-        *reinterpret_cast<uint4*>(tok + ((size_t)(r0 + row) * d.V + v) * d.D + c0 + col) =
-            *reinterpret_cast<const uint4*>(sO + row * OROW + ch * 16);
-    }
-    __syncwarp();
-  }
+  if (TMA_OUT && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the staging tiles outlive the stores
 }
 
 // ---------------------------------------------------------------- backward ---------------------------------
@@ -362,7 +378,22 @@ static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long co
 
 int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, const void* bp, void* tok, cudaStream_t s) {
   const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
-  dim3 grid(d.V * cdiv(d.D, DCH), cdiv((long long)d.B * L, 128));
+  // persistent over the patch blocks: grid.y CTAs per (variable, column chunk), chosen so that the grid fills whole waves
+  // of 3 CTAs per SM (the shared-memory limit) as evenly as possible, 4+ patch blocks per CTA when there are enough
+  const int gx = d.V * cdiv(d.D, DCH), npb = cdiv((long long)d.B * L, 128);
+  int gy = 1;
+  {
+    const long long slots = (long long)num_sms() * 3;
+    double best = -1.0;
+    for (int c = 1; c <= npb && c <= 64; c++) {
+      const int per = cdiv(npb, c);                          // patch blocks of the longest CTA
+      const long long waves = ((long long)gx * c + slots - 1) / slots;
+      const double eff = (double)gx * npb / ((double)waves * slots * per);      // useful / available block slots
+      if (per < (npb < 4 ? npb : 4)) break;                  // keep at least 4 patch blocks per CTA (the point of the loop)
+      if (eff > best + 1e-9) { best = eff; gy = c; }
+    }
+  }
+  dim3 grid(gx, gy);
   const bool tma_out = d.D % 64 == 0 && (long long)d.V * d.D < (1ll << 31);
   CUtensorMap tm;
   memset(&tm, 0, sizeof(tm));

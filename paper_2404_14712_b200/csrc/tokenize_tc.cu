@@ -246,13 +246,27 @@ __global__ void __launch_bounds__(NT) tok_fwd_tc_kernel(orbit_embed_desc d, cons
 
 // ---------------------------------------------------------------- backward ---------------------------------
 // accW[v, r, c] += sum_patches pix[patch, r] dtok[patch, v, c];  accB[v, c] += sum_patches dtok[patch, v, c]
-template <int P2>
+// TMA_IN (D % 64 == 0): the dtok rows of a chunk arrive as eight [16 patches x 64 columns] TMA boxes (128B swizzle; warp w's 64
+// columns = box w) issued by one thread, instead of four cp.async per thread with their address arithmetic (the kernel was
+// issue-bound: 498 M warp instructions for 3 GB at 52 % issue-active, profiles/r1_twocall_front.md).
+template <int P2, bool TMA_IN>
 __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, const float* __restrict__ x,
-    const bf16* __restrict__ dtok, float* __restrict__ accW, float* __restrict__ accB, int L, int patches_per_cta) {
+    const bf16* __restrict__ dtok, float* __restrict__ accW, float* __restrict__ accB, int L, int patches_per_cta,
+    const __grid_constant__ CUtensorMap tmTok) {
   constexpr int STG = 4, KC = 16;                         // ring stages; patches per k-chunk
-  extern __shared__ __align__(128) uint8_t smem[];
-  uint8_t* sB = smem;                                     // [STG][KC][DCH + 8] bf16
-  float* sP = reinterpret_cast<float*>(smem + STG * KC * BROW);   // [STG][KC][16] pixels (fp32)
+  constexpr int STB = TMA_IN ? KC * DCH * 2 : KC * BROW;   // bytes of a stage of dtok rows (TMA: 8 swizzled 2 KB boxes)
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t* sB = smem;                                     // [STG] stages of dtok rows
+  float* sP = reinterpret_cast<float*>(smem + STG * STB);  // [STG][KC][16] pixels (fp32)
+  __shared__ __align__(8) uint64_t full_bar[STG];
+  if (TMA_IN) {
+    if (s_u32(smem) & 1023u) __trap();
+    if (threadIdx.x == 0) {
+      for (int i = 0; i < STG; i++) ptx::mbar_init(s_u32(&full_bar[i]), 1);
+      ptx::fence_barrier_init();
+    }
+    __syncthreads();
+  }
   // blockIdx.x = (v, column chunk): CTAs that run together read neighbouring 1 KB pieces of the same token rows
   const int nz = gridDim.x / d.V;
   const int v = blockIdx.x / nz, c0 = (blockIdx.x - v * nz) * DCH;
@@ -272,8 +286,17 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
     const int l = bl - pb * L;
     pi = l / gw; pj = l - pi * gw;
   }
+  const int nblk = (ncol + 63) / 64;                       // 64-column boxes of this CTA's chunk
   auto load = [&](int ci) {
     const int st = ci % STG, base = p0 + ci * KC;
+    if (TMA_IN) {
+      if (threadIdx.x == 0) {                                // rows >= B L read as zero; the patch range of a CTA is a multiple of KC
+        const uint32_t bar = s_u32(&full_bar[st]);
+        ptx::mbar_expect_tx(bar, nblk * KC * 128);
+        for (int bk = 0; bk < nblk; bk++)
+          ptx::tma_load_2d(s_u32(sB + st * STB + bk * (KC * 128)), &tmTok, bar, v * d.D + c0 + bk * 64, base);
+      }
+    } else
     for (int idx = threadIdx.x; idx < KC * (DCH / 8); idx += NT) {
       const int k = idx / (DCH / 8), ch = idx - k * (DCH / 8);
       const uint32_t dst = s_u32(sB + (st * KC + k) * BROW + ch * 16);
@@ -316,10 +339,18 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
     split_pair(pt[(2 * t) * 16 + g + 8], pt[(2 * t + 1) * 16 + g + 8], ah[1], al[1]);
     split_pair(pt[(2 * t + 8) * 16 + g], pt[(2 * t + 9) * 16 + g], ah[2], al[2]);
     split_pair(pt[(2 * t + 8) * 16 + g + 8], pt[(2 * t + 9) * 16 + g + 8], ah[3], al[3]);
-    const uint32_t bt = s_u32(sB + st * KC * BROW);
+    const uint32_t bt = s_u32(sB + st * STB);
+    if (TMA_IN) {
+      if (warp >= nblk) continue;                            // this warp's box was not loaded (columns >= D): nothing to add
+      ptx::mbar_wait(s_u32(&full_bar[st]), (ci / STG) & 1);
+    }
 #pragma unroll
     for (int np = 0; np < 4; np++) {                       // this warp's 64 columns = 4 pairs of n-tiles
       uint32_t b[4];
+      if (TMA_IN) {                                          // box `warp`: [16 rows x 128 B], 16-byte chunks XOR-swizzled with (row & 7)
+        const int row = (lane & 7) + ((lane >> 3) & 1) * 8, chunk = np * 2 + (lane >> 4);
+        ldsm4t(bt + warp * (KC * 128) + row * 128 + ((chunk ^ (row & 7)) << 4), b);
+      } else
       ldB(bt, 0, warp * 64 + np * 16, b);
       mma16816(aw[2 * np], ah, b[0], b[1]);     mma16816(aw[2 * np + 1], ah, b[2], b[3]);
       mma16816(aw[2 * np], al, b[0], b[1]);     mma16816(aw[2 * np + 1], al, b[2], b[3]);
@@ -355,7 +386,8 @@ bool tokenize_tc_supported(const orbit_embed_desc& d) {
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long cols) {
+static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long cols,
+                        CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE) {
   static std::atomic<EncodeTiledFn> enc_c{nullptr};
   EncodeTiledFn enc = enc_c.load(std::memory_order_relaxed);
   if (!enc) {
@@ -371,7 +403,7 @@ static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long co
   cuuint32_t box[2] = {64, 16};
   cuuint32_t es[2] = {1, 1};
   CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, tok, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                   CU_TENSOR_MAP_SWIZZLE_128B, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { set_error("tokenize: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
   return ORBIT_OK;
 }
@@ -436,10 +468,19 @@ int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* d
   ppc = ((ppc + 15) / 16) * 16;
   if (ppc < 64) ppc = 64;
   dim3 grid(d.V * nz, cdiv(BL, ppc));
-  const size_t smb = (size_t)4 * 16 * BROW + (size_t)4 * 16 * 16 * sizeof(float);
+  const bool tma_in = d.D % 64 == 0 && (long long)d.V * d.D < (1ll << 31);
+  CUtensorMap tm;
+  memset(&tm, 0, sizeof(tm));
+  if (tma_in) ORBIT_TRY(make_tok_map(&tm, const_cast<void*>(dtok), BL, (long long)d.V * d.D, CU_TENSOR_MAP_L2_PROMOTION_L2_256B));
+  const size_t smb = (size_t)4 * (tma_in ? 16 * DCH * 2 : 16 * BROW) + (size_t)4 * 16 * 16 * sizeof(float);
 #define TB(P) do {                                                                                            \
-    ORBIT_SMEM_ATTR(tok_bwd_tc_kernel<P>, smb);                                                               \
-    tok_bwd_tc_kernel<P><<<grid, NT, smb, s>>>(d, x, (const bf16*)dtok, accW, accB, L, ppc); } while (0)
+    if (tma_in) {                                                                                             \
+      ORBIT_SMEM_ATTR((tok_bwd_tc_kernel<P, true>), smb);                                                     \
+      tok_bwd_tc_kernel<P, true><<<grid, NT, smb, s>>>(d, x, (const bf16*)dtok, accW, accB, L, ppc, tm);      \
+    } else {                                                                                                  \
+      ORBIT_SMEM_ATTR((tok_bwd_tc_kernel<P, false>), smb);                                                    \
+      tok_bwd_tc_kernel<P, false><<<grid, NT, smb, s>>>(d, x, (const bf16*)dtok, accW, accB, L, ppc, tm);     \
+    } } while (0)
   if (P2 == 16) TB(16);
   else if (P2 == 4) TB(4);
   else TB(1);

@@ -243,6 +243,7 @@ __global__ void __launch_bounds__(NTF + 32) agg_fwd_tma_kernel(const __grid_cons
 // staging tile (aliasing the dalpha / alpha score buffers, dead in pass 2) as 16-byte pieces, 128 contiguous bytes of a
 // token row per 8 lanes, instead of 4-byte pieces of 16 rows.
 constexpr int NTB = 512;                    // consumer threads; warp 16 is the TMA producer
+constexpr int TMEM_ACC_COLS = 512;          // dUt^T accumulator: 2 warps per lane quarter x (D / 64 chunks) x 4 columns -> D <= 4096
 constexpr int BT = 2 * UT;                   // B tile: rows 0-15 dXbar chunk, 16-31 Ut chunk
 template <int STG>
 __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_constant__ CUtensorMap tmX,
@@ -259,9 +260,12 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
   constexpr int ADROW = 2 * HP + 8;
   bf16* sDT = sAD + Vp * ADROW;                                              // ds^T [HP][DTROW]
   constexpr int DTROW = VP_MAX + 8;
-  float* sAcc = reinterpret_cast<float*>(sDT + HP * DTROW);                  // [HP][D + 8] block-private dUt^T accumulator
-  const int AR = D + 8;                                                       // padded: rows g, g + 1 are 8 banks apart
-  const uint32_t bar0 = s_u32(sAcc + HP * AR), ebar0 = bar0 + 8 * STG;       // full[STG], empty[STG]
+  // The block-private dUt^T accumulator [HP][D] fp32 (131 KB at D = 2048) lives in TENSOR MEMORY, not in shared memory: every
+  // thread of the 8 accumulating warps owns 4 values per 64-column chunk, kept in 4 columns of its own TMEM lane (tcgen05.ld /
+  // add / tcgen05.st, no hazards: nobody else touches the cell).  The shared memory it occupied now holds a 12-stage ring
+  // instead of 4 stages: the kernel was bound by the mbarrier waits of the shallow ring (3.6 TB/s of DRAM traffic).
+  const uint32_t tslot = s_u32(sDT + HP * DTROW);                             // TMEM base address word (+ padding to 16 bytes)
+  const uint32_t bar0 = tslot + 16, ebar0 = bar0 + 8 * STG;                   // full[STG], empty[STG]
   const uint32_t sADu = s_u32(sAD), sDTu = s_u32(sDT);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int wt = warp & 7, wh = warp >> 3;
@@ -269,7 +273,7 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
   uint8_t* sO = reinterpret_cast<uint8_t*>(sS) + wt * (16 * 128);            // [16][64] bf16, swizzled: 2 KB per dX warp (wt < mtiles)
   static_assert(16 * 128 <= 2 * 16 * SROW * 4, "staging tiles (2 KB per 16 rows) must fit in the score buffers (2 x 16 x SROW floats)");
 
-  for (int i = threadIdx.x; i < HP * AR; i += NTB + 32) sAcc[i] = 0.f;
+  if (warp == 0) { tmem_alloc(tslot, TMEM_ACC_COLS); tmem_relinquish(); }
   for (int j = 0; j < STG; j++) {
     zero_tail_rows(smem + j * XTb, V, Vp, NTB + 32);
     zero_tail_rows(smem + STG * XTb + j * BT, h, HP, NTB + 32);
@@ -279,7 +283,15 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
     fence_barrier_init();
   }
   fence_proxy_async();
+  tc_fence_before();
   __syncthreads();
+  tc_fence_after();
+  uint32_t tacc;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tacc) : "r"(tslot));
+  const uint32_t tacc0 = tacc;
+  // this thread's accumulator cells: lane = its lane in the warp's TMEM quarter, 4 columns per chunk, the two warps of a quarter
+  // (wt and wt + 4) side by side
+  tacc += ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(wt >> 2) * (TMEM_ACC_COLS / 2);
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   const int per = 2 * nch, total = npat * per;
@@ -412,22 +424,45 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
             mma16816(o, a, b[0], b[1]);
           }
         }
-        const int d = c0 + wt * 8 + 2 * t;
-        float2* p0 = reinterpret_cast<float2*>(sAcc + g * AR + d);
-        float2* p1 = reinterpret_cast<float2*>(sAcc + (g + 8) * AR + d);
-        float2 v0 = *p0, v1 = *p1;
-        v0.x += o[0]; v0.y += o[1]; v1.x += o[2]; v1.y += o[3];
-        *p0 = v0; *p1 = v1;
+        // o[0..3] = (head g, columns d, d + 1), (head g + 8, d, d + 1) with d = c0 + 8 wt + 2 t: added to this thread's 4 TMEM cells of the chunk
+        const uint32_t cell = tacc + (uint32_t)(c0 / TB) * 4;
+        uint32_t av[4];
+        if (pi == 0) {
+#pragma unroll
+          for (int q = 0; q < 4; q++) av[q] = __float_as_uint(o[q]);
+        } else {
+          tmem_st_wait();                // this thread's store to the cell (previous patch) has completed
+          tmem_ld_32x4(cell, av);
+          tmem_ld_wait();
+#pragma unroll
+          for (int q = 0; q < 4; q++) av[q] = __float_as_uint(__uint_as_float(av[q]) + o[q]);
+        }
+        tmem_st_32x4(cell, av);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(ebar0 + 8 * st);
     }
   }
-  consumer_sync();
-  for (int i = threadIdx.x; i < h * D; i += NTB) {
-    int a = i / D, d = i - a * D;
-    atomicAdd(dUt_acc + (size_t)d * h + a, sAcc[a * AR + d]);
+  if (wh == 1 && npat > 0) {            // flush this thread's cells: one pass over the chunks
+    tmem_st_wait();
+    for (int c = 0; c < nch; c++) {
+      uint32_t av[4];
+      tmem_ld_32x4(tacc + (uint32_t)c * 4, av);
+      tmem_ld_wait();
+      const int d = c * TB + wt * 8 + 2 * t;
+      if (g < h) {
+        atomicAdd(dUt_acc + (size_t)d * h + g, __uint_as_float(av[0]));
+        atomicAdd(dUt_acc + (size_t)(d + 1) * h + g, __uint_as_float(av[1]));
+      }
+      if (g + 8 < h) {
+        atomicAdd(dUt_acc + (size_t)d * h + g + 8, __uint_as_float(av[2]));
+        atomicAdd(dUt_acc + (size_t)(d + 1) * h + g + 8, __uint_as_float(av[3]));
+      }
+    }
   }
+  tc_fence_before();
+  consumer_sync();
+  if (warp == 0) { tc_fence_after(); tmem_dealloc(tacc0, TMEM_ACC_COLS); }
 }
 
 // Ut [D, h] fp32 -> Utb [HP, D] bf16 (rows >= h zero)
@@ -443,8 +478,9 @@ size_t fwd_smem(int stg) {
 }
 size_t bwd_smem(int V, int D, int stg) {
   const size_t Vp = (V + 15) & ~15;
+  (void)D;                               // the [HP][D] accumulator is in tensor memory
   return 1024 + (size_t)stg * (Vp * TB * 2 + BT) + 2 * Vp * SROW * 4 + Vp * (2 * HP + 8) * 2 +
-         (size_t)HP * (VP_MAX + 8) * 2 + (size_t)HP * (D + 8) * 4 + 16 * stg;
+         (size_t)HP * (VP_MAX + 8) * 2 + 64 + 16 * stg;
 }
 constexpr size_t SMEM_MAX = 227 * 1024;
 
@@ -474,7 +510,8 @@ int make_map(CUtensorMap* tm, const void* base, long long rows, int D, int box_r
 }  // namespace
 
 bool agg_tc_supported(int dt, int V, int D, int heads) {
-  return dt == ORBIT_BF16 && heads <= HP && V <= VP_MAX && D % 128 == 0 && bwd_smem(V, D, 2) <= SMEM_MAX;
+  // D / 64 chunks x 4 accumulator columns x 2 warps per TMEM lane quarter <= TMEM_ACC_COLS
+  return dt == ORBIT_BF16 && heads <= HP && V <= VP_MAX && D % 128 == 0 && D / TB * 8 <= TMEM_ACC_COLS && bwd_smem(V, D, 2) <= SMEM_MAX;
 }
 size_t agg_tc_utb_bytes(int D) { return (size_t)HP * D * sizeof(bf16); }
 
@@ -501,13 +538,14 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
   ORBIT_TRY(make_map(&tmG, dXbar, (long long)BL * heads, D, heads));
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
   const int grid = BL < 148 ? BL : 148;
-  int stg = 6;                          // deepest ring that fits beside the [HP][D] fp32 dUt accumulator
-  while (stg > 2 && bwd_smem(V, D, stg) > SMEM_MAX) stg--;
+  int stg = 12;                         // deepest ring that fits (the dUt accumulator is in tensor memory)
+  while (stg > 2 && bwd_smem(V, D, stg) > SMEM_MAX) stg -= (stg > 6 ? 2 : 1);
   const size_t smb = bwd_smem(V, D, stg);
 #define AB(S) do {                                                                                            \
     ORBIT_SMEM_ATTR(agg_bwd_tma_kernel<S>, smb);                                                              \
     agg_bwd_tma_kernel<S><<<grid, NTB + 32, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads); } while (0)
-  if (stg == 6) AB(6); else if (stg == 5) AB(5); else if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
+  if (stg == 12) AB(12); else if (stg == 10) AB(10); else if (stg == 8) AB(8); else if (stg == 6) AB(6); else if (stg == 5) AB(5);
+  else if (stg == 4) AB(4); else if (stg == 3) AB(3); else AB(2);
 #undef AB
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;

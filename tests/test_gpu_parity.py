@@ -321,6 +321,8 @@ def test_front_end_fused_shapes(rn, case):
     dict(B=3, V=48, Hg=24, Wg=20, p=2, D=256, heads=16, rd="bf16"),     # BL = 360: 2-3 patches per CTA through one ring
     dict(B=2, V=5, Hg=6, Wg=10, p=1, D=128, heads=8, rd="f32"),         # patch 1, V < 16 (one row tile, 11 zero rows)
     dict(B=5, V=17, Hg=16, Wg=16, p=2, D=384, heads=12, rd="bf16"),     # odd chunk count (D = 6 x 64), V = 16 + 1, BL = 320
+    dict(B=1, V=9, Hg=8, Wg=8, p=2, D=4096, heads=16, rd="bf16"),       # widest D of the TMA kernels: the [16][D] dUt accumulator fills
+                                                                        # all 512 TMEM columns (64 chunks x 4 columns x 2 warps per quarter)
 ])
 def test_front_end_twocall_shapes(rn, case):
     """orbit_tokenize + orbit_var_aggregate (+ backward) on the tensor-core / TMA kernels over edge shapes, <= 1e-2."""

@@ -63,7 +63,14 @@ __device__ __forceinline__ void tile_coords2(int t, int tiles_m, int tiles_n, in
 // round that keeps 19 % of the SMs busy) are split into `parts` column sub-tiles of W = 256 / parts columns each, so that
 // the last round takes 1 / parts of a tile time on parts x as many clusters.
 // hint_a / hint_b / hint_c: L2 eviction priority of the A loads, B loads and C stores (0 normal, 1 evict_first, 2 evict_last)
-struct Sched { int full, parts, total, group_m, hint_a, hint_b, hint_c; };
+// round_bar: the TMA producers of all clusters meet at a counter in global memory before each round of tiles, so that the 8-9
+// clusters sharing an operand panel sweep K in step and fetch it from DRAM once: without it they drift apart and re-fetch (C5: 30.0
+// -> 23.4 GB of DRAM traffic per step, fc2 4.1 -> 2.6 GB; step time unchanged on a typical box, profiles/r2_gemm_schedule.md; some
+// boxes of the pool move 40 GB without it).  The wait is BOUNDED (20 us): the grid is not a cooperative launch, and a cluster that
+// cannot become resident (another stream's kernel holds its SMs) must not hang the others; after a timeout the cluster stops waiting
+// but keeps arriving.  ORBIT_GEMM_ROUND_SYNC=0 switches it off.
+struct Sched { int full, parts, total, group_m, hint_a, hint_b, hint_c; unsigned int* round_bar; };
+__device__ unsigned int g_round_bar[2 * 64];     // per slot: [arrivals, exits]; the last cluster to leave zeroes its slot
 __device__ __forceinline__ void unit_of(const Sched& sc, int u, int& t, int& part, int& W) {
   if (u < sc.full) { t = u; part = 0; W = BN2; }
   else { const int r = u - sc.full; t = sc.full + r / sc.parts; part = r % sc.parts; W = BN2 / sc.parts; }
@@ -120,7 +127,24 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
       const uint64_t pol_a = ptx::l2_policy(sc.hint_a), pol_b = ptx::l2_policy(sc.hint_b);
-      for (int u = cluster_id; u < sc.total; u += num_clusters) {
+      unsigned int target = 0;
+      bool gave_up = false;
+      for (int u = cluster_id, round = 0; u < sc.total; u += num_clusters, round++) {
+        if (sc.round_bar && round > 0) {         // all clusters that have a unit in this round start it together
+          const int left = sc.total - round * num_clusters;
+          target += (unsigned int)(left < num_clusters ? left : num_clusters);
+          if (leader) atomicAdd(sc.round_bar, 1u);
+          if (!gave_up) {
+            unsigned long long t0, t1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+            unsigned int seen;
+            do {
+              asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(sc.round_bar) : "memory");
+              asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+              if (t1 - t0 > 20000ull) { gave_up = true; break; }
+            } while (seen < target);
+          }
+        }
         int t, part, W;
         unit_of(sc, u, t, part, W);
         const int bi = t / tiles_per_batch;
@@ -148,6 +172,10 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           }
           if (++s == STAGES) { s = 0; ph ^= 1; }
         }
+      }
+      if (sc.round_bar && leader) {            // every cluster has passed its last meeting point once all have left: reset the slot
+        __threadfence();
+        if (atomicAdd(sc.round_bar + 1, 1u) == (unsigned int)num_clusters - 1) { sc.round_bar[0] = 0; sc.round_bar[1] = 0; __threadfence(); }
       }
     }
   } else if (warp == 1) {
@@ -366,6 +394,14 @@ bool tail_split_enabled() {
   static const int v = [] { const char* e = getenv("ORBIT_GEMM_TAIL_SPLIT"); return (e && e[0] == '0') ? 0 : 1; }();
   return v != 0;
 }
+double round_sync_min_bytes() {
+  static const double v = [] { const char* e = getenv("ORBIT_GEMM_ROUND_SYNC_MINMB"); return (e ? atof(e) : 256.0) * 1e6; }();
+  return v;
+}
+bool round_sync_enabled() {
+  static const int v = [] { const char* e = getenv("ORBIT_GEMM_ROUND_SYNC"); return (e && e[0] == '0') ? 0 : 1; }();
+  return v != 0;
+}
 int l2_hint_mode() {
   static const int v = [] { const char* e = getenv("ORBIT_GEMM_L2HINT"); return e ? atoi(e) : 1; }();
   return v;
@@ -408,6 +444,16 @@ int launch2(const CUtensorMap& ma, const CUtensorMap& mb, const CUtensorMap* mc,
       if (hm & 4) (bytes_a < bytes_b ? sc.hint_b : sc.hint_a) = 1;
     }
     if ((hm & 2) && bytes_c > 100e6) sc.hint_c = 1;
+  }
+  sc.round_bar = nullptr;
+  // only where the operands cannot stay in the 126 MB L2 anyway (C5: 1.2-1.4 GB per GEMM); at C3 / C4 sizes (< 70 MB per GEMM) the
+  // panels are L2-resident whatever the skew and the meeting costs 1-2 % of the step
+  if (round_sync_enabled() && tiles > 2 * clusters && 2.0 * K * ((double)M + N) * batch >= round_sync_min_bytes()) {
+    static std::atomic<unsigned int> next_slot{0};
+    static std::atomic<unsigned int*> base_c{nullptr};
+    unsigned int* base = base_c.load(std::memory_order_relaxed);
+    if (!base) { ORBIT_CUDA_CHECK(cudaGetSymbolAddress((void**)&base, g_round_bar)); base_c.store(base, std::memory_order_relaxed); }
+    sc.round_bar = base + 2 * (next_slot.fetch_add(1) % 64);      // zero on entry: static storage, then reset by the last cluster out
   }
   ORBIT_CUDA_CHECK(launch_pdl(gemm_tc2_kernel<A_MN, B_MN>, dim3(2 * clusters), dim3(NTHREADS), SMEM_BYTES, s, ma, mb, mc ? *mc : ma,
                               mx ? *mx : ma, (mc ? (g.out_dtype == ORBIT_F32 ? 4 : 1) : 0) | (mx ? 2 : 0), e, M, N, K, batch, g.c_bs,

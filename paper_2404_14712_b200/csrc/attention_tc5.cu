@@ -45,7 +45,13 @@ __device__ unsigned long long g_attn_probe[32];
 #define PWAIT(slot, bar, par) do { long long t0_ = clock64(); ptx::mbar_wait(bar, par); pw_[slot] += clock64() - t0_; } while (0)
 #define PTIME(slot, stmt) do { long long t0_ = clock64(); stmt; pw_[slot] += clock64() - t0_; } while (0)
 #define PFLUSH(a, b) do { if (pon_) for (int i_ = a; i_ <= b; i_++) atomicAdd(&g_attn_probe[i_], (unsigned long long)pw_[i_]); } while (0)
+#define PROBE_T0 const long long pt0_ = clock64()
+#define PSINCE(slot) pw_[slot] = clock64() - pt0_
+#define PSET(slot, v) pw_[slot] = (v)
 #else
+#define PROBE_T0
+#define PSINCE(slot)
+#define PSET(slot, v)
 #define PROBE_DECL
 #define PWAIT(slot, bar, par) ptx::mbar_wait(bar, par)
 #define PTIME(slot, stmt) stmt
@@ -384,9 +390,25 @@ constexpr int NTHB = 640;
 // i.e. 224 KB = 1750 cycles at 128 B/clk against 1024 cycles of MMA; without the operand tiles (written and read once
 // each) it is 160 KB.  A buffer of S^T / dP^T is then free only once the gradient MMAs that read it have completed.
 constexpr bool TS_DKV = true;
-// the same for dS in the dQ kernel measured no gain (C5: attention backward 417 vs 423-429 TFLOP/s of model FLOPs): that
-// kernel has one operand tile, not two, and releasing its S / dP buffer only after the dQ product costs the overlap back
+// the same for dS in the dQ kernel measured no gain, with two S / dP buffers (C5: attention backward 417 vs 423-429 TFLOP/s of
+// model FLOPs) and with three (ncu, same box: 312.4 vs 312.5 us at C5, 207.6 vs 207.7 us at C3 / C4).
 constexpr bool TS_DQ = false;
+// Q / dO as tensor-memory A operands of the S / dP products (dQ kernel): SLOWER, 339 us vs 312 us at C5 (368 us with dS in
+// tensor memory as well).  What the round-2 probes of this kernel say (A/B builds, C5, ncu per-launch times):
+//   timeline (ORBIT_PROBE_TIMELINE): 1565 cycles per 64-key tile; the S-issuing thread waits 150 of them on barriers and sits in
+//   tcgen05.mma issue for the rest (back-pressure of the tensor pipe), the softmax warps wait 640 cycles per tile for S / dP, the
+//   dQ issuer 570 for dS: the MMAs themselves take ~1400 cycles per tile against a floor of 768 (3 products of 128 x 64 x 128);
+//   no softmax work at all (ORBIT_PROBE_DQ_NOSM) 313 -> 282 us; no exponentials (.._NOEXP) 317 us; half the tcgen05.ld (.._HALFLD)
+//   319 us; one of eight k-steps of S / dP (.._NOS) 252 us; no dQ product (.._NOG) 280 us.
+// A model that fits all of these: one tcgen05.mma of M = 128, K = 16 costs max(N / 2, shared-memory operand bytes / 128 B/clk,
+// tensor-memory A bytes / 64 B/clk) cycles.  The A operand is 4 KB either way, so an SS product needs N >= 128 to reach the
+// floor (N = 64: 6 KB = 48 cycles against 32, i.e. 67 %) and a TS product costs 64 cycles whatever N is: equal to SS at
+// N = 128 (P V, dV, dK, dQ: no gain, no loss, less shared-memory traffic), slower at N = 64 (S, dP here).  Per tile: S 384 +
+// dP 384 + dQ 256 = 1024 cycles of operand reads, + 256 of TMA writes of K / V + 128 of dS writes ~ 1400.  The N = 64 of the
+// S / dP products is set by tensor memory (2 x 2 x 64 S / dP columns + 128 dQ columns; 128-key tiles would leave one buffer),
+// so this kernel stays at ~55 % of its tensor floor; the remedy is a CTA pair per 256 queries (cta_group::2 halves the B
+// operand and the K / V stream per SM: 40 cycles per S / dP instruction instead of 48) -- not built, see DESIGN.md §13.
+constexpr bool TSA_DQ = false;
 
 template <int DH>
 struct CfgB {
@@ -713,6 +735,28 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
   if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
 }
 
+// ---- measurement probes of the dQ kernel (A/B build only, ORBIT_NVCC_EXTRA; wrong results) ----------------------------
+#ifdef ORBIT_PROBE_DQ_NOS
+#define DQ_PROBE_KS(n) 1
+#else
+#define DQ_PROBE_KS(n) (n)
+#endif
+#ifdef ORBIT_PROBE_DQ_NOG
+#define DQ_PROBE_KG(n) 0
+#else
+#define DQ_PROBE_KG(n) (n)
+#endif
+#ifdef ORBIT_PROBE_DQ_NOEXP
+#define DQ_PROBE_EX2(x) (x)
+#else
+#define DQ_PROBE_EX2(x) fast_ex2(x)
+#endif
+#ifdef ORBIT_PROBE_DQ_NOSM
+#define DQ_PROBE_NG(n) 0
+#else
+#define DQ_PROBE_NG(n) (n)
+#endif
+
 // ---------------------------------------------------------------- dQ : rows = queries -------------------
 template <int DH>
 __global__ void __launch_bounds__(NTHB, 1)
@@ -727,9 +771,18 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   auto sK = [&](int st) { return sRing + st * 2 * C::SMALL; };
   auto sV = [&](int st) { return sRing + st * 2 * C::SMALL + C::SMALL; };
   constexpr int NST = C::NST_DQ;
+  // S / dP buffers: with dS kept in tensor memory a buffer stays busy until the dQ MMAs of its tile have read it, so a
+  // third one keeps the S / dP products of tile j+2 from waiting on them
+  // Q and dO (stationary) as tensor-memory A operands of the S / dP products where the columns allow it: those products
+  // then read only the streamed K / V tile from shared memory
+  constexpr int NB = !TS_DQ ? 2 : (TSA_DQ && 4 * BT + 2 * DH <= 512 && 6 * BT + 2 * DH > 512) ? 2 : 3;
+  constexpr bool TSA = TSA_DQ && 2 * NB * BT + 2 * DH <= 512;
+  static_assert(2 * NB * BT + DH <= 512, "attention backward (dQ): TMEM budget");
   const uint32_t q_full = bar, kv_full0 = bar + 8, kv_empty0 = kv_full0 + 8 * NST, s_full0 = kv_empty0 + 8 * NST,
-                 s_empty0 = s_full0 + 16, p_full0 = s_empty0 + 16, p_done0 = p_full0 + 16, tmem_slot = p_done0 + 16;
+                 s_empty0 = s_full0 + 8 * NB, p_full0 = s_empty0 + 8 * NB, p_done0 = p_full0 + 8 * NB, tmem_slot = p_done0 + 8 * NB;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  PROBE_DECL;
+  PROBE_T0;
   const int bh = blockIdx.y, b = bh / a.heads, h = bh - b * a.heads, N = a.N;
   const int q0 = blockIdx.x * 128;
   const int ntiles = (N + BT - 1) / BT;
@@ -738,10 +791,10 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmBig); ptx::prefetch_tmap(&tmSmall); ptx::prefetch_tmap(&tmdOBig);
-    ptx::mbar_init(q_full, 1);
+    ptx::mbar_init(q_full, TSA ? 16 : 1);
     for (int i = 0; i < NST; i++) { ptx::mbar_init(kv_full0 + 8 * i, 1); ptx::mbar_init(kv_empty0 + 8 * i, 1); }
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(s_full0 + 8 * i, 2);  ptx::mbar_init(s_empty0 + 8 * i, TS_DQ ? 1 : 8); }   // as in the dK / dV kernel
-    for (int i = 0; i < 2; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
+    for (int i = 0; i < NB; i++) { ptx::mbar_init(s_full0 + 8 * i, 2);  ptx::mbar_init(s_empty0 + 8 * i, TS_DQ ? 1 : 8); }   // as in the dK / dV kernel
+    for (int i = 0; i < NB; i++) { ptx::mbar_init(p_full0 + 8 * i, 8); ptx::mbar_init(p_done0 + 8 * i, 1); }
     ptx::fence_barrier_init();
   }
   if (warp == 1) { ptx::tmem_alloc(tmem_slot, 512); ptx::tmem_relinquish(); }
@@ -752,19 +805,19 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tmem_slot));
   pdl_wait();                                    // on-chip prologue done; first global access is below
   pdl_trigger();
-  const uint32_t tS = tmem, tdP = tmem + 2 * BT, tdQ = tmem + 4 * BT;
+  const uint32_t tS = tmem, tdP = tmem + NB * BT, tdQ = tmem + 2 * NB * BT, tQ = tdQ + DH, tdO = tQ + DH / 2;
 
   if (warp == 0) {
     if (lane == 0) {
-      ptx::mbar_expect_tx(q_full, 2 * C::BIG);
+      if (!TSA) ptx::mbar_expect_tx(q_full, 2 * C::BIG);
 #pragma unroll
-      for (int bk = 0; bk < C::NBLK; bk++) {
+      for (int bk = 0; bk < (TSA ? 0 : C::NBLK); bk++) {
         ptx::tma_load_2d(sQ + bk * C::BBLK, &tmBig, q_full, qc + bk * 64, row0 + q0);
         ptx::tma_load_2d(sdO + bk * C::BBLK, &tmdOBig, q_full, h * DH + bk * 64, row0 + q0);
       }
       for (int j = 0; j < ntiles; j++) {
         const int st = j % NST;
-        ptx::mbar_wait(kv_empty0 + 8 * st, ((j / NST) & 1) ^ 1);
+        PWAIT(0, kv_empty0 + 8 * st, ((j / NST) & 1) ^ 1);
         ptx::mbar_expect_tx(kv_full0 + 8 * st, 2 * C::SMALL);
 #pragma unroll
         for (int bk = 0; bk < C::NBLK; bk++) {
@@ -772,42 +825,46 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
           ptx::tma_load_2d(sV(st) + bk * C::SBLK, &tmSmall, kv_full0 + 8 * st, vc + bk * 64, row0 + j * BT);
         }
       }
+      PSINCE(11); PFLUSH(0, 0); PFLUSH(11, 11);
     }
   } else if (warp == 1 || warp >= NTHB / 32 - 2) {   // warp 1: dQ MMAs; last warp: S / dP MMAs
     if (lane == 0) {
       constexpr uint32_t idesc_s = ptx::make_idesc_bf16(128, BT, 0, 0);
       constexpr uint32_t idesc_g = ptx::make_idesc_bf16(128, DH, 0, 1);
       auto issue_s = [&](int j) {
-        const int st = j % NST, tb = j & 1;
-        ptx::mbar_wait(kv_full0 + 8 * st, (j / NST) & 1);
-        ptx::mbar_wait(s_empty0 + 8 * tb, ((j >> 1) & 1) ^ 1);
+        const int st = j % NST, tb = j % NB;
+        PWAIT(1, kv_full0 + 8 * st, (j / NST) & 1);
+        PWAIT(2, s_empty0 + 8 * tb, ((j / NB) & 1) ^ 1);
         ptx::tc_fence_after();
         const uint64_t dQ0 = ptx::make_smem_desc(sQ, 16, 1024), dO0 = ptx::make_smem_desc(sdO, 16, 1024);
         const uint64_t dKs = ptx::make_smem_desc(sK(st), 16, 1024), dVs = ptx::make_smem_desc(sV(st), 16, 1024);
         if (warp == NTHB / 32 - 1) {
 #pragma unroll
-          for (int ks = 0; ks < DH / 16; ks++) {
+          for (int ks = 0; ks < DQ_PROBE_KS(DH / 16); ks++) {
             const uint32_t ob = (ks >> 2) * C::BBLK + (ks & 3) * 32, os = (ks >> 2) * C::SBLK + (ks & 3) * 32;
-            ptx::mma_f16_ss(tS + tb * BT, desc_adv(dQ0, ob), desc_adv(dKs, os), idesc_s, ks != 0);
+            if (TSA) ptx::mma_f16_ts(tS + tb * BT, tQ + ks * 8, desc_adv(dKs, os), idesc_s, ks != 0);
+            else ptx::mma_f16_ss(tS + tb * BT, desc_adv(dQ0, ob), desc_adv(dKs, os), idesc_s, ks != 0);
           }
         } else {
 #pragma unroll
-          for (int ks = 0; ks < DH / 16; ks++) {
+          for (int ks = 0; ks < DQ_PROBE_KS(DH / 16); ks++) {
             const uint32_t ob = (ks >> 2) * C::BBLK + (ks & 3) * 32, os = (ks >> 2) * C::SBLK + (ks & 3) * 32;
-            ptx::mma_f16_ss(tdP + tb * BT, desc_adv(dO0, ob), desc_adv(dVs, os), idesc_s, ks != 0);
+            if (TSA) ptx::mma_f16_ts(tdP + tb * BT, tdO + ks * 8, desc_adv(dVs, os), idesc_s, ks != 0);
+            else ptx::mma_f16_ss(tdP + tb * BT, desc_adv(dO0, ob), desc_adv(dVs, os), idesc_s, ks != 0);
           }
         }
         ptx::mma_commit(s_full0 + 8 * tb);
       };
-      ptx::mbar_wait(q_full, 0);
+      PWAIT(15, q_full, 0);
       if (warp != 1) {
         for (int j = 0; j < ntiles; j++) issue_s(j);
+        if (warp == NTHB / 32 - 1) { PSINCE(8); PFLUSH(1, 2); PFLUSH(8, 8); PFLUSH(15, 15); }
       } else
       for (int j = 0; j < ntiles; j++) {
-        ptx::mbar_wait(kv_full0 + 8 * (j % NST), (j / NST) & 1);
-        const int pb = j & 1;
-        const uint32_t sdS = sdS0 + pb * C::PT;
-        ptx::mbar_wait(p_full0 + 8 * pb, (j >> 1) & 1);
+        PWAIT(3, kv_full0 + 8 * (j % NST), (j / NST) & 1);
+        const int pb = j % NB;
+        const uint32_t sdS = sdS0 + (pb & 1) * C::PT;
+        PWAIT(4, p_full0 + 8 * pb, (j / NB) & 1);
         ptx::tc_fence_after();
         const int st = j % NST;
         const uint64_t dSd = optile_desc<BT>(sdS), dKm = ptx::make_smem_desc(sK(st), C::SBLK, 1024);
@@ -818,12 +875,13 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
           ptx::mma_commit(s_empty0 + 8 * pb);
         } else {
 #pragma unroll
-          for (int ks = 0; ks < BT / 16; ks++)    // dQ += dS K_j   (contraction over the tile's 64 keys)
+          for (int ks = 0; ks < DQ_PROBE_KG(BT / 16); ks++)    // dQ += dS K_j   (contraction over the tile's 64 keys)
             ptx::mma_f16_ss(tdQ, desc_adv(dSd, ks * 32), desc_adv(dKm, ks * 2048), idesc_g, (j | ks) != 0);
         }
         ptx::mma_commit(kv_empty0 + 8 * st);
         ptx::mma_commit(p_done0 + 8 * pb);
       }
+      if (warp == 1) { PSINCE(9); PFLUSH(3, 4); PFLUSH(9, 9); }
     }
   } else {
     const int sw = warp - 2, grp = sw >> 3;                  // two groups of 8 warps alternate over the tiles (see NTHB)
@@ -833,17 +891,40 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
     const int qrow = q0 + r;
     const float lse2 = qrow < N ? a.lse[(size_t)bh * N + qrow] * LOG2E : 0.f;
     const float dl = qrow < N ? a.delta[(size_t)bh * N + qrow] : 0.f;
+    if (TSA) {                                               // this thread's row of Q / dO, a quarter of the columns per warp
+      const int part = sw >> 2;
+      const bf16* src = part < 2 ? (const bf16*)a.qkv + (size_t)(row0 + qrow) * a.ld + qc + part * (DH / 2)
+                                 : (const bf16*)a.dO + (size_t)(row0 + qrow) * a.lddo + h * DH + (part - 2) * (DH / 2);
+      const uint32_t dst = (part < 2 ? tQ + part * (DH / 4) : tdO + (part - 2) * (DH / 4)) + lane_off;
+#pragma unroll
+      for (int c = 0; c < DH / 32; c++) {                    // 8 columns = 16 bf16 per store
+        uint4 v0 = make_uint4(0, 0, 0, 0), v1 = v0;
+        if (qrow < N) { v0 = __ldg(reinterpret_cast<const uint4*>(src + c * 16)); v1 = __ldg(reinterpret_cast<const uint4*>(src + c * 16 + 8)); }
+        const uint32_t pk[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+        ptx::tmem_st_32x8(dst + c * 8, pk);
+      }
+      ptx::tmem_st_wait();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(q_full);
+    }
     for (int j = grp; j < ntiles; j += 2) {
-      const int st = grp;
-      ptx::mbar_wait(s_full0 + 8 * st, (j >> 1) & 1);
+      const int st = j % NB, ph = (j / NB) & 1;
+      PWAIT(5, s_full0 + 8 * st, ph);
       ptx::tc_fence_after();
       const int nvalid = N - j * BT - half * CW;             // keys (columns) >= N are masked (ragged last tile only)
 #pragma unroll
-      for (int g = 0; g < CW / 16; g++) {
+      for (int g = 0; g < DQ_PROBE_NG(CW / 16); g++) {
         uint32_t s[16], dp[16];
         ptx::tmem_ld_32x16(tS + st * BT + half * CW + g * 16 + lane_off, s);
+#ifndef ORBIT_PROBE_DQ_HALFLD
         ptx::tmem_ld_32x16(tdP + st * BT + half * CW + g * 16 + lane_off, dp);
+#endif
         ptx::tmem_ld_wait();
+#ifdef ORBIT_PROBE_DQ_HALFLD
+#pragma unroll
+        for (int c = 0; c < 16; c++) dp[c] = s[c];
+#endif
         if (!TS_DQ && g == CW / 16 - 1) {
           ptx::tc_fence_before();
           __syncwarp();
@@ -852,7 +933,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
         float ds[16];
 #pragma unroll
         for (int c = 0; c < 16; c++) {
-          const float pv = fast_ex2(__uint_as_float(s[c]) * sl2 - lse2);
+          const float pv = DQ_PROBE_EX2(__uint_as_float(s[c]) * sl2 - lse2);
           ds[c] = (g * 16 + c < nvalid) ? pv * (__uint_as_float(dp[c]) - dl) : 0.f;
         }
         if (TS_DQ) {
@@ -861,16 +942,22 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
           for (int i = 0; i < 8; i++) { __nv_bfloat162 t2 = __floats2bfloat162_rn(ds[2 * i], ds[2 * i + 1]); pk[i] = *reinterpret_cast<uint32_t*>(&t2); }
           ptx::tmem_st_32x8(tdP + st * BT + half * CW + g * 16 + lane_off, pk);
         } else {
-          if (g == 0 && j > 1) ptx::mbar_wait(p_done0 + 8 * st, ((j >> 1) & 1) ^ 1);
+          if (g == 0 && j >= NB) PWAIT(6, p_done0 + 8 * st, ph ^ 1);
           write_cols16<BT>(sdS0 + st * C::PT, r, ds, half * (CW / 16) + g);
         }
       }
+#ifdef ORBIT_PROBE_DQ_NOSM
+      if (j >= NB) ptx::mbar_wait(p_done0 + 8 * st, ph ^ 1);
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(s_empty0 + 8 * st);
+#endif
       if (TS_DQ) ptx::tmem_st_wait(); else ptx::fence_proxy_async();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full0 + 8 * st);
     }
-    if (ntiles > grp) { const int jl = ((ntiles - 1 - grp) & ~1) + grp; ptx::mbar_wait(p_done0 + 8 * grp, (jl >> 1) & 1); }
+    PSINCE(7);
+    if (ntiles > grp) { const int jl = ((ntiles - 1 - grp) & ~1) + grp; PWAIT(12, p_done0 + 8 * (jl % NB), (jl / NB) & 1); }
     named_bar_sync(3, 512);                                  // see the dK / dV kernel
     if (grp == 0) {
       ptx::tc_fence_after();
@@ -880,6 +967,7 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (warp == 2 && lane == 0) { PSINCE(13); PSET(10, ntiles); PFLUSH(5, 7); PFLUSH(10, 10); PFLUSH(12, 13); }
   if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
 }
 

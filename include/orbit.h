@@ -65,6 +65,17 @@ int orbit_tokenize(const orbit_embed_desc* d, const float* x, const void* Wp, co
 int orbit_tokenize_bwd(const orbit_embed_desc* d, const float* x, const void* dtok, void* dWp, void* dbp,
                        void* ws, size_t ws_bytes, void* stream);
 size_t orbit_tokenize_bwd_workspace_bytes(const orbit_embed_desc* d);
+/* orbit_tokenize_bwd for callers that cannot allocate a workspace (CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, results and kernels, but the fp32 accumulators live in a file-scope device array
+ * inside the library (csrc/tokenize_noalloc.cu) of orbit_tokenize_bwd_noalloc_max_bytes() = 16 MiB, held by every GPU
+ * that loads liborbit.so until the process exits.  Calls no cudaMalloc / cudaFree / allocating routine.
+ * ORBIT_ERR_WORKSPACE (nothing written) when orbit_tokenize_bwd_workspace_bytes(d) exceeds that maximum, i.e. when
+ * V (p*p + 1) D > 4 Mi.  All calls on a device share the one array (cleared by each call before use): calls that
+ * OVERLAP on the GPU -- different streams -- race and must be serialised by the caller; back-to-back calls on one
+ * stream are independent. */
+int orbit_tokenize_bwd_noalloc(const orbit_embed_desc* d, const float* x, const void* dtok, void* dWp, void* dbp,
+                               void* stream);
+size_t orbit_tokenize_bwd_noalloc_max_bytes(void);
 
 /* ---- a2 / a2': variable aggregation, cross-attention over the V tokens of a patch (R3, R4)
  * At every (b,l), X = tok[b,l] (V x D):  qt = q Wq + bq;  K = X Wk + bk;  U = X Wv + bv;  per head a:

@@ -123,6 +123,8 @@ if HAS_DEBUG_SWITCH:
 _proto("orbit_tokenize", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp])
 _proto("orbit_tokenize_bwd", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp, _sz, _vp])
 _proto("orbit_tokenize_bwd_workspace_bytes", _sz, [C.POINTER(orbit_embed_desc)])
+_proto("orbit_tokenize_bwd_noalloc", C.c_int, [C.POINTER(orbit_embed_desc), _vp, _vp, _vp, _vp, _vp])
+_proto("orbit_tokenize_bwd_noalloc_max_bytes", _sz, [])
 _proto("orbit_var_aggregate", C.c_int,
        [C.POINTER(orbit_agg_desc), _vp, C.POINTER(orbit_agg_params), _vp, _vp, _vp, _vp, _sz, _vp])
 _proto("orbit_var_aggregate_bwd", C.c_int,
@@ -177,7 +179,8 @@ EXPORTS = ["orbit_tokenize", "orbit_tokenize_bwd", "orbit_tokenize_bwd_workspace
            "orbit_debug_layernorm_fwd", "orbit_debug_layernorm_bwd", "orbit_debug_gemm_out",
            "orbit_rank_fwd_attn", "orbit_rank_fwd_mlp", "orbit_rank_fwd_out", "orbit_rank_bwd_mlp", "orbit_rank_bwd_attn",
            "orbit_rank_bwd_out", "orbit_rank_saved_bytes", "orbit_rank_bwd_workspace_bytes",
-           "orbit_grads_unscale_check", "orbit_grads_accumulate", "orbit_grad_scale_update"]
+           "orbit_grads_unscale_check", "orbit_grads_accumulate", "orbit_grad_scale_update",
+           "orbit_tokenize_bwd_noalloc", "orbit_tokenize_bwd_noalloc_max_bytes"]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------------------
@@ -243,6 +246,16 @@ def orbit_tokenize_bwd_workspace_bytes(d):
 def orbit_tokenize_bwd(d, x, dtok, dWp, dbp, ws, stream=None):
     _check(lib.orbit_tokenize_bwd(C.byref(d), _ptr(x), _ptr(dtok), _ptr(dWp), _ptr(dbp), _ptr(ws), ws.numel() * ws.element_size(),
                                   _stream(stream)), "orbit_tokenize_bwd")
+
+
+def orbit_tokenize_bwd_noalloc_max_bytes():
+    return lib.orbit_tokenize_bwd_noalloc_max_bytes()
+
+
+def orbit_tokenize_bwd_noalloc(d, x, dtok, dWp, dbp, stream=None):
+    """orbit_tokenize_bwd with the workspace inside the library (include/orbit.h): no allocation on the path."""
+    _check(lib.orbit_tokenize_bwd_noalloc(C.byref(d), _ptr(x), _ptr(dtok), _ptr(dWp), _ptr(dbp), _stream(stream)),
+           "orbit_tokenize_bwd_noalloc")
 
 
 def orbit_var_aggregate_saved_bytes(d):

@@ -465,6 +465,435 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
   if (warp == 0) { tc_fence_after(); tmem_dealloc(tacc0, TMEM_ACC_COLS); }
 }
 
+// ============================================ forward on tcgen05 ============================================
+// ncu of the mma.sync forward above (config 3): no unit is busy (DRAM 60 %, L2 54 %, issue slots 31 %); the 16 consumer warps
+// spend ~3/4 of their time in the ldmatrix -> HMMA -> store chains of a step (short-scoreboard / fixed-latency stalls) and only
+// 22 % waiting for data: a latency-bound consumer loop, ~1000 cycles per 128-column step.  (A variant that kept a patch's tile
+// resident across a 4- or 8-CTA cluster, exchanging the partial scores through distributed shared memory, read X once but was
+// 2.6x / 6.6x slower: 1.5k cycles per release-arrive on a peer's mbarrier, 5k per round of remote loads, per patch.)
+// Here the two products run on the 5th-generation tensor cores straight from the TMA tiles, issued by one thread:
+//   pass 1: S[v, a]   (TMEM, 128 lanes x 16 columns)  = sum over the chunks of  X[128 x 64] (A, K-major) . Ut[16 x 64]^T (B, K-major)
+//   pass 2: Xbar[a, d] (TMEM, lanes 0..15 of 128 x 128 columns, double buffered) = alpha^T[128 x V] (A, K-major, rows >= 16 zero) . X[V x 128 d] (B, MN-major: the same tiles)
+//           (X^T as an MN-major A operand with N = 16 took ~128 cycles per instruction: 780 cycles per 128-column step)
+// A stage is released by tcgen05.commit.  Four worker warps (one TMEM lane quarter each) read S, run the softmax over v through
+// shared memory as before (16 warps, one head each), write alpha^T as a 128B-swizzled K-major operand tile, and the first
+// quarter's four warps drain the pass-2 accumulators: thread = head row, 32 columns each = 64 contiguous bytes of Xbar.
+constexpr int AT5 = 128 * TB * 2;             // one 64-v block of the alpha^T operand tile: 128 rows x 128 bytes
+constexpr int NW5 = 16;                      // worker warps: TMEM lane quarter (warp & 3) x 4 heads of the 16 ((warp - 2) >> 2)
+constexpr int NT5 = 64 + NW5 * 32;           // warp 0 TMA producer, warp 1 MMA issuer, warps 2..17 workers
+__device__ __forceinline__ void worker_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
+struct T5Layout { int sX, sU, sAT, sS, bars, total; };
+__host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int stg) {
+  T5Layout L;
+  L.sX = 0;
+  L.sU = stg * 2 * Vp * TB * 2;
+  L.sAT = L.sU + stg * 2 * UT;                 // multiple of 1024: Vp * 128 is a multiple of 2048
+  L.sS = L.sAT + 2 * AT5;                      // (the 128-row A operand of pass 1 reads past the Vp rows of a sub-tile: into the next one / sU)
+  L.bars = L.sS + VP_MAX * SROW * 4;
+  L.total = L.bars + 8 * (2 * stg + 6) + 16;
+  return L;
+}
+#ifdef ORBIT_PROBE_AGG_P1ONLY   // A/B build only: pass 1 alone (no second read of X, no Xbar): wrong results
+#define AGG_PROBE_PASSES 1
+#else
+#define AGG_PROBE_PASSES 2
+#endif
+// SM-inbound traffic is what bounds this kernel (pass 1 alone streams X from DRAM at 5.2 TB/s; the second read, from L2, adds
+// its bytes to the same ~6.5 TB/s L2 -> SM budget instead of overlapping), so the last R steps of pass 1 are KEPT in the ring
+// and pass 2 starts with them: R / nch of the second read never happens.  The ring stays FIFO: pass 1 releases steps
+// 0 .. nch-R-1, pass 2 releases the kept ones in ring order, then the re-loaded chunks nch-R-1 .. 0.
+#ifdef ORBIT_PROBE_AGG          // A/B build only: cycles the MMA-issuing thread of CTA 0 spends in its waits, per patch
+#define TPROBE_DECL long long tp_[6] = {0, 0, 0, 0, 0, 0}; const long long tt0_ = clock64()
+#define TPROBE(slot, stmt) do { long long t0_ = clock64(); stmt; tp_[slot] += clock64() - t0_; } while (0)
+#define TPROBE_PRINT do { if (blockIdx.x == 0 && npat > 0) printf("agg t5 probe: patches %d  per patch: total %lld  wait pass-1 data %lld  wait alpha %lld  wait pass-2 data %lld  wait o_empty %lld  issue pass-1 %lld  issue pass-2 %lld\n", npat, (clock64() - tt0_) / npat, tp_[0] / npat, tp_[1] / npat, tp_[2] / npat, tp_[3] / npat, tp_[4] / npat, tp_[5] / npat); } while (0)
+#else
+#define TPROBE_DECL
+#define TPROBE(slot, stmt) stmt
+#define TPROBE_PRINT
+#endif
+__global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constant__ CUtensorMap tmX,
+    const __grid_constant__ CUtensorMap tmU, float* __restrict__ alpha, bf16* __restrict__ Xbar, int BL, int V, int D, int h,
+    int STG, int R) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
+  const int Vp = (V + 15) & ~15, XTb = Vp * TB * 2;
+  const T5Layout L = t5_fwd_layout(Vp, STG);
+  const uint32_t sX = s_u32(smem) + L.sX, sU = s_u32(smem) + L.sU, sAT = s_u32(smem) + L.sAT;
+  float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [128][SROW]
+  const uint32_t bar0 = s_u32(smem) + L.bars, ebar0 = bar0 + 8 * STG, s_full = ebar0 + 8 * STG, at_full = s_full + 8,
+                 o_full0 = at_full + 8, o_empty0 = o_full0 + 16, tslot = o_empty0 + 16;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nch = D / (2 * TB), mtiles = Vp / 16;
+  const int nre = (AGG_PROBE_PASSES - 1) * (nch - R);        // chunks read a second time
+  const int np2 = (AGG_PROBE_PASSES - 1) * nch;              // pass-2 steps
+
+  for (int j = 0; j < STG * 2; j++) zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(ebar0 + 8 * i, 1); }
+    mbar_init(s_full, 1); mbar_init(at_full, 1);
+    for (int i = 0; i < 2; i++) { mbar_init(o_full0 + 8 * i, 1); mbar_init(o_empty0 + 8 * i, 4); }
+    fence_barrier_init();
+  }
+  if (warp == 1) { tmem_alloc(tslot, 512); tmem_relinquish(); }
+  for (int i = threadIdx.x; i < 2 * AT5 / 16; i += NT5) reinterpret_cast<uint4*>(smem + L.sAT)[i] = make_uint4(0, 0, 0, 0);   // rows 16..127 of alpha^T stay zero
+  fence_proxy_async();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
+  const uint32_t tS = tmem, tO = tmem + 128;
+
+  const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+  if (warp == 0) {
+    if (lane == 0) {
+      int st = 0; uint32_t ph = 0;
+      for (int pi = 0; pi < npat; pi++) {
+        const int row0 = (blockIdx.x + pi * gridDim.x) * V;
+        for (int i = 0; i < nch + nre; i++) {            // pass 1 (X and Ut chunks), then the second read of chunks nch-R-1 .. 0
+          const int c = i < nch ? i : 2 * nch - R - 1 - i;
+          const uint32_t bar = bar0 + 8 * st;
+          mbar_wait(ebar0 + 8 * st, ph ^ 1);
+          mbar_expect_tx(bar, 2 * (V * TB * 2 + (i < nch ? UT : 0)));
+#pragma unroll
+          for (int j = 0; j < 2; j++) {
+            tma_load_2d(sX + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, row0);
+            if (i < nch) tma_load_2d(sU + (st * 2 + j) * UT, &tmU, bar, (c * 2 + j) * TB, 0);
+          }
+          if (++st == STG) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0), idesc2 = make_idesc_bf16(128, 2 * TB, 0, 1);
+      int st = 0; uint32_t ph = 0, u = 0;
+      TPROBE_DECL;
+      for (int pi = 0; pi < npat; pi++) {
+        int kst = 0;                                     // ring slot of the first kept step
+        for (int i = 0; i < nch; i++) {
+          TPROBE(0, mbar_wait(bar0 + 8 * st, ph));
+          tc_fence_after();
+          TPROBE(4, {
+#pragma unroll
+          for (int j = 0; j < 2; j++)
+#pragma unroll
+            for (int ks = 0; ks < TB / 16; ks++)
+              mma_f16_ss(tS, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
+                         make_smem_desc(sU + (st * 2 + j) * UT + ks * 32, 16, 1024), idesc1, (i | j | ks) != 0);
+          });
+          if (i == nch - R) kst = st;
+          if (i < nch - R || AGG_PROBE_PASSES == 1) mma_commit(ebar0 + 8 * st);
+          if (++st == STG) { st = 0; ph ^= 1; }
+        }
+        mma_commit(s_full);
+        TPROBE(1, mbar_wait(at_full, pi & 1));
+        for (int i = 0; i < np2; i++, u++) {
+          const uint32_t ob = u & 1;
+          int slot;
+          if (i < R) { slot = kst; if (++kst == STG) kst = 0; }          // kept steps: already in shared memory
+          else { slot = st; TPROBE(2, mbar_wait(bar0 + 8 * st, ph)); if (++st == STG) { st = 0; ph ^= 1; } }
+          TPROBE(3, mbar_wait(o_empty0 + 8 * ob, ((u >> 1) & 1) ^ 1));
+          tc_fence_after();
+          TPROBE(5, {
+          for (int ks = 0; ks < mtiles; ks++)
+            mma_f16_ss(tO + ob * (2 * TB), make_smem_desc(sAT + (ks >> 2) * AT5 + (ks & 3) * 32, 16, 1024),
+                       make_smem_desc(sX + (slot * 2) * XTb + ks * 2048, XTb, 1024), idesc2, ks != 0);
+          });
+          mma_commit(ebar0 + 8 * slot);
+          mma_commit(o_full0 + 8 * ob);
+        }
+      }
+      TPROBE_PRINT;
+    }
+  } else {
+    const int w = warp - 2, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
+    const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
+    uint8_t* at = smem + L.sAT;
+    uint32_t u = 0;
+    for (int pi = 0; pi < npat; pi++) {
+      const int bl = blockIdx.x + pi * gridDim.x;
+      mbar_wait(s_full, pi & 1);
+      tc_fence_after();
+      uint32_t sv[4];
+      tmem_ld_32x4(tS + sub * 4 + lane_off, sv);
+      tmem_ld_wait();
+#pragma unroll
+      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]);
+      tc_fence_before();
+      worker_sync();
+      // ---- softmax over v per head (one warp each); alpha -> global (fp32), alpha^T -> the K-major operand tile (two blocks
+      // of 64 v, 128B swizzle)
+      {
+        const int a = w;
+        float m = -INFINITY, l = 0.f;
+        if (a < h) {
+          for (int v = lane; v < V; v += 32) m = fmaxf(m, sS[v * SROW + a]);
+          m = warp_max(m);
+          for (int v = lane; v < V; v += 32) l += __expf(sS[v * SROW + a] - m);
+          l = warp_sum(l);
+        }
+        const float inv = a < h ? 1.f / l : 0.f;
+        for (int v = lane; v < 2 * TB; v += 32) {
+          const float p = (a < h && v < V) ? __expf(sS[v * SROW + a] - m) * inv : 0.f;
+          if (a < h && v < V) alpha[((size_t)bl * h + a) * V + v] = p;
+          *reinterpret_cast<bf16*>(at + (v >> 6) * AT5 + a * 128 + ((((v & 63) >> 3) ^ (a & 7)) << 4) + (v & 7) * 2) = __float2bfloat16_rn(p);
+        }
+      }
+      fence_proxy_async();
+      worker_sync();
+      if (w == 0 && lane == 0) mbar_arrive(at_full);
+      // ---- pass 2: drain Xbar^T[d, a] of each 128-column chunk: the kept chunks nch-R .. nch-1, then nch-R-1 .. 0
+      for (int i = 0; i < np2; i++, u++) {
+        const uint32_t ob = u & 1;
+        const int c = i < R ? nch - R + i : nch - 1 - i;
+        if (quarter != 0) continue;                            // the 16 head rows sit in TMEM lanes 0..15: the first quarter's warps
+        mbar_wait(o_full0 + 8 * ob, (u >> 1) & 1);
+        tc_fence_after();
+        uint32_t ov[32];
+        tmem_ld_32x32(tO + ob * (2 * TB) + sub * 32, ov);      // this warp's 32 of the chunk's 128 columns
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(o_empty0 + 8 * ob);
+        if (lane < h) {
+          uint4* dst = reinterpret_cast<uint4*>(Xbar + ((size_t)bl * h + lane) * D + c * (2 * TB) + sub * 32);
+#pragma unroll
+          for (int q = 0; q < 4; q++)
+            __stcs(dst + q, make_uint4(pack_bf16(__uint_as_float(ov[q * 8]), __uint_as_float(ov[q * 8 + 1])),
+                                       pack_bf16(__uint_as_float(ov[q * 8 + 2]), __uint_as_float(ov[q * 8 + 3])),
+                                       pack_bf16(__uint_as_float(ov[q * 8 + 4]), __uint_as_float(ov[q * 8 + 5])),
+                                       pack_bf16(__uint_as_float(ov[q * 8 + 6]), __uint_as_float(ov[q * 8 + 7]))));
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
+}
+
+// ============================================ backward on tcgen05 ============================================
+// Same structure as the forward: the TMA ring feeds one MMA-issuing thread, 16 worker warps own the TMEM lanes.
+//   pass 1: dalpha[v, a] (TMEM, 16 columns) = sum over chunks of X[128 x 64] (A, K-major) . dXbar[16 x 64]^T (B, K-major)
+//   workers: dalpha -> shared memory, ds = alpha (dalpha - sum_w alpha_w dalpha_w); (alpha | ds) as packed bf16 INTO TENSOR MEMORY
+//            (thread = token row v: the A operand of the dX product, never in shared memory), ds^T as a K-major B tile
+//   pass 2, per 64-column sub-tile:  dX[v, d] (TMEM, 64 columns, double buffered) = (alpha | ds)[128 x 32] (A, TMEM)
+//                                                                               . [dXbar ; Ut][32 x 64] (B, MN-major)
+//           per 128-column step:     dUt^T[d, a] (TMEM, 16 columns per step, kept for ALL patches of the CTA)
+//                                      += X^T[128 d x V] (A, MN-major: the X tiles as they are) . ds^T[16 x V]^T (B, K-major)
+//   workers drain dX (thread = token row, 16 columns = 32 bytes each) and, after the last patch, dUt^T (fp32 atomics).
+// The last R steps of pass 1 stay in the ring for pass 2 (as in the forward); their Ut chunks come with them.
+constexpr int BT5 = 2 * UT;                  // B tile of a 64-column sub-tile: rows 0-15 dXbar, rows 16-31 Ut
+struct T5BLayout { int sX, sB, sDT, sS, sAl, bars, total; };
+__host__ __device__ inline T5BLayout t5_bwd_layout(int Vp, int stg) {
+  T5BLayout L;
+  L.sX = 0;
+  L.sB = stg * 2 * Vp * TB * 2;
+  L.sDT = L.sB + stg * 2 * BT5;
+  L.sS = L.sDT + 2 * UT;
+  L.sAl = L.sS + VP_MAX * SROW * 4;
+  L.bars = L.sAl + VP_MAX * SROW * 4;
+  L.total = L.bars + 8 * (2 * stg + 8) + 16;
+  return L;
+}
+
+__global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constant__ CUtensorMap tmX,
+    const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmU, const float* __restrict__ alpha,
+    bf16* __restrict__ dtok, float* __restrict__ dUt_acc, int BL, int V, int D, int h, int STG, int R) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
+  const int Vp = (V + 15) & ~15, XTb = Vp * TB * 2;
+  const T5BLayout L = t5_bwd_layout(Vp, STG);
+  const uint32_t sX = s_u32(smem) + L.sX, sB = s_u32(smem) + L.sB, sDT = s_u32(smem) + L.sDT;
+  float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [128][SROW] dalpha, then ds
+  float* sAl = reinterpret_cast<float*>(smem + L.sAl);                        // [128][SROW] alpha
+  const uint32_t bar0 = s_u32(smem) + L.bars, ebar0 = bar0 + 8 * STG, a_full = ebar0 + 8 * STG, ad_full = a_full + 8,
+                 x_full0 = ad_full + 8, x_empty0 = x_full0 + 16, u_done = x_empty0 + 16, tslot = u_done + 8;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nch = D / (2 * TB), mtiles = Vp / 16;
+  const int nre = nch - R;
+
+  for (int j = 0; j < STG * 2; j++) {
+    zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);
+    zero_tail_rows(smem + L.sB + j * BT5, h, HP, NT5);                          // dXbar rows h..15 (the TMA box has h rows)
+  }
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(ebar0 + 8 * i, 1); }
+    mbar_init(a_full, 1); mbar_init(ad_full, 1); mbar_init(u_done, 1);
+    for (int i = 0; i < 2; i++) { mbar_init(x_full0 + 8 * i, 1); mbar_init(x_empty0 + 8 * i, NW5); }
+    fence_barrier_init();
+  }
+  if (warp == 1) { tmem_alloc(tslot, 512); tmem_relinquish(); }
+  fence_proxy_async();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
+  const uint32_t tA = tmem, tAD = tmem + 16, tdX = tmem + 32, tdU = tmem + 32 + 2 * TB;
+
+  const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+  if (warp == 0) {
+    if (lane == 0) {
+      int st = 0; uint32_t ph = 0;
+      for (int pi = 0; pi < npat; pi++) {
+        const int bl = blockIdx.x + pi * gridDim.x;
+        for (int i = 0; i < nch + nre; i++) {            // pass 1 (X, dXbar; Ut too for the kept steps), then chunks nch-R-1 .. 0 again
+          const int c = i < nch ? i : 2 * nch - R - 1 - i;
+          const bool ut = i >= nch - R;
+          const uint32_t bar = bar0 + 8 * st;
+          mbar_wait(ebar0 + 8 * st, ph ^ 1);
+          mbar_expect_tx(bar, 2 * ((V + h) * TB * 2 + (ut ? UT : 0)));
+#pragma unroll
+          for (int j = 0; j < 2; j++) {
+            tma_load_2d(sX + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, bl * V);
+            tma_load_2d(sB + (st * 2 + j) * BT5, &tmG, bar, (c * 2 + j) * TB, bl * h);
+            if (ut) tma_load_2d(sB + (st * 2 + j) * BT5 + UT, &tmU, bar, (c * 2 + j) * TB, 0);
+          }
+          if (++st == STG) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0), idesc_x = make_idesc_bf16(128, TB, 0, 1),
+                         idesc_u = make_idesc_bf16(128, HP, 1, 0);
+      int st = 0; uint32_t ph = 0, u = 0;
+      for (int pi = 0; pi < npat; pi++) {
+        int kst = 0;
+        for (int i = 0; i < nch; i++) {
+          mbar_wait(bar0 + 8 * st, ph);
+          tc_fence_after();
+#pragma unroll
+          for (int j = 0; j < 2; j++)
+#pragma unroll
+            for (int ks = 0; ks < TB / 16; ks++)
+              mma_f16_ss(tA, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
+                         make_smem_desc(sB + (st * 2 + j) * BT5 + ks * 32, 16, 1024), idesc1, (i | j | ks) != 0);
+          if (i == nch - R) kst = st;
+          if (i < nch - R) mma_commit(ebar0 + 8 * st);
+          if (++st == STG) { st = 0; ph ^= 1; }
+        }
+        mma_commit(a_full);
+        mbar_wait(ad_full, pi & 1);
+        for (int i = 0; i < nch; i++) {
+          int slot;
+          if (i < R) { slot = kst; if (++kst == STG) kst = 0; }
+          else { slot = st; mbar_wait(bar0 + 8 * st, ph); if (++st == STG) { st = 0; ph ^= 1; } }
+          const int c = i < R ? nch - R + i : nch - 1 - i;
+          tc_fence_after();
+#pragma unroll
+          for (int j = 0; j < 2; j++, u++) {
+            const uint32_t xb = u & 1;
+            mbar_wait(x_empty0 + 8 * xb, ((u >> 1) & 1) ^ 1);
+            tc_fence_after();
+#pragma unroll
+            for (int ks = 0; ks < 2; ks++)                 // k = (alpha | ds): rows 0-15 dXbar, 16-31 Ut of the B tile
+              mma_f16_ts(tdX + xb * TB, tAD + ks * 8, make_smem_desc(sB + (slot * 2 + j) * BT5 + ks * 2048, 16, 1024), idesc_x, ks != 0);
+            mma_commit(x_full0 + 8 * xb);
+          }
+          for (int ks = 0; ks < mtiles; ks++)
+            mma_f16_ss(tdU + c * HP, make_smem_desc(sX + (slot * 2) * XTb + ks * 2048, XTb, 1024),
+                       make_smem_desc(sDT + (ks >> 2) * UT + (ks & 3) * 32, 16, 1024), idesc_u, (pi | ks) != 0);
+          mma_commit(ebar0 + 8 * slot);
+        }
+      }
+      mma_commit(u_done);
+    }
+  } else {
+    const int w = warp - 2, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
+    const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
+    uint8_t* dt = smem + L.sDT;
+    uint32_t u = 0;
+    for (int pi = 0; pi < npat; pi++) {
+      const int bl = blockIdx.x + pi * gridDim.x;
+      // alpha of this patch (dead since the previous patch's (alpha | ds) went to tensor memory)
+      for (int i = threadIdx.x - 64; i < 128 * HP; i += NW5 * 32) {
+        const int a = i >> 7, v = i & 127;
+        sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
+      }
+      mbar_wait(a_full, pi & 1);
+      tc_fence_after();
+      uint32_t sv[4];
+      tmem_ld_32x4(tA + sub * 4 + lane_off, sv);
+      tmem_ld_wait();
+#pragma unroll
+      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]);
+      tc_fence_before();
+      worker_sync();
+      // ---- ds[v, a] = alpha (dalpha - sum_w alpha_w dalpha_w), one head per warp; ds^T -> the K-major B tile of the dUt product
+      {
+        const int a = w;
+        float dot = 0.f;
+        for (int v = lane; v < V; v += 32) dot += sAl[v * SROW + a] * sS[v * SROW + a];
+        dot = warp_sum(dot);
+        for (int v = lane; v < 2 * TB; v += 32) {
+          const float ds = v < V ? sAl[v * SROW + a] * (sS[v * SROW + a] - dot) : 0.f;   // (rows >= Vp of dalpha are not data)
+          sS[v * SROW + a] = ds;
+          *reinterpret_cast<bf16*>(dt + (v >> 6) * UT + a * 128 + ((((v & 63) >> 3) ^ (a & 7)) << 4) + (v & 7) * 2) = __float2bfloat16_rn(ds);
+        }
+      }
+      worker_sync();
+      // ---- (alpha | ds) of this thread's token row -> tensor memory: warp (quarter, sub) writes k = 8 sub .. 8 sub + 7
+      {
+        const float* src = (sub < 2 ? sAl : sS) + r * SROW + (sub & 1) * 8;
+        uint32_t pk[4];
+#pragma unroll
+        for (int q = 0; q < 4; q++) pk[q] = pack_bf16(src[2 * q], src[2 * q + 1]);
+        tmem_st_32x4(tAD + sub * 4 + lane_off, pk);
+        tmem_st_wait();
+      }
+      tc_fence_before();
+      fence_proxy_async();
+      worker_sync();
+      if (w == 0 && lane == 0) mbar_arrive(ad_full);
+      // ---- pass 2: drain dX of each 64-column sub-tile: thread = token row, this warp's 16 columns
+      for (int i = 0; i < nch; i++) {
+        const int c = i < R ? nch - R + i : nch - 1 - i;
+#pragma unroll
+        for (int j = 0; j < 2; j++, u++) {
+          const uint32_t xb = u & 1;
+          mbar_wait(x_full0 + 8 * xb, (u >> 1) & 1);
+          tc_fence_after();
+          uint32_t ov[16];
+          tmem_ld_32x16(tdX + xb * TB + sub * 16 + lane_off, ov);
+          tmem_ld_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(x_empty0 + 8 * xb);
+          if (r < V) {
+            uint4* dst = reinterpret_cast<uint4*>(dtok + ((size_t)bl * V + r) * D + (c * 2 + j) * TB + sub * 16);
+#pragma unroll
+            for (int q = 0; q < 2; q++)
+              __stcs(dst + q, make_uint4(pack_bf16(__uint_as_float(ov[q * 8]), __uint_as_float(ov[q * 8 + 1])),
+                                         pack_bf16(__uint_as_float(ov[q * 8 + 2]), __uint_as_float(ov[q * 8 + 3])),
+                                         pack_bf16(__uint_as_float(ov[q * 8 + 4]), __uint_as_float(ov[q * 8 + 5])),
+                                         pack_bf16(__uint_as_float(ov[q * 8 + 6]), __uint_as_float(ov[q * 8 + 7]))));
+          }
+        }
+      }
+    }
+    // ---- dUt^T accumulated over all patches of this CTA: thread = column d of a 128-column step, this warp's 4 heads
+    if (npat > 0) {
+      mbar_wait(u_done, 0);
+      tc_fence_after();
+      for (int c = 0; c < nch; c++) {
+        uint32_t av[4];
+        tmem_ld_32x4(tdU + c * HP + sub * 4 + lane_off, av);
+        tmem_ld_wait();
+        const int d = c * (2 * TB) + r;
+#pragma unroll
+        for (int q = 0; q < 4; q++)
+          if (sub * 4 + q < h) atomicAdd(dUt_acc + (size_t)d * h + sub * 4 + q, __uint_as_float(av[q]));
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
+}
+
 // Ut [D, h] fp32 -> Utb [HP, D] bf16 (rows >= h zero)
 __global__ void agg_ut_to_bf16_kernel(const float* __restrict__ Ut, bf16* __restrict__ Utb, int D, int h) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -515,6 +944,11 @@ bool agg_tc_supported(int dt, int V, int D, int heads) {
 }
 size_t agg_tc_utb_bytes(int D) { return (size_t)HP * D * sizeof(bf16); }
 
+bool t5_enabled() {                     // ORBIT_AGG_T5=0: the mma.sync ring kernels (A/B)
+  static const int v = [] { const char* e = getenv("ORBIT_AGG_T5"); return (e && e[0] == '0') ? 0 : 1; }();
+  return v != 0;
+}
+
 int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, void* Xbar, int BL, int V, int D, int heads,
                      cudaStream_t s) {
   agg_ut_to_bf16_kernel<<<cdiv((long long)HP * D, 256), 256, 0, s>>>(Ut, (bf16*)Utb, D, heads);
@@ -522,6 +956,22 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
   CUtensorMap tmX, tmU;
   ORBIT_TRY(make_map(&tmX, tok, (long long)BL * V, D, V));
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
+  if (t5_enabled()) {
+    const int Vp = (V + 15) & ~15;
+    int stg = 12;
+    while (stg > 2 && 1024 + (size_t)t5_fwd_layout(Vp, stg).total > SMEM_MAX) stg--;
+    const size_t smb = 1024 + (size_t)t5_fwd_layout(Vp, stg).total;
+    ORBIT_SMEM_ATTR(agg_fwd_t5_kernel, SMEM_MAX);
+    const int grid = BL < num_sms() ? BL : num_sms();
+    static const int keep_env = [] { const char* e = getenv("ORBIT_AGG_KEEP"); return e ? atoi(e) : -1; }();
+    const int nch = D / (2 * TB);
+    int keep = keep_env >= 0 ? keep_env : stg - 2;     // kept steps of pass 1; the other slots prefetch during the softmax
+    if (keep > stg - 1) keep = stg - 1;
+    if (keep > nch) keep = nch;
+    agg_fwd_t5_kernel<<<grid, NT5, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads, stg, keep);
+    ORBIT_LAUNCH_CHECK();
+    return ORBIT_OK;
+  }
   constexpr int STG = 5;                // 5 x 36 KB stages + 13 KB, one CTA per SM
   const size_t smb = fwd_smem(STG);
   ORBIT_SMEM_ATTR(agg_fwd_tma_kernel<STG>, smb);
@@ -537,6 +987,22 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
   ORBIT_TRY(make_map(&tmX, tok, (long long)BL * V, D, V));
   ORBIT_TRY(make_map(&tmG, dXbar, (long long)BL * heads, D, heads));
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
+  if (t5_enabled() && D <= 2048) {      // dUt^T of all D / 128 steps stays in tensor memory: 16 columns each beside 160 others
+    const int Vp = (V + 15) & ~15;
+    int stg = 12;
+    while (stg > 2 && 1024 + (size_t)t5_bwd_layout(Vp, stg).total > SMEM_MAX) stg--;
+    const size_t smb = 1024 + (size_t)t5_bwd_layout(Vp, stg).total;
+    ORBIT_SMEM_ATTR(agg_bwd_t5_kernel, SMEM_MAX);
+    static const int keep_env = [] { const char* e = getenv("ORBIT_AGG_KEEP"); return e ? atoi(e) : -1; }();
+    const int nch = D / (2 * TB);
+    int keep = keep_env >= 0 ? keep_env : stg - 2;
+    if (keep > stg - 1) keep = stg - 1;
+    if (keep > nch) keep = nch;
+    const int grid5 = BL < num_sms() ? BL : num_sms();
+    agg_bwd_t5_kernel<<<grid5, NT5, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads, stg, keep);
+    ORBIT_LAUNCH_CHECK();
+    return ORBIT_OK;
+  }
   const int grid = BL < 148 ? BL : 148;
   int stg = 12;                         // deepest ring that fits (the dUt accumulator is in tensor memory)
   while (stg > 2 && bwd_smem(V, D, stg) > SMEM_MAX) stg -= (stg > 6 ? 2 : 1);

@@ -503,10 +503,12 @@ __host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int stg) {
 // and pass 2 starts with them: R / nch of the second read never happens.  The ring stays FIFO: pass 1 releases steps
 // 0 .. nch-R-1, pass 2 releases the kept ones in ring order, then the re-loaded chunks nch-R-1 .. 0.
 #ifdef ORBIT_PROBE_AGG          // A/B build only: cycles the MMA-issuing thread of CTA 0 spends in its waits, per patch
-#define TPROBE_DECL long long tp_[6] = {0, 0, 0, 0, 0, 0}; const long long tt0_ = clock64()
+#define TPROBE_DECL long long tp_[7] = {0, 0, 0, 0, 0, 0, 0}; const long long tt0_ = clock64()
 #define TPROBE(slot, stmt) do { long long t0_ = clock64(); stmt; tp_[slot] += clock64() - t0_; } while (0)
 #define TPROBE_PRINT do { if (blockIdx.x == 0 && npat > 0) printf("agg t5 probe: patches %d  per patch: total %lld  wait pass-1 data %lld  wait alpha %lld  wait pass-2 data %lld  wait o_empty %lld  issue pass-1 %lld  issue pass-2 %lld\n", npat, (clock64() - tt0_) / npat, tp_[0] / npat, tp_[1] / npat, tp_[2] / npat, tp_[3] / npat, tp_[4] / npat, tp_[5] / npat); } while (0)
+#define TPROBE_PRINT7 do { if (blockIdx.x == 0 && npat > 0) printf("agg bwd t5 probe: patches %d  per patch: total %lld  wait pass-1 data %lld  wait (alpha|ds) %lld  wait pass-2 data %lld  wait x_empty %lld  issue pass-1 %lld  issue dX %lld  issue dUt %lld\n", npat, (clock64() - tt0_) / npat, tp_[0] / npat, tp_[1] / npat, tp_[2] / npat, tp_[3] / npat, tp_[4] / npat, tp_[5] / npat, tp_[6] / npat); } while (0)
 #else
+#define TPROBE_PRINT7
 #define TPROBE_DECL
 #define TPROBE(slot, stmt) stmt
 #define TPROBE_PRINT
@@ -685,13 +687,22 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
 //   workers drain dX (thread = token row, 16 columns = 32 bytes each) and, after the last patch, dUt^T (fp32 atomics).
 // The last R steps of pass 1 stay in the ring for pass 2 (as in the forward); their Ut chunks come with them.
 constexpr int BT5 = 2 * UT;                  // B tile of a 64-column sub-tile: rows 0-15 dXbar, rows 16-31 Ut
-struct T5BLayout { int sX, sB, sDT, sS, sAl, bars, total; };
+constexpr int OT5 = 32 * TB * 2;             // dX staging tile of one TMEM lane quarter: 32 token rows x 64 columns, 128B swizzle
+__device__ __forceinline__ void quarter_sync(int q) { asm volatile("bar.sync %0, 128;" ::"r"(2 + q) : "memory"); }
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(m), "r"(src), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+struct T5BLayout { int sX, sB, sDT, sO, sS, sAl, bars, total; };
 __host__ __device__ inline T5BLayout t5_bwd_layout(int Vp, int stg) {
   T5BLayout L;
   L.sX = 0;
   L.sB = stg * 2 * Vp * TB * 2;
   L.sDT = L.sB + stg * 2 * BT5;
-  L.sS = L.sDT + 2 * UT;
+  L.sO = L.sDT + 2 * UT;
+  L.sS = L.sO + 8 * OT5;
   L.sAl = L.sS + VP_MAX * SROW * 4;
   L.bars = L.sAl + VP_MAX * SROW * 4;
   L.total = L.bars + 8 * (2 * stg + 8) + 16;
@@ -699,13 +710,13 @@ __host__ __device__ inline T5BLayout t5_bwd_layout(int Vp, int stg) {
 }
 
 __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constant__ CUtensorMap tmX,
-    const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmU, const float* __restrict__ alpha,
-    bf16* __restrict__ dtok, float* __restrict__ dUt_acc, int BL, int V, int D, int h, int STG, int R) {
+    const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmD,
+    const float* __restrict__ alpha, float* __restrict__ dUt_acc, int BL, int V, int D, int h, int STG, int R) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
   const int Vp = (V + 15) & ~15, XTb = Vp * TB * 2;
   const T5BLayout L = t5_bwd_layout(Vp, STG);
-  const uint32_t sX = s_u32(smem) + L.sX, sB = s_u32(smem) + L.sB, sDT = s_u32(smem) + L.sDT;
+  const uint32_t sX = s_u32(smem) + L.sX, sB = s_u32(smem) + L.sB, sDT = s_u32(smem) + L.sDT, sO = s_u32(smem) + L.sO;
   float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [128][SROW] dalpha, then ds
   float* sAl = reinterpret_cast<float*>(smem + L.sAl);                        // [128][SROW] alpha
   const uint32_t bar0 = s_u32(smem) + L.bars, ebar0 = bar0 + 8 * STG, a_full = ebar0 + 8 * STG, ad_full = a_full + 8,
@@ -760,45 +771,53 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
       constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0), idesc_x = make_idesc_bf16(128, TB, 0, 1),
                          idesc_u = make_idesc_bf16(128, HP, 1, 0);
       int st = 0; uint32_t ph = 0, u = 0;
+      TPROBE_DECL;
       for (int pi = 0; pi < npat; pi++) {
         int kst = 0;
         for (int i = 0; i < nch; i++) {
-          mbar_wait(bar0 + 8 * st, ph);
+          TPROBE(0, mbar_wait(bar0 + 8 * st, ph));
           tc_fence_after();
+          TPROBE(4, {
 #pragma unroll
           for (int j = 0; j < 2; j++)
 #pragma unroll
             for (int ks = 0; ks < TB / 16; ks++)
               mma_f16_ss(tA, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
                          make_smem_desc(sB + (st * 2 + j) * BT5 + ks * 32, 16, 1024), idesc1, (i | j | ks) != 0);
+          });
           if (i == nch - R) kst = st;
           if (i < nch - R) mma_commit(ebar0 + 8 * st);
           if (++st == STG) { st = 0; ph ^= 1; }
         }
         mma_commit(a_full);
-        mbar_wait(ad_full, pi & 1);
+        TPROBE(1, mbar_wait(ad_full, pi & 1));
         for (int i = 0; i < nch; i++) {
           int slot;
           if (i < R) { slot = kst; if (++kst == STG) kst = 0; }
-          else { slot = st; mbar_wait(bar0 + 8 * st, ph); if (++st == STG) { st = 0; ph ^= 1; } }
+          else { slot = st; TPROBE(2, mbar_wait(bar0 + 8 * st, ph)); if (++st == STG) { st = 0; ph ^= 1; } }
           const int c = i < R ? nch - R + i : nch - 1 - i;
           tc_fence_after();
 #pragma unroll
           for (int j = 0; j < 2; j++, u++) {
             const uint32_t xb = u & 1;
-            mbar_wait(x_empty0 + 8 * xb, ((u >> 1) & 1) ^ 1);
+            TPROBE(3, mbar_wait(x_empty0 + 8 * xb, ((u >> 1) & 1) ^ 1));
             tc_fence_after();
+            TPROBE(5, {
 #pragma unroll
             for (int ks = 0; ks < 2; ks++)                 // k = (alpha | ds): rows 0-15 dXbar, 16-31 Ut of the B tile
               mma_f16_ts(tdX + xb * TB, tAD + ks * 8, make_smem_desc(sB + (slot * 2 + j) * BT5 + ks * 2048, 16, 1024), idesc_x, ks != 0);
+            });
             mma_commit(x_full0 + 8 * xb);
           }
+          TPROBE(6, {
           for (int ks = 0; ks < mtiles; ks++)
             mma_f16_ss(tdU + c * HP, make_smem_desc(sX + (slot * 2) * XTb + ks * 2048, XTb, 1024),
                        make_smem_desc(sDT + (ks >> 2) * UT + (ks & 3) * 32, 16, 1024), idesc_u, (pi | ks) != 0);
+          });
           mma_commit(ebar0 + 8 * slot);
         }
       }
+      TPROBE_PRINT7;
       mma_commit(u_done);
     }
   } else {
@@ -862,18 +881,30 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(x_empty0 + 8 * xb);
-          if (r < V) {
-            uint4* dst = reinterpret_cast<uint4*>(dtok + ((size_t)bl * V + r) * D + (c * 2 + j) * TB + sub * 16);
+          // the quarter's four warps fill a [32 rows x 64 columns] staging tile (this warp: 16 columns = two 16-byte chunks
+          // of every row), which leaves as ONE TMA box store over dtok seen as [BL][V][D]: rows >= V are clipped by the map.
+          // (Row-per-thread 32-byte stores to rows 4 KB apart made this drain the critical path: 10.8k of 48k cycles per patch.)
+          if (quarter * 32 < V) {
+            const uint32_t so = sO + (quarter * 2 + xb) * OT5;
+            if (sub == 0 && lane == 0) bulk_wait_read<1>();          // the store issued two sub-tiles ago has left this buffer
+            quarter_sync(quarter);
 #pragma unroll
-            for (int q = 0; q < 2; q++)
-              __stcs(dst + q, make_uint4(pack_bf16(__uint_as_float(ov[q * 8]), __uint_as_float(ov[q * 8 + 1])),
-                                         pack_bf16(__uint_as_float(ov[q * 8 + 2]), __uint_as_float(ov[q * 8 + 3])),
-                                         pack_bf16(__uint_as_float(ov[q * 8 + 4]), __uint_as_float(ov[q * 8 + 5])),
-                                         pack_bf16(__uint_as_float(ov[q * 8 + 6]), __uint_as_float(ov[q * 8 + 7]))));
+            for (int q = 0; q < 2; q++) {
+              const uint32_t addr = so + lane * 128 + (((sub * 2 + q) ^ (lane & 7)) << 4);
+              asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr),
+                           "r"(pack_bf16(__uint_as_float(ov[q * 8]), __uint_as_float(ov[q * 8 + 1]))),
+                           "r"(pack_bf16(__uint_as_float(ov[q * 8 + 2]), __uint_as_float(ov[q * 8 + 3]))),
+                           "r"(pack_bf16(__uint_as_float(ov[q * 8 + 4]), __uint_as_float(ov[q * 8 + 5]))),
+                           "r"(pack_bf16(__uint_as_float(ov[q * 8 + 6]), __uint_as_float(ov[q * 8 + 7]))) : "memory");
+            }
+            fence_proxy_async();
+            quarter_sync(quarter);
+            if (sub == 0 && lane == 0) { tma_store_3d(&tmD, so, (c * 2 + j) * TB, quarter * 32, bl); bulk_commit(); }
           }
         }
       }
     }
+    if (sub == 0 && lane == 0) bulk_wait_all();              // the staging tiles outlive the last stores
     // ---- dUt^T accumulated over all patches of this CTA: thread = column d of a 128-column step, this warp's 4 heads
     if (npat > 0) {
       mbar_wait(u_done, 0);
@@ -934,6 +965,22 @@ int make_map(CUtensorMap* tm, const void* base, long long rows, int D, int box_r
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { set_error("aggregate: cuTensorMapEncodeTiled failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
+  return ORBIT_OK;
+}
+// dtok seen as [BL][V][D] bf16 -> boxes of [1][32 rows][64 columns], 128-byte swizzle: a store clips the rows >= V of a patch
+int make_map_rows3(CUtensorMap* tm, const void* base, long long BL, int V, int D) {
+  void* p = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+      qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
+  cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)V, (cuuint64_t)BL};
+  cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)V * D * 2};
+  cuuint32_t box[3] = {(cuuint32_t)TB, 32, 1};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = ((EncodeTiledFn)p)(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("aggregate: cuTensorMapEncodeTiled (dtok) failed (%d)", (int)r); return ORBIT_ERR_CUDA; }
   return ORBIT_OK;
 }
 }  // namespace
@@ -999,7 +1046,9 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
     if (keep > stg - 1) keep = stg - 1;
     if (keep > nch) keep = nch;
     const int grid5 = BL < num_sms() ? BL : num_sms();
-    agg_bwd_t5_kernel<<<grid5, NT5, smb, s>>>(tmX, tmG, tmU, alpha, (bf16*)dtok, dUt_acc, BL, V, D, heads, stg, keep);
+    CUtensorMap tmD;
+    ORBIT_TRY(make_map_rows3(&tmD, dtok, BL, V, D));
+    agg_bwd_t5_kernel<<<grid5, NT5, smb, s>>>(tmX, tmG, tmU, tmD, alpha, dUt_acc, BL, V, D, heads, stg, keep);
     ORBIT_LAUNCH_CHECK();
     return ORBIT_OK;
   }

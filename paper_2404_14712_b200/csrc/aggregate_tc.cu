@@ -479,8 +479,11 @@ __global__ void __launch_bounds__(NTB + 32) agg_bwd_tma_kernel(const __grid_cons
 // shared memory as before (16 warps, one head each), write alpha^T as a 128B-swizzled K-major operand tile, and the first
 // quarter's four warps drain the pass-2 accumulators: thread = head row, 32 columns each = 64 contiguous bytes of Xbar.
 constexpr int AT5 = 128 * TB * 2;             // one 64-v block of the alpha^T operand tile: 128 rows x 128 bytes
-constexpr int NW5 = 16;                      // worker warps: TMEM lane quarter (warp & 3) x 4 heads of the 16 ((warp - 2) >> 2)
-constexpr int NT5 = 64 + NW5 * 32;           // warp 0 TMA producer, warp 1 MMA issuer, warps 2..17 workers
+#ifndef NACC5
+#define NACC5 2                              // pass-1 accumulators: one per sub-tile of a step (probe: -DNACC5=1)
+#endif
+constexpr int NW5 = 16;                      // worker warps: TMEM lane quarter (warp & 3) x 4 heads of the 16 ((warp - 3) >> 2)
+constexpr int NT5 = 96 + NW5 * 32;           // warp 0 TMA producer, warps 1 / 2 MMA issuers (pass 1 / pass 2), warps 3..18 workers
 __device__ __forceinline__ void worker_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 struct T5Layout { int sX, sU, sAT, sS, bars, total; };
 __host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int stg) {
@@ -490,7 +493,7 @@ __host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int stg) {
   L.sAT = L.sU + stg * 2 * UT;                 // multiple of 1024: Vp * 128 is a multiple of 2048
   L.sS = L.sAT + 2 * AT5;                      // (the 128-row A operand of pass 1 reads past the Vp rows of a sub-tile: into the next one / sU)
   L.bars = L.sS + VP_MAX * SROW * 4;
-  L.total = L.bars + 8 * (2 * stg + 6) + 16;
+  L.total = L.bars + 8 * (3 * stg + 9) + 16;
   return L;
 }
 #ifdef ORBIT_PROBE_AGG_P1ONLY   // A/B build only: pass 1 alone (no second read of X, no Xbar): wrong results
@@ -522,18 +525,24 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
   const T5Layout L = t5_fwd_layout(Vp, STG);
   const uint32_t sX = s_u32(smem) + L.sX, sU = s_u32(smem) + L.sU, sAT = s_u32(smem) + L.sAT;
   float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [128][SROW]
-  const uint32_t bar0 = s_u32(smem) + L.bars, ebar0 = bar0 + 8 * STG, s_full = ebar0 + 8 * STG, at_full = s_full + 8,
-                 o_full0 = at_full + 8, o_empty0 = o_full0 + 16, tslot = o_empty0 + 16;
+  // full barriers: bar0[] for the pass-1 loads, bar2[] for the second read -- each issuer waits only on its own set and so
+  // follows every phase of it (a parity wait on a barrier whose phases somebody else consumes aliases two phases later)
+  const uint32_t bar0 = s_u32(smem) + L.bars, bar2 = bar0 + 8 * STG, ebar0 = bar2 + 8 * STG, s_full0 = ebar0 + 8 * STG, s_free0 = s_full0 + 16,
+                 at_full = s_free0 + 16, o_full0 = at_full + 8, o_empty0 = o_full0 + 16, tslot = o_empty0 + 16;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nch = D / (2 * TB), mtiles = Vp / 16;
   const int nre = (AGG_PROBE_PASSES - 1) * (nch - R);        // chunks read a second time
+  const int per = nch + nre;                                  // ring steps per patch
   const int np2 = (AGG_PROBE_PASSES - 1) * nch;              // pass-2 steps
 
   for (int j = 0; j < STG * 2; j++) zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);
   if (threadIdx.x == 0) {
-    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(ebar0 + 8 * i, 1); }
-    mbar_init(s_full, 1); mbar_init(at_full, 1);
-    for (int i = 0; i < 2; i++) { mbar_init(o_full0 + 8 * i, 1); mbar_init(o_empty0 + 8 * i, 4); }
+    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(bar2 + 8 * i, 1); mbar_init(ebar0 + 8 * i, 1); }
+    mbar_init(at_full, 1);
+    for (int i = 0; i < 2; i++) {
+      mbar_init(s_full0 + 8 * i, 1); mbar_init(s_free0 + 8 * i, NW5);
+      mbar_init(o_full0 + 8 * i, 1); mbar_init(o_empty0 + 8 * i, 4);
+    }
     fence_barrier_init();
   }
   if (warp == 1) { tmem_alloc(tslot, 512); tmem_relinquish(); }
@@ -544,7 +553,7 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
   tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
-  const uint32_t tS = tmem, tO = tmem + 128;
+  const uint32_t tS0 = tmem, tO = tmem + 128;            // S of patch parity pb at tS0 + 32 pb (+ 16: the second accumulator)
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   if (warp == 0) {
@@ -554,7 +563,7 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
         const int row0 = (blockIdx.x + pi * gridDim.x) * V;
         for (int i = 0; i < nch + nre; i++) {            // pass 1 (X and Ut chunks), then the second read of chunks nch-R-1 .. 0
           const int c = i < nch ? i : 2 * nch - R - 1 - i;
-          const uint32_t bar = bar0 + 8 * st;
+          const uint32_t bar = (i < nch ? bar0 : bar2) + 8 * st;
           mbar_wait(ebar0 + 8 * st, ph ^ 1);
           mbar_expect_tx(bar, 2 * (V * TB * 2 + (i < nch ? UT : 0)));
 #pragma unroll
@@ -567,62 +576,70 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
       }
     }
   } else if (warp == 1) {
+    // pass-1 issuer: runs up to one patch ahead of the softmax (S is double buffered by patch parity)
     if (lane == 0) {
-      constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0), idesc2 = make_idesc_bf16(128, 2 * TB, 0, 1);
-      int st = 0; uint32_t ph = 0, u = 0;
-      TPROBE_DECL;
+      constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0);
+      uint32_t par = 0;                               // bit s: parity of the next phase of bar0[s] this thread waits for
       for (int pi = 0; pi < npat; pi++) {
-        int kst = 0;                                     // ring slot of the first kept step
+        const uint32_t pb = pi & 1, tS = tS0 + pb * 32;
+        mbar_wait(s_free0 + 8 * pb, ((pi >> 1) & 1) ^ 1);
         for (int i = 0; i < nch; i++) {
-          TPROBE(0, mbar_wait(bar0 + 8 * st, ph));
+          const int n = pi * per + i, st = n % STG;
+          mbar_wait(bar0 + 8 * st, (par >> st) & 1);
+          par ^= 1u << st;
           tc_fence_after();
-          TPROBE(4, {
 #pragma unroll
           for (int j = 0; j < 2; j++)
 #pragma unroll
             for (int ks = 0; ks < TB / 16; ks++)
-              mma_f16_ss(tS, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
-                         make_smem_desc(sU + (st * 2 + j) * UT + ks * 32, 16, 1024), idesc1, (i | j | ks) != 0);
-          });
-          if (i == nch - R) kst = st;
+              mma_f16_ss(NACC5 == 2 && j ? tS + 16 : tS, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
+                         make_smem_desc(sU + (st * 2 + j) * UT + ks * 32, 16, 1024), idesc1, (NACC5 == 2 ? (i | ks) : (i | j | ks)) != 0);
           if (i < nch - R || AGG_PROBE_PASSES == 1) mma_commit(ebar0 + 8 * st);
-          if (++st == STG) { st = 0; ph ^= 1; }
         }
-        mma_commit(s_full);
-        TPROBE(1, mbar_wait(at_full, pi & 1));
+        mma_commit(s_full0 + 8 * pb);
+      }
+    }
+  } else if (warp == 2) {
+    // pass-2 issuer: a second issuing thread, so that pass 2 of a patch overlaps pass 1 of the next one and the tensor pipe
+    // is fed by two instruction streams (one thread kept it ~50 % active: ~60-95 cycles per dispatch)
+    if (lane == 0) {
+      constexpr uint32_t idesc2 = make_idesc_bf16(128, 2 * TB, 0, 1);
+      uint32_t u = 0, par = 0;
+      for (int pi = 0; pi < npat; pi++) {
+        mbar_wait(at_full, pi & 1);
         for (int i = 0; i < np2; i++, u++) {
           const uint32_t ob = u & 1;
-          int slot;
-          if (i < R) { slot = kst; if (++kst == STG) kst = 0; }          // kept steps: already in shared memory
-          else { slot = st; TPROBE(2, mbar_wait(bar0 + 8 * st, ph)); if (++st == STG) { st = 0; ph ^= 1; } }
-          TPROBE(3, mbar_wait(o_empty0 + 8 * ob, ((u >> 1) & 1) ^ 1));
+          const int n = pi * per + (i < R ? nch - R + i : nch + i - R), slot = n % STG;   // kept steps first, then the re-read ones
+          if (i >= R) { mbar_wait(bar2 + 8 * slot, (par >> slot) & 1); par ^= 1u << slot; }   // (kept steps: pass 1 has used them)
+          mbar_wait(o_empty0 + 8 * ob, ((u >> 1) & 1) ^ 1);
           tc_fence_after();
-          TPROBE(5, {
           for (int ks = 0; ks < mtiles; ks++)
             mma_f16_ss(tO + ob * (2 * TB), make_smem_desc(sAT + (ks >> 2) * AT5 + (ks & 3) * 32, 16, 1024),
                        make_smem_desc(sX + (slot * 2) * XTb + ks * 2048, XTb, 1024), idesc2, ks != 0);
-          });
           mma_commit(ebar0 + 8 * slot);
           mma_commit(o_full0 + 8 * ob);
         }
       }
-      TPROBE_PRINT;
     }
   } else {
-    const int w = warp - 2, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
+    const int w = warp - 3, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     uint8_t* at = smem + L.sAT;
     uint32_t u = 0;
     for (int pi = 0; pi < npat; pi++) {
       const int bl = blockIdx.x + pi * gridDim.x;
-      mbar_wait(s_full, pi & 1);
+      const uint32_t pb = pi & 1, tS = tS0 + pb * 32;
+      mbar_wait(s_full0 + 8 * pb, (pi >> 1) & 1);
       tc_fence_after();
-      uint32_t sv[4];
+      uint32_t sv[4], sv2[4] = {0u, 0u, 0u, 0u};
       tmem_ld_32x4(tS + sub * 4 + lane_off, sv);
+      if (NACC5 == 2) tmem_ld_32x4(tS + 16 + sub * 4 + lane_off, sv2);
       tmem_ld_wait();
 #pragma unroll
-      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]);
+      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]) + (NACC5 == 2 ? __uint_as_float(sv2[a]) : 0.f);
       tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(s_free0 + 8 * pb);
       worker_sync();
       // ---- softmax over v per head (one warp each); alpha -> global (fp32), alpha^T -> the K-major operand tile (two blocks
       // of 64 v, 128B swizzle)
@@ -743,6 +760,7 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
   const uint32_t tA = tmem, tAD = tmem + 16, tdX = tmem + 32, tdU = tmem + 32 + 2 * TB;
+  const uint32_t tA2 = tmem + 480;                   // second dalpha accumulator (see NACC5)
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   if (warp == 0) {
@@ -782,8 +800,8 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
           for (int j = 0; j < 2; j++)
 #pragma unroll
             for (int ks = 0; ks < TB / 16; ks++)
-              mma_f16_ss(tA, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
-                         make_smem_desc(sB + (st * 2 + j) * BT5 + ks * 32, 16, 1024), idesc1, (i | j | ks) != 0);
+              mma_f16_ss(NACC5 == 2 && j ? tA2 : tA, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
+                         make_smem_desc(sB + (st * 2 + j) * BT5 + ks * 32, 16, 1024), idesc1, (NACC5 == 2 ? (i | ks) : (i | j | ks)) != 0);
           });
           if (i == nch - R) kst = st;
           if (i < nch - R) mma_commit(ebar0 + 8 * st);
@@ -820,25 +838,26 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
       TPROBE_PRINT7;
       mma_commit(u_done);
     }
-  } else {
-    const int w = warp - 2, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
+  } else if (warp >= 3) {
+    const int w = warp - 3, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     uint8_t* dt = smem + L.sDT;
     uint32_t u = 0;
     for (int pi = 0; pi < npat; pi++) {
       const int bl = blockIdx.x + pi * gridDim.x;
       // alpha of this patch (dead since the previous patch's (alpha | ds) went to tensor memory)
-      for (int i = threadIdx.x - 64; i < 128 * HP; i += NW5 * 32) {
+      for (int i = threadIdx.x - 96; i < 128 * HP; i += NW5 * 32) {
         const int a = i >> 7, v = i & 127;
         sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
       }
       mbar_wait(a_full, pi & 1);
       tc_fence_after();
-      uint32_t sv[4];
+      uint32_t sv[4], sv2[4] = {0u, 0u, 0u, 0u};
       tmem_ld_32x4(tA + sub * 4 + lane_off, sv);
+      if (NACC5 == 2) tmem_ld_32x4(tA2 + sub * 4 + lane_off, sv2);
       tmem_ld_wait();
 #pragma unroll
-      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]);
+      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]) + (NACC5 == 2 ? __uint_as_float(sv2[a]) : 0.f);
       tc_fence_before();
       worker_sync();
       // ---- ds[v, a] = alpha (dalpha - sum_w alpha_w dalpha_w), one head per warp; ds^T -> the K-major B tile of the dUt product

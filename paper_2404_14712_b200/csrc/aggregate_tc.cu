@@ -482,18 +482,19 @@ constexpr int AT5 = 128 * TB * 2;             // one 64-v block of the alpha^T o
 #ifndef NACC5
 #define NACC5 2                              // pass-1 accumulators: one per sub-tile of a step (probe: -DNACC5=1)
 #endif
-constexpr int NW5 = 16;                      // worker warps: TMEM lane quarter (warp & 3) x 4 heads of the 16 ((warp - 3) >> 2)
-constexpr int NT5 = 96 + NW5 * 32;           // warp 0 TMA producer, warps 1 / 2 MMA issuers (pass 1 / pass 2), warps 3..18 workers
+constexpr int NW5 = 16;                      // worker warps: TMEM lane quarter (warp & 3) x 4 heads of the 16 ((warp - 4) >> 2)
+constexpr int NT5 = 128 + NW5 * 32;          // warps 0 / 3 TMA producers, warps 1 / 2 MMA issuers (pass 1 / pass 2), warps 4..19 workers
 __device__ __forceinline__ void worker_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
-struct T5Layout { int sX, sU, sAT, sS, bars, total; };
-__host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int stg) {
+struct T5Layout { int sX, sXB, sU, sAT, sS, bars, total; };
+__host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int sta, int stb) {
   T5Layout L;
-  L.sX = 0;
-  L.sU = stg * 2 * Vp * TB * 2;
-  L.sAT = L.sU + stg * 2 * UT;                 // multiple of 1024: Vp * 128 is a multiple of 2048
+  L.sX = 0;                                    // ring A: X sub-tile pairs of pass 1
+  L.sXB = sta * 2 * Vp * TB * 2;               // ring B: X sub-tile pairs of pass 2
+  L.sU = L.sXB + stb * 2 * Vp * TB * 2;        // ring A: Ut sub-tile pairs
+  L.sAT = L.sU + sta * 2 * UT;                 // multiple of 1024: Vp * 128 is a multiple of 2048
   L.sS = L.sAT + 2 * AT5;                      // (the 128-row A operand of pass 1 reads past the Vp rows of a sub-tile: into the next one / sU)
   L.bars = L.sS + VP_MAX * SROW * 4;
-  L.total = L.bars + 8 * (3 * stg + 9) + 16;
+  L.total = L.bars + 8 * (2 * sta + 2 * stb + 9) + 16;
   return L;
 }
 #ifdef ORBIT_PROBE_AGG_P1ONLY   // A/B build only: pass 1 alone (no second read of X, no Xbar): wrong results
@@ -501,43 +502,30 @@ __host__ __device__ inline T5Layout t5_fwd_layout(int Vp, int stg) {
 #else
 #define AGG_PROBE_PASSES 2
 #endif
-// SM-inbound traffic is what bounds this kernel (pass 1 alone streams X from DRAM at 5.2 TB/s; the second read, from L2, adds
-// its bytes to the same ~6.5 TB/s L2 -> SM budget instead of overlapping), so the last R steps of pass 1 are KEPT in the ring
-// and pass 2 starts with them: R / nch of the second read never happens.  The ring stays FIFO: pass 1 releases steps
-// 0 .. nch-R-1, pass 2 releases the kept ones in ring order, then the re-loaded chunks nch-R-1 .. 0.
-#ifdef ORBIT_PROBE_AGG          // A/B build only: cycles the MMA-issuing thread of CTA 0 spends in its waits, per patch
-#define TPROBE_DECL long long tp_[7] = {0, 0, 0, 0, 0, 0, 0}; const long long tt0_ = clock64()
-#define TPROBE(slot, stmt) do { long long t0_ = clock64(); stmt; tp_[slot] += clock64() - t0_; } while (0)
-#define TPROBE_PRINT do { if (blockIdx.x == 0 && npat > 0) printf("agg t5 probe: patches %d  per patch: total %lld  wait pass-1 data %lld  wait alpha %lld  wait pass-2 data %lld  wait o_empty %lld  issue pass-1 %lld  issue pass-2 %lld\n", npat, (clock64() - tt0_) / npat, tp_[0] / npat, tp_[1] / npat, tp_[2] / npat, tp_[3] / npat, tp_[4] / npat, tp_[5] / npat); } while (0)
-#define TPROBE_PRINT7 do { if (blockIdx.x == 0 && npat > 0) printf("agg bwd t5 probe: patches %d  per patch: total %lld  wait pass-1 data %lld  wait (alpha|ds) %lld  wait pass-2 data %lld  wait x_empty %lld  issue pass-1 %lld  issue dX %lld  issue dUt %lld\n", npat, (clock64() - tt0_) / npat, tp_[0] / npat, tp_[1] / npat, tp_[2] / npat, tp_[3] / npat, tp_[4] / npat, tp_[5] / npat, tp_[6] / npat); } while (0)
-#else
-#define TPROBE_PRINT7
-#define TPROBE_DECL
-#define TPROBE(slot, stmt) stmt
-#define TPROBE_PRINT
-#endif
+// Two rings: ring A streams X (and Ut) for pass 1, ring B re-reads X for pass 2 (from L2: a patch's tile is requested again as
+// soon as its pass 1 has completed, last chunk first).  With ONE ring the stream was a FIFO of [pass 1 of patch p][second read of
+// p][pass 1 of p + 1]: the DRAM stream of the next patch could not start before pass 2 had drained the slots, and every patch
+// paid the softmax bubble plus a DRAM latency ramp.  Each ring has its own producer thread and its own consumer (issuing) thread.
 __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constant__ CUtensorMap tmX,
     const __grid_constant__ CUtensorMap tmU, float* __restrict__ alpha, bf16* __restrict__ Xbar, int BL, int V, int D, int h,
-    int STG, int R) {
+    int STA, int STB, int HINT) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
   const int Vp = (V + 15) & ~15, XTb = Vp * TB * 2;
-  const T5Layout L = t5_fwd_layout(Vp, STG);
-  const uint32_t sX = s_u32(smem) + L.sX, sU = s_u32(smem) + L.sU, sAT = s_u32(smem) + L.sAT;
+  const T5Layout L = t5_fwd_layout(Vp, STA, STB);
+  const uint32_t sXA = s_u32(smem) + L.sX, sXB = s_u32(smem) + L.sXB, sU = s_u32(smem) + L.sU, sAT = s_u32(smem) + L.sAT;
   float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [128][SROW]
-  // full barriers: bar0[] for the pass-1 loads, bar2[] for the second read -- each issuer waits only on its own set and so
-  // follows every phase of it (a parity wait on a barrier whose phases somebody else consumes aliases two phases later)
-  const uint32_t bar0 = s_u32(smem) + L.bars, bar2 = bar0 + 8 * STG, ebar0 = bar2 + 8 * STG, s_full0 = ebar0 + 8 * STG, s_free0 = s_full0 + 16,
-                 at_full = s_free0 + 16, o_full0 = at_full + 8, o_empty0 = o_full0 + 16, tslot = o_empty0 + 16;
+  const uint32_t fullA = s_u32(smem) + L.bars, emptyA = fullA + 8 * STA, fullB = emptyA + 8 * STA, emptyB = fullB + 8 * STB,
+                 s_full0 = emptyB + 8 * STB, s_free0 = s_full0 + 16, at_full = s_free0 + 16, o_full0 = at_full + 8,
+                 o_empty0 = o_full0 + 16, tslot = o_empty0 + 16;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nch = D / (2 * TB), mtiles = Vp / 16;
-  const int nre = (AGG_PROBE_PASSES - 1) * (nch - R);        // chunks read a second time
-  const int per = nch + nre;                                  // ring steps per patch
   const int np2 = (AGG_PROBE_PASSES - 1) * nch;              // pass-2 steps
 
-  for (int j = 0; j < STG * 2; j++) zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);
+  for (int j = 0; j < (STA + STB) * 2; j++) zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);     // ring B follows ring A
   if (threadIdx.x == 0) {
-    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(bar2 + 8 * i, 1); mbar_init(ebar0 + 8 * i, 1); }
+    for (int i = 0; i < STA; i++) { mbar_init(fullA + 8 * i, 1); mbar_init(emptyA + 8 * i, 1); }
+    for (int i = 0; i < STB; i++) { mbar_init(fullB + 8 * i, 1); mbar_init(emptyB + 8 * i, 1); }
     mbar_init(at_full, 1);
     for (int i = 0; i < 2; i++) {
       mbar_init(s_full0 + 8 * i, 1); mbar_init(s_free0 + 8 * i, NW5);
@@ -557,21 +545,38 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   if (warp == 0) {
-    if (lane == 0) {
+    if (lane == 0) {                                      // producer A: X and Ut chunks of pass 1, patch after patch
       int st = 0; uint32_t ph = 0;
+      const uint64_t pol = l2_policy(HINT & 1 ? 2 : 0);     // the tile is read again within a patch time: keep it in L2
       for (int pi = 0; pi < npat; pi++) {
         const int row0 = (blockIdx.x + pi * gridDim.x) * V;
-        for (int i = 0; i < nch + nre; i++) {            // pass 1 (X and Ut chunks), then the second read of chunks nch-R-1 .. 0
-          const int c = i < nch ? i : 2 * nch - R - 1 - i;
-          const uint32_t bar = (i < nch ? bar0 : bar2) + 8 * st;
-          mbar_wait(ebar0 + 8 * st, ph ^ 1);
-          mbar_expect_tx(bar, 2 * (V * TB * 2 + (i < nch ? UT : 0)));
+        for (int c = 0; c < nch; c++) {
+          const uint32_t bar = fullA + 8 * st;
+          mbar_wait(emptyA + 8 * st, ph ^ 1);
+          mbar_expect_tx(bar, 2 * (V * TB * 2 + UT));
 #pragma unroll
           for (int j = 0; j < 2; j++) {
-            tma_load_2d(sX + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, row0);
-            if (i < nch) tma_load_2d(sU + (st * 2 + j) * UT, &tmU, bar, (c * 2 + j) * TB, 0);
+            tma_load_2d_hint(sXA + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, row0, pol);
+            tma_load_2d(sU + (st * 2 + j) * UT, &tmU, bar, (c * 2 + j) * TB, 0);
           }
-          if (++st == STG) { st = 0; ph ^= 1; }
+          if (++st == STA) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 3) {
+    if (lane == 0 && np2 > 0) {                           // producer B: the second read of a patch, once its pass 1 is complete
+      int st = 0; uint32_t ph = 0;
+      const uint64_t pol = l2_policy(HINT & 2 ? 1 : 0);     // ... and not after that
+      for (int pi = 0; pi < npat; pi++) {
+        const int row0 = (blockIdx.x + pi * gridDim.x) * V;
+        mbar_wait(s_full0 + 8 * (pi & 1), (pi >> 1) & 1);
+        for (int c = nch - 1; c >= 0; c--) {               // most recently read lines first
+          const uint32_t bar = fullB + 8 * st;
+          mbar_wait(emptyB + 8 * st, ph ^ 1);
+          mbar_expect_tx(bar, 2 * V * TB * 2);
+#pragma unroll
+          for (int j = 0; j < 2; j++) tma_load_2d_hint(sXB + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, row0, pol);
+          if (++st == STB) { st = 0; ph ^= 1; }
         }
       }
     }
@@ -579,50 +584,48 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
     // pass-1 issuer: runs up to one patch ahead of the softmax (S is double buffered by patch parity)
     if (lane == 0) {
       constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0);
-      uint32_t par = 0;                               // bit s: parity of the next phase of bar0[s] this thread waits for
+      int st = 0; uint32_t ph = 0;
       for (int pi = 0; pi < npat; pi++) {
         const uint32_t pb = pi & 1, tS = tS0 + pb * 32;
         mbar_wait(s_free0 + 8 * pb, ((pi >> 1) & 1) ^ 1);
         for (int i = 0; i < nch; i++) {
-          const int n = pi * per + i, st = n % STG;
-          mbar_wait(bar0 + 8 * st, (par >> st) & 1);
-          par ^= 1u << st;
+          mbar_wait(fullA + 8 * st, ph);
           tc_fence_after();
 #pragma unroll
           for (int j = 0; j < 2; j++)
 #pragma unroll
             for (int ks = 0; ks < TB / 16; ks++)
-              mma_f16_ss(NACC5 == 2 && j ? tS + 16 : tS, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
+              mma_f16_ss(NACC5 == 2 && j ? tS + 16 : tS, make_smem_desc(sXA + (st * 2 + j) * XTb + ks * 32, 16, 1024),
                          make_smem_desc(sU + (st * 2 + j) * UT + ks * 32, 16, 1024), idesc1, (NACC5 == 2 ? (i | ks) : (i | j | ks)) != 0);
-          if (i < nch - R || AGG_PROBE_PASSES == 1) mma_commit(ebar0 + 8 * st);
+          mma_commit(emptyA + 8 * st);
+          if (++st == STA) { st = 0; ph ^= 1; }
         }
         mma_commit(s_full0 + 8 * pb);
       }
     }
   } else if (warp == 2) {
-    // pass-2 issuer: a second issuing thread, so that pass 2 of a patch overlaps pass 1 of the next one and the tensor pipe
-    // is fed by two instruction streams (one thread kept it ~50 % active: ~60-95 cycles per dispatch)
+    // pass-2 issuer
     if (lane == 0) {
       constexpr uint32_t idesc2 = make_idesc_bf16(128, 2 * TB, 0, 1);
-      uint32_t u = 0, par = 0;
+      int st = 0; uint32_t ph = 0, u = 0;
       for (int pi = 0; pi < npat; pi++) {
         mbar_wait(at_full, pi & 1);
         for (int i = 0; i < np2; i++, u++) {
           const uint32_t ob = u & 1;
-          const int n = pi * per + (i < R ? nch - R + i : nch + i - R), slot = n % STG;   // kept steps first, then the re-read ones
-          if (i >= R) { mbar_wait(bar2 + 8 * slot, (par >> slot) & 1); par ^= 1u << slot; }   // (kept steps: pass 1 has used them)
+          mbar_wait(fullB + 8 * st, ph);
           mbar_wait(o_empty0 + 8 * ob, ((u >> 1) & 1) ^ 1);
           tc_fence_after();
           for (int ks = 0; ks < mtiles; ks++)
             mma_f16_ss(tO + ob * (2 * TB), make_smem_desc(sAT + (ks >> 2) * AT5 + (ks & 3) * 32, 16, 1024),
-                       make_smem_desc(sX + (slot * 2) * XTb + ks * 2048, XTb, 1024), idesc2, ks != 0);
-          mma_commit(ebar0 + 8 * slot);
+                       make_smem_desc(sXB + (st * 2) * XTb + ks * 2048, XTb, 1024), idesc2, ks != 0);
+          mma_commit(emptyB + 8 * st);
           mma_commit(o_full0 + 8 * ob);
+          if (++st == STB) { st = 0; ph ^= 1; }
         }
       }
     }
   } else {
-    const int w = warp - 3, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
+    const int w = warp - 4, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     uint8_t* at = smem + L.sAT;
     uint32_t u = 0;
@@ -662,10 +665,10 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
       fence_proxy_async();
       worker_sync();
       if (w == 0 && lane == 0) mbar_arrive(at_full);
-      // ---- pass 2: drain Xbar^T[d, a] of each 128-column chunk: the kept chunks nch-R .. nch-1, then nch-R-1 .. 0
+      // ---- pass 2: drain Xbar[a, d] of each 128-column chunk (chunks come last to first)
       for (int i = 0; i < np2; i++, u++) {
         const uint32_t ob = u & 1;
-        const int c = i < R ? nch - R + i : nch - 1 - i;
+        const int c = nch - 1 - i;
         if (quarter != 0) continue;                            // the 16 head rows sit in TMEM lanes 0..15: the first quarter's warps
         mbar_wait(o_full0 + 8 * ob, (u >> 1) & 1);
         tc_fence_after();
@@ -692,6 +695,15 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
   if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
 }
 
+#ifdef ORBIT_PROBE_AGG          // A/B build only: cycles the MMA-issuing thread of CTA 0 spends in its waits / issuing, per patch
+#define TPROBE_DECL long long tp_[7] = {0, 0, 0, 0, 0, 0, 0}; const long long tt0_ = clock64()
+#define TPROBE(slot, stmt) do { long long t0_ = clock64(); stmt; tp_[slot] += clock64() - t0_; } while (0)
+#define TPROBE_PRINT7 do { if (blockIdx.x == 0 && npat > 0) printf("agg bwd t5 probe: patches %d  per patch: total %lld  wait pass-1 data %lld  wait (alpha|ds) %lld  wait pass-2 data %lld  wait x_empty %lld  issue pass-1 %lld  issue dX %lld  issue dUt %lld\n", npat, (clock64() - tt0_) / npat, tp_[0] / npat, tp_[1] / npat, tp_[2] / npat, tp_[3] / npat, tp_[4] / npat, tp_[5] / npat, tp_[6] / npat); } while (0)
+#else
+#define TPROBE_PRINT7
+#define TPROBE_DECL
+#define TPROBE(slot, stmt) stmt
+#endif
 // ============================================ backward on tcgen05 ============================================
 // Same structure as the forward: the TMA ring feeds one MMA-issuing thread, 16 worker warps own the TMEM lanes.
 //   pass 1: dalpha[v, a] (TMEM, 16 columns) = sum over chunks of X[128 x 64] (A, K-major) . dXbar[16 x 64]^T (B, K-major)
@@ -838,15 +850,15 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
       TPROBE_PRINT7;
       mma_commit(u_done);
     }
-  } else if (warp >= 3) {
-    const int w = warp - 3, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
+  } else if (warp >= 4) {
+    const int w = warp - 4, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     uint8_t* dt = smem + L.sDT;
     uint32_t u = 0;
     for (int pi = 0; pi < npat; pi++) {
       const int bl = blockIdx.x + pi * gridDim.x;
       // alpha of this patch (dead since the previous patch's (alpha | ds) went to tensor memory)
-      for (int i = threadIdx.x - 96; i < 128 * HP; i += NW5 * 32) {
+      for (int i = threadIdx.x - 128; i < 128 * HP; i += NW5 * 32) {
         const int a = i >> 7, v = i & 127;
         sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
       }
@@ -1024,17 +1036,17 @@ int agg_patch_fwd_tc(const void* tok, const float* Ut, void* Utb, float* alpha, 
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
   if (t5_enabled()) {
     const int Vp = (V + 15) & ~15;
-    int stg = 12;
-    while (stg > 2 && 1024 + (size_t)t5_fwd_layout(Vp, stg).total > SMEM_MAX) stg--;
-    const size_t smb = 1024 + (size_t)t5_fwd_layout(Vp, stg).total;
+    // ring A (DRAM stream) gets the stages that ring B (L2 re-read, shorter latency) does not need
+    static const int stb_env = [] { const char* e = getenv("ORBIT_AGG_STB"); return e ? atoi(e) : 0; }();
+    static const int sta_env = [] { const char* e = getenv("ORBIT_AGG_STA"); return e ? atoi(e) : 0; }();
+    static const int hint_env = [] { const char* e = getenv("ORBIT_AGG_HINT"); return e ? atoi(e) : 2; }();
+    int stb = stb_env > 0 ? stb_env : 4, sta = sta_env > 0 ? sta_env : 12;
+    while (sta > 1 && 1024 + (size_t)t5_fwd_layout(Vp, sta, stb).total > SMEM_MAX) sta--;
+    while (stb > 1 && 1024 + (size_t)t5_fwd_layout(Vp, sta, stb).total > SMEM_MAX) stb--;
+    const size_t smb = 1024 + (size_t)t5_fwd_layout(Vp, sta, stb).total;
     ORBIT_SMEM_ATTR(agg_fwd_t5_kernel, SMEM_MAX);
     const int grid = BL < num_sms() ? BL : num_sms();
-    static const int keep_env = [] { const char* e = getenv("ORBIT_AGG_KEEP"); return e ? atoi(e) : -1; }();
-    const int nch = D / (2 * TB);
-    int keep = keep_env >= 0 ? keep_env : stg - 2;     // kept steps of pass 1; the other slots prefetch during the softmax
-    if (keep > stg - 1) keep = stg - 1;
-    if (keep > nch) keep = nch;
-    agg_fwd_t5_kernel<<<grid, NT5, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads, stg, keep);
+    agg_fwd_t5_kernel<<<grid, NT5, smb, s>>>(tmX, tmU, alpha, (bf16*)Xbar, BL, V, D, heads, sta, stb, hint_env);
     ORBIT_LAUNCH_CHECK();
     return ORBIT_OK;
   }

@@ -714,54 +714,65 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
 //           per 128-column step:     dUt^T[d, a] (TMEM, 16 columns per step, kept for ALL patches of the CTA)
 //                                      += X^T[128 d x V] (A, MN-major: the X tiles as they are) . ds^T[16 x V]^T (B, K-major)
 //   workers drain dX (thread = token row, 16 columns = 32 bytes each) and, after the last patch, dUt^T (fp32 atomics).
-// The last R steps of pass 1 stay in the ring for pass 2 (as in the forward); their Ut chunks come with them.
 constexpr int BT5 = 2 * UT;                  // B tile of a 64-column sub-tile: rows 0-15 dXbar, rows 16-31 Ut
 constexpr int OT5 = 32 * TB * 2;             // dX staging tile of one TMEM lane quarter: 32 token rows x 64 columns, 128B swizzle
 __device__ __forceinline__ void quarter_sync(int q) { asm volatile("bar.sync %0, 128;" ::"r"(2 + q) : "memory"); }
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(m), "r"(src), "r"(c0), "r"(c1), "r"(c2) : "memory");
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, uint32_t src, int c0, int c1, int c2, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;" ::"l"(m), "r"(src), "r"(c0),
+               "r"(c1), "r"(c2), "l"(policy) : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-struct T5BLayout { int sX, sB, sDT, sO, sS, sAl, bars, total; };
-__host__ __device__ inline T5BLayout t5_bwd_layout(int Vp, int stg) {
+struct T5BLayout { int sX, sXB, sBA, sBB, sDT, sO, sS, sAl, bars, total; };
+__host__ __device__ inline T5BLayout t5_bwd_layout(int V, int sta, int stb) {
+  const int Vp = (V + 15) & ~15, nq = (V + 31) / 32;
   T5BLayout L;
-  L.sX = 0;
-  L.sB = stg * 2 * Vp * TB * 2;
-  L.sDT = L.sB + stg * 2 * BT5;
-  L.sO = L.sDT + 2 * UT;
-  L.sS = L.sO + 8 * OT5;
-  L.sAl = L.sS + VP_MAX * SROW * 4;
-  L.bars = L.sAl + VP_MAX * SROW * 4;
-  L.total = L.bars + 8 * (2 * stg + 8) + 16;
+  L.sX = 0;                                    // ring A: X sub-tile pairs of pass 1
+  L.sXB = sta * 2 * Vp * TB * 2;               // ring B: X sub-tile pairs of pass 2
+  L.sBA = L.sXB + stb * 2 * Vp * TB * 2;       // ring A: dXbar sub-tile pairs [16 x 64]
+  L.sBB = L.sBA + sta * 2 * UT;                // ring B: [dXbar ; Ut] sub-tile pairs [32 x 64]
+  L.sDT = L.sBB + stb * 2 * BT5;
+  L.sO = L.sDT + 2 * UT;                       // dX staging: two tiles per live TMEM lane quarter
+  L.sS = L.sO + nq * 2 * OT5;
+  L.sAl = L.sS + Vp * SROW * 4;
+  L.bars = L.sAl + Vp * SROW * 4;
+  L.total = L.bars + 8 * (2 * sta + 2 * stb + 12) + 16;
   return L;
 }
 
+// Two rings and two issuing threads, as in the forward: ring A streams X and dXbar for pass 1 (issuer A: dalpha, double buffered
+// by patch parity so that it runs one patch ahead), ring B re-reads X with [dXbar ; Ut] for pass 2 once pass 1 of the patch is
+// complete (issuer B: per 128-column step the dUt^T product first, then the two dX sub-tiles, so that the last dX commit of a
+// patch covers all of its products and the workers may overwrite (alpha | ds) / ds^T for the next patch once they have drained it).
 __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constant__ CUtensorMap tmX,
     const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmD,
-    const float* __restrict__ alpha, float* __restrict__ dUt_acc, int BL, int V, int D, int h, int STG, int R) {
+    const float* __restrict__ alpha, float* __restrict__ dUt_acc, int BL, int V, int D, int h, int STA, int STB, int HINT) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
   const int Vp = (V + 15) & ~15, XTb = Vp * TB * 2;
-  const T5BLayout L = t5_bwd_layout(Vp, STG);
-  const uint32_t sX = s_u32(smem) + L.sX, sB = s_u32(smem) + L.sB, sDT = s_u32(smem) + L.sDT, sO = s_u32(smem) + L.sO;
-  float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [128][SROW] dalpha, then ds
-  float* sAl = reinterpret_cast<float*>(smem + L.sAl);                        // [128][SROW] alpha
-  const uint32_t bar0 = s_u32(smem) + L.bars, ebar0 = bar0 + 8 * STG, a_full = ebar0 + 8 * STG, ad_full = a_full + 8,
-                 x_full0 = ad_full + 8, x_empty0 = x_full0 + 16, u_done = x_empty0 + 16, tslot = u_done + 8;
+  const T5BLayout L = t5_bwd_layout(V, STA, STB);
+  const uint32_t sXA = s_u32(smem) + L.sX, sXB = s_u32(smem) + L.sXB, sBA = s_u32(smem) + L.sBA, sBB = s_u32(smem) + L.sBB,
+                 sDT = s_u32(smem) + L.sDT, sO = s_u32(smem) + L.sO;
+  float* sS = reinterpret_cast<float*>(smem + L.sS);                          // [Vp][SROW] dalpha, then ds
+  float* sAl = reinterpret_cast<float*>(smem + L.sAl);                        // [Vp][SROW] alpha
+  const uint32_t fullA = s_u32(smem) + L.bars, emptyA = fullA + 8 * STA, fullB = emptyA + 8 * STA, emptyB = fullB + 8 * STB,
+                 a_full0 = emptyB + 8 * STB, a_free0 = a_full0 + 16, ad_full = a_free0 + 16, x_full0 = ad_full + 8,
+                 x_empty0 = x_full0 + 16, u_done = x_empty0 + 16, tslot = u_done + 8;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nch = D / (2 * TB), mtiles = Vp / 16;
-  const int nre = nch - R;
 
-  for (int j = 0; j < STG * 2; j++) {
-    zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);
-    zero_tail_rows(smem + L.sB + j * BT5, h, HP, NT5);                          // dXbar rows h..15 (the TMA box has h rows)
-  }
+  for (int j = 0; j < (STA + STB) * 2; j++) zero_tail_rows(smem + L.sX + j * XTb, V, Vp, NT5);
+  for (int j = 0; j < STA * 2; j++) zero_tail_rows(smem + L.sBA + j * UT, h, HP, NT5);     // dXbar rows h..15 (the TMA box has h rows)
+  for (int j = 0; j < STB * 2; j++) zero_tail_rows(smem + L.sBB + j * BT5, h, HP, NT5);
   if (threadIdx.x == 0) {
-    for (int i = 0; i < STG; i++) { mbar_init(bar0 + 8 * i, 1); mbar_init(ebar0 + 8 * i, 1); }
-    mbar_init(a_full, 1); mbar_init(ad_full, 1); mbar_init(u_done, 1);
-    for (int i = 0; i < 2; i++) { mbar_init(x_full0 + 8 * i, 1); mbar_init(x_empty0 + 8 * i, NW5); }
+    for (int i = 0; i < STA; i++) { mbar_init(fullA + 8 * i, 1); mbar_init(emptyA + 8 * i, 1); }
+    for (int i = 0; i < STB; i++) { mbar_init(fullB + 8 * i, 1); mbar_init(emptyB + 8 * i, 1); }
+    mbar_init(ad_full, 1); mbar_init(u_done, 1);
+    for (int i = 0; i < 2; i++) {
+      mbar_init(a_full0 + 8 * i, 1); mbar_init(a_free0 + 8 * i, NW5);
+      mbar_init(x_full0 + 8 * i, 1); mbar_init(x_empty0 + 8 * i, NW5);
+    }
     fence_barrier_init();
   }
   if (warp == 1) { tmem_alloc(tslot, 512); tmem_relinquish(); }
@@ -771,106 +782,127 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
   tc_fence_after();
   uint32_t tmem;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
-  const uint32_t tA = tmem, tAD = tmem + 16, tdX = tmem + 32, tdU = tmem + 32 + 2 * TB;
-  const uint32_t tA2 = tmem + 480;                   // second dalpha accumulator (see NACC5)
+  // dalpha of patch parity pb at tA0 + 32 pb (+ 16: the second accumulator), (alpha | ds), dX (2 x 64), dUt^T (16 per step)
+  const uint32_t tA0 = tmem, tAD = tmem + 64, tdX = tmem + 80, tdU = tmem + 80 + 2 * TB;
 
   const int npat = blockIdx.x < BL ? (BL - 1 - blockIdx.x) / gridDim.x + 1 : 0;
   if (warp == 0) {
-    if (lane == 0) {
+    if (lane == 0) {                                      // producer A: X and dXbar chunks of pass 1
       int st = 0; uint32_t ph = 0;
+      const uint64_t polA = l2_policy(HINT & 1 ? 2 : 0);
       for (int pi = 0; pi < npat; pi++) {
         const int bl = blockIdx.x + pi * gridDim.x;
-        for (int i = 0; i < nch + nre; i++) {            // pass 1 (X, dXbar; Ut too for the kept steps), then chunks nch-R-1 .. 0 again
-          const int c = i < nch ? i : 2 * nch - R - 1 - i;
-          const bool ut = i >= nch - R;
-          const uint32_t bar = bar0 + 8 * st;
-          mbar_wait(ebar0 + 8 * st, ph ^ 1);
-          mbar_expect_tx(bar, 2 * ((V + h) * TB * 2 + (ut ? UT : 0)));
+        for (int c = 0; c < nch; c++) {
+          const uint32_t bar = fullA + 8 * st;
+          mbar_wait(emptyA + 8 * st, ph ^ 1);
+          mbar_expect_tx(bar, 2 * (V + h) * TB * 2);
 #pragma unroll
           for (int j = 0; j < 2; j++) {
-            tma_load_2d(sX + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, bl * V);
-            tma_load_2d(sB + (st * 2 + j) * BT5, &tmG, bar, (c * 2 + j) * TB, bl * h);
-            if (ut) tma_load_2d(sB + (st * 2 + j) * BT5 + UT, &tmU, bar, (c * 2 + j) * TB, 0);
+            tma_load_2d_hint(sXA + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, bl * V, polA);
+            tma_load_2d_hint(sBA + (st * 2 + j) * UT, &tmG, bar, (c * 2 + j) * TB, bl * h, polA);
           }
-          if (++st == STG) { st = 0; ph ^= 1; }
+          if (++st == STA) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 3) {
+    if (lane == 0) {                                      // producer B: X again (from L2), dXbar and Ut, once pass 1 of the patch is done
+      int st = 0; uint32_t ph = 0;
+      const uint64_t pol = l2_policy(HINT & 2 ? 1 : 0);
+      for (int pi = 0; pi < npat; pi++) {
+        const int bl = blockIdx.x + pi * gridDim.x;
+        mbar_wait(a_full0 + 8 * (pi & 1), (pi >> 1) & 1);
+        for (int c = nch - 1; c >= 0; c--) {
+          const uint32_t bar = fullB + 8 * st;
+          mbar_wait(emptyB + 8 * st, ph ^ 1);
+          mbar_expect_tx(bar, 2 * ((V + h) * TB * 2 + UT));
+#pragma unroll
+          for (int j = 0; j < 2; j++) {
+            tma_load_2d_hint(sXB + (st * 2 + j) * XTb, &tmX, bar, (c * 2 + j) * TB, bl * V, pol);
+            tma_load_2d_hint(sBB + (st * 2 + j) * BT5, &tmG, bar, (c * 2 + j) * TB, bl * h, pol);
+            tma_load_2d(sBB + (st * 2 + j) * BT5 + UT, &tmU, bar, (c * 2 + j) * TB, 0);
+          }
+          if (++st == STB) { st = 0; ph ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0), idesc_x = make_idesc_bf16(128, TB, 0, 1),
-                         idesc_u = make_idesc_bf16(128, HP, 1, 0);
-      int st = 0; uint32_t ph = 0, u = 0;
-      TPROBE_DECL;
+    if (lane == 0) {                                      // issuer A: dalpha
+      constexpr uint32_t idesc1 = make_idesc_bf16(128, HP, 0, 0);
+      int st = 0; uint32_t ph = 0;
       for (int pi = 0; pi < npat; pi++) {
-        int kst = 0;
+        const uint32_t pb = pi & 1, tA = tA0 + pb * 32;
+        mbar_wait(a_free0 + 8 * pb, ((pi >> 1) & 1) ^ 1);
         for (int i = 0; i < nch; i++) {
-          TPROBE(0, mbar_wait(bar0 + 8 * st, ph));
+          mbar_wait(fullA + 8 * st, ph);
           tc_fence_after();
-          TPROBE(4, {
 #pragma unroll
           for (int j = 0; j < 2; j++)
 #pragma unroll
             for (int ks = 0; ks < TB / 16; ks++)
-              mma_f16_ss(NACC5 == 2 && j ? tA2 : tA, make_smem_desc(sX + (st * 2 + j) * XTb + ks * 32, 16, 1024),
-                         make_smem_desc(sB + (st * 2 + j) * BT5 + ks * 32, 16, 1024), idesc1, (NACC5 == 2 ? (i | ks) : (i | j | ks)) != 0);
-          });
-          if (i == nch - R) kst = st;
-          if (i < nch - R) mma_commit(ebar0 + 8 * st);
-          if (++st == STG) { st = 0; ph ^= 1; }
+              mma_f16_ss(NACC5 == 2 && j ? tA + 16 : tA, make_smem_desc(sXA + (st * 2 + j) * XTb + ks * 32, 16, 1024),
+                         make_smem_desc(sBA + (st * 2 + j) * UT + ks * 32, 16, 1024), idesc1, (NACC5 == 2 ? (i | ks) : (i | j | ks)) != 0);
+          mma_commit(emptyA + 8 * st);
+          if (++st == STA) { st = 0; ph ^= 1; }
         }
-        mma_commit(a_full);
-        TPROBE(1, mbar_wait(ad_full, pi & 1));
+        mma_commit(a_full0 + 8 * pb);
+      }
+    }
+  } else if (warp == 2) {
+    if (lane == 0) {                                      // issuer B: dUt^T and dX
+      constexpr uint32_t idesc_x = make_idesc_bf16(128, TB, 0, 1), idesc_u = make_idesc_bf16(128, HP, 1, 0);
+      int st = 0; uint32_t ph = 0, u = 0;
+      for (int pi = 0; pi < npat; pi++) {
+        mbar_wait(ad_full, pi & 1);
         for (int i = 0; i < nch; i++) {
-          int slot;
-          if (i < R) { slot = kst; if (++kst == STG) kst = 0; }
-          else { slot = st; TPROBE(2, mbar_wait(bar0 + 8 * st, ph)); if (++st == STG) { st = 0; ph ^= 1; } }
-          const int c = i < R ? nch - R + i : nch - 1 - i;
+          const int c = nch - 1 - i;
+          mbar_wait(fullB + 8 * st, ph);
           tc_fence_after();
+          for (int ks = 0; ks < mtiles; ks++)
+            mma_f16_ss(tdU + c * HP, make_smem_desc(sXB + (st * 2) * XTb + ks * 2048, XTb, 1024),
+                       make_smem_desc(sDT + (ks >> 2) * UT + (ks & 3) * 32, 16, 1024), idesc_u, (pi | ks) != 0);
 #pragma unroll
           for (int j = 0; j < 2; j++, u++) {
             const uint32_t xb = u & 1;
-            TPROBE(3, mbar_wait(x_empty0 + 8 * xb, ((u >> 1) & 1) ^ 1));
+            mbar_wait(x_empty0 + 8 * xb, ((u >> 1) & 1) ^ 1);
             tc_fence_after();
-            TPROBE(5, {
 #pragma unroll
             for (int ks = 0; ks < 2; ks++)                 // k = (alpha | ds): rows 0-15 dXbar, 16-31 Ut of the B tile
-              mma_f16_ts(tdX + xb * TB, tAD + ks * 8, make_smem_desc(sB + (slot * 2 + j) * BT5 + ks * 2048, 16, 1024), idesc_x, ks != 0);
-            });
+              mma_f16_ts(tdX + xb * TB, tAD + ks * 8, make_smem_desc(sBB + (st * 2 + j) * BT5 + ks * 2048, 16, 1024), idesc_x, ks != 0);
             mma_commit(x_full0 + 8 * xb);
           }
-          TPROBE(6, {
-          for (int ks = 0; ks < mtiles; ks++)
-            mma_f16_ss(tdU + c * HP, make_smem_desc(sX + (slot * 2) * XTb + ks * 2048, XTb, 1024),
-                       make_smem_desc(sDT + (ks >> 2) * UT + (ks & 3) * 32, 16, 1024), idesc_u, (pi | ks) != 0);
-          });
-          mma_commit(ebar0 + 8 * slot);
+          mma_commit(emptyB + 8 * st);
+          if (++st == STB) { st = 0; ph ^= 1; }
         }
       }
-      TPROBE_PRINT7;
       mma_commit(u_done);
     }
   } else if (warp >= 4) {
     const int w = warp - 4, quarter = warp & 3, sub = w >> 2, r = quarter * 32 + lane;
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     uint8_t* dt = smem + L.sDT;
+    const uint64_t pol_st = l2_policy(HINT & 4 ? 1 : 0);     // dX is not read again here: it should not push the X tiles out of L2
     uint32_t u = 0;
     for (int pi = 0; pi < npat; pi++) {
       const int bl = blockIdx.x + pi * gridDim.x;
       // alpha of this patch (dead since the previous patch's (alpha | ds) went to tensor memory)
       for (int i = threadIdx.x - 128; i < 128 * HP; i += NW5 * 32) {
         const int a = i >> 7, v = i & 127;
-        sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
+        if (v < Vp) sAl[v * SROW + a] = (v < V && a < h) ? alpha[((size_t)bl * h + a) * V + v] : 0.f;
       }
-      mbar_wait(a_full, pi & 1);
+      const uint32_t pb = pi & 1, tA = tA0 + pb * 32;
+      mbar_wait(a_full0 + 8 * pb, (pi >> 1) & 1);
       tc_fence_after();
       uint32_t sv[4], sv2[4] = {0u, 0u, 0u, 0u};
       tmem_ld_32x4(tA + sub * 4 + lane_off, sv);
-      if (NACC5 == 2) tmem_ld_32x4(tA2 + sub * 4 + lane_off, sv2);
+      if (NACC5 == 2) tmem_ld_32x4(tA + 16 + sub * 4 + lane_off, sv2);
       tmem_ld_wait();
 #pragma unroll
-      for (int a = 0; a < 4; a++) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]) + (NACC5 == 2 ? __uint_as_float(sv2[a]) : 0.f);
+      for (int a = 0; a < 4; a++)
+        if (r < Vp) sS[r * SROW + sub * 4 + a] = __uint_as_float(sv[a]) + (NACC5 == 2 ? __uint_as_float(sv2[a]) : 0.f);   // (lanes >= Vp: not data)
       tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(a_free0 + 8 * pb);
       worker_sync();
       // ---- ds[v, a] = alpha (dalpha - sum_w alpha_w dalpha_w), one head per warp; ds^T -> the K-major B tile of the dUt product
       {
@@ -879,8 +911,8 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
         for (int v = lane; v < V; v += 32) dot += sAl[v * SROW + a] * sS[v * SROW + a];
         dot = warp_sum(dot);
         for (int v = lane; v < 2 * TB; v += 32) {
-          const float ds = v < V ? sAl[v * SROW + a] * (sS[v * SROW + a] - dot) : 0.f;   // (rows >= Vp of dalpha are not data)
-          sS[v * SROW + a] = ds;
+          const float ds = v < V ? sAl[v * SROW + a] * (sS[v * SROW + a] - dot) : 0.f;
+          if (v < Vp) sS[v * SROW + a] = ds;
           *reinterpret_cast<bf16*>(dt + (v >> 6) * UT + a * 128 + ((((v & 63) >> 3) ^ (a & 7)) << 4) + (v & 7) * 2) = __float2bfloat16_rn(ds);
         }
       }
@@ -890,7 +922,7 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
         const float* src = (sub < 2 ? sAl : sS) + r * SROW + (sub & 1) * 8;
         uint32_t pk[4];
 #pragma unroll
-        for (int q = 0; q < 4; q++) pk[q] = pack_bf16(src[2 * q], src[2 * q + 1]);
+        for (int q = 0; q < 4; q++) pk[q] = r < Vp ? pack_bf16(src[2 * q], src[2 * q + 1]) : 0u;
         tmem_st_32x4(tAD + sub * 4 + lane_off, pk);
         tmem_st_wait();
       }
@@ -900,7 +932,7 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
       if (w == 0 && lane == 0) mbar_arrive(ad_full);
       // ---- pass 2: drain dX of each 64-column sub-tile: thread = token row, this warp's 16 columns
       for (int i = 0; i < nch; i++) {
-        const int c = i < R ? nch - R + i : nch - 1 - i;
+        const int c = nch - 1 - i;
 #pragma unroll
         for (int j = 0; j < 2; j++, u++) {
           const uint32_t xb = u & 1;
@@ -930,7 +962,7 @@ __global__ void __launch_bounds__(NT5, 1) agg_bwd_t5_kernel(const __grid_constan
             }
             fence_proxy_async();
             quarter_sync(quarter);
-            if (sub == 0 && lane == 0) { tma_store_3d(&tmD, so, (c * 2 + j) * TB, quarter * 32, bl); bulk_commit(); }
+            if (sub == 0 && lane == 0) { tma_store_3d(&tmD, so, (c * 2 + j) * TB, quarter * 32, bl, pol_st); bulk_commit(); }
           }
         }
       }
@@ -1066,20 +1098,22 @@ int agg_patch_bwd_tc(const void* tok, const void* Utb, const float* alpha, const
   ORBIT_TRY(make_map(&tmG, dXbar, (long long)BL * heads, D, heads));
   ORBIT_TRY(make_map(&tmU, Utb, HP, D, HP));
   if (t5_enabled() && D <= 2048) {      // dUt^T of all D / 128 steps stays in tensor memory: 16 columns each beside 160 others
-    const int Vp = (V + 15) & ~15;
-    int stg = 12;
-    while (stg > 2 && 1024 + (size_t)t5_bwd_layout(Vp, stg).total > SMEM_MAX) stg--;
-    const size_t smb = 1024 + (size_t)t5_bwd_layout(Vp, stg).total;
+    static const int stb_env = [] { const char* e = getenv("ORBIT_AGG_BSTB"); return e ? atoi(e) : 0; }();
+    static const int sta_env = [] { const char* e = getenv("ORBIT_AGG_BSTA"); return e ? atoi(e) : 0; }();
+    // L2 hints: bit 0 evict_last on the first read, bit 1 evict_first on the second read, bit 2 evict_first on the dX stores.
+    // At config 3 one patch time moves ~180 MB through the 126 MB L2 (X, X again, dX, dXbar twice), so about half of the second
+    // read misses whatever the hints are: DRAM traffic is 1.35x the algorithmic bytes and the kernel runs at ~95 % of hbm_gbs of
+    // actual DRAM traffic.
+    static const int hint_env = [] { const char* e = getenv("ORBIT_AGG_BHINT"); return e ? atoi(e) : 6; }();
+    int stb = stb_env > 0 ? stb_env : 4, sta = sta_env > 0 ? sta_env : 12;
+    while (sta > 1 && 1024 + (size_t)t5_bwd_layout(V, sta, stb).total > SMEM_MAX) sta--;
+    while (stb > 1 && 1024 + (size_t)t5_bwd_layout(V, sta, stb).total > SMEM_MAX) stb--;
+    const size_t smb = 1024 + (size_t)t5_bwd_layout(V, sta, stb).total;
     ORBIT_SMEM_ATTR(agg_bwd_t5_kernel, SMEM_MAX);
-    static const int keep_env = [] { const char* e = getenv("ORBIT_AGG_KEEP"); return e ? atoi(e) : -1; }();
-    const int nch = D / (2 * TB);
-    int keep = keep_env >= 0 ? keep_env : stg - 2;
-    if (keep > stg - 1) keep = stg - 1;
-    if (keep > nch) keep = nch;
     const int grid5 = BL < num_sms() ? BL : num_sms();
     CUtensorMap tmD;
     ORBIT_TRY(make_map_rows3(&tmD, dtok, BL, V, D));
-    agg_bwd_t5_kernel<<<grid5, NT5, smb, s>>>(tmX, tmG, tmU, tmD, alpha, dUt_acc, BL, V, D, heads, stg, keep);
+    agg_bwd_t5_kernel<<<grid5, NT5, smb, s>>>(tmX, tmG, tmU, tmD, alpha, dUt_acc, BL, V, D, heads, sta, stb, hint_env);
     ORBIT_LAUNCH_CHECK();
     return ORBIT_OK;
   }

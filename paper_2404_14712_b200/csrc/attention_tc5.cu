@@ -761,7 +761,7 @@ attn_bwd_dkv_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_
 template <int DH>
 __global__ void __launch_bounds__(NTHB, 1)
 attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_constant__ CUtensorMap tmSmall,
-                       const __grid_constant__ CUtensorMap tmdOBig, AttnArgs a, float scale, float sl2) {
+                       const __grid_constant__ CUtensorMap tmdOBig, AttnArgs a, float scale, float sl2, int delta_here) {
   using C = CfgB<DH>;
   constexpr int BT = C::BT, CW = BT / 2;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -890,7 +890,45 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
     const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
     const int qrow = q0 + r;
     const float lse2 = qrow < N ? a.lse[(size_t)bh * N + qrow] * LOG2E : 0.f;
-    const float dl = qrow < N ? a.delta[(size_t)bh * N + qrow] : 0.f;
+    // delta[row] = sum_d dO[row, d] O[row, d]: read from the delta kernel's output, or -- short sequences (N <= 1024), where a
+    // launch of its own costs more than it computes (C2: +10 % on the attention backward, one launch less per block) --
+    // computed HERE: the four threads that share a query row (two groups x two column halves) take a quarter of the head's
+    // columns each while the first K / V tiles are in flight, exchange the partial sums through the (not yet used) dS tile,
+    // and the row's value is written out for the dK / dV kernel, which runs after this one.  At N = 2048 the in-kernel
+    // version delays the first softmax tile by more than the separate kernel takes (C5: 417 -> 409 TFLOP/s; a coalesced
+    // warp-per-row variant: 407, and 184 instead of 207 at C2).
+    float dl = 0.f;
+    if (!delta_here) {
+      dl = qrow < N ? a.delta[(size_t)bh * N + qrow] : 0.f;
+    } else {
+      const int part = grp * 2 + half;
+      float acc = 0.f;
+      if (qrow < N) {
+        const bf16* po = (const bf16*)a.O + (size_t)(row0 + qrow) * a.ldo + h * DH + part * (DH / 4);
+        const bf16* pd = (const bf16*)a.dO + (size_t)(row0 + qrow) * a.lddo + h * DH + part * (DH / 4);
+#pragma unroll
+        for (int c = 0; c < DH / 32; c++) {
+          const uint4 xo = __ldg(reinterpret_cast<const uint4*>(po) + c), xd = __ldg(reinterpret_cast<const uint4*>(pd) + c);
+          const uint32_t wo[4] = {xo.x, xo.y, xo.z, xo.w}, wd[4] = {xd.x, xd.y, xd.z, xd.w};
+#pragma unroll
+          for (int q = 0; q < 4; q++) {
+            const float2 fo = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wo[q]));
+            const float2 fd = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wd[q]));
+            acc += fo.x * fd.x + fo.y * fd.y;
+          }
+        }
+      }
+      asm volatile("st.shared.f32 [%0], %1;" ::"r"(sdS0 + (uint32_t)(part * 128 + r) * 4), "f"(acc) : "memory");
+      named_bar_sync(3, 512);
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        float v;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(sdS0 + (uint32_t)(q * 128 + r) * 4) : "memory");
+        dl += v;
+      }
+      named_bar_sync(3, 512);                                // the dS tile may be written from here on
+      if (part == 0 && qrow < N) a.delta[(size_t)bh * N + qrow] = dl;
+    }
     if (TSA) {                                               // this thread's row of Q / dO, a quarter of the columns per warp
       const int part = sw >> 2;
       const bf16* src = part < 2 ? (const bf16*)a.qkv + (size_t)(row0 + qrow) * a.ld + qc + part * (DH / 2)
@@ -1045,12 +1083,15 @@ int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_TRY(make_map5(&tmdOSmall, a.dO, a.lddo, rows, C::BT));
   ORBIT_SMEM_ATTR(attn_bwd_dkv_tc5_kernel<DH>, C::SMEM_DKV);
   ORBIT_SMEM_ATTR(attn_bwd_dq_tc5_kernel<DH>, C::SMEM_DQ);
-  const int total_w = a.B * a.heads * a.N;
-  ORBIT_CUDA_CHECK(launch_pdl(attn_delta5_kernel, dim3(cdiv((long long)total_w * 32, 256)), dim3(256), 0, s, a));
-  ORBIT_LAUNCH_CHECK();
+  const int delta_here = a.N <= 1024;
+  if (!delta_here) {
+    const int total_w = a.B * a.heads * a.N;
+    ORBIT_CUDA_CHECK(launch_pdl(attn_delta5_kernel, dim3(cdiv((long long)total_w * 32, 256)), dim3(256), 0, s, a));
+    ORBIT_LAUNCH_CHECK();
+  }
   dim3 grid(cdiv(a.N, 128), a.B * a.heads);
   const float scale = 1.0f / sqrtf((float)DH);
-  ORBIT_CUDA_CHECK(launch_pdl(attn_bwd_dq_tc5_kernel<DH>, grid, dim3(NTHB), C::SMEM_DQ, s, tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E));
+  ORBIT_CUDA_CHECK(launch_pdl(attn_bwd_dq_tc5_kernel<DH>, grid, dim3(NTHB), C::SMEM_DQ, s, tmBig, tmSmall, tmdOBig, a, scale, scale * LOG2E, delta_here));
   ORBIT_LAUNCH_CHECK();
   dim3 grid_kv(cdiv(a.N, 128), a.B * a.heads, C::NSPLIT);
   ORBIT_CUDA_CHECK(launch_pdl(attn_bwd_dkv_tc5_kernel<DH>, grid_kv, dim3(NTHB), C::SMEM_DKV, s, tmBig, tmSmall, tmdOSmall, a, scale, scale * LOG2E));

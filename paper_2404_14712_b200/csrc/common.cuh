@@ -206,6 +206,19 @@ struct CastSegs {
   void add(const float* src, void* dst, size_t n) { s[count].src = src; s[count].dst = dst; s[count].n = n; count++; }
 };
 int cast_multi(const CastSegs& segs, int out_dt, cudaStream_t s);
+// The tail of a block backward in ONE launch: up to 12 column sums (acc[n] += sum_m in[m, n], as colsum), each 256-column group
+// cast to `out` (out_dt) by the LAST of its row blocks to finish (one ticket word per group, zero on entry and on exit), plus the
+// fp32 -> out_dt casts of accumulators that were complete before the launch, spread over all blocks.
+struct TailSeg { const void* in; int in_dt; long long ld; int M, N; float* acc; void* out; int first_block, first_group, gx, gy, rows_per_block; };
+struct TailSegs {
+  TailSeg s[12]; int count = 0;
+  void add(const void* in, int in_dt, long long ld, int M, int N, float* acc, void* out) {
+    TailSeg& t = s[count++]; t.in = in; t.in_dt = in_dt; t.ld = ld; t.M = M; t.N = N; t.acc = acc; t.out = out;
+    t.first_block = t.first_group = t.gx = t.gy = t.rows_per_block = 0;
+  }
+};
+inline size_t block_tail_tickets(size_t total_columns, int segments) { return total_columns / 256 + segments + 8; }
+int block_tail(TailSegs& sums, const CastSegs& casts, int out_dt, unsigned int* tickets, cudaStream_t s);
 int fill_zero(void* p, size_t bytes, cudaStream_t s);
 // out = a (a_dt) + b_f32 + bias (p_dt)  (combine of fp32 Hybrid-STOP partials)
 int add_partial(const void* a, int a_dt, const float* part, const void* bias, int p_dt, void* out, int out_dt,

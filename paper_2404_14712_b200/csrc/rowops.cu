@@ -250,6 +250,59 @@ __global__ void cast_kernel(const void* __restrict__ in, int in_dt, void* __rest
     stf(out, i, ldf(in, i, in_dt), out_dt);
 }
 
+// column sums of several matrices + casts of their and of other accumulators: see block_tail() in common.cuh
+__global__ void __launch_bounds__(256) block_tail_kernel(TailSegs sums, CastSegs casts, int out_dt, unsigned int* tickets) {
+  pdl_wait();
+  pdl_trigger();
+  __shared__ float sh[8][32][9];
+  __shared__ unsigned int last;
+  // accumulators that were complete before this launch: every block takes a slice
+  for (int c = 0; c < casts.count; c++) {
+    const CastSeg cs = casts.s[c];
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < cs.n; i += (size_t)gridDim.x * 256) stf(cs.dst, i, cs.src[i], out_dt);
+  }
+  int si = 0;
+#pragma unroll 1
+  while (si + 1 < sums.count && (int)blockIdx.x >= sums.s[si + 1].first_block) si++;
+  const TailSeg sg = sums.s[si];
+  const int b = blockIdx.x - sg.first_block, bx = b % sg.gx, by = b / sg.gx;
+  const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
+  const int col = (bx * 32 + cx) * 8;
+  const int r0 = by * sg.rows_per_block;
+  const int r1 = min(sg.M, r0 + sg.rows_per_block);
+  float s[8];
+#pragma unroll
+  for (int j = 0; j < 8; j++) s[j] = 0.f;
+  if (col < sg.N) {
+    for (int r = r0 + ry; r < r1; r += 8) {
+      float v[8];
+      ld8(sg.in, (size_t)r * sg.ld + col, sg.in_dt, v);
+#pragma unroll
+      for (int j = 0; j < 8; j++) s[j] += v[j];
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 8; j++) sh[ry][cx][j] = s[j];
+  __syncthreads();
+  const int t = threadIdx.x, colt = bx * 256 + t;
+  if (colt < sg.N) {
+    const int c2 = t >> 3, j = t & 7;
+    float tot = 0.f;
+#pragma unroll
+    for (int y = 0; y < 8; y++) tot += sh[y][c2][j];
+    atomicAdd(sg.acc + colt, tot);
+  }
+  __threadfence();                       // this block's atomics are performed before its ticket
+  __syncthreads();
+  unsigned int* ticket = tickets + sg.first_group + bx;
+  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == (unsigned int)sg.gy - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  if (colt < sg.N) stf(sg.out, colt, __ldcg(sg.acc + colt), out_dt);
+  if (threadIdx.x == 0) *ticket = 0u;
+}
+
 // several fp32 -> out_dt casts in one launch (the small parameter-gradient accumulators of a block backward)
 __global__ void cast_multi_kernel(CastSegs segs, int out_dt) {
   pdl_wait();
@@ -375,6 +428,27 @@ int cast_copy(const void* in, int in_dt, void* out, int out_dt, size_t n, cudaSt
   if (blocks < 1) blocks = 1;
   if (blocks > 148 * 8) blocks = 148 * 8;
   cast_kernel<<<(int)blocks, 256, 0, s>>>(in, in_dt, out, out_dt, n);
+  ORBIT_LAUNCH_CHECK();
+  return ORBIT_OK;
+}
+
+int block_tail(TailSegs& sums, const CastSegs& casts, int out_dt, unsigned int* tickets, cudaStream_t s) {
+  int total = 0, groups = 0;
+  for (int i = 0; i < sums.count; i++) {
+    TailSeg& t = sums.s[i];
+    t.gx = cdiv(t.N, 256);
+    int want_y = cdiv(148 * 4, t.gx * sums.count);
+    if (want_y < 1) want_y = 1;
+    int rpb = cdiv(t.M, want_y);
+    rpb = ((rpb + 7) / 8) * 8;
+    if (rpb < 8) rpb = 8;
+    t.rows_per_block = rpb;
+    t.gy = cdiv(t.M, rpb);
+    t.first_block = total; t.first_group = groups;
+    total += t.gx * t.gy; groups += t.gx;
+  }
+  if (total == 0) return cast_multi(casts, out_dt, s);
+  ORBIT_CUDA_CHECK(launch_pdl(block_tail_kernel, dim3(total), dim3(256), 0, s, sums, casts, out_dt, tickets));
   ORBIT_LAUNCH_CHECK();
   return ORBIT_OK;
 }

@@ -376,6 +376,147 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
     }
   }
 }
+// ---------------------------------------------------------------- backward on tcgen05 -----------------------
+// dWp^T[d, r] = sum over patches of dtok[patch, v, d] pix[patch, r]: M = d (the dtok tiles as they arrive from TMA, an MN-major A
+// operand), K = patches, N = 48 pixel-side columns (16 bf16 "hi" parts of the p^2 pixels, 16 "lo" residuals, a column of ones for
+// dbp, zeros).  The mma.sync kernel above spends its warps on HMMA (6 per 16 patches x 16 columns, a third of them for the ones
+// row: legacy tensor pipe 38 % busy, 65 % of hbm_gbs); here one thread issues 16 tcgen05.mma per stage of 64 patches x 512
+// columns, eight warps only build the small pixel tile (hi / lo split, K-major, 128B swizzle) and the accumulators
+// [128 lanes x 48 columns] per 128-column group stay in tensor memory for the CTA's whole patch range.
+constexpr int KS5 = 64;                        // patches per stage
+constexpr int BOX5 = KS5 * 128;                // one [64 patches x 64 columns] TMA box
+constexpr int NB5 = 48;                        // columns of the pixel-side operand
+constexpr int BT5B = NB5 * 128;                // its tile: [48 rows (n) x 64 patches (k)] bf16, K-major
+constexpr int ST5 = 3;
+constexpr int NT5B = 64 + 256;                 // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 pixel tile / epilogue
+constexpr size_t SMEM_TOKB5 = 1024 + (size_t)ST5 * (8 * BOX5 + BT5B) + 64;
+__global__ void __launch_bounds__(NT5B, 1) tok_bwd_t5_kernel(orbit_embed_desc d, const float* __restrict__ x,
+    float* __restrict__ accW, float* __restrict__ accB, int L, int patches_per_cta, const __grid_constant__ CUtensorMap tmTok) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
+  const uint32_t sA = s_u32(smem), sBt = sA + ST5 * 8 * BOX5;
+  const uint32_t full0 = sBt + ST5 * BT5B, bfull0 = full0 + 8 * ST5, empty0 = bfull0 + 8 * ST5, done = empty0 + 8 * ST5, tslot = done + 8;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int P = d.p, P2 = P * P;
+  const int nz = gridDim.x / d.V;
+  const int v = blockIdx.x / nz, c0 = (blockIdx.x - v * nz) * DCH;
+  const int BL = d.B * L;
+  const int p0 = blockIdx.y * patches_per_cta, p1 = min(BL, p0 + patches_per_cta);
+  const int nst = (p1 - p0 + KS5 - 1) / KS5;
+  const int ncol = min(DCH, d.D - c0), nblk = ncol / 64, ncg = (ncol + 127) / 128;
+
+  for (int i = threadIdx.x; i < ST5 * BT5B / 16; i += NT5B) reinterpret_cast<uint4*>(smem + ST5 * 8 * BOX5)[i] = make_uint4(0, 0, 0, 0);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < ST5; i++) { ptx::mbar_init(full0 + 8 * i, 1); ptx::mbar_init(bfull0 + 8 * i, 8); ptx::mbar_init(empty0 + 8 * i, 1); }
+    ptx::mbar_init(done, 1);
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) { ptx::tmem_alloc(tslot, 256); ptx::tmem_relinquish(); }
+  ptx::fence_proxy_async();
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
+
+  if (warp == 0) {
+    if (lane == 0) {
+      int st = 0; uint32_t ph = 0;
+      for (int ci = 0; ci < nst; ci++) {
+        ptx::mbar_wait(empty0 + 8 * st, ph ^ 1);
+        ptx::mbar_expect_tx(full0 + 8 * st, nblk * BOX5);
+        for (int bk = 0; bk < nblk; bk++)                    // rows >= B L read as zero
+          ptx::tma_load_2d(sA + (st * 8 + bk) * BOX5, &tmTok, full0 + 8 * st, v * d.D + c0 + bk * 64, p0 + ci * KS5);
+        if (++st == ST5) { st = 0; ph ^= 1; }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(128, NB5, 1, 0);
+      int st = 0; uint32_t ph = 0;
+      for (int ci = 0; ci < nst; ci++) {
+        ptx::mbar_wait(full0 + 8 * st, ph);
+        ptx::mbar_wait(bfull0 + 8 * st, ph);
+        ptx::tc_fence_after();
+        for (int cg = 0; cg < ncg; cg++)
+#pragma unroll
+          for (int ks = 0; ks < KS5 / 16; ks++)
+            ptx::mma_f16_ss(tmem + cg * NB5, ptx::make_smem_desc(sA + (st * 8 + cg * 2) * BOX5 + ks * 2048, BOX5, 1024),
+                            ptx::make_smem_desc(sBt + st * BT5B + ks * 32, 16, 1024), idesc, (ci | ks) != 0);
+        ptx::mma_commit(empty0 + 8 * st);
+        if (++st == ST5) { st = 0; ph ^= 1; }
+      }
+      ptx::mma_commit(done);
+    }
+  } else {
+    // pixel tile of a stage: thread = (patch k of the stage, quarter of its pixels), loaded one stage ahead
+    const int tt = threadIdx.x - 64, k = tt >> 2, sub = tt & 3;
+    const int gw = d.Wg / P;
+    const int RP = P2 >= 4 ? P2 / 4 : 1, r0 = sub * RP;                      // this thread's pixels r0 .. r0 + RP - 1 (if < P2)
+    float px[4] = {0.f, 0.f, 0.f, 0.f};
+    bool valid = false;
+    auto fetch = [&](int ci) {
+      const int bl = p0 + ci * KS5 + k;
+      valid = ci < nst && bl < p1;
+#pragma unroll
+      for (int q = 0; q < 4; q++) px[q] = 0.f;
+      if (valid && r0 < P2) {
+        const int b = bl / L, l = bl - b * L, pi = l / gw, pj = l - pi * gw;
+        const float* base = x + (((size_t)b * d.V + v) * d.Hg + pi * P) * d.Wg + pj * P;
+        if (P == 4) {                                        // r0 = 4 sub: one pixel row of the patch, 16 aligned bytes
+          const float4 f = __ldg(reinterpret_cast<const float4*>(base + (size_t)sub * d.Wg));
+          px[0] = f.x; px[1] = f.y; px[2] = f.z; px[3] = f.w;
+        } else {
+          px[0] = __ldg(base + (size_t)(r0 / P) * d.Wg + r0 % P);
+        }
+      }
+    };
+    fetch(0);
+    int st = 0; uint32_t ph = 0;
+    for (int ci = 0; ci < nst; ci++) {
+      ptx::mbar_wait(empty0 + 8 * st, ph ^ 1);               // the products of the stage that used this tile have completed
+      uint8_t* bt = smem + ST5 * 8 * BOX5 + st * BT5B;
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        const int r = r0 + q;
+        if (q < RP && r < P2) {
+          const bf16 hi = __float2bfloat16_rn(px[q]);
+          const bf16 lo = __float2bfloat16_rn(px[q] - __bfloat162float(hi));
+          *reinterpret_cast<bf16*>(bt + r * 128 + (((k >> 3) ^ (r & 7)) << 4) + (k & 7) * 2) = hi;
+          *reinterpret_cast<bf16*>(bt + (16 + r) * 128 + (((k >> 3) ^ ((16 + r) & 7)) << 4) + (k & 7) * 2) = lo;
+        }
+      }
+      if (sub == 0) *reinterpret_cast<bf16*>(bt + 32 * 128 + (((k >> 3) ^ 0) << 4) + (k & 7) * 2) = __float2bfloat16_rn(valid ? 1.f : 0.f);
+      ptx::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bfull0 + 8 * st);
+      fetch(ci + 1);
+      if (++st == ST5) { st = 0; ph ^= 1; }
+    }
+    // accumulators -> fp32 atomics: thread = column d of a 128-column group; the two warps of a TMEM lane quarter split the groups
+    ptx::mbar_wait(done, 0);
+    ptx::tc_fence_after();
+    const int quarter = warp & 3, half = (warp - 2) >> 2;
+    const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
+    for (int cg = half; cg < ncg; cg += 2) {
+      uint32_t a[NB5];
+      ptx::tmem_ld_32x16(tmem + cg * NB5 + lane_off, a);
+      ptx::tmem_ld_32x16(tmem + cg * NB5 + 16 + lane_off, a + 16);
+      ptx::tmem_ld_32x16(tmem + cg * NB5 + 32 + lane_off, a + 32);
+      ptx::tmem_ld_wait();
+      const int col = cg * 128 + quarter * 32 + lane;
+      if (col < ncol && nst > 0) {
+#pragma unroll
+        for (int r = 0; r < 16; r++)
+          if (r < P2) atomicAdd(accW + ((size_t)v * P2 + r) * d.D + c0 + col, __uint_as_float(a[r]) + __uint_as_float(a[16 + r]));
+        atomicAdd(accB + (size_t)v * d.D + c0 + col, __uint_as_float(a[32]));
+      }
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 256); }
+}
 }  // namespace
 
 bool tokenize_tc_supported(const orbit_embed_desc& d) {
@@ -387,7 +528,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long cols,
-                        CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE) {
+                        CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE, int box_rows = 16) {
   static std::atomic<EncodeTiledFn> enc_c{nullptr};
   EncodeTiledFn enc = enc_c.load(std::memory_order_relaxed);
   if (!enc) {
@@ -400,7 +541,7 @@ static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long co
   }
   cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
   cuuint64_t strides[1] = {(cuuint64_t)cols * 2};
-  cuuint32_t box[2] = {64, 16};
+  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
   cuuint32_t es[2] = {1, 1};
   CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, tok, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                    CU_TENSOR_MAP_SWIZZLE_128B, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -452,6 +593,31 @@ int tokenize_bwd_acc_tc(const orbit_embed_desc& d, const float* x, const void* d
   const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
   const long long BL = (long long)d.B * L;
   const int nz = cdiv(d.D, DCH);
+  static const int t5_env = [] { const char* e = getenv("ORBIT_TOK_T5"); return (e && e[0] == '0') ? 0 : 1; }();
+  if (t5_env && d.D % 64 == 0 && (long long)d.V * d.D < (1ll << 31) && P2 <= 16) {
+    // one CTA per SM (192 KB of stages): patch splits so that the grid fills whole waves of the SMs
+    int splits = 1;
+    {
+      const long long slots = num_sms(), per = (long long)d.V * nz;
+      double best = 0.0;
+      for (int sp = 1; sp <= 32; sp++) {
+        if (cdiv(BL, sp) < 4 * KS5 && sp > 1) break;         // keep at least 4 stages per CTA
+        const long long n = per * sp, waves = (n + slots - 1) / slots;
+        const double eff = (double)n / (double)(waves * slots);
+        if (eff > best + 1e-9) { best = eff; splits = sp; }
+        if (eff >= 0.97) { splits = sp; break; }
+      }
+    }
+    int ppc = cdiv(BL, splits);
+    ppc = ((ppc + KS5 - 1) / KS5) * KS5;
+    dim3 grid(d.V * nz, cdiv(BL, ppc));
+    CUtensorMap tm;
+    ORBIT_TRY(make_tok_map(&tm, const_cast<void*>(dtok), BL, (long long)d.V * d.D, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, KS5));
+    ORBIT_SMEM_ATTR(tok_bwd_t5_kernel, SMEM_TOKB5);
+    tok_bwd_t5_kernel<<<grid, NT5B, SMEM_TOKB5, s>>>(d, x, accW, accB, L, ppc, tm);
+    ORBIT_LAUNCH_CHECK();
+    return ORBIT_OK;
+  }
   // patch splits: the first count whose grid fills whole waves of 2 CTAs per SM to >= 95 % (else the fullest)
   int splits = 1;
   {

@@ -70,7 +70,7 @@ def compare_block(br, y, dx, P, x, dy, heads, T, tol, eps=1e-5):
 
 
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("T", [1, 2, 4])
+@pytest.mark.parametrize("T", [1, 2, 4, 8])      # T = 8: more bias-gradient segments than the one-launch tail of the backward takes
 def test_block_fp32_shard_recombination(rn, T):
     """fp32 shard-recombination check (north_star; R15): sharded CUDA block (fp32 storage, true fp32
     FMA, fp32 partials) vs the UNSHARDED fp64 oracle, <= 1e-4."""

@@ -376,6 +376,175 @@ __global__ void __launch_bounds__(NT) tok_bwd_tc_kernel(orbit_embed_desc d, cons
     }
   }
 }
+__device__ __forceinline__ void bulk_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
+// ---------------------------------------------------------------- forward on tcgen05 ------------------------
+// tok[patch, v, c0 .. c0 + 512) = [hi | lo | 1] (A: 128 patches x 48, K-major, built by the worker warps) . [Wp[v] ; Wp[v] ; bp[v]]
+// (B: 48 x 512 columns, MN-major, resident for the CTA's life), two N = 256 halves per stage of 128 patches into the two halves of
+// tensor memory; 16 worker warps (TMEM lane quarter x 64 of a half's 256 columns) drain them: fp32 -> bf16 -> a warp-private
+// swizzled [32 rows x 64 columns] staging tile -> one TMA box store (rows >= B L clipped by the map), two tiles in flight per warp.
+constexpr int PT5 = 128;                       // patches per stage
+constexpr int WB5 = 48 * 128;                  // one 64-column block of the B operand: 48 k-rows x 128 bytes
+constexpr int AT5F = PT5 * 128;                // A tile: 128 patches x 64 k (48 used) bf16, K-major
+constexpr int OT5F = 32 * 128;                 // staging tile of a warp
+constexpr int NW5F = 16;
+constexpr int NT5F = 32 + NW5F * 32;           // warp 0 MMA issuer, warps 1..16 workers
+constexpr size_t SMEM_TOKF5 = 1024 + 8 * WB5 + 2 * AT5F + NW5F * 2 * OT5F + 64;
+__global__ void __launch_bounds__(NT5F, 1) tok_fwd_t5_kernel(orbit_embed_desc d, const float* __restrict__ x,
+    const bf16* __restrict__ Wp, const bf16* __restrict__ bp, int L, int patches_per_cta, const __grid_constant__ CUtensorMap tmTok, int STORE_HINT) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024 - (s_u32(smem_raw) & 1023)) & 1023);
+  uint8_t* pW = smem;                          // [8][48][128 B]
+  uint8_t* pA = pW + 8 * WB5;                  // [2][128][128 B]
+  const uint32_t sW = s_u32(pW), sA = s_u32(pA), sO = sA + 2 * AT5F;
+  const uint32_t a_full0 = sO + NW5F * 2 * OT5F, a_empty0 = a_full0 + 16, t_full0 = a_empty0 + 16, t_empty0 = t_full0 + 16, tslot = t_empty0 + 16;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int P = d.p, P2 = P * P;
+  const int nz = gridDim.x / d.V;
+  const int v = blockIdx.x / nz, c0 = (blockIdx.x - v * nz) * DCH;
+  const int BL = d.B * L;
+  const int p0 = blockIdx.y * patches_per_cta, p1 = min(BL, p0 + patches_per_cta);
+  const int nst = (p1 - p0 + PT5 - 1) / PT5;
+  const int ncol = min(DCH, d.D - c0), nhalf = (ncol + 255) / 256;
+
+  // B operand, once: k-rows 0..P2-1 and 16..16+P2-1 = Wp[v] (the hi and the lo product), row 32 = bp[v], the rest zero
+  for (int idx = threadIdx.x; idx < 48 * (DCH / 8); idx += NT5F) {
+    const int k = idx / (DCH / 8), ch = idx - k * (DCH / 8), col = ch * 8;
+    uint4 val = make_uint4(0, 0, 0, 0);
+    if (col < ncol) {
+      if ((k & 15) < P2 && k < 32) val = *reinterpret_cast<const uint4*>(Wp + ((size_t)v * P2 + (k & 15)) * d.D + c0 + col);
+      else if (k == 32) val = *reinterpret_cast<const uint4*>(bp + (size_t)v * d.D + c0 + col);
+    }
+    *reinterpret_cast<uint4*>(pW + (col >> 6) * WB5 + k * 128 + ((((col & 63) >> 3) ^ (k & 7)) << 4)) = val;
+  }
+  for (int i = threadIdx.x; i < 2 * AT5F / 16; i += NT5F) reinterpret_cast<uint4*>(pA)[i] = make_uint4(0, 0, 0, 0);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 2; i++) {
+      ptx::mbar_init(a_full0 + 8 * i, NW5F); ptx::mbar_init(a_empty0 + 8 * i, 1);
+      ptx::mbar_init(t_full0 + 8 * i, 1); ptx::mbar_init(t_empty0 + 8 * i, NW5F);
+    }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 0) { ptx::tmem_alloc(tslot, 512); ptx::tmem_relinquish(); }
+  ptx::fence_proxy_async();
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(tslot));
+
+  if (warp == 0) {
+    if (lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(128, 256, 0, 1);
+      for (int ci = 0; ci < nst; ci++) {
+        const uint32_t ab = ci & 1;
+        ptx::mbar_wait(a_full0 + 8 * ab, (ci >> 1) & 1);
+        for (int hf = 0; hf < nhalf; hf++) {
+          ptx::mbar_wait(t_empty0 + 8 * hf, (ci & 1) ^ 1);
+          ptx::tc_fence_after();
+#pragma unroll
+          for (int ks = 0; ks < 3; ks++)
+            ptx::mma_f16_ss(tmem + hf * 256, ptx::make_smem_desc(sA + ab * AT5F + ks * 32, 16, 1024),
+                            ptx::make_smem_desc(sW + hf * 4 * WB5 + ks * 2048, WB5, 1024), idesc, ks != 0);
+          ptx::mma_commit(t_full0 + 8 * hf);
+        }
+        ptx::mma_commit(a_empty0 + 8 * ab);
+      }
+    }
+  } else {
+    const int w = warp - 1, tt = threadIdx.x - 32, k = tt >> 2, sub = tt & 3;       // pixel tile: thread = (patch k, quarter of its pixels)
+    const int quarter = warp & 3, cb = w >> 2;                                        // drain: TMEM lane quarter, 64-column block of a half
+    const uint32_t lane_off = (uint32_t)(quarter * 32) << 16;
+    const int gw = d.Wg / P;
+    const int RP = P2 >= 4 ? P2 / 4 : 1, r0 = sub * RP;
+    float px[4] = {0.f, 0.f, 0.f, 0.f};
+    bool valid = false;
+    auto fetch = [&](int ci) {
+      const int bl = p0 + ci * PT5 + k;
+      valid = ci < nst && bl < p1;
+#pragma unroll
+      for (int q = 0; q < 4; q++) px[q] = 0.f;
+      if (valid && r0 < P2) {
+        const int b = bl / L, l = bl - b * L, pi = l / gw, pj = l - pi * gw;
+        const float* base = x + (((size_t)b * d.V + v) * d.Hg + pi * P) * d.Wg + pj * P;
+        if (P == 4) {
+          const float4 f = __ldg(reinterpret_cast<const float4*>(base + (size_t)sub * d.Wg));
+          px[0] = f.x; px[1] = f.y; px[2] = f.z; px[3] = f.w;
+        } else {
+          px[0] = __ldg(base + (size_t)(r0 / P) * d.Wg + r0 % P);
+        }
+      }
+    };
+    fetch(0);
+    uint32_t ob = 0;                                         // this warp's staging tile in use
+    const uint64_t pol = ptx::l2_policy(STORE_HINT == 2 ? 2 : 1);
+    auto build = [&](int ci) {                               // A tile of stage ci from the pixels fetched for it
+      const uint32_t ab = ci & 1;
+      ptx::mbar_wait(a_empty0 + 8 * ab, ((ci >> 1) & 1) ^ 1);
+      uint8_t* at = pA + ab * AT5F + k * 128;                // row k: [hi (k 0..15) | lo (16..31) | 1 (32)] as 16-byte chunks ^ (k & 7)
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        const int r = r0 + q;
+        if (q < RP && r < P2) {
+          const bf16 hi = __float2bfloat16_rn(px[q]);
+          const bf16 lo = __float2bfloat16_rn(px[q] - __bfloat162float(hi));
+          *reinterpret_cast<bf16*>(at + (((r >> 3) ^ (k & 7)) << 4) + (r & 7) * 2) = hi;
+          *reinterpret_cast<bf16*>(at + ((((16 + r) >> 3) ^ (k & 7)) << 4) + (r & 7) * 2) = lo;
+        }
+      }
+      if (sub == 0) *reinterpret_cast<bf16*>(at + ((4 ^ (k & 7)) << 4)) = __float2bfloat16_rn(valid ? 1.f : 0.f);
+      ptx::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(a_full0 + 8 * ab);
+    };
+    for (int ci = 0; ci < nst; ci++) {
+      // (building the NEXT stage's operand before draining this one, so that its products overlap the drain, measured SLOWER:
+      // 625 vs 568-592 us at C3)
+      build(ci);
+      fetch(ci + 1);
+      for (int hf = 0; hf < nhalf; hf++) {
+        ptx::mbar_wait(t_full0 + 8 * hf, ci & 1);
+        ptx::tc_fence_after();
+        uint32_t o[64];
+        ptx::tmem_ld_32x32(tmem + hf * 256 + cb * 64 + lane_off, o);
+        ptx::tmem_ld_32x32(tmem + hf * 256 + cb * 64 + 32 + lane_off, o + 32);
+        ptx::tmem_ld_wait();
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(t_empty0 + 8 * hf);
+        const int col = hf * 256 + cb * 64;
+        if (col < ncol) {
+          const uint32_t so = sO + (w * 2 + ob) * OT5F;
+          if (lane == 0) bulk_wait_read1();                  // the store issued two tiles ago has left this buffer
+          __syncwarp();
+#pragma unroll
+          for (int c = 0; c < 8; c++) {
+            const uint32_t addr = so + lane * 128 + ((c ^ (lane & 7)) << 4);
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr),
+                         "r"(pack_bf16(__uint_as_float(o[c * 8]), __uint_as_float(o[c * 8 + 1]))),
+                         "r"(pack_bf16(__uint_as_float(o[c * 8 + 2]), __uint_as_float(o[c * 8 + 3]))),
+                         "r"(pack_bf16(__uint_as_float(o[c * 8 + 4]), __uint_as_float(o[c * 8 + 5]))),
+                         "r"(pack_bf16(__uint_as_float(o[c * 8 + 6]), __uint_as_float(o[c * 8 + 7]))) : "memory");
+          }
+          ptx::fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) {
+            if (STORE_HINT)
+              asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;" ::"l"(&tmTok), "r"(so),
+                           "r"(v * d.D + c0 + col), "r"(p0 + ci * PT5 + quarter * 32), "l"(pol) : "memory");
+            else tma_store_2d(&tmTok, so, v * d.D + c0 + col, p0 + ci * PT5 + quarter * 32);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+          }
+          ob ^= 1;
+        }
+      }
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 0) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
+}
+
 // ---------------------------------------------------------------- backward on tcgen05 -----------------------
 // dWp^T[d, r] = sum over patches of dtok[patch, v, d] pix[patch, r]: M = d (the dtok tiles as they arrive from TMA, an MN-major A
 // operand), K = patches, N = 48 pixel-side columns (16 bf16 "hi" parts of the p^2 pixels, 16 "lo" residuals, a column of ones for
@@ -551,6 +720,33 @@ static int make_tok_map(CUtensorMap* tm, void* tok, long long rows, long long co
 
 int tokenize_fwd_tc(const orbit_embed_desc& d, const float* x, const void* Wp, const void* bp, void* tok, cudaStream_t s) {
   const int L = (d.Hg / d.p) * (d.Wg / d.p), P2 = d.p * d.p;
+  static const int t5_env = [] { const char* e = getenv("ORBIT_TOK_T5"); return (e && e[0] == '0') ? 0 : 1; }();
+  if (t5_env && d.D % 64 == 0 && (long long)d.V * d.D < (1ll << 31) && P2 <= 16) {
+    const long long BL = (long long)d.B * L;
+    const int nz = cdiv(d.D, DCH);
+    int splits = 1;                      // one CTA per SM: patch splits so that the grid fills whole waves of the SMs
+    {
+      const long long slots = num_sms(), per = (long long)d.V * nz;
+      double best = 0.0;
+      for (int sp = 1; sp <= 32; sp++) {
+        if (cdiv(BL, sp) < 4 * PT5 && sp > 1) break;         // keep at least 4 stages per CTA
+        const long long n = per * sp, waves = (n + slots - 1) / slots;
+        const double eff = (double)n / (double)(waves * slots);
+        if (eff > best + 1e-9) { best = eff; splits = sp; }
+        if (eff >= 0.97) { splits = sp; break; }
+      }
+    }
+    int ppc = cdiv(BL, splits);
+    ppc = ((ppc + PT5 - 1) / PT5) * PT5;
+    dim3 grid(d.V * nz, cdiv(BL, ppc));
+    CUtensorMap tm;
+    ORBIT_TRY(make_tok_map(&tm, tok, BL, (long long)d.V * d.D, CU_TENSOR_MAP_L2_PROMOTION_NONE, 32));
+    ORBIT_SMEM_ATTR(tok_fwd_t5_kernel, SMEM_TOKF5);
+    static const int hint_env = [] { const char* e = getenv("ORBIT_TOK_HINT"); return e ? atoi(e) : 1; }();
+    tok_fwd_t5_kernel<<<grid, NT5F, SMEM_TOKF5, s>>>(d, x, (const bf16*)Wp, (const bf16*)bp, L, ppc, tm, hint_env);
+    ORBIT_LAUNCH_CHECK();
+    return ORBIT_OK;
+  }
   // persistent over the patch blocks: grid.y CTAs per (variable, column chunk), chosen so that the grid fills whole waves
   // of 3 CTAs per SM (the shared-memory limit) as evenly as possible, 4+ patch blocks per CTA when there are enough
   const int gx = d.V * cdiv(d.D, DCH), npb = cdiv((long long)d.B * L, 128);

@@ -323,6 +323,9 @@ def test_front_end_fused_shapes(rn, case):
     dict(B=5, V=17, Hg=16, Wg=16, p=2, D=384, heads=12, rd="bf16"),     # odd chunk count (D = 6 x 64), V = 16 + 1, BL = 320
     dict(B=1, V=9, Hg=8, Wg=8, p=2, D=4096, heads=16, rd="bf16"),       # widest D of the TMA kernels: the [16][D] dUt accumulator fills
                                                                         # all 512 TMEM columns (64 chunks x 4 columns x 2 warps per quarter)
+    dict(B=2, V=6, Hg=12, Wg=20, p=2, D=192, heads=4, rd="bf16"),       # tcgen05 tokeniser with an odd number of 64-column boxes (the last
+                                                                        # 128-column group is half loaded); SIMT aggregation (D % 128 != 0)
+    dict(B=3, V=3, Hg=20, Wg=28, p=4, D=64, heads=4, rd="f32"),         # one 64-column box, p = 4, B L = 105 (one ragged stage)
 ])
 def test_front_end_twocall_shapes(rn, case):
     """orbit_tokenize + orbit_var_aggregate (+ backward) on the tensor-core / TMA kernels over edge shapes, <= 1e-2."""

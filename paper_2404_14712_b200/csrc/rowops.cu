@@ -274,6 +274,7 @@ __global__ void __launch_bounds__(256) block_tail_kernel(TailSegs sums, CastSegs
 #pragma unroll
   for (int j = 0; j < 8; j++) s[j] = 0.f;
   if (col < sg.N) {
+#pragma unroll 4
     for (int r = r0 + ry; r < r1; r += 8) {
       float v[8];
       ld8(sg.in, (size_t)r * sg.ld + col, sg.in_dt, v);
@@ -433,11 +434,12 @@ int cast_copy(const void* in, int in_dt, void* out, int out_dt, size_t n, cudaSt
 }
 
 int block_tail(TailSegs& sums, const CastSegs& casts, int out_dt, unsigned int* tickets, cudaStream_t s) {
-  int total = 0, groups = 0;
+  int total = 0, groups = 0, all_gx = 0;
+  for (int i = 0; i < sums.count; i++) all_gx += cdiv(sums.s[i].N, 256);
   for (int i = 0; i < sums.count; i++) {
     TailSeg& t = sums.s[i];
     t.gx = cdiv(t.N, 256);
-    int want_y = cdiv(148 * 4, t.gx * sums.count);
+    int want_y = cdiv(num_sms() * 8, all_gx > 0 ? all_gx : 1);      // ~8 blocks per SM over all segments
     if (want_y < 1) want_y = 1;
     int rpb = cdiv(t.M, want_y);
     rpb = ((rpb + 7) / 8) * 8;

@@ -23,6 +23,7 @@
 // S: the tensor pipe was starved by shared-memory bandwidth (Cfg above).  With P in tensor memory: 2090 cycles per tile, MMA thread
 // 1540 busy, softmax wait for S 240; same-box A/B of the kernel: 53.3 -> 48.0 us at C4 (644 -> 715 TFLOP/s), 370 -> 344 us at C5,
 // 195 -> 180 us at C3.  Both agents are now about equally loaded (softmax ~1850 busy cycles per tile).
+// Four softmax warps per lane quarter (32 key columns each, a four-way row-max exchange) measured SLOWER: 175 vs 166 us at C3.
 // S_{j+1} is issued before the softmax of tile j finishes, so the tensor pipe overlaps the exponentials.
 // V tiles are consumed as an MN-major B operand straight from their row-major [keys, d] layout.
 #include <cuda.h>

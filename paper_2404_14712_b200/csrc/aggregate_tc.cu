@@ -547,7 +547,9 @@ __global__ void __launch_bounds__(NT5, 1) agg_fwd_t5_kernel(const __grid_constan
   if (warp == 0) {
     if (lane == 0) {                                      // producer A: X and Ut chunks of pass 1, patch after patch
       int st = 0; uint32_t ph = 0;
-      const uint64_t pol = l2_policy(HINT & 1 ? 2 : 0);     // the tile is read again within a patch time: keep it in L2
+      // (evict_last on all first reads: 711 vs 701 us; on the 2-8 chunks read first, which are re-read last and are the ones the L2
+      // loses: 693-702 vs 689 us, DRAM bytes unchanged -- the hint does not keep them)
+      const uint64_t pol = l2_policy(HINT & 1 ? 2 : 0);
       for (int pi = 0; pi < npat; pi++) {
         const int row0 = (blockIdx.x + pi * gridDim.x) * V;
         for (int c = 0; c < nch; c++) {

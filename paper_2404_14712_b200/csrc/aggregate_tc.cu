@@ -8,6 +8,7 @@
 // X is read twice per direction (second pass mostly from L2); everything else is tiny.  This makes the kernels
 // HBM/L2-bound instead of fp32-ALU-bound (2*heads .. 4*heads FMA per token element on CUDA cores).
 #include <cuda.h>
+#include <atomic>
 #include "frontend.cuh"
 #include "ptx.cuh"
 
@@ -1014,13 +1015,15 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 // bf16 matrix [rows, D] row-major -> boxes of [box_rows x 64 columns], 128-byte swizzle
 int make_map(CUtensorMap* tm, const void* base, long long rows, int D, int box_rows) {
-  static EncodeTiledFn enc = nullptr;
+  static std::atomic<EncodeTiledFn> enc_c{nullptr};
+  EncodeTiledFn enc = enc_c.load(std::memory_order_relaxed);
   if (!enc) {
     void* p = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
         qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
     enc = (EncodeTiledFn)p;
+    enc_c.store(enc, std::memory_order_relaxed);
   }
   cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)rows};
   cuuint64_t strides[1] = {(cuuint64_t)D * 2};
@@ -1034,10 +1037,14 @@ int make_map(CUtensorMap* tm, const void* base, long long rows, int D, int box_r
 }
 // dtok seen as [BL][V][D] bf16 -> boxes of [1][32 rows][64 columns], 128-byte swizzle: a store clips the rows >= V of a patch
 int make_map_rows3(CUtensorMap* tm, const void* base, long long BL, int V, int D) {
-  void* p = nullptr;
-  cudaDriverEntryPointQueryResult qres;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
-      qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
+  static std::atomic<void*> enc_c{nullptr};                 // the entry point is process-wide: looked up once
+  void* p = enc_c.load(std::memory_order_relaxed);
+  if (!p) {
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled entry point not found"); return ORBIT_ERR_CUDA; }
+    enc_c.store(p, std::memory_order_relaxed);
+  }
   cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)V, (cuuint64_t)BL};
   cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)V * D * 2};
   cuuint32_t box[3] = {(cuuint32_t)TB, 32, 1};

@@ -27,6 +27,7 @@
 // S_{j+1} is issued before the softmax of tile j finishes, so the tensor pipe overlaps the exponentials.
 // V tiles are consumed as an MN-major B operand straight from their row-major [keys, d] layout.
 #include <cuda.h>
+#include <atomic>
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -1035,13 +1036,16 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn get_encode5() {
-  static EncodeTiledFn fn = nullptr;
+  static std::atomic<EncodeTiledFn> cached{nullptr};     // process-wide entry point; host threads may race to fill it (same value)
+  EncodeTiledFn fn = cached.load(std::memory_order_relaxed);
   if (!fn) {
     void* p = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
+        qres == cudaDriverEntryPointSuccess) {
       fn = (EncodeTiledFn)p;
+      cached.store(fn, std::memory_order_relaxed);
+    }
   }
   return fn;
 }

@@ -7,6 +7,7 @@
 // dW GEMMs read activations as an M-major A and an N-major B.  All four combinations go through
 // the same kernel: only the TMA boxes, the UMMA descriptors' LBO/SBO and the per-k-step advance differ.
 #include <cuda.h>
+#include <atomic>
 #include "common.cuh"
 #include "gemm_epi.cuh"
 #include "ptx.cuh"
@@ -182,13 +183,16 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn get_encode() {
-  static EncodeTiledFn fn = nullptr;
+  static std::atomic<EncodeTiledFn> cached{nullptr};     // process-wide entry point; host threads may race to fill it (same value)
+  EncodeTiledFn fn = cached.load(std::memory_order_relaxed);
   if (!fn) {
     void* p = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
+        qres == cudaDriverEntryPointSuccess) {
       fn = (EncodeTiledFn)p;
+      cached.store(fn, std::memory_order_relaxed);
+    }
   }
   return fn;
 }

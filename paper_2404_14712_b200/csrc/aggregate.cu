@@ -201,8 +201,20 @@ __global__ void __launch_bounds__(256) agg_dqt_kernel(const float* __restrict__ 
   const int c = blockIdx.x * 32 + cx;
   const int da = D / h, a = c < D ? c / da : 0;
   float s = 0.f;
-  if (c < D)
-    for (int d = ry; d < D; d += 8) s = fmaf(dUt[(size_t)d * h + a], ldf(Wk, (size_t)d * D + c, p_dt), s);
+  if (c < D) {
+    int d = ry;
+    if (p_dt == ORBIT_BF16) {               // eight rows requested before the first FMA (one 2-byte load per thread in flight: 42 us at D = 2048)
+      const bf16* W = (const bf16*)Wk + c;
+      for (; d + 56 < D; d += 64) {
+        float w[8], u[8];
+#pragma unroll
+        for (int i = 0; i < 8; i++) { w[i] = __bfloat162float(W[(size_t)(d + 8 * i) * D]); u[i] = dUt[(size_t)(d + 8 * i) * h + a]; }
+#pragma unroll
+        for (int i = 0; i < 8; i++) s = fmaf(u[i], w[i], s);
+      }
+    }
+    for (; d < D; d += 8) s = fmaf(dUt[(size_t)d * h + a], ldf(Wk, (size_t)d * D + c, p_dt), s);
+  }
   sh[ry][cx] = s;
   __syncthreads();
   if (ry == 0 && c < D) {
@@ -219,8 +231,21 @@ __global__ void __launch_bounds__(256) agg_qt_kernel(const void* __restrict__ q,
   const int cx = threadIdx.x & 31, ry = threadIdx.x >> 5;
   const int n = blockIdx.x * 32 + cx;
   float s = 0.f;
-  if (n < D)
-    for (int k = ry; k < D; k += 8) s = fmaf(ldf(q, k, p_dt), ldf(Wq, (size_t)k * D + n, p_dt), s);
+  if (n < D) {
+    int k = ry;
+    if (p_dt == ORBIT_BF16) {               // as in agg_dqt_kernel: eight loads in flight per thread (48 -> ~10 us at D = 2048)
+      const bf16* W = (const bf16*)Wq + n;
+      const bf16* qv = (const bf16*)q;
+      for (; k + 56 < D; k += 64) {
+        float w[8], u[8];
+#pragma unroll
+        for (int i = 0; i < 8; i++) { w[i] = __bfloat162float(W[(size_t)(k + 8 * i) * D]); u[i] = __bfloat162float(qv[k + 8 * i]); }
+#pragma unroll
+        for (int i = 0; i < 8; i++) s = fmaf(u[i], w[i], s);
+      }
+    }
+    for (; k < D; k += 8) s = fmaf(ldf(q, k, p_dt), ldf(Wq, (size_t)k * D + n, p_dt), s);
+  }
   sh[ry][cx] = s;
   __syncthreads();
   if (ry == 0 && n < D) {

@@ -1011,25 +1011,33 @@ attn_bwd_dq_tc5_kernel(const __grid_constant__ CUtensorMap tmBig, const __grid_c
   if (warp == 1) { ptx::tc_fence_after(); ptx::tmem_dealloc(tmem, 512); }
 }
 
-// delta[b,h,i] = sum_d dO[i, h*dh+d] * O[i, h*dh+d]
+// delta[b,h,i] = sum_d dO[i, h*dh+d] * O[i, h*dh+d].  A lane takes 16 bytes of a row (8 of its d_h values); a warp covers 4 rows
+// (d_h 64), 2 (d_h 128) or 1 (d_h 192 / 256) per pass: 4-byte loads with one row per warp ran at 2.6 TB/s.
 __global__ void attn_delta5_kernel(AttnArgs a) {
   pdl_wait();
   pdl_trigger();
-  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  const int total = a.B * a.heads * a.N;
-  if (w >= total) return;
-  const int bh = w / a.N, i = w - bh * a.N, b = bh / a.heads, h = bh - b * a.heads;
-  const size_t row = (size_t)b * a.N + i;
-  const bf16* po = (const bf16*)a.O + row * a.ldo + h * a.dh;
-  const bf16* pd = (const bf16*)a.dO + row * a.lddo + h * a.dh;
+  const int nchunk = a.dh >> 3;                                  // 16-byte pieces per row
+  const int rpw = nchunk <= 8 ? 4 : (nchunk <= 16 ? 2 : 1), gs = 32 / rpw;
+  const int lane = threadIdx.x & 31, sub = lane / gs, ch = lane - sub * gs;
+  const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long long total = (long long)a.B * a.heads * a.N;
+  const long long row_id = w * rpw + sub;
   float s = 0.f;
-  for (int d = lane * 2; d < a.dh; d += 64) {
-    float2 x = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(po + d));
-    float2 y = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(pd + d));
-    s += x.x * y.x + x.y * y.y;
+  if (row_id < total && ch < nchunk) {
+    const int bh = (int)(row_id / a.N), i = (int)(row_id - (long long)bh * a.N), b = bh / a.heads, h = bh - b * a.heads;
+    const size_t row = (size_t)b * a.N + i;
+    const uint4 xo = __ldg(reinterpret_cast<const uint4*>((const bf16*)a.O + row * a.ldo + h * a.dh) + ch);
+    const uint4 xd = __ldg(reinterpret_cast<const uint4*>((const bf16*)a.dO + row * a.lddo + h * a.dh) + ch);
+    const uint32_t wo[4] = {xo.x, xo.y, xo.z, xo.w}, wd[4] = {xd.x, xd.y, xd.z, xd.w};
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+      const float2 fo = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wo[q]));
+      const float2 fd = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wd[q]));
+      s += fo.x * fd.x + fo.y * fd.y;
+    }
   }
-  s = warp_sum(s);
-  if (lane == 0) a.delta[w] = s;
+  for (int o = gs >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (ch == 0 && row_id < total) a.delta[row_id] = s;
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -1090,8 +1098,9 @@ int launch_bwd5(const AttnArgs& a, cudaStream_t s) {
   ORBIT_SMEM_ATTR(attn_bwd_dq_tc5_kernel<DH>, C::SMEM_DQ);
   const int delta_here = a.N <= 1024;
   if (!delta_here) {
-    const int total_w = a.B * a.heads * a.N;
-    ORBIT_CUDA_CHECK(launch_pdl(attn_delta5_kernel, dim3(cdiv((long long)total_w * 32, 256)), dim3(256), 0, s, a));
+    const long long rows_d = (long long)a.B * a.heads * a.N;
+    const int rpw = (a.dh >> 3) <= 8 ? 4 : ((a.dh >> 3) <= 16 ? 2 : 1);
+    ORBIT_CUDA_CHECK(launch_pdl(attn_delta5_kernel, dim3(cdiv((rows_d + rpw - 1) / rpw * 32, 256)), dim3(256), 0, s, a));
     ORBIT_LAUNCH_CHECK();
   }
   dim3 grid(cdiv(a.N, 128), a.B * a.heads);

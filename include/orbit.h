@@ -7,6 +7,8 @@
  *  - All tensor pointers are DEVICE memory owned by the caller; descriptors and parameter structs are HOST
  *    memory, read during the call only.  The library allocates no device memory, keeps no pointer after
  *    return, and writes only outputs, `saved`, `ws` and gradients.  Outputs are overwritten (no accumulate).
+ *    (One exception, by design: orbit_tokenize_bwd_noalloc uses a 16 MiB file-scope device array of the library
+ *    instead of `ws`; see its declaration.)
  *  - Dense row-major, last index contiguous.  Weights are [in, out] so that y = x A exactly as in Eq. (1)-(3)
  *    (PAPER.md:70-82): a column shard is A[:, k n/T:(k+1) n/T], a row shard is B[k n/T:(k+1) n/T, :].
  *    Wqkv columns are [Q | K | V], heads contiguous inside each third.  tok is [B, L, V, D].
